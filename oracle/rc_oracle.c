@@ -1,0 +1,348 @@
+/*
+ * rc_oracle.c — fp64 CPU oracle for the radiance-cascades formal solution (flatland).
+ *
+ * TEST INFRASTRUCTURE, NOT PRODUCT.  Only tests/, __graft_entry__.smoke() and bench.py's
+ * cpu_baseline / --impl reference legs may build, load or call this file.  It shares no code,
+ * header, table or constant with the CUDA path under paper_2408_14425_b200/csrc/.
+ *
+ * It follows the paper (Osborne & Sannikov, arxiv 2408.14425; /root/reference/PAPER.md) step by
+ * step, in the paper's order, in double precision, with no blocking, tiling or early exit:
+ *
+ *   radiance interval  R_{a,b}(p,w) = [I, tau] along p + t w, t in [a,b]   PAPER.md:137-139 (eq. 9)
+ *   per-cell update    tau += chi ds; I <- I e^{-chi ds} + (eta/chi)(1-e^{-chi ds})
+ *                                                                         PAPER.md:297-300 (eq. 16)
+ *   grid walk          uniform-grid DDA
+ *   cascade i          probe spacing 2^i, 4^(i+1) directions, shell [t_i,t_{i+1}],
+ *                      t_i = c0 (4^i-1)/3  (eq. 12-13 with alpha = 2)
+ *   cascade 0 probes   at the cell centres
+ *   top cascade        runs to the domain edge; boundary intensity there
+ *   merge              near interval attenuates the far one (eq. 11)
+ *   interpolation      bilinear over the 4 parent probes of cascade i+1,
+ *                      each interval merged with its 4 children in the cone PAPER.md:199-207
+ *   lattice edge       parent lookup clamped
+ *   J                  mean over the 4 merged cascade-0 directions         PAPER.md:36 (eq. 1), 191
+ *
+ * Readings where the paper is silent or garbled are DESIGN.md §3 (G1..G19 of SURVEY.md §8(c)).
+ * The only loop restructuring relative to SURVEY.md's listing: the wavelength loop is innermost
+ * (the cell segments of a ray do not depend on the wavelength), which changes no arithmetic of
+ * any (probe, direction, wavelength) triple.
+ *
+ * The per-segment update is written in the equivalent front-to-back form ("works
+ * equally well"):  I += T * eta*ds*f(chi ds),  T *= exp(-chi ds),  f(x) = (1-e^{-x})/x, f(0)=1,
+ * which is eq. 16 rearranged and has the chi -> 0 limit built in (reading G11).  A back-to-front
+ * variant (eq. 16 literally, towards the probe) is kept beside it and tested to agree (G13).
+ *
+ * Pinned by tests/test_oracle_pins.py (closed forms, invariants, brute force).  Not pinned against
+ * any number printed in the paper (it prints none for this path): the direction convention (G4)
+ * and the probe placement for i >= 1 (G5) are "parity unpinned vs the paper" — see DESIGN.md.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#ifndef M_PI
+#define M_PI 3.14159265358979323846
+#endif
+
+typedef struct {
+    int nx, ny, L;
+    const float *chi, *eta; /* [ny][nx][L], wavelength fastest, y = 0 bottom row */
+} grid_t;
+
+typedef struct {
+    int cell;  /* y*nx + x */
+    double ds; /* path length inside the cell */
+} seg_t;
+
+/* Interval ends, eq. 12-13 with alpha = 2 as fixed by BASELINE.json: t_i = c0 (4^i - 1)/3. */
+static double t_of(int i, double c0) { return c0 * (pow(4.0, (double)i) - 1.0) / 3.0; }
+
+/* f(x) = (1 - exp(-x))/x, f(0) = 1 (reading G11). */
+static double f_emis(double x) { return x == 0.0 ? 1.0 : -expm1(-x) / x; }
+
+/*
+ * Cell segments of {p + t w : ta <= t <= tb} inside the box [0,nx] x [0,ny]: standard 2D DDA
+ * (PAPER.md:314).  Probes lie inside the box and the box is convex, so a ray whose start point
+ * p + ta w is outside never re-enters (reading G10: outside is vacuum).  Each crossing parameter
+ * is recomputed from the grid line it belongs to, not accumulated.  Returns the segment count.
+ */
+static int dda_segments(int nx, int ny, double px, double py, double wx, double wy, double ta,
+                        double tb, seg_t *out) {
+    double x0 = px + ta * wx, y0 = py + ta * wy;
+    if (!(x0 >= 0.0 && x0 <= nx && y0 >= 0.0 && y0 <= ny)) return 0;
+    int ix = (int)floor(x0), iy = (int)floor(y0);
+    if ((double)ix == x0 && wx < 0.0) ix--; /* on a grid line: the cell the ray moves into */
+    if ((double)iy == y0 && wy < 0.0) iy--;
+    if (ix < 0 || ix >= nx || iy < 0 || iy >= ny) return 0;
+    int sx = wx > 0.0 ? 1 : -1, sy = wy > 0.0 ? 1 : -1;
+    int gx = wx > 0.0 ? ix + 1 : ix; /* next grid line crossed in x */
+    int gy = wy > 0.0 ? iy + 1 : iy;
+    double tmx = wx != 0.0 ? (gx - px) / wx : INFINITY;
+    double tmy = wy != 0.0 ? (gy - py) / wy : INFINITY;
+    double t = ta;
+    int n = 0;
+    for (;;) {
+        double tn = fmin(fmin(tmx, tmy), tb);
+        double ds = tn - t;
+        if (ds > 0.0) {
+            out[n].cell = iy * nx + ix;
+            out[n].ds = ds;
+            n++;
+        }
+        if (tn >= tb) break;
+        int stepx = tmx <= tmy, stepy = tmy <= tmx; /* a tie is a corner: step both */
+        if (stepx) { ix += sx; gx += sx; tmx = (gx - px) / wx; }
+        if (stepy) { iy += sy; gy += sy; tmy = (gy - py) / wy; }
+        if (ix < 0 || ix >= nx || iy < 0 || iy >= ny) break;
+        t = tn;
+    }
+    return n;
+}
+
+/*
+ * Cascade 0: the four directions are the diagonals (reading G4) and start at a cell centre
+ * (PAPER.md:312), so they pass exactly through cell corners; the segments are written in closed
+ * form (reading G12): cell m along the diagonal covers t in [sqrt2 (m - 1/2), sqrt2 (m + 1/2)].
+ * quadrant q = 0..3: (+,+), (-,+), (-,-), (+,-), i.e. theta = pi/4 + q pi/2.
+ */
+static int diag_segments(int nx, int ny, int cx, int cy, int q, double ta, double tb, seg_t *out) {
+    static const int SX[4] = {1, -1, -1, 1}, SY[4] = {1, 1, -1, -1};
+    const double r2 = sqrt(2.0);
+    int n = 0;
+    for (int m = 0;; m++) {
+        int ix = cx + m * SX[q], iy = cy + m * SY[q];
+        if (ix < 0 || ix >= nx || iy < 0 || iy >= ny) break;
+        double lo = m == 0 ? 0.0 : r2 * (m - 0.5), hi = r2 * (m + 0.5);
+        if (lo >= tb) break;
+        if (lo < ta) lo = ta;
+        if (hi > tb) hi = tb;
+        if (hi > lo) {
+            out[n].cell = iy * nx + ix;
+            out[n].ds = hi - lo;
+            n++;
+        }
+    }
+    return n;
+}
+
+/* eq. 16 along the segments, front-to-back, all wavelengths: I[l], T[l] = exp(-tau[l]). */
+static void integrate_ftb(const grid_t *g, const seg_t *seg, int n, double *I, double *T) {
+    for (int l = 0; l < g->L; l++) {
+        double Il = 0.0, Tl = 1.0;
+        for (int s = 0; s < n; s++) {
+            size_t c = (size_t)seg[s].cell * g->L + l;
+            double ds = seg[s].ds, x = (double)g->chi[c] * ds;
+            Il += Tl * (double)g->eta[c] * ds * f_emis(x);
+            Tl *= exp(-x);
+        }
+        I[l] = Il;
+        T[l] = Tl;
+    }
+}
+
+/* eq. 16 literally: start at the far end with I = 0 and integrate towards the probe
+ * ("back-to-front"); tau accumulated, T = exp(-tau). */
+static void integrate_btf(const grid_t *g, const seg_t *seg, int n, double *I, double *T) {
+    for (int l = 0; l < g->L; l++) {
+        double Il = 0.0, tau = 0.0;
+        for (int s = n - 1; s >= 0; s--) {
+            size_t c = (size_t)seg[s].cell * g->L + l;
+            double ds = seg[s].ds, chi = g->chi[c], eta = g->eta[c], x = chi * ds;
+            tau += x;
+            Il = Il * exp(-x) + (chi > 0.0 ? (eta / chi) * (-expm1(-x)) : eta * ds);
+        }
+        I[l] = Il;
+        T[l] = exp(-tau);
+    }
+}
+
+/* Position of child probe a among the parents of the next cascade (n of them per axis):
+ * a/2 - 1/4 in parent index units (reading G5), indices clamped at the lattice edge
+ * (reading G6). */
+static void parent_axis(int a, int n, int *q0, int *q1, double *frac) {
+    int base;
+    if ((a & 1) == 0) { base = a / 2 - 1; *frac = 0.75; }
+    else              { base = (a - 1) / 2; *frac = 0.25; }
+    int b1 = base + 1;
+    *q0 = base < 0 ? 0 : (base > n - 1 ? n - 1 : base);
+    *q1 = b1 < 0 ? 0 : (b1 > n - 1 ? n - 1 : b1);
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* Exported entry points (host pointers throughout).                                           */
+/* ------------------------------------------------------------------------------------------ */
+
+/* Segments of one ray, for the tests that pin the DDA.  diag_q >= 0 selects the cascade-0 closed
+ * form from the centre of cell (floor(px), floor(py)); otherwise direction angle theta.
+ * cells[] / ds[] must hold nx + ny + 4 entries.  Returns the count. */
+int rc_oracle_ray_segments(int nx, int ny, double px, double py, double theta, int diag_q,
+                           double ta, double tb, int *cells, double *ds) {
+    seg_t *seg = (seg_t *)malloc(sizeof(seg_t) * (size_t)(nx + ny + 4));
+    int n = diag_q >= 0 ? diag_segments(nx, ny, (int)floor(px), (int)floor(py), diag_q, ta, tb, seg)
+                        : dda_segments(nx, ny, px, py, cos(theta), sin(theta), ta, tb, seg);
+    for (int s = 0; s < n; s++) { cells[s] = seg[s].cell; ds[s] = seg[s].ds; }
+    free(seg);
+    return n;
+}
+
+/* One radiance interval [I[l], T[l]] (eq. 9) of one ray; order: 0 front-to-back, 1 back-to-front. */
+int rc_oracle_interval(const float *chi, const float *eta, int nx, int ny, int L, double px,
+                       double py, double theta, int diag_q, double ta, double tb, int order,
+                       double *I, double *T) {
+    grid_t g = {nx, ny, L, chi, eta};
+    seg_t *seg = (seg_t *)malloc(sizeof(seg_t) * (size_t)(nx + ny + 4));
+    int n = diag_q >= 0 ? diag_segments(nx, ny, (int)floor(px), (int)floor(py), diag_q, ta, tb, seg)
+                        : dda_segments(nx, ny, px, py, cos(theta), sin(theta), ta, tb, seg);
+    if (order == 0) integrate_ftb(&g, seg, n, I, T); else integrate_btf(&g, seg, n, I, T);
+    free(seg);
+    return n;
+}
+
+/* Merge operator, eq. 11 in the physical reading G1: near = [a,b], far = [b,c]. */
+void rc_oracle_merge(double I_near, double tau_near, double I_far, double tau_far, double *I_out,
+                     double *tau_out) {
+    *I_out = I_near + exp(-tau_near) * I_far;
+    *tau_out = tau_near + tau_far;
+}
+
+typedef struct {
+    int64_t intervals[16]; /* intervals computed per cascade (inside the requested window) */
+    int64_t segments[16];  /* cell segments walked per cascade (per wavelength)             */
+} rc_oracle_counts;
+
+/*
+ * The whole path for the cascade-0 cells x0 <= x < x1, y0 <= y < y1 (the full grid for the full
+ * solve).  Cascade i is computed only on the probes the window's cells depend on through the
+ * bilinear parent lookups; every computed number is the same as in the full solve.
+ *
+ *   J_out   [(y1-y0)][(x1-x0)][L]  double
+ *   Jbar_out[(y1-y0)][(x1-x0)]     double, = sum_l w[l] J[..][l]; may be NULL
+ *   I_below/I_above/w: [L] or NULL (zero / zero / ones)
+ *   dump_cascade >= 0: also write that cascade's intervals before merging (dump_I, dump_T) and
+ *   after merging (dump_M), each [wy][wx][N][L] over that cascade's probe window; dump_win gets
+ *   {ax0, ax1, by0, by1} (inclusive probe index ranges).
+ *   order: 0 front-to-back, 1 back-to-front (G13).
+ * Returns 0, or -1 on bad arguments / -2 out of memory.
+ */
+int rc_oracle_solve(const float *chi, const float *eta, int nx, int ny, int L, int ncasc,
+                    double c0, const float *I_below, const float *I_above, const float *w,
+                    int x0, int x1, int y0, int y1, double *J_out, double *Jbar_out, int nthreads,
+                    int order, int dump_cascade, double *dump_I, double *dump_T, double *dump_M,
+                    int *dump_win, rc_oracle_counts *counts) {
+    if (!chi || !eta || !J_out || nx <= 0 || ny <= 0 || L <= 0 || ncasc < 1 || ncasc > 15)
+        return -1;
+    int top = ncasc - 1;
+    if (nx % (1 << top) || ny % (1 << top)) return -1; /* reading G19 */
+    if (x0 < 0 || y0 < 0 || x1 > nx || y1 > ny || x0 >= x1 || y0 >= y1) return -1;
+    grid_t g = {nx, ny, L, chi, eta};
+    if (counts) memset(counts, 0, sizeof(*counts));
+#ifdef _OPENMP
+    if (nthreads > 0) omp_set_num_threads(nthreads);
+#endif
+    /* probe windows per cascade (inclusive), propagated through parent_axis */
+    int ax0[16], ax1[16], by0[16], by1[16];
+    ax0[0] = x0; ax1[0] = x1 - 1; by0[0] = y0; by1[0] = y1 - 1;
+    for (int i = 0; i < top; i++) {
+        int npx = nx >> (i + 1), npy = ny >> (i + 1), q0, q1; double fr;
+        parent_axis(ax0[i], npx, &q0, &q1, &fr); ax0[i + 1] = q0;
+        parent_axis(ax1[i], npx, &q0, &q1, &fr); ax1[i + 1] = q1;
+        parent_axis(by0[i], npy, &q0, &q1, &fr); by0[i + 1] = q0;
+        parent_axis(by1[i], npy, &q0, &q1, &fr); by1[i + 1] = q1;
+    }
+    double *Mup = NULL; /* merged cascade i+1: [wy][wx][N_{i+1}][L] */
+    int upx0 = 0, upy0 = 0, upwx = 0;
+    long upN = 0;
+    int status = 0;
+    for (int i = top; i >= 0; i--) {
+        int s = 1 << i;
+        int npx = nx / s, npy = ny / s;
+        long N = 1L << (2 * (i + 1)); /* 4^(i+1) directions */
+        double ta = t_of(i, c0), tb = i == top ? INFINITY : t_of(i + 1, c0); /* G8 */
+        int wx = ax1[i] - ax0[i] + 1, wy = by1[i] - by0[i] + 1;
+        double *M = (double *)malloc(sizeof(double) * (size_t)wx * wy * N * L);
+        if (!M) { status = -2; break; }
+        int dump = i == dump_cascade;
+        if (dump && dump_win) { dump_win[0] = ax0[i]; dump_win[1] = ax1[i]; dump_win[2] = by0[i]; dump_win[3] = by1[i]; }
+        int64_t nseg_total = 0;
+#pragma omp parallel reduction(+ : nseg_total)
+        {
+            seg_t *seg = (seg_t *)malloc(sizeof(seg_t) * (size_t)(nx + ny + 4));
+            double *I = (double *)malloc(sizeof(double) * L);
+            double *T = (double *)malloc(sizeof(double) * L);
+#pragma omp for collapse(2) schedule(dynamic, 1)
+            for (int b = by0[i]; b <= by1[i]; b++) {
+                for (int a = ax0[i]; a <= ax1[i]; a++) {
+                    double px = (a + 0.5) * s, py = (b + 0.5) * s; /* PAPER.md:312, reading G5 */
+                    for (long k = 0; k < N; k++) {
+                        double theta = 2.0 * M_PI * (k + 0.5) / (double)N; /* reading G4 */
+                        /* a1: the radiance interval of this probe and direction */
+                        int n = i == 0 ? diag_segments(nx, ny, a, b, (int)k, ta, tb, seg)
+                                       : dda_segments(nx, ny, px, py, cos(theta), sin(theta), ta, tb, seg);
+                        nseg_total += n;
+                        if (order == 0) integrate_ftb(&g, seg, n, I, T); else integrate_btf(&g, seg, n, I, T);
+                        size_t o = ((((size_t)(b - by0[i])) * wx + (a - ax0[i])) * N + k) * L;
+                        if (dump) for (int l = 0; l < L; l++) { dump_I[o + l] = I[l]; dump_T[o + l] = T[l]; }
+                        if (i == top) {
+                            /* a2: boundary intensity enters on the top cascade only (G9) */
+                            for (int l = 0; l < L; l++) {
+                                double Ib = sin(theta) < 0.0 ? (I_below ? I_below[l] : 0.0)
+                                                             : (I_above ? I_above[l] : 0.0);
+                                M[o + l] = I[l] + T[l] * Ib;
+                            }
+                        } else {
+                            /* a3: bilinear over the 4 parents, mean over the 4 children, eq. 11 */
+                            int a0, a1, b0, b1; double fa, fb;
+                            parent_axis(a, npx / 2, &a0, &a1, &fa);
+                            parent_axis(b, npy / 2, &b0, &b1, &fb);
+                            for (int l = 0; l < L; l++) {
+                                double U = 0.0;
+                                for (int j = 0; j < 4; j++) {
+                                    long kk = 4 * k + j;
+#define MUP(bb, aa) Mup[((((size_t)((bb) - upy0)) * upwx + ((aa) - upx0)) * upN + kk) * L + l]
+                                    U += (1.0 - fb) * ((1.0 - fa) * MUP(b0, a0) + fa * MUP(b0, a1))
+                                       +        fb  * ((1.0 - fa) * MUP(b1, a0) + fa * MUP(b1, a1));
+#undef MUP
+                                }
+                                M[o + l] = I[l] + T[l] * U / 4.0;
+                            }
+                        }
+                        if (dump) for (int l = 0; l < L; l++) dump_M[o + l] = M[o + l];
+                    }
+                }
+            }
+            free(seg); free(I); free(T);
+        }
+        if (counts) { counts->intervals[i] = (int64_t)wx * wy * N; counts->segments[i] = nseg_total; }
+        free(Mup);
+        Mup = M; upx0 = ax0[i]; upy0 = by0[i]; upwx = wx; upN = N;
+    }
+    if (status == 0) {
+        /* a4: J = mean of the 4 merged cascade-0 directions (eq. 1 in flatland, reading G14) */
+        int wx = x1 - x0, wy = y1 - y0;
+        for (int y = 0; y < wy; y++)
+            for (int x = 0; x < wx; x++) {
+                double jb = 0.0;
+                for (int l = 0; l < L; l++) {
+                    const double *m = Mup + (((size_t)y * wx + x) * 4) * L + l;
+                    double J = (m[0] + m[(size_t)L] + m[2 * (size_t)L] + m[3 * (size_t)L]) / 4.0;
+                    J_out[((size_t)y * wx + x) * L + l] = J;
+                    jb += (w ? (double)w[l] : 1.0) * J;
+                }
+                if (Jbar_out) Jbar_out[(size_t)y * wx + x] = jb;
+            }
+    }
+    free(Mup);
+    return status;
+}
+
+int rc_oracle_num_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}

@@ -1,0 +1,135 @@
+"""ctypes wrapper around oracle/rc_oracle.c (the fp64 CPU oracle).
+
+TEST INFRASTRUCTURE, NOT PRODUCT: only tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs may import this.  It imports nothing from the CUDA package.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from pathlib import Path
+
+import numpy as np
+
+_HERE = Path(__file__).resolve().parent
+_SRC = _HERE / "rc_oracle.c"
+_SO = _HERE / "librc_oracle.so"
+_lib = None
+
+
+def build(force: bool = False) -> Path:
+    """gcc -O2 -fopenmp; no -ffast-math (the oracle's arithmetic is exactly what the source says)."""
+    if force or not _SO.exists() or _SO.stat().st_mtime < _SRC.stat().st_mtime:
+        tmp = _SO.with_suffix(f".tmp{os.getpid()}.so")
+        subprocess.check_call(["gcc", "-O2", "-std=c11", "-fopenmp", "-fPIC", "-shared",
+                               "-o", str(tmp), str(_SRC), "-lm"])
+        os.replace(tmp, _SO)
+    return _SO
+
+
+class Counts(C.Structure):
+    _fields_ = [("intervals", C.c_int64 * 16), ("segments", C.c_int64 * 16)]
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(str(build()))
+        _lib.rc_oracle_ray_segments.restype = C.c_int
+        _lib.rc_oracle_ray_segments.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_double,
+                                                C.c_int, C.c_double, C.c_double, C.c_void_p, C.c_void_p]
+        _lib.rc_oracle_interval.restype = C.c_int
+        _lib.rc_oracle_interval.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int,
+                                            C.c_double, C.c_double, C.c_double, C.c_int, C.c_double,
+                                            C.c_double, C.c_int, C.c_void_p, C.c_void_p]
+        _lib.rc_oracle_merge.restype = None
+        _lib.rc_oracle_merge.argtypes = [C.c_double] * 4 + [C.c_void_p, C.c_void_p]
+        _lib.rc_oracle_solve.restype = C.c_int
+        _lib.rc_oracle_solve.argtypes = ([C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int,
+                                          C.c_double, C.c_void_p, C.c_void_p, C.c_void_p] +
+                                         [C.c_int] * 4 + [C.c_void_p, C.c_void_p, C.c_int, C.c_int,
+                                                          C.c_int, C.c_void_p, C.c_void_p, C.c_void_p,
+                                                          C.c_void_p, C.c_void_p])
+        _lib.rc_oracle_num_threads.restype = C.c_int
+    return _lib
+
+
+def _f32(a):
+    return np.ascontiguousarray(a, dtype=np.float32)
+
+
+def _ptr(a):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def num_threads() -> int:
+    return int(lib().rc_oracle_num_threads())
+
+
+def ray_segments(nx, ny, px, py, theta=0.0, diag_q=-1, ta=0.0, tb=np.inf):
+    cells = np.empty(nx + ny + 4, np.int32)
+    ds = np.empty(nx + ny + 4, np.float64)
+    n = lib().rc_oracle_ray_segments(nx, ny, px, py, theta, diag_q, ta, tb, _ptr(cells), _ptr(ds))
+    return cells[:n].copy(), ds[:n].copy()
+
+
+def interval(chi, eta, px, py, theta=0.0, diag_q=-1, ta=0.0, tb=np.inf, order=0):
+    chi, eta = _f32(chi), _f32(eta)
+    ny, nx, L = chi.shape
+    I = np.empty(L)
+    T = np.empty(L)
+    lib().rc_oracle_interval(_ptr(chi), _ptr(eta), nx, ny, L, px, py, theta, diag_q, ta, tb, order,
+                             _ptr(I), _ptr(T))
+    return I, T
+
+
+def merge(I_near, tau_near, I_far, tau_far):
+    a = C.c_double()
+    b = C.c_double()
+    lib().rc_oracle_merge(I_near, tau_near, I_far, tau_far, C.byref(a), C.byref(b))
+    return a.value, b.value
+
+
+def solve(chi, eta, ncascades, c0=1.0, I_below=None, I_above=None, weights=None, window=None,
+          nthreads=0, order=0, dump_cascade=-1, want_counts=False):
+    """J [wy][wx][L] (float64) for the cascade-0 cell window (x0, x1, y0, y1) (default: whole grid).
+
+    Returns a dict: J, Jbar, and if asked counts / dump_{I,T,M,win} of one cascade."""
+    chi, eta = _f32(chi), _f32(eta)
+    ny, nx, L = chi.shape
+    assert eta.shape == chi.shape
+    x0, x1, y0, y1 = (0, nx, 0, ny) if window is None else window
+    J = np.empty((y1 - y0, x1 - x0, L))
+    Jbar = np.empty((y1 - y0, x1 - x0))
+    Ib = None if I_below is None else _f32(I_below)
+    Ia = None if I_above is None else _f32(I_above)
+    w = None if weights is None else _f32(weights)
+    cnt = Counts()
+    dI = dT = dM = None
+    win = np.zeros(4, np.int32)
+    if dump_cascade >= 0:
+        # upper bound on the window of that cascade: the whole lattice
+        s = 1 << dump_cascade
+        N = 4 ** (dump_cascade + 1)
+        shape = (ny // s, nx // s, N, L)
+        dI, dT, dM = np.zeros(shape), np.zeros(shape), np.zeros(shape)
+        assert window is None, "dump only with the full window (dense layout)"
+    rc = lib().rc_oracle_solve(_ptr(chi), _ptr(eta), nx, ny, L, ncascades, c0, _ptr(Ib), _ptr(Ia),
+                               _ptr(w), x0, x1, y0, y1, _ptr(J), _ptr(Jbar), nthreads, order,
+                               dump_cascade, _ptr(dI), _ptr(dT), _ptr(dM), _ptr(win), C.byref(cnt))
+    if rc != 0:
+        raise ValueError(f"rc_oracle_solve failed: {rc}")
+    out = {"J": J, "Jbar": Jbar}
+    if want_counts:
+        out["intervals"] = np.array(cnt.intervals[:ncascades])
+        out["segments"] = np.array(cnt.segments[:ncascades])
+    if dump_cascade >= 0:
+        out.update(dump_I=dI, dump_T=dT, dump_M=dM, dump_win=win)
+    return out
+
+
+def solve_atmosphere(atm, **kw):
+    """Convenience: oracle solve of a paper_2408_14425_b200.atmospheres.Atmosphere-like object."""
+    return solve(atm.chi, atm.eta, atm.ncascades, c0=atm.c0_interval, I_below=atm.I_below,
+                 I_above=atm.I_above, weights=atm.weights, **kw)

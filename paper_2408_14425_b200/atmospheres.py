@@ -1,0 +1,249 @@
+"""Seeded synthetic atmospheres for the five BASELINE.json configurations.
+
+This module holds NO arithmetic of the radiance-cascades method: it only draws the
+input fields (`chi`, `eta`), the boundary intensities and the wavelength weights.
+It is the one module shared by the CPU oracle's tests and the CUDA path's tests
+and bench (numpy only; it never imports the CUDA binding nor `oracle/`).
+
+The recipes are the ones SURVEY.md §8(d) states (restated in DESIGN.md §4); they
+are synthetic stand-ins with the shapes and structure of the paper's workloads
+(PAPER.md:52 and 241 test scenes; PAPER.md:429-460 prominence snapshot), not the
+paper's data, which is not available here.
+
+Layout of every field: C-contiguous float32 `[ny][nx][nlambda]`, wavelength
+fastest, `y = 0` the bottom row (include/rc.h conventions).
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass, field
+
+import numpy as np
+
+SQRT_PI = float(np.sqrt(np.pi))
+
+
+@dataclass
+class Atmosphere:
+    name: str
+    nx: int
+    ny: int
+    nlambda: int
+    ncascades: int
+    chi: np.ndarray  # float32 [ny][nx][nlambda]
+    eta: np.ndarray  # float32 [ny][nx][nlambda]
+    I_below: np.ndarray  # float32 [nlambda], seen by rays heading down (omega_y < 0)
+    I_above: np.ndarray  # float32 [nlambda], seen by rays heading up
+    weights: np.ndarray  # float32 [nlambda] wavelength weights (for Jbar)
+    accumulate: bool = False  # config 4: the checked output is Jbar = sum_l w_l J_l
+    c0_interval: float = 1.0
+    meta: dict = field(default_factory=dict)
+
+
+# (nx, ny, nlambda, ncascades) of BASELINE.json's configs
+FULL_SHAPES = {
+    0: (64, 64, 1, 5),
+    1: (512, 512, 16, 7),
+    2: (1024, 1024, 64, 8),
+    3: (2048, 2048, 32, 9),
+    4: (4096, 1024, 64, 9),
+}
+
+
+def _smooth_normal(rng: np.random.Generator, ny: int, nx: int, sigma: float) -> np.ndarray:
+    """Standard-normal field, periodic Gaussian filter via FFT, kernel exp(-2 pi^2 sigma^2 |k|^2)."""
+    f = rng.standard_normal((ny, nx))
+    ky = np.fft.fftfreq(ny)[:, None]
+    kx = np.fft.rfftfreq(nx)[None, :]
+    kern = np.exp(-2.0 * np.pi**2 * sigma**2 * (kx * kx + ky * ky))
+    return np.fft.irfft2(np.fft.rfft2(f) * kern, s=(ny, nx))
+
+
+def _unit01(f: np.ndarray) -> np.ndarray:
+    return (f - f.min()) / (f.max() - f.min())
+
+
+def _unitvar(f: np.ndarray) -> np.ndarray:
+    return (f - f.mean()) / f.std()
+
+
+def _phi(x):
+    """Gaussian line profile in Doppler units."""
+    return np.exp(-np.square(x)) / SQRT_PI
+
+
+def _finish(name, nx, ny, L, ncasc, chi, eta, I_below=None, I_above=None, weights=None,
+            accumulate=False, meta=None) -> Atmosphere:
+    chi = np.ascontiguousarray(chi, dtype=np.float32)
+    eta = np.ascontiguousarray(eta, dtype=np.float32)
+    assert chi.shape == (ny, nx, L) and eta.shape == (ny, nx, L)
+    z = np.zeros(L, np.float32)
+    return Atmosphere(
+        name=name, nx=nx, ny=ny, nlambda=L, ncascades=ncasc, chi=chi, eta=eta,
+        I_below=z.copy() if I_below is None else np.asarray(I_below, np.float32),
+        I_above=z.copy() if I_above is None else np.asarray(I_above, np.float32),
+        weights=np.ones(L, np.float32) if weights is None else np.asarray(weights, np.float32),
+        accumulate=accumulate, meta=meta or {})
+
+
+def _dims(idx, nx, ny, nlambda, ncascades):
+    fx, fy, fl, fc = FULL_SHAPES[idx]
+    nx = fx if nx is None else nx
+    ny = fy if ny is None else ny
+    nlambda = fl if nlambda is None else nlambda
+    ncascades = fc if ncascades is None else ncascades
+    scale = nx / fx  # feature lengths (in cells) follow the grid
+    return nx, ny, nlambda, ncascades, scale
+
+
+def config0(nx=None, ny=None, nlambda=None, ncascades=None, seed=1000) -> Atmosphere:
+    """64x64x1, 5 cascades: smooth chi in [0.01,10], S in [1,1.5], zero boundary."""
+    nx, ny, L, nc, sc = _dims(0, nx, ny, nlambda, ncascades)
+    rng = np.random.default_rng(seed)
+    g = _unit01(_smooth_normal(rng, ny, nx, 4.0 * sc))
+    h = _unit01(_smooth_normal(rng, ny, nx, 4.0 * sc))
+    chi = 10.0 ** (3.0 * g - 2.0)
+    S = 1.0 + 0.5 * h
+    # extra wavelengths (only when a test asks for them): a plain geometric dimming of chi
+    fac = 10.0 ** (-np.arange(L) / 4.0)
+    chi3 = chi[:, :, None] * fac[None, None, :]
+    return _finish("cfg0", nx, ny, L, nc, chi3, chi3 * S[:, :, None])
+
+
+def config1(nx=None, ny=None, nlambda=None, ncascades=None, seed=1001) -> Atmosphere:
+    """512x512x16, 7 cascades: 40 optically thick discs in a thin background."""
+    nx, ny, L, nc, sc = _dims(1, nx, ny, nlambda, ncascades)
+    rng = np.random.default_rng(seed)
+    chi = np.full((ny, nx), 1e-3)
+    S = np.zeros((ny, nx))
+    yy, xx = np.mgrid[0:ny, 0:nx]
+    xc, yc = xx + 0.5, yy + 0.5
+    for _ in range(40):
+        cx, cy = rng.uniform(0, nx), rng.uniform(0, ny)
+        r = rng.uniform(5.0, 30.0) * sc
+        chi_d = rng.uniform(1.0, 100.0)
+        S_d = rng.uniform(0.5, 2.0)
+        m = (xc - cx) ** 2 + (yc - cy) ** 2 <= r * r
+        chi[m] = chi_d
+        S[m] = S_d
+    fac = 10.0 ** (-np.arange(L) / 5.0)
+    chi3 = chi[:, :, None] * fac[None, None, :]
+    return _finish("cfg1", nx, ny, L, nc, chi3, chi3 * S[:, :, None])
+
+
+def _line_fields(rng, ny, nx, sc):
+    g1 = _unitvar(_smooth_normal(rng, ny, nx, 8.0 * sc))
+    g2 = _unitvar(_smooth_normal(rng, ny, nx, 8.0 * sc))
+    u = _unit01(_smooth_normal(rng, ny, nx, 16.0 * sc))
+    h = _unit01(_smooth_normal(rng, ny, nx, 8.0 * sc))
+    return g1, g2, 3.0 * (2.0 * u - 1.0), 10.0 ** (2.0 * h - 1.0)
+
+
+def _xgrid(L):
+    return np.array([0.0]) if L == 1 else -5.0 + 10.0 * np.arange(L) / (L - 1)
+
+
+def config2(nx=None, ny=None, nlambda=None, ncascades=None, seed=1002) -> Atmosphere:
+    """1024x1024x64, 8 cascades: Doppler-shifted Gaussian line over a lognormal continuum."""
+    nx, ny, L, nc, sc = _dims(2, nx, ny, nlambda, ncascades)
+    rng = np.random.default_rng(seed)
+    g1, g2, v, S = _line_fields(rng, ny, nx, sc)
+    chi_c = (1e-3 * np.exp(g1)).astype(np.float32)
+    chi_line = np.exp(g2).astype(np.float32)
+    x = _xgrid(L).astype(np.float32)
+    chi = np.empty((ny, nx, L), np.float32)
+    for l in range(L):  # plane by plane: keeps the peak memory at one copy
+        chi[:, :, l] = chi_c + chi_line * _phi(x[l] - v)
+    eta = chi * S.astype(np.float32)[:, :, None]
+    return _finish("cfg2", nx, ny, L, nc, chi, eta)
+
+
+def config3(nx=None, ny=None, nlambda=None, ncascades=None, seed=1003) -> Atmosphere:
+    """2048x2048x32, 9 cascades: dense sheet + strands in a 1e-6 corona, lit from below."""
+    nx, ny, L, nc, sc = _dims(3, nx, ny, nlambda, ncascades)
+    rng = np.random.default_rng(seed)
+    yy, xx = np.mgrid[0:ny, 0:nx]
+    xc, yc = xx + 0.5, yy + 0.5
+    chi_line = np.zeros((ny, nx))
+    S = np.zeros((ny, nx))
+    for _ in range(80):  # strands first; the sheet is painted over them
+        x0, y0 = rng.uniform(0, nx), rng.uniform(0, ny)
+        length = rng.uniform(150.0, 700.0) * sc
+        ang = np.pi / 2 + np.deg2rad(rng.uniform(-30.0, 30.0))
+        width = max(rng.uniform(2.0, 10.0) * sc, 1.0)
+        amp = 10.0 ** rng.uniform(1.0, 4.0)
+        S_s = rng.uniform(0.1, 0.5)
+        ux, uy = np.cos(ang), np.sin(ang)
+        along = (xc - x0) * ux + (yc - y0) * uy
+        perp = np.abs(-(xc - x0) * uy + (yc - y0) * ux)
+        m = (along >= 0) & (along <= length) & (perp <= 0.5 * width)
+        chi_line[m] = amp
+        S[m] = S_s
+    g = _unit01(_smooth_normal(rng, ny, nx, 6.0 * sc))
+    ycen = 0.55 * ny + 40.0 * sc * np.sin(2.0 * np.pi * xc / nx * 3.0)
+    m = np.abs(yc - ycen) <= 24.0 * sc
+    chi_line[m] = (1e4 * (0.3 + 0.7 * g))[m]
+    S[m] = 0.2
+    x = _xgrid(L).astype(np.float32)
+    chi = np.empty((ny, nx, L), np.float32)
+    cl = chi_line.astype(np.float32)
+    for l in range(L):
+        chi[:, :, l] = np.float32(1e-6) + cl * np.float32(_phi(x[l]))
+    eta = chi * S.astype(np.float32)[:, :, None]
+    return _finish("cfg3", nx, ny, L, nc, chi, eta, I_below=np.ones(L), I_above=np.zeros(L))
+
+
+def config4(nx=None, ny=None, nlambda=None, ncascades=None, seed=1004) -> Atmosphere:
+    """4096x1024x64, 9 cascades: >90% exactly-empty cells, truncated Gaussian blobs, Jbar output."""
+    nx, ny, L, nc, sc = _dims(4, nx, ny, nlambda, ncascades)
+    rng = np.random.default_rng(seed)
+    yy, xx = np.mgrid[0:ny, 0:nx]
+    xc, yc = (xx + 0.5).astype(np.float32), (yy + 0.5).astype(np.float32)
+    blobs = [(rng.uniform(0, nx), rng.uniform(0, ny), rng.uniform(4.0, 18.0) * sc,
+              10.0 ** rng.uniform(-1.0, 2.0)) for _ in range(130)]
+    nblob = len(blobs)
+    while True:
+        chi_line = np.zeros((ny, nx), np.float32)
+        for (bx, by, sb, amp) in blobs[:nblob]:
+            r = 2.5 * sb
+            xa, xb = max(int(bx - r) - 1, 0), min(int(bx + r) + 2, nx)
+            ya, yb = max(int(by - r) - 1, 0), min(int(by + r) + 2, ny)
+            if xa >= xb or ya >= yb:
+                continue
+            d2 = (xc[ya:yb, xa:xb] - bx) ** 2 + (yc[ya:yb, xa:xb] - by) ** 2
+            add = amp * np.exp(-d2 / (2.0 * sb * sb))
+            add[d2 > r * r] = 0.0
+            chi_line[ya:yb, xa:xb] += add.astype(np.float32)
+        empty = float(np.mean(chi_line == 0.0))
+        if empty > 0.90 or nblob <= 1:
+            break
+        nblob -= 5
+    _, _, v, S = _line_fields(rng, ny, nx, sc)
+    x = _xgrid(L).astype(np.float32)
+    chi = np.empty((ny, nx, L), np.float32)
+    for l in range(L):
+        chi[:, :, l] = chi_line * _phi(x[l] - v).astype(np.float32)
+    eta = chi * S.astype(np.float32)[:, :, None]
+    w = _phi(_xgrid(L))
+    w = w / w.sum()
+    return _finish("cfg4", nx, ny, L, nc, chi, eta, weights=w, accumulate=True,
+                   meta={"empty_fraction": empty, "nblobs": nblob})
+
+
+CONFIGS = {0: config0, 1: config1, 2: config2, 3: config3, 4: config4}
+
+
+def make_config(idx: int, **kw) -> Atmosphere:
+    """Config `idx` of BASELINE.json; keyword overrides (nx, ny, nlambda, ncascades, seed)
+    give the reduced-size variants the parity tests use (feature sizes scale with nx)."""
+    return CONFIGS[idx](**kw)
+
+
+def random_field(nx: int, ny: int, nlambda: int, seed: int, chi_lo=1e-3, chi_hi=10.0,
+                 zero_fraction=0.0):
+    """Unstructured log-uniform chi and uniform S in [0.1, 2]; for unit tests."""
+    rng = np.random.default_rng(seed)
+    chi = np.exp(rng.uniform(np.log(chi_lo), np.log(chi_hi), (ny, nx, nlambda)))
+    if zero_fraction > 0:
+        chi[rng.uniform(size=(ny, nx)) < zero_fraction] = 0.0
+    S = rng.uniform(0.1, 2.0, (ny, nx, nlambda))
+    return chi.astype(np.float32), (chi * S).astype(np.float32)
