@@ -1,0 +1,134 @@
+/*
+ * rc.h — C ABI of librc.so: the radiance-cascades formal solution on a 2D grid ("flatland"),
+ * B200 (sm_100a) only.  Method: Osborne & Sannikov, arxiv 2408.14425 (PAPER.md = the paper's text).
+ *
+ * The interface is the paper's `GivenFs` problem statement (§3.8): "the input model
+ * provides a set of isotropic emissivities and opacities at each point in the domain.  These are
+ * solved for J".  One rc_solve_J call runs the whole hot path:
+ *
+ *   a1  per-cascade radiance-interval ray march: DDA through the chi/eta voxel grids with the
+ *       piecewise-constant update of eq. 16
+ *   a2  boundary intensity on the top cascade
+ *   a3  bilinear interpolation over the 4 parent probes of cascade i+1, mean over the 4 child
+ *       directions, merge (eq. 11)
+ *   a4  J = mean over the 4 merged cascade-0 directions      PAPER.md:36 (eq. 1), 191
+ *
+ * Cascade geometry (eq. 12-13 with branching factor alpha = 2):
+ * cascade i has probes at ((a+1/2) 2^i, (b+1/2) 2^i), 4^(i+1) directions
+ * theta_k = 2 pi (k+1/2)/4^(i+1), interval [t_i, t_(i+1)], t_i = c0_interval (4^i - 1)/3; the top
+ * cascade runs to the domain edge.  Cell size is 1.
+ *
+ * Conventions
+ *   Layout   chi[(y*nx + x)*nlambda + l], wavelength fastest, y = 0 the bottom row; same for eta
+ *            and J_out.  float32.  chi in 1/cell, eta = chi * S.
+ *   Memory   "device" pointers are CUDA device memory of the context's device, "host" pointers
+ *            ordinary host memory.  The library never allocates device memory: inputs, output,
+ *            workspace and the stream are the caller's (e.g. torch tensors / torch streams).
+ *            Pointers given to rc_set_atmosphere / rc_set_workspace are BORROWED until replaced
+ *            or rc_destroy.  Small host arrays (boundary, weights) are copied at the call.
+ *   Async    rc_solve_J only enqueues work on the context's stream and returns; it does not
+ *            synchronise.  rc_solve_J_host synchronises that stream before returning.
+ *   Errors   every call returns RC_OK (0) or a negative RC_ERR_*; nothing throws across the ABI;
+ *            rc_last_error(ctx) gives text for the last failure on that context.
+ *   Inputs   chi >= 0, eta >= 0, finite; eta must be 0 where chi is 0 (emission without opacity
+ *            is not representable as chi*S; such cells are treated as vacuum).
+ *   There is no CPU fallback and no other backend: without an sm_100 device rc_create fails.
+ */
+#ifndef RC_H_
+#define RC_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define RC_OK 0
+#define RC_ERR_NULL_ARG (-1)
+#define RC_ERR_BAD_SHAPE (-2)    /* nx, ny not positive multiples of 2^(ncascades-1); nlambda < 1; too large */
+#define RC_ERR_NO_DEVICE (-3)    /* no CUDA device, or not compute capability 10.x */
+#define RC_ERR_NO_WORKSPACE (-4) /* workspace missing or smaller than rc_workspace_bytes */
+#define RC_ERR_BAD_VALUE (-5)    /* bad config value; or (RC_VALIDATE) negative / non-finite chi or eta */
+#define RC_ERR_CUDA (-6)         /* a CUDA runtime call failed; see rc_last_error */
+#define RC_ERR_NO_ATMOSPHERE (-7)
+
+#define RC_MAX_CASCADES 12
+#define RC_MAX_DIM 16384
+
+/* rc_config.flags */
+#define RC_ACCUM_J 1   /* J_out is Jbar[ny][nx] = sum_l w_l J_l (rc_set_lambda_weights) */
+#define RC_VALIDATE 2  /* rc_set_atmosphere checks chi, eta on the device (synchronises) */
+#define RC_NO_EARLY_EXIT 4 /* never stop a ray early.  Default: a warp stops marching once every live
+                              lane has tau*log2(e) > 126 at all its wavelengths, where the fp32
+                              transmittance has already flushed to exactly 0, so the result is
+                              bit-identical (front-to-back early termination) */
+
+typedef struct rc_ctx rc_ctx; /* opaque, owned by the library */
+
+typedef struct {
+    int ncascades;     /* 1..RC_MAX_CASCADES */
+    float c0_interval; /* length of the cascade-0 interval in cells; > 0; the configs use 1 */
+    int device;        /* CUDA ordinal */
+    int lambda_batch;  /* wavelengths per thread (1, 2, 4 or 8); 0 = library chooses */
+    int flags;         /* RC_ACCUM_J | RC_VALIDATE | RC_NO_EARLY_EXIT */
+} rc_config;
+
+typedef struct {
+    int ncascades;
+    int lambda_batch;                     /* wavelengths per thread actually used */
+    int kernel_launches;                  /* kernels enqueued by the last rc_solve_J */
+    float ms_cascade[RC_MAX_CASCADES];    /* device time per cascade (pack + march), last timed solve */
+    float ms_prep;                        /* chi,eta -> (chi log2e, S) repack */
+    float ms_total;
+    int64_t rays[RC_MAX_CASCADES];        /* intervals per cascade per wavelength = 4 nx ny */
+    int64_t table_steps[RC_MAX_CASCADES]; /* step-table entries per cascade (all directions) */
+    size_t workspace_bytes;
+} rc_stats;
+
+/* Create a context on cfg->device.  Fails with RC_ERR_NO_DEVICE unless that device is sm_100. */
+int rc_create(rc_ctx **out, const rc_config *cfg);
+
+/* Bytes of device workspace rc_solve_J needs for an nx x ny x nlambda atmosphere (0 on bad shape).
+ * host_io != 0 adds room for the device copies rc_solve_J_host makes of chi, eta and J. */
+size_t rc_workspace_bytes(const rc_ctx *ctx, int nx, int ny, int nlambda, int host_io);
+
+/* Caller-owned device workspace (256-byte aligned), borrowed. */
+int rc_set_workspace(rc_ctx *ctx, void *dev_ptr, size_t bytes);
+
+/* Caller-owned CUDA stream (cudaStream_t as void*; NULL = the legacy default stream). */
+int rc_set_stream(rc_ctx *ctx, void *cuda_stream);
+
+/* chi, eta: device, [ny][nx][nlambda] float32, borrowed.  Builds the per-direction step tables for
+ * this grid size (device kernels, fp64 geometry) if the shape changed; needs the workspace set.
+ * PAPER.md:409. */
+int rc_set_atmosphere(rc_ctx *ctx, const float *chi, const float *eta, int nx, int ny, int nlambda);
+
+/* Boundary intensity sampled by the top cascade: I_below[l] is seen by rays heading
+ * down (omega_y < 0), I_above[l] by rays heading up.  host, [nlambda] each; NULL = 0 (free space,
+ * PAPER.md:371).  Call after rc_set_atmosphere. */
+int rc_set_boundary(rc_ctx *ctx, const float *I_below, const float *I_above);
+
+/* Wavelength weights for RC_ACCUM_J: host, [nlambda]; NULL = all 1.  After rc_set_atmosphere. */
+int rc_set_lambda_weights(rc_ctx *ctx, const float *w);
+
+/* Enqueue one full solve.  J_out: device, [ny][nx][nlambda] float32, or [ny][nx] with RC_ACCUM_J. */
+int rc_solve_J(rc_ctx *ctx, float *J_out);
+
+/* Same path with HOST buffers: copies chi, eta to the device (workspace, host_io != 0), solves,
+ * copies J back, synchronises the stream.  Pinned host memory makes the copies asynchronous. */
+int rc_solve_J_host(rc_ctx *ctx, const float *chi_host, const float *eta_host, int nx, int ny,
+                    int nlambda, float *J_host);
+
+/* time_cascades != 0 makes the next solves record per-cascade CUDA-event times (adds events only). */
+int rc_set_timing(rc_ctx *ctx, int time_cascades);
+int rc_get_stats(rc_ctx *ctx, rc_stats *out); /* synchronises the timing events of the last solve */
+
+const char *rc_last_error(const rc_ctx *ctx);
+const char *rc_version(void);
+int rc_destroy(rc_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RC_H_ */

@@ -273,11 +273,11 @@ int rc_oracle_solve(const float *chi, const float *eta, int nx, int ny, int L, i
             seg_t *seg = (seg_t *)malloc(sizeof(seg_t) * (size_t)(nx + ny + 4));
             double *I = (double *)malloc(sizeof(double) * L);
             double *T = (double *)malloc(sizeof(double) * L);
-#pragma omp for collapse(2) schedule(dynamic, 1)
+#pragma omp for collapse(3) schedule(dynamic, 16)
             for (int b = by0[i]; b <= by1[i]; b++) {
                 for (int a = ax0[i]; a <= ax1[i]; a++) {
-                    double px = (a + 0.5) * s, py = (b + 0.5) * s; /* PAPER.md:312, reading G5 */
                     for (long k = 0; k < N; k++) {
+                        double px = (a + 0.5) * s, py = (b + 0.5) * s; /* PAPER.md:312, reading G5 */
                         double theta = 2.0 * M_PI * (k + 0.5) / (double)N; /* reading G4 */
                         /* a1: the radiance interval of this probe and direction */
                         int n = i == 0 ? diag_segments(nx, ny, a, b, (int)k, ta, tb, seg)

@@ -1,0 +1,218 @@
+"""Thin ctypes binding over librc.so — same names as include/rc.h, argument marshalling only.
+
+Every step of the path (ray march, boundary, interpolate + merge, J) runs in the CUDA kernels
+behind the C ABI; PyTorch is used for device memory and streams.  There is no CPU fallback:
+`load()` raises if the library cannot be loaded.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+
+import numpy as np
+
+from . import build as _build
+
+RC_OK = 0
+RC_ACCUM_J, RC_VALIDATE, RC_NO_EARLY_EXIT = 1, 2, 4
+RC_MAX_CASCADES = 12
+ERRORS = {-1: "RC_ERR_NULL_ARG", -2: "RC_ERR_BAD_SHAPE", -3: "RC_ERR_NO_DEVICE", -4: "RC_ERR_NO_WORKSPACE",
+          -5: "RC_ERR_BAD_VALUE", -6: "RC_ERR_CUDA", -7: "RC_ERR_NO_ATMOSPHERE"}
+
+
+class rc_config(C.Structure):
+    _fields_ = [("ncascades", C.c_int), ("c0_interval", C.c_float), ("device", C.c_int),
+                ("lambda_batch", C.c_int), ("flags", C.c_int)]
+
+
+class rc_stats(C.Structure):
+    _fields_ = [("ncascades", C.c_int), ("lambda_batch", C.c_int), ("kernel_launches", C.c_int),
+                ("ms_cascade", C.c_float * RC_MAX_CASCADES), ("ms_prep", C.c_float), ("ms_total", C.c_float),
+                ("rays", C.c_int64 * RC_MAX_CASCADES), ("table_steps", C.c_int64 * RC_MAX_CASCADES),
+                ("workspace_bytes", C.c_size_t)]
+
+
+# every symbol include/rc.h declares: name -> (restype, argtypes)
+SYMBOLS = {
+    "rc_create": (C.c_int, [C.POINTER(C.c_void_p), C.POINTER(rc_config)]),
+    "rc_workspace_bytes": (C.c_size_t, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int]),
+    "rc_set_workspace": (C.c_int, [C.c_void_p, C.c_void_p, C.c_size_t]),
+    "rc_set_stream": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "rc_set_atmosphere": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int]),
+    "rc_set_boundary": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
+    "rc_set_lambda_weights": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "rc_solve_J": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "rc_solve_J_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p]),
+    "rc_set_timing": (C.c_int, [C.c_void_p, C.c_int]),
+    "rc_get_stats": (C.c_int, [C.c_void_p, C.POINTER(rc_stats)]),
+    "rc_last_error": (C.c_char_p, [C.c_void_p]),
+    "rc_version": (C.c_char_p, []),
+    "rc_destroy": (C.c_int, [C.c_void_p]),
+}
+
+_lib = None
+
+
+def library_path() -> Path:
+    return _build.LIB
+
+
+def load(build_if_missing: bool = True):
+    """dlopen librc.so (building it with nvcc first if it is missing or stale)."""
+    global _lib
+    if _lib is None:
+        if build_if_missing:
+            try:
+                _build.build()
+            except Exception:
+                if not _build.LIB.exists():
+                    raise
+        if not _build.LIB.exists():
+            raise RuntimeError(f"{_build.LIB} is missing: build it with paper_2408_14425_b200.build.build(); "
+                               "there is no CPU fallback")
+        lib = C.CDLL(str(_build.LIB))
+        for name, (res, args) in SYMBOLS.items():
+            fn = getattr(lib, name)
+            fn.restype, fn.argtypes = res, args
+        _lib = lib
+    return _lib
+
+
+class RcError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"{ERRORS.get(code, code)}: {msg}")
+        self.code = code
+
+
+def _host_f32(a, n):
+    if a is None:
+        return None, None
+    arr = np.ascontiguousarray(a, dtype=np.float32)
+    assert arr.size == n, f"expected {n} values, got {arr.size}"
+    return arr, arr.ctypes.data_as(C.c_void_p)
+
+
+class RadianceCascades:
+    """One rc_ctx plus the torch-owned workspace it borrows.  Methods mirror the C entry points."""
+
+    def __init__(self, ncascades, c0_interval=1.0, device=0, lambda_batch=0, flags=0):
+        self.lib = load()
+        self.cfg = rc_config(int(ncascades), float(c0_interval), int(device), int(lambda_batch), int(flags))
+        self.handle = C.c_void_p()
+        rc = self.lib.rc_create(C.byref(self.handle), C.byref(self.cfg))
+        if rc != RC_OK:
+            self.handle = C.c_void_p()
+            raise RcError(rc, "rc_create failed")
+        self.device = int(device)
+        self.flags = int(flags)
+        self._ws = None
+        self._keep = ()
+        self.shape = None
+
+    def _check(self, rc):
+        if rc != RC_OK:
+            raise RcError(rc, self.lib.rc_last_error(self.handle).decode())
+
+    def workspace_bytes(self, nx, ny, nlambda, host_io=False) -> int:
+        return int(self.lib.rc_workspace_bytes(self.handle, nx, ny, nlambda, int(host_io)))
+
+    def set_workspace(self, tensor):
+        self._ws = tensor
+        self._check(self.lib.rc_set_workspace(self.handle, C.c_void_p(tensor.data_ptr()), tensor.numel() * tensor.element_size()))
+
+    def ensure_workspace(self, nx, ny, nlambda, host_io=False):
+        import torch
+        need = self.workspace_bytes(nx, ny, nlambda, host_io)
+        if need == 0:
+            raise RcError(-2, f"bad shape {nx}x{ny}x{nlambda} for {self.cfg.ncascades} cascades")
+        if self._ws is None or self._ws.numel() < need:
+            self._ws = None
+            self.set_workspace(torch.empty(need, dtype=torch.uint8, device=f"cuda:{self.device}"))
+
+    def set_stream(self, stream=None):
+        import torch
+        s = torch.cuda.current_stream(self.device) if stream is None else stream
+        self._check(self.lib.rc_set_stream(self.handle, C.c_void_p(s.cuda_stream)))
+
+    def set_atmosphere(self, chi, eta):
+        """chi, eta: CUDA float32 tensors [ny][nx][nlambda] (borrowed until replaced)."""
+        assert chi.is_cuda and eta.is_cuda and chi.dtype == eta.dtype and chi.shape == eta.shape
+        assert chi.is_contiguous() and eta.is_contiguous() and chi.dim() == 3
+        ny, nx, L = chi.shape
+        self.ensure_workspace(nx, ny, L)
+        self.set_stream()
+        self._check(self.lib.rc_set_atmosphere(self.handle, C.c_void_p(chi.data_ptr()), C.c_void_p(eta.data_ptr()), nx, ny, L))
+        self._keep = (chi, eta)
+        self.shape = (ny, nx, L)
+
+    def set_boundary(self, I_below=None, I_above=None):
+        L = self.shape[2]
+        a, pa = _host_f32(I_below, L)
+        b, pb = _host_f32(I_above, L)
+        self._check(self.lib.rc_set_boundary(self.handle, pa, pb))
+
+    def set_lambda_weights(self, w=None):
+        a, pa = _host_f32(w, self.shape[2])
+        self._check(self.lib.rc_set_lambda_weights(self.handle, pa))
+
+    def solve_J(self, out=None):
+        """Enqueue one solve on torch's current stream; returns the output tensor (not synchronised)."""
+        import torch
+        ny, nx, L = self.shape
+        shape = (ny, nx) if self.flags & RC_ACCUM_J else (ny, nx, L)
+        if out is None:
+            out = torch.empty(shape, dtype=torch.float32, device=f"cuda:{self.device}")
+        assert out.is_cuda and out.is_contiguous() and tuple(out.shape) == shape
+        self.set_stream()
+        self._check(self.lib.rc_solve_J(self.handle, C.c_void_p(out.data_ptr())))
+        return out
+
+    def solve_J_host(self, chi_host, eta_host, out_host=None):
+        """Host tensors (ideally pinned) in, host tensor out; H2D + solve + D2H, synchronised."""
+        import torch
+        ny, nx, L = chi_host.shape
+        self.ensure_workspace(nx, ny, L, host_io=True)
+        self.set_stream()
+        shape = (ny, nx) if self.flags & RC_ACCUM_J else (ny, nx, L)
+        if out_host is None:
+            out_host = torch.empty(shape, dtype=torch.float32, pin_memory=True)
+        self._check(self.lib.rc_solve_J_host(self.handle, C.c_void_p(chi_host.data_ptr()), C.c_void_p(eta_host.data_ptr()),
+                                             nx, ny, L, C.c_void_p(out_host.data_ptr())))
+        self.shape = (ny, nx, L)
+        return out_host
+
+    def set_timing(self, on=True):
+        self._check(self.lib.rc_set_timing(self.handle, int(on)))
+
+    def get_stats(self) -> rc_stats:
+        st = rc_stats()
+        self._check(self.lib.rc_get_stats(self.handle, C.byref(st)))
+        return st
+
+    def close(self):
+        if self.handle:
+            self.lib.rc_destroy(self.handle)
+            self.handle = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def solve_atmosphere(atm, device=0, lambda_batch=0, flags=0, rc=None):
+    """Convenience for tests/bench: upload an `atmospheres.Atmosphere`, solve, return (J tensor, ctx)."""
+    import torch
+    dev = f"cuda:{device}"
+    fl = flags | (RC_ACCUM_J if atm.accumulate else 0)
+    if rc is None:
+        rc = RadianceCascades(atm.ncascades, atm.c0_interval, device, lambda_batch, fl)
+    chi = torch.from_numpy(atm.chi).to(dev)
+    eta = torch.from_numpy(atm.eta).to(dev)
+    rc.set_atmosphere(chi, eta)
+    rc.set_boundary(atm.I_below, atm.I_above)
+    rc.set_lambda_weights(atm.weights)
+    J = rc.solve_J()
+    torch.cuda.synchronize(device)
+    return J, rc

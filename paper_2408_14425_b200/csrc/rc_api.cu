@@ -1,0 +1,428 @@
+// rc_api.cu — the C ABI of include/rc.h: context, validation, workspace layout, launch sequence.
+// Host logic only; every arithmetic step of the path runs in rc_kernels.cu.  No CPU fallback.
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/rc.h"
+#include "rc_internal.h"
+
+namespace {
+
+constexpr size_t ALIGN = 256;
+inline size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
+
+struct CascadePlan {
+    long long ndir = 0;         // 4^(i+1)
+    bool empty = true;          // interval starts beyond the box diagonal: no ray of it is inside
+    long long slots = 0;        // step-table capacity, all directions
+    size_t off_off = 0, cnt_off = 0, steps_off = 0;  // byte offsets into the workspace
+    double ta = 0, tb = 0;
+};
+
+struct Plan {
+    int nx = 0, ny = 0, L = 0, ncasc = 0;
+    int LV = 1, nb = 1, Lpad = 1;
+    CascadePlan c[RC_MAX_CASCADES];
+    size_t chiT = 0, ST = 0, A[2] = {0, 0}, Jpart = 0, bc_below = 0, bc_above = 0, weights = 0, flag = 0;
+    size_t io_chi = 0, io_eta = 0, io_J = 0;
+    size_t total = 0;
+};
+
+}  // namespace
+
+struct rc_ctx {
+    rc_config cfg{};
+    cudaStream_t stream = nullptr;
+    char *ws = nullptr;
+    size_t ws_bytes = 0;
+    const float *chi = nullptr, *eta = nullptr;
+    Plan plan{};
+    bool have_atm = false;
+    int tab_nx = 0, tab_ny = 0;  // shape the step tables in the workspace were built for
+    bool host_io = false;
+    std::vector<std::vector<long long>> off_host;  // kept alive for the async uploads
+    std::vector<float> stage;                      // host staging for boundary / weights
+    bool timing = false, timed = false;
+    cudaEvent_t ev[RC_MAX_CASCADES + 2]{};
+    bool have_events = false;
+    rc_stats stats{};
+    char err[512] = {0};
+};
+
+namespace {
+
+int fail(rc_ctx *ctx, int code, const char *fmt, ...) {
+    if (ctx) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(ctx->err, sizeof(ctx->err), fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+#define RC_CUDA(ctx, call)                                                                       \
+    do {                                                                                         \
+        cudaError_t e_ = (call);                                                                 \
+        if (e_ != cudaSuccess)                                                                   \
+            return fail(ctx, RC_ERR_CUDA, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), \
+                        __FILE__, __LINE__);                                                     \
+    } while (0)
+
+// Interval ends, PAPER.md:171-176 (eq. 12-13) with alpha = 2: t_i = c0 (4^i - 1)/3.
+double t_of(int i, double c0) { return c0 * (std::pow(4.0, (double)i) - 1.0) / 3.0; }
+
+bool shape_ok(const rc_config &cfg, int nx, int ny, int L) {
+    if (nx <= 0 || ny <= 0 || L <= 0 || nx > RC_MAX_DIM || ny > RC_MAX_DIM) return false;
+    const int m = 1 << (cfg.ncascades - 1);
+    return nx % m == 0 && ny % m == 0;
+}
+
+int choose_lv(const rc_config &cfg, int L) {
+    if (cfg.lambda_batch == 1 || cfg.lambda_batch == 2 || cfg.lambda_batch == 4 || cfg.lambda_batch == 8)
+        return cfg.lambda_batch;
+    int lv = 1;
+    while (lv < L && lv < 8) lv <<= 1;
+    return lv;
+}
+
+// Workspace layout for a shape.  When `offs` is given, also fills the per-direction slot offsets.
+bool make_plan(const rc_config &cfg, int nx, int ny, int L, bool host_io, Plan &P,
+               std::vector<std::vector<long long>> *offs) {
+    if (!shape_ok(cfg, nx, ny, L)) return false;
+    P = Plan{};
+    P.nx = nx; P.ny = ny; P.L = L; P.ncasc = cfg.ncascades;
+    P.LV = choose_lv(cfg, L);
+    P.nb = (L + P.LV - 1) / P.LV;
+    P.Lpad = P.nb * P.LV;
+    const size_t ncell = (size_t)nx * ny;
+    const double diag = std::sqrt((double)nx * nx + (double)ny * ny);
+    const int top = cfg.ncascades - 1;
+    size_t cur = 0;
+    if (offs) offs->assign(cfg.ncascades, {});
+    for (int i = 0; i <= top; i++) {
+        CascadePlan &c = P.c[i];
+        c.ndir = 1LL << (2 * (i + 1));
+        c.ta = t_of(i, cfg.c0_interval);
+        c.tb = i == top ? INFINITY : t_of(i + 1, cfg.c0_interval);
+        c.empty = !(c.ta < diag);
+        c.slots = 0;
+        if (c.empty) continue;
+        std::vector<long long> local;
+        std::vector<long long> &o = offs ? (*offs)[i] : local;
+        o.resize((size_t)c.ndir + 1);
+        long long acc = 0;
+        for (long long k = 0; k < c.ndir; k++) {
+            o[(size_t)k] = acc;
+            long long n;
+            if (i == 0) {
+                const double cells = std::isinf(c.tb) ? (double)std::min(nx, ny)
+                                                      : std::min((double)std::min(nx, ny), std::ceil(c.tb / std::sqrt(2.0) + 0.5) + 1.0);
+                n = (long long)cells;
+            } else {
+                const double th = 2.0 * M_PI * ((double)k + 0.5) / (double)c.ndir;
+                const double wx = std::fabs(std::cos(th)), wy = std::fabs(std::sin(th));
+                const double tb = std::fmin(c.tb, std::fmin(nx / wx, ny / wy));
+                n = tb > c.ta ? (long long)((tb - c.ta) * (wx + wy)) + 6 : 0;
+            }
+            acc += n;
+        }
+        o[(size_t)c.ndir] = acc;
+        c.slots = acc;
+        c.off_off = cur;   cur = align_up(cur + sizeof(long long) * ((size_t)c.ndir + 1));
+        c.cnt_off = cur;   cur = align_up(cur + sizeof(int) * (size_t)c.ndir);
+        c.steps_off = cur; cur = align_up(cur + sizeof(rc::Step) * (size_t)acc);
+    }
+    const size_t field = align_up(ncell * P.Lpad * sizeof(float));
+    P.chiT = cur; cur += field;
+    P.ST = cur;   cur += field;
+    P.A[0] = cur; cur += field;
+    P.A[1] = cur; cur += field;
+    if (cfg.flags & RC_ACCUM_J) { P.Jpart = cur; cur += align_up(ncell * P.nb * sizeof(float)); }
+    P.bc_below = cur; cur += align_up(P.Lpad * sizeof(float));
+    P.bc_above = cur; cur += align_up(P.Lpad * sizeof(float));
+    P.weights = cur;  cur += align_up(P.Lpad * sizeof(float));
+    P.flag = cur;     cur += ALIGN;
+    if (host_io) {
+        const size_t io = align_up(ncell * L * sizeof(float));
+        P.io_chi = cur; cur += io;
+        P.io_eta = cur; cur += io;
+        P.io_J = cur;   cur += (cfg.flags & RC_ACCUM_J) ? align_up(ncell * sizeof(float)) : io;
+    }
+    P.total = cur;
+    return true;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------------
+// Exported C ABI
+// ------------------------------------------------------------------------------------------------
+extern "C" {
+
+const char *rc_version(void) { return "rc-b200 0.1 (sm_100a)"; }
+
+const char *rc_last_error(const rc_ctx *ctx) { return ctx ? ctx->err : "null context"; }
+
+int rc_create(rc_ctx **out, const rc_config *cfg) {
+    if (!out || !cfg) return RC_ERR_NULL_ARG;
+    *out = nullptr;
+    if (cfg->ncascades < 1 || cfg->ncascades > RC_MAX_CASCADES || !(cfg->c0_interval > 0.f) ||
+        !std::isfinite(cfg->c0_interval))
+        return RC_ERR_BAD_VALUE;
+    if (cfg->lambda_batch != 0 && cfg->lambda_batch != 1 && cfg->lambda_batch != 2 &&
+        cfg->lambda_batch != 4 && cfg->lambda_batch != 8)
+        return RC_ERR_BAD_VALUE;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || cfg->device < 0 || cfg->device >= ndev) {
+        cudaGetLastError();
+        return RC_ERR_NO_DEVICE;
+    }
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, cfg->device) != cudaSuccess || prop.major != 10)
+        return RC_ERR_NO_DEVICE;  // sm_100a code only: no other backend, no fallback
+    rc_ctx *ctx = new (std::nothrow) rc_ctx();
+    if (!ctx) return RC_ERR_CUDA;
+    ctx->cfg = *cfg;
+    *out = ctx;
+    return RC_OK;
+}
+
+int rc_destroy(rc_ctx *ctx) {
+    if (!ctx) return RC_ERR_NULL_ARG;
+    if (ctx->have_events) {
+        cudaSetDevice(ctx->cfg.device);
+        for (auto &e : ctx->ev) cudaEventDestroy(e);
+    }
+    delete ctx;
+    return RC_OK;
+}
+
+size_t rc_workspace_bytes(const rc_ctx *ctx, int nx, int ny, int nlambda, int host_io) {
+    if (!ctx) return 0;
+    Plan P;
+    if (!make_plan(ctx->cfg, nx, ny, nlambda, host_io != 0, P, nullptr)) return 0;
+    return P.total;
+}
+
+int rc_set_workspace(rc_ctx *ctx, void *dev_ptr, size_t bytes) {
+    if (!ctx) return RC_ERR_NULL_ARG;
+    if (!dev_ptr || ((uintptr_t)dev_ptr % ALIGN) != 0)
+        return fail(ctx, RC_ERR_NO_WORKSPACE, "workspace pointer is null or not %zu-byte aligned", ALIGN);
+    ctx->ws = (char *)dev_ptr;
+    ctx->ws_bytes = bytes;
+    ctx->tab_nx = ctx->tab_ny = 0;  // tables live in the workspace: rebuild
+    ctx->have_atm = false;
+    return RC_OK;
+}
+
+int rc_set_stream(rc_ctx *ctx, void *cuda_stream) {
+    if (!ctx) return RC_ERR_NULL_ARG;
+    ctx->stream = (cudaStream_t)cuda_stream;
+    return RC_OK;
+}
+
+int rc_set_timing(rc_ctx *ctx, int time_cascades) {
+    if (!ctx) return RC_ERR_NULL_ARG;
+    RC_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    if (time_cascades && !ctx->have_events) {
+        for (auto &e : ctx->ev) RC_CUDA(ctx, cudaEventCreate(&e));
+        ctx->have_events = true;
+    }
+    ctx->timing = time_cascades != 0;
+    ctx->timed = false;
+    return RC_OK;
+}
+
+int rc_set_atmosphere(rc_ctx *ctx, const float *chi, const float *eta, int nx, int ny, int nlambda) {
+    if (!ctx || !chi || !eta) return ctx ? fail(ctx, RC_ERR_NULL_ARG, "null chi/eta") : RC_ERR_NULL_ARG;
+    if (!shape_ok(ctx->cfg, nx, ny, nlambda))
+        return fail(ctx, RC_ERR_BAD_SHAPE, "nx=%d ny=%d nlambda=%d: need positive multiples of 2^(ncascades-1)=%d, <= %d",
+                    nx, ny, nlambda, 1 << (ctx->cfg.ncascades - 1), RC_MAX_DIM);
+    if (!ctx->ws) return fail(ctx, RC_ERR_NO_WORKSPACE, "rc_set_workspace has not been called");
+    RC_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    const bool same_shape = ctx->have_atm && ctx->plan.nx == nx && ctx->plan.ny == ny && ctx->plan.L == nlambda;
+    if (!same_shape) {
+        Plan P, Pio;
+        std::vector<std::vector<long long>> offs;
+        make_plan(ctx->cfg, nx, ny, nlambda, false, P, &offs);
+        if (P.total > ctx->ws_bytes)
+            return fail(ctx, RC_ERR_NO_WORKSPACE, "workspace has %zu bytes, %zu needed", ctx->ws_bytes, P.total);
+        make_plan(ctx->cfg, nx, ny, nlambda, true, Pio, nullptr);
+        ctx->host_io = Pio.total <= ctx->ws_bytes;
+        ctx->plan = ctx->host_io ? Pio : P;
+        ctx->have_atm = false;
+        // geometry tables: only when the grid size changed (they do not depend on nlambda)
+        if (ctx->tab_nx != nx || ctx->tab_ny != ny) {
+            ctx->off_host.swap(offs);
+            const int top = ctx->cfg.ncascades - 1;
+            for (int i = 0; i <= top; i++) {
+                const CascadePlan &c = ctx->plan.c[i];
+                ctx->stats.table_steps[i] = c.slots;
+                if (c.empty) continue;
+                RC_CUDA(ctx, cudaMemcpyAsync(ctx->ws + c.off_off, ctx->off_host[i].data(),
+                                             sizeof(long long) * ((size_t)c.ndir + 1), cudaMemcpyHostToDevice, ctx->stream));
+                rc::TableBuildParams tp;
+                tp.steps = (rc::Step *)(ctx->ws + c.steps_off);
+                tp.off = (const long long *)(ctx->ws + c.off_off);
+                tp.cnt = (int *)(ctx->ws + c.cnt_off);
+                tp.cascade = i; tp.top = i == top; tp.ndir = c.ndir;
+                tp.ta = c.ta; tp.tb = c.tb; tp.nx = nx; tp.ny = ny;
+                RC_CUDA(ctx, rc::launch_table_build(tp, ctx->stream));
+            }
+            ctx->tab_nx = nx; ctx->tab_ny = ny;
+        }
+        // defaults: free-space boundary, unit weights
+        ctx->stage.assign((size_t)ctx->plan.Lpad, 0.f);
+        RC_CUDA(ctx, cudaMemsetAsync(ctx->ws + ctx->plan.bc_below, 0, ctx->plan.Lpad * sizeof(float), ctx->stream));
+        RC_CUDA(ctx, cudaMemsetAsync(ctx->ws + ctx->plan.bc_above, 0, ctx->plan.Lpad * sizeof(float), ctx->stream));
+        std::vector<float> ones((size_t)ctx->plan.Lpad, 0.f);
+        for (int l = 0; l < nlambda; l++) ones[l] = 1.f;
+        RC_CUDA(ctx, cudaMemcpyAsync(ctx->ws + ctx->plan.weights, ones.data(), ones.size() * sizeof(float),
+                                     cudaMemcpyHostToDevice, ctx->stream));
+        RC_CUDA(ctx, cudaStreamSynchronize(ctx->stream));  // `ones` and the offsets are host temporaries
+    }
+    if (ctx->cfg.flags & RC_VALIDATE) {
+        int *flag = (int *)(ctx->ws + ctx->plan.flag);
+        int h = 0;
+        RC_CUDA(ctx, cudaMemsetAsync(flag, 0, sizeof(int), ctx->stream));
+        RC_CUDA(ctx, rc::launch_validate(chi, eta, (long long)nx * ny * nlambda, flag, ctx->stream));
+        RC_CUDA(ctx, cudaMemcpyAsync(&h, flag, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+        RC_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+        if (h & 1) return fail(ctx, RC_ERR_BAD_VALUE, "chi or eta has a negative or non-finite value");
+        if (h & 2) return fail(ctx, RC_ERR_BAD_VALUE, "eta > 0 in a cell with chi == 0");
+    }
+    ctx->chi = chi;
+    ctx->eta = eta;
+    ctx->have_atm = true;
+    return RC_OK;
+}
+
+static int upload_lambda_array(rc_ctx *ctx, const float *src, size_t dst_off, float fill) {
+    if (!ctx->have_atm) return fail(ctx, RC_ERR_NO_ATMOSPHERE, "call rc_set_atmosphere first");
+    RC_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    std::vector<float> h((size_t)ctx->plan.Lpad, 0.f);
+    for (int l = 0; l < ctx->plan.L; l++) h[l] = src ? src[l] : fill;
+    RC_CUDA(ctx, cudaMemcpyAsync(ctx->ws + dst_off, h.data(), h.size() * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
+    RC_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return RC_OK;
+}
+
+int rc_set_boundary(rc_ctx *ctx, const float *I_below, const float *I_above) {
+    if (!ctx) return RC_ERR_NULL_ARG;
+    int rc = upload_lambda_array(ctx, I_below, ctx->plan.bc_below, 0.f);
+    if (rc != RC_OK) return rc;
+    return upload_lambda_array(ctx, I_above, ctx->plan.bc_above, 0.f);
+}
+
+int rc_set_lambda_weights(rc_ctx *ctx, const float *w) {
+    if (!ctx) return RC_ERR_NULL_ARG;
+    return upload_lambda_array(ctx, w, ctx->plan.weights, 1.f);
+}
+
+// One full solve: for cascade i = top .. 0 { pack chi/eta for spacing 2^i ; march + merge }  (PAPER.md:207:
+// "after calculation, each interval of cascade i merges with the child intervals of cascade i+1.
+// Cascade i-1 is then computed and merged with cascade i").
+int rc_solve_J(rc_ctx *ctx, float *J_out) {
+    if (!ctx || !J_out) return ctx ? fail(ctx, RC_ERR_NULL_ARG, "null J_out") : RC_ERR_NULL_ARG;
+    if (!ctx->have_atm) return fail(ctx, RC_ERR_NO_ATMOSPHERE, "call rc_set_atmosphere first");
+    RC_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    const Plan &P = ctx->plan;
+    const int top = ctx->cfg.ncascades - 1;
+    const bool accum = (ctx->cfg.flags & RC_ACCUM_J) != 0;
+    const bool timing = ctx->timing && ctx->have_events;
+    int launches = 0;
+    if (timing) RC_CUDA(ctx, cudaEventRecord(ctx->ev[0], ctx->stream));
+    for (int i = top; i >= 0; i--) {
+        const CascadePlan &c = P.c[i];
+        if (!c.empty) {
+            rc::PackParams pp;
+            pp.chi = ctx->chi; pp.eta = ctx->eta;
+            pp.chiT = (float *)(ctx->ws + P.chiT); pp.ST = (float *)(ctx->ws + P.ST);
+            pp.nx = P.nx; pp.ny = P.ny; pp.L = P.L; pp.nb = P.nb; pp.shift = i;
+            RC_CUDA(ctx, rc::launch_pack(pp, P.LV, ctx->stream));
+            launches++;
+        }
+        rc::MarchParams mp;
+        mp.chiT = (const float *)(ctx->ws + P.chiT);
+        mp.ST = (const float *)(ctx->ws + P.ST);
+        mp.Aup = i == top ? nullptr : (const float *)(ctx->ws + P.A[(i + 1) & 1]);
+        mp.out = i > 0 ? (float *)(ctx->ws + P.A[i & 1]) : (accum ? (float *)(ctx->ws + P.Jpart) : J_out);
+        mp.steps = c.empty ? nullptr : (const rc::Step *)(ctx->ws + c.steps_off);
+        mp.off = c.empty ? nullptr : (const long long *)(ctx->ws + c.off_off);
+        mp.cnt = c.empty ? nullptr : (const int *)(ctx->ws + c.cnt_off);
+        mp.I_below = (const float *)(ctx->ws + P.bc_below);
+        mp.I_above = (const float *)(ctx->ws + P.bc_above);
+        mp.weights = (const float *)(ctx->ws + P.weights);
+        mp.nx = P.nx; mp.ny = P.ny; mp.L = P.L; mp.nb = P.nb;
+        mp.cascade = i; mp.shift = i;
+        mp.npx = P.nx >> i; mp.npy = P.ny >> i;
+        mp.ngroups = 1 << (2 * i);
+        mp.mode = i > 0 ? 0 : (accum ? 2 : 1);
+        mp.early_exit = (ctx->cfg.flags & RC_NO_EARLY_EXIT) ? 0 : 1;
+        mp.group_major = 0;
+        RC_CUDA(ctx, rc::launch_march(mp, P.LV, ctx->stream));
+        launches++;
+        if (timing) RC_CUDA(ctx, cudaEventRecord(ctx->ev[1 + (top - i)], ctx->stream));
+    }
+    if (accum) {
+        RC_CUDA(ctx, rc::launch_reduce_jbar((const float *)(ctx->ws + P.Jpart), J_out, (long long)P.nx * P.ny, P.nb, ctx->stream));
+        launches++;
+    }
+    if (timing) {
+        RC_CUDA(ctx, cudaEventRecord(ctx->ev[top + 2], ctx->stream));
+        ctx->timed = true;
+    }
+    ctx->stats.kernel_launches = launches;
+    return RC_OK;
+}
+
+int rc_solve_J_host(rc_ctx *ctx, const float *chi_host, const float *eta_host, int nx, int ny,
+                    int nlambda, float *J_host) {
+    if (!ctx || !chi_host || !eta_host || !J_host) return ctx ? fail(ctx, RC_ERR_NULL_ARG, "null host buffer") : RC_ERR_NULL_ARG;
+    if (!shape_ok(ctx->cfg, nx, ny, nlambda)) return fail(ctx, RC_ERR_BAD_SHAPE, "bad shape %dx%dx%d", nx, ny, nlambda);
+    if (!ctx->ws) return fail(ctx, RC_ERR_NO_WORKSPACE, "rc_set_workspace has not been called");
+    RC_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    Plan Pio;
+    make_plan(ctx->cfg, nx, ny, nlambda, true, Pio, nullptr);
+    if (Pio.total > ctx->ws_bytes)
+        return fail(ctx, RC_ERR_NO_WORKSPACE, "workspace has %zu bytes, %zu needed with host_io", ctx->ws_bytes, Pio.total);
+    const size_t n = (size_t)nx * ny * nlambda * sizeof(float);
+    float *dchi = (float *)(ctx->ws + Pio.io_chi), *deta = (float *)(ctx->ws + Pio.io_eta), *dJ = (float *)(ctx->ws + Pio.io_J);
+    RC_CUDA(ctx, cudaMemcpyAsync(dchi, chi_host, n, cudaMemcpyHostToDevice, ctx->stream));
+    RC_CUDA(ctx, cudaMemcpyAsync(deta, eta_host, n, cudaMemcpyHostToDevice, ctx->stream));
+    int rc = rc_set_atmosphere(ctx, dchi, deta, nx, ny, nlambda);
+    if (rc != RC_OK) return rc;
+    rc = rc_solve_J(ctx, dJ);
+    if (rc != RC_OK) return rc;
+    const size_t nout = (ctx->cfg.flags & RC_ACCUM_J) ? (size_t)nx * ny * sizeof(float) : n;
+    RC_CUDA(ctx, cudaMemcpyAsync(J_host, dJ, nout, cudaMemcpyDeviceToHost, ctx->stream));
+    RC_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return RC_OK;
+}
+
+int rc_get_stats(rc_ctx *ctx, rc_stats *out) {
+    if (!ctx || !out) return RC_ERR_NULL_ARG;
+    rc_stats &s = ctx->stats;
+    s.ncascades = ctx->cfg.ncascades;
+    s.lambda_batch = ctx->plan.LV;
+    s.workspace_bytes = ctx->plan.total;
+    const int top = ctx->cfg.ncascades - 1;
+    for (int i = 0; i <= top; i++) s.rays[i] = 4LL * ctx->plan.nx * ctx->plan.ny;
+    if (ctx->timed) {
+        RC_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+        RC_CUDA(ctx, cudaEventSynchronize(ctx->ev[top + 2]));
+        for (int i = top; i >= 0; i--)
+            RC_CUDA(ctx, cudaEventElapsedTime(&s.ms_cascade[i], ctx->ev[top - i], ctx->ev[top - i + 1]));
+        RC_CUDA(ctx, cudaEventElapsedTime(&s.ms_total, ctx->ev[0], ctx->ev[top + 2]));
+        s.ms_prep = 0.f;
+    }
+    *out = s;
+    return RC_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,68 @@
+// rc_internal.h — shared between rc_api.cu (C ABI, host logic) and rc_kernels.cu (sm_100a kernels).
+// Not part of the public interface (include/rc.h is).  Nothing here is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace rc {
+
+// One step of a ray through the grid: the cell it is in, relative to the probe's lattice vertex
+// (cascade i >= 1) or cell (cascade 0), and the path length inside that cell.  8 bytes.
+struct Step {
+    int16_t dx, dy;
+    float ds;
+};
+
+// Per-cascade geometry tables (device memory, inside the workspace).
+struct CascadeTable {
+    const Step *steps;      // all directions back to back
+    const long long *off;   // [N+1] start of direction k's slot in `steps` (host-computed bounds)
+    const int *cnt;         // [N]   entries actually used by direction k (device-built)
+    long long total_slots;  // sum of slot sizes
+    int empty;              // every direction's interval lies outside any box of this size
+};
+
+struct MarchParams {
+    const float *chiT;  // packed opacity * log2(e): [nb][ny][s][npx][LV]  (x split as xm = x mod s, xd = x div s)
+    const float *ST;    // packed source function eta/chi, same layout
+    const float *Aup;   // merged cascade i+1, pre-averaged over the 4 children: [nb][N_i][npy/2][npx/2][LV]; null on the top cascade
+    float *out;         // mode 0: A_i [nb][N_i/4][npy][npx][LV]; mode 1: J [ny][nx][L]; mode 2: Jpart [nb][ny][nx]
+    const Step *steps;
+    const long long *off;
+    const int *cnt;
+    const float *I_below;  // [Lpad] device
+    const float *I_above;  // [Lpad] device
+    const float *weights;  // [Lpad] device
+    int nx, ny, L, nb;
+    int cascade, shift;    // s = 1 << shift
+    int npx, npy;          // probes per axis of this cascade
+    int ngroups;           // direction groups = 4^cascade (4 directions each)
+    int mode;
+    int early_exit;
+    int group_major;       // warp order: 0 = direction group fastest, 1 = probe chunk fastest
+};
+
+struct PackParams {
+    const float *chi, *eta;  // [ny][nx][L]
+    float *chiT, *ST;        // [nb][ny][s][npx][LV]
+    int nx, ny, L, nb, shift;
+};
+
+struct TableBuildParams {
+    Step *steps;
+    const long long *off;
+    int *cnt;
+    int cascade, top;
+    long long ndir;
+    double ta, tb;  // interval ends (tb = +inf on the top cascade)
+    int nx, ny;
+};
+
+// launchers (rc_kernels.cu); LV in {1,2,4,8}
+cudaError_t launch_pack(const PackParams &p, int LV, cudaStream_t st);
+cudaError_t launch_march(const MarchParams &p, int LV, cudaStream_t st);
+cudaError_t launch_table_build(const TableBuildParams &p, cudaStream_t st);
+cudaError_t launch_reduce_jbar(const float *Jpart, float *Jbar, long long ncell, int nb, cudaStream_t st);
+cudaError_t launch_validate(const float *chi, const float *eta, long long n, int *flag, cudaStream_t st);
+
+}  // namespace rc
