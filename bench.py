@@ -1,0 +1,259 @@
+#!/usr/bin/env python
+"""bench.py — one JSON line for the radiance-cascades hot path.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl ours|reference]
+
+A "step" is one full J solve (every cascade: pack, march, boundary, merge, J) of one synthetic
+atmosphere.  Default workload: BASELINE.json configs[2] (1024x1024 cells, 64 wavelengths, 8 cascades),
+the configuration the metric's target is quoted on.  value = probe-ray-wavelength segments per second,
+whole job, inputs resident in HBM; e2e = the same through rc_solve_J_host with pinned HOST buffers
+(H2D of chi, eta and D2H of J inside the timed region).  N > 1: one process per GPU, each solving its
+own wavelength block of 64 (the path shards by wavelength with no exchange) - weak scaling.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+sys.path.insert(0, str(ROOT))
+
+from paper_2408_14425_b200 import atmospheres  # noqa: E402
+
+METRIC = "probe-ray-wavelength segments/sec"
+UNIT = "seg-lambda/s"
+SM_COUNT, MUFU_PER_CLK_SM = 148, 16  # one ex2 per segment-wavelength; DESIGN.md §7
+
+
+def peaks():
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        d = json.loads(p.read_text())
+        return float(d["hbm_gbs"]), float(d.get("sm_max_mhz", 1965.0)), "measured (MEASURED_PEAKS.json)"
+    return 6650.0, 1965.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+    NAMES = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+
+    def __init__(self, index):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100", "-i", str(self.index)], stdout=subprocess.PIPE, text=True)
+            threading.Thread(target=lambda: self.lines.extend(self.proc.stdout), daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, v in zip(self.NAMES, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_sample(atm, nwin, size=8, seed=0):
+    """Time the fp64 oracle, as it stands, on `nwin` windows of size x size cells (all wavelengths)."""
+    from oracle import rc_oracle
+    rc_oracle.build()
+    rng = np.random.default_rng(seed)
+    segl, secs = 0, 0.0
+    for _ in range(nwin):
+        x0 = int(rng.integers(0, atm.nx - size + 1))
+        y0 = int(rng.integers(0, atm.ny - size + 1))
+        t = time.perf_counter()
+        out = rc_oracle.solve_atmosphere(atm, window=(x0, x0 + size, y0, y0 + size), want_counts=True)
+        secs += time.perf_counter() - t
+        segl += int(out["segments"].sum()) * atm.nlambda
+    return segl, secs, rc_oracle.num_threads()
+
+
+def run_reference(args, atm, workload):
+    """--impl reference: the oracle on the host cores, each step a bounded sample of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    oracle_sample(atm, args.warmup, seed=99)
+    segl, secs, cores = oracle_sample(atm, args.steps, seed=7)
+    v = segl / secs
+    sample = f"{args.steps} windows of 8x8 cells x {atm.nlambda} wavelengths (all cascades they depend on), one per step"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * secs / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": {"workload": workload},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=2)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--lambda-batch", type=int, default=0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    fx, fy, fl, fc = atmospheres.FULL_SHAPES[args.config]
+    workload = (f"BASELINE.json configs[{args.config}]: {fx}x{fy} cells, {fl} wavelengths, {fc} cascades, "
+                f"seeded synthetic atmosphere (DESIGN.md §4)")
+    atm = atmospheres.make_config(args.config, seed=1000 + args.config + 17 * rank)
+    if args.impl == "reference":
+        run_reference(args, atm, workload)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_2408_14425_b200 import binding
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
+    torch.cuda.set_device(local_rank)
+    dev = f"cuda:{local_rank}"
+    hbm_peak, sm_max_mhz, peak_src = peaks()
+
+    flags = binding.RC_ACCUM_J if atm.accumulate else 0
+    rc = binding.RadianceCascades(atm.ncascades, atm.c0_interval, local_rank, args.lambda_batch, flags)
+    rc.ensure_workspace(atm.nx, atm.ny, atm.nlambda, host_io=True)
+    chi_h = torch.from_numpy(atm.chi).pin_memory()
+    eta_h = torch.from_numpy(atm.eta).pin_memory()
+    chi, eta = chi_h.to(dev), eta_h.to(dev)
+    rc.set_atmosphere(chi, eta)
+    rc.set_boundary(atm.I_below, atm.I_above)
+    rc.set_lambda_weights(atm.weights)
+    seg = rc.count_segments()
+    segl_per_step = sum(seg) * atm.nlambda
+    J = rc.solve_J()
+    for _ in range(args.warmup - 1):
+        rc.solve_J(out=J)
+    torch.cuda.synchronize()
+    rc.set_timing(args.steps)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier(); torch.cuda.synchronize()
+    e0.record()
+    for _ in range(args.steps):
+        rc.solve_J(out=J)
+    e1.record()
+    torch.cuda.synchronize(); barrier()
+    clocks = sampler.stop()
+    ms = torch.tensor([e0.elapsed_time(e1)], device=dev)
+    if world > 1:
+        dist.all_reduce(ms, op=dist.ReduceOp.MAX)
+    ms_total = float(ms.item())
+    st = rc.get_stats()
+    launches = st.kernel_launches * args.steps
+    rc.set_timing(0)
+
+    # end to end: host buffers in, host buffer out, every step
+    out_h = torch.empty(J.shape, dtype=torch.float32, pin_memory=True)
+    rc.solve_J_host(chi_h, eta_h, out_h)
+    rc.set_boundary(atm.I_below, atm.I_above)
+    rc.set_lambda_weights(atm.weights)
+    rc.solve_J_host(chi_h, eta_h, out_h)
+    barrier(); torch.cuda.synchronize()
+    e0.record()
+    for _ in range(args.e2e_steps):
+        rc.solve_J_host(chi_h, eta_h, out_h)
+    e1.record()
+    torch.cuda.synchronize(); barrier()
+    ms2 = torch.tensor([e0.elapsed_time(e1)], device=dev)
+    if world > 1:
+        dist.all_reduce(ms2, op=dist.ReduceOp.MAX)
+    e2e_ms = float(ms2.item()) / args.e2e_steps
+    same = bool(torch.equal(out_h, J.cpu()))
+
+    if rank == 0:
+        ms_step = ms_total / args.steps
+        value = world * segl_per_step / (ms_step * 1e-3)
+        # dominant kernel: the march+merge launch of the heaviest cascade
+        ms_march = [st.ms_march[i] for i in range(atm.ncascades)]
+        dom = int(np.argmax(ms_march))
+        casc_bytes = 2 * 4 * atm.nx * atm.ny * atm.nlambda  # read merged cascade i+1, write cascade i
+        alg_bytes = 8 * seg[dom] * atm.nlambda + casc_bytes  # chi+eta gather: 8 B per segment-wavelength
+        ach = alg_bytes / (ms_march[dom] * 1e-3) / 1e9
+        sfu_peak = SM_COUNT * MUFU_PER_CLK_SM * sm_max_mhz * 1e6
+        ach_alu = seg[dom] * atm.nlambda / (ms_march[dom] * 1e-3)
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+            "data": "synthetic",
+            "config": {"workload": workload, "seg_lambda_per_step_per_gpu": segl_per_step, "lambda_batch": st.lambda_batch,
+                       "l2": "inputs (chi+eta %.0f MB) larger than L2" % (2 * atm.chi.nbytes / 1e6),
+                       "parallelism": f"wavelength blocks x{world}, no collective"},
+            "solve_ms": ms_step,
+            "hbm_effective_frac": (8 * segl_per_step + 2 * casc_bytes * atm.ncascades) / (ms_step * 1e-3) / 1e9 / hbm_peak,
+            "roofline": {"bound": "hbm", "kernel": f"march_kernel<{st.lambda_batch}> cascade {dom}", "achieved": ach,
+                         "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak, "traffic": None,
+                         "peak_source": peak_src, "ms_per_launch": ms_march[dom],
+                         "note": "effective: algorithmic gather bytes (8 B per segment-wavelength) are mostly served "
+                                 "from L1/L2, so frac may exceed 1; see roofline_alu for the binding on-chip ceiling"},
+            "roofline_alu": {"bound": "alu", "pipe": "MUFU.EX2, 16/clk/SM x 148 SMs at sm_max_mhz", "achieved": ach_alu,
+                             "peak": sfu_peak, "unit": UNIT, "frac": ach_alu / sfu_peak},
+            "per_cascade_ms": {"march": ms_march, "pack": [st.ms_pack[i] for i in range(atm.ncascades)]},
+            "segments_per_cascade": seg,
+            "e2e": {"value": world * segl_per_step / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms,
+                    "h2d_bytes_per_step": int(2 * atm.chi.nbytes), "d2h_bytes_per_step": int(out_h.numel() * 4),
+                    "matches_device_path": same},
+            "gpu_launches": launches, "clocks": clocks,
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            nwin = 3
+            segl, secs, cores = oracle_sample(atm, nwin)
+            line["cpu_baseline"] = {"value": segl / secs, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                    "sample": f"{nwin} windows of 8x8 cells x {atm.nlambda} wavelengths, "
+                                              f"{segl:.3e} segment-wavelengths in {secs:.1f} s"}
+        print(json.dumps(line))
+    rc.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -78,9 +78,10 @@ typedef struct {
     int ncascades;
     int lambda_batch;                     /* wavelengths per thread actually used */
     int kernel_launches;                  /* kernels enqueued by the last rc_solve_J */
-    float ms_cascade[RC_MAX_CASCADES];    /* device time per cascade (pack + march), last timed solve */
-    float ms_prep;                        /* chi,eta -> (chi log2e, S) repack */
-    float ms_total;
+    int solves_timed;                     /* solves the ms_* figures average over (rc_set_timing) */
+    float ms_pack[RC_MAX_CASCADES];       /* mean device ms of cascade i's pack kernel  */
+    float ms_march[RC_MAX_CASCADES];      /* mean device ms of cascade i's march+merge kernel */
+    float ms_total;                       /* mean device ms of a whole solve */
     int64_t rays[RC_MAX_CASCADES];        /* intervals per cascade per wavelength = 4 nx ny */
     int64_t table_steps[RC_MAX_CASCADES]; /* step-table entries per cascade (all directions) */
     size_t workspace_bytes;
@@ -120,9 +121,16 @@ int rc_solve_J(rc_ctx *ctx, float *J_out);
 int rc_solve_J_host(rc_ctx *ctx, const float *chi_host, const float *eta_host, int nx, int ny,
                     int nlambda, float *J_host);
 
-/* time_cascades != 0 makes the next solves record per-cascade CUDA-event times (adds events only). */
-int rc_set_timing(rc_ctx *ctx, int time_cascades);
-int rc_get_stats(rc_ctx *ctx, rc_stats *out); /* synchronises the timing events of the last solve */
+/* nsets > 0: the next solves record CUDA events on the context's stream around every kernel, solve
+ * number n into event set n % nsets (no synchronisation is added); 0 switches timing off.
+ * rc_get_stats waits for the recorded sets and averages over them. */
+int rc_set_timing(rc_ctx *ctx, int nsets);
+int rc_get_stats(rc_ctx *ctx, rc_stats *out);
+
+/* Geometric work of one solve, the unit of the throughput metric: per_cascade[i] (host,
+ * [ncascades]) = number of (probe, direction) cell segments of cascade i inside the box, per
+ * wavelength.  Counted on the device from the step tables; synchronises. */
+int rc_count_segments(rc_ctx *ctx, int64_t *per_cascade);
 
 const char *rc_last_error(const rc_ctx *ctx);
 const char *rc_version(void);

@@ -27,7 +27,8 @@ class rc_config(C.Structure):
 
 class rc_stats(C.Structure):
     _fields_ = [("ncascades", C.c_int), ("lambda_batch", C.c_int), ("kernel_launches", C.c_int),
-                ("ms_cascade", C.c_float * RC_MAX_CASCADES), ("ms_prep", C.c_float), ("ms_total", C.c_float),
+                ("solves_timed", C.c_int), ("ms_pack", C.c_float * RC_MAX_CASCADES),
+                ("ms_march", C.c_float * RC_MAX_CASCADES), ("ms_total", C.c_float),
                 ("rays", C.c_int64 * RC_MAX_CASCADES), ("table_steps", C.c_int64 * RC_MAX_CASCADES),
                 ("workspace_bytes", C.c_size_t)]
 
@@ -45,6 +46,7 @@ SYMBOLS = {
     "rc_solve_J_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p]),
     "rc_set_timing": (C.c_int, [C.c_void_p, C.c_int]),
     "rc_get_stats": (C.c_int, [C.c_void_p, C.POINTER(rc_stats)]),
+    "rc_count_segments": (C.c_int, [C.c_void_p, C.c_void_p]),
     "rc_last_error": (C.c_char_p, [C.c_void_p]),
     "rc_version": (C.c_char_p, []),
     "rc_destroy": (C.c_int, [C.c_void_p]),
@@ -181,8 +183,14 @@ class RadianceCascades:
         self.shape = (ny, nx, L)
         return out_host
 
-    def set_timing(self, on=True):
-        self._check(self.lib.rc_set_timing(self.handle, int(on)))
+    def set_timing(self, nsets=1):
+        self._check(self.lib.rc_set_timing(self.handle, int(nsets)))
+
+    def count_segments(self):
+        """Per-cascade geometric segment counts (per wavelength) of the current atmosphere's grid."""
+        out = (C.c_int64 * RC_MAX_CASCADES)()
+        self._check(self.lib.rc_count_segments(self.handle, out))
+        return [int(out[i]) for i in range(self.cfg.ncascades)]
 
     def get_stats(self) -> rc_stats:
         st = rc_stats()

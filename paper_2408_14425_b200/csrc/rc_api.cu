@@ -1,5 +1,6 @@
 // rc_api.cu — the C ABI of include/rc.h: context, validation, workspace layout, launch sequence.
 // Host logic only; every arithmetic step of the path runs in rc_kernels.cu.  No CPU fallback.
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -46,9 +47,10 @@ struct rc_ctx {
     bool host_io = false;
     std::vector<std::vector<long long>> off_host;  // kept alive for the async uploads
     std::vector<float> stage;                      // host staging for boundary / weights
-    bool timing = false, timed = false;
-    cudaEvent_t ev[RC_MAX_CASCADES + 2]{};
-    bool have_events = false;
+    // timing: `nsets` rings of (2 per cascade + 2) events; solve number n records into set n % nsets
+    int nsets = 0;
+    long long solves_timed = 0;
+    std::vector<cudaEvent_t> ev;
     rc_stats stats{};
     char err[512] = {0};
 };
@@ -194,7 +196,7 @@ int rc_create(rc_ctx **out, const rc_config *cfg) {
 
 int rc_destroy(rc_ctx *ctx) {
     if (!ctx) return RC_ERR_NULL_ARG;
-    if (ctx->have_events) {
+    if (!ctx->ev.empty()) {
         cudaSetDevice(ctx->cfg.device);
         for (auto &e : ctx->ev) cudaEventDestroy(e);
     }
@@ -226,15 +228,17 @@ int rc_set_stream(rc_ctx *ctx, void *cuda_stream) {
     return RC_OK;
 }
 
-int rc_set_timing(rc_ctx *ctx, int time_cascades) {
+int rc_set_timing(rc_ctx *ctx, int nsets) {
     if (!ctx) return RC_ERR_NULL_ARG;
+    if (nsets < 0 || nsets > 4096) return fail(ctx, RC_ERR_BAD_VALUE, "nsets must be in [0, 4096]");
     RC_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
-    if (time_cascades && !ctx->have_events) {
-        for (auto &e : ctx->ev) RC_CUDA(ctx, cudaEventCreate(&e));
-        ctx->have_events = true;
-    }
-    ctx->timing = time_cascades != 0;
-    ctx->timed = false;
+    for (auto &e : ctx->ev) cudaEventDestroy(e);
+    ctx->ev.clear();
+    const int per = 2 * ctx->cfg.ncascades + 2;
+    ctx->ev.resize((size_t)nsets * per);
+    for (auto &e : ctx->ev) RC_CUDA(ctx, cudaEventCreate(&e));
+    ctx->nsets = nsets;
+    ctx->solves_timed = 0;
     return RC_OK;
 }
 
@@ -324,6 +328,33 @@ int rc_set_lambda_weights(rc_ctx *ctx, const float *w) {
     return upload_lambda_array(ctx, w, ctx->plan.weights, 1.f);
 }
 
+// Parameters of cascade i's march launch.
+static rc::MarchParams march_params(const rc_ctx *ctx, int i, float *J_out) {
+    const Plan &P = ctx->plan;
+    const CascadePlan &c = P.c[i];
+    const int top = ctx->cfg.ncascades - 1;
+    const bool accum = (ctx->cfg.flags & RC_ACCUM_J) != 0;
+    rc::MarchParams mp;
+    mp.chiT = (const float *)(ctx->ws + P.chiT);
+    mp.ST = (const float *)(ctx->ws + P.ST);
+    mp.Aup = i == top ? nullptr : (const float *)(ctx->ws + P.A[(i + 1) & 1]);
+    mp.out = i > 0 ? (float *)(ctx->ws + P.A[i & 1]) : (accum ? (float *)(ctx->ws + P.Jpart) : J_out);
+    mp.steps = c.empty ? nullptr : (const rc::Step *)(ctx->ws + c.steps_off);
+    mp.off = c.empty ? nullptr : (const long long *)(ctx->ws + c.off_off);
+    mp.cnt = c.empty ? nullptr : (const int *)(ctx->ws + c.cnt_off);
+    mp.I_below = (const float *)(ctx->ws + P.bc_below);
+    mp.I_above = (const float *)(ctx->ws + P.bc_above);
+    mp.weights = (const float *)(ctx->ws + P.weights);
+    mp.nx = P.nx; mp.ny = P.ny; mp.L = P.L; mp.nb = P.nb;
+    mp.cascade = i; mp.shift = i;
+    mp.npx = P.nx >> i; mp.npy = P.ny >> i;
+    mp.ngroups = 1 << (2 * i);
+    mp.mode = i > 0 ? 0 : (accum ? 2 : 1);
+    mp.early_exit = (ctx->cfg.flags & RC_NO_EARLY_EXIT) ? 0 : 1;
+    mp.group_major = 0;
+    return mp;
+}
+
 // One full solve: for cascade i = top .. 0 { pack chi/eta for spacing 2^i ; march + merge }  (PAPER.md:207:
 // "after calculation, each interval of cascade i merges with the child intervals of cascade i+1.
 // Cascade i-1 is then computed and merged with cascade i").
@@ -334,9 +365,10 @@ int rc_solve_J(rc_ctx *ctx, float *J_out) {
     const Plan &P = ctx->plan;
     const int top = ctx->cfg.ncascades - 1;
     const bool accum = (ctx->cfg.flags & RC_ACCUM_J) != 0;
-    const bool timing = ctx->timing && ctx->have_events;
+    const int per = 2 * ctx->cfg.ncascades + 2;
+    cudaEvent_t *ev = ctx->nsets > 0 ? ctx->ev.data() + (size_t)(ctx->solves_timed % ctx->nsets) * per : nullptr;
     int launches = 0;
-    if (timing) RC_CUDA(ctx, cudaEventRecord(ctx->ev[0], ctx->stream));
+    if (ev) RC_CUDA(ctx, cudaEventRecord(ev[0], ctx->stream));
     for (int i = top; i >= 0; i--) {
         const CascadePlan &c = P.c[i];
         if (!c.empty) {
@@ -347,37 +379,36 @@ int rc_solve_J(rc_ctx *ctx, float *J_out) {
             RC_CUDA(ctx, rc::launch_pack(pp, P.LV, ctx->stream));
             launches++;
         }
-        rc::MarchParams mp;
-        mp.chiT = (const float *)(ctx->ws + P.chiT);
-        mp.ST = (const float *)(ctx->ws + P.ST);
-        mp.Aup = i == top ? nullptr : (const float *)(ctx->ws + P.A[(i + 1) & 1]);
-        mp.out = i > 0 ? (float *)(ctx->ws + P.A[i & 1]) : (accum ? (float *)(ctx->ws + P.Jpart) : J_out);
-        mp.steps = c.empty ? nullptr : (const rc::Step *)(ctx->ws + c.steps_off);
-        mp.off = c.empty ? nullptr : (const long long *)(ctx->ws + c.off_off);
-        mp.cnt = c.empty ? nullptr : (const int *)(ctx->ws + c.cnt_off);
-        mp.I_below = (const float *)(ctx->ws + P.bc_below);
-        mp.I_above = (const float *)(ctx->ws + P.bc_above);
-        mp.weights = (const float *)(ctx->ws + P.weights);
-        mp.nx = P.nx; mp.ny = P.ny; mp.L = P.L; mp.nb = P.nb;
-        mp.cascade = i; mp.shift = i;
-        mp.npx = P.nx >> i; mp.npy = P.ny >> i;
-        mp.ngroups = 1 << (2 * i);
-        mp.mode = i > 0 ? 0 : (accum ? 2 : 1);
-        mp.early_exit = (ctx->cfg.flags & RC_NO_EARLY_EXIT) ? 0 : 1;
-        mp.group_major = 0;
-        RC_CUDA(ctx, rc::launch_march(mp, P.LV, ctx->stream));
+        if (ev) RC_CUDA(ctx, cudaEventRecord(ev[1 + 2 * (top - i)], ctx->stream));
+        RC_CUDA(ctx, rc::launch_march(march_params(ctx, i, J_out), P.LV, ctx->stream));
         launches++;
-        if (timing) RC_CUDA(ctx, cudaEventRecord(ctx->ev[1 + (top - i)], ctx->stream));
+        if (ev) RC_CUDA(ctx, cudaEventRecord(ev[2 + 2 * (top - i)], ctx->stream));
     }
     if (accum) {
         RC_CUDA(ctx, rc::launch_reduce_jbar((const float *)(ctx->ws + P.Jpart), J_out, (long long)P.nx * P.ny, P.nb, ctx->stream));
         launches++;
     }
-    if (timing) {
-        RC_CUDA(ctx, cudaEventRecord(ctx->ev[top + 2], ctx->stream));
-        ctx->timed = true;
+    if (ev) {
+        RC_CUDA(ctx, cudaEventRecord(ev[per - 1], ctx->stream));
+        ctx->solves_timed++;
     }
     ctx->stats.kernel_launches = launches;
+    return RC_OK;
+}
+
+// Geometric segment count per cascade and wavelength (the unit of the throughput metric).
+int rc_count_segments(rc_ctx *ctx, int64_t *per_cascade) {
+    if (!ctx || !per_cascade) return ctx ? fail(ctx, RC_ERR_NULL_ARG, "null output") : RC_ERR_NULL_ARG;
+    if (!ctx->have_atm) return fail(ctx, RC_ERR_NO_ATMOSPHERE, "call rc_set_atmosphere first");
+    RC_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    unsigned long long *d = (unsigned long long *)(ctx->ws + ctx->plan.flag);
+    RC_CUDA(ctx, cudaMemsetAsync(d, 0, ALIGN, ctx->stream));
+    for (int i = 0; i < ctx->cfg.ncascades; i++)
+        if (!ctx->plan.c[i].empty) RC_CUDA(ctx, rc::launch_count(march_params(ctx, i, nullptr), d + i, ctx->stream));
+    unsigned long long h[RC_MAX_CASCADES];
+    RC_CUDA(ctx, cudaMemcpyAsync(h, d, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream));
+    RC_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    for (int i = 0; i < ctx->cfg.ncascades; i++) per_cascade[i] = (int64_t)h[i];
     return RC_OK;
 }
 
@@ -412,14 +443,27 @@ int rc_get_stats(rc_ctx *ctx, rc_stats *out) {
     s.lambda_batch = ctx->plan.LV;
     s.workspace_bytes = ctx->plan.total;
     const int top = ctx->cfg.ncascades - 1;
-    for (int i = 0; i <= top; i++) s.rays[i] = 4LL * ctx->plan.nx * ctx->plan.ny;
-    if (ctx->timed) {
+    for (int i = 0; i <= top; i++) { s.rays[i] = 4LL * ctx->plan.nx * ctx->plan.ny; s.ms_pack[i] = s.ms_march[i] = 0.f; }
+    s.ms_total = 0.f;
+    s.solves_timed = (int)std::min<long long>(ctx->solves_timed, ctx->nsets);
+    if (s.solves_timed > 0) {
         RC_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
-        RC_CUDA(ctx, cudaEventSynchronize(ctx->ev[top + 2]));
-        for (int i = top; i >= 0; i--)
-            RC_CUDA(ctx, cudaEventElapsedTime(&s.ms_cascade[i], ctx->ev[top - i], ctx->ev[top - i + 1]));
-        RC_CUDA(ctx, cudaEventElapsedTime(&s.ms_total, ctx->ev[0], ctx->ev[top + 2]));
-        s.ms_prep = 0.f;
+        const int per = 2 * ctx->cfg.ncascades + 2;
+        for (int n = 0; n < s.solves_timed; n++) {
+            cudaEvent_t *ev = ctx->ev.data() + (size_t)n * per;
+            RC_CUDA(ctx, cudaEventSynchronize(ev[per - 1]));
+            float ms;
+            for (int i = top; i >= 0; i--) {
+                RC_CUDA(ctx, cudaEventElapsedTime(&ms, ev[2 * (top - i)], ev[1 + 2 * (top - i)]));
+                s.ms_pack[i] += ms;
+                RC_CUDA(ctx, cudaEventElapsedTime(&ms, ev[1 + 2 * (top - i)], ev[2 + 2 * (top - i)]));
+                s.ms_march[i] += ms;
+            }
+            RC_CUDA(ctx, cudaEventElapsedTime(&ms, ev[0], ev[per - 1]));
+            s.ms_total += ms;
+        }
+        for (int i = 0; i <= top; i++) { s.ms_pack[i] /= s.solves_timed; s.ms_march[i] /= s.solves_timed; }
+        s.ms_total /= s.solves_timed;
     }
     *out = s;
     return RC_OK;

@@ -63,6 +63,7 @@ cudaError_t launch_pack(const PackParams &p, int LV, cudaStream_t st);
 cudaError_t launch_march(const MarchParams &p, int LV, cudaStream_t st);
 cudaError_t launch_table_build(const TableBuildParams &p, cudaStream_t st);
 cudaError_t launch_reduce_jbar(const float *Jpart, float *Jbar, long long ncell, int nb, cudaStream_t st);
+cudaError_t launch_count(const MarchParams &p, unsigned long long *total, cudaStream_t st);
 cudaError_t launch_validate(const float *chi, const float *eta, long long n, int *flag, cudaStream_t st);
 
 }  // namespace rc

@@ -371,4 +371,52 @@ cudaError_t launch_validate(const float *chi, const float *eta, long long n, int
     return cudaGetLastError();
 }
 
+// ------------------------------------------------------------------------------------------------
+// Geometric work count: the number of (probe, direction) cell segments of one cascade that lie inside
+// the box, per wavelength — the unit of BASELINE.json's metric.  Walks the same tables with the same
+// in-box test as march_kernel, loads nothing, never exits early.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) count_kernel(MarchParams p, unsigned long long *total) {
+    const int lane = threadIdx.x & 31;
+    const long long nprobe = (long long)p.npx * p.npy;
+    const long long npc = (nprobe + 31) >> 5;
+    const long long nwarps = npc * p.ngroups;
+    const long long W = (long long)blockIdx.x * WARPS_PER_BLOCK + (threadIdx.x >> 5);
+    if (W >= nwarps || p.cnt == nullptr) return;
+    const long long pc = W / p.ngroups;
+    const int kg = (int)(W - pc * p.ngroups);
+    const long long probe = pc * 32 + lane;
+    const bool valid = probe < nprobe;
+    const int b = valid ? (int)(probe / p.npx) : 0;
+    const int a = valid ? (int)(probe - (long long)b * p.npx) : 0;
+    const int s = 1 << p.shift, half = s >> 1;
+    const int Y0 = (b << p.shift) + half;
+    unsigned long long mine = 0;
+    for (int j = 0; j < 4; j++) {
+        const long long k = 4LL * kg + j;
+        const Step *tab = p.steps + __ldg(p.off + k);
+        const int n = __ldg(p.cnt + k);
+        for (int st = 0; st < n; st++) {
+            const uint2 e = __ldg(reinterpret_cast<const uint2 *>(tab) + st);
+            const int dx = (int)(short)(e.x & 0xffffu), dy = (int)(short)(e.x >> 16);
+            const int ax = a + ((dx + half) >> p.shift);
+            const int Y = Y0 + dy;
+            const bool in = valid && (unsigned)ax < (unsigned)p.npx && (unsigned)Y < (unsigned)p.ny;
+            if (!__any_sync(FULL, in)) break;
+            mine += in ? 1ull : 0ull;
+        }
+    }
+    for (int o = 16; o > 0; o >>= 1) mine += __shfl_down_sync(FULL, mine, o);
+    if (lane == 0 && mine) atomicAdd(total, mine);
+}
+
+cudaError_t launch_count(const MarchParams &p, unsigned long long *total, cudaStream_t st) {
+    const long long nprobe = (long long)p.npx * p.npy;
+    const long long nwarps = ((nprobe + 31) >> 5) * p.ngroups;
+    const long long blocks = (nwarps + WARPS_PER_BLOCK - 1) / WARPS_PER_BLOCK;
+    if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+    count_kernel<<<(unsigned)blocks, WARPS_PER_BLOCK * 32, 0, st>>>(p, total);
+    return cudaGetLastError();
+}
+
 }  // namespace rc

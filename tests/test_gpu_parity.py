@@ -171,3 +171,18 @@ def test_error_codes():
         rc.set_atmosphere(bad, bad.abs())
     assert e.value.code == -5
     rc.close()
+
+
+def test_segment_counts_match_the_oracle(oracle):
+    """The metric's unit: geometric (probe, direction) cell segments per cascade, counted on the device
+    from the step tables, equal the oracle's own DDA counts (slivers at fp64 near-ties aside)."""
+    import torch
+    from paper_2408_14425_b200 import binding
+    for atm in (A.make_config(0), A.make_config(4, nx=256, ny=64, nlambda=1, ncascades=6)):
+        J, rc = binding.solve_atmosphere(atm)
+        seg = rc.count_segments()
+        rc.close()
+        ref = oracle.solve_atmosphere(atm, want_counts=True)["segments"]
+        assert len(seg) == atm.ncascades
+        for g, o in zip(seg, ref):
+            assert abs(g - int(o)) <= max(2, 1e-5 * int(o)), (seg, list(ref))
