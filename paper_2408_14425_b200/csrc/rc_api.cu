@@ -20,7 +20,7 @@ struct CascadePlan {
     long long ndir = 0;         // 4^(i+1)
     bool empty = true;          // interval starts beyond the box diagonal: no ray of it is inside
     long long slots = 0;        // step-table capacity, all directions
-    size_t off_off = 0, cnt_off = 0, steps_off = 0;  // byte offsets into the workspace
+    size_t off_off = 0, cnt_off = 0, steps_off = 0, xy_off = 0;  // byte offsets into the workspace
     double ta = 0, tb = 0;
 };
 
@@ -137,7 +137,9 @@ bool make_plan(const rc_config &cfg, int nx, int ny, int L, bool host_io, Plan &
         c.slots = acc;
         c.off_off = cur;   cur = align_up(cur + sizeof(long long) * ((size_t)c.ndir + 1));
         c.cnt_off = cur;   cur = align_up(cur + sizeof(int) * (size_t)c.ndir);
-        c.steps_off = cur; cur = align_up(cur + sizeof(rc::Step) * (size_t)acc);
+        // + 4 entries: the march loop reads the table up to 2 entries ahead of the one it uses
+        c.steps_off = cur; cur = align_up(cur + sizeof(rc::Step) * ((size_t)acc + 4));
+        c.xy_off = cur;    cur = align_up(cur + sizeof(rc::StepXY) * ((size_t)acc + 4));
     }
     const size_t field = align_up(ncell * P.Lpad * sizeof(float));
     P.chiT = cur; cur += field;
@@ -272,6 +274,7 @@ int rc_set_atmosphere(rc_ctx *ctx, const float *chi, const float *eta, int nx, i
                                              sizeof(long long) * ((size_t)c.ndir + 1), cudaMemcpyHostToDevice, ctx->stream));
                 rc::TableBuildParams tp;
                 tp.steps = (rc::Step *)(ctx->ws + c.steps_off);
+                tp.xy = (rc::StepXY *)(ctx->ws + c.xy_off);
                 tp.off = (const long long *)(ctx->ws + c.off_off);
                 tp.cnt = (int *)(ctx->ws + c.cnt_off);
                 tp.cascade = i; tp.top = i == top; tp.ndir = c.ndir;
@@ -340,6 +343,7 @@ static rc::MarchParams march_params(const rc_ctx *ctx, int i, float *J_out) {
     mp.Aup = i == top ? nullptr : (const float *)(ctx->ws + P.A[(i + 1) & 1]);
     mp.out = i > 0 ? (float *)(ctx->ws + P.A[i & 1]) : (accum ? (float *)(ctx->ws + P.Jpart) : J_out);
     mp.steps = c.empty ? nullptr : (const rc::Step *)(ctx->ws + c.steps_off);
+    mp.xy = c.empty ? nullptr : (const rc::StepXY *)(ctx->ws + c.xy_off);
     mp.off = c.empty ? nullptr : (const long long *)(ctx->ws + c.off_off);
     mp.cnt = c.empty ? nullptr : (const int *)(ctx->ws + c.cnt_off);
     mp.I_below = (const float *)(ctx->ws + P.bc_below);

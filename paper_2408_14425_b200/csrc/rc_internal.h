@@ -6,11 +6,18 @@
 
 namespace rc {
 
-// One step of a ray through the grid: the cell it is in, relative to the probe's lattice vertex
-// (cascade i >= 1) or cell (cascade 0), and the path length inside that cell.  8 bytes.
+// One step of a ray through the grid, shared by every probe of the cascade (they are integer
+// translates of one another).  `delta` is the offset, in cells of the cascade's packed layout
+// [y][x mod s][x div s], from the cell that holds the probe's vertex (cascade 0: the probe's cell)
+// to the cell the ray is in; `ds` the path length inside it.  8 bytes, read warp-uniformly.
 struct Step {
-    int16_t dx, dy;
+    int32_t delta;
     float ds;
+};
+
+// The same step as (dx, dy) cell offsets: only used to find, per probe, how many steps lie in the box.
+struct StepXY {
+    int16_t dx, dy;
 };
 
 // Per-cascade geometry tables (device memory, inside the workspace).
@@ -28,6 +35,7 @@ struct MarchParams {
     const float *Aup;   // merged cascade i+1, pre-averaged over the 4 children: [nb][N_i][npy/2][npx/2][LV]; null on the top cascade
     float *out;         // mode 0: A_i [nb][N_i/4][npy][npx][LV]; mode 1: J [ny][nx][L]; mode 2: Jpart [nb][ny][nx]
     const Step *steps;
+    const StepXY *xy;
     const long long *off;
     const int *cnt;
     const float *I_below;  // [Lpad] device
@@ -50,6 +58,7 @@ struct PackParams {
 
 struct TableBuildParams {
     Step *steps;
+    StepXY *xy;
     const long long *off;
     int *cnt;
     int cascade, top;

@@ -17,6 +17,7 @@
 #include "rc_internal.h"
 
 #include <math_constants.h>
+#include <cstdlib>
 
 namespace rc {
 
@@ -30,7 +31,17 @@ __global__ void table_build_kernel(TableBuildParams p) {
     long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= p.ndir) return;
     Step *out = p.steps + p.off[k];
+    StepXY *oxy = p.xy + p.off[k];
     const long long cap = p.off[k + 1] - p.off[k];
+    const int shift = p.cascade, s = 1 << shift, half = s >> 1, npx = p.nx >> shift;
+    // cell (vertex + (dx, dy)) in the packed layout [y][x mod s][x div s], relative to the vertex's cell
+    auto emit = [&](int n, int dx, int dy, double ds) {
+        const int tx = dx + half;
+        out[n].delta = dy * p.nx + (tx & (s - 1)) * npx + (tx >> shift) - half * npx;
+        out[n].ds = (float)ds;
+        oxy[n].dx = (int16_t)dx;
+        oxy[n].dy = (int16_t)dy;
+    };
     int n = 0;
     if (p.cascade == 0) {
         // The 4 diagonals from a cell centre pass exactly through cell corners: closed form.
@@ -43,12 +54,7 @@ __global__ void table_build_kernel(TableBuildParams p) {
             if (lo >= p.tb) break;
             lo = fmax(lo, p.ta);
             hi = fmin(hi, p.tb);
-            if (hi > lo) {
-                out[n].dx = (int16_t)(m * sx);
-                out[n].dy = (int16_t)(m * sy);
-                out[n].ds = (float)(hi - lo);
-                n++;
-            }
+            if (hi > lo) emit(n++, m * sx, m * sy, hi - lo);
         }
         p.cnt[k] = n;
         return;
@@ -70,12 +76,7 @@ __global__ void table_build_kernel(TableBuildParams p) {
     while (n < cap) {
         const double tn = fmin(fmin(tmx, tmy), tb);
         const double ds = tn - t;
-        if (ds > 0.0) {
-            out[n].dx = (int16_t)ix;
-            out[n].dy = (int16_t)iy;
-            out[n].ds = (float)ds;
-            n++;
-        }
+        if (ds > 0.0) emit(n++, ix, iy, ds);
         if (tn >= tb) break;
         const bool stepx = tmx <= tmy, stepy = tmy <= tmx;
         if (stepx) { ix += sx; gx += sx; tmx = (double)gx / wx; }
@@ -159,10 +160,10 @@ __device__ __forceinline__ float ex2_neg(float tau2) {  // 2^-tau2, flushes to 0
 template <int LV>
 __device__ __forceinline__ void load_vec(const float *p, float (&v)[LV]) {
     if constexpr (LV == 8) {
-        const float4 a = __ldg(reinterpret_cast<const float4 *>(p));
-        const float4 b = __ldg(reinterpret_cast<const float4 *>(p) + 1);
-        v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w;
-        v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
+        // one 256-bit load (sm_100: LDG.E.256): 32 lanes x 32 B = 8 full 128-byte lines per request
+        asm("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+            : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]), "=f"(v[4]), "=f"(v[5]), "=f"(v[6]), "=f"(v[7])
+            : "l"(p));
     } else if constexpr (LV == 4) {
         const float4 a = __ldg(reinterpret_cast<const float4 *>(p));
         v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w;
@@ -197,32 +198,83 @@ __device__ __forceinline__ void parent_axis(int a, int n, int &q0, int &q1, floa
     q1 = min(max(base + 1, 0), n - 1);
 }
 
-template <int LV>
-__global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) march_kernel(MarchParams p) {
+// Warp -> work mapping shared by march_kernel and count_kernel.  A block holds G = min(ngroups, 8)
+// ADJACENT direction groups of the same 32-probe chunk (their rays overlap near the probes: L1 reuse)
+// and, when a cascade has fewer than 8 groups, 8/G neighbouring chunks.  Across blocks the probe
+// chunk varies fastest, then the direction, then the wavelength batch: the blocks resident at any
+// time share a narrow fan of directions (a few MB of step tables) and one batch's planes (L2).
+struct WarpWork {
+    int nbI, kg;
+    long long pc;
+    bool any;
+};
+
+__device__ __forceinline__ WarpWork warp_work(const MarchParams &p, long long npc) {
+    const int w = threadIdx.x >> 5;
+    const int G = min(p.ngroups, WARPS_PER_BLOCK), Pb = WARPS_PER_BLOCK / G;
+    const long long pcb_n = (npc + Pb - 1) / Pb;
+    const int kgb_n = p.ngroups / G;
+    long long bid = blockIdx.x;
+    const long long pcb = bid % pcb_n;
+    bid /= pcb_n;
+    const int kgb = (int)(bid % kgb_n);
+    WarpWork r;
+    r.nbI = (int)(bid / kgb_n);
+    r.kg = kgb * G + (w % G);
+    r.pc = pcb * Pb + (w / G);
+    r.any = r.pc < npc && r.nbI < p.nb;
+    return r;
+}
+
+__host__ __device__ inline long long march_blocks(int ngroups, long long npc, int nb) {
+    const int G = ngroups < WARPS_PER_BLOCK ? ngroups : WARPS_PER_BLOCK, Pb = WARPS_PER_BLOCK / G;
+    return ((npc + Pb - 1) / Pb) * (ngroups / G) * nb;
+}
+
+// Number of leading steps of direction k's table that lie inside the box for this lane's probe.
+// The box is convex and the probe is inside it, so the in-box steps are a prefix; dx and dy are
+// monotone along the ray, so the first step outside is found by bisection on the (dx, dy) table.
+__device__ __forceinline__ int steps_inside(const StepXY *xy, int n, bool valid, int dxlo, int dxhi, int dylo, int dyhi) {
+    int lo = 0, hi = valid ? n : 0;  // smallest st in [0, n] that is outside (n: none is)
+    const int iters = 32 - __clz(n);  // ceil(log2(n + 1)); warp-uniform
+    for (int it = 0; it < iters; it++) {
+        const int mid = (lo + hi) >> 1;
+        if (lo < hi) {
+            const unsigned e = __ldg(reinterpret_cast<const unsigned *>(xy) + mid);
+            const int dx = (int)(short)(e & 0xffffu), dy = (int)(short)(e >> 16);
+            const bool out = dx < dxlo || dx > dxhi || dy < dylo || dy > dyhi;
+            if (out) hi = mid; else lo = mid + 1;
+        }
+    }
+    return lo;
+}
+
+// One warp = 32 adjacent probes x 1 direction group (its 4 child directions in turn) x LV wavelengths
+// per lane.  Per step the warp reads one 8-byte table entry (uniform address) and each lane its
+// cell's LV opacities and source functions; the loads of step st+1 are in flight while step st is
+// integrated, and the table is read two steps ahead.
+template <int LV, int MINB>
+__global__ void __launch_bounds__(WARPS_PER_BLOCK * 32, MINB) march_kernel(MarchParams p) {
     const int lane = threadIdx.x & 31;
     const long long nprobe = (long long)p.npx * p.npy;
-    const long long npc = (nprobe + 31) >> 5;  // probe chunks of 32
-    const long long nwarps = npc * p.ngroups * p.nb;
-    const long long W = (long long)blockIdx.x * WARPS_PER_BLOCK + (threadIdx.x >> 5);
-    if (W >= nwarps) return;
-    // warp -> (wavelength batch, probe chunk, direction group); the batch is slowest so that the
-    // blocks resident at any time work on one batch's planes (L2 residency)
-    const int nbI = (int)(W / (npc * p.ngroups));
-    const long long r = W - (long long)nbI * npc * p.ngroups;
-    long long pc;
-    int kg;
-    if (p.group_major) { kg = (int)(r / npc); pc = r - (long long)kg * npc; }
-    else               { pc = r / p.ngroups;  kg = (int)(r - pc * p.ngroups); }
-    const long long probe = pc * 32 + lane;
+    const long long npc = (nprobe + 31) >> 5;
+    const WarpWork ww = warp_work(p, npc);
+    if (!ww.any) return;
+    const int nbI = ww.nbI, kg = ww.kg;
+    const long long probe = ww.pc * 32 + lane;
     const bool valid = probe < nprobe;
     const int b = valid ? (int)(probe / p.npx) : 0;
     const int a = valid ? (int)(probe - (long long)b * p.npx) : 0;
     const int s = 1 << p.shift, half = s >> 1;
     const int Y0 = (b << p.shift) + half;
     const long long ncell = (long long)p.nx * p.ny;
-    const float *chiT = p.chiT + (long long)nbI * ncell * LV;
-    const float *ST = p.ST + (long long)nbI * ncell * LV;
+    const long long base = (long long)Y0 * p.nx + (long long)half * p.npx + a;  // the vertex's cell, packed layout
+    const float *chi0 = p.chiT + ((long long)nbI * ncell + base) * LV;
+    const float *S0 = p.ST + ((long long)nbI * ncell + base) * LV;
     const long long ndir = 4LL * p.ngroups;
+    // (dx, dy) ranges that keep this lane's ray inside the box
+    const int dxlo = -(a << p.shift) - half, dxhi = ((p.npx - a) << p.shift) - 1 - half;
+    const int dylo = -Y0, dyhi = p.ny - 1 - Y0;
 
     float acc[LV];
 #pragma unroll
@@ -230,45 +282,53 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) march_kernel(MarchParams
 
     for (int j = 0; j < 4; j++) {
         const long long k = 4LL * kg + j;
-        // cnt == null: the whole cascade lies outside any box of this size (pure boundary term)
-        const Step *tab = p.cnt ? p.steps + __ldg(p.off + k) : nullptr;
-        const int n = p.cnt ? __ldg(p.cnt + k) : 0;
         float I[LV], tau[LV], T[LV];
 #pragma unroll
         for (int v = 0; v < LV; v++) { I[v] = 0.f; tau[v] = 0.f; T[v] = 1.f; }
-        // a1: eq. 16 along the interval, front to back: with tau accumulated,
-        // T_n = 2^-tau2_n and the cell's contribution is S (T_{n-1} - T_n)  [= S T (1 - e^{-chi ds})]
-        for (int st = 0; st < n; st++) {
-            const uint2 e = __ldg(reinterpret_cast<const uint2 *>(tab) + st);  // warp-uniform
-            const int dx = (int)(short)(e.x & 0xffffu), dy = (int)(short)(e.x >> 16);
-            const float ds = __uint_as_float(e.y);
-            const int tx = dx + half;
-            const int ax = a + (tx >> p.shift), xm = tx & (s - 1);
-            const int Y = Y0 + dy;
-            const bool in = valid && (unsigned)ax < (unsigned)p.npx && (unsigned)Y < (unsigned)p.ny;
-            if (!__any_sync(FULL, in)) break;  // the box is convex: a ray that left never returns
-            float c2[LV], S[LV];
-            if (in) {
-                const long long cell = (long long)Y * p.nx + xm * p.npx + ax;
-                load_vec<LV>(chiT + cell * LV, c2);
-                load_vec<LV>(ST + cell * LV, S);
-            } else {
-#pragma unroll
-                for (int v = 0; v < LV; v++) { c2[v] = 0.f; S[v] = 0.f; }
+        // cnt == null: the whole cascade lies outside any box of this size (pure boundary term)
+        if (p.cnt != nullptr) {
+            const long long o = __ldg(p.off + k);
+            const int n = __ldg(p.cnt + k);
+            const uint2 *tab = reinterpret_cast<const uint2 *>(p.steps + o);
+            const int nin = steps_inside(p.xy + o, n, valid, dxlo, dxhi, dylo, dyhi);
+            const int nw = __reduce_max_sync(FULL, nin);  // steps this warp walks
+            // a lane past its last in-box step re-reads its own vertex cell over ds = 0: no branch, no effect
+            float c2[LV], S[LV], c2n[LV], Sn[LV];
+            uint2 e0 = __ldg(tab), e1 = __ldg(tab + 1);  // slots have 4 spare entries at the end
+            {
+                const bool in = 0 < nin;
+                const long long d = in ? (long long)(int)e0.x : 0;
+                load_vec<LV>(chi0 + d * LV, c2);
+                load_vec<LV>(S0 + d * LV, S);
             }
+            float ds = 0 < nin ? __uint_as_float(e0.y) : 0.f;
+            // a1: eq. 16 along the interval, front to back: with tau accumulated,
+            // T_n = 2^-tau2_n and the cell's contribution is S (T_{n-1} - T_n)  [= S T (1 - e^{-chi ds})]
+#pragma unroll 2
+            for (int st = 0; st < nw; st++) {
+                const bool inn = st + 1 < nin;
+                const long long d = inn ? (long long)(int)e1.x : 0;
+                load_vec<LV>(chi0 + d * LV, c2n);
+                load_vec<LV>(S0 + d * LV, Sn);
+                const float dsn = inn ? __uint_as_float(e1.y) : 0.f;
+                e1 = __ldg(tab + st + 2);
 #pragma unroll
-            for (int v = 0; v < LV; v++) {
-                tau[v] = fmaf(c2[v], ds, tau[v]);
-                const float Tn = ex2_neg(tau[v]);
-                I[v] = fmaf(S[v], T[v] - Tn, I[v]);
-                T[v] = Tn;
-            }
-            if (p.early_exit && (st & 7) == 7) {
-                float tmin = tau[0];
+                for (int v = 0; v < LV; v++) {
+                    tau[v] = fmaf(c2[v], ds, tau[v]);
+                    const float Tn = ex2_neg(tau[v]);
+                    I[v] = fmaf(S[v], T[v] - Tn, I[v]);
+                    T[v] = Tn;
+                }
+                if (p.early_exit && (st & 7) == 7) {
+                    float tmin = tau[0];
 #pragma unroll
-                for (int v = 1; v < LV; v++) tmin = fminf(tmin, tau[v]);
-                // every live lane opaque at every wavelength: T is exactly 0, nothing more can arrive
-                if (__all_sync(FULL, !in || tmin > 126.f)) break;
+                    for (int v = 1; v < LV; v++) tmin = fminf(tmin, tau[v]);
+                    // every live lane opaque at every wavelength: T is exactly 0, nothing more can arrive
+                    if (__all_sync(FULL, st >= nin || tmin > 126.f)) break;
+                }
+#pragma unroll
+                for (int v = 0; v < LV; v++) { c2[v] = c2n[v]; S[v] = Sn[v]; }
+                ds = dsn;
             }
         }
         if (p.Aup == nullptr) {
@@ -325,15 +385,18 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) march_kernel(MarchParams
 
 cudaError_t launch_march(const MarchParams &p, int LV, cudaStream_t st) {
     const long long nprobe = (long long)p.npx * p.npy;
-    const long long nwarps = ((nprobe + 31) >> 5) * p.ngroups * p.nb;
-    const long long blocks = (nwarps + WARPS_PER_BLOCK - 1) / WARPS_PER_BLOCK;
+    const long long blocks = march_blocks(p.ngroups, (nprobe + 31) >> 5, p.nb);
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     const dim3 grid((unsigned)blocks), block(WARPS_PER_BLOCK * 32);
+    // TEMPORARY tuning hook (removed once the variants are settled): RC_TUNE_MINB
+    static int mb = getenv("RC_TUNE_MINB") ? atoi(getenv("RC_TUNE_MINB")) : 2;
+#define RC_LAUNCH(LV_, MB_) march_kernel<LV_, MB_><<<grid, block, 0, st>>>(p)
+#define RC_PICK(LV_) do { if (mb >= 4) RC_LAUNCH(LV_, 4); else if (mb == 3) RC_LAUNCH(LV_, 3); else RC_LAUNCH(LV_, 2); } while (0)
     switch (LV) {
-        case 8: march_kernel<8><<<grid, block, 0, st>>>(p); break;
-        case 4: march_kernel<4><<<grid, block, 0, st>>>(p); break;
-        case 2: march_kernel<2><<<grid, block, 0, st>>>(p); break;
-        default: march_kernel<1><<<grid, block, 0, st>>>(p); break;
+        case 8: RC_PICK(8); break;
+        case 4: RC_PICK(4); break;
+        case 2: RC_LAUNCH(2, 4); break;
+        default: RC_LAUNCH(1, 4); break;
     }
     return cudaGetLastError();
 }
@@ -373,8 +436,8 @@ cudaError_t launch_validate(const float *chi, const float *eta, long long n, int
 
 // ------------------------------------------------------------------------------------------------
 // Geometric work count: the number of (probe, direction) cell segments of one cascade that lie inside
-// the box, per wavelength — the unit of BASELINE.json's metric.  Walks the same tables with the same
-// in-box test as march_kernel, loads nothing, never exits early.
+// the box, per wavelength — the unit of BASELINE.json's metric: the sum over probes and directions of
+// the in-box step counts march_kernel itself uses.
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) count_kernel(MarchParams p, unsigned long long *total) {
     const int lane = threadIdx.x & 31;
@@ -391,20 +454,13 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) count_kernel(MarchParams
     const int a = valid ? (int)(probe - (long long)b * p.npx) : 0;
     const int s = 1 << p.shift, half = s >> 1;
     const int Y0 = (b << p.shift) + half;
+    const int dxlo = -(a << p.shift) - half, dxhi = ((p.npx - a) << p.shift) - 1 - half;
+    const int dylo = -Y0, dyhi = p.ny - 1 - Y0;
     unsigned long long mine = 0;
     for (int j = 0; j < 4; j++) {
         const long long k = 4LL * kg + j;
-        const Step *tab = p.steps + __ldg(p.off + k);
-        const int n = __ldg(p.cnt + k);
-        for (int st = 0; st < n; st++) {
-            const uint2 e = __ldg(reinterpret_cast<const uint2 *>(tab) + st);
-            const int dx = (int)(short)(e.x & 0xffffu), dy = (int)(short)(e.x >> 16);
-            const int ax = a + ((dx + half) >> p.shift);
-            const int Y = Y0 + dy;
-            const bool in = valid && (unsigned)ax < (unsigned)p.npx && (unsigned)Y < (unsigned)p.ny;
-            if (!__any_sync(FULL, in)) break;
-            mine += in ? 1ull : 0ull;
-        }
+        const long long o = __ldg(p.off + k);
+        mine += (unsigned long long)steps_inside(p.xy + o, __ldg(p.cnt + k), valid, dxlo, dxhi, dylo, dyhi);
     }
     for (int o = 16; o > 0; o >>= 1) mine += __shfl_down_sync(FULL, mine, o);
     if (lane == 0 && mine) atomicAdd(total, mine);
