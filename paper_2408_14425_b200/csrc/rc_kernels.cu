@@ -17,7 +17,6 @@
 #include "rc_internal.h"
 
 #include <math_constants.h>
-#include <cstdlib>
 
 namespace rc {
 
@@ -388,15 +387,12 @@ cudaError_t launch_march(const MarchParams &p, int LV, cudaStream_t st) {
     const long long blocks = march_blocks(p.ngroups, (nprobe + 31) >> 5, p.nb);
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     const dim3 grid((unsigned)blocks), block(WARPS_PER_BLOCK * 32);
-    // TEMPORARY tuning hook (removed once the variants are settled): RC_TUNE_MINB
-    static int mb = getenv("RC_TUNE_MINB") ? atoi(getenv("RC_TUNE_MINB")) : 2;
-#define RC_LAUNCH(LV_, MB_) march_kernel<LV_, MB_><<<grid, block, 0, st>>>(p)
-#define RC_PICK(LV_) do { if (mb >= 4) RC_LAUNCH(LV_, 4); else if (mb == 3) RC_LAUNCH(LV_, 3); else RC_LAUNCH(LV_, 2); } while (0)
+    // minimum resident blocks per SM (register cap) measured best on cfg 2: LV=8 -> 3 (80 regs), LV=4 -> 4 (64 regs)
     switch (LV) {
-        case 8: RC_PICK(8); break;
-        case 4: RC_PICK(4); break;
-        case 2: RC_LAUNCH(2, 4); break;
-        default: RC_LAUNCH(1, 4); break;
+        case 8: march_kernel<8, 3><<<grid, block, 0, st>>>(p); break;
+        case 4: march_kernel<4, 4><<<grid, block, 0, st>>>(p); break;
+        case 2: march_kernel<2, 4><<<grid, block, 0, st>>>(p); break;
+        default: march_kernel<1, 4><<<grid, block, 0, st>>>(p); break;
     }
     return cudaGetLastError();
 }
