@@ -1,0 +1,59 @@
+"""The N > 1 path on CPU: wavelength blocks over a world-size-2 gloo group.
+Each rank solves its block (with the oracle here — there is no GPU; on a GPU box bench.py does the
+same with the CUDA library), J is all-gathered, Jbar all-reduced, and both equal the one-rank solve."""
+import os
+import socket
+
+import numpy as np
+import pytest
+
+from paper_2408_14425_b200 import atmospheres as A
+from paper_2408_14425_b200 import sharding
+
+
+def test_wavelength_blocks_partition():
+    for L in (1, 2, 5, 16, 64, 709):
+        for world in (1, 2, 3, 4, 8):
+            blocks = [sharding.wavelength_block(L, r, world) for r in range(world)]
+            assert blocks[0][0] == 0 and blocks[-1][1] == L
+            assert all(blocks[i][1] == blocks[i + 1][0] for i in range(world - 1))
+            sizes = [b - a for a, b in blocks]
+            assert max(sizes) - min(sizes) <= 1
+
+
+def _worker(rank, world, port, q):
+    import torch
+    import torch.distributed as dist
+    from oracle import rc_oracle
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    atm = A.make_config(4, nx=64, ny=16, nlambda=5, ncascades=3)
+    mine = sharding.shard_atmosphere(atm, rank, world)
+    out = rc_oracle.solve_atmosphere(mine, nthreads=2)
+    J = sharding.allgather_j(torch.from_numpy(out["J"]), atm.nlambda)
+    Jbar = sharding.allreduce_jbar(torch.from_numpy(out["Jbar"].copy()))
+    if rank == 0:
+        q.put((J.numpy(), Jbar.numpy()))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_two_rank_gloo_matches_single_rank(oracle):
+    import torch.multiprocessing as mp
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    J, Jbar = q.get(timeout=300)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    atm = A.make_config(4, nx=64, ny=16, nlambda=5, ncascades=3)
+    ref = oracle.solve_atmosphere(atm)
+    assert np.array_equal(J, ref["J"])
+    assert np.allclose(Jbar, ref["Jbar"], rtol=1e-14, atol=0)
