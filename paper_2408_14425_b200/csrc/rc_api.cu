@@ -4,6 +4,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -17,6 +18,7 @@ constexpr size_t ALIGN = 256;
 inline size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 
 struct CascadePlan {
+    int pw_log2 = 5;            // lane patch of the march: 2^pw_log2 probes wide, 32 >> pw_log2 high
     long long ndir = 0;         // 4^(i+1)
     bool empty = true;          // interval starts beyond the box diagonal: no ray of it is inside
     long long slots = 0;        // step-table capacity, all directions
@@ -45,6 +47,9 @@ struct rc_ctx {
     bool have_atm = false;
     int tab_nx = 0, tab_ny = 0;  // shape the step tables in the workspace were built for
     bool host_io = false;
+    // developer overrides (environment, read by rc_create): RC_MARCH_VARIANT = 0..3 (register ring depth /
+    // occupancy of march_kernel), RC_PATCH_LOG2 = 2..5 forces the lane patch width for cascades >= RC_PATCH_FROM
+    int tune_variant = 2, tune_patch = -1, tune_patch_from = 0;
     std::vector<std::vector<long long>> off_host;  // kept alive for the async uploads
     std::vector<float> stage;                      // host staging for boundary / weights
     // timing: `nsets` rings of (2 per cascade + 2) events; solve number n records into set n % nsets
@@ -84,6 +89,51 @@ bool shape_ok(const rc_config &cfg, int nx, int ny, int L) {
     return nx % m == 0 && ny % m == 0;
 }
 
+// Shape of the 32-probe patch one warp marches in lock step.  All lanes walk until the patch's last
+// ray has left the box, so the patch should hold probes whose rays have similar in-box lengths:
+// estimated here from the geometry alone (ray length to the box edge, clipped to the interval) for
+// the candidate shapes 32x1 .. 4x8, over a sample of directions.  Wider patches gather longer
+// contiguous runs, so the widest shape within 2 % of the best utilisation wins.
+int choose_patch(int nx, int ny, int i, double ta, double tb) {
+    const int s = 1 << i, npx = nx >> i, npy = ny >> i;
+    int widest = 5;
+    while (widest > 0 && (1 << widest) > npx) widest--;
+    if (std::fmin(tb, std::hypot((double)nx, (double)ny)) <= std::min(nx, ny) / 16.0) return widest;
+    const long long ndir = 1LL << (2 * (i + 1));
+    const int nsample = (int)std::min<long long>(ndir, 128);
+    std::vector<double> len((size_t)npx * npy);
+    double total = 0.0, cost[6] = {0, 0, 0, 0, 0, 0};
+    const int narrowest = std::min(widest, 2);
+    for (int n = 0; n < nsample; n++) {
+        const long long k = (2 * n + 1) * ndir / (2 * nsample);
+        const double th = 2.0 * M_PI * ((double)k + 0.5) / (double)ndir, cx = std::cos(th), sy = std::sin(th);
+        for (int b = 0; b < npy; b++)
+            for (int a = 0; a < npx; a++) {
+                const double X = (a + 0.5) * s, Y = (b + 0.5) * s;
+                const double te = std::fmin(cx > 0 ? (nx - X) / cx : -X / cx, sy > 0 ? (ny - Y) / sy : -Y / sy);
+                const double l = std::fmax(std::fmin(te, tb) - ta, 0.0) * (std::fabs(cx) + std::fabs(sy));
+                len[(size_t)b * npx + a] = l;
+                total += l;
+            }
+        for (int c = narrowest; c <= widest; c++) {
+            const int pw = 1 << c, ph = 32 >> c;
+            for (int b0 = 0; b0 < npy; b0 += ph)
+                for (int a0 = 0; a0 < npx; a0 += pw) {
+                    double m = 0.0;
+                    for (int b = b0; b < std::min(b0 + ph, npy); b++)
+                        for (int a = a0; a < std::min(a0 + pw, npx); a++) m = std::fmax(m, len[(size_t)b * npx + a]);
+                    cost[c] += 32.0 * m;
+                }
+        }
+    }
+    if (!(total > 0.0)) return widest;
+    double best = 0.0;
+    for (int c = narrowest; c <= widest; c++) best = std::fmax(best, total / cost[c]);
+    for (int c = widest; c >= narrowest; c--)
+        if (total / cost[c] >= best - 0.02) return c;
+    return widest;
+}
+
 int choose_lv(const rc_config &cfg, int L) {
     if (cfg.lambda_batch == 1 || cfg.lambda_batch == 2 || cfg.lambda_batch == 4 || cfg.lambda_batch == 8)
         return cfg.lambda_batch;
@@ -113,7 +163,10 @@ bool make_plan(const rc_config &cfg, int nx, int ny, int L, bool host_io, Plan &
         c.tb = i == top ? INFINITY : t_of(i + 1, cfg.c0_interval);
         c.empty = !(c.ta < diag);
         c.slots = 0;
+        c.pw_log2 = 5;
+        while (c.pw_log2 > 0 && (1 << c.pw_log2) > (nx >> i)) c.pw_log2--;
         if (c.empty) continue;
+        if (offs) c.pw_log2 = choose_patch(nx, ny, i, c.ta, c.tb);
         std::vector<long long> local;
         std::vector<long long> &o = offs ? (*offs)[i] : local;
         o.resize((size_t)c.ndir + 1);
@@ -137,9 +190,9 @@ bool make_plan(const rc_config &cfg, int nx, int ny, int L, bool host_io, Plan &
         c.slots = acc;
         c.off_off = cur;   cur = align_up(cur + sizeof(long long) * ((size_t)c.ndir + 1));
         c.cnt_off = cur;   cur = align_up(cur + sizeof(int) * (size_t)c.ndir);
-        // + 4 entries: the march loop reads the table up to 2 entries ahead of the one it uses
-        c.steps_off = cur; cur = align_up(cur + sizeof(rc::Step) * ((size_t)acc + 4));
-        c.xy_off = cur;    cur = align_up(cur + sizeof(rc::StepXY) * ((size_t)acc + 4));
+        // + 16 entries: the march loop reads the table up to 2 x (ring depth) entries past the last step
+        c.steps_off = cur; cur = align_up(cur + sizeof(rc::Step) * ((size_t)acc + 16));
+        c.xy_off = cur;    cur = align_up(cur + sizeof(rc::StepXY) * ((size_t)acc + 16));
     }
     const size_t field = align_up(ncell * P.Lpad * sizeof(float));
     P.chiT = cur; cur += field;
@@ -192,6 +245,9 @@ int rc_create(rc_ctx **out, const rc_config *cfg) {
     rc_ctx *ctx = new (std::nothrow) rc_ctx();
     if (!ctx) return RC_ERR_CUDA;
     ctx->cfg = *cfg;
+    if (const char *e = std::getenv("RC_MARCH_VARIANT")) ctx->tune_variant = std::max(0, std::min(3, std::atoi(e)));
+    if (const char *e = std::getenv("RC_PATCH_LOG2")) ctx->tune_patch = std::max(2, std::min(5, std::atoi(e)));
+    if (const char *e = std::getenv("RC_PATCH_FROM")) ctx->tune_patch_from = std::atoi(e);
     *out = ctx;
     return RC_OK;
 }
@@ -260,6 +316,7 @@ int rc_set_atmosphere(rc_ctx *ctx, const float *chi, const float *eta, int nx, i
             return fail(ctx, RC_ERR_NO_WORKSPACE, "workspace has %zu bytes, %zu needed", ctx->ws_bytes, P.total);
         make_plan(ctx->cfg, nx, ny, nlambda, true, Pio, nullptr);
         ctx->host_io = Pio.total <= ctx->ws_bytes;
+        for (int i = 0; i < ctx->cfg.ncascades; i++) Pio.c[i].pw_log2 = P.c[i].pw_log2;  // chosen only when offs is built
         ctx->plan = ctx->host_io ? Pio : P;
         ctx->have_atm = false;
         // geometry tables: only when the grid size changed (they do not depend on nlambda)
@@ -355,7 +412,11 @@ static rc::MarchParams march_params(const rc_ctx *ctx, int i, float *J_out) {
     mp.ngroups = 1 << (2 * i);
     mp.mode = i > 0 ? 0 : (accum ? 2 : 1);
     mp.early_exit = (ctx->cfg.flags & RC_NO_EARLY_EXIT) ? 0 : 1;
-    mp.group_major = 0;
+    mp.pw_log2 = ctx->tune_patch >= 0 && i >= ctx->tune_patch_from ? ctx->tune_patch : c.pw_log2;
+    while (mp.pw_log2 > 0 && (1 << mp.pw_log2) > mp.npx) mp.pw_log2--;
+    const int pw = 1 << mp.pw_log2, ph = 32 >> mp.pw_log2;
+    mp.npatch_x = (mp.npx + pw - 1) / pw;
+    mp.npatch_y = (mp.npy + ph - 1) / ph;
     return mp;
 }
 
@@ -384,7 +445,7 @@ int rc_solve_J(rc_ctx *ctx, float *J_out) {
             launches++;
         }
         if (ev) RC_CUDA(ctx, cudaEventRecord(ev[1 + 2 * (top - i)], ctx->stream));
-        RC_CUDA(ctx, rc::launch_march(march_params(ctx, i, J_out), P.LV, ctx->stream));
+        RC_CUDA(ctx, rc::launch_march(march_params(ctx, i, J_out), P.LV, ctx->tune_variant, ctx->stream));
         launches++;
         if (ev) RC_CUDA(ctx, cudaEventRecord(ev[2 + 2 * (top - i)], ctx->stream));
     }

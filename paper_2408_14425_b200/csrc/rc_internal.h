@@ -8,8 +8,8 @@ namespace rc {
 
 // One step of a ray through the grid, shared by every probe of the cascade (they are integer
 // translates of one another).  `delta` is the offset, in cells of the cascade's packed layout
-// [y][x mod s][x div s], from the cell that holds the probe's vertex (cascade 0: the probe's cell)
-// to the cell the ray is in; `ds` the path length inside it.  8 bytes, read warp-uniformly.
+// [y mod s][x mod s][y div s][x div s], from the probe's own entry (b, a) of phase plane 0 to the
+// cell the ray is in; `ds` the path length inside it.  8 bytes, read warp-uniformly.
 struct Step {
     int32_t delta;
     float ds;
@@ -30,7 +30,7 @@ struct CascadeTable {
 };
 
 struct MarchParams {
-    const float *chiT;  // packed opacity * log2(e): [nb][ny][s][npx][LV]  (x split as xm = x mod s, xd = x div s)
+    const float *chiT;  // packed opacity * log2(e): [nb][s][s][npy][npx][LV]  (phase (y mod s, x mod s), then y div s, x div s)
     const float *ST;    // packed source function eta/chi, same layout
     const float *Aup;   // merged cascade i+1, pre-averaged over the 4 children: [nb][N_i][npy/2][npx/2][LV]; null on the top cascade
     float *out;         // mode 0: A_i [nb][N_i/4][npy][npx][LV]; mode 1: J [ny][nx][L]; mode 2: Jpart [nb][ny][nx]
@@ -47,12 +47,13 @@ struct MarchParams {
     int ngroups;           // direction groups = 4^cascade (4 directions each)
     int mode;
     int early_exit;
-    int group_major;       // warp order: 0 = direction group fastest, 1 = probe chunk fastest
+    int pw_log2;           // one warp's 32 probes form a patch 2^pw_log2 wide, 32 >> pw_log2 high
+    int npatch_x, npatch_y;  // patches per axis
 };
 
 struct PackParams {
     const float *chi, *eta;  // [ny][nx][L]
-    float *chiT, *ST;        // [nb][ny][s][npx][LV]
+    float *chiT, *ST;        // [nb][s][s][npy][npx][LV]
     int nx, ny, L, nb, shift;
 };
 
@@ -69,7 +70,7 @@ struct TableBuildParams {
 
 // launchers (rc_kernels.cu); LV in {1,2,4,8}
 cudaError_t launch_pack(const PackParams &p, int LV, cudaStream_t st);
-cudaError_t launch_march(const MarchParams &p, int LV, cudaStream_t st);
+cudaError_t launch_march(const MarchParams &p, int LV, int variant, cudaStream_t st);
 cudaError_t launch_table_build(const TableBuildParams &p, cudaStream_t st);
 cudaError_t launch_reduce_jbar(const float *Jpart, float *Jbar, long long ncell, int nb, cudaStream_t st);
 cudaError_t launch_count(const MarchParams &p, unsigned long long *total, cudaStream_t st);

@@ -6,13 +6,14 @@
 //                       so every probe's ray in direction k is an integer translate of this one: the
 //                       cells it crosses and the lengths inside them are shared.
 //   pack_kernel         chi, eta [y][x][l]  ->  chi*log2(e), S = eta/chi in the probe-strided layout
-//                       [batch][y][x mod s][x div s][LV]: the cells that 32 x-adjacent probes of
-//                       cascade i touch at the same step are contiguous (coalesced gathers).
+//                       [batch][y mod s][x mod s][y div s][x div s][LV]: the cells that a patch of
+//                       neighbouring probes of cascade i touches at the same step form a patch of
+//                       the same shape in one phase plane (rows of contiguous 32-byte sectors).
 //   march_kernel        a1 (eq. 16 along the interval) + a2 (boundary)
 //                       + a3 (bilinear parents, mean of the 4 children, merge eq. 11,
 //                       PAPER.md:149-157, 199-207) + a4 on cascade 0 (J), fused.
-//                       One warp = 32 adjacent probes x 1 direction group (4 child directions in
-//                       turn) x LV wavelengths per lane; geometry is warp-uniform (no divergence from
+//                       One warp = a pw x ph patch of 32 probes x 1 direction group (4 child directions
+//                       in turn) x LV wavelengths per lane; geometry is warp-uniform (no divergence from
 //                       the DDA itself), radiance in fp32, I and T never leave registers.
 #include "rc_internal.h"
 
@@ -33,10 +34,13 @@ __global__ void table_build_kernel(TableBuildParams p) {
     StepXY *oxy = p.xy + p.off[k];
     const long long cap = p.off[k + 1] - p.off[k];
     const int shift = p.cascade, s = 1 << shift, half = s >> 1, npx = p.nx >> shift;
-    // cell (vertex + (dx, dy)) in the packed layout [y][x mod s][x div s], relative to the vertex's cell
+    // cell (vertex cell + (dx, dy)) in the packed layout [y mod s][x mod s][y div s][x div s], relative to
+    // the probe's own entry (y div s, x div s) = (b, a) of phase plane 0
+    const int npy = p.ny >> shift;
     auto emit = [&](int n, int dx, int dy, double ds) {
-        const int tx = dx + half;
-        out[n].delta = dy * p.nx + (tx & (s - 1)) * npx + (tx >> shift) - half * npx;
+        const int tx = dx + half, ty = dy + half;
+        const int phase = ((ty & (s - 1)) << shift) + (tx & (s - 1));
+        out[n].delta = phase * (npx * npy) + (ty >> shift) * npx + (tx >> shift);
         out[n].ds = (float)ds;
         oxy[n].dx = (int16_t)dx;
         oxy[n].dy = (int16_t)dy;
@@ -93,7 +97,75 @@ cudaError_t launch_table_build(const TableBuildParams &p, cudaStream_t st) {
 }
 
 // ------------------------------------------------------------------------------------------------
-// Pack: one thread per (batch, y, xm, xd); moves LV wavelengths of one cell.
+// March + merge.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ float ex2_neg(float tau2) {  // 2^-tau2, flushes to 0 below 2^-126
+    float r;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(-tau2));
+    return r;
+}
+
+template <int LV>
+__device__ __forceinline__ void load_vec(const float *p, float (&v)[LV]) {
+    if constexpr (LV == 8) {
+        // one 256-bit load (sm_100: LDG.E.256): 32 B = one sector per lane
+        asm("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+            : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]), "=f"(v[4]), "=f"(v[5]), "=f"(v[6]), "=f"(v[7])
+            : "l"(p));
+    } else if constexpr (LV == 4) {
+        const float4 a = __ldg(reinterpret_cast<const float4 *>(p));
+        v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w;
+    } else if constexpr (LV == 2) {
+        const float2 a = __ldg(reinterpret_cast<const float2 *>(p));
+        v[0] = a.x; v[1] = a.y;
+    } else {
+        v[0] = __ldg(p);
+    }
+}
+
+// Predicated gather: lanes with pred == 0 issue no load and keep the (finite) values their registers
+// already hold; the step length they integrate over is 0, so those values have no effect.
+template <int LV>
+__device__ __forceinline__ void load_vec_if(const float *p, float (&v)[LV], int pred) {
+    if constexpr (LV == 8) {
+        asm("{\n\t.reg .pred q;\n\tsetp.ne.s32 q, %9, 0;\n\t"
+            "@q ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];\n\t}"
+            : "+f"(v[0]), "+f"(v[1]), "+f"(v[2]), "+f"(v[3]), "+f"(v[4]), "+f"(v[5]), "+f"(v[6]), "+f"(v[7])
+            : "l"(p), "r"(pred));
+    } else if constexpr (LV == 4) {
+        asm("{\n\t.reg .pred q;\n\tsetp.ne.s32 q, %5, 0;\n\t"
+            "@q ld.global.nc.v4.f32 {%0,%1,%2,%3}, [%4];\n\t}"
+            : "+f"(v[0]), "+f"(v[1]), "+f"(v[2]), "+f"(v[3])
+            : "l"(p), "r"(pred));
+    } else if constexpr (LV == 2) {
+        asm("{\n\t.reg .pred q;\n\tsetp.ne.s32 q, %3, 0;\n\t"
+            "@q ld.global.nc.v2.f32 {%0,%1}, [%2];\n\t}"
+            : "+f"(v[0]), "+f"(v[1])
+            : "l"(p), "r"(pred));
+    } else {
+        asm("{\n\t.reg .pred q;\n\tsetp.ne.s32 q, %2, 0;\n\t"
+            "@q ld.global.nc.f32 %0, [%1];\n\t}"
+            : "+f"(v[0])
+            : "l"(p), "r"(pred));
+    }
+}
+
+template <int LV>
+__device__ __forceinline__ void store_vec(float *p, const float (&v)[LV]) {
+    if constexpr (LV == 8) {
+        reinterpret_cast<float4 *>(p)[0] = make_float4(v[0], v[1], v[2], v[3]);
+        reinterpret_cast<float4 *>(p)[1] = make_float4(v[4], v[5], v[6], v[7]);
+    } else if constexpr (LV == 4) {
+        reinterpret_cast<float4 *>(p)[0] = make_float4(v[0], v[1], v[2], v[3]);
+    } else if constexpr (LV == 2) {
+        reinterpret_cast<float2 *>(p)[0] = make_float2(v[0], v[1]);
+    } else {
+        p[0] = v[0];
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Pack: one thread per (batch, ym, xm, yd, xd); moves LV wavelengths of one cell.
 // ------------------------------------------------------------------------------------------------
 template <int LV>
 __global__ void __launch_bounds__(256) pack_kernel(PackParams p) {
@@ -101,21 +173,31 @@ __global__ void __launch_bounds__(256) pack_kernel(PackParams p) {
     const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= ncell * p.nb) return;
     const int nbI = (int)(idx / ncell);
-    const long long c = idx - (long long)nbI * ncell;  // output cell index: (y*s + xm)*npx + xd
-    const int npx = p.nx >> p.shift;
-    const int y = (int)(c / p.nx);
-    const int r = (int)(c - (long long)y * p.nx);
-    const int xm = r / npx, xd = r - xm * npx;
-    const int x = (xd << p.shift) + xm;
+    const long long c = idx - (long long)nbI * ncell;  // output cell index ((ym*s + xm)*npy + yd)*npx + xd
+    const int npx = p.nx >> p.shift, npy = p.ny >> p.shift, smask = (1 << p.shift) - 1;
+    const int xd = (int)(c % npx);
+    long long t = c / npx;
+    const int yd = (int)(t % npy);
+    t /= npy;
+    const int xm = (int)t & smask, ym = (int)(t >> p.shift);
+    const int x = (xd << p.shift) + xm, y = (yd << p.shift) + ym;
     const long long src = ((long long)y * p.nx + x) * p.L + (long long)nbI * LV;
-    float c2[LV], S[LV];
+    float ch[LV], et[LV], c2[LV], S[LV];
+    if ((nbI + 1) * LV <= p.L && (p.L % LV) == 0) {
+        load_vec<LV>(p.chi + src, ch);  // one 32-byte sector per thread at LV = 8
+        load_vec<LV>(p.eta + src, et);
+    } else {
+#pragma unroll
+        for (int v = 0; v < LV; v++) {
+            const bool ok = nbI * LV + v < p.L;
+            ch[v] = ok ? __ldg(p.chi + src + v) : 0.f;
+            et[v] = ok ? __ldg(p.eta + src + v) : 0.f;
+        }
+    }
 #pragma unroll
     for (int v = 0; v < LV; v++) {
-        const bool ok = nbI * LV + v < p.L;
-        const float ch = ok ? __ldg(p.chi + src + v) : 0.f;
-        const float et = ok ? __ldg(p.eta + src + v) : 0.f;
-        c2[v] = ch * 1.4426950408889634f;           // tau in units of ln 2: T = 2^-tau2
-        S[v] = ch > 0.f ? et / ch : 0.f;             // vacuum cells emit nothing (include/rc.h "Inputs")
+        c2[v] = ch[v] * 1.4426950408889634f;            // tau in units of ln 2: T = 2^-tau2
+        S[v] = ch[v] > 0.f ? et[v] / ch[v] : 0.f;        // vacuum cells emit nothing (include/rc.h "Inputs")
     }
     float *oc = p.chiT + idx * LV, *os = p.ST + idx * LV;
     if constexpr (LV == 8) {
@@ -147,47 +229,6 @@ cudaError_t launch_pack(const PackParams &p, int LV, cudaStream_t st) {
     return cudaGetLastError();
 }
 
-// ------------------------------------------------------------------------------------------------
-// March + merge.
-// ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ float ex2_neg(float tau2) {  // 2^-tau2, flushes to 0 below 2^-126
-    float r;
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(-tau2));
-    return r;
-}
-
-template <int LV>
-__device__ __forceinline__ void load_vec(const float *p, float (&v)[LV]) {
-    if constexpr (LV == 8) {
-        // one 256-bit load (sm_100: LDG.E.256): 32 lanes x 32 B = 8 full 128-byte lines per request
-        asm("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
-            : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]), "=f"(v[4]), "=f"(v[5]), "=f"(v[6]), "=f"(v[7])
-            : "l"(p));
-    } else if constexpr (LV == 4) {
-        const float4 a = __ldg(reinterpret_cast<const float4 *>(p));
-        v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w;
-    } else if constexpr (LV == 2) {
-        const float2 a = __ldg(reinterpret_cast<const float2 *>(p));
-        v[0] = a.x; v[1] = a.y;
-    } else {
-        v[0] = __ldg(p);
-    }
-}
-
-template <int LV>
-__device__ __forceinline__ void store_vec(float *p, const float (&v)[LV]) {
-    if constexpr (LV == 8) {
-        reinterpret_cast<float4 *>(p)[0] = make_float4(v[0], v[1], v[2], v[3]);
-        reinterpret_cast<float4 *>(p)[1] = make_float4(v[4], v[5], v[6], v[7]);
-    } else if constexpr (LV == 4) {
-        reinterpret_cast<float4 *>(p)[0] = make_float4(v[0], v[1], v[2], v[3]);
-    } else if constexpr (LV == 2) {
-        reinterpret_cast<float2 *>(p)[0] = make_float2(v[0], v[1]);
-    } else {
-        p[0] = v[0];
-    }
-}
-
 // Position of child probe a among the n parents per axis: a/2 - 1/4 in parent index units, clamped
 // at the lattice edge.  Weight `f` goes to q1.
 __device__ __forceinline__ void parent_axis(int a, int n, int &q0, int &q1, float &f) {
@@ -197,37 +238,39 @@ __device__ __forceinline__ void parent_axis(int a, int n, int &q0, int &q1, floa
     q1 = min(max(base + 1, 0), n - 1);
 }
 
-// Warp -> work mapping shared by march_kernel and count_kernel.  A block holds G = min(ngroups, 8)
-// ADJACENT direction groups of the same 32-probe chunk (their rays overlap near the probes: L1 reuse)
-// and, when a cascade has fewer than 8 groups, 8/G neighbouring chunks.  Across blocks the probe
-// chunk varies fastest, then the direction, then the wavelength batch: the blocks resident at any
-// time share a narrow fan of directions (a few MB of step tables) and one batch's planes (L2).
+// Warp -> work mapping shared by march_kernel and count_kernel.  One warp = one PATCH of pw x ph = 32
+// probes (lanes) x one direction group.  Warps are numbered flat: the G = min(ngroups, 8) adjacent
+// direction groups of one patch are neighbours (their rays overlap near the probes), then the patch,
+// then the remaining direction bits, then the wavelength batch: the warps resident at any time
+// share a narrow fan of directions (a few MB of step tables) and one batch's planes (L2).
 struct WarpWork {
-    int nbI, kg;
-    long long pc;
-    bool any;
+    int nbI, kg, a, b;
+    bool any, valid;
 };
 
-__device__ __forceinline__ WarpWork warp_work(const MarchParams &p, long long npc) {
-    const int w = threadIdx.x >> 5;
-    const int G = min(p.ngroups, WARPS_PER_BLOCK), Pb = WARPS_PER_BLOCK / G;
-    const long long pcb_n = (npc + Pb - 1) / Pb;
-    const int kgb_n = p.ngroups / G;
-    long long bid = blockIdx.x;
-    const long long pcb = bid % pcb_n;
-    bid /= pcb_n;
-    const int kgb = (int)(bid % kgb_n);
+__device__ __forceinline__ WarpWork warp_work(const MarchParams &p, long long W, int lane) {
+    const int G = min(p.ngroups, 8);
+    const long long npatch = (long long)p.npatch_x * p.npatch_y;
     WarpWork r;
-    r.nbI = (int)(bid / kgb_n);
-    r.kg = kgb * G + (w % G);
-    r.pc = pcb * Pb + (w / G);
-    r.any = r.pc < npc && r.nbI < p.nb;
+    const int kg_lo = (int)(W % G);
+    W /= G;
+    const long long patch = W % npatch;
+    W /= npatch;
+    const int kgb_n = p.ngroups / G;
+    r.kg = (int)(W % kgb_n) * G + kg_lo;
+    r.nbI = (int)(W / kgb_n);
+    r.any = r.nbI < p.nb;
+    const int py = (int)(patch / p.npatch_x), px = (int)(patch - (long long)py * p.npatch_x);
+    const int pw = 1 << p.pw_log2;
+    r.a = (px << p.pw_log2) + (lane & (pw - 1));
+    r.b = py * (32 >> p.pw_log2) + (lane >> p.pw_log2);
+    r.valid = r.a < p.npx && r.b < p.npy;
+    if (!r.valid) r.a = r.b = 0;
     return r;
 }
 
-__host__ __device__ inline long long march_blocks(int ngroups, long long npc, int nb) {
-    const int G = ngroups < WARPS_PER_BLOCK ? ngroups : WARPS_PER_BLOCK, Pb = WARPS_PER_BLOCK / G;
-    return ((npc + Pb - 1) / Pb) * (ngroups / G) * nb;
+__host__ __device__ inline long long march_warps(const MarchParams &p) {
+    return (long long)p.npatch_x * p.npatch_y * p.ngroups * p.nb;
 }
 
 // Number of leading steps of direction k's table that lie inside the box for this lane's probe.
@@ -248,36 +291,36 @@ __device__ __forceinline__ int steps_inside(const StepXY *xy, int n, bool valid,
     return lo;
 }
 
-// One warp = 32 adjacent probes x 1 direction group (its 4 child directions in turn) x LV wavelengths
-// per lane.  Per step the warp reads one 8-byte table entry (uniform address) and each lane its
-// cell's LV opacities and source functions; the loads of step st+1 are in flight while step st is
-// integrated, and the table is read two steps ahead.
-template <int LV, int MINB>
-__global__ void __launch_bounds__(WARPS_PER_BLOCK * 32, MINB) march_kernel(MarchParams p) {
+// One warp = 32 probes (a pw x ph patch of the probe lattice) x 1 direction group (its 4 child
+// directions in turn) x LV wavelengths per lane.  Per step the warp reads one 8-byte table entry
+// (uniform address) and each lane its cell's LV opacities and source functions.  The gathers run
+// PD steps ahead of the integration in a register ring (slot = step mod PD, loop unrolled by PD):
+// while step st is integrated the loads of steps st+1 .. st+PD-1 are in flight.
+template <int LV, int PD, int WARPS, int MINB>
+__global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) {
+    // sum over the 4 child directions, per thread: parked in shared memory between children so the
+    // marching loop has the registers to itself
+    __shared__ float acc_s[LV][WARPS * 32];
     const int lane = threadIdx.x & 31;
-    const long long nprobe = (long long)p.npx * p.npy;
-    const long long npc = (nprobe + 31) >> 5;
-    const WarpWork ww = warp_work(p, npc);
+    const long long W = (long long)blockIdx.x * WARPS + (threadIdx.x >> 5);
+    const WarpWork ww = warp_work(p, W, lane);
     if (!ww.any) return;
-    const int nbI = ww.nbI, kg = ww.kg;
-    const long long probe = ww.pc * 32 + lane;
-    const bool valid = probe < nprobe;
-    const int b = valid ? (int)(probe / p.npx) : 0;
-    const int a = valid ? (int)(probe - (long long)b * p.npx) : 0;
-    const int s = 1 << p.shift, half = s >> 1;
+    const int nbI = ww.nbI, kg = ww.kg, a = ww.a, b = ww.b;
+    const bool valid = ww.valid;
+    const unsigned probe = (unsigned)b * p.npx + a;
+    const int half = (1 << p.shift) >> 1;
     const int Y0 = (b << p.shift) + half;
     const long long ncell = (long long)p.nx * p.ny;
-    const long long base = (long long)Y0 * p.nx + (long long)half * p.npx + a;  // the vertex's cell, packed layout
-    const float *chi0 = p.chiT + ((long long)nbI * ncell + base) * LV;
-    const float *S0 = p.ST + ((long long)nbI * ncell + base) * LV;
-    const long long ndir = 4LL * p.ngroups;
+    // packed layout [batch][y mod s][x mod s][y div s][x div s][LV]: the lane's probe owns cell
+    // (y div s, x div s) = (b, a) of every phase plane; a step's delta is lane-independent
+    const float *chiB = p.chiT + (long long)nbI * ncell * LV;  // warp-uniform
+    const float *SB = p.ST + (long long)nbI * ncell * LV;
     // (dx, dy) ranges that keep this lane's ray inside the box
     const int dxlo = -(a << p.shift) - half, dxhi = ((p.npx - a) << p.shift) - 1 - half;
     const int dylo = -Y0, dyhi = p.ny - 1 - Y0;
 
-    float acc[LV];
 #pragma unroll
-    for (int v = 0; v < LV; v++) acc[v] = 0.f;
+    for (int v = 0; v < LV; v++) acc_s[v][threadIdx.x] = 0.f;
 
     for (int j = 0; j < 4; j++) {
         const long long k = 4LL * kg + j;
@@ -291,45 +334,52 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32, MINB) march_kernel(March
             const uint2 *tab = reinterpret_cast<const uint2 *>(p.steps + o);
             const int nin = steps_inside(p.xy + o, n, valid, dxlo, dxhi, dylo, dyhi);
             const int nw = __reduce_max_sync(FULL, nin);  // steps this warp walks
-            // a lane past its last in-box step re-reads its own vertex cell over ds = 0: no branch, no effect
-            float c2[LV], S[LV], c2n[LV], Sn[LV];
-            uint2 e0 = __ldg(tab), e1 = __ldg(tab + 1);  // slots have 4 spare entries at the end
-            {
-                const bool in = 0 < nin;
-                const long long d = in ? (long long)(int)e0.x : 0;
-                load_vec<LV>(chi0 + d * LV, c2);
-                load_vec<LV>(S0 + d * LV, S);
+            float c2[PD][LV], S[PD][LV], ds[PD];
+            // prologue: steps 0 .. PD-1 into the ring (the table has 2 PD spare entries at its end)
+#pragma unroll
+            for (int u = 0; u < PD; u++) {
+#pragma unroll
+                for (int v = 0; v < LV; v++) { c2[u][v] = 0.f; S[u][v] = 0.f; }
+                const uint2 e = __ldg(tab + u);
+                const bool in = u < nin;
+                const unsigned long long d = (unsigned long long)(probe + e.x) * (LV * sizeof(float));
+                load_vec_if<LV>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(chiB) + d), c2[u], in);
+                load_vec_if<LV>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(SB) + d), S[u], in);
+                ds[u] = in ? __uint_as_float(e.y) : 0.f;
             }
-            float ds = 0 < nin ? __uint_as_float(e0.y) : 0.f;
+            int chk = 0;
             // a1: eq. 16 along the interval, front to back: with tau accumulated,
             // T_n = 2^-tau2_n and the cell's contribution is S (T_{n-1} - T_n)  [= S T (1 - e^{-chi ds})]
-#pragma unroll 2
-            for (int st = 0; st < nw; st++) {
-                const bool inn = st + 1 < nin;
-                const long long d = inn ? (long long)(int)e1.x : 0;
-                load_vec<LV>(chi0 + d * LV, c2n);
-                load_vec<LV>(S0 + d * LV, Sn);
-                const float dsn = inn ? __uint_as_float(e1.y) : 0.f;
-                e1 = __ldg(tab + st + 2);
+            for (int st = 0; st < nw; st += PD) {
 #pragma unroll
-                for (int v = 0; v < LV; v++) {
-                    tau[v] = fmaf(c2[v], ds, tau[v]);
-                    const float Tn = ex2_neg(tau[v]);
-                    I[v] = fmaf(S[v], T[v] - Tn, I[v]);
-                    T[v] = Tn;
+                for (int u = 0; u < PD; u++) {
+                    const uint2 en = __ldg(tab + st + u + PD);
+                    // integrate step st + u (a slot past the lane's last in-box step has ds = 0: no effect)
+                    const float dsu = ds[u];
+#pragma unroll
+                    for (int v = 0; v < LV; v++) {
+                        tau[v] = fmaf(c2[u][v], dsu, tau[v]);
+                        const float Tn = ex2_neg(tau[v]);
+                        I[v] = fmaf(S[u][v], T[v] - Tn, I[v]);
+                        T[v] = Tn;
+                    }
+                    // refill the slot with step st + u + PD
+                    const bool in = st + u + PD < nin;
+                    const unsigned long long d = (unsigned long long)(probe + en.x) * (LV * sizeof(float));
+                    load_vec_if<LV>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(chiB) + d), c2[u], in);
+                    load_vec_if<LV>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(SB) + d), S[u], in);
+                    ds[u] = in ? __uint_as_float(en.y) : 0.f;
                 }
-                if (p.early_exit && (st & 7) == 7) {
+                if (p.early_exit && (++chk & 3) == 0) {
                     float tmin = tau[0];
 #pragma unroll
                     for (int v = 1; v < LV; v++) tmin = fminf(tmin, tau[v]);
                     // every live lane opaque at every wavelength: T is exactly 0, nothing more can arrive
-                    if (__all_sync(FULL, st >= nin || tmin > 126.f)) break;
+                    if (__all_sync(FULL, st + PD >= nin || tmin > 126.f)) break;
                 }
-#pragma unroll
-                for (int v = 0; v < LV; v++) { c2[v] = c2n[v]; S[v] = Sn[v]; }
-                ds = dsn;
             }
         }
+        const long long ndir = 4LL * p.ngroups;
         if (p.Aup == nullptr) {
             // a2: boundary intensity enters on the top cascade only: rays heading up
             // (sin theta_k > 0  <=>  k < N/2) see I_above, rays heading down I_below
@@ -358,15 +408,17 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32, MINB) march_kernel(March
             }
         }
 #pragma unroll
-        for (int v = 0; v < LV; v++) acc[v] += I[v];
+        for (int v = 0; v < LV; v++) acc_s[v][threadIdx.x] += I[v];
     }
     if (!valid) return;
+    const long long nprobe = (long long)p.npx * p.npy;
+    float acc[LV];
 #pragma unroll
-    for (int v = 0; v < LV; v++) acc[v] *= 0.25f;  // mean over the 4 children (cascade 0: a4, J)
+    for (int v = 0; v < LV; v++) acc[v] = 0.25f * acc_s[v][threadIdx.x];  // mean over the 4 children (cascade 0: a4, J)
     if (p.mode == 0) {
         store_vec<LV>(p.out + (((long long)nbI * p.ngroups + kg) * nprobe + probe) * LV, acc);
     } else if (p.mode == 1) {
-        float *o = p.out + probe * p.L + nbI * LV;
+        float *o = p.out + (long long)probe * p.L + nbI * LV;
         if ((nbI + 1) * LV <= p.L && (p.L % LV) == 0) {
             store_vec<LV>(o, acc);
         } else {
@@ -382,19 +434,33 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32, MINB) march_kernel(March
     }
 }
 
-cudaError_t launch_march(const MarchParams &p, int LV, cudaStream_t st) {
-    const long long nprobe = (long long)p.npx * p.npy;
-    const long long blocks = march_blocks(p.ngroups, (nprobe + 31) >> 5, p.nb);
+template <int LV, int PD, int WARPS, int MINB>
+static cudaError_t launch_march_variant(const MarchParams &p, cudaStream_t st) {
+    const long long blocks = (march_warps(p) + WARPS - 1) / WARPS;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-    const dim3 grid((unsigned)blocks), block(WARPS_PER_BLOCK * 32);
-    // minimum resident blocks per SM (register cap) measured best on cfg 2: LV=8 -> 3 (80 regs), LV=4 -> 4 (64 regs)
-    switch (LV) {
-        case 8: march_kernel<8, 3><<<grid, block, 0, st>>>(p); break;
-        case 4: march_kernel<4, 4><<<grid, block, 0, st>>>(p); break;
-        case 2: march_kernel<2, 4><<<grid, block, 0, st>>>(p); break;
-        default: march_kernel<1, 4><<<grid, block, 0, st>>>(p); break;
-    }
+    march_kernel<LV, PD, WARPS, MINB><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
     return cudaGetLastError();
+}
+
+// variant: 0 = ring of 2 steps, 24 warps/SM (<= 80 registers); 1 = ring of 3, 20 warps/SM (<= 96);
+//          2 = ring of 3, 16 warps/SM (<= 128); 3 = ring of 4, 16 warps/SM (<= 128)
+template <int LV>
+static cudaError_t launch_march_lv(const MarchParams &p, int variant, cudaStream_t st) {
+    switch (variant) {
+        case 1: return launch_march_variant<LV, 3, 5, 4>(p, st);
+        case 2: return launch_march_variant<LV, 3, 8, 2>(p, st);
+        case 3: return launch_march_variant<LV, 4, 8, 2>(p, st);
+        default: return launch_march_variant<LV, 2, 8, 3>(p, st);
+    }
+}
+
+cudaError_t launch_march(const MarchParams &p, int LV, int variant, cudaStream_t st) {
+    switch (LV) {
+        case 8: return launch_march_lv<8>(p, variant, st);
+        case 4: return launch_march_lv<4>(p, variant, st);
+        case 2: return launch_march_lv<2>(p, variant, st);
+        default: return launch_march_lv<1>(p, variant, st);
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -437,17 +503,10 @@ cudaError_t launch_validate(const float *chi, const float *eta, long long n, int
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) count_kernel(MarchParams p, unsigned long long *total) {
     const int lane = threadIdx.x & 31;
-    const long long nprobe = (long long)p.npx * p.npy;
-    const long long npc = (nprobe + 31) >> 5;
-    const long long nwarps = npc * p.ngroups;
     const long long W = (long long)blockIdx.x * WARPS_PER_BLOCK + (threadIdx.x >> 5);
-    if (W >= nwarps || p.cnt == nullptr) return;
-    const long long pc = W / p.ngroups;
-    const int kg = (int)(W - pc * p.ngroups);
-    const long long probe = pc * 32 + lane;
-    const bool valid = probe < nprobe;
-    const int b = valid ? (int)(probe / p.npx) : 0;
-    const int a = valid ? (int)(probe - (long long)b * p.npx) : 0;
+    if (W >= (long long)p.npatch_x * p.npatch_y * p.ngroups || p.cnt == nullptr) return;
+    const WarpWork ww = warp_work(p, W, lane);  // batch index is the slowest: W covers batch 0 only
+    const int a = ww.a, b = ww.b, kg = ww.kg;
     const int s = 1 << p.shift, half = s >> 1;
     const int Y0 = (b << p.shift) + half;
     const int dxlo = -(a << p.shift) - half, dxhi = ((p.npx - a) << p.shift) - 1 - half;
@@ -456,15 +515,14 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) count_kernel(MarchParams
     for (int j = 0; j < 4; j++) {
         const long long k = 4LL * kg + j;
         const long long o = __ldg(p.off + k);
-        mine += (unsigned long long)steps_inside(p.xy + o, __ldg(p.cnt + k), valid, dxlo, dxhi, dylo, dyhi);
+        mine += (unsigned long long)steps_inside(p.xy + o, __ldg(p.cnt + k), ww.valid, dxlo, dxhi, dylo, dyhi);
     }
     for (int o = 16; o > 0; o >>= 1) mine += __shfl_down_sync(FULL, mine, o);
     if (lane == 0 && mine) atomicAdd(total, mine);
 }
 
 cudaError_t launch_count(const MarchParams &p, unsigned long long *total, cudaStream_t st) {
-    const long long nprobe = (long long)p.npx * p.npy;
-    const long long nwarps = ((nprobe + 31) >> 5) * p.ngroups;
+    const long long nwarps = (long long)p.npatch_x * p.npatch_y * p.ngroups;
     const long long blocks = (nwarps + WARPS_PER_BLOCK - 1) / WARPS_PER_BLOCK;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     count_kernel<<<(unsigned)blocks, WARPS_PER_BLOCK * 32, 0, st>>>(p, total);

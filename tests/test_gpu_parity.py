@@ -186,3 +186,23 @@ def test_segment_counts_match_the_oracle(oracle):
         assert len(seg) == atm.ncascades
         for g, o in zip(seg, ref):
             assert abs(g - int(o)) <= max(2, 1e-5 * int(o)), (seg, list(ref))
+
+
+# ------------------------------------------------------------------ launch variants
+@pytest.mark.parametrize("variant", [0, 1, 2, 3])
+@pytest.mark.parametrize("patch", [None, 2, 3, 4, 5])
+def test_patch_shapes_and_ring_depths_are_bit_identical(oracle, monkeypatch, variant, patch):
+    """The lane patch (32x1 .. 4x8 probes per warp) and the register-ring depth / occupancy variant of
+    march_kernel only change which lane marches which ray and how far ahead it gathers: every ray's
+    arithmetic is the same, so J is bit-identical to the default launch, and within TOL of the oracle.
+    Non-square grid with a ragged last wavelength batch; 6 cascades so that the top ones are clipped."""
+    atm = A.make_config(3, nx=192, ny=128, nlambda=11, ncascades=6, seed=5)
+    ref = gpu_solve(atm)
+    monkeypatch.setenv("RC_MARCH_VARIANT", str(variant))
+    if patch is not None:
+        monkeypatch.setenv("RC_PATCH_LOG2", str(patch))
+    got = gpu_solve(atm)
+    assert np.array_equal(ref, got)
+    if variant == 0 and patch is None:
+        Jo = oracle.solve_atmosphere(atm)["J"]
+        assert rel_err(got, Jo) <= TOL
