@@ -162,6 +162,8 @@ def main():
     rc.set_boundary(atm.I_below, atm.I_above)
     rc.set_lambda_weights(atm.weights)
     seg = rc.count_segments()
+    l2_gather_gbs = rc.probe_gather_bandwidth(64)      # L2 -> SM ceiling of the gather pattern (64 MB region)
+    hbm_gather_gbs = rc.probe_gather_bandwidth(1024) if rc._ws.numel() > (1100 << 20) else None
     segl_per_step = sum(seg) * atm.nlambda
     J = rc.solve_J()
     for _ in range(args.warmup - 1):
@@ -234,6 +236,10 @@ def main():
                          "peak_source": peak_src, "ms_per_launch": ms_march[dom],
                          "note": "effective: algorithmic gather bytes (8 B per segment-wavelength) are mostly served "
                                  "from L1/L2, so frac may exceed 1; see roofline_alu for the binding on-chip ceiling"},
+            "roofline_l2": {"bound": "l2", "achieved": ach, "peak": l2_gather_gbs, "unit": "GB/s", "frac": ach / l2_gather_gbs,
+                            "peak_source": "rc_probe_gather_bandwidth(64 MB), measured in this run: random 1 KB warp-wide runs "
+                                           "(LDG.256), 48 warps/SM, region L2-resident",
+                            "hbm_gather_gbs_1GB_region": hbm_gather_gbs},
             "roofline_alu": {"bound": "alu", "pipe": "MUFU.EX2, 16/clk/SM x 148 SMs at sm_max_mhz", "achieved": ach_alu,
                              "peak": sfu_peak, "unit": UNIT, "frac": ach_alu / sfu_peak},
             "per_cascade_ms": {"march": ms_march, "pack": [st.ms_pack[i] for i in range(atm.ncascades)]},

@@ -132,6 +132,13 @@ int rc_get_stats(rc_ctx *ctx, rc_stats *out);
  * wavelength.  Counted on the device from the step tables; synchronises. */
 int rc_count_segments(rc_ctx *ctx, int64_t *per_cascade);
 
+/* Measurement aid for the roofline: achieved GB/s (*gbs, host) of the access pattern the
+ * march gathers with and nothing else - every warp reads pseudo-random 1 KB runs (32 lanes x 32 B), 48
+ * warps per SM - over the first `mbytes` MB of the workspace (read only; contents irrelevant).  A region
+ * that fits the 126 MB L2 gives the L2 -> SM gather ceiling, a larger one the HBM gather ceiling.
+ * Runs on the context's stream and synchronises it.  RC_ERR_BAD_VALUE if the region does not fit. */
+int rc_probe_gather_bandwidth(rc_ctx *ctx, int mbytes, double *gbs);
+
 const char *rc_last_error(const rc_ctx *ctx);
 const char *rc_version(void);
 int rc_destroy(rc_ctx *ctx);

@@ -47,6 +47,7 @@ SYMBOLS = {
     "rc_set_timing": (C.c_int, [C.c_void_p, C.c_int]),
     "rc_get_stats": (C.c_int, [C.c_void_p, C.POINTER(rc_stats)]),
     "rc_count_segments": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "rc_probe_gather_bandwidth": (C.c_int, [C.c_void_p, C.c_int, C.POINTER(C.c_double)]),
     "rc_last_error": (C.c_char_p, [C.c_void_p]),
     "rc_version": (C.c_char_p, []),
     "rc_destroy": (C.c_int, [C.c_void_p]),
@@ -191,6 +192,12 @@ class RadianceCascades:
         out = (C.c_int64 * RC_MAX_CASCADES)()
         self._check(self.lib.rc_count_segments(self.handle, out))
         return [int(out[i]) for i in range(self.cfg.ncascades)]
+
+    def probe_gather_bandwidth(self, mbytes=64):
+        """GB/s of the march's gather pattern alone over the first `mbytes` MB of the workspace."""
+        gbs = C.c_double(0.0)
+        self._check(self.lib.rc_probe_gather_bandwidth(self.handle, int(mbytes), C.byref(gbs)))
+        return float(gbs.value)
 
     def get_stats(self) -> rc_stats:
         st = rc_stats()

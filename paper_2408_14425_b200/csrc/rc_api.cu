@@ -18,6 +18,7 @@ constexpr size_t ALIGN = 256;
 inline size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 
 struct CascadePlan {
+    bool banded = false;        // marched band by band (Plan::nbands launches per direction half)
     int pw_log2 = 5;            // lane patch of the march: 2^pw_log2 probes wide, 32 >> pw_log2 high
     long long ndir = 0;         // 4^(i+1)
     bool empty = true;          // interval starts beyond the box diagonal: no ray of it is inside
@@ -29,6 +30,8 @@ struct CascadePlan {
 struct Plan {
     int nx = 0, ny = 0, L = 0, ncasc = 0;
     int LV = 1, nb = 1, Lpad = 1;
+    int nbands = 1, band_axis = 0;  // L2 banding of the long-ray cascades (1 = off); axis 0 = rows, 1 = columns
+    size_t state = 0;               // parked ray state of the banded launches
     CascadePlan c[RC_MAX_CASCADES];
     size_t chiT = 0, ST = 0, A[2] = {0, 0}, Jpart = 0, bc_below = 0, bc_above = 0, weights = 0, flag = 0;
     size_t io_chi = 0, io_eta = 0, io_J = 0;
@@ -166,7 +169,7 @@ bool make_plan(const rc_config &cfg, int nx, int ny, int L, bool host_io, Plan &
         c.pw_log2 = 5;
         while (c.pw_log2 > 0 && (1 << c.pw_log2) > (nx >> i)) c.pw_log2--;
         if (c.empty) continue;
-        if (offs) c.pw_log2 = choose_patch(nx, ny, i, c.ta, c.tb);
+        c.pw_log2 = choose_patch(nx, ny, i, c.ta, c.tb);
         std::vector<long long> local;
         std::vector<long long> &o = offs ? (*offs)[i] : local;
         o.resize((size_t)c.ndir + 1);
@@ -195,6 +198,29 @@ bool make_plan(const rc_config &cfg, int nx, int ny, int L, bool host_io, Plan &
         c.xy_off = cur;    cur = align_up(cur + sizeof(rc::StepXY) * ((size_t)acc + 16));
     }
     const size_t field = align_up(ncell * P.Lpad * sizeof(float));
+    // L2 banding: one wavelength batch of packed chi and S is ncell * LV * 8 bytes; when that exceeds the
+    // L2 budget the cascades with long rays are marched band by band
+    {
+        const double batch_mb = (double)ncell * P.LV * 8.0 / (1 << 20);
+        double budget_mb = 72.0;
+        if (const char *e = std::getenv("RC_L2_MB")) budget_mb = std::max(1.0, std::atof(e));
+        P.nbands = (int)std::ceil(batch_mb / budget_mb);
+        if (const char *e = std::getenv("RC_BANDS")) P.nbands = std::max(1, std::atoi(e));
+        P.band_axis = nx > ny ? 1 : 0;
+        const int n_axis = P.band_axis ? nx : ny;
+        P.nbands = std::max(1, std::min(P.nbands, n_axis / 32));
+        const int ext = (n_axis + P.nbands - 1) / P.nbands;
+        bool any = false;
+        for (int i = 1; i <= top; i++) {
+            CascadePlan &c = P.c[i];
+            // worth it for long rays only, and only while one warp's patch of probes is small against a
+            // band (its lanes enter and leave a band at different steps: lock-step waste otherwise)
+            const int patch_ext = (P.band_axis ? 1 << c.pw_log2 : 32 >> c.pw_log2) << i;
+            c.banded = P.nbands > 1 && !c.empty && std::fmin(c.tb, diag) > 100.0 && (4 * patch_ext <= ext || std::getenv("RC_BANDS"));
+            any = any || c.banded;
+        }
+        if (any) { P.state = cur; cur += 8 * field; }
+    }
     P.chiT = cur; cur += field;
     P.ST = cur;   cur += field;
     P.A[0] = cur; cur += field;
@@ -316,7 +342,6 @@ int rc_set_atmosphere(rc_ctx *ctx, const float *chi, const float *eta, int nx, i
             return fail(ctx, RC_ERR_NO_WORKSPACE, "workspace has %zu bytes, %zu needed", ctx->ws_bytes, P.total);
         make_plan(ctx->cfg, nx, ny, nlambda, true, Pio, nullptr);
         ctx->host_io = Pio.total <= ctx->ws_bytes;
-        for (int i = 0; i < ctx->cfg.ncascades; i++) Pio.c[i].pw_log2 = P.c[i].pw_log2;  // chosen only when offs is built
         ctx->plan = ctx->host_io ? Pio : P;
         ctx->have_atm = false;
         // geometry tables: only when the grid size changed (they do not depend on nlambda)
@@ -417,6 +442,9 @@ static rc::MarchParams march_params(const rc_ctx *ctx, int i, float *J_out) {
     const int pw = 1 << mp.pw_log2, ph = 32 >> mp.pw_log2;
     mp.npatch_x = (mp.npx + pw - 1) / pw;
     mp.npatch_y = (mp.npy + ph - 1) / ph;
+    mp.kg_n = mp.ngroups; mp.kg_off = 0;
+    mp.state = nullptr;
+    mp.band_axis = 0; mp.band_sign = 1; mp.band_lo = 0; mp.band_hi = 0; mp.band_final = 1;
     return mp;
 }
 
@@ -445,8 +473,31 @@ int rc_solve_J(rc_ctx *ctx, float *J_out) {
             launches++;
         }
         if (ev) RC_CUDA(ctx, cudaEventRecord(ev[1 + 2 * (top - i)], ctx->stream));
-        RC_CUDA(ctx, rc::launch_march(march_params(ctx, i, J_out), P.LV, ctx->tune_variant, ctx->stream));
-        launches++;
+        rc::MarchParams mp = march_params(ctx, i, J_out);
+        if (!c.banded) {
+            RC_CUDA(ctx, rc::launch_march(mp, P.LV, ctx->tune_variant, ctx->stream));
+            launches++;
+        } else {
+            // rays heading up (right) cross the bands in ascending order, the others in descending order;
+            // the last band of each half does the merge and writes the cascade
+            const int n_axis = P.band_axis ? P.nx : P.ny, ext = (n_axis + P.nbands - 1) / P.nbands;
+            mp.state = (float *)(ctx->ws + P.state);
+            mp.band_axis = P.band_axis;
+            mp.kg_n = mp.ngroups / 2;
+            for (int h = 0; h < 2; h++) {
+                mp.band_sign = h == 0 ? 1 : -1;
+                // rows: sin(theta_k) > 0 for the first half of the circle; columns: cos > 0 for the quarter either side of k = 0
+                mp.kg_off = P.band_axis ? (h == 0 ? mp.ngroups - mp.ngroups / 4 : mp.ngroups / 4) : (h == 0 ? 0 : mp.ngroups / 2);
+                for (int bi = 0; bi < P.nbands; bi++) {
+                    const int beta = h == 0 ? bi : P.nbands - 1 - bi;
+                    mp.band_lo = beta * ext;
+                    mp.band_hi = std::min(n_axis, (beta + 1) * ext);
+                    mp.band_final = bi == P.nbands - 1;
+                    RC_CUDA(ctx, rc::launch_march(mp, P.LV, ctx->tune_variant, ctx->stream));
+                    launches++;
+                }
+            }
+        }
         if (ev) RC_CUDA(ctx, cudaEventRecord(ev[2 + 2 * (top - i)], ctx->stream));
     }
     if (accum) {
@@ -498,6 +549,37 @@ int rc_solve_J_host(rc_ctx *ctx, const float *chi_host, const float *eta_host, i
     const size_t nout = (ctx->cfg.flags & RC_ACCUM_J) ? (size_t)nx * ny * sizeof(float) : n;
     RC_CUDA(ctx, cudaMemcpyAsync(J_host, dJ, nout, cudaMemcpyDeviceToHost, ctx->stream));
     RC_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return RC_OK;
+}
+
+// Achieved GB/s of the march's gather pattern alone over the first `mbytes` MB of the workspace.
+int rc_probe_gather_bandwidth(rc_ctx *ctx, int mbytes, double *gbs) {
+    if (!ctx || !gbs) return ctx ? fail(ctx, RC_ERR_NULL_ARG, "null output") : RC_ERR_NULL_ARG;
+    if (!ctx->ws) return fail(ctx, RC_ERR_NO_WORKSPACE, "rc_set_workspace has not been called");
+    const size_t bytes = (size_t)mbytes << 20;
+    if (mbytes < 1 || bytes + ALIGN > ctx->ws_bytes)
+        return fail(ctx, RC_ERR_BAD_VALUE, "probe region of %d MB does not fit the workspace (%zu bytes)", mbytes, ctx->ws_bytes);
+    RC_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    cudaDeviceProp prop;
+    RC_CUDA(ctx, cudaGetDeviceProperties(&prop, ctx->cfg.device));
+    const int blocks = prop.multiProcessorCount * 6, iters = 2048;  // 48 warps per SM
+    float *sink = (float *)(ctx->ws + bytes);
+    cudaEvent_t e0, e1;
+    RC_CUDA(ctx, cudaEventCreate(&e0));
+    RC_CUDA(ctx, cudaEventCreate(&e1));
+    float best = 1e30f;
+    for (int rep = 0; rep < 4; rep++) {  // the first pass also brings the region into L2
+        RC_CUDA(ctx, cudaEventRecord(e0, ctx->stream));
+        RC_CUDA(ctx, rc::launch_gather_probe((const float *)ctx->ws, bytes / 32, iters, blocks, sink, ctx->stream));
+        RC_CUDA(ctx, cudaEventRecord(e1, ctx->stream));
+        RC_CUDA(ctx, cudaEventSynchronize(e1));
+        float ms = 0.f;
+        RC_CUDA(ctx, cudaEventElapsedTime(&ms, e0, e1));
+        if (rep > 0 && ms < best) best = ms;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    *gbs = (double)blocks * 8 * iters * 1024.0 / (best * 1e-3) / 1e9;
     return RC_OK;
 }
 

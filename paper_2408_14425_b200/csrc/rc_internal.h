@@ -49,6 +49,11 @@ struct MarchParams {
     int early_exit;
     int pw_log2;           // one warp's 32 probes form a patch 2^pw_log2 wide, 32 >> pw_log2 high
     int npatch_x, npatch_y;  // patches per axis
+    int kg_n, kg_off;      // the launch covers direction groups (kg_off + 0 .. kg_n-1) mod ngroups
+    // banded launch (state != null): only the steps inside [band_lo, band_hi) along band_axis
+    // (0 = rows, 1 = columns), for rays travelling in direction band_sign along that axis
+    float *state;          // parked rays: [nb][ngroups][4][npy][npx][2][LV]  (I, tau*log2 e)
+    int band_axis, band_sign, band_lo, band_hi, band_final;
 };
 
 struct PackParams {
@@ -74,6 +79,7 @@ cudaError_t launch_march(const MarchParams &p, int LV, int variant, cudaStream_t
 cudaError_t launch_table_build(const TableBuildParams &p, cudaStream_t st);
 cudaError_t launch_reduce_jbar(const float *Jpart, float *Jbar, long long ncell, int nb, cudaStream_t st);
 cudaError_t launch_count(const MarchParams &p, unsigned long long *total, cudaStream_t st);
+cudaError_t launch_gather_probe(const float *buf, unsigned long long nsector, int iters, int blocks, float *sink, cudaStream_t st);
 cudaError_t launch_validate(const float *chi, const float *eta, long long n, int *flag, cudaStream_t st);
 
 }  // namespace rc

@@ -229,6 +229,33 @@ cudaError_t launch_pack(const PackParams &p, int LV, cudaStream_t st) {
     return cudaGetLastError();
 }
 
+// Streaming (evict-first) access for the banded launches' parked ray state: read once, written once.
+template <int LV>
+__device__ __forceinline__ void load_vec_cs(const float *p, float (&v)[LV]) {
+    if constexpr (LV >= 4) {
+#pragma unroll
+        for (int q = 0; q < LV / 4; q++) {
+            const float4 a = __ldcs(reinterpret_cast<const float4 *>(p) + q);
+            v[4 * q] = a.x; v[4 * q + 1] = a.y; v[4 * q + 2] = a.z; v[4 * q + 3] = a.w;
+        }
+    } else {
+#pragma unroll
+        for (int q = 0; q < LV; q++) v[q] = __ldcs(p + q);
+    }
+}
+
+template <int LV>
+__device__ __forceinline__ void store_vec_cs(float *p, const float (&v)[LV]) {
+    if constexpr (LV >= 4) {
+#pragma unroll
+        for (int q = 0; q < LV / 4; q++)
+            __stcs(reinterpret_cast<float4 *>(p) + q, make_float4(v[4 * q], v[4 * q + 1], v[4 * q + 2], v[4 * q + 3]));
+    } else {
+#pragma unroll
+        for (int q = 0; q < LV; q++) __stcs(p + q, v[q]);
+    }
+}
+
 // Position of child probe a among the n parents per axis: a/2 - 1/4 in parent index units, clamped
 // at the lattice edge.  Weight `f` goes to q1.
 __device__ __forceinline__ void parent_axis(int a, int n, int &q0, int &q1, float &f) {
@@ -249,15 +276,16 @@ struct WarpWork {
 };
 
 __device__ __forceinline__ WarpWork warp_work(const MarchParams &p, long long W, int lane) {
-    const int G = min(p.ngroups, 8);
+    const int G = min(p.kg_n, 8);
     const long long npatch = (long long)p.npatch_x * p.npatch_y;
     WarpWork r;
     const int kg_lo = (int)(W % G);
     W /= G;
     const long long patch = W % npatch;
     W /= npatch;
-    const int kgb_n = p.ngroups / G;
-    r.kg = (int)(W % kgb_n) * G + kg_lo;
+    const int kgb_n = p.kg_n / G;
+    // a launch covers kg_n consecutive direction groups starting at kg_off, modulo the full circle
+    r.kg = ((int)(W % kgb_n) * G + kg_lo + p.kg_off) & (p.ngroups - 1);
     r.nbI = (int)(W / kgb_n);
     r.any = r.nbI < p.nb;
     const int py = (int)(patch / p.npatch_x), px = (int)(patch - (long long)py * p.npatch_x);
@@ -270,7 +298,7 @@ __device__ __forceinline__ WarpWork warp_work(const MarchParams &p, long long W,
 }
 
 __host__ __device__ inline long long march_warps(const MarchParams &p) {
-    return (long long)p.npatch_x * p.npatch_y * p.ngroups * p.nb;
+    return (long long)p.npatch_x * p.npatch_y * p.kg_n * p.nb;
 }
 
 // Number of leading steps of direction k's table that lie inside the box for this lane's probe.
@@ -291,12 +319,35 @@ __device__ __forceinline__ int steps_inside(const StepXY *xy, int n, bool valid,
     return lo;
 }
 
+// Banded launches (grids whose wavelength batch does not fit L2): first step st in [0, n] whose cell
+// coordinate along the band axis, c0 + d(st), has reached `thr` in the ray's direction of travel
+// (sg = +1: c >= thr, sg = -1: c <= thr).  d is monotone along the ray, so this is a bisection.
+__device__ __forceinline__ int first_step_reaching(const StepXY *xy, int n, int axis, int sg, int c0, int thr) {
+    int lo = 0, hi = n;
+    const int iters = 32 - __clz(n);
+    for (int it = 0; it < iters; it++) {
+        const int mid = (lo + hi) >> 1;
+        if (lo < hi) {
+            const unsigned e = __ldg(reinterpret_cast<const unsigned *>(xy) + mid);
+            const int d = axis ? (int)(short)(e & 0xffffu) : (int)(short)(e >> 16);
+            const bool reached = sg * (c0 + d) >= sg * thr;
+            if (reached) hi = mid; else lo = mid + 1;
+        }
+    }
+    return lo;
+}
+
 // One warp = 32 probes (a pw x ph patch of the probe lattice) x 1 direction group (its 4 child
 // directions in turn) x LV wavelengths per lane.  Per step the warp reads one 8-byte table entry
 // (uniform address) and each lane its cell's LV opacities and source functions.  The gathers run
 // PD steps ahead of the integration in a register ring (slot = step mod PD, loop unrolled by PD):
 // while step st is integrated the loads of steps st+1 .. st+PD-1 are in flight.
-template <int LV, int PD, int WARPS, int MINB>
+//
+// BANDED: the launch covers only the steps inside one band of rows (or columns) of the grid and only the
+// half of the directions that crosses the bands in ascending (or descending) order; a ray's (I, tau)
+// is carried from band to band through `state`, so the arithmetic - and the result - is that of the
+// unbanded launch, bit for bit, while the cells gathered by one launch fit L2.
+template <int LV, int PD, int WARPS, int MINB, bool BANDED>
 __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) {
     // sum over the 4 child directions, per thread: parked in shared memory between children so the
     // marching loop has the registers to itself
@@ -332,7 +383,29 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
             const long long o = __ldg(p.off + k);
             const int n = __ldg(p.cnt + k);
             const uint2 *tab = reinterpret_cast<const uint2 *>(p.steps + o);
-            const int nin = steps_inside(p.xy + o, n, valid, dxlo, dxhi, dylo, dyhi);
+            int nin = steps_inside(p.xy + o, n, valid, dxlo, dxhi, dylo, dyhi);
+            int n0 = 0;       // this lane's first step of this launch
+            bool has = true;  // banded: the lane has steps in this band
+            if constexpr (BANDED) {
+                const int c0 = p.band_axis ? (a << p.shift) + half : Y0;
+                const int sg = p.band_sign;
+                // steps [n0, n1) of this launch: those inside rows/columns [band_lo, band_hi)
+                n0 = min(nin, first_step_reaching(p.xy + o, n, p.band_axis, sg, c0, sg > 0 ? p.band_lo : p.band_hi - 1));
+                const int n1 = min(nin, first_step_reaching(p.xy + o, n, p.band_axis, sg, c0, sg > 0 ? p.band_hi : p.band_lo - 1));
+                has = n1 > n0;
+                if (valid && n0 > 0 && (has || p.band_final)) {  // steps were taken in earlier bands: resume
+                    const float *stp = p.state + ((((long long)nbI * p.ngroups + kg) * 4 + j) * ((long long)p.npx * p.npy) + probe) * (2 * LV);
+                    load_vec_cs<LV>(stp, I);
+                    load_vec_cs<LV>(stp + LV, tau);
+#pragma unroll
+                    for (int v = 0; v < LV; v++) T[v] = ex2_neg(tau[v]);
+                }
+                int w0 = __reduce_min_sync(FULL, has ? n0 : 0x7fffffff);  // the warp's first step
+                if (w0 == 0x7fffffff) w0 = 0;
+                tab += w0;  // from here on step indices are relative to the warp's first step
+                nin = has ? n1 - w0 : 0;
+                n0 = has ? n0 - w0 : 0;
+            }
             const int nw = __reduce_max_sync(FULL, nin);  // steps this warp walks
             float c2[PD][LV], S[PD][LV], ds[PD];
             // prologue: steps 0 .. PD-1 into the ring (the table has 2 PD spare entries at its end)
@@ -341,7 +414,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
 #pragma unroll
                 for (int v = 0; v < LV; v++) { c2[u][v] = 0.f; S[u][v] = 0.f; }
                 const uint2 e = __ldg(tab + u);
-                const bool in = u < nin;
+                const bool in = u < nin && (!BANDED || u >= n0);
                 const unsigned long long d = (unsigned long long)(probe + e.x) * (LV * sizeof(float));
                 load_vec_if<LV>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(chiB) + d), c2[u], in);
                 load_vec_if<LV>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(SB) + d), S[u], in);
@@ -364,7 +437,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
                         T[v] = Tn;
                     }
                     // refill the slot with step st + u + PD
-                    const bool in = st + u + PD < nin;
+                    const bool in = st + u + PD < nin && (!BANDED || st + u + PD >= n0);
                     const unsigned long long d = (unsigned long long)(probe + en.x) * (LV * sizeof(float));
                     load_vec_if<LV>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(chiB) + d), c2[u], in);
                     load_vec_if<LV>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(SB) + d), S[u], in);
@@ -376,6 +449,16 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
                     for (int v = 1; v < LV; v++) tmin = fminf(tmin, tau[v]);
                     // every live lane opaque at every wavelength: T is exactly 0, nothing more can arrive
                     if (__all_sync(FULL, st + PD >= nin || tmin > 126.f)) break;
+                }
+            }
+            if constexpr (BANDED) {
+                if (!p.band_final) {  // park the ray; the launch of its next band resumes it
+                    if (valid && has) {
+                        float *stp = p.state + ((((long long)nbI * p.ngroups + kg) * 4 + j) * ((long long)p.npx * p.npy) + probe) * (2 * LV);
+                        store_vec_cs<LV>(stp, I);
+                        store_vec_cs<LV>(stp + LV, tau);
+                    }
+                    continue;
                 }
             }
         }
@@ -411,6 +494,9 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
         for (int v = 0; v < LV; v++) acc_s[v][threadIdx.x] += I[v];
     }
     if (!valid) return;
+    if constexpr (BANDED) {
+        if (!p.band_final) return;
+    }
     const long long nprobe = (long long)p.npx * p.npy;
     float acc[LV];
 #pragma unroll
@@ -438,7 +524,10 @@ template <int LV, int PD, int WARPS, int MINB>
 static cudaError_t launch_march_variant(const MarchParams &p, cudaStream_t st) {
     const long long blocks = (march_warps(p) + WARPS - 1) / WARPS;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-    march_kernel<LV, PD, WARPS, MINB><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
+    if (p.state != nullptr)
+        march_kernel<LV, PD, WARPS, MINB, true><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
+    else
+        march_kernel<LV, PD, WARPS, MINB, false><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
     return cudaGetLastError();
 }
 
@@ -447,10 +536,10 @@ static cudaError_t launch_march_variant(const MarchParams &p, cudaStream_t st) {
 template <int LV>
 static cudaError_t launch_march_lv(const MarchParams &p, int variant, cudaStream_t st) {
     switch (variant) {
+        case 0: return launch_march_variant<LV, 2, 8, 3>(p, st);
         case 1: return launch_march_variant<LV, 3, 5, 4>(p, st);
-        case 2: return launch_march_variant<LV, 3, 8, 2>(p, st);
         case 3: return launch_march_variant<LV, 4, 8, 2>(p, st);
-        default: return launch_march_variant<LV, 2, 8, 3>(p, st);
+        default: return launch_march_variant<LV, 3, 8, 2>(p, st);
     }
 }
 
@@ -526,6 +615,40 @@ cudaError_t launch_count(const MarchParams &p, unsigned long long *total, cudaSt
     const long long blocks = (nwarps + WARPS_PER_BLOCK - 1) / WARPS_PER_BLOCK;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     count_kernel<<<(unsigned)blocks, WARPS_PER_BLOCK * 32, 0, st>>>(p, total);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
+// Measurement aid (rc_probe_gather_bandwidth): the march's access pattern with nothing else — every
+// warp reads pseudo-random 1 KB runs (32 lanes x 32 B, LDG.256), two in flight per warp, 48 warps per
+// SM — over a region of `nsector` 32-byte sectors.  Region inside L2: the L2 -> SM gather ceiling.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned hash32(unsigned x) {
+    x ^= x >> 16; x *= 0x7feb352du; x ^= x >> 15; x *= 0x846ca68bu; x ^= x >> 16;
+    return x;
+}
+
+__global__ void __launch_bounds__(256) gather_probe_kernel(const float *buf, unsigned long long nsector, int iters, float *sink) {
+    const int lane = threadIdx.x & 31;
+    const unsigned warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    float acc = 0.f;
+    for (int it = 0; it < iters; it += 2) {
+        float v[2][8];
+#pragma unroll
+        for (int u = 0; u < 2; u++) {
+            const unsigned long long c = hash32(warp * 7919u + it + u) % (nsector - 32);
+            load_vec<8>(buf + (c + lane) * 8, v[u]);
+        }
+#pragma unroll
+        for (int u = 0; u < 2; u++)
+#pragma unroll
+            for (int k = 0; k < 8; k++) acc += v[u][k];
+    }
+    if (acc == 12345.678f) sink[0] = acc;  // never true in practice: keeps the loads alive
+}
+
+cudaError_t launch_gather_probe(const float *buf, unsigned long long nsector, int iters, int blocks, float *sink, cudaStream_t st) {
+    gather_probe_kernel<<<blocks, 256, 0, st>>>(buf, nsector, iters, sink);
     return cudaGetLastError();
 }
 
