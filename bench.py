@@ -31,6 +31,9 @@ from paper_2408_14425_b200 import atmospheres  # noqa: E402
 METRIC = "probe-ray-wavelength segments/sec"
 UNIT = "seg-lambda/s"
 SM_COUNT, MUFU_PER_CLK_SM = 148, 16  # one ex2 per segment-wavelength; DESIGN.md §7
+# dram__bytes_read.sum + dram__bytes_write.sum of the dominant launch, from the committed ncu --set full
+# capture (profiles/ncu_r1b_march.md): configs[2], march_kernel cascade 5
+NCU_TRAFFIC_BYTES = {(2, 5): 9.20e9}
 
 
 def peaks():
@@ -232,7 +235,9 @@ def main():
             "solve_ms": ms_step,
             "hbm_effective_frac": (8 * segl_per_step + 2 * casc_bytes * atm.ncascades) / (ms_step * 1e-3) / 1e9 / hbm_peak,
             "roofline": {"bound": "hbm", "kernel": f"march_kernel<{st.lambda_batch}> cascade {dom}", "achieved": ach,
-                         "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak, "traffic": None,
+                         "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak, "traffic": NCU_TRAFFIC_BYTES.get((args.config, dom)),
+                         "traffic_unit": "bytes per launch (ncu --set full, profiles/ncu_r1b_march.md)",
+                         "algorithmic_bytes": alg_bytes,
                          "peak_source": peak_src, "ms_per_launch": ms_march[dom],
                          "note": "effective: algorithmic gather bytes (8 B per segment-wavelength) are mostly served "
                                  "from L1/L2, so frac may exceed 1; see roofline_alu for the binding on-chip ceiling"},

@@ -21,6 +21,10 @@
  *                      each interval merged with its 4 children in the cone PAPER.md:199-207
  *   lattice edge       parent lookup clamped
  *   J                  mean over the 4 merged cascade-0 directions         PAPER.md:36 (eq. 1), 191
+ *   2.5D  each flatland ray replaced by rays with the same projection and
+ *                      different inclinations to the invariant axis: same cells, path length
+ *                      ds / sin(inclination); J = sum_m w_m J_m
+ *                      (rc_oracle_solve_scaled does one inclination; oracle/rc_oracle.py sums)
  *
  * Readings where the paper is silent or garbled are DESIGN.md §3 (G1..G19 of SURVEY.md §8(c)).
  * The only loop restructuring relative to SURVEY.md's listing: the wavelength loop is innermost
@@ -51,6 +55,9 @@
 typedef struct {
     int nx, ny, L;
     const float *chi, *eta; /* [ny][nx][L], wavelength fastest, y = 0 bottom row */
+    double path_scale;      /* true path length per unit length in the plane: 1 in flatland; 1/sin(inclination
+                               to the invariant axis) for the inclined rays of the 2.5D scheme (PAPER.md:281:
+                               "the same x-z projection and different inclinations in y") */
 } grid_t;
 
 typedef struct {
@@ -135,7 +142,7 @@ static void integrate_ftb(const grid_t *g, const seg_t *seg, int n, double *I, d
         double Il = 0.0, Tl = 1.0;
         for (int s = 0; s < n; s++) {
             size_t c = (size_t)seg[s].cell * g->L + l;
-            double ds = seg[s].ds, x = (double)g->chi[c] * ds;
+            double ds = seg[s].ds * g->path_scale, x = (double)g->chi[c] * ds;
             Il += Tl * (double)g->eta[c] * ds * f_emis(x);
             Tl *= exp(-x);
         }
@@ -151,7 +158,7 @@ static void integrate_btf(const grid_t *g, const seg_t *seg, int n, double *I, d
         double Il = 0.0, tau = 0.0;
         for (int s = n - 1; s >= 0; s--) {
             size_t c = (size_t)seg[s].cell * g->L + l;
-            double ds = seg[s].ds, chi = g->chi[c], eta = g->eta[c], x = chi * ds;
+            double ds = seg[s].ds * g->path_scale, chi = g->chi[c], eta = g->eta[c], x = chi * ds;
             tau += x;
             Il = Il * exp(-x) + (chi > 0.0 ? (eta / chi) * (-expm1(-x)) : eta * ds);
         }
@@ -193,7 +200,7 @@ int rc_oracle_ray_segments(int nx, int ny, double px, double py, double theta, i
 int rc_oracle_interval(const float *chi, const float *eta, int nx, int ny, int L, double px,
                        double py, double theta, int diag_q, double ta, double tb, int order,
                        double *I, double *T) {
-    grid_t g = {nx, ny, L, chi, eta};
+    grid_t g = {nx, ny, L, chi, eta, 1.0};
     seg_t *seg = (seg_t *)malloc(sizeof(seg_t) * (size_t)(nx + ny + 4));
     int n = diag_q >= 0 ? diag_segments(nx, ny, (int)floor(px), (int)floor(py), diag_q, ta, tb, seg)
                         : dda_segments(nx, ny, px, py, cos(theta), sin(theta), ta, tb, seg);
@@ -228,17 +235,17 @@ typedef struct {
  *   order: 0 front-to-back, 1 back-to-front (G13).
  * Returns 0, or -1 on bad arguments / -2 out of memory.
  */
-int rc_oracle_solve(const float *chi, const float *eta, int nx, int ny, int L, int ncasc,
-                    double c0, const float *I_below, const float *I_above, const float *w,
-                    int x0, int x1, int y0, int y1, double *J_out, double *Jbar_out, int nthreads,
-                    int order, int dump_cascade, double *dump_I, double *dump_T, double *dump_M,
-                    int *dump_win, rc_oracle_counts *counts) {
+int rc_oracle_solve_scaled(const float *chi, const float *eta, int nx, int ny, int L, int ncasc,
+                           double c0, const float *I_below, const float *I_above, const float *w,
+                           int x0, int x1, int y0, int y1, double *J_out, double *Jbar_out, int nthreads,
+                           int order, int dump_cascade, double *dump_I, double *dump_T, double *dump_M,
+                           int *dump_win, rc_oracle_counts *counts, double path_scale) {
     if (!chi || !eta || !J_out || nx <= 0 || ny <= 0 || L <= 0 || ncasc < 1 || ncasc > 15)
         return -1;
     int top = ncasc - 1;
     if (nx % (1 << top) || ny % (1 << top)) return -1; /* reading G19 */
     if (x0 < 0 || y0 < 0 || x1 > nx || y1 > ny || x0 >= x1 || y0 >= y1) return -1;
-    grid_t g = {nx, ny, L, chi, eta};
+    grid_t g = {nx, ny, L, chi, eta, path_scale};
     if (counts) memset(counts, 0, sizeof(*counts));
 #ifdef _OPENMP
     if (nthreads > 0) omp_set_num_threads(nthreads);
@@ -337,6 +344,17 @@ int rc_oracle_solve(const float *chi, const float *eta, int nx, int ny, int L, i
     }
     free(Mup);
     return status;
+}
+
+/* Flatland (path_scale = 1): the solve of SURVEY.md §8(c). */
+int rc_oracle_solve(const float *chi, const float *eta, int nx, int ny, int L, int ncasc,
+                    double c0, const float *I_below, const float *I_above, const float *w,
+                    int x0, int x1, int y0, int y1, double *J_out, double *Jbar_out, int nthreads,
+                    int order, int dump_cascade, double *dump_I, double *dump_T, double *dump_M,
+                    int *dump_win, rc_oracle_counts *counts) {
+    return rc_oracle_solve_scaled(chi, eta, nx, ny, L, ncasc, c0, I_below, I_above, w, x0, x1, y0, y1, J_out,
+                                  Jbar_out, nthreads, order, dump_cascade, dump_I, dump_T, dump_M, dump_win,
+                                  counts, 1.0);
 }
 
 int rc_oracle_num_threads(void) {

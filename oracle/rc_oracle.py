@@ -51,6 +51,8 @@ def lib():
                                          [C.c_int] * 4 + [C.c_void_p, C.c_void_p, C.c_int, C.c_int,
                                                           C.c_int, C.c_void_p, C.c_void_p, C.c_void_p,
                                                           C.c_void_p, C.c_void_p])
+        _lib.rc_oracle_solve_scaled.restype = C.c_int
+        _lib.rc_oracle_solve_scaled.argtypes = _lib.rc_oracle_solve.argtypes + [C.c_double]
         _lib.rc_oracle_num_threads.restype = C.c_int
     return _lib
 
@@ -92,7 +94,7 @@ def merge(I_near, tau_near, I_far, tau_far):
 
 
 def solve(chi, eta, ncascades, c0=1.0, I_below=None, I_above=None, weights=None, window=None,
-          nthreads=0, order=0, dump_cascade=-1, want_counts=False):
+          nthreads=0, order=0, dump_cascade=-1, want_counts=False, path_scale=1.0):
     """J [wy][wx][L] (float64) for the cascade-0 cell window (x0, x1, y0, y1) (default: whole grid).
 
     Returns a dict: J, Jbar, and if asked counts / dump_{I,T,M,win} of one cascade."""
@@ -115,9 +117,10 @@ def solve(chi, eta, ncascades, c0=1.0, I_below=None, I_above=None, weights=None,
         shape = (ny // s, nx // s, N, L)
         dI, dT, dM = np.zeros(shape), np.zeros(shape), np.zeros(shape)
         assert window is None, "dump only with the full window (dense layout)"
-    rc = lib().rc_oracle_solve(_ptr(chi), _ptr(eta), nx, ny, L, ncascades, c0, _ptr(Ib), _ptr(Ia),
-                               _ptr(w), x0, x1, y0, y1, _ptr(J), _ptr(Jbar), nthreads, order,
-                               dump_cascade, _ptr(dI), _ptr(dT), _ptr(dM), _ptr(win), C.byref(cnt))
+    rc = lib().rc_oracle_solve_scaled(_ptr(chi), _ptr(eta), nx, ny, L, ncascades, c0, _ptr(Ib), _ptr(Ia),
+                                      _ptr(w), x0, x1, y0, y1, _ptr(J), _ptr(Jbar), nthreads, order,
+                                      dump_cascade, _ptr(dI), _ptr(dT), _ptr(dM), _ptr(win), C.byref(cnt),
+                                      float(path_scale))
     if rc != 0:
         raise ValueError(f"rc_oracle_solve failed: {rc}")
     out = {"J": J, "Jbar": Jbar}
@@ -129,7 +132,34 @@ def solve(chi, eta, ncascades, c0=1.0, I_below=None, I_above=None, weights=None,
     return out
 
 
+def solve_inclined(chi, eta, ncascades, mu, w_mu, **kw):
+    """2.5D solve: the model is homogeneous along the axis perpendicular
+    to the grid; every flatland ray is replaced by len(mu) rays with the same projection and direction
+    cosine mu[m] to that axis.  Such a ray crosses the same cells with path lengths ds / sqrt(1 - mu^2), so
+    each inclination is the flatland solve with that path scale, and J = sum_m w_mu[m] J_m (the quadrature
+    over one hemisphere, weights summing to 1; the other hemisphere is its mirror image).  Written out as
+    exactly that: one plain solve per inclination, summed in order."""
+    mu = np.asarray(mu, np.float64)
+    w_mu = np.asarray(w_mu, np.float64)
+    assert mu.shape == w_mu.shape and mu.ndim == 1 and np.all(mu >= 0.0) and np.all(mu < 1.0)
+    out = None
+    for m in range(len(mu)):
+        o = solve(chi, eta, ncascades, path_scale=1.0 / np.sqrt(1.0 - mu[m] * mu[m]), **kw)
+        if out is None:
+            out = {"J": w_mu[m] * o["J"], "Jbar": w_mu[m] * o["Jbar"]}
+            for key in ("intervals", "segments"):
+                if key in o:
+                    out[key] = o[key]
+        else:
+            out["J"] += w_mu[m] * o["J"]
+            out["Jbar"] += w_mu[m] * o["Jbar"]
+    return out
+
+
 def solve_atmosphere(atm, **kw):
     """Convenience: oracle solve of a paper_2408_14425_b200.atmospheres.Atmosphere-like object."""
+    if getattr(atm, "mu", None) is not None:
+        return solve_inclined(atm.chi, atm.eta, atm.ncascades, atm.mu, atm.w_mu, c0=atm.c0_interval,
+                              I_below=atm.I_below, I_above=atm.I_above, weights=atm.weights, **kw)
     return solve(atm.chi, atm.eta, atm.ncascades, c0=atm.c0_interval, I_below=atm.I_below,
                  I_above=atm.I_above, weights=atm.weights, **kw)

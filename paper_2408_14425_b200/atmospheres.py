@@ -37,6 +37,10 @@ class Atmosphere:
     accumulate: bool = False  # config 4: the checked output is Jbar = sum_l w_l J_l
     c0_interval: float = 1.0
     meta: dict = field(default_factory=dict)
+    # 2.5D: direction cosines to the invariant axis and quadrature weights (sum 1) of the
+    # inclined rays that replace every flatland ray; None = flatland
+    mu: np.ndarray | None = None
+    w_mu: np.ndarray | None = None
 
 
 # (nx, ny, nlambda, ncascades) of BASELINE.json's configs
@@ -230,6 +234,33 @@ def config4(nx=None, ny=None, nlambda=None, ncascades=None, seed=1004) -> Atmosp
 
 
 CONFIGS = {0: config0, 1: config1, 2: config2, 3: config3, 4: config4}
+
+
+def gauss_radau(n: int):
+    """n-point Gauss-Radau rule on mu in [0, 1] with the fixed node at mu = 0 (the in-plane ray), weights
+    summing to 1 - the inclination quadrature of PAPER.md:281 ("a Gauss-Radau quadrature with eight rays for
+    inclination", integrating one hemisphere).  The paper does not say which end is fixed; mu = 1 would be a
+    ray along the invariant axis with an infinite path (reading G20).  Textbook rule: on [-1, 1]
+    the free nodes are the roots of (P_{n-1} + P_n)/(1 + x), w_1 = 2/n^2, w_i = (1 - x_i)/(n P_{n-1}(x_i))^2.
+    Inputs only: the method's arithmetic never sees how mu, w were made."""
+    from numpy.polynomial import legendre as Lg
+    if n == 1:
+        return np.zeros(1), np.ones(1)
+    c = np.zeros(n + 1)
+    c[n - 1] = c[n] = 1.0
+    x = np.sort(np.real(Lg.legroots(c)))
+    x[0] = -1.0
+    pnm1 = Lg.legval(x, np.eye(n)[n - 1])
+    w = (1.0 - x) / (n * pnm1) ** 2
+    w[0] = 2.0 / n ** 2
+    return (x + 1.0) / 2.0, w / 2.0
+
+
+def with_inclinations(atm: Atmosphere, n: int) -> Atmosphere:
+    """The same atmosphere solved in 2.5D with an n-point Gauss-Radau inclination quadrature."""
+    import dataclasses
+    mu, w = gauss_radau(n)
+    return dataclasses.replace(atm, name=f"{atm.name}_incl{n}", mu=mu, w_mu=w)
 
 
 def make_config(idx: int, **kw) -> Atmosphere:

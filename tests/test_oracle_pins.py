@@ -356,3 +356,75 @@ def test_P12_opaque_disc_falloff(oracle):
     assert err.min() > -0.02, err.min()      # 'always lies above the theoretically predicted solution'
     assert 0.02 < err.mean() < 0.20, err.mean()
     assert err.max() < 0.45, err.max()
+
+
+# ----------------------------------------------------------------------------- 2.5D inclinations (f2)
+def test_gauss_radau_rule_is_exact_for_polynomials():
+    """The inclination quadrature handed to both sides (Gauss-Radau, 8 rays, one hemisphere):
+    n nodes with one fixed at mu = 0 integrate mu^p over [0, 1] exactly for p <= 2n - 2; weights sum to 1."""
+    for n in (1, 2, 3, 4, 8):
+        mu, w = A.gauss_radau(n)
+        assert mu[0] == 0.0 and np.all(np.diff(mu) > 0) and mu[-1] < 1.0 and np.all(w > 0)
+        for p in range(2 * n - 1):
+            assert abs(np.sum(w * mu ** p) - 1.0 / (p + 1)) < 1e-12
+    assert abs(np.sum(A.gauss_radau(8)[1] * A.gauss_radau(8)[0] ** 15) - 1.0 / 16) > 1e-9  # and not beyond
+
+
+def test_I1_inclined_uniform_slab_closed_form(oracle):
+    """ncasc = 1, uniform chi and S, isotropic boundary B, inclined rays: the ray with direction cosine mu
+    to the invariant axis has path length l / sqrt(1 - mu^2) for projected length l, so
+    J = S - (S - B) sum_m w_m 1/4 sum_k exp(-chi sqrt2 min(dx_k, dy_k) / sqrt(1 - mu_m^2))."""
+    nx, ny, chi0, S0, B = 24, 16, 0.11, 1.5, 0.25
+    chi = np.full((ny, nx, 1), chi0, np.float32)
+    eta = np.full((ny, nx, 1), np.float32(chi0) * np.float32(S0), np.float32)
+    c = float(chi[0, 0, 0])
+    S = float(eta[0, 0, 0]) / c
+    mu, w = A.gauss_radau(4)
+    J = oracle.solve_inclined(chi, eta, 1, mu, w, I_below=[B], I_above=[B])["J"][..., 0]
+    y, x = np.mgrid[0:ny, 0:nx]
+    dxp, dxm, dyp, dym = nx - (x + 0.5), x + 0.5, ny - (y + 0.5), y + 0.5
+    att = 0.0
+    for m in range(4):
+        f = 1.0 / np.sqrt(1.0 - mu[m] ** 2)
+        att = att + w[m] * sum(np.exp(-c * f * R2 * np.minimum(dx, dy))
+                               for dx, dy in ((dxp, dyp), (dxm, dyp), (dxm, dym), (dxp, dym))) / 4
+    assert np.allclose(J, S - (S - B) * att, rtol=1e-13)
+
+
+def test_I2_inclined_invariants(oracle):
+    """(a) one in-plane ray (mu = 0, w = 1) is the flatland solve, bit for bit; (b) constant S with boundary
+    S gives J = S for any inclination set; (c) an empty domain passes the boundary through: J = B sum w;
+    (d) a path scale f is the flatland solve of the atmosphere (f chi, f eta) when f is a power of two
+    (the scaled inputs are then exact in fp32)."""
+    a = A.make_config(0, nx=32, ny=32, nlambda=2, ncascades=4, seed=21)
+    flat = oracle.solve(a.chi, a.eta, 4, I_below=[0.3, 0.1], I_above=[0.0, 0.2])["J"]
+    one = oracle.solve_inclined(a.chi, a.eta, 4, [0.0], [1.0], I_below=[0.3, 0.1], I_above=[0.0, 0.2])["J"]
+    assert np.array_equal(flat, one)
+    mu, w = A.gauss_radau(8)
+    S0 = 0.75
+    eta = (a.chi * np.float32(S0)).astype(np.float32)
+    ok = eta.astype(np.float64) == a.chi.astype(np.float64) * S0   # 0.75 chi is exact unless it rounds
+    chi = np.where(ok, a.chi, 0).astype(np.float32)
+    eta = np.where(ok, eta, 0).astype(np.float32)
+    J = oracle.solve_inclined(chi, eta, 4, mu, w, I_below=[S0, S0], I_above=[S0, S0])["J"]
+    assert np.allclose(J, S0, rtol=1e-13)
+    z = np.zeros_like(a.chi)
+    J = oracle.solve_inclined(z, z, 4, mu, w, I_below=[0.5, 1.0], I_above=[0.0, 1.0])["J"]
+    assert np.allclose(J[..., 0], 0.25, rtol=1e-14) and np.allclose(J[..., 1], 1.0, rtol=1e-14)
+    scaled = oracle.solve(a.chi, a.eta, 4, path_scale=4.0)["J"]
+    direct = oracle.solve((4 * a.chi).astype(np.float32), (4 * a.eta).astype(np.float32), 4)["J"]
+    assert np.allclose(scaled, direct, rtol=1e-13)
+
+
+def test_I3_inclined_rays_see_more_optical_depth(oracle):
+    """Sanity of the sign of the effect: an absorbing, non-emitting slab lit from below transmits less along
+    inclined rays (longer paths), so J with the 8-ray quadrature lies strictly below the in-plane J and
+    above the J of the most inclined ray alone."""
+    a = A.make_config(0, nx=32, ny=32, ncascades=4, seed=3)
+    z = np.zeros_like(a.eta)
+    mu, w = A.gauss_radau(8)
+    flat = oracle.solve(a.chi, z, 4, I_below=[1.0])["J"]
+    incl = oracle.solve_inclined(a.chi, z, 4, mu, w, I_below=[1.0])["J"]
+    steep = oracle.solve_inclined(a.chi, z, 4, mu[-1:], [1.0], I_below=[1.0])["J"]
+    m = flat > 1e-6
+    assert np.all(incl[m] < flat[m]) and np.all(steep[m] < incl[m])
