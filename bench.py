@@ -99,7 +99,7 @@ def oracle_sample(atm, nwin, size=8, seed=0):
         t = time.perf_counter()
         out = rc_oracle.solve_atmosphere(atm, window=(x0, x0 + size, y0, y0 + size), want_counts=True)
         secs += time.perf_counter() - t
-        segl += int(out["segments"].sum()) * atm.nlambda
+        segl += int(out["segments"].sum()) * atm.nlambda * (1 if atm.mu is None else len(atm.mu))
     return segl, secs, rc_oracle.num_threads()
 
 
@@ -129,6 +129,9 @@ def main():
     ap.add_argument("--config", type=int, default=2)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--lambda-batch", type=int, default=0)
+    ap.add_argument("--inclinations", type=int, default=1,
+                    help="2.5D: N Gauss-Radau inclined rays per flatland ray (SURVEY §8(f) f2); the unit count "
+                         "becomes segment-wavelength-inclinations")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=3)
     args = ap.parse_args()
@@ -141,6 +144,9 @@ def main():
     workload = (f"BASELINE.json configs[{args.config}]: {fx}x{fy} cells, {fl} wavelengths, {fc} cascades, "
                 f"seeded synthetic atmosphere (DESIGN.md §4)")
     atm = atmospheres.make_config(args.config, seed=1000 + args.config + 17 * rank)
+    if args.inclinations > 1:
+        atm = atmospheres.with_inclinations(atm, args.inclinations)
+        workload += f", 2.5D with {args.inclinations} Gauss-Radau inclinations per ray (value counts segment-wavelength-inclinations)"
     if args.impl == "reference":
         run_reference(args, atm, workload)
         return
@@ -157,6 +163,8 @@ def main():
 
     flags = binding.RC_ACCUM_J if atm.accumulate else 0
     rc = binding.RadianceCascades(atm.ncascades, atm.c0_interval, local_rank, args.lambda_batch, flags)
+    if atm.mu is not None:
+        rc.set_inclinations(atm.mu, atm.w_mu)
     rc.ensure_workspace(atm.nx, atm.ny, atm.nlambda, host_io=True)
     chi_h = torch.from_numpy(atm.chi).pin_memory()
     eta_h = torch.from_numpy(atm.eta).pin_memory()
@@ -167,7 +175,8 @@ def main():
     seg = rc.count_segments()
     l2_gather_gbs = rc.probe_gather_bandwidth(64)      # L2 -> SM ceiling of the gather pattern (64 MB region)
     hbm_gather_gbs = rc.probe_gather_bandwidth(1024) if rc._ws.numel() > (1100 << 20) else None
-    segl_per_step = sum(seg) * atm.nlambda
+    nincl = 1 if atm.mu is None else len(atm.mu)
+    segl_per_step = sum(seg) * atm.nlambda * nincl
     J = rc.solve_J()
     for _ in range(args.warmup - 1):
         rc.solve_J(out=J)
@@ -220,11 +229,11 @@ def main():
         # dominant kernel: the march+merge launch of the heaviest cascade
         ms_march = [st.ms_march[i] for i in range(atm.ncascades)]
         dom = int(np.argmax(ms_march))
-        casc_bytes = 2 * 4 * atm.nx * atm.ny * atm.nlambda  # read merged cascade i+1, write cascade i
+        casc_bytes = 2 * 4 * atm.nx * atm.ny * atm.nlambda * nincl  # read merged cascade i+1, write cascade i
         alg_bytes = 8 * seg[dom] * atm.nlambda + casc_bytes  # chi+eta gather: 8 B per segment-wavelength
         ach = alg_bytes / (ms_march[dom] * 1e-3) / 1e9
         sfu_peak = SM_COUNT * MUFU_PER_CLK_SM * sm_max_mhz * 1e6
-        ach_alu = seg[dom] * atm.nlambda / (ms_march[dom] * 1e-3)
+        ach_alu = seg[dom] * atm.nlambda * nincl / (ms_march[dom] * 1e-3)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",

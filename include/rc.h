@@ -110,6 +110,16 @@ int rc_set_atmosphere(rc_ctx *ctx, const float *chi, const float *eta, int nx, i
  * PAPER.md:371).  Call after rc_set_atmosphere. */
 int rc_set_boundary(rc_ctx *ctx, const float *I_below, const float *I_above);
 
+/* 2.5D inclination quadrature: the model is taken homogeneous along
+ * the axis perpendicular to the grid, and every flatland ray is replaced by n rays with the same
+ * projection and direction cosine mu[m] to that axis (0 <= mu < 1): the same cells, path lengths
+ * ds / sqrt(1 - mu^2).  J_l = sum_m w[m] * (mean over the 4 merged cascade-0 directions of inclination m);
+ * the weights should sum to 1 (one hemisphere; the other is its mirror image).  The boundary intensities
+ * of rc_set_boundary apply to every inclination.  n = 1, 2, 4 or 8; mu, w: host, [n]; n = 1 with
+ * mu = w = NULL restores flatland (the default).  Call BEFORE rc_workspace_bytes / rc_set_atmosphere:
+ * it changes the workspace size (merged cascades hold n x nlambda channels) and drops the atmosphere. */
+int rc_set_inclinations(rc_ctx *ctx, int n, const float *mu, const float *w);
+
 /* Wavelength weights for RC_ACCUM_J: host, [nlambda]; NULL = all 1.  After rc_set_atmosphere. */
 int rc_set_lambda_weights(rc_ctx *ctx, const float *w);
 

@@ -42,6 +42,7 @@ SYMBOLS = {
     "rc_set_atmosphere": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int]),
     "rc_set_boundary": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
     "rc_set_lambda_weights": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "rc_set_inclinations": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]),
     "rc_solve_J": (C.c_int, [C.c_void_p, C.c_void_p]),
     "rc_solve_J_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p]),
     "rc_set_timing": (C.c_int, [C.c_void_p, C.c_int]),
@@ -158,6 +159,19 @@ class RadianceCascades:
         a, pa = _host_f32(w, self.shape[2])
         self._check(self.lib.rc_set_lambda_weights(self.handle, pa))
 
+    def set_inclinations(self, mu=None, w=None):
+        """2.5D inclination quadrature (before set_atmosphere); mu = None restores flatland."""
+        import numpy as np
+        if mu is None:
+            self._check(self.lib.rc_set_inclinations(self.handle, 1, None, None))
+        else:
+            m = np.ascontiguousarray(mu, dtype=np.float32)
+            ww = np.ascontiguousarray(w, dtype=np.float32)
+            assert m.shape == ww.shape and m.ndim == 1
+            self._check(self.lib.rc_set_inclinations(self.handle, int(m.size), m.ctypes.data_as(C.c_void_p),
+                                                     ww.ctypes.data_as(C.c_void_p)))
+        self._ws = None  # the workspace size depends on the number of inclinations
+
     def solve_J(self, out=None):
         """Enqueue one solve on torch's current stream; returns the output tensor (not synchronised)."""
         import torch
@@ -225,6 +239,8 @@ def solve_atmosphere(atm, device=0, lambda_batch=0, flags=0, rc=None):
         rc = RadianceCascades(atm.ncascades, atm.c0_interval, device, lambda_batch, fl)
     chi = torch.from_numpy(atm.chi).to(dev)
     eta = torch.from_numpy(atm.eta).to(dev)
+    if getattr(atm, "mu", None) is not None:
+        rc.set_inclinations(atm.mu, atm.w_mu)
     rc.set_atmosphere(chi, eta)
     rc.set_boundary(atm.I_below, atm.I_above)
     rc.set_lambda_weights(atm.weights)

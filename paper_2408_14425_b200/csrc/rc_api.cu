@@ -29,7 +29,8 @@ struct CascadePlan {
 
 struct Plan {
     int nx = 0, ny = 0, L = 0, ncasc = 0;
-    int LV = 1, nb = 1, Lpad = 1;
+    int LV = 1, nb = 1, Lpad = 1;   // wavelengths per lane, batches, nb * LV
+    int NM = 1;                     // inclinations (2.5D); a lane carries LV * NM channels
     int nbands = 1, band_axis = 0;  // L2 banding of the long-ray cascades (1 = off); axis 0 = rows, 1 = columns
     size_t state = 0;               // parked ray state of the banded launches
     CascadePlan c[RC_MAX_CASCADES];
@@ -53,6 +54,9 @@ struct rc_ctx {
     // developer overrides (environment, read by rc_create): RC_MARCH_VARIANT = 0..3 (register ring depth /
     // occupancy of march_kernel), RC_PATCH_LOG2 = 2..5 forces the lane patch width for cascades >= RC_PATCH_FROM
     int tune_variant = 2, tune_patch = -1, tune_patch_from = 0;
+    // 2.5D inclination quadrature (rc_set_inclinations); nm = 1, f = w = 1: flatland
+    int nm = 1;
+    float incl_f[8] = {1, 1, 1, 1, 1, 1, 1, 1}, incl_w[8] = {1, 0, 0, 0, 0, 0, 0, 0};
     std::vector<std::vector<long long>> off_host;  // kept alive for the async uploads
     std::vector<float> stage;                      // host staging for boundary / weights
     // timing: `nsets` rings of (2 per cascade + 2) events; solve number n records into set n % nsets
@@ -137,21 +141,25 @@ int choose_patch(int nx, int ny, int i, double ta, double tb) {
     return widest;
 }
 
-int choose_lv(const rc_config &cfg, int L) {
-    if (cfg.lambda_batch == 1 || cfg.lambda_batch == 2 || cfg.lambda_batch == 4 || cfg.lambda_batch == 8)
+// Wavelengths per lane: a lane carries LV * nm <= 8 channels (registers).
+int choose_lv(const rc_config &cfg, int L, int nm) {
+    const int cap = 8 / nm;
+    if ((cfg.lambda_batch == 1 || cfg.lambda_batch == 2 || cfg.lambda_batch == 4 || cfg.lambda_batch == 8) &&
+        cfg.lambda_batch <= cap)
         return cfg.lambda_batch;
     int lv = 1;
-    while (lv < L && lv < 8) lv <<= 1;
+    while (lv < L && lv < cap) lv <<= 1;
     return lv;
 }
 
 // Workspace layout for a shape.  When `offs` is given, also fills the per-direction slot offsets.
-bool make_plan(const rc_config &cfg, int nx, int ny, int L, bool host_io, Plan &P,
+bool make_plan(const rc_config &cfg, int nm, int nx, int ny, int L, bool host_io, Plan &P,
                std::vector<std::vector<long long>> *offs) {
     if (!shape_ok(cfg, nx, ny, L)) return false;
     P = Plan{};
     P.nx = nx; P.ny = ny; P.L = L; P.ncasc = cfg.ncascades;
-    P.LV = choose_lv(cfg, L);
+    P.NM = nm;
+    P.LV = choose_lv(cfg, L, nm);
     P.nb = (L + P.LV - 1) / P.LV;
     P.Lpad = P.nb * P.LV;
     const size_t ncell = (size_t)nx * ny;
@@ -219,12 +227,12 @@ bool make_plan(const rc_config &cfg, int nx, int ny, int L, bool host_io, Plan &
             c.banded = P.nbands > 1 && !c.empty && std::fmin(c.tb, diag) > 100.0 && (4 * patch_ext <= ext || std::getenv("RC_BANDS"));
             any = any || c.banded;
         }
-        if (any) { P.state = cur; cur += 8 * field; }
+        if (any) { P.state = cur; cur += 8 * field * P.NM; }
     }
     P.chiT = cur; cur += field;
     P.ST = cur;   cur += field;
-    P.A[0] = cur; cur += field;
-    P.A[1] = cur; cur += field;
+    P.A[0] = cur; cur += field * P.NM;  // merged cascades hold every (wavelength, inclination) channel
+    P.A[1] = cur; cur += field * P.NM;
     if (cfg.flags & RC_ACCUM_J) { P.Jpart = cur; cur += align_up(ncell * P.nb * sizeof(float)); }
     P.bc_below = cur; cur += align_up(P.Lpad * sizeof(float));
     P.bc_above = cur; cur += align_up(P.Lpad * sizeof(float));
@@ -291,7 +299,7 @@ int rc_destroy(rc_ctx *ctx) {
 size_t rc_workspace_bytes(const rc_ctx *ctx, int nx, int ny, int nlambda, int host_io) {
     if (!ctx) return 0;
     Plan P;
-    if (!make_plan(ctx->cfg, nx, ny, nlambda, host_io != 0, P, nullptr)) return 0;
+    if (!make_plan(ctx->cfg, ctx->nm, nx, ny, nlambda, host_io != 0, P, nullptr)) return 0;
     return P.total;
 }
 
@@ -337,10 +345,10 @@ int rc_set_atmosphere(rc_ctx *ctx, const float *chi, const float *eta, int nx, i
     if (!same_shape) {
         Plan P, Pio;
         std::vector<std::vector<long long>> offs;
-        make_plan(ctx->cfg, nx, ny, nlambda, false, P, &offs);
+        make_plan(ctx->cfg, ctx->nm, nx, ny, nlambda, false, P, &offs);
         if (P.total > ctx->ws_bytes)
             return fail(ctx, RC_ERR_NO_WORKSPACE, "workspace has %zu bytes, %zu needed", ctx->ws_bytes, P.total);
-        make_plan(ctx->cfg, nx, ny, nlambda, true, Pio, nullptr);
+        make_plan(ctx->cfg, ctx->nm, nx, ny, nlambda, true, Pio, nullptr);
         ctx->host_io = Pio.total <= ctx->ws_bytes;
         ctx->plan = ctx->host_io ? Pio : P;
         ctx->have_atm = false;
@@ -408,6 +416,25 @@ int rc_set_boundary(rc_ctx *ctx, const float *I_below, const float *I_above) {
     return upload_lambda_array(ctx, I_above, ctx->plan.bc_above, 0.f);
 }
 
+// 2.5D: every flatland ray becomes n rays with the same projection and direction cosine mu[m] to the
+// invariant axis; changes the workspace plan, so the atmosphere must be set again.
+int rc_set_inclinations(rc_ctx *ctx, int n, const float *mu, const float *w) {
+    if (!ctx) return RC_ERR_NULL_ARG;
+    if (n != 1 && n != 2 && n != 4 && n != 8) return fail(ctx, RC_ERR_BAD_VALUE, "n = %d inclinations: must be 1, 2, 4 or 8", n);
+    if ((!mu || !w) && n != 1) return fail(ctx, RC_ERR_NULL_ARG, "null mu / w");
+    for (int m = 0; m < n && mu && w; m++)
+        if (!(mu[m] >= 0.f) || !(mu[m] < 1.f) || !(w[m] >= 0.f) || !std::isfinite(w[m]))
+            return fail(ctx, RC_ERR_BAD_VALUE, "inclination %d: need 0 <= mu < 1 and a finite weight >= 0", m);
+    ctx->nm = n;
+    for (int m = 0; m < 8; m++) {
+        const bool on = m < n && mu && w;
+        ctx->incl_f[m] = on ? (float)(1.0 / std::sqrt(1.0 - (double)mu[m] * (double)mu[m])) : 1.f;
+        ctx->incl_w[m] = on ? w[m] : (m == 0 ? 1.f : 0.f);
+    }
+    ctx->have_atm = false;  // the plan (channels per lane, cascade storage) depends on n
+    return RC_OK;
+}
+
 int rc_set_lambda_weights(rc_ctx *ctx, const float *w) {
     if (!ctx) return RC_ERR_NULL_ARG;
     return upload_lambda_array(ctx, w, ctx->plan.weights, 1.f);
@@ -443,6 +470,7 @@ static rc::MarchParams march_params(const rc_ctx *ctx, int i, float *J_out) {
     mp.npatch_x = (mp.npx + pw - 1) / pw;
     mp.npatch_y = (mp.npy + ph - 1) / ph;
     mp.kg_n = mp.ngroups; mp.kg_off = 0;
+    for (int m = 0; m < 8; m++) { mp.incl_f[m] = ctx->incl_f[m]; mp.incl_w[m] = ctx->incl_w[m]; }
     mp.state = nullptr;
     mp.band_axis = 0; mp.band_sign = 1; mp.band_lo = 0; mp.band_hi = 0; mp.band_final = 1;
     return mp;
@@ -475,7 +503,7 @@ int rc_solve_J(rc_ctx *ctx, float *J_out) {
         if (ev) RC_CUDA(ctx, cudaEventRecord(ev[1 + 2 * (top - i)], ctx->stream));
         rc::MarchParams mp = march_params(ctx, i, J_out);
         if (!c.banded) {
-            RC_CUDA(ctx, rc::launch_march(mp, P.LV, ctx->tune_variant, ctx->stream));
+            RC_CUDA(ctx, rc::launch_march(mp, P.LV * P.NM, P.NM, ctx->tune_variant, ctx->stream));
             launches++;
         } else {
             // rays heading up (right) cross the bands in ascending order, the others in descending order;
@@ -493,7 +521,7 @@ int rc_solve_J(rc_ctx *ctx, float *J_out) {
                     mp.band_lo = beta * ext;
                     mp.band_hi = std::min(n_axis, (beta + 1) * ext);
                     mp.band_final = bi == P.nbands - 1;
-                    RC_CUDA(ctx, rc::launch_march(mp, P.LV, ctx->tune_variant, ctx->stream));
+                    RC_CUDA(ctx, rc::launch_march(mp, P.LV * P.NM, P.NM, ctx->tune_variant, ctx->stream));
                     launches++;
                 }
             }
@@ -535,7 +563,7 @@ int rc_solve_J_host(rc_ctx *ctx, const float *chi_host, const float *eta_host, i
     if (!ctx->ws) return fail(ctx, RC_ERR_NO_WORKSPACE, "rc_set_workspace has not been called");
     RC_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
     Plan Pio;
-    make_plan(ctx->cfg, nx, ny, nlambda, true, Pio, nullptr);
+    make_plan(ctx->cfg, ctx->nm, nx, ny, nlambda, true, Pio, nullptr);
     if (Pio.total > ctx->ws_bytes)
         return fail(ctx, RC_ERR_NO_WORKSPACE, "workspace has %zu bytes, %zu needed with host_io", ctx->ws_bytes, Pio.total);
     const size_t n = (size_t)nx * ny * nlambda * sizeof(float);

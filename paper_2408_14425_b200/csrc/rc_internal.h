@@ -54,6 +54,8 @@ struct MarchParams {
     // (0 = rows, 1 = columns), for rays travelling in direction band_sign along that axis
     float *state;          // parked rays: [nb][ngroups][4][npy][npx][2][LV]  (I, tau*log2 e)
     int band_axis, band_sign, band_lo, band_hi, band_final;
+    // 2.5D inclination quadrature: path scale 1/sqrt(1 - mu_m^2) and weight of inclination m
+    float incl_f[8], incl_w[8];
 };
 
 struct PackParams {
@@ -75,7 +77,7 @@ struct TableBuildParams {
 
 // launchers (rc_kernels.cu); LV in {1,2,4,8}
 cudaError_t launch_pack(const PackParams &p, int LV, cudaStream_t st);
-cudaError_t launch_march(const MarchParams &p, int LV, int variant, cudaStream_t st);
+cudaError_t launch_march(const MarchParams &p, int LV, int NM, int variant, cudaStream_t st);
 cudaError_t launch_table_build(const TableBuildParams &p, cudaStream_t st);
 cudaError_t launch_reduce_jbar(const float *Jpart, float *Jbar, long long ncell, int nb, cudaStream_t st);
 cudaError_t launch_count(const MarchParams &p, unsigned long long *total, cudaStream_t st);

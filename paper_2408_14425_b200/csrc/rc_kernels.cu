@@ -347,10 +347,11 @@ __device__ __forceinline__ int first_step_reaching(const StepXY *xy, int n, int 
 // half of the directions that crosses the bands in ascending (or descending) order; a ray's (I, tau)
 // is carried from band to band through `state`, so the arithmetic - and the result - is that of the
 // unbanded launch, bit for bit, while the cells gathered by one launch fit L2.
-template <int LV, int PD, int WARPS, int MINB, bool BANDED>
+template <int LV, int NM, int PD, int WARPS, int MINB, bool BANDED>
 __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) {
     // sum over the 4 child directions, per thread: parked in shared memory between children so the
     // marching loop has the registers to itself
+    constexpr int LL = LV / NM;  // wavelengths per lane; channel ch = l * NM + m (inclination fastest)
     __shared__ float acc_s[LV][WARPS * 32];
     const int lane = threadIdx.x & 31;
     const long long W = (long long)blockIdx.x * WARPS + (threadIdx.x >> 5);
@@ -364,8 +365,8 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
     const long long ncell = (long long)p.nx * p.ny;
     // packed layout [batch][y mod s][x mod s][y div s][x div s][LV]: the lane's probe owns cell
     // (y div s, x div s) = (b, a) of every phase plane; a step's delta is lane-independent
-    const float *chiB = p.chiT + (long long)nbI * ncell * LV;  // warp-uniform
-    const float *SB = p.ST + (long long)nbI * ncell * LV;
+    const float *chiB = p.chiT + (long long)nbI * ncell * LL;  // warp-uniform
+    const float *SB = p.ST + (long long)nbI * ncell * LL;
     // (dx, dy) ranges that keep this lane's ray inside the box
     const int dxlo = -(a << p.shift) - half, dxhi = ((p.npx - a) << p.shift) - 1 - half;
     const int dylo = -Y0, dyhi = p.ny - 1 - Y0;
@@ -407,17 +408,17 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
                 n0 = has ? n0 - w0 : 0;
             }
             const int nw = __reduce_max_sync(FULL, nin);  // steps this warp walks
-            float c2[PD][LV], S[PD][LV], ds[PD];
+            float c2[PD][LL], S[PD][LL], ds[PD];
             // prologue: steps 0 .. PD-1 into the ring (the table has 2 PD spare entries at its end)
 #pragma unroll
             for (int u = 0; u < PD; u++) {
 #pragma unroll
-                for (int v = 0; v < LV; v++) { c2[u][v] = 0.f; S[u][v] = 0.f; }
+                for (int v = 0; v < LL; v++) { c2[u][v] = 0.f; S[u][v] = 0.f; }
                 const uint2 e = __ldg(tab + u);
                 const bool in = u < nin && (!BANDED || u >= n0);
-                const unsigned long long d = (unsigned long long)(probe + e.x) * (LV * sizeof(float));
-                load_vec_if<LV>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(chiB) + d), c2[u], in);
-                load_vec_if<LV>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(SB) + d), S[u], in);
+                const unsigned long long d = (unsigned long long)(probe + e.x) * (LL * sizeof(float));
+                load_vec_if<LL>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(chiB) + d), c2[u], in);
+                load_vec_if<LL>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(SB) + d), S[u], in);
                 ds[u] = in ? __uint_as_float(e.y) : 0.f;
             }
             int chk = 0;
@@ -428,19 +429,22 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
                 for (int u = 0; u < PD; u++) {
                     const uint2 en = __ldg(tab + st + u + PD);
                     // integrate step st + u (a slot past the lane's last in-box step has ds = 0: no effect)
-                    const float dsu = ds[u];
+                    // 2.5D: inclination m crosses the same cell over ds / sin(inclination)
+                    float dsm[NM];
+#pragma unroll
+                    for (int m = 0; m < NM; m++) dsm[m] = NM == 1 ? ds[u] : ds[u] * p.incl_f[m];
 #pragma unroll
                     for (int v = 0; v < LV; v++) {
-                        tau[v] = fmaf(c2[u][v], dsu, tau[v]);
+                        tau[v] = fmaf(c2[u][v / NM], dsm[v % NM], tau[v]);
                         const float Tn = ex2_neg(tau[v]);
-                        I[v] = fmaf(S[u][v], T[v] - Tn, I[v]);
+                        I[v] = fmaf(S[u][v / NM], T[v] - Tn, I[v]);
                         T[v] = Tn;
                     }
                     // refill the slot with step st + u + PD
                     const bool in = st + u + PD < nin && (!BANDED || st + u + PD >= n0);
-                    const unsigned long long d = (unsigned long long)(probe + en.x) * (LV * sizeof(float));
-                    load_vec_if<LV>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(chiB) + d), c2[u], in);
-                    load_vec_if<LV>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(SB) + d), S[u], in);
+                    const unsigned long long d = (unsigned long long)(probe + en.x) * (LL * sizeof(float));
+                    load_vec_if<LL>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(chiB) + d), c2[u], in);
+                    load_vec_if<LL>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(SB) + d), S[u], in);
                     ds[u] = in ? __uint_as_float(en.y) : 0.f;
                 }
                 if (p.early_exit && (++chk & 3) == 0) {
@@ -468,7 +472,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
             // (sin theta_k > 0  <=>  k < N/2) see I_above, rays heading down I_below
             const float *Ib = (2 * k < ndir) ? p.I_above : p.I_below;
 #pragma unroll
-            for (int v = 0; v < LV; v++) I[v] = fmaf(T[v], __ldg(Ib + nbI * LV + v), I[v]);
+            for (int v = 0; v < LV; v++) I[v] = fmaf(T[v], __ldg(Ib + nbI * LL + v / NM), I[v]);
         } else if (valid) {
             // a3: bilinear over the 4 parents of cascade i+1 (already averaged over the 4 children of
             // direction k when they were written), then eq. 11: I <- I + T * U
@@ -503,52 +507,78 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
     for (int v = 0; v < LV; v++) acc[v] = 0.25f * acc_s[v][threadIdx.x];  // mean over the 4 children (cascade 0: a4, J)
     if (p.mode == 0) {
         store_vec<LV>(p.out + (((long long)nbI * p.ngroups + kg) * nprobe + probe) * LV, acc);
-    } else if (p.mode == 1) {
-        float *o = p.out + (long long)probe * p.L + nbI * LV;
-        if ((nbI + 1) * LV <= p.L && (p.L % LV) == 0) {
-            store_vec<LV>(o, acc);
+        return;
+    }
+    // cascade 0: J_l = sum over the inclinations of w_m x (mean of the 4 directions)  (a4)
+    float Jl[LL];
+#pragma unroll
+    for (int l = 0; l < LL; l++) {
+        Jl[l] = NM == 1 ? acc[l] : 0.f;
+        if constexpr (NM > 1) {
+#pragma unroll
+            for (int m = 0; m < NM; m++) Jl[l] = fmaf(p.incl_w[m], acc[l * NM + m], Jl[l]);
+        }
+    }
+    if (p.mode == 1) {
+        float *o = p.out + (long long)probe * p.L + nbI * LL;
+        if ((nbI + 1) * LL <= p.L && (p.L % LL) == 0) {
+            store_vec<LL>(o, Jl);
         } else {
 #pragma unroll
-            for (int v = 0; v < LV; v++)
-                if (nbI * LV + v < p.L) o[v] = acc[v];
+            for (int v = 0; v < LL; v++)
+                if (nbI * LL + v < p.L) o[v] = Jl[v];
         }
     } else {
         float sum = 0.f;
 #pragma unroll
-        for (int v = 0; v < LV; v++) sum = fmaf(__ldg(p.weights + nbI * LV + v), acc[v], sum);
+        for (int v = 0; v < LL; v++) sum = fmaf(__ldg(p.weights + nbI * LL + v), Jl[v], sum);
         p.out[(long long)nbI * nprobe + probe] = sum;
     }
 }
 
-template <int LV, int PD, int WARPS, int MINB>
+template <int LV, int NM, int PD, int WARPS, int MINB>
 static cudaError_t launch_march_variant(const MarchParams &p, cudaStream_t st) {
     const long long blocks = (march_warps(p) + WARPS - 1) / WARPS;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     if (p.state != nullptr)
-        march_kernel<LV, PD, WARPS, MINB, true><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
+        march_kernel<LV, NM, PD, WARPS, MINB, true><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
     else
-        march_kernel<LV, PD, WARPS, MINB, false><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
+        march_kernel<LV, NM, PD, WARPS, MINB, false><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
     return cudaGetLastError();
 }
 
 // variant: 0 = ring of 2 steps, 24 warps/SM (<= 80 registers); 1 = ring of 3, 20 warps/SM (<= 96);
 //          2 = ring of 3, 16 warps/SM (<= 128); 3 = ring of 4, 16 warps/SM (<= 128)
 template <int LV>
-static cudaError_t launch_march_lv(const MarchParams &p, int variant, cudaStream_t st) {
+static cudaError_t launch_march_flat(const MarchParams &p, int variant, cudaStream_t st) {
     switch (variant) {
-        case 0: return launch_march_variant<LV, 2, 8, 3>(p, st);
-        case 1: return launch_march_variant<LV, 3, 5, 4>(p, st);
-        case 3: return launch_march_variant<LV, 4, 8, 2>(p, st);
-        default: return launch_march_variant<LV, 3, 8, 2>(p, st);
+        case 0: return launch_march_variant<LV, 1, 2, 8, 3>(p, st);
+        case 1: return launch_march_variant<LV, 1, 3, 5, 4>(p, st);
+        case 3: return launch_march_variant<LV, 1, 4, 8, 2>(p, st);
+        default: return launch_march_variant<LV, 1, 3, 8, 2>(p, st);
     }
 }
 
-cudaError_t launch_march(const MarchParams &p, int LV, int variant, cudaStream_t st) {
-    switch (LV) {
-        case 8: return launch_march_lv<8>(p, variant, st);
-        case 4: return launch_march_lv<4>(p, variant, st);
-        case 2: return launch_march_lv<2>(p, variant, st);
-        default: return launch_march_lv<1>(p, variant, st);
+// LV = channels per lane = (wavelengths per lane) x NM inclinations; the inclined launches come in one
+// variant only
+cudaError_t launch_march(const MarchParams &p, int LV, int NM, int variant, cudaStream_t st) {
+    if (NM == 1) {
+        switch (LV) {
+            case 8: return launch_march_flat<8>(p, variant, st);
+            case 4: return launch_march_flat<4>(p, variant, st);
+            case 2: return launch_march_flat<2>(p, variant, st);
+            default: return launch_march_flat<1>(p, variant, st);
+        }
+    }
+    // inclined launches are MUFU-bound (NM ex2 per gathered value): ring of 2, 24 warps/SM measured best
+    switch (LV * 16 + NM) {
+        case 8 * 16 + 8: return launch_march_variant<8, 8, 2, 8, 3>(p, st);
+        case 8 * 16 + 4: return launch_march_variant<8, 4, 2, 8, 3>(p, st);
+        case 8 * 16 + 2: return launch_march_variant<8, 2, 2, 8, 3>(p, st);
+        case 4 * 16 + 4: return launch_march_variant<4, 4, 2, 8, 3>(p, st);
+        case 4 * 16 + 2: return launch_march_variant<4, 2, 2, 8, 3>(p, st);
+        case 2 * 16 + 2: return launch_march_variant<2, 2, 2, 8, 3>(p, st);
+        default: return cudaErrorInvalidValue;
     }
 }
 

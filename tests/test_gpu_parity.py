@@ -225,3 +225,36 @@ def test_banded_march_is_bit_identical(monkeypatch, nx, ny, bands):
     monkeypatch.setenv("RC_PATCH_LOG2", "5")
     monkeypatch.setenv("RC_MARCH_VARIANT", "0")
     assert np.array_equal(ref, gpu_solve(atm))
+
+
+# ------------------------------------------------------------------ 2.5D inclination quadrature (f2)
+@pytest.mark.parametrize("idx,kw,n", [
+    (0, dict(nx=64, ny=64, nlambda=1, ncascades=5), 8),
+    (1, dict(nx=128, ny=128, nlambda=5, ncascades=6), 8),
+    (2, dict(nx=128, ny=64, nlambda=6, ncascades=5), 4),
+    (3, dict(nx=128, ny=128, nlambda=3, ncascades=6), 2),
+    (4, dict(nx=256, ny=64, nlambda=9, ncascades=5), 8),
+    (2, dict(nx=64, ny=64, nlambda=2, ncascades=5), 1),
+])
+def test_inclined_rays_match_the_oracle(oracle, idx, kw, n):
+    """each flatland ray replaced by n Gauss-Radau inclinations (same cells, path / sin):
+    J = sum_m w_m J_m against the oracle's one-plain-solve-per-inclination sum; ragged wavelength batches,
+    boundary illumination (config 3), Jbar accumulation (config 4)."""
+    atm = A.with_inclinations(A.make_config(idx, **kw), n)
+    e = check(atm, oracle)
+    print(atm.name, "max rel err", e)
+
+
+def test_inclinations_reset_to_flatland(oracle):
+    from paper_2408_14425_b200 import binding
+    atm = A.make_config(0, nx=32, ny=32, nlambda=2, ncascades=4)
+    flat = gpu_solve(atm)
+    J, rc = binding.solve_atmosphere(A.with_inclinations(atm, 4))
+    rc.set_inclinations(None)
+    J2, _ = binding.solve_atmosphere(atm, rc=rc)
+    assert np.array_equal(J2.cpu().numpy(), flat) and not np.array_equal(J.cpu().numpy(), flat)
+    with pytest.raises(binding.RcError):
+        rc.set_inclinations([0.0, 0.5, 0.7], [0.2, 0.4, 0.4])   # 3 is not 1, 2, 4 or 8
+    with pytest.raises(binding.RcError):
+        rc.set_inclinations([0.0, 1.0], [0.5, 0.5])             # mu = 1: infinite path
+    rc.close()
