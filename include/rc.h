@@ -85,6 +85,7 @@ typedef struct {
     int64_t rays[RC_MAX_CASCADES];        /* intervals per cascade per wavelength = 4 nx ny */
     int64_t table_steps[RC_MAX_CASCADES]; /* step-table entries per cascade (all directions) */
     size_t workspace_bytes;
+    int64_t empty_cells;                  /* cells with chi == 0 at every wavelength (counted by rc_set_atmosphere) */
 } rc_stats;
 
 /* Create a context on cfg->device.  Fails with RC_ERR_NO_DEVICE unless that device is sm_100. */
@@ -102,7 +103,9 @@ int rc_set_stream(rc_ctx *ctx, void *cuda_stream);
 
 /* chi, eta: device, [ny][nx][nlambda] float32, borrowed.  Builds the per-direction step tables for
  * this grid size (device kernels, fp64 geometry) if the shape changed; needs the workspace set.
- * PAPER.md:409. */
+ * Also counts the cells that are empty (chi == 0 at every wavelength) and synchronises the stream: when
+ * more than two thirds are, the march skips the gathers of empty cells (sparsity; the result
+ * is bit-identical).  PAPER.md:409. */
 int rc_set_atmosphere(rc_ctx *ctx, const float *chi, const float *eta, int nx, int ny, int nlambda);
 
 /* Boundary intensity sampled by the top cascade: I_below[l] is seen by rays heading

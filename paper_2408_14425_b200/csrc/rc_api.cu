@@ -33,6 +33,8 @@ struct Plan {
     int NM = 1;                     // inclinations (2.5D); a lane carries LV * NM channels
     int nbands = 1, band_axis = 0;  // L2 banding of the long-ray cascades (1 = off); axis 0 = rows, 1 = columns
     size_t state = 0;               // parked ray state of the banded launches
+    size_t occ = 0;                 // occupancy bitmap of the packed cells (0: none, nx ny not a multiple of 32)
+    bool has_occ = false;
     CascadePlan c[RC_MAX_CASCADES];
     size_t chiT = 0, ST = 0, A[2] = {0, 0}, Jpart = 0, bc_below = 0, bc_above = 0, weights = 0, flag = 0;
     size_t io_chi = 0, io_eta = 0, io_J = 0;
@@ -51,6 +53,7 @@ struct rc_ctx {
     bool have_atm = false;
     int tab_nx = 0, tab_ny = 0;  // shape the step tables in the workspace were built for
     bool host_io = false;
+    bool sparse = false;  // most cells have chi == 0 at every wavelength (counted by rc_set_atmosphere): skip their gathers
     // developer overrides (environment, read by rc_create): RC_MARCH_VARIANT = 0..3 (register ring depth /
     // occupancy of march_kernel), RC_PATCH_LOG2 = 2..5 forces the lane patch width for cascades >= RC_PATCH_FROM
     int tune_variant = 2, tune_patch = -1, tune_patch_from = 0;
@@ -229,6 +232,8 @@ bool make_plan(const rc_config &cfg, int nm, int nx, int ny, int L, bool host_io
         }
         if (any) { P.state = cur; cur += 8 * field * P.NM; }
     }
+    P.has_occ = ncell % 32 == 0 && P.NM == 1;
+    if (P.has_occ) { P.occ = cur; cur += align_up((ncell / 32) * P.nb * sizeof(unsigned)); }
     P.chiT = cur; cur += field;
     P.ST = cur;   cur += field;
     P.A[0] = cur; cur += field * P.NM;  // merged cascades hold every (wavelength, inclination) channel
@@ -393,6 +398,21 @@ int rc_set_atmosphere(rc_ctx *ctx, const float *chi, const float *eta, int nx, i
         if (h & 1) return fail(ctx, RC_ERR_BAD_VALUE, "chi or eta has a negative or non-finite value");
         if (h & 2) return fail(ctx, RC_ERR_BAD_VALUE, "eta > 0 in a cell with chi == 0");
     }
+    {
+        // sparsity (many models are mostly empty): with more than two thirds of the cells at
+        // chi == 0 for every wavelength the march tests an occupancy bitmap before each gather
+        unsigned long long *cnt = (unsigned long long *)(ctx->ws + ctx->plan.flag);
+        unsigned long long h = 0;
+        ctx->sparse = false;
+        if (ctx->plan.has_occ && !std::getenv("RC_NO_SPARSE")) {
+            RC_CUDA(ctx, cudaMemsetAsync(cnt, 0, sizeof(*cnt), ctx->stream));
+            RC_CUDA(ctx, rc::launch_count_empty(chi, (long long)nx * ny, nlambda, cnt, ctx->stream));
+            RC_CUDA(ctx, cudaMemcpyAsync(&h, cnt, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream));
+            RC_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+            ctx->sparse = 3 * h > 2ULL * nx * ny || std::getenv("RC_FORCE_SPARSE");
+        }
+        ctx->stats.empty_cells = (int64_t)h;
+    }
     ctx->chi = chi;
     ctx->eta = eta;
     ctx->have_atm = true;
@@ -449,6 +469,7 @@ static rc::MarchParams march_params(const rc_ctx *ctx, int i, float *J_out) {
     rc::MarchParams mp;
     mp.chiT = (const float *)(ctx->ws + P.chiT);
     mp.ST = (const float *)(ctx->ws + P.ST);
+    mp.occ = ctx->sparse && P.has_occ && !c.empty ? (const unsigned *)(ctx->ws + P.occ) : nullptr;
     mp.Aup = i == top ? nullptr : (const float *)(ctx->ws + P.A[(i + 1) & 1]);
     mp.out = i > 0 ? (float *)(ctx->ws + P.A[i & 1]) : (accum ? (float *)(ctx->ws + P.Jpart) : J_out);
     mp.steps = c.empty ? nullptr : (const rc::Step *)(ctx->ws + c.steps_off);
@@ -496,6 +517,7 @@ int rc_solve_J(rc_ctx *ctx, float *J_out) {
             rc::PackParams pp;
             pp.chi = ctx->chi; pp.eta = ctx->eta;
             pp.chiT = (float *)(ctx->ws + P.chiT); pp.ST = (float *)(ctx->ws + P.ST);
+            pp.occ = ctx->sparse && P.has_occ ? (unsigned *)(ctx->ws + P.occ) : nullptr;
             pp.nx = P.nx; pp.ny = P.ny; pp.L = P.L; pp.nb = P.nb; pp.shift = i;
             RC_CUDA(ctx, rc::launch_pack(pp, P.LV, ctx->stream));
             launches++;

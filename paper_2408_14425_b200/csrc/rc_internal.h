@@ -32,6 +32,7 @@ struct CascadeTable {
 struct MarchParams {
     const float *chiT;  // packed opacity * log2(e): [nb][s][s][npy][npx][LV]  (phase (y mod s, x mod s), then y div s, x div s)
     const float *ST;    // packed source function eta/chi, same layout
+    const unsigned *occ;  // null (dense), or the occupancy bitmap pack_kernel wrote: empty cells are not gathered
     const float *Aup;   // merged cascade i+1, pre-averaged over the 4 children: [nb][N_i][npy/2][npx/2][LV]; null on the top cascade
     float *out;         // mode 0: A_i [nb][N_i/4][npy][npx][LV]; mode 1: J [ny][nx][L]; mode 2: Jpart [nb][ny][nx]
     const Step *steps;
@@ -61,6 +62,7 @@ struct MarchParams {
 struct PackParams {
     const float *chi, *eta;  // [ny][nx][L]
     float *chiT, *ST;        // [nb][s][s][npy][npx][LV]
+    unsigned *occ;           // null, or [nb][nx ny / 32]: bit = packed cell has chi > 0 at some wavelength of the batch
     int nx, ny, L, nb, shift;
 };
 
@@ -82,6 +84,7 @@ cudaError_t launch_table_build(const TableBuildParams &p, cudaStream_t st);
 cudaError_t launch_reduce_jbar(const float *Jpart, float *Jbar, long long ncell, int nb, cudaStream_t st);
 cudaError_t launch_count(const MarchParams &p, unsigned long long *total, cudaStream_t st);
 cudaError_t launch_gather_probe(const float *buf, unsigned long long nsector, int iters, int blocks, float *sink, cudaStream_t st);
+cudaError_t launch_count_empty(const float *chi, long long ncell, int L, unsigned long long *count, cudaStream_t st);
 cudaError_t launch_validate(const float *chi, const float *eta, long long n, int *flag, cudaStream_t st);
 
 }  // namespace rc

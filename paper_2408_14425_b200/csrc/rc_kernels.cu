@@ -199,6 +199,15 @@ __global__ void __launch_bounds__(256) pack_kernel(PackParams p) {
         c2[v] = ch[v] * 1.4426950408889634f;            // tau in units of ln 2: T = 2^-tau2
         S[v] = ch[v] > 0.f ? et[v] / ch[v] : 0.f;        // vacuum cells emit nothing (include/rc.h "Inputs")
     }
+    if (p.occ != nullptr) {
+        // occupancy bitmap of the packed cells of this batch (ncell is a multiple of 32 when occ is given, so a
+        // warp's 32 consecutive cells are one word): bit = some wavelength of the batch has chi > 0
+        bool nz = false;
+#pragma unroll
+        for (int v = 0; v < LV; v++) nz = nz || c2[v] != 0.f;
+        const unsigned w = __ballot_sync(FULL, nz);
+        if ((threadIdx.x & 31) == 0) p.occ[idx >> 5] = w;
+    }
     float *oc = p.chiT + idx * LV, *os = p.ST + idx * LV;
     if constexpr (LV == 8) {
         reinterpret_cast<float4 *>(oc)[0] = make_float4(c2[0], c2[1], c2[2], c2[3]);
@@ -347,7 +356,7 @@ __device__ __forceinline__ int first_step_reaching(const StepXY *xy, int n, int 
 // half of the directions that crosses the bands in ascending (or descending) order; a ray's (I, tau)
 // is carried from band to band through `state`, so the arithmetic - and the result - is that of the
 // unbanded launch, bit for bit, while the cells gathered by one launch fit L2.
-template <int LV, int NM, int PD, int WARPS, int MINB, bool BANDED>
+template <int LV, int NM, int PD, int WARPS, int MINB, bool BANDED, bool SPARSE>
 __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) {
     // sum over the 4 child directions, per thread: parked in shared memory between children so the
     // marching loop has the registers to itself
@@ -367,6 +376,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
     // (y div s, x div s) = (b, a) of every phase plane; a step's delta is lane-independent
     const float *chiB = p.chiT + (long long)nbI * ncell * LL;  // warp-uniform
     const float *SB = p.ST + (long long)nbI * ncell * LL;
+    const unsigned *occB = SPARSE ? p.occ + (long long)nbI * (ncell >> 5) : nullptr;
     // (dx, dy) ranges that keep this lane's ray inside the box
     const int dxlo = -(a << p.shift) - half, dxhi = ((p.npx - a) << p.shift) - 1 - half;
     const int dylo = -Y0, dyhi = p.ny - 1 - Y0;
@@ -415,33 +425,58 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
 #pragma unroll
                 for (int v = 0; v < LL; v++) { c2[u][v] = 0.f; S[u][v] = 0.f; }
                 const uint2 e = __ldg(tab + u);
-                const bool in = u < nin && (!BANDED || u >= n0);
+                bool in = u < nin && (!BANDED || u >= n0);
+                if constexpr (SPARSE) {  // empty cells (chi = 0 at every wavelength of the batch) are not gathered
+                    const unsigned c = probe + e.x;
+                    if (in) in = (__ldg(occB + (c >> 5)) >> (c & 31)) & 1u;
+                }
                 const unsigned long long d = (unsigned long long)(probe + e.x) * (LL * sizeof(float));
                 load_vec_if<LL>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(chiB) + d), c2[u], in);
                 load_vec_if<LL>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(SB) + d), S[u], in);
                 ds[u] = in ? __uint_as_float(e.y) : 0.f;
             }
             int chk = 0;
+            // SPARSE: the table entry and the occupancy word of the NEXT step to gather, read one step early
+            uint2 en_next = make_uint2(0u, 0u);
+            unsigned occ_next = 0u;
+            if constexpr (SPARSE) {
+                en_next = __ldg(tab + PD);
+                if (PD < nin && (!BANDED || PD >= n0)) occ_next = __ldg(occB + ((probe + en_next.x) >> 5));
+            }
             // a1: eq. 16 along the interval, front to back: with tau accumulated,
             // T_n = 2^-tau2_n and the cell's contribution is S (T_{n-1} - T_n)  [= S T (1 - e^{-chi ds})]
             for (int st = 0; st < nw; st += PD) {
 #pragma unroll
                 for (int u = 0; u < PD; u++) {
-                    const uint2 en = __ldg(tab + st + u + PD);
+                    uint2 en;
+                    unsigned occ_cur = 0u;
+                    if constexpr (SPARSE) {
+                        en = en_next;
+                        occ_cur = occ_next;
+                        en_next = __ldg(tab + st + u + PD + 1);
+                        occ_next = 0u;
+                        if (st + u + PD + 1 < nin && (!BANDED || st + u + PD + 1 >= n0))
+                            occ_next = __ldg(occB + ((probe + en_next.x) >> 5));
+                    } else {
+                        en = __ldg(tab + st + u + PD);
+                    }
                     // integrate step st + u (a slot past the lane's last in-box step has ds = 0: no effect)
                     // 2.5D: inclination m crosses the same cell over ds / sin(inclination)
                     float dsm[NM];
 #pragma unroll
                     for (int m = 0; m < NM; m++) dsm[m] = NM == 1 ? ds[u] : ds[u] * p.incl_f[m];
+                    if (!SPARSE || __any_sync(FULL, ds[u] != 0.f)) {  // SPARSE: no lane has an occupied cell: nothing to do
 #pragma unroll
-                    for (int v = 0; v < LV; v++) {
-                        tau[v] = fmaf(c2[u][v / NM], dsm[v % NM], tau[v]);
-                        const float Tn = ex2_neg(tau[v]);
-                        I[v] = fmaf(S[u][v / NM], T[v] - Tn, I[v]);
-                        T[v] = Tn;
+                        for (int v = 0; v < LV; v++) {
+                            tau[v] = fmaf(c2[u][v / NM], dsm[v % NM], tau[v]);
+                            const float Tn = ex2_neg(tau[v]);
+                            I[v] = fmaf(S[u][v / NM], T[v] - Tn, I[v]);
+                            T[v] = Tn;
+                        }
                     }
                     // refill the slot with step st + u + PD
-                    const bool in = st + u + PD < nin && (!BANDED || st + u + PD >= n0);
+                    bool in = st + u + PD < nin && (!BANDED || st + u + PD >= n0);
+                    if constexpr (SPARSE) in = in && ((occ_cur >> ((probe + en.x) & 31)) & 1u);
                     const unsigned long long d = (unsigned long long)(probe + en.x) * (LL * sizeof(float));
                     load_vec_if<LL>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(chiB) + d), c2[u], in);
                     load_vec_if<LL>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(SB) + d), S[u], in);
@@ -541,16 +576,30 @@ static cudaError_t launch_march_variant(const MarchParams &p, cudaStream_t st) {
     const long long blocks = (march_warps(p) + WARPS - 1) / WARPS;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     if (p.state != nullptr)
-        march_kernel<LV, NM, PD, WARPS, MINB, true><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
+        march_kernel<LV, NM, PD, WARPS, MINB, true, false><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
     else
-        march_kernel<LV, NM, PD, WARPS, MINB, false><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
+        march_kernel<LV, NM, PD, WARPS, MINB, false, false><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
     return cudaGetLastError();
 }
 
 // variant: 0 = ring of 2 steps, 24 warps/SM (<= 80 registers); 1 = ring of 3, 20 warps/SM (<= 96);
 //          2 = ring of 3, 16 warps/SM (<= 128); 3 = ring of 4, 16 warps/SM (<= 128)
+// Mostly-empty atmospheres (occ != null): the default variant with the occupancy test.
+template <int LV>
+static cudaError_t launch_march_sparse(const MarchParams &p, cudaStream_t st) {
+    constexpr int WARPS = 8;
+    const long long blocks = (march_warps(p) + WARPS - 1) / WARPS;
+    if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+    if (p.state != nullptr)
+        march_kernel<LV, 1, 3, WARPS, 2, true, true><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
+    else
+        march_kernel<LV, 1, 3, WARPS, 2, false, true><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
+    return cudaGetLastError();
+}
+
 template <int LV>
 static cudaError_t launch_march_flat(const MarchParams &p, int variant, cudaStream_t st) {
+    if (p.occ != nullptr) return launch_march_sparse<LV>(p, st);
     switch (variant) {
         case 0: return launch_march_variant<LV, 1, 2, 8, 3>(p, st);
         case 1: return launch_march_variant<LV, 1, 3, 5, 4>(p, st);
@@ -608,6 +657,23 @@ __global__ void validate_kernel(const float *chi, const float *eta, long long n,
         if (c == 0.f && e > 0.f) bad |= 2;
     }
     if (bad) atomicOr(flag, bad);
+}
+
+// Number of cells with chi == 0 at every wavelength (rc_set_atmosphere: is the atmosphere mostly empty?).
+__global__ void count_empty_kernel(const float *chi, long long ncell, int L, unsigned long long *count) {
+    unsigned long long mine = 0;
+    for (long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x; c < ncell; c += (long long)gridDim.x * blockDim.x) {
+        bool empty = true;
+        for (int l = 0; l < L; l++) empty = empty && chi[c * L + l] == 0.f;
+        mine += empty;
+    }
+    for (int o = 16; o > 0; o >>= 1) mine += __shfl_down_sync(FULL, mine, o);
+    if ((threadIdx.x & 31) == 0 && mine) atomicAdd(count, mine);
+}
+
+cudaError_t launch_count_empty(const float *chi, long long ncell, int L, unsigned long long *count, cudaStream_t st) {
+    count_empty_kernel<<<148 * 8, 256, 0, st>>>(chi, ncell, L, count);
+    return cudaGetLastError();
 }
 
 cudaError_t launch_validate(const float *chi, const float *eta, long long n, int *flag, cudaStream_t st) {

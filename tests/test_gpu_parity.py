@@ -258,3 +258,30 @@ def test_inclinations_reset_to_flatland(oracle):
     with pytest.raises(binding.RcError):
         rc.set_inclinations([0.0, 1.0], [0.5, 0.5])             # mu = 1: infinite path
     rc.close()
+
+
+# ------------------------------------------------------------------ sparsity
+@pytest.mark.parametrize("bands", [1, 3])
+def test_sparse_march_is_bit_identical(oracle, monkeypatch, bands):
+    """Mostly-empty atmospheres (config 4's recipe: > 90 % of cells exactly 0): rc_set_atmosphere counts the
+    empty cells, pack_kernel writes an occupancy bitmap and the march gathers occupied cells only.  An empty
+    cell contributes nothing (chi = 0, S = 0), so J must be bit-identical to the dense march (RC_NO_SPARSE),
+    also when banded, and match the oracle."""
+    from paper_2408_14425_b200 import binding
+    atm = A.make_config(4, nx=256, ny=128, nlambda=11, ncascades=6)
+    monkeypatch.setenv("RC_BANDS", str(bands))
+    J, rc = binding.solve_atmosphere(atm, flags=0)
+    st = rc.get_stats()
+    rc.close()
+    assert st.empty_cells > 0.8 * atm.nx * atm.ny
+    monkeypatch.setenv("RC_NO_SPARSE", "1")
+    J2, rc2 = binding.solve_atmosphere(atm, flags=0)
+    rc2.close()
+    assert np.array_equal(J.cpu().numpy(), J2.cpu().numpy())
+    monkeypatch.delenv("RC_NO_SPARSE")
+    check(atm, oracle)
+    # and forced on a dense atmosphere (every bit set): still bit-identical
+    dense = A.make_config(2, nx=128, ny=64, nlambda=5, ncascades=5)
+    ref = gpu_solve(dense)
+    monkeypatch.setenv("RC_FORCE_SPARSE", "1")
+    assert np.array_equal(ref, gpu_solve(dense))
