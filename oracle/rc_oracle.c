@@ -58,7 +58,32 @@ typedef struct {
     double path_scale;      /* true path length per unit length in the plane: 1 in flatland; 1/sin(inclination
                                to the invariant axis) for the inclined rays of the 2.5D scheme (PAPER.md:281:
                                "the same x-z projection and different inclinations in y") */
+    /* velocity-dependent line mode ("velocity-dependent terms (spectral lines) are computed
+       on the fly for each ray given its specific direction, and thus projected plasma velocity"): when
+       `line` is set, chi/eta above are unused and the opacity and emissivity of cell c at wavelength l
+       seen by a ray are those of cell_chi_eta() below */
+    const float *line;  /* [ny][nx][6]: chi_c, S_c, chi_line, S_line, v_x, v_y (velocities in Doppler widths) */
+    const double *xl;   /* [L] wavelengths as offsets from line centre, in Doppler widths */
 } grid_t;
+
+/* Opacity and emissivity of cell `cell` at wavelength l for the photons that travel along a ray traced
+ * from its probe in direction (wx, wy): they move along n = -(wx, wy), so in the observer's frame the line
+ * of a cell with velocity v is centred at x = v.n:
+ *     a = x_l - v.n ,  phi = exp(-a^2)/sqrt(pi) ,
+ *     chi = chi_c + chi_line phi ,  eta = chi_c S_c + chi_line S_line phi . */
+static void cell_chi_eta(const grid_t *g, int cell, int l, double wx, double wy, double *chi, double *eta) {
+    if (!g->line) {
+        size_t c = (size_t)cell * g->L + l;
+        *chi = (double)g->chi[c];
+        *eta = (double)g->eta[c];
+        return;
+    }
+    const float *f = g->line + (size_t)cell * 6;
+    double a = g->xl[l] + ((double)f[4] * wx + (double)f[5] * wy);
+    double phi = exp(-a * a) / sqrt(M_PI);
+    *chi = (double)f[0] + (double)f[2] * phi;
+    *eta = (double)f[0] * (double)f[1] + (double)f[2] * (double)f[3] * phi;
+}
 
 typedef struct {
     int cell;  /* y*nx + x */
@@ -137,13 +162,14 @@ static int diag_segments(int nx, int ny, int cx, int cy, int q, double ta, doubl
 }
 
 /* eq. 16 along the segments, front-to-back, all wavelengths: I[l], T[l] = exp(-tau[l]). */
-static void integrate_ftb(const grid_t *g, const seg_t *seg, int n, double *I, double *T) {
+static void integrate_ftb(const grid_t *g, const seg_t *seg, int n, double wx, double wy, double *I, double *T) {
     for (int l = 0; l < g->L; l++) {
         double Il = 0.0, Tl = 1.0;
         for (int s = 0; s < n; s++) {
-            size_t c = (size_t)seg[s].cell * g->L + l;
-            double ds = seg[s].ds * g->path_scale, x = (double)g->chi[c] * ds;
-            Il += Tl * (double)g->eta[c] * ds * f_emis(x);
+            double chi, eta;
+            cell_chi_eta(g, seg[s].cell, l, wx, wy, &chi, &eta);
+            double ds = seg[s].ds * g->path_scale, x = chi * ds;
+            Il += Tl * eta * ds * f_emis(x);
             Tl *= exp(-x);
         }
         I[l] = Il;
@@ -153,12 +179,13 @@ static void integrate_ftb(const grid_t *g, const seg_t *seg, int n, double *I, d
 
 /* eq. 16 literally: start at the far end with I = 0 and integrate towards the probe
  * ("back-to-front"); tau accumulated, T = exp(-tau). */
-static void integrate_btf(const grid_t *g, const seg_t *seg, int n, double *I, double *T) {
+static void integrate_btf(const grid_t *g, const seg_t *seg, int n, double wx, double wy, double *I, double *T) {
     for (int l = 0; l < g->L; l++) {
         double Il = 0.0, tau = 0.0;
         for (int s = n - 1; s >= 0; s--) {
-            size_t c = (size_t)seg[s].cell * g->L + l;
-            double ds = seg[s].ds * g->path_scale, chi = g->chi[c], eta = g->eta[c], x = chi * ds;
+            double chi, eta;
+            cell_chi_eta(g, seg[s].cell, l, wx, wy, &chi, &eta);
+            double ds = seg[s].ds * g->path_scale, x = chi * ds;
             tau += x;
             Il = Il * exp(-x) + (chi > 0.0 ? (eta / chi) * (-expm1(-x)) : eta * ds);
         }
@@ -200,11 +227,13 @@ int rc_oracle_ray_segments(int nx, int ny, double px, double py, double theta, i
 int rc_oracle_interval(const float *chi, const float *eta, int nx, int ny, int L, double px,
                        double py, double theta, int diag_q, double ta, double tb, int order,
                        double *I, double *T) {
-    grid_t g = {nx, ny, L, chi, eta, 1.0};
+    grid_t g = {nx, ny, L, chi, eta, 1.0, NULL, NULL};
     seg_t *seg = (seg_t *)malloc(sizeof(seg_t) * (size_t)(nx + ny + 4));
     int n = diag_q >= 0 ? diag_segments(nx, ny, (int)floor(px), (int)floor(py), diag_q, ta, tb, seg)
                         : dda_segments(nx, ny, px, py, cos(theta), sin(theta), ta, tb, seg);
-    if (order == 0) integrate_ftb(&g, seg, n, I, T); else integrate_btf(&g, seg, n, I, T);
+    if (diag_q >= 0) theta = 2.0 * M_PI * (diag_q + 0.5) / 4.0;
+    if (order == 0) integrate_ftb(&g, seg, n, cos(theta), sin(theta), I, T);
+    else integrate_btf(&g, seg, n, cos(theta), sin(theta), I, T);
     free(seg);
     return n;
 }
@@ -235,17 +264,18 @@ typedef struct {
  *   order: 0 front-to-back, 1 back-to-front (G13).
  * Returns 0, or -1 on bad arguments / -2 out of memory.
  */
-int rc_oracle_solve_scaled(const float *chi, const float *eta, int nx, int ny, int L, int ncasc,
+static int solve_impl(const float *chi, const float *eta, const float *line, const double *xl, int nx, int ny,
+                      int L, int ncasc,
                            double c0, const float *I_below, const float *I_above, const float *w,
                            int x0, int x1, int y0, int y1, double *J_out, double *Jbar_out, int nthreads,
                            int order, int dump_cascade, double *dump_I, double *dump_T, double *dump_M,
                            int *dump_win, rc_oracle_counts *counts, double path_scale) {
-    if (!chi || !eta || !J_out || nx <= 0 || ny <= 0 || L <= 0 || ncasc < 1 || ncasc > 15)
+    if (!((chi && eta) || (line && xl)) || !J_out || nx <= 0 || ny <= 0 || L <= 0 || ncasc < 1 || ncasc > 15)
         return -1;
     int top = ncasc - 1;
     if (nx % (1 << top) || ny % (1 << top)) return -1; /* reading G19 */
     if (x0 < 0 || y0 < 0 || x1 > nx || y1 > ny || x0 >= x1 || y0 >= y1) return -1;
-    grid_t g = {nx, ny, L, chi, eta, path_scale};
+    grid_t g = {nx, ny, L, chi, eta, path_scale, line, xl};
     if (counts) memset(counts, 0, sizeof(*counts));
 #ifdef _OPENMP
     if (nthreads > 0) omp_set_num_threads(nthreads);
@@ -290,7 +320,8 @@ int rc_oracle_solve_scaled(const float *chi, const float *eta, int nx, int ny, i
                         int n = i == 0 ? diag_segments(nx, ny, a, b, (int)k, ta, tb, seg)
                                        : dda_segments(nx, ny, px, py, cos(theta), sin(theta), ta, tb, seg);
                         nseg_total += n;
-                        if (order == 0) integrate_ftb(&g, seg, n, I, T); else integrate_btf(&g, seg, n, I, T);
+                        if (order == 0) integrate_ftb(&g, seg, n, cos(theta), sin(theta), I, T);
+                        else integrate_btf(&g, seg, n, cos(theta), sin(theta), I, T);
                         size_t o = ((((size_t)(b - by0[i])) * wx + (a - ax0[i])) * N + k) * L;
                         if (dump) for (int l = 0; l < L; l++) { dump_I[o + l] = I[l]; dump_T[o + l] = T[l]; }
                         if (i == top) {
@@ -344,6 +375,24 @@ int rc_oracle_solve_scaled(const float *chi, const float *eta, int nx, int ny, i
     }
     free(Mup);
     return status;
+}
+
+int rc_oracle_solve_scaled(const float *chi, const float *eta, int nx, int ny, int L, int ncasc,
+                           double c0, const float *I_below, const float *I_above, const float *w,
+                           int x0, int x1, int y0, int y1, double *J_out, double *Jbar_out, int nthreads,
+                           int order, int dump_cascade, double *dump_I, double *dump_T, double *dump_M,
+                           int *dump_win, rc_oracle_counts *counts, double path_scale) {
+    return solve_impl(chi, eta, NULL, NULL, nx, ny, L, ncasc, c0, I_below, I_above, w, x0, x1, y0, y1, J_out,
+                      Jbar_out, nthreads, order, dump_cascade, dump_I, dump_T, dump_M, dump_win, counts, path_scale);
+}
+
+/* Velocity-dependent line mode: line [ny][nx][6] and xl [L] instead of chi, eta (cell_chi_eta above). */
+int rc_oracle_solve_line(const float *line, const double *xl, int nx, int ny, int L, int ncasc, double c0,
+                         const float *I_below, const float *I_above, const float *w, int x0, int x1, int y0,
+                         int y1, double *J_out, double *Jbar_out, int nthreads, int order,
+                         rc_oracle_counts *counts) {
+    return solve_impl(NULL, NULL, line, xl, nx, ny, L, ncasc, c0, I_below, I_above, w, x0, x1, y0, y1, J_out,
+                      Jbar_out, nthreads, order, -1, NULL, NULL, NULL, NULL, counts, 1.0);
 }
 
 /* Flatland (path_scale = 1): the solve of SURVEY.md §8(c). */

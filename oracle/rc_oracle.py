@@ -53,6 +53,10 @@ def lib():
                                                           C.c_void_p, C.c_void_p])
         _lib.rc_oracle_solve_scaled.restype = C.c_int
         _lib.rc_oracle_solve_scaled.argtypes = _lib.rc_oracle_solve.argtypes + [C.c_double]
+        _lib.rc_oracle_solve_line.restype = C.c_int
+        _lib.rc_oracle_solve_line.argtypes = ([C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double,
+                                               C.c_void_p, C.c_void_p, C.c_void_p] + [C.c_int] * 4 +
+                                              [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p])
         _lib.rc_oracle_num_threads.restype = C.c_int
     return _lib
 
@@ -156,8 +160,39 @@ def solve_inclined(chi, eta, ncascades, mu, w_mu, **kw):
     return out
 
 
+def solve_line(line, xl, ncascades, c0=1.0, I_below=None, I_above=None, weights=None, window=None,
+               nthreads=0, order=0, want_counts=False):
+    """Velocity-dependent line mode: per cell chi_c, S_c, chi_line, S_line,
+    v_x, v_y; opacity and emissivity are evaluated per ray from the projected velocity (rc_oracle.c,
+    cell_chi_eta).  line: float32 [ny][nx][6]; xl: [L] Doppler-width offsets.  Returns J, Jbar like solve()."""
+    line = _f32(line)
+    xl = np.ascontiguousarray(xl, dtype=np.float64)
+    ny, nx, six = line.shape
+    assert six == 6
+    L = xl.size
+    x0, x1, y0, y1 = (0, nx, 0, ny) if window is None else window
+    J = np.empty((y1 - y0, x1 - x0, L))
+    Jbar = np.empty((y1 - y0, x1 - x0))
+    Ib = None if I_below is None else _f32(I_below)
+    Ia = None if I_above is None else _f32(I_above)
+    w = None if weights is None else _f32(weights)
+    cnt = Counts()
+    rc = lib().rc_oracle_solve_line(_ptr(line), _ptr(xl), nx, ny, L, ncascades, c0, _ptr(Ib), _ptr(Ia), _ptr(w),
+                                    x0, x1, y0, y1, _ptr(J), _ptr(Jbar), nthreads, order, C.byref(cnt))
+    if rc != 0:
+        raise ValueError(f"rc_oracle_solve_line failed: {rc}")
+    out = {"J": J, "Jbar": Jbar}
+    if want_counts:
+        out["intervals"] = np.array(cnt.intervals[:ncascades])
+        out["segments"] = np.array(cnt.segments[:ncascades])
+    return out
+
+
 def solve_atmosphere(atm, **kw):
     """Convenience: oracle solve of a paper_2408_14425_b200.atmospheres.Atmosphere-like object."""
+    if getattr(atm, "line", None) is not None:
+        return solve_line(atm.line, atm.xl, atm.ncascades, c0=atm.c0_interval, I_below=atm.I_below,
+                          I_above=atm.I_above, weights=atm.weights, **kw)
     if getattr(atm, "mu", None) is not None:
         return solve_inclined(atm.chi, atm.eta, atm.ncascades, atm.mu, atm.w_mu, c0=atm.c0_interval,
                               I_below=atm.I_below, I_above=atm.I_above, weights=atm.weights, **kw)

@@ -41,6 +41,9 @@ class Atmosphere:
     # inclined rays that replace every flatland ray; None = flatland
     mu: np.ndarray | None = None
     w_mu: np.ndarray | None = None
+    # velocity-dependent line mode: per-cell line parameters instead of chi, eta (then None)
+    line: np.ndarray | None = None  # float32 [ny][nx][6]: chi_c, S_c, chi_line, S_line, v_x, v_y (Doppler widths)
+    xl: np.ndarray | None = None    # float64 [nlambda] offsets from line centre in Doppler widths
 
 
 # (nx, ny, nlambda, ncascades) of BASELINE.json's configs
@@ -159,6 +162,27 @@ def config2(nx=None, ny=None, nlambda=None, ncascades=None, seed=1002) -> Atmosp
         chi[:, :, l] = chi_c + chi_line * _phi(x[l] - v)
     eta = chi * S.astype(np.float32)[:, :, None]
     return _finish("cfg2", nx, ny, L, nc, chi, eta)
+
+
+def line_config2(nx=None, ny=None, nlambda=None, ncascades=None, seed=1002) -> Atmosphere:
+    """Config 2's recipe as a moving-line atmosphere: the same chi_c, chi_line, speed and
+    S fields, but the velocity is a vector (speed x a smooth direction field) and the line is Doppler shifted
+    per ray by the projected velocity; the line has its own source function field.  chi, eta are None."""
+    nx, ny, L, nc, sc = _dims(2, nx, ny, nlambda, ncascades)
+    rng = np.random.default_rng(seed)
+    g1, g2, v, S = _line_fields(rng, ny, nx, sc)
+    psi = 2.0 * np.pi * _unit01(_smooth_normal(rng, ny, nx, 16.0 * sc))
+    h2 = _unit01(_smooth_normal(rng, ny, nx, 8.0 * sc))
+    line = np.empty((ny, nx, 6), np.float32)
+    line[..., 0] = 1e-3 * np.exp(g1)
+    line[..., 1] = S
+    line[..., 2] = np.exp(g2)
+    line[..., 3] = 10.0 ** (2.0 * h2 - 1.0)
+    line[..., 4] = v * np.cos(psi)
+    line[..., 5] = v * np.sin(psi)
+    z = np.zeros(L, np.float32)
+    return Atmosphere(name="line2", nx=nx, ny=ny, nlambda=L, ncascades=nc, chi=None, eta=None, I_below=z.copy(),
+                      I_above=z.copy(), weights=np.ones(L, np.float32), line=line, xl=_xgrid(L).astype(np.float64))
 
 
 def config3(nx=None, ny=None, nlambda=None, ncascades=None, seed=1003) -> Atmosphere:

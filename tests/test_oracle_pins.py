@@ -428,3 +428,76 @@ def test_I3_inclined_rays_see_more_optical_depth(oracle):
     steep = oracle.solve_inclined(a.chi, z, 4, mu[-1:], [1.0], I_below=[1.0])["J"]
     m = flat > 1e-6
     assert np.all(incl[m] < flat[m]) and np.all(steep[m] < incl[m])
+
+
+# ----------------------------------------------------------------------------- moving line (f1)
+def _static_fields(line, xl, wx=0.0, wy=0.0):
+    """chi, eta [ny][nx][L] in fp64 of a line atmosphere as seen along one direction (test-side restatement)."""
+    f = line.astype(np.float64)
+    a = xl[None, None, :] + (f[..., 4] * wx + f[..., 5] * wy)[..., None]
+    phi = np.exp(-a * a) / np.sqrt(np.pi)
+    chi = f[..., 0:1] + f[..., 2:3] * phi
+    eta = f[..., 0:1] * f[..., 1:2] + f[..., 2:3] * f[..., 3:4] * phi
+    return chi, eta
+
+
+def test_V1_static_line_equals_precomputed_opacities(oracle):
+    """v = 0: the on-the-fly line mode is the GivenFs solve of chi_l = chi_c + chi_line phi(x_l),
+    eta_l = chi_c S_c + chi_line S_line phi(x_l); equal up to the fp32 rounding of the precomputed inputs."""
+    a = A.line_config2(nx=32, ny=32, nlambda=5, ncascades=4)
+    a.line[..., 4:6] = 0.0
+    chi, eta = _static_fields(a.line, a.xl)
+    J1 = oracle.solve_line(a.line, a.xl, 4, I_below=[0.2] * 5)["J"]
+    J0 = oracle.solve(chi.astype(np.float32), eta.astype(np.float32), 4, I_below=[0.2] * 5)["J"]
+    assert np.allclose(J1, J0, rtol=5e-7)
+
+
+def test_V2_uniform_flow_single_cascade_closed_form(oracle):
+    """ncasc = 1 (4 diagonal rays to the edge), uniform medium with a uniform flow v: the ray traced along
+    w_k carries photons moving along -w_k, which see the line at x = -v.w_k:
+    J_l = 1/4 sum_k [S_kl (1 - e^{-chi_kl d_k}) + B e^{-chi_kl d_k}], chi_kl = chi_c + chi_line phi(x_l + v.w_k)."""
+    nx, ny, L = 12, 20, 7
+    xl = np.linspace(-3, 3, L)
+    cell = np.array([0.01, 0.7, 0.4, 2.0, 1.3, -0.6], np.float32)
+    line = np.broadcast_to(cell, (ny, nx, 6)).copy()
+    B = 0.35
+    J = oracle.solve_line(line, xl, 1, I_below=[B] * L, I_above=[B] * L)["J"]
+    c = cell.astype(np.float64)
+    y, x = np.mgrid[0:ny, 0:nx]
+    dxp, dxm, dyp, dym = nx - (x + 0.5), x + 0.5, ny - (y + 0.5), y + 0.5
+    want = np.zeros((ny, nx, L))
+    for (sx, sy), (dx, dy) in zip(((1, 1), (-1, 1), (-1, -1), (1, -1)), ((dxp, dyp), (dxm, dyp), (dxm, dym), (dxp, dym))):
+        wx, wy = sx / R2, sy / R2
+        d = R2 * np.minimum(dx, dy)
+        for l in range(L):
+            a_ = xl[l] + (c[4] * wx + c[5] * wy)
+            phi = np.exp(-a_ * a_) / np.sqrt(np.pi)
+            chi = c[0] + c[2] * phi
+            S = (c[0] * c[1] + c[2] * c[3] * phi) / chi
+            att = np.exp(-chi * d)
+            want[..., l] += (S * (1 - att) + B * att) / 4
+    assert np.allclose(J, want, rtol=1e-12)
+
+
+def test_V3_moving_line_symmetries(oracle):
+    """(a) reversing every velocity and mirroring the wavelength grid leaves J_l -> J_{L-1-l} (phi is even);
+    (b) rotating the atmosphere by 90 degrees, velocities included, rotates J; (c) a velocity field changes J
+    (the mode is not ignoring it)."""
+    a = A.line_config2(nx=32, ny=32, nlambda=6, ncascades=4, seed=4)
+    J = oracle.solve_line(a.line, a.xl, 4)["J"]
+    rev = a.line.copy()
+    rev[..., 4:6] *= -1
+    Jr = oracle.solve_line(rev, -a.xl[::-1], 4)["J"]
+    assert np.allclose(Jr, J[..., ::-1], rtol=1e-12)
+    # np.rot90(f, 1, axes=(0, 1)): r[y'][x'] = f[x'][n-1-y'], i.e. the point (x, y) goes to (y, -x): a clockwise
+    # quarter turn, under which a vector (v_x, v_y) becomes (v_y, -v_x)
+    rot = np.rot90(a.line, 1, axes=(0, 1)).copy()
+    vx, vy = rot[..., 4].copy(), rot[..., 5].copy()
+    rot[..., 4], rot[..., 5] = vy, -vx
+    J90 = oracle.solve_line(rot, a.xl, 4)["J"]
+    assert np.allclose(J90, np.rot90(J, 1, axes=(0, 1)), rtol=1e-11)
+    rot[..., 4], rot[..., 5] = -vy, vx                     # the vector turned the wrong way must NOT match
+    assert not np.allclose(oracle.solve_line(rot, a.xl, 4)["J"], np.rot90(J, 1, axes=(0, 1)), rtol=1e-4)
+    still = a.line.copy()
+    still[..., 4:6] = 0
+    assert np.max(np.abs(oracle.solve_line(still, a.xl, 4)["J"] / J - 1)) > 1e-2
