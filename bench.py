@@ -129,6 +129,9 @@ def main():
     ap.add_argument("--config", type=int, default=2)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--lambda-batch", type=int, default=0)
+    ap.add_argument("--line", action="store_true",
+                    help="velocity-dependent line mode (SURVEY §8(f) f1): configs[2]'s recipe as a moving-line "
+                         "atmosphere, opacities evaluated per ray (rc_set_line_atmosphere)")
     ap.add_argument("--inclinations", type=int, default=1,
                     help="2.5D: N Gauss-Radau inclined rays per flatland ray (SURVEY §8(f) f2); the unit count "
                          "becomes segment-wavelength-inclinations")
@@ -144,6 +147,11 @@ def main():
     workload = (f"BASELINE.json configs[{args.config}]: {fx}x{fy} cells, {fl} wavelengths, {fc} cascades, "
                 f"seeded synthetic atmosphere (DESIGN.md §4)")
     atm = atmospheres.make_config(args.config, seed=1000 + args.config + 17 * rank)
+    if args.line:
+        atm = atmospheres.line_config2(seed=1002 + 17 * rank)
+        fx, fy, fl, fc = atm.nx, atm.ny, atm.nlambda, atm.ncascades
+        workload = (f"moving-line variant of BASELINE.json configs[2]: {fx}x{fy} cells, {fl} wavelengths, {fc} cascades, "
+                    "line opacity evaluated per ray from the projected velocity (SURVEY §8(f) f1)")
     if args.inclinations > 1:
         atm = atmospheres.with_inclinations(atm, args.inclinations)
         workload += f", 2.5D with {args.inclinations} Gauss-Radau inclinations per ray (value counts segment-wavelength-inclinations)"
@@ -166,10 +174,17 @@ def main():
     if atm.mu is not None:
         rc.set_inclinations(atm.mu, atm.w_mu)
     rc.ensure_workspace(atm.nx, atm.ny, atm.nlambda, host_io=True)
-    chi_h = torch.from_numpy(atm.chi).pin_memory()
-    eta_h = torch.from_numpy(atm.eta).pin_memory()
-    chi, eta = chi_h.to(dev), eta_h.to(dev)
-    rc.set_atmosphere(chi, eta)
+    if rc._ws.numel() < (80 << 20):  # room for the 64 MB region of the gather-bandwidth probe
+        rc.set_workspace(torch.empty(80 << 20, dtype=torch.uint8, device=dev))
+    if atm.line is not None:
+        line_h = torch.from_numpy(atm.line).pin_memory()
+        line_d = line_h.to(dev)
+        rc.set_line_atmosphere(line_d, atm.xl)
+    else:
+        chi_h = torch.from_numpy(atm.chi).pin_memory()
+        eta_h = torch.from_numpy(atm.eta).pin_memory()
+        chi, eta = chi_h.to(dev), eta_h.to(dev)
+        rc.set_atmosphere(chi, eta)
     rc.set_boundary(atm.I_below, atm.I_above)
     rc.set_lambda_weights(atm.weights)
     seg = rc.count_segments()
@@ -207,14 +222,28 @@ def main():
 
     # end to end: host buffers in, host buffer out, every step
     out_h = torch.empty(J.shape, dtype=torch.float32, pin_memory=True)
-    rc.solve_J_host(chi_h, eta_h, out_h)
+    if atm.line is not None:
+        h2d_bytes = int(atm.line.nbytes)
+
+        def e2e_step():  # line mode: the same public calls a user makes, host buffers both ends
+            line_d.copy_(line_h, non_blocking=True)
+            rc.set_line_atmosphere(line_d, atm.xl)
+            rc.solve_J(out=J)
+            out_h.copy_(J, non_blocking=True)
+            torch.cuda.synchronize()
+    else:
+        h2d_bytes = int(2 * atm.chi.nbytes)
+
+        def e2e_step():
+            rc.solve_J_host(chi_h, eta_h, out_h)
+    e2e_step()
     rc.set_boundary(atm.I_below, atm.I_above)
     rc.set_lambda_weights(atm.weights)
-    rc.solve_J_host(chi_h, eta_h, out_h)
+    e2e_step()
     barrier(); torch.cuda.synchronize()
     e0.record()
     for _ in range(args.e2e_steps):
-        rc.solve_J_host(chi_h, eta_h, out_h)
+        e2e_step()
     e1.record()
     torch.cuda.synchronize(); barrier()
     ms2 = torch.tensor([e0.elapsed_time(e1)], device=dev)
@@ -239,7 +268,9 @@ def main():
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
             "data": "synthetic",
             "config": {"workload": workload, "seg_lambda_per_step_per_gpu": segl_per_step, "lambda_batch": st.lambda_batch,
-                       "l2": "inputs (chi+eta %.0f MB) larger than L2" % (2 * atm.chi.nbytes / 1e6),
+                       "l2": ("inputs (chi+eta %.0f MB) larger than L2" % (h2d_bytes / 1e6)) if atm.line is None else
+                             "line parameters (%.0f MB) fit L2; merged cascades (2 x %.0f MB per cascade) stream through it"
+                             % (h2d_bytes / 1e6, 4 * atm.nx * atm.ny * atm.nlambda / 1e6),
                        "parallelism": f"wavelength blocks x{world}, no collective"},
             "solve_ms": ms_step,
             "hbm_effective_frac": (8 * segl_per_step + 2 * casc_bytes * atm.ncascades) / (ms_step * 1e-3) / 1e9 / hbm_peak,
@@ -259,7 +290,7 @@ def main():
             "per_cascade_ms": {"march": ms_march, "pack": [st.ms_pack[i] for i in range(atm.ncascades)]},
             "segments_per_cascade": seg,
             "e2e": {"value": world * segl_per_step / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms,
-                    "h2d_bytes_per_step": int(2 * atm.chi.nbytes), "d2h_bytes_per_step": int(out_h.numel() * 4),
+                    "h2d_bytes_per_step": h2d_bytes, "d2h_bytes_per_step": int(out_h.numel() * 4),
                     "matches_device_path": same},
             "gpu_launches": launches, "clocks": clocks,
         }

@@ -93,7 +93,7 @@ int rc_create(rc_ctx **out, const rc_config *cfg);
 
 /* Bytes of device workspace rc_solve_J needs for an nx x ny x nlambda atmosphere (0 on bad shape).
  * host_io != 0 adds room for the device copies rc_solve_J_host makes of chi, eta and J. */
-size_t rc_workspace_bytes(const rc_ctx *ctx, int nx, int ny, int nlambda, int host_io);
+size_t rc_workspace_bytes(const rc_ctx *ctx, int nx, int ny, int nlambda, int host_io);  /* enough for rc_set_atmosphere and rc_set_line_atmosphere alike */
 
 /* Caller-owned device workspace (256-byte aligned), borrowed. */
 int rc_set_workspace(rc_ctx *ctx, void *dev_ptr, size_t bytes);
@@ -107,6 +107,17 @@ int rc_set_stream(rc_ctx *ctx, void *cuda_stream);
  * more than two thirds are, the march skips the gathers of empty cells (sparsity; the result
  * is bit-identical).  PAPER.md:409. */
 int rc_set_atmosphere(rc_ctx *ctx, const float *chi, const float *eta, int nx, int ny, int nlambda);
+
+/* Velocity-dependent line mode ("velocity-dependent terms (spectral lines) are computed on the
+ * fly for each ray given its specific direction, and thus projected plasma velocity"),
+ * instead of rc_set_atmosphere.  line: device, [ny][nx][6] float32, borrowed: chi_c, S_c (continuum opacity
+ * and source function), chi_line, S_line (line opacity scale and source function), v_x, v_y (bulk velocity in
+ * Doppler widths).  x_lambda: host, [nlambda], wavelength offsets from line centre in Doppler widths.  For a
+ * ray traced from its probe in direction w the photons travel along -w, and in every cell
+ *     a = x_l + v.w,  phi = exp(-a^2)/sqrt(pi),  chi = chi_c + chi_line phi,  eta = chi_c S_c + chi_line S_line phi
+ * enter eq. 16.  Flatland only (RC_ERR_BAD_VALUE while inclinations are set).  rc_solve_J, rc_set_boundary,
+ * rc_set_lambda_weights, RC_ACCUM_J work as usual; rc_solve_J_host does not apply. */
+int rc_set_line_atmosphere(rc_ctx *ctx, const float *line, int nx, int ny, const float *x_lambda, int nlambda);
 
 /* Boundary intensity sampled by the top cascade: I_below[l] is seen by rays heading
  * down (omega_y < 0), I_above[l] by rays heading up.  host, [nlambda] each; NULL = 0 (free space,

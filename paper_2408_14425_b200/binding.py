@@ -40,6 +40,7 @@ SYMBOLS = {
     "rc_set_workspace": (C.c_int, [C.c_void_p, C.c_void_p, C.c_size_t]),
     "rc_set_stream": (C.c_int, [C.c_void_p, C.c_void_p]),
     "rc_set_atmosphere": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int]),
+    "rc_set_line_atmosphere": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_int]),
     "rc_set_boundary": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
     "rc_set_lambda_weights": (C.c_int, [C.c_void_p, C.c_void_p]),
     "rc_set_inclinations": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]),
@@ -149,6 +150,19 @@ class RadianceCascades:
         self._keep = (chi, eta)
         self.shape = (ny, nx, L)
 
+    def set_line_atmosphere(self, line, xl):
+        """line: CUDA float32 tensor [ny][nx][6] (borrowed); xl: host array [nlambda] in Doppler widths."""
+        import numpy as np
+        assert line.is_cuda and line.is_contiguous() and line.dim() == 3 and line.shape[2] == 6
+        ny, nx, _ = line.shape
+        x = np.ascontiguousarray(xl, dtype=np.float32)
+        self.ensure_workspace(nx, ny, int(x.size))
+        self.set_stream()
+        self._check(self.lib.rc_set_line_atmosphere(self.handle, C.c_void_p(line.data_ptr()), nx, ny,
+                                                    x.ctypes.data_as(C.c_void_p), int(x.size)))
+        self._keep = (line,)
+        self.shape = (ny, nx, int(x.size))
+
     def set_boundary(self, I_below=None, I_above=None):
         L = self.shape[2]
         a, pa = _host_f32(I_below, L)
@@ -237,11 +251,14 @@ def solve_atmosphere(atm, device=0, lambda_batch=0, flags=0, rc=None):
     fl = flags | (RC_ACCUM_J if atm.accumulate else 0)
     if rc is None:
         rc = RadianceCascades(atm.ncascades, atm.c0_interval, device, lambda_batch, fl)
-    chi = torch.from_numpy(atm.chi).to(dev)
-    eta = torch.from_numpy(atm.eta).to(dev)
-    if getattr(atm, "mu", None) is not None:
-        rc.set_inclinations(atm.mu, atm.w_mu)
-    rc.set_atmosphere(chi, eta)
+    if getattr(atm, "line", None) is not None:
+        rc.set_line_atmosphere(torch.from_numpy(atm.line).to(dev), atm.xl)
+    else:
+        chi = torch.from_numpy(atm.chi).to(dev)
+        eta = torch.from_numpy(atm.eta).to(dev)
+        if getattr(atm, "mu", None) is not None:
+            rc.set_inclinations(atm.mu, atm.w_mu)
+        rc.set_atmosphere(chi, eta)
     rc.set_boundary(atm.I_below, atm.I_above)
     rc.set_lambda_weights(atm.weights)
     J = rc.solve_J()

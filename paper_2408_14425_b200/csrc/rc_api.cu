@@ -33,6 +33,8 @@ struct Plan {
     int NM = 1;                     // inclinations (2.5D); a lane carries LV * NM channels
     int nbands = 1, band_axis = 0;  // L2 banding of the long-ray cascades (1 = off); axis 0 = rows, 1 = columns
     size_t state = 0;               // parked ray state of the banded launches
+    bool line = false;              // velocity-dependent line mode: chiT holds 6 packed line parameters per cell
+    size_t xls = 0;                 // line mode: scaled wavelengths [Lpad]
     size_t occ = 0;                 // occupancy bitmap of the packed cells (0: none, nx ny not a multiple of 32)
     bool has_occ = false;
     CascadePlan c[RC_MAX_CASCADES];
@@ -49,10 +51,16 @@ struct rc_ctx {
     char *ws = nullptr;
     size_t ws_bytes = 0;
     const float *chi = nullptr, *eta = nullptr;
+    const float *line = nullptr;  // line mode: [ny][nx][6], borrowed
     Plan plan{};
     bool have_atm = false;
     int tab_nx = 0, tab_ny = 0;  // shape the step tables in the workspace were built for
     bool host_io = false;
+    // CUDA graph of the launch sequence of small grids (rc_solve_J) and what it was captured for
+    struct GraphKey { const void *J, *chi, *eta, *line, *ws; int nx, ny, L, nm, sparse; size_t total; float f[8], w[8]; };
+    GraphKey graph_key{};
+    cudaGraphExec_t graph_exec = nullptr;
+    cudaStream_t cap_stream = nullptr;
     bool sparse = false;  // most cells have chi == 0 at every wavelength (counted by rc_set_atmosphere): skip their gathers
     // developer overrides (environment, read by rc_create): RC_MARCH_VARIANT = 0..3 (register ring depth /
     // occupancy of march_kernel), RC_PATCH_LOG2 = 2..5 forces the lane patch width for cascades >= RC_PATCH_FROM
@@ -110,7 +118,7 @@ int choose_patch(int nx, int ny, int i, double ta, double tb) {
     while (widest > 0 && (1 << widest) > npx) widest--;
     if (std::fmin(tb, std::hypot((double)nx, (double)ny)) <= std::min(nx, ny) / 16.0) return widest;
     const long long ndir = 1LL << (2 * (i + 1));
-    const int nsample = (int)std::min<long long>(ndir, 128);
+    const int nsample = (int)std::min<long long>(ndir, 32);
     std::vector<double> len((size_t)npx * npy);
     double total = 0.0, cost[6] = {0, 0, 0, 0, 0, 0};
     const int narrowest = std::min(widest, 2);
@@ -156,12 +164,13 @@ int choose_lv(const rc_config &cfg, int L, int nm) {
 }
 
 // Workspace layout for a shape.  When `offs` is given, also fills the per-direction slot offsets.
-bool make_plan(const rc_config &cfg, int nm, int nx, int ny, int L, bool host_io, Plan &P,
-               std::vector<std::vector<long long>> *offs) {
+bool make_plan_uncached(const rc_config &cfg, int nm, bool line, int nx, int ny, int L, bool host_io, Plan &P,
+                        std::vector<std::vector<long long>> *offs) {
     if (!shape_ok(cfg, nx, ny, L)) return false;
     P = Plan{};
     P.nx = nx; P.ny = ny; P.L = L; P.ncasc = cfg.ncascades;
     P.NM = nm;
+    P.line = line;
     P.LV = choose_lv(cfg, L, nm);
     P.nb = (L + P.LV - 1) / P.LV;
     P.Lpad = P.nb * P.LV;
@@ -212,7 +221,7 @@ bool make_plan(const rc_config &cfg, int nm, int nx, int ny, int L, bool host_io
     // L2 banding: one wavelength batch of packed chi and S is ncell * LV * 8 bytes; when that exceeds the
     // L2 budget the cascades with long rays are marched band by band
     {
-        const double batch_mb = (double)ncell * P.LV * 8.0 / (1 << 20);
+        const double batch_mb = line ? 0.0 : (double)ncell * P.LV * 8.0 / (1 << 20);  // line mode: 24 B per cell
         double budget_mb = 72.0;
         if (const char *e = std::getenv("RC_L2_MB")) budget_mb = std::max(1.0, std::atof(e));
         P.nbands = (int)std::ceil(batch_mb / budget_mb);
@@ -232,10 +241,15 @@ bool make_plan(const rc_config &cfg, int nm, int nx, int ny, int L, bool host_io
         }
         if (any) { P.state = cur; cur += 8 * field * P.NM; }
     }
-    P.has_occ = ncell % 32 == 0 && P.NM == 1;
+    P.has_occ = ncell % 32 == 0 && P.NM == 1 && !line;
     if (P.has_occ) { P.occ = cur; cur += align_up((ncell / 32) * P.nb * sizeof(unsigned)); }
-    P.chiT = cur; cur += field;
-    P.ST = cur;   cur += field;
+    if (line) {
+        P.chiT = cur; cur += align_up(ncell * 6 * sizeof(float));
+        P.xls = cur;  cur += align_up(P.Lpad * sizeof(float));
+    } else {
+        P.chiT = cur; cur += field;
+        P.ST = cur;   cur += field;
+    }
     P.A[0] = cur; cur += field * P.NM;  // merged cascades hold every (wavelength, inclination) channel
     P.A[1] = cur; cur += field * P.NM;
     if (cfg.flags & RC_ACCUM_J) { P.Jpart = cur; cur += align_up(ncell * P.nb * sizeof(float)); }
@@ -250,6 +264,27 @@ bool make_plan(const rc_config &cfg, int nm, int nx, int ny, int L, bool host_io
         P.io_J = cur;   cur += (cfg.flags & RC_ACCUM_J) ? align_up(ncell * sizeof(float)) : io;
     }
     P.total = cur;
+    return true;
+}
+
+// The plan is pure host arithmetic but not free (choose_patch); the last few are remembered.
+bool make_plan(const rc_config &cfg, int nm, bool line, int nx, int ny, int L, bool host_io, Plan &P,
+               std::vector<std::vector<long long>> *offs) {
+    struct Entry { double k[13]; Plan p; };
+    static thread_local std::vector<Entry> cache;
+    if (offs) return make_plan_uncached(cfg, nm, line, nx, ny, L, host_io, P, offs);
+    const char *e1 = std::getenv("RC_BANDS"), *e2 = std::getenv("RC_L2_MB");
+    const double k[13] = {(double)cfg.ncascades, (double)cfg.lambda_batch, (double)cfg.flags, (double)nm, (double)line,
+                          (double)nx, (double)ny, (double)L, (double)host_io, (double)cfg.c0_interval,
+                          e1 ? std::atof(e1) : -1.0, e2 ? std::atof(e2) : -1.0, 0.0};
+    for (const Entry &e : cache)
+        if (std::equal(k, k + 13, e.k)) { P = e.p; return true; }
+    if (!make_plan_uncached(cfg, nm, line, nx, ny, L, host_io, P, nullptr)) return false;
+    if (cache.size() >= 16) cache.erase(cache.begin());
+    Entry en;
+    std::copy(k, k + 13, en.k);
+    en.p = P;
+    cache.push_back(en);
     return true;
 }
 
@@ -293,10 +328,10 @@ int rc_create(rc_ctx **out, const rc_config *cfg) {
 
 int rc_destroy(rc_ctx *ctx) {
     if (!ctx) return RC_ERR_NULL_ARG;
-    if (!ctx->ev.empty()) {
-        cudaSetDevice(ctx->cfg.device);
-        for (auto &e : ctx->ev) cudaEventDestroy(e);
-    }
+    if (!ctx->ev.empty() || ctx->graph_exec || ctx->cap_stream) cudaSetDevice(ctx->cfg.device);
+    for (auto &e : ctx->ev) cudaEventDestroy(e);
+    if (ctx->graph_exec) cudaGraphExecDestroy(ctx->graph_exec);
+    if (ctx->cap_stream) cudaStreamDestroy(ctx->cap_stream);
     delete ctx;
     return RC_OK;
 }
@@ -304,8 +339,10 @@ int rc_destroy(rc_ctx *ctx) {
 size_t rc_workspace_bytes(const rc_ctx *ctx, int nx, int ny, int nlambda, int host_io) {
     if (!ctx) return 0;
     Plan P;
-    if (!make_plan(ctx->cfg, ctx->nm, nx, ny, nlambda, host_io != 0, P, nullptr)) return 0;
-    return P.total;
+    if (!make_plan(ctx->cfg, ctx->nm, false, nx, ny, nlambda, host_io != 0, P, nullptr)) return 0;
+    size_t need = P.total;
+    if (ctx->nm == 1 && make_plan(ctx->cfg, 1, true, nx, ny, nlambda, false, P, nullptr)) need = std::max(need, P.total);  // line mode
+    return need;
 }
 
 int rc_set_workspace(rc_ctx *ctx, void *dev_ptr, size_t bytes) {
@@ -339,21 +376,21 @@ int rc_set_timing(rc_ctx *ctx, int nsets) {
     return RC_OK;
 }
 
-int rc_set_atmosphere(rc_ctx *ctx, const float *chi, const float *eta, int nx, int ny, int nlambda) {
-    if (!ctx || !chi || !eta) return ctx ? fail(ctx, RC_ERR_NULL_ARG, "null chi/eta") : RC_ERR_NULL_ARG;
+// Plan, step tables and defaults for a shape (shared by rc_set_atmosphere and rc_set_line_atmosphere).
+static int prepare_shape(rc_ctx *ctx, int nx, int ny, int nlambda, bool line) {
     if (!shape_ok(ctx->cfg, nx, ny, nlambda))
         return fail(ctx, RC_ERR_BAD_SHAPE, "nx=%d ny=%d nlambda=%d: need positive multiples of 2^(ncascades-1)=%d, <= %d",
                     nx, ny, nlambda, 1 << (ctx->cfg.ncascades - 1), RC_MAX_DIM);
     if (!ctx->ws) return fail(ctx, RC_ERR_NO_WORKSPACE, "rc_set_workspace has not been called");
     RC_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
-    const bool same_shape = ctx->have_atm && ctx->plan.nx == nx && ctx->plan.ny == ny && ctx->plan.L == nlambda;
+    const bool same_shape = ctx->have_atm && ctx->plan.nx == nx && ctx->plan.ny == ny && ctx->plan.L == nlambda && ctx->plan.line == line;
     if (!same_shape) {
         Plan P, Pio;
         std::vector<std::vector<long long>> offs;
-        make_plan(ctx->cfg, ctx->nm, nx, ny, nlambda, false, P, &offs);
+        make_plan(ctx->cfg, ctx->nm, line, nx, ny, nlambda, false, P, &offs);
         if (P.total > ctx->ws_bytes)
             return fail(ctx, RC_ERR_NO_WORKSPACE, "workspace has %zu bytes, %zu needed", ctx->ws_bytes, P.total);
-        make_plan(ctx->cfg, ctx->nm, nx, ny, nlambda, true, Pio, nullptr);
+        make_plan(ctx->cfg, ctx->nm, line, nx, ny, nlambda, true, Pio, nullptr);
         ctx->host_io = Pio.total <= ctx->ws_bytes;
         ctx->plan = ctx->host_io ? Pio : P;
         ctx->have_atm = false;
@@ -388,6 +425,16 @@ int rc_set_atmosphere(rc_ctx *ctx, const float *chi, const float *eta, int nx, i
                                      cudaMemcpyHostToDevice, ctx->stream));
         RC_CUDA(ctx, cudaStreamSynchronize(ctx->stream));  // `ones` and the offsets are host temporaries
     }
+    return RC_OK;
+}
+
+int rc_set_atmosphere(rc_ctx *ctx, const float *chi, const float *eta, int nx, int ny, int nlambda) {
+    if (!ctx || !chi || !eta) return ctx ? fail(ctx, RC_ERR_NULL_ARG, "null chi/eta") : RC_ERR_NULL_ARG;
+    {
+        const int rc = prepare_shape(ctx, nx, ny, nlambda, false);
+        if (rc != RC_OK) return rc;
+    }
+    ctx->line = nullptr;
     if (ctx->cfg.flags & RC_VALIDATE) {
         int *flag = (int *)(ctx->ws + ctx->plan.flag);
         int h = 0;
@@ -406,7 +453,7 @@ int rc_set_atmosphere(rc_ctx *ctx, const float *chi, const float *eta, int nx, i
         ctx->sparse = false;
         if (ctx->plan.has_occ && !std::getenv("RC_NO_SPARSE")) {
             RC_CUDA(ctx, cudaMemsetAsync(cnt, 0, sizeof(*cnt), ctx->stream));
-            RC_CUDA(ctx, rc::launch_count_empty(chi, (long long)nx * ny, nlambda, cnt, ctx->stream));
+            RC_CUDA(ctx, rc::launch_count_empty(chi, (long long)nx * ny, nlambda, (int *)(ctx->ws + ctx->plan.A[0]), cnt, ctx->stream));  // A[0] is free between solves
             RC_CUDA(ctx, cudaMemcpyAsync(&h, cnt, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream));
             RC_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
             ctx->sparse = 3 * h > 2ULL * nx * ny || std::getenv("RC_FORCE_SPARSE");
@@ -415,6 +462,27 @@ int rc_set_atmosphere(rc_ctx *ctx, const float *chi, const float *eta, int nx, i
     }
     ctx->chi = chi;
     ctx->eta = eta;
+    ctx->have_atm = true;
+    return RC_OK;
+}
+
+// Velocity-dependent line mode.
+int rc_set_line_atmosphere(rc_ctx *ctx, const float *line, int nx, int ny, const float *x_lambda, int nlambda) {
+    if (!ctx || !line || !x_lambda) return ctx ? fail(ctx, RC_ERR_NULL_ARG, "null line / x_lambda") : RC_ERR_NULL_ARG;
+    if (ctx->nm != 1) return fail(ctx, RC_ERR_BAD_VALUE, "line mode with inclinations is not supported: call rc_set_inclinations(ctx, 1, NULL, NULL)");
+    {
+        const int rc = prepare_shape(ctx, nx, ny, nlambda, true);
+        if (rc != RC_OK) return rc;
+    }
+    for (int l = 0; l < nlambda; l++)
+        if (!std::isfinite(x_lambda[l])) return fail(ctx, RC_ERR_BAD_VALUE, "x_lambda[%d] is not finite", l);
+    std::vector<float> h((size_t)ctx->plan.Lpad, 0.f);
+    for (int l = 0; l < nlambda; l++) h[l] = (float)((double)x_lambda[l] * 1.2011224087864498);  // sqrt(log2 e)
+    RC_CUDA(ctx, cudaMemcpyAsync(ctx->ws + ctx->plan.xls, h.data(), h.size() * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
+    RC_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    ctx->line = line;
+    ctx->chi = ctx->eta = nullptr;
+    ctx->sparse = false;
     ctx->have_atm = true;
     return RC_OK;
 }
@@ -469,6 +537,8 @@ static rc::MarchParams march_params(const rc_ctx *ctx, int i, float *J_out) {
     rc::MarchParams mp;
     mp.chiT = (const float *)(ctx->ws + P.chiT);
     mp.ST = (const float *)(ctx->ws + P.ST);
+    mp.linepk = ctx->line ? (const float *)(ctx->ws + P.chiT) : nullptr;
+    mp.xls = ctx->line ? (const float *)(ctx->ws + P.xls) : nullptr;
     mp.occ = ctx->sparse && P.has_occ && !c.empty ? (const unsigned *)(ctx->ws + P.occ) : nullptr;
     mp.Aup = i == top ? nullptr : (const float *)(ctx->ws + P.A[(i + 1) & 1]);
     mp.out = i > 0 ? (float *)(ctx->ws + P.A[i & 1]) : (accum ? (float *)(ctx->ws + P.Jpart) : J_out);
@@ -500,10 +570,7 @@ static rc::MarchParams march_params(const rc_ctx *ctx, int i, float *J_out) {
 // One full solve: for cascade i = top .. 0 { pack chi/eta for spacing 2^i ; march + merge }  (PAPER.md:207:
 // "after calculation, each interval of cascade i merges with the child intervals of cascade i+1.
 // Cascade i-1 is then computed and merged with cascade i").
-int rc_solve_J(rc_ctx *ctx, float *J_out) {
-    if (!ctx || !J_out) return ctx ? fail(ctx, RC_ERR_NULL_ARG, "null J_out") : RC_ERR_NULL_ARG;
-    if (!ctx->have_atm) return fail(ctx, RC_ERR_NO_ATMOSPHERE, "call rc_set_atmosphere first");
-    RC_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+static int enqueue_solve(rc_ctx *ctx, float *J_out) {
     const Plan &P = ctx->plan;
     const int top = ctx->cfg.ncascades - 1;
     const bool accum = (ctx->cfg.flags & RC_ACCUM_J) != 0;
@@ -519,7 +586,12 @@ int rc_solve_J(rc_ctx *ctx, float *J_out) {
             pp.chiT = (float *)(ctx->ws + P.chiT); pp.ST = (float *)(ctx->ws + P.ST);
             pp.occ = ctx->sparse && P.has_occ ? (unsigned *)(ctx->ws + P.occ) : nullptr;
             pp.nx = P.nx; pp.ny = P.ny; pp.L = P.L; pp.nb = P.nb; pp.shift = i;
-            RC_CUDA(ctx, rc::launch_pack(pp, P.LV, ctx->stream));
+            if (ctx->line) {
+                pp.chi = ctx->line; pp.eta = nullptr; pp.occ = nullptr;
+                RC_CUDA(ctx, rc::launch_pack_line(pp, ctx->stream));
+            } else {
+                RC_CUDA(ctx, rc::launch_pack(pp, P.LV, ctx->stream));
+            }
             launches++;
         }
         if (ev) RC_CUDA(ctx, cudaEventRecord(ev[1 + 2 * (top - i)], ctx->stream));
@@ -562,6 +634,51 @@ int rc_solve_J(rc_ctx *ctx, float *J_out) {
     return RC_OK;
 }
 
+// Small grids are launch bound (config 0: 11 launches of a few microseconds each): their launch sequence is
+// captured once into a CUDA graph (on a private stream, so the caller's stream may be the legacy default
+// stream) and replayed into the caller's stream until anything the launches depend on changes.
+int rc_solve_J(rc_ctx *ctx, float *J_out) {
+    if (!ctx || !J_out) return ctx ? fail(ctx, RC_ERR_NULL_ARG, "null J_out") : RC_ERR_NULL_ARG;
+    if (!ctx->have_atm) return fail(ctx, RC_ERR_NO_ATMOSPHERE, "call rc_set_atmosphere first");
+    RC_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    const Plan &P = ctx->plan;
+    bool use_graph = ctx->nsets == 0 && (long long)P.nx * P.ny * P.Lpad * P.NM <= (1LL << 21) && !std::getenv("RC_NO_GRAPH");
+    if (use_graph) {
+        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+        if (cudaStreamIsCapturing(ctx->stream, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) {
+            cudaGetLastError();
+            use_graph = false;  // the caller is capturing us: just enqueue
+        }
+    }
+    if (!use_graph) return enqueue_solve(ctx, J_out);
+    rc_ctx::GraphKey key;
+    std::memset(&key, 0, sizeof(key));
+    key.J = J_out; key.chi = ctx->chi; key.eta = ctx->eta; key.line = ctx->line; key.ws = ctx->ws;
+    key.nx = P.nx; key.ny = P.ny; key.L = P.L; key.nm = P.NM; key.sparse = ctx->sparse; key.total = P.total;
+    for (int m = 0; m < 8; m++) { key.f[m] = ctx->incl_f[m]; key.w[m] = ctx->incl_w[m]; }
+    if (!ctx->graph_exec || std::memcmp(&key, &ctx->graph_key, sizeof(key)) != 0) {
+        if (ctx->graph_exec) { cudaGraphExecDestroy(ctx->graph_exec); ctx->graph_exec = nullptr; }
+        if (!ctx->cap_stream) RC_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->cap_stream, cudaStreamNonBlocking));
+        cudaStream_t user = ctx->stream;
+        ctx->stream = ctx->cap_stream;
+        cudaGraph_t g = nullptr;
+        cudaError_t e = cudaStreamBeginCapture(ctx->cap_stream, cudaStreamCaptureModeThreadLocal);
+        int rc = e == cudaSuccess ? enqueue_solve(ctx, J_out) : RC_ERR_CUDA;
+        cudaError_t e2 = e == cudaSuccess ? cudaStreamEndCapture(ctx->cap_stream, &g) : e;
+        ctx->stream = user;
+        if (rc == RC_OK && e2 == cudaSuccess && g) e2 = cudaGraphInstantiate(&ctx->graph_exec, g, 0);
+        if (g) cudaGraphDestroy(g);
+        if (rc != RC_OK || e2 != cudaSuccess || !ctx->graph_exec) {
+            cudaGetLastError();
+            ctx->graph_exec = nullptr;
+            return enqueue_solve(ctx, J_out);  // no graph: plain launches
+        }
+        ctx->graph_key = key;
+    }
+    RC_CUDA(ctx, cudaGraphLaunch(ctx->graph_exec, ctx->stream));
+    return RC_OK;
+}
+
 // Geometric segment count per cascade and wavelength (the unit of the throughput metric).
 int rc_count_segments(rc_ctx *ctx, int64_t *per_cascade) {
     if (!ctx || !per_cascade) return ctx ? fail(ctx, RC_ERR_NULL_ARG, "null output") : RC_ERR_NULL_ARG;
@@ -585,7 +702,7 @@ int rc_solve_J_host(rc_ctx *ctx, const float *chi_host, const float *eta_host, i
     if (!ctx->ws) return fail(ctx, RC_ERR_NO_WORKSPACE, "rc_set_workspace has not been called");
     RC_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
     Plan Pio;
-    make_plan(ctx->cfg, ctx->nm, nx, ny, nlambda, true, Pio, nullptr);
+    make_plan(ctx->cfg, ctx->nm, false, nx, ny, nlambda, true, Pio, nullptr);
     if (Pio.total > ctx->ws_bytes)
         return fail(ctx, RC_ERR_NO_WORKSPACE, "workspace has %zu bytes, %zu needed with host_io", ctx->ws_bytes, Pio.total);
     const size_t n = (size_t)nx * ny * nlambda * sizeof(float);

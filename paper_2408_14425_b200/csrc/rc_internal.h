@@ -32,6 +32,8 @@ struct CascadeTable {
 struct MarchParams {
     const float *chiT;  // packed opacity * log2(e): [nb][s][s][npy][npx][LV]  (phase (y mod s, x mod s), then y div s, x div s)
     const float *ST;    // packed source function eta/chi, same layout
+    const float *linepk;  // null, or line mode: packed line parameters [s][s][npy][npx][6] (pack_line_kernel)
+    const float *xls;     // line mode: [Lpad] wavelengths x_l * sqrt(log2 e), device
     const unsigned *occ;  // null (dense), or the occupancy bitmap pack_kernel wrote: empty cells are not gathered
     const float *Aup;   // merged cascade i+1, pre-averaged over the 4 children: [nb][N_i][npy/2][npx/2][LV]; null on the top cascade
     float *out;         // mode 0: A_i [nb][N_i/4][npy][npx][LV]; mode 1: J [ny][nx][L]; mode 2: Jpart [nb][ny][nx]
@@ -79,12 +81,13 @@ struct TableBuildParams {
 
 // launchers (rc_kernels.cu); LV in {1,2,4,8}
 cudaError_t launch_pack(const PackParams &p, int LV, cudaStream_t st);
+cudaError_t launch_pack_line(const PackParams &p, cudaStream_t st);  // p.chi = line [ny][nx][6], p.chiT = packed [..][6]
 cudaError_t launch_march(const MarchParams &p, int LV, int NM, int variant, cudaStream_t st);
 cudaError_t launch_table_build(const TableBuildParams &p, cudaStream_t st);
 cudaError_t launch_reduce_jbar(const float *Jpart, float *Jbar, long long ncell, int nb, cudaStream_t st);
 cudaError_t launch_count(const MarchParams &p, unsigned long long *total, cudaStream_t st);
 cudaError_t launch_gather_probe(const float *buf, unsigned long long nsector, int iters, int blocks, float *sink, cudaStream_t st);
-cudaError_t launch_count_empty(const float *chi, long long ncell, int L, unsigned long long *count, cudaStream_t st);
+cudaError_t launch_count_empty(const float *chi, long long ncell, int L, int *mark, unsigned long long *count, cudaStream_t st);
 cudaError_t launch_validate(const float *chi, const float *eta, long long n, int *flag, cudaStream_t st);
 
 }  // namespace rc

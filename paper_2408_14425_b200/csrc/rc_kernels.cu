@@ -226,6 +226,36 @@ __global__ void __launch_bounds__(256) pack_kernel(PackParams p) {
     }
 }
 
+// Line mode: line [y][x][6] = chi_c, S_c, chi_line, S_line, v_x, v_y  ->  phase-plane layout, 6 floats per cell:
+// chi_c log2e, chi_c log2e S_c, chi_line log2e/sqrt(pi), chi_line log2e/sqrt(pi) S_line, v_x sqrt(log2e), v_y sqrt(log2e)
+// (tau in units of ln 2; phi(a) = 2^-(a sqrt(log2e))^2 / sqrt(pi)).
+__global__ void __launch_bounds__(256) pack_line_kernel(PackParams p) {
+    const long long ncell = (long long)p.nx * p.ny;
+    const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= ncell) return;
+    const int npx = p.nx >> p.shift, npy = p.ny >> p.shift, smask = (1 << p.shift) - 1;
+    const int xd = (int)(c % npx);
+    long long t = c / npx;
+    const int yd = (int)(t % npy);
+    t /= npy;
+    const int xm = (int)t & smask, ym = (int)(t >> p.shift);
+    const int x = (xd << p.shift) + xm, y = (yd << p.shift) + ym;
+    const float2 *src = reinterpret_cast<const float2 *>(p.chi + ((long long)y * p.nx + x) * 6);
+    const float2 a = __ldg(src), b = __ldg(src + 1), v = __ldg(src + 2);
+    const float L2E = 1.4426950408889634f, RSPI = 0.5641895835477563f, SL2E = 1.2011224087864498f;
+    const float cc = a.x * L2E, cl = b.x * L2E * RSPI;
+    float2 *dst = reinterpret_cast<float2 *>(p.chiT + c * 6);
+    dst[0] = make_float2(cc, cc * a.y);
+    dst[1] = make_float2(cl, cl * b.y);
+    dst[2] = make_float2(v.x * SL2E, v.y * SL2E);
+}
+
+cudaError_t launch_pack_line(const PackParams &p, cudaStream_t st) {
+    const long long n = (long long)p.nx * p.ny;
+    pack_line_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(p);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_pack(const PackParams &p, int LV, cudaStream_t st) {
     const long long n = (long long)p.nx * p.ny * p.nb;
     const unsigned blocks = (unsigned)((n + 255) / 256);
@@ -356,7 +386,7 @@ __device__ __forceinline__ int first_step_reaching(const StepXY *xy, int n, int 
 // half of the directions that crosses the bands in ascending (or descending) order; a ray's (I, tau)
 // is carried from band to band through `state`, so the arithmetic - and the result - is that of the
 // unbanded launch, bit for bit, while the cells gathered by one launch fit L2.
-template <int LV, int NM, int PD, int WARPS, int MINB, bool BANDED, bool SPARSE>
+template <int LV, int NM, int PD, int WARPS, int MINB, bool BANDED, bool SPARSE, bool LINE>
 __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) {
     // sum over the 4 child directions, per thread: parked in shared memory between children so the
     // marching loop has the registers to itself
@@ -374,8 +404,16 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
     const long long ncell = (long long)p.nx * p.ny;
     // packed layout [batch][y mod s][x mod s][y div s][x div s][LV]: the lane's probe owns cell
     // (y div s, x div s) = (b, a) of every phase plane; a step's delta is lane-independent
-    const float *chiB = p.chiT + (long long)nbI * ncell * LL;  // warp-uniform
-    const float *SB = p.ST + (long long)nbI * ncell * LL;
+    const float *chiB = LINE ? p.linepk : p.chiT + (long long)nbI * ncell * LL;  // warp-uniform
+    const float *SB = LINE ? nullptr : p.ST + (long long)nbI * ncell * LL;
+    // LINE: the packed cell holds the 6 line parameters; chi and S of each wavelength are
+    // evaluated per step from the velocity projected on this ray.  xs = x_l sqrt(log2 e) of the lane's wavelengths.
+    constexpr int NR = LINE ? 6 : LL;  // floats gathered per cell
+    float xs[LINE ? LV : 1];
+    if constexpr (LINE) {
+#pragma unroll
+        for (int v = 0; v < LV; v++) xs[v] = __ldg(p.xls + nbI * LV + v);
+    }
     const unsigned *occB = SPARSE ? p.occ + (long long)nbI * (ncell >> 5) : nullptr;
     // (dx, dy) ranges that keep this lane's ray inside the box
     const int dxlo = -(a << p.shift) - half, dxhi = ((p.npx - a) << p.shift) - 1 - half;
@@ -418,21 +456,40 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
                 n0 = has ? n0 - w0 : 0;
             }
             const int nw = __reduce_max_sync(FULL, nin);  // steps this warp walks
-            float c2[PD][LL], S[PD][LL], ds[PD];
+            float c2[PD][NR], S[PD][LINE ? 1 : LL], ds[PD];
+            // LINE: photons on this ray travel along -(wx, wy); the line of a cell moving with v is centred at
+            // x = -v.w, so a = x_l + v.w  (packed v and x_l carry the factor sqrt(log2 e): phi ~ 2^(-a^2))
+            float wx = 0.f, wy = 0.f;
+            if constexpr (LINE) sincospif(2.f * ((float)k + 0.5f) / (float)(4LL * p.ngroups), &wy, &wx);
+            auto gather = [&](int u, unsigned delta, bool in) {
+                if constexpr (LINE) {
+                    const float *src = reinterpret_cast<const float *>(reinterpret_cast<const char *>(chiB) +
+                                                                        (unsigned long long)(probe + delta) * 24ull);
+                    float t0[2] = {c2[u][0], c2[u][1]}, t1[2] = {c2[u][2], c2[u][3]}, t2[2] = {c2[u][4], c2[u][5]};
+                    load_vec_if<2>(src, t0, in);
+                    load_vec_if<2>(src + 2, t1, in);
+                    load_vec_if<2>(src + 4, t2, in);
+                    c2[u][0] = t0[0]; c2[u][1] = t0[1]; c2[u][2] = t1[0]; c2[u][3] = t1[1]; c2[u][4] = t2[0]; c2[u][5] = t2[1];
+                } else {
+                    const unsigned long long d = (unsigned long long)(probe + delta) * (LL * sizeof(float));
+                    load_vec_if<LL>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(chiB) + d), c2[u], in);
+                    load_vec_if<LL>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(SB) + d), S[u], in);
+                }
+            };
             // prologue: steps 0 .. PD-1 into the ring (the table has 2 PD spare entries at its end)
 #pragma unroll
             for (int u = 0; u < PD; u++) {
 #pragma unroll
-                for (int v = 0; v < LL; v++) { c2[u][v] = 0.f; S[u][v] = 0.f; }
+                for (int v = 0; v < NR; v++) c2[u][v] = 0.f;
+#pragma unroll
+                for (int v = 0; v < (LINE ? 1 : LL); v++) S[u][v] = 0.f;
                 const uint2 e = __ldg(tab + u);
                 bool in = u < nin && (!BANDED || u >= n0);
                 if constexpr (SPARSE) {  // empty cells (chi = 0 at every wavelength of the batch) are not gathered
                     const unsigned c = probe + e.x;
                     if (in) in = (__ldg(occB + (c >> 5)) >> (c & 31)) & 1u;
                 }
-                const unsigned long long d = (unsigned long long)(probe + e.x) * (LL * sizeof(float));
-                load_vec_if<LL>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(chiB) + d), c2[u], in);
-                load_vec_if<LL>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(SB) + d), S[u], in);
+                gather(u, e.x, in);
                 ds[u] = in ? __uint_as_float(e.y) : 0.f;
             }
             int chk = 0;
@@ -465,7 +522,22 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
                     float dsm[NM];
 #pragma unroll
                     for (int m = 0; m < NM; m++) dsm[m] = NM == 1 ? ds[u] : ds[u] * p.incl_f[m];
-                    if (!SPARSE || __any_sync(FULL, ds[u] != 0.f)) {  // SPARSE: no lane has an occupied cell: nothing to do
+                    if constexpr (LINE) {
+                        // packed cell: chi_c', chi_c' S_c, chi_line', chi_line' S_line, v_x', v_y'   (' = scaled, pack_line_kernel)
+                        const float vw = fmaf(c2[u][4], wx, c2[u][5] * wy);
+#pragma unroll
+                        for (int v = 0; v < LV; v++) {
+                            const float aa = xs[v] + vw;
+                            const float phi = ex2_neg(aa * aa);
+                            const float chi2 = fmaf(c2[u][2], phi, c2[u][0]);
+                            const float num = fmaf(c2[u][3], phi, c2[u][1]);
+                            const float Sv = chi2 > 0.f ? __fdividef(num, chi2) : 0.f;  // eta/chi; vacuum emits nothing
+                            tau[v] = fmaf(chi2, dsm[0], tau[v]);
+                            const float Tn = ex2_neg(tau[v]);
+                            I[v] = fmaf(Sv, T[v] - Tn, I[v]);
+                            T[v] = Tn;
+                        }
+                    } else if (!SPARSE || __any_sync(FULL, ds[u] != 0.f)) {  // SPARSE: no lane has an occupied cell: nothing to do
 #pragma unroll
                         for (int v = 0; v < LV; v++) {
                             tau[v] = fmaf(c2[u][v / NM], dsm[v % NM], tau[v]);
@@ -477,9 +549,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
                     // refill the slot with step st + u + PD
                     bool in = st + u + PD < nin && (!BANDED || st + u + PD >= n0);
                     if constexpr (SPARSE) in = in && ((occ_cur >> ((probe + en.x) & 31)) & 1u);
-                    const unsigned long long d = (unsigned long long)(probe + en.x) * (LL * sizeof(float));
-                    load_vec_if<LL>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(chiB) + d), c2[u], in);
-                    load_vec_if<LL>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(SB) + d), S[u], in);
+                    gather(u, en.x, in);
                     ds[u] = in ? __uint_as_float(en.y) : 0.f;
                 }
                 if (p.early_exit && (++chk & 3) == 0) {
@@ -576,9 +646,9 @@ static cudaError_t launch_march_variant(const MarchParams &p, cudaStream_t st) {
     const long long blocks = (march_warps(p) + WARPS - 1) / WARPS;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     if (p.state != nullptr)
-        march_kernel<LV, NM, PD, WARPS, MINB, true, false><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
+        march_kernel<LV, NM, PD, WARPS, MINB, true, false, false><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
     else
-        march_kernel<LV, NM, PD, WARPS, MINB, false, false><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
+        march_kernel<LV, NM, PD, WARPS, MINB, false, false, false><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
     return cudaGetLastError();
 }
 
@@ -591,14 +661,25 @@ static cudaError_t launch_march_sparse(const MarchParams &p, cudaStream_t st) {
     const long long blocks = (march_warps(p) + WARPS - 1) / WARPS;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     if (p.state != nullptr)
-        march_kernel<LV, 1, 3, WARPS, 2, true, true><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
+        march_kernel<LV, 1, 3, WARPS, 2, true, true, false><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
     else
-        march_kernel<LV, 1, 3, WARPS, 2, false, true><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
+        march_kernel<LV, 1, 3, WARPS, 2, false, true, false><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
+    return cudaGetLastError();
+}
+
+// Velocity-dependent line mode (linepk != null): 3 MUFU per segment-wavelength, ring of 2, 24 warps/SM.
+template <int LV>
+static cudaError_t launch_march_line(const MarchParams &p, cudaStream_t st) {
+    constexpr int WARPS = 8;
+    const long long blocks = (march_warps(p) + WARPS - 1) / WARPS;
+    if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+    march_kernel<LV, 1, 2, WARPS, 3, false, false, true><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
     return cudaGetLastError();
 }
 
 template <int LV>
 static cudaError_t launch_march_flat(const MarchParams &p, int variant, cudaStream_t st) {
+    if (p.linepk != nullptr) return launch_march_line<LV>(p, st);
     if (p.occ != nullptr) return launch_march_sparse<LV>(p, st);
     switch (variant) {
         case 0: return launch_march_variant<LV, 1, 2, 8, 3>(p, st);
@@ -660,19 +741,38 @@ __global__ void validate_kernel(const float *chi, const float *eta, long long n,
 }
 
 // Number of cells with chi == 0 at every wavelength (rc_set_atmosphere: is the atmosphere mostly empty?).
-__global__ void count_empty_kernel(const float *chi, long long ncell, int L, unsigned long long *count) {
-    unsigned long long mine = 0;
-    for (long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x; c < ncell; c += (long long)gridDim.x * blockDim.x) {
-        bool empty = true;
-        for (int l = 0; l < L; l++) empty = empty && chi[c * L + l] == 0.f;
-        mine += empty;
+// Pass 1 marks the cells that have a non-zero value (coalesced over the whole array), pass 2 counts the rest.
+template <int W>  // floats per thread: 4 when nlambda is a multiple of 4, else 1
+__global__ void mark_occupied_kernel(const float *chi, long long nchunk, int chunks_per_cell, int *mark) {
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < nchunk; i += (long long)gridDim.x * blockDim.x) {
+        bool nz;
+        if constexpr (W == 4) {
+            const float4 v = __ldg(reinterpret_cast<const float4 *>(chi) + i);
+            nz = v.x != 0.f || v.y != 0.f || v.z != 0.f || v.w != 0.f;
+        } else {
+            nz = __ldg(chi + i) != 0.f;
+        }
+        if (nz) mark[i / chunks_per_cell] = 1;
     }
+}
+
+__global__ void count_unmarked_kernel(const int *mark, long long ncell, unsigned long long *count) {
+    unsigned long long mine = 0;
+    for (long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x; c < ncell; c += (long long)gridDim.x * blockDim.x)
+        mine += mark[c] == 0;
     for (int o = 16; o > 0; o >>= 1) mine += __shfl_down_sync(FULL, mine, o);
     if ((threadIdx.x & 31) == 0 && mine) atomicAdd(count, mine);
 }
 
-cudaError_t launch_count_empty(const float *chi, long long ncell, int L, unsigned long long *count, cudaStream_t st) {
-    count_empty_kernel<<<148 * 8, 256, 0, st>>>(chi, ncell, L, count);
+// mark: scratch of ncell ints (device); count: zeroed by the caller
+cudaError_t launch_count_empty(const float *chi, long long ncell, int L, int *mark, unsigned long long *count, cudaStream_t st) {
+    cudaError_t e = cudaMemsetAsync(mark, 0, sizeof(int) * (size_t)ncell, st);
+    if (e != cudaSuccess) return e;
+    if (L % 4 == 0 && (reinterpret_cast<uintptr_t>(chi) & 15) == 0)
+        mark_occupied_kernel<4><<<148 * 16, 256, 0, st>>>(chi, ncell * (L / 4), L / 4, mark);
+    else
+        mark_occupied_kernel<1><<<148 * 16, 256, 0, st>>>(chi, ncell * L, L, mark);
+    count_unmarked_kernel<<<148 * 4, 256, 0, st>>>(mark, ncell, count);
     return cudaGetLastError();
 }
 

@@ -285,3 +285,61 @@ def test_sparse_march_is_bit_identical(oracle, monkeypatch, bands):
     ref = gpu_solve(dense)
     monkeypatch.setenv("RC_FORCE_SPARSE", "1")
     assert np.array_equal(ref, gpu_solve(dense))
+
+
+# ------------------------------------------------------------------ moving line (f1)
+@pytest.mark.parametrize("kw", [
+    dict(nx=128, ny=128, nlambda=16, ncascades=6),
+    dict(nx=192, ny=64, nlambda=11, ncascades=5),
+    dict(nx=64, ny=64, nlambda=1, ncascades=5),
+])
+def test_moving_line_matches_the_oracle(oracle, kw):
+    """line opacity and emissivity evaluated on the fly from the velocity projected on each ray
+    (rc_set_line_atmosphere), against the oracle's per-ray evaluation; ragged wavelength batches."""
+    atm = A.line_config2(**kw)
+    atm.I_below[:] = 0.3
+    e = check(atm, oracle)
+    print(atm.name, kw, "max rel err", e)
+
+
+def test_static_line_equals_givenfs_path(oracle):
+    """v = 0: the line mode and the GivenFs mode (chi, eta precomputed on the host) agree to fp32 rounding."""
+    atm = A.line_config2(nx=64, ny=64, nlambda=8, ncascades=5)
+    atm.line[..., 4:6] = 0.0
+    Jl = gpu_solve(atm)
+    f = atm.line.astype(np.float64)
+    phi = np.exp(-atm.xl ** 2) / np.sqrt(np.pi)
+    chi = f[..., 0:1] + f[..., 2:3] * phi
+    eta = f[..., 0:1] * f[..., 1:2] + f[..., 2:3] * f[..., 3:4] * phi
+    import dataclasses
+    flat = dataclasses.replace(atm, line=None, xl=None, chi=chi.astype(np.float32), eta=eta.astype(np.float32))
+    Jf = gpu_solve(flat)
+    assert np.max(np.abs(Jl / Jf - 1)) < 2e-5
+
+
+# ------------------------------------------------------------------ CUDA graph replay (small grids)
+def test_graph_replay_matches_plain_launches(monkeypatch):
+    """Small grids replay a captured CUDA graph of the launch sequence.  Same bits as plain launches
+    (RC_NO_GRAPH), on first use and on replay; boundary / weights updates (device buffers the kernels read)
+    take effect without re-capture; a new atmosphere or output buffer re-captures."""
+    import torch
+    from paper_2408_14425_b200 import binding
+    atm = A.make_config(3, nx=64, ny=64, nlambda=3, ncascades=5)
+    monkeypatch.setenv("RC_NO_GRAPH", "1")
+    ref = gpu_solve(atm)
+    atm2 = A.make_config(0, nx=64, ny=64, nlambda=3, ncascades=5, seed=5)
+    ref2 = gpu_solve(atm2)
+    monkeypatch.delenv("RC_NO_GRAPH")
+    J, rc = binding.solve_atmosphere(atm)
+    assert np.array_equal(J.cpu().numpy(), ref)
+    J2 = rc.solve_J(out=J)                                   # replay into the same buffer
+    torch.cuda.synchronize()
+    assert np.array_equal(J2.cpu().numpy(), ref)
+    rc.set_boundary(np.zeros(3, np.float32), None)           # config 3 is lit from below: J must change
+    dark = rc.solve_J().cpu().numpy()                        # new output buffer: re-capture
+    assert not np.array_equal(dark, ref)
+    rc.set_boundary(atm.I_below, atm.I_above)
+    assert np.array_equal(rc.solve_J().cpu().numpy(), ref)
+    Jb, _ = binding.solve_atmosphere(atm2, rc=rc)            # new atmosphere on the same context
+    assert np.array_equal(Jb.cpu().numpy(), ref2)
+    rc.close()
