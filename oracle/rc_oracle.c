@@ -64,6 +64,9 @@ typedef struct {
        seen by a ray are those of cell_chi_eta() below */
     const float *line;  /* [ny][nx][6]: chi_c, S_c, chi_line, S_line, v_x, v_y (velocities in Doppler widths) */
     const double *xl;   /* [L] wavelengths as offsets from line centre, in Doppler widths */
+    double vel_scale;   /* 2.5D line mode: an inclined ray with direction cosine mu to the invariant axis has the
+                           in-plane direction sqrt(1-mu^2) (wx, wy); velocities are in the plane, so v.n is scaled by
+                           sqrt(1-mu^2) = 1/path_scale.  1 in flatland. */
 } grid_t;
 
 /* Opacity and emissivity of cell `cell` at wavelength l for the photons that travel along a ray traced
@@ -79,7 +82,7 @@ static void cell_chi_eta(const grid_t *g, int cell, int l, double wx, double wy,
         return;
     }
     const float *f = g->line + (size_t)cell * 6;
-    double a = g->xl[l] + ((double)f[4] * wx + (double)f[5] * wy);
+    double a = g->xl[l] + g->vel_scale * ((double)f[4] * wx + (double)f[5] * wy);
     double phi = exp(-a * a) / sqrt(M_PI);
     *chi = (double)f[0] + (double)f[2] * phi;
     *eta = (double)f[0] * (double)f[1] + (double)f[2] * (double)f[3] * phi;
@@ -227,7 +230,7 @@ int rc_oracle_ray_segments(int nx, int ny, double px, double py, double theta, i
 int rc_oracle_interval(const float *chi, const float *eta, int nx, int ny, int L, double px,
                        double py, double theta, int diag_q, double ta, double tb, int order,
                        double *I, double *T) {
-    grid_t g = {nx, ny, L, chi, eta, 1.0, NULL, NULL};
+    grid_t g = {nx, ny, L, chi, eta, 1.0, NULL, NULL, 1.0};
     seg_t *seg = (seg_t *)malloc(sizeof(seg_t) * (size_t)(nx + ny + 4));
     int n = diag_q >= 0 ? diag_segments(nx, ny, (int)floor(px), (int)floor(py), diag_q, ta, tb, seg)
                         : dda_segments(nx, ny, px, py, cos(theta), sin(theta), ta, tb, seg);
@@ -275,7 +278,7 @@ static int solve_impl(const float *chi, const float *eta, const float *line, con
     int top = ncasc - 1;
     if (nx % (1 << top) || ny % (1 << top)) return -1; /* reading G19 */
     if (x0 < 0 || y0 < 0 || x1 > nx || y1 > ny || x0 >= x1 || y0 >= y1) return -1;
-    grid_t g = {nx, ny, L, chi, eta, path_scale, line, xl};
+    grid_t g = {nx, ny, L, chi, eta, path_scale, line, xl, 1.0 / path_scale};
     if (counts) memset(counts, 0, sizeof(*counts));
 #ifdef _OPENMP
     if (nthreads > 0) omp_set_num_threads(nthreads);
@@ -390,9 +393,9 @@ int rc_oracle_solve_scaled(const float *chi, const float *eta, int nx, int ny, i
 int rc_oracle_solve_line(const float *line, const double *xl, int nx, int ny, int L, int ncasc, double c0,
                          const float *I_below, const float *I_above, const float *w, int x0, int x1, int y0,
                          int y1, double *J_out, double *Jbar_out, int nthreads, int order,
-                         rc_oracle_counts *counts) {
+                         rc_oracle_counts *counts, double path_scale) {
     return solve_impl(NULL, NULL, line, xl, nx, ny, L, ncasc, c0, I_below, I_above, w, x0, x1, y0, y1, J_out,
-                      Jbar_out, nthreads, order, -1, NULL, NULL, NULL, NULL, counts, 1.0);
+                      Jbar_out, nthreads, order, -1, NULL, NULL, NULL, NULL, counts, path_scale);
 }
 
 /* Flatland (path_scale = 1): the solve of SURVEY.md §8(c). */

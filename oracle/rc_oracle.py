@@ -56,7 +56,7 @@ def lib():
         _lib.rc_oracle_solve_line.restype = C.c_int
         _lib.rc_oracle_solve_line.argtypes = ([C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double,
                                                C.c_void_p, C.c_void_p, C.c_void_p] + [C.c_int] * 4 +
-                                              [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p])
+                                              [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_double])
         _lib.rc_oracle_num_threads.restype = C.c_int
     return _lib
 
@@ -161,10 +161,25 @@ def solve_inclined(chi, eta, ncascades, mu, w_mu, **kw):
 
 
 def solve_line(line, xl, ncascades, c0=1.0, I_below=None, I_above=None, weights=None, window=None,
-               nthreads=0, order=0, want_counts=False):
+               nthreads=0, order=0, want_counts=False, mu=None, w_mu=None, path_scale=1.0):
     """Velocity-dependent line mode: per cell chi_c, S_c, chi_line, S_line,
     v_x, v_y; opacity and emissivity are evaluated per ray from the projected velocity (rc_oracle.c,
     cell_chi_eta).  line: float32 [ny][nx][6]; xl: [L] Doppler-width offsets.  Returns J, Jbar like solve()."""
+    if mu is not None:
+        # 2.5D: one plain solve per inclination (path 1/sqrt(1-mu^2), in-plane velocity projection sqrt(1-mu^2)),
+        # summed with the quadrature weights, exactly as solve_inclined does for the GivenFs mode
+        out = None
+        for m in range(len(mu)):
+            o = solve_line(line, xl, ncascades, c0, I_below, I_above, weights, window, nthreads, order, want_counts,
+                           path_scale=1.0 / np.sqrt(1.0 - float(mu[m]) ** 2))
+            if out is None:
+                out = dict(o)
+                out["J"] = w_mu[m] * o["J"]
+                out["Jbar"] = w_mu[m] * o["Jbar"]
+            else:
+                out["J"] += w_mu[m] * o["J"]
+                out["Jbar"] += w_mu[m] * o["Jbar"]
+        return out
     line = _f32(line)
     xl = np.ascontiguousarray(xl, dtype=np.float64)
     ny, nx, six = line.shape
@@ -178,7 +193,8 @@ def solve_line(line, xl, ncascades, c0=1.0, I_below=None, I_above=None, weights=
     w = None if weights is None else _f32(weights)
     cnt = Counts()
     rc = lib().rc_oracle_solve_line(_ptr(line), _ptr(xl), nx, ny, L, ncascades, c0, _ptr(Ib), _ptr(Ia), _ptr(w),
-                                    x0, x1, y0, y1, _ptr(J), _ptr(Jbar), nthreads, order, C.byref(cnt))
+                                    x0, x1, y0, y1, _ptr(J), _ptr(Jbar), nthreads, order, C.byref(cnt),
+                                    float(path_scale))
     if rc != 0:
         raise ValueError(f"rc_oracle_solve_line failed: {rc}")
     out = {"J": J, "Jbar": Jbar}
@@ -192,7 +208,8 @@ def solve_atmosphere(atm, **kw):
     """Convenience: oracle solve of a paper_2408_14425_b200.atmospheres.Atmosphere-like object."""
     if getattr(atm, "line", None) is not None:
         return solve_line(atm.line, atm.xl, atm.ncascades, c0=atm.c0_interval, I_below=atm.I_below,
-                          I_above=atm.I_above, weights=atm.weights, **kw)
+                          I_above=atm.I_above, weights=atm.weights, mu=getattr(atm, "mu", None),
+                          w_mu=getattr(atm, "w_mu", None), **kw)
     if getattr(atm, "mu", None) is not None:
         return solve_inclined(atm.chi, atm.eta, atm.ncascades, atm.mu, atm.w_mu, c0=atm.c0_interval,
                               I_below=atm.I_below, I_above=atm.I_above, weights=atm.weights, **kw)

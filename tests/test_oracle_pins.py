@@ -501,3 +501,37 @@ def test_V3_moving_line_symmetries(oracle):
     still = a.line.copy()
     still[..., 4:6] = 0
     assert np.max(np.abs(oracle.solve_line(still, a.xl, 4)["J"] / J - 1)) > 1e-2
+
+
+def test_V4_inclined_moving_line(oracle):
+    """f1 x f2: (a) v = 0 is the inclined GivenFs solve of the precomputed opacities; (b) uniform flow, one
+    cascade, one inclined ray set: per-ray closed form with path d / sin(i) and projected velocity v.w sin(i)."""
+    a = A.line_config2(nx=32, ny=32, nlambda=4, ncascades=4)
+    mu, w = A.gauss_radau(4)
+    still = a.line.copy()
+    still[..., 4:6] = 0.0
+    chi, eta = _static_fields(still, a.xl)
+    J1 = oracle.solve_line(still, a.xl, 4, mu=mu, w_mu=w)["J"]
+    J0 = oracle.solve_inclined(chi.astype(np.float32), eta.astype(np.float32), 4, mu, w)["J"]
+    assert np.allclose(J1, J0, rtol=5e-7)
+    nx, ny, L = 10, 14, 5
+    xl = np.linspace(-2, 2, L)
+    cell = np.array([0.02, 0.5, 0.3, 1.7, -0.9, 1.1], np.float32)
+    line = np.broadcast_to(cell, (ny, nx, 6)).copy()
+    B, m0 = 0.2, 0.6
+    J = oracle.solve_line(line, xl, 1, I_below=[B] * L, I_above=[B] * L, mu=[m0], w_mu=[1.0])["J"]
+    c = cell.astype(np.float64)
+    si = np.sqrt(1 - m0 * m0)
+    y, x = np.mgrid[0:ny, 0:nx]
+    dxp, dxm, dyp, dym = nx - (x + 0.5), x + 0.5, ny - (y + 0.5), y + 0.5
+    want = np.zeros((ny, nx, L))
+    for (sx, sy), (dx, dy) in zip(((1, 1), (-1, 1), (-1, -1), (1, -1)), ((dxp, dyp), (dxm, dyp), (dxm, dym), (dxp, dym))):
+        d = R2 * np.minimum(dx, dy) / si
+        for l in range(L):
+            a_ = xl[l] + si * (c[4] * sx + c[5] * sy) / R2
+            phi = np.exp(-a_ * a_) / np.sqrt(np.pi)
+            chi_ = c[0] + c[2] * phi
+            S = (c[0] * c[1] + c[2] * c[3] * phi) / chi_
+            att = np.exp(-chi_ * d)
+            want[..., l] += (S * (1 - att) + B * att) / 4
+    assert np.allclose(J, want, rtol=1e-12)
