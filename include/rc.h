@@ -115,8 +115,9 @@ int rc_set_atmosphere(rc_ctx *ctx, const float *chi, const float *eta, int nx, i
  * Doppler widths).  x_lambda: host, [nlambda], wavelength offsets from line centre in Doppler widths.  For a
  * ray traced from its probe in direction w the photons travel along -w, and in every cell
  *     a = x_l + v.w,  phi = exp(-a^2)/sqrt(pi),  chi = chi_c + chi_line phi,  eta = chi_c S_c + chi_line S_line phi
- * enter eq. 16.  Flatland only (RC_ERR_BAD_VALUE while inclinations are set).  rc_solve_J, rc_set_boundary,
- * rc_set_lambda_weights, RC_ACCUM_J work as usual; rc_solve_J_host does not apply. */
+ * enter eq. 16.  With inclinations set (rc_set_inclinations, before this call) the velocities are taken to lie
+ * in the plane: inclination m sees v.w sqrt(1 - mu_m^2) over the path ds / sqrt(1 - mu_m^2).  rc_solve_J,
+ * rc_set_boundary, rc_set_lambda_weights, RC_ACCUM_J work as usual; rc_solve_J_host does not apply. */
 int rc_set_line_atmosphere(rc_ctx *ctx, const float *line, int nx, int ny, const float *x_lambda, int nlambda);
 
 /* Boundary intensity sampled by the top cascade: I_below[l] is seen by rays heading

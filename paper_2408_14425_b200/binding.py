@@ -252,6 +252,8 @@ def solve_atmosphere(atm, device=0, lambda_batch=0, flags=0, rc=None):
     if rc is None:
         rc = RadianceCascades(atm.ncascades, atm.c0_interval, device, lambda_batch, fl)
     if getattr(atm, "line", None) is not None:
+        if getattr(atm, "mu", None) is not None:
+            rc.set_inclinations(atm.mu, atm.w_mu)
         rc.set_line_atmosphere(torch.from_numpy(atm.line).to(dev), atm.xl)
     else:
         chi = torch.from_numpy(atm.chi).to(dev)

@@ -341,7 +341,7 @@ size_t rc_workspace_bytes(const rc_ctx *ctx, int nx, int ny, int nlambda, int ho
     Plan P;
     if (!make_plan(ctx->cfg, ctx->nm, false, nx, ny, nlambda, host_io != 0, P, nullptr)) return 0;
     size_t need = P.total;
-    if (ctx->nm == 1 && make_plan(ctx->cfg, 1, true, nx, ny, nlambda, false, P, nullptr)) need = std::max(need, P.total);  // line mode
+    if (make_plan(ctx->cfg, ctx->nm, true, nx, ny, nlambda, false, P, nullptr)) need = std::max(need, P.total);  // line mode
     return need;
 }
 
@@ -469,7 +469,6 @@ int rc_set_atmosphere(rc_ctx *ctx, const float *chi, const float *eta, int nx, i
 // Velocity-dependent line mode.
 int rc_set_line_atmosphere(rc_ctx *ctx, const float *line, int nx, int ny, const float *x_lambda, int nlambda) {
     if (!ctx || !line || !x_lambda) return ctx ? fail(ctx, RC_ERR_NULL_ARG, "null line / x_lambda") : RC_ERR_NULL_ARG;
-    if (ctx->nm != 1) return fail(ctx, RC_ERR_BAD_VALUE, "line mode with inclinations is not supported: call rc_set_inclinations(ctx, 1, NULL, NULL)");
     {
         const int rc = prepare_shape(ctx, nx, ny, nlambda, true);
         if (rc != RC_OK) return rc;
@@ -561,7 +560,7 @@ static rc::MarchParams march_params(const rc_ctx *ctx, int i, float *J_out) {
     mp.npatch_x = (mp.npx + pw - 1) / pw;
     mp.npatch_y = (mp.npy + ph - 1) / ph;
     mp.kg_n = mp.ngroups; mp.kg_off = 0;
-    for (int m = 0; m < 8; m++) { mp.incl_f[m] = ctx->incl_f[m]; mp.incl_w[m] = ctx->incl_w[m]; }
+    for (int m = 0; m < 8; m++) { mp.incl_f[m] = ctx->incl_f[m]; mp.incl_w[m] = ctx->incl_w[m]; mp.incl_s[m] = 1.f / ctx->incl_f[m]; }
     mp.state = nullptr;
     mp.band_axis = 0; mp.band_sign = 1; mp.band_lo = 0; mp.band_hi = 0; mp.band_final = 1;
     return mp;

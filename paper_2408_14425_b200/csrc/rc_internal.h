@@ -58,7 +58,7 @@ struct MarchParams {
     float *state;          // parked rays: [nb][ngroups][4][npy][npx][2][LV]  (I, tau*log2 e)
     int band_axis, band_sign, band_lo, band_hi, band_final;
     // 2.5D inclination quadrature: path scale 1/sqrt(1 - mu_m^2) and weight of inclination m
-    float incl_f[8], incl_w[8];
+    float incl_f[8], incl_w[8], incl_s[8];  // incl_s = sqrt(1 - mu^2): projection of in-plane velocities (line mode)
 };
 
 struct PackParams {

@@ -409,10 +409,10 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
     // LINE: the packed cell holds the 6 line parameters; chi and S of each wavelength are
     // evaluated per step from the velocity projected on this ray.  xs = x_l sqrt(log2 e) of the lane's wavelengths.
     constexpr int NR = LINE ? 6 : LL;  // floats gathered per cell
-    float xs[LINE ? LV : 1];
+    float xs[LINE ? LL : 1];
     if constexpr (LINE) {
 #pragma unroll
-        for (int v = 0; v < LV; v++) xs[v] = __ldg(p.xls + nbI * LV + v);
+        for (int v = 0; v < LL; v++) xs[v] = __ldg(p.xls + nbI * LL + v);
     }
     const unsigned *occB = SPARSE ? p.occ + (long long)nbI * (ncell >> 5) : nullptr;
     // (dx, dy) ranges that keep this lane's ray inside the box
@@ -524,15 +524,19 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
                     for (int m = 0; m < NM; m++) dsm[m] = NM == 1 ? ds[u] : ds[u] * p.incl_f[m];
                     if constexpr (LINE) {
                         // packed cell: chi_c', chi_c' S_c, chi_line', chi_line' S_line, v_x', v_y'   (' = scaled, pack_line_kernel)
+                        // inclination m sees the in-plane velocity projected with sin(inclination) (2.5D line mode)
                         const float vw = fmaf(c2[u][4], wx, c2[u][5] * wy);
+                        float vwm[NM];
+#pragma unroll
+                        for (int m = 0; m < NM; m++) vwm[m] = NM == 1 ? vw : vw * p.incl_s[m];
 #pragma unroll
                         for (int v = 0; v < LV; v++) {
-                            const float aa = xs[v] + vw;
+                            const float aa = xs[v / NM] + vwm[v % NM];
                             const float phi = ex2_neg(aa * aa);
                             const float chi2 = fmaf(c2[u][2], phi, c2[u][0]);
                             const float num = fmaf(c2[u][3], phi, c2[u][1]);
                             const float Sv = chi2 > 0.f ? __fdividef(num, chi2) : 0.f;  // eta/chi; vacuum emits nothing
-                            tau[v] = fmaf(chi2, dsm[0], tau[v]);
+                            tau[v] = fmaf(chi2, dsm[v % NM], tau[v]);
                             const float Tn = ex2_neg(tau[v]);
                             I[v] = fmaf(Sv, T[v] - Tn, I[v]);
                             T[v] = Tn;
@@ -667,13 +671,13 @@ static cudaError_t launch_march_sparse(const MarchParams &p, cudaStream_t st) {
     return cudaGetLastError();
 }
 
-// Velocity-dependent line mode (linepk != null): 3 MUFU per segment-wavelength, ring of 2, 24 warps/SM.
-template <int LV>
+// Velocity-dependent line mode (linepk != null): 3 MUFU per segment-channel, ring of 2, 24 warps/SM.
+template <int LV, int NM = 1>
 static cudaError_t launch_march_line(const MarchParams &p, cudaStream_t st) {
     constexpr int WARPS = 8;
     const long long blocks = (march_warps(p) + WARPS - 1) / WARPS;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-    march_kernel<LV, 1, 2, WARPS, 3, false, false, true><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
+    march_kernel<LV, NM, 2, WARPS, 3, false, false, true><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
     return cudaGetLastError();
 }
 
@@ -698,6 +702,17 @@ cudaError_t launch_march(const MarchParams &p, int LV, int NM, int variant, cuda
             case 4: return launch_march_flat<4>(p, variant, st);
             case 2: return launch_march_flat<2>(p, variant, st);
             default: return launch_march_flat<1>(p, variant, st);
+        }
+    }
+    if (p.linepk != nullptr) {
+        switch (LV * 16 + NM) {
+            case 8 * 16 + 8: return launch_march_line<8, 8>(p, st);
+            case 8 * 16 + 4: return launch_march_line<8, 4>(p, st);
+            case 8 * 16 + 2: return launch_march_line<8, 2>(p, st);
+            case 4 * 16 + 4: return launch_march_line<4, 4>(p, st);
+            case 4 * 16 + 2: return launch_march_line<4, 2>(p, st);
+            case 2 * 16 + 2: return launch_march_line<2, 2>(p, st);
+            default: return cudaErrorInvalidValue;
         }
     }
     // inclined launches are MUFU-bound (NM ex2 per gathered value): ring of 2, 24 warps/SM measured best

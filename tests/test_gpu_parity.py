@@ -343,3 +343,15 @@ def test_graph_replay_matches_plain_launches(monkeypatch):
     Jb, _ = binding.solve_atmosphere(atm2, rc=rc)            # new atmosphere on the same context
     assert np.array_equal(Jb.cpu().numpy(), ref2)
     rc.close()
+
+
+@pytest.mark.parametrize("kw,n", [
+    (dict(nx=128, ny=64, nlambda=5, ncascades=5), 8),
+    (dict(nx=64, ny=64, nlambda=6, ncascades=5), 4),
+    (dict(nx=64, ny=128, nlambda=9, ncascades=5), 2),
+])
+def test_inclined_moving_line_matches_the_oracle(oracle, kw, n):
+    """f1 x f2 (the paper's actual set-up, PAPER.md:281 + 304): moving line, n Gauss-Radau inclinations."""
+    atm = A.with_inclinations(A.line_config2(**kw), n)
+    e = check(atm, oracle)
+    print(atm.name, kw, n, "max rel err", e)
