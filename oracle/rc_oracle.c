@@ -264,7 +264,7 @@ typedef struct {
  *   dump_cascade >= 0: also write that cascade's intervals before merging (dump_I, dump_T) and
  *   after merging (dump_M), each [wy][wx][N][L] over that cascade's probe window; dump_win gets
  *   {ax0, ax1, by0, by1} (inclusive probe index ranges).
- *   order: 0 front-to-back, 1 back-to-front (G13).
+ *   order: bit 0: 0 front-to-back, 1 back-to-front (G13); bit 1: the bilinear fix.
  * Returns 0, or -1 on bad arguments / -2 out of memory.
  */
 static int solve_impl(const float *chi, const float *eta, const float *line, const double *xl, int nx, int ny,
@@ -279,6 +279,7 @@ static int solve_impl(const float *chi, const float *eta, const float *line, con
     if (nx % (1 << top) || ny % (1 << top)) return -1; /* reading G19 */
     if (x0 < 0 || y0 < 0 || x1 > nx || y1 > ny || x0 >= x1 || y0 >= y1) return -1;
     grid_t g = {nx, ny, L, chi, eta, path_scale, line, xl, 1.0 / path_scale};
+    const int fix = (order & 2) != 0; /* order: bit 0 = back-to-front (G13), bit 1 = bilinear fix */
     if (counts) memset(counts, 0, sizeof(*counts));
 #ifdef _OPENMP
     if (nthreads > 0) omp_set_num_threads(nthreads);
@@ -319,13 +320,47 @@ static int solve_impl(const float *chi, const float *eta, const float *line, con
                     for (long k = 0; k < N; k++) {
                         double px = (a + 0.5) * s, py = (b + 0.5) * s; /* PAPER.md:312, reading G5 */
                         double theta = 2.0 * M_PI * (k + 0.5) / (double)N; /* reading G4 */
+                        size_t o = ((((size_t)(b - by0[i])) * wx + (a - ax0[i])) * N + k) * L;
+                        if (fix && i < top) {
+                            /* Bilinear fix: "each radiance interval in cascade i is traced from its
+                             * usual starting position to the starting position of the associated child cone on each
+                             * of the four probes of cascade i+1 that are normally bilinearly interpolated ... the four
+                             * distinct radiance intervals are each merged with their associated samples from cascade
+                             * i+1, and then averaged using the usual bilinear weights".  Reading G24: the child cone of
+                             * direction k on parent q starts at P_q + t_{i+1} w_k; its sample is the mean of the 4
+                             * children 4k..4k+3 of q.  A sub-ray whose start lies outside the box is vacuum (G10). */
+                            int a0, a1, b0, b1; double fa, fb;
+                            parent_axis(a, npx / 2, &a0, &a1, &fa);
+                            parent_axis(b, npy / 2, &b0, &b1, &fb);
+                            for (int l = 0; l < L; l++) M[o + l] = 0.0;
+                            double Ax = px + ta * cos(theta), Ay = py + ta * sin(theta);
+                            for (int slot = 0; slot < 4; slot++) {
+                                int aq = (slot & 1) ? a1 : a0, bq = (slot & 2) ? b1 : b0;
+                                double wq = ((slot & 1) ? fa : 1.0 - fa) * ((slot & 2) ? fb : 1.0 - fb);
+                                double Bx = (aq + 0.5) * (2 * s) + tb * cos(theta), By = (bq + 0.5) * (2 * s) + tb * sin(theta);
+                                double dx = Bx - Ax, dy = By - Ay, len = sqrt(dx * dx + dy * dy);
+                                int n = dda_segments(nx, ny, Ax, Ay, dx / len, dy / len, 0.0, len, seg);
+                                nseg_total += n;
+                                if (order & 1) integrate_btf(&g, seg, n, dx / len, dy / len, I, T);
+                                else integrate_ftb(&g, seg, n, dx / len, dy / len, I, T);
+                                for (int l = 0; l < L; l++) {
+                                    double U = 0.0;
+                                    for (int j = 0; j < 4; j++) {
+                                        long kk = 4 * k + j;
+                                        U += Mup[((((size_t)(bq - upy0)) * upwx + (aq - upx0)) * upN + kk) * L + l];
+                                    }
+                                    M[o + l] += wq * (I[l] + T[l] * U / 4.0);
+                                }
+                            }
+                            if (dump) for (int l = 0; l < L; l++) dump_M[o + l] = M[o + l];
+                            continue;
+                        }
                         /* a1: the radiance interval of this probe and direction */
                         int n = i == 0 ? diag_segments(nx, ny, a, b, (int)k, ta, tb, seg)
                                        : dda_segments(nx, ny, px, py, cos(theta), sin(theta), ta, tb, seg);
                         nseg_total += n;
-                        if (order == 0) integrate_ftb(&g, seg, n, cos(theta), sin(theta), I, T);
-                        else integrate_btf(&g, seg, n, cos(theta), sin(theta), I, T);
-                        size_t o = ((((size_t)(b - by0[i])) * wx + (a - ax0[i])) * N + k) * L;
+                        if (order & 1) integrate_btf(&g, seg, n, cos(theta), sin(theta), I, T);
+                        else integrate_ftb(&g, seg, n, cos(theta), sin(theta), I, T);
                         if (dump) for (int l = 0; l < L; l++) { dump_I[o + l] = I[l]; dump_T[o + l] = T[l]; }
                         if (i == top) {
                             /* a2: boundary intensity enters on the top cascade only (G9) */

@@ -98,7 +98,7 @@ def merge(I_near, tau_near, I_far, tau_far):
 
 
 def solve(chi, eta, ncascades, c0=1.0, I_below=None, I_above=None, weights=None, window=None,
-          nthreads=0, order=0, dump_cascade=-1, want_counts=False, path_scale=1.0):
+          nthreads=0, order=0, dump_cascade=-1, want_counts=False, path_scale=1.0, bilinear_fix=False):
     """J [wy][wx][L] (float64) for the cascade-0 cell window (x0, x1, y0, y1) (default: whole grid).
 
     Returns a dict: J, Jbar, and if asked counts / dump_{I,T,M,win} of one cascade."""
@@ -121,6 +121,7 @@ def solve(chi, eta, ncascades, c0=1.0, I_below=None, I_above=None, weights=None,
         shape = (ny // s, nx // s, N, L)
         dI, dT, dM = np.zeros(shape), np.zeros(shape), np.zeros(shape)
         assert window is None, "dump only with the full window (dense layout)"
+    order = int(order) | (2 if bilinear_fix else 0)  # bit 1: the bilinear fix
     rc = lib().rc_oracle_solve_scaled(_ptr(chi), _ptr(eta), nx, ny, L, ncascades, c0, _ptr(Ib), _ptr(Ia),
                                       _ptr(w), x0, x1, y0, y1, _ptr(J), _ptr(Jbar), nthreads, order,
                                       dump_cascade, _ptr(dI), _ptr(dT), _ptr(dM), _ptr(win), C.byref(cnt),
@@ -161,7 +162,7 @@ def solve_inclined(chi, eta, ncascades, mu, w_mu, **kw):
 
 
 def solve_line(line, xl, ncascades, c0=1.0, I_below=None, I_above=None, weights=None, window=None,
-               nthreads=0, order=0, want_counts=False, mu=None, w_mu=None, path_scale=1.0):
+               nthreads=0, order=0, want_counts=False, mu=None, w_mu=None, path_scale=1.0, bilinear_fix=False):
     """Velocity-dependent line mode: per cell chi_c, S_c, chi_line, S_line,
     v_x, v_y; opacity and emissivity are evaluated per ray from the projected velocity (rc_oracle.c,
     cell_chi_eta).  line: float32 [ny][nx][6]; xl: [L] Doppler-width offsets.  Returns J, Jbar like solve()."""
@@ -171,7 +172,7 @@ def solve_line(line, xl, ncascades, c0=1.0, I_below=None, I_above=None, weights=
         out = None
         for m in range(len(mu)):
             o = solve_line(line, xl, ncascades, c0, I_below, I_above, weights, window, nthreads, order, want_counts,
-                           path_scale=1.0 / np.sqrt(1.0 - float(mu[m]) ** 2))
+                           path_scale=1.0 / np.sqrt(1.0 - float(mu[m]) ** 2), bilinear_fix=bilinear_fix)
             if out is None:
                 out = dict(o)
                 out["J"] = w_mu[m] * o["J"]
@@ -192,6 +193,7 @@ def solve_line(line, xl, ncascades, c0=1.0, I_below=None, I_above=None, weights=
     Ia = None if I_above is None else _f32(I_above)
     w = None if weights is None else _f32(weights)
     cnt = Counts()
+    order = int(order) | (2 if bilinear_fix else 0)
     rc = lib().rc_oracle_solve_line(_ptr(line), _ptr(xl), nx, ny, L, ncascades, c0, _ptr(Ib), _ptr(Ia), _ptr(w),
                                     x0, x1, y0, y1, _ptr(J), _ptr(Jbar), nthreads, order, C.byref(cnt),
                                     float(path_scale))
@@ -206,6 +208,8 @@ def solve_line(line, xl, ncascades, c0=1.0, I_below=None, I_above=None, weights=
 
 def solve_atmosphere(atm, **kw):
     """Convenience: oracle solve of a paper_2408_14425_b200.atmospheres.Atmosphere-like object."""
+    if getattr(atm, "bilinear_fix", False):
+        kw.setdefault("bilinear_fix", True)
     if getattr(atm, "line", None) is not None:
         return solve_line(atm.line, atm.xl, atm.ncascades, c0=atm.c0_interval, I_below=atm.I_below,
                           I_above=atm.I_above, weights=atm.weights, mu=getattr(atm, "mu", None),

@@ -44,6 +44,7 @@ class Atmosphere:
     # velocity-dependent line mode: per-cell line parameters instead of chi, eta (then None)
     line: np.ndarray | None = None  # float32 [ny][nx][6]: chi_c, S_c, chi_line, S_line, v_x, v_y (Doppler widths)
     xl: np.ndarray | None = None    # float64 [nlambda] offsets from line centre in Doppler widths
+    bilinear_fix: bool = False      # solve with the bilinear fix
 
 
 # (nx, ny, nlambda, ncascades) of BASELINE.json's configs
