@@ -64,6 +64,11 @@ extern "C" {
                               transmittance has already flushed to exactly 0, so the result is
                               bit-identical (front-to-back early termination) */
 
+#define RC_BILINEAR_FIX 8 /* the bilinear fix: every interval below the top
+                             cascade is traced four times, from its usual start to the start of the child cone on
+                             each of the four parent probes, merged with that parent alone and then weighted
+                             bilinearly: removes most of the ringing around bright compact sources at 4x the rays */
+
 typedef struct rc_ctx rc_ctx; /* opaque, owned by the library */
 
 typedef struct {
@@ -71,7 +76,7 @@ typedef struct {
     float c0_interval; /* length of the cascade-0 interval in cells; > 0; the configs use 1 */
     int device;        /* CUDA ordinal */
     int lambda_batch;  /* wavelengths per thread (1, 2, 4 or 8); 0 = library chooses */
-    int flags;         /* RC_ACCUM_J | RC_VALIDATE | RC_NO_EARLY_EXIT */
+    int flags;         /* RC_ACCUM_J | RC_VALIDATE | RC_NO_EARLY_EXIT | RC_BILINEAR_FIX */
 } rc_config;
 
 typedef struct {

@@ -14,7 +14,7 @@ import numpy as np
 from . import build as _build
 
 RC_OK = 0
-RC_ACCUM_J, RC_VALIDATE, RC_NO_EARLY_EXIT = 1, 2, 4
+RC_ACCUM_J, RC_VALIDATE, RC_NO_EARLY_EXIT, RC_BILINEAR_FIX = 1, 2, 4, 8
 RC_MAX_CASCADES = 12
 ERRORS = {-1: "RC_ERR_NULL_ARG", -2: "RC_ERR_BAD_SHAPE", -3: "RC_ERR_NO_DEVICE", -4: "RC_ERR_NO_WORKSPACE",
           -5: "RC_ERR_BAD_VALUE", -6: "RC_ERR_CUDA", -7: "RC_ERR_NO_ATMOSPHERE"}
@@ -248,7 +248,7 @@ def solve_atmosphere(atm, device=0, lambda_batch=0, flags=0, rc=None):
     """Convenience for tests/bench: upload an `atmospheres.Atmosphere`, solve, return (J tensor, ctx)."""
     import torch
     dev = f"cuda:{device}"
-    fl = flags | (RC_ACCUM_J if atm.accumulate else 0)
+    fl = flags | (RC_ACCUM_J if atm.accumulate else 0) | (RC_BILINEAR_FIX if getattr(atm, "bilinear_fix", False) else 0)
     if rc is None:
         rc = RadianceCascades(atm.ncascades, atm.c0_interval, device, lambda_batch, fl)
     if getattr(atm, "line", None) is not None:

@@ -18,6 +18,8 @@ constexpr size_t ALIGN = 256;
 inline size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 
 struct CascadePlan {
+    bool fix = false;           // bilinear fix: 16 tables per direction, lanes = one parity class, packed with spacing 2s
+    size_t subdir_off = 0;      // fix: unit directions of the sub-rays [ndir*16] float2
     bool banded = false;        // marched band by band (Plan::nbands launches per direction half)
     int pw_log2 = 5;            // lane patch of the march: 2^pw_log2 probes wide, 32 >> pw_log2 high
     long long ndir = 0;         // 4^(i+1)
@@ -190,29 +192,36 @@ bool make_plan_uncached(const rc_config &cfg, int nm, bool line, int nx, int ny,
         while (c.pw_log2 > 0 && (1 << c.pw_log2) > (nx >> i)) c.pw_log2--;
         if (c.empty) continue;
         c.pw_log2 = choose_patch(nx, ny, i, c.ta, c.tb);
+        c.fix = (cfg.flags & RC_BILINEAR_FIX) != 0 && i < top;
         std::vector<long long> local;
         std::vector<long long> &o = offs ? (*offs)[i] : local;
-        o.resize((size_t)c.ndir + 1);
+        const int nsub = c.fix ? 16 : 1;
+        o.resize((size_t)c.ndir * nsub + 1);
         long long acc = 0;
-        for (long long k = 0; k < c.ndir; k++) {
+        for (long long k = 0; k < c.ndir * nsub; k++) {
             o[(size_t)k] = acc;
             long long n;
-            if (i == 0) {
+            if (c.fix) {
+                // sub-ray from p + t_i w to q + t_(i+1) w: at most (t_(i+1) - t_i) + 1.5 sqrt2 s long, clipped by the box
+                const double len = std::fmin(c.tb - c.ta + 2.2 * (1 << i), diag + 2.0 * (1 << i));
+                n = (long long)(len * 1.4143) + 8;
+            } else if (i == 0) {
                 const double cells = std::isinf(c.tb) ? (double)std::min(nx, ny)
                                                       : std::min((double)std::min(nx, ny), std::ceil(c.tb / std::sqrt(2.0) + 0.5) + 1.0);
                 n = (long long)cells;
             } else {
-                const double th = 2.0 * M_PI * ((double)k + 0.5) / (double)c.ndir;
+                const double th = 2.0 * M_PI * ((double)k + 0.5) / (double)c.ndir;  // (nsub == 1 here)
                 const double wx = std::fabs(std::cos(th)), wy = std::fabs(std::sin(th));
                 const double tb = std::fmin(c.tb, std::fmin(nx / wx, ny / wy));
                 n = tb > c.ta ? (long long)((tb - c.ta) * (wx + wy)) + 6 : 0;
             }
             acc += n;
         }
-        o[(size_t)c.ndir] = acc;
+        o[(size_t)c.ndir * nsub] = acc;
         c.slots = acc;
-        c.off_off = cur;   cur = align_up(cur + sizeof(long long) * ((size_t)c.ndir + 1));
-        c.cnt_off = cur;   cur = align_up(cur + sizeof(int) * (size_t)c.ndir);
+        c.off_off = cur;   cur = align_up(cur + sizeof(long long) * ((size_t)c.ndir * nsub + 1));
+        c.cnt_off = cur;   cur = align_up(cur + sizeof(int) * (size_t)c.ndir * nsub);
+        if (c.fix) { c.subdir_off = cur; cur = align_up(cur + sizeof(float2) * (size_t)c.ndir * 16); }
         // + 16 entries: the march loop reads the table up to 2 x (ring depth) entries past the last step
         c.steps_off = cur; cur = align_up(cur + sizeof(rc::Step) * ((size_t)acc + 16));
         c.xy_off = cur;    cur = align_up(cur + sizeof(rc::StepXY) * ((size_t)acc + 16));
@@ -236,7 +245,7 @@ bool make_plan_uncached(const rc_config &cfg, int nm, bool line, int nx, int ny,
             // worth it for long rays only, and only while one warp's patch of probes is small against a
             // band (its lanes enter and leave a band at different steps: lock-step waste otherwise)
             const int patch_ext = (P.band_axis ? 1 << c.pw_log2 : 32 >> c.pw_log2) << i;
-            c.banded = P.nbands > 1 && !c.empty && std::fmin(c.tb, diag) > 100.0 && (4 * patch_ext <= ext || std::getenv("RC_BANDS"));
+            c.banded = P.nbands > 1 && !c.empty && !c.fix && std::fmin(c.tb, diag) > 100.0 && (4 * patch_ext <= ext || std::getenv("RC_BANDS"));
             any = any || c.banded;
         }
         if (any) { P.state = cur; cur += 8 * field * P.NM; }
@@ -403,7 +412,7 @@ static int prepare_shape(rc_ctx *ctx, int nx, int ny, int nlambda, bool line) {
                 ctx->stats.table_steps[i] = c.slots;
                 if (c.empty) continue;
                 RC_CUDA(ctx, cudaMemcpyAsync(ctx->ws + c.off_off, ctx->off_host[i].data(),
-                                             sizeof(long long) * ((size_t)c.ndir + 1), cudaMemcpyHostToDevice, ctx->stream));
+                                             sizeof(long long) * ctx->off_host[i].size(), cudaMemcpyHostToDevice, ctx->stream));
                 rc::TableBuildParams tp;
                 tp.steps = (rc::Step *)(ctx->ws + c.steps_off);
                 tp.xy = (rc::StepXY *)(ctx->ws + c.xy_off);
@@ -411,6 +420,7 @@ static int prepare_shape(rc_ctx *ctx, int nx, int ny, int nlambda, bool line) {
                 tp.cnt = (int *)(ctx->ws + c.cnt_off);
                 tp.cascade = i; tp.top = i == top; tp.ndir = c.ndir;
                 tp.ta = c.ta; tp.tb = c.tb; tp.nx = nx; tp.ny = ny;
+                tp.fix = c.fix; tp.subdir = c.fix ? (float2 *)(ctx->ws + c.subdir_off) : nullptr;
                 RC_CUDA(ctx, rc::launch_table_build(tp, ctx->stream));
             }
             ctx->tab_nx = nx; ctx->tab_ny = ny;
@@ -555,10 +565,13 @@ static rc::MarchParams march_params(const rc_ctx *ctx, int i, float *J_out) {
     mp.mode = i > 0 ? 0 : (accum ? 2 : 1);
     mp.early_exit = (ctx->cfg.flags & RC_NO_EARLY_EXIT) ? 0 : 1;
     mp.pw_log2 = ctx->tune_patch >= 0 && i >= ctx->tune_patch_from ? ctx->tune_patch : c.pw_log2;
-    while (mp.pw_log2 > 0 && (1 << mp.pw_log2) > mp.npx) mp.pw_log2--;
+    mp.fix = c.fix && !c.empty;
+    mp.subdir = mp.fix ? (const float2 *)(ctx->ws + c.subdir_off) : nullptr;
+    const int lx = mp.fix ? mp.npx >> 1 : mp.npx, ly = mp.fix ? mp.npy >> 1 : mp.npy;  // lane lattice
+    while (mp.pw_log2 > 0 && (1 << mp.pw_log2) > lx) mp.pw_log2--;
     const int pw = 1 << mp.pw_log2, ph = 32 >> mp.pw_log2;
-    mp.npatch_x = (mp.npx + pw - 1) / pw;
-    mp.npatch_y = (mp.npy + ph - 1) / ph;
+    mp.npatch_x = (lx + pw - 1) / pw;
+    mp.npatch_y = (ly + ph - 1) / ph;
     mp.kg_n = mp.ngroups; mp.kg_off = 0;
     for (int m = 0; m < 8; m++) { mp.incl_f[m] = ctx->incl_f[m]; mp.incl_w[m] = ctx->incl_w[m]; mp.incl_s[m] = 1.f / ctx->incl_f[m]; }
     mp.state = nullptr;
@@ -584,7 +597,7 @@ static int enqueue_solve(rc_ctx *ctx, float *J_out) {
             pp.chi = ctx->chi; pp.eta = ctx->eta;
             pp.chiT = (float *)(ctx->ws + P.chiT); pp.ST = (float *)(ctx->ws + P.ST);
             pp.occ = ctx->sparse && P.has_occ ? (unsigned *)(ctx->ws + P.occ) : nullptr;
-            pp.nx = P.nx; pp.ny = P.ny; pp.L = P.L; pp.nb = P.nb; pp.shift = i;
+            pp.nx = P.nx; pp.ny = P.ny; pp.L = P.L; pp.nb = P.nb; pp.shift = c.fix ? i + 1 : i;
             if (ctx->line) {
                 pp.chi = ctx->line; pp.eta = nullptr; pp.occ = nullptr;
                 RC_CUDA(ctx, rc::launch_pack_line(pp, ctx->stream));

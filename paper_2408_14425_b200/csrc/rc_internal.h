@@ -52,6 +52,9 @@ struct MarchParams {
     int early_exit;
     int pw_log2;           // one warp's 32 probes form a patch 2^pw_log2 wide, 32 >> pw_log2 high
     int npatch_x, npatch_y;  // patches per axis
+    int fix;               // bilinear fix: 4 sub-rays per ray, lanes = probes of one parity class,
+                           // packed layout of spacing 2s, tables indexed (k*16 + class*4 + slot)
+    const float2 *subdir;  // fix: unit direction of each sub-ray (line mode)
     int kg_n, kg_off;      // the launch covers direction groups (kg_off + 0 .. kg_n-1) mod ngroups
     // banded launch (state != null): only the steps inside [band_lo, band_hi) along band_axis
     // (0 = rows, 1 = columns), for rays travelling in direction band_sign along that axis
@@ -77,6 +80,8 @@ struct TableBuildParams {
     long long ndir;
     double ta, tb;  // interval ends (tb = +inf on the top cascade)
     int nx, ny;
+    int fix;         // bilinear fix: 16 tables per direction (parity class x parent slot), off/cnt indexed k*16 + sub
+    float2 *subdir;  // fix: [ndir*16] unit direction of each sub-ray
 };
 
 // launchers (rc_kernels.cu); LV in {1,2,4,8}

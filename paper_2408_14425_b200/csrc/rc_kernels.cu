@@ -28,23 +28,70 @@ static constexpr int WARPS_PER_BLOCK = 8;
 // Geometry tables (fp64).  Restates PAPER.md:171-176 (shell [t_i, t_{i+1}]) and PAPER.md:314 (DDA).
 // ------------------------------------------------------------------------------------------------
 __global__ void table_build_kernel(TableBuildParams p) {
-    long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= p.ndir) return;
-    Step *out = p.steps + p.off[k];
-    StepXY *oxy = p.xy + p.off[k];
-    const long long cap = p.off[k + 1] - p.off[k];
-    const int shift = p.cascade, s = 1 << shift, half = s >> 1, npx = p.nx >> shift;
-    // cell (vertex cell + (dx, dy)) in the packed layout [y mod s][x mod s][y div s][x div s], relative to
-    // the probe's own entry (y div s, x div s) = (b, a) of phase plane 0
-    const int npy = p.ny >> shift;
+    // one thread per table: direction k, and with the bilinear fix (p.fix) one of the 16 sub-rays
+    // (parity class of the probe x parent slot) of that direction
+    const int nsub = p.fix ? 16 : 1;
+    const long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (id >= p.ndir * nsub) return;
+    const long long k = id / nsub;
+    const int sub = (int)(id - k * nsub);
+    Step *out = p.steps + p.off[id];
+    StepXY *oxy = p.xy + p.off[id];
+    const long long cap = p.off[id + 1] - p.off[id];
+    const int s = 1 << p.cascade, half = s >> 1;
+    // cell (vertex cell + (dx, dy)) in the packed layout [y mod S][x mod S][y div S][x div S], relative to the
+    // lane's own entry of phase plane 0.  Plain: S = s, the entry is the probe's (b, a), the vertex cell sits at
+    // (half, half) of its S x S block.  Bilinear fix: lanes are probes of one parity class (pa, pb), packed with
+    // S = 2s (the parents' spacing), entry (b div 2, a div 2), vertex cell at (pa s + half, pb s + half).
+    const int pa = (sub >> 2) & 1, pb = sub >> 3;
+    const int shift = p.cascade + (p.fix ? 1 : 0), S = 1 << shift;
+    const int npx = p.nx >> shift, npy = p.ny >> shift;
+    const int offx = (p.fix ? pa * s : 0) + half, offy = (p.fix ? pb * s : 0) + half;
     auto emit = [&](int n, int dx, int dy, double ds) {
-        const int tx = dx + half, ty = dy + half;
-        const int phase = ((ty & (s - 1)) << shift) + (tx & (s - 1));
+        const int tx = dx + offx, ty = dy + offy;
+        const int phase = ((ty & (S - 1)) << shift) + (tx & (S - 1));
         out[n].delta = phase * (npx * npy) + (ty >> shift) * npx + (tx >> shift);
         out[n].ds = (float)ds;
         oxy[n].dx = (int16_t)dx;
         oxy[n].dy = (int16_t)dy;
     };
+    if (p.fix) {
+        // Bilinear fix: from the usual start p + t_i w to the start of the child cone on parent q,
+        // P_q + t_(i+1) w.  P_q - P_p per axis: even probe index -1.5 s (slot 0), +0.5 s (slot 1); odd -0.5 s, +1.5 s.
+        const int sa = sub & 1, sb = (sub >> 1) & 1;
+        double wx, wy;
+        sincospi(2.0 * ((double)k + 0.5) / (double)p.ndir, &wy, &wx);
+        const double ox = (pa == 0 ? (sa ? 0.5 : -1.5) : (sa ? 1.5 : -0.5)) * s;
+        const double oy = (pb == 0 ? (sb ? 0.5 : -1.5) : (sb ? 1.5 : -0.5)) * s;
+        const double pc = p.cascade == 0 ? 0.5 : 0.0;  // probe position relative to the corner of its vertex cell
+        const double x0 = pc + p.ta * wx, y0 = pc + p.ta * wy;
+        double ux = ox + (p.tb - p.ta) * wx, uy = oy + (p.tb - p.ta) * wy;
+        double len = sqrt(ux * ux + uy * uy);
+        ux /= len; uy /= len;
+        p.subdir[id] = make_float2((float)ux, (float)uy);
+        // no ray from inside the box is still inside beyond this
+        len = fmin(len, fmin(ux != 0.0 ? (double)p.nx / fabs(ux) : INFINITY, uy != 0.0 ? (double)p.ny / fabs(uy) : INFINITY) + 2.0 * s);
+        int ix = (int)floor(x0), iy = (int)floor(y0);
+        if ((double)ix == x0 && ux < 0.0) ix--;
+        if ((double)iy == y0 && uy < 0.0) iy--;
+        const int sx = ux > 0.0 ? 1 : -1, sy = uy > 0.0 ? 1 : -1;
+        int gx = ux > 0.0 ? ix + 1 : ix, gy = uy > 0.0 ? iy + 1 : iy;
+        double tmx = ux != 0.0 ? ((double)gx - x0) / ux : INFINITY, tmy = uy != 0.0 ? ((double)gy - y0) / uy : INFINITY;
+        double t = 0.0;
+        int n = 0;
+        while (n < cap) {
+            const double tn = fmin(fmin(tmx, tmy), len);
+            const double ds = tn - t;
+            if (ds > 0.0) emit(n++, ix, iy, ds);
+            if (tn >= len) break;
+            const bool stepx = tmx <= tmy, stepy = tmy <= tmx;  // a tie is a corner: step both
+            if (stepx) { ix += sx; gx += sx; tmx = ((double)gx - x0) / ux; }
+            if (stepy) { iy += sy; gy += sy; tmy = ((double)gy - y0) / uy; }
+            t = tn;
+        }
+        p.cnt[id] = n;
+        return;
+    }
     int n = 0;
     if (p.cascade == 0) {
         // The 4 diagonals from a cell centre pass exactly through cell corners: closed form.
@@ -91,7 +138,7 @@ __global__ void table_build_kernel(TableBuildParams p) {
 
 cudaError_t launch_table_build(const TableBuildParams &p, cudaStream_t st) {
     const int threads = 128;
-    const long long blocks = (p.ndir + threads - 1) / threads;
+    const long long blocks = (p.ndir * (p.fix ? 16 : 1) + threads - 1) / threads;
     table_build_kernel<<<(unsigned)blocks, threads, 0, st>>>(p);
     return cudaGetLastError();
 }
@@ -311,17 +358,22 @@ __device__ __forceinline__ void parent_axis(int a, int n, int &q0, int &q1, floa
 // share a narrow fan of directions (a few MB of step tables) and one batch's planes (L2).
 struct WarpWork {
     int nbI, kg, a, b;
+    int cls;        // bilinear fix: parity class (a & 1) + 2 (b & 1) of the warp's probes
+    unsigned gidx;  // the lane's own entry in a phase plane of the packed layout (gather base)
     bool any, valid;
 };
 
 __device__ __forceinline__ WarpWork warp_work(const MarchParams &p, long long W, int lane) {
     const int G = min(p.kg_n, 8);
-    const long long npatch = (long long)p.npatch_x * p.npatch_y;
+    const int ncls = p.fix ? 4 : 1;
+    const long long npatch = (long long)p.npatch_x * p.npatch_y * ncls;
     WarpWork r;
     const int kg_lo = (int)(W % G);
     W /= G;
-    const long long patch = W % npatch;
+    long long patch = W % npatch;
     W /= npatch;
+    r.cls = (int)(patch % ncls);
+    patch /= ncls;
     const int kgb_n = p.kg_n / G;
     // a launch covers kg_n consecutive direction groups starting at kg_off, modulo the full circle
     r.kg = ((int)(W % kgb_n) * G + kg_lo + p.kg_off) & (p.ngroups - 1);
@@ -329,15 +381,19 @@ __device__ __forceinline__ WarpWork warp_work(const MarchParams &p, long long W,
     r.any = r.nbI < p.nb;
     const int py = (int)(patch / p.npatch_x), px = (int)(patch - (long long)py * p.npatch_x);
     const int pw = 1 << p.pw_log2;
-    r.a = (px << p.pw_log2) + (lane & (pw - 1));
-    r.b = py * (32 >> p.pw_log2) + (lane >> p.pw_log2);
-    r.valid = r.a < p.npx && r.b < p.npy;
-    if (!r.valid) r.a = r.b = 0;
+    // lane lattice: all probes, or (bilinear fix) the probes of one parity class, spacing 2s
+    const int la = (px << p.pw_log2) + (lane & (pw - 1)), lb = py * (32 >> p.pw_log2) + (lane >> p.pw_log2);
+    const int lx = p.fix ? p.npx >> 1 : p.npx, ly = p.fix ? p.npy >> 1 : p.npy;
+    r.valid = la < lx && lb < ly;
+    r.a = p.fix ? 2 * la + (r.cls & 1) : la;
+    r.b = p.fix ? 2 * lb + (r.cls >> 1) : lb;
+    r.gidx = (unsigned)lb * lx + la;
+    if (!r.valid) { r.a = r.cls & 1; r.b = r.cls >> 1; r.gidx = 0; }
     return r;
 }
 
 __host__ __device__ inline long long march_warps(const MarchParams &p) {
-    return (long long)p.npatch_x * p.npatch_y * p.kg_n * p.nb;
+    return (long long)p.npatch_x * p.npatch_y * (p.fix ? 4 : 1) * p.kg_n * p.nb;
 }
 
 // Number of leading steps of direction k's table that lie inside the box for this lane's probe.
@@ -398,7 +454,8 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
     if (!ww.any) return;
     const int nbI = ww.nbI, kg = ww.kg, a = ww.a, b = ww.b;
     const bool valid = ww.valid;
-    const unsigned probe = (unsigned)b * p.npx + a;
+    const unsigned probe = (unsigned)b * p.npx + a;  // output / parked-state index
+    const unsigned gidx = ww.gidx;                    // gather base in the packed layout
     const int half = (1 << p.shift) >> 1;
     const int Y0 = (b << p.shift) + half;
     const long long ncell = (long long)p.nx * p.ny;
@@ -422,17 +479,26 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
 #pragma unroll
     for (int v = 0; v < LV; v++) acc_s[v][threadIdx.x] = 0.f;
 
-    for (int j = 0; j < 4; j++) {
+    // bilinear fix (p.fix): every ray is traced four times, once towards each parent (slot)
+    const int nsub = p.fix ? 4 : 1;
+    for (int jj = 0; jj < 4 * nsub; jj++) {
+        const int j = p.fix ? jj >> 2 : jj, slot = p.fix ? jj & 3 : 0;
         const long long k = 4LL * kg + j;
+        const long long tid = p.fix ? k * 16 + ww.cls * 4 + slot : k;  // table of this (sub-)ray
         float I[LV], tau[LV], T[LV];
 #pragma unroll
         for (int v = 0; v < LV; v++) { I[v] = 0.f; tau[v] = 0.f; T[v] = 1.f; }
         // cnt == null: the whole cascade lies outside any box of this size (pure boundary term)
         if (p.cnt != nullptr) {
-            const long long o = __ldg(p.off + k);
-            const int n = __ldg(p.cnt + k);
+            const long long o = __ldg(p.off + tid);
+            const int n = __ldg(p.cnt + tid);
             const uint2 *tab = reinterpret_cast<const uint2 *>(p.steps + o);
             int nin = steps_inside(p.xy + o, n, valid, dxlo, dxhi, dylo, dyhi);
+            if (p.fix && n > 0) {  // a sub-ray that starts outside the box is vacuum (reading G10)
+                const unsigned e = __ldg(reinterpret_cast<const unsigned *>(p.xy + o));
+                const int dx = (int)(short)(e & 0xffffu), dy = (int)(short)(e >> 16);
+                if (dx < dxlo || dx > dxhi || dy < dylo || dy > dyhi) nin = 0;
+            }
             int n0 = 0;       // this lane's first step of this launch
             bool has = true;  // banded: the lane has steps in this band
             if constexpr (BANDED) {
@@ -460,18 +526,21 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
             // LINE: photons on this ray travel along -(wx, wy); the line of a cell moving with v is centred at
             // x = -v.w, so a = x_l + v.w  (packed v and x_l carry the factor sqrt(log2 e): phi ~ 2^(-a^2))
             float wx = 0.f, wy = 0.f;
-            if constexpr (LINE) sincospif(2.f * ((float)k + 0.5f) / (float)(4LL * p.ngroups), &wy, &wx);
+            if constexpr (LINE) {
+                if (p.fix) { const float2 d = __ldg(p.subdir + tid); wx = d.x; wy = d.y; }
+                else sincospif(2.f * ((float)k + 0.5f) / (float)(4LL * p.ngroups), &wy, &wx);
+            }
             auto gather = [&](int u, unsigned delta, bool in) {
                 if constexpr (LINE) {
                     const float *src = reinterpret_cast<const float *>(reinterpret_cast<const char *>(chiB) +
-                                                                        (unsigned long long)(probe + delta) * 24ull);
+                                                                        (unsigned long long)(gidx + delta) * 24ull);
                     float t0[2] = {c2[u][0], c2[u][1]}, t1[2] = {c2[u][2], c2[u][3]}, t2[2] = {c2[u][4], c2[u][5]};
                     load_vec_if<2>(src, t0, in);
                     load_vec_if<2>(src + 2, t1, in);
                     load_vec_if<2>(src + 4, t2, in);
                     c2[u][0] = t0[0]; c2[u][1] = t0[1]; c2[u][2] = t1[0]; c2[u][3] = t1[1]; c2[u][4] = t2[0]; c2[u][5] = t2[1];
                 } else {
-                    const unsigned long long d = (unsigned long long)(probe + delta) * (LL * sizeof(float));
+                    const unsigned long long d = (unsigned long long)(gidx + delta) * (LL * sizeof(float));
                     load_vec_if<LL>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(chiB) + d), c2[u], in);
                     load_vec_if<LL>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(SB) + d), S[u], in);
                 }
@@ -486,7 +555,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
                 const uint2 e = __ldg(tab + u);
                 bool in = u < nin && (!BANDED || u >= n0);
                 if constexpr (SPARSE) {  // empty cells (chi = 0 at every wavelength of the batch) are not gathered
-                    const unsigned c = probe + e.x;
+                    const unsigned c = gidx + e.x;
                     if (in) in = (__ldg(occB + (c >> 5)) >> (c & 31)) & 1u;
                 }
                 gather(u, e.x, in);
@@ -498,7 +567,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
             unsigned occ_next = 0u;
             if constexpr (SPARSE) {
                 en_next = __ldg(tab + PD);
-                if (PD < nin && (!BANDED || PD >= n0)) occ_next = __ldg(occB + ((probe + en_next.x) >> 5));
+                if (PD < nin && (!BANDED || PD >= n0)) occ_next = __ldg(occB + ((gidx + en_next.x) >> 5));
             }
             // a1: eq. 16 along the interval, front to back: with tau accumulated,
             // T_n = 2^-tau2_n and the cell's contribution is S (T_{n-1} - T_n)  [= S T (1 - e^{-chi ds})]
@@ -513,7 +582,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
                         en_next = __ldg(tab + st + u + PD + 1);
                         occ_next = 0u;
                         if (st + u + PD + 1 < nin && (!BANDED || st + u + PD + 1 >= n0))
-                            occ_next = __ldg(occB + ((probe + en_next.x) >> 5));
+                            occ_next = __ldg(occB + ((gidx + en_next.x) >> 5));
                     } else {
                         en = __ldg(tab + st + u + PD);
                     }
@@ -552,7 +621,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
                     }
                     // refill the slot with step st + u + PD
                     bool in = st + u + PD < nin && (!BANDED || st + u + PD >= n0);
-                    if constexpr (SPARSE) in = in && ((occ_cur >> ((probe + en.x) & 31)) & 1u);
+                    if constexpr (SPARSE) in = in && ((occ_cur >> ((gidx + en.x) & 31)) & 1u);
                     gather(u, en.x, in);
                     ds[u] = in ? __uint_as_float(en.y) : 0.f;
                 }
@@ -582,6 +651,29 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
             const float *Ib = (2 * k < ndir) ? p.I_above : p.I_below;
 #pragma unroll
             for (int v = 0; v < LV; v++) I[v] = fmaf(T[v], __ldg(Ib + nbI * LL + v / NM), I[v]);
+        } else if (valid && p.fix) {
+            // a3 with the bilinear fix: this sub-ray ends where parent `slot`'s child cone starts; merge it with that
+            // parent alone (eq. 11), then weight it bilinearly.  At the lattice edge both slots of an axis are the
+            // same (clamped) parent, reached by the ray of the slot that is NOT clamped: that slot takes the whole
+            // weight (the oracle traces the same ray twice, with weights 1/4 + 3/4).
+            const int npxu = p.npx >> 1, npyu = p.npy >> 1;
+            int a0, a1, b0, b1;
+            float fa, fb;
+            parent_axis(a, npxu, a0, a1, fa);
+            parent_axis(b, npyu, b0, b1, fb);
+            const int sa = slot & 1, sb = slot >> 1;
+            const int base_a = (a & 1) ? (a - 1) >> 1 : (a >> 1) - 1, base_b = (b & 1) ? (b - 1) >> 1 : (b >> 1) - 1;
+            float wa = sa ? fa : 1.f - fa, wb = sb ? fb : 1.f - fb;
+            if (base_a < 0) wa = sa ? 1.f : 0.f;
+            if (base_a + 1 > npxu - 1) wa = sa ? 0.f : 1.f;
+            if (base_b < 0) wb = sb ? 1.f : 0.f;
+            if (base_b + 1 > npyu - 1) wb = sb ? 0.f : 1.f;
+            const float *up = p.Aup + (((long long)nbI * ndir + k) * npyu) * (long long)npxu * LV;
+            float uq[LV];
+            load_vec<LV>(up + ((long long)(sb ? b1 : b0) * npxu + (sa ? a1 : a0)) * LV, uq);
+            const float wq = wa * wb;
+#pragma unroll
+            for (int v = 0; v < LV; v++) I[v] = wq * fmaf(T[v], uq[v], I[v]);
         } else if (valid) {
             // a3: bilinear over the 4 parents of cascade i+1 (already averaged over the 4 children of
             // direction k when they were written), then eq. 11: I <- I + T * U
@@ -804,7 +896,7 @@ cudaError_t launch_validate(const float *chi, const float *eta, long long n, int
 __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) count_kernel(MarchParams p, unsigned long long *total) {
     const int lane = threadIdx.x & 31;
     const long long W = (long long)blockIdx.x * WARPS_PER_BLOCK + (threadIdx.x >> 5);
-    if (W >= (long long)p.npatch_x * p.npatch_y * p.ngroups || p.cnt == nullptr) return;
+    if (W >= (long long)p.npatch_x * p.npatch_y * (p.fix ? 4 : 1) * p.ngroups || p.cnt == nullptr) return;
     const WarpWork ww = warp_work(p, W, lane);  // batch index is the slowest: W covers batch 0 only
     const int a = ww.a, b = ww.b, kg = ww.kg;
     const int s = 1 << p.shift, half = s >> 1;
@@ -812,17 +904,24 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) count_kernel(MarchParams
     const int dxlo = -(a << p.shift) - half, dxhi = ((p.npx - a) << p.shift) - 1 - half;
     const int dylo = -Y0, dyhi = p.ny - 1 - Y0;
     unsigned long long mine = 0;
-    for (int j = 0; j < 4; j++) {
-        const long long k = 4LL * kg + j;
-        const long long o = __ldg(p.off + k);
-        mine += (unsigned long long)steps_inside(p.xy + o, __ldg(p.cnt + k), ww.valid, dxlo, dxhi, dylo, dyhi);
+    for (int jj = 0; jj < (p.fix ? 16 : 4); jj++) {
+        const long long tid = p.fix ? (4LL * kg + (jj >> 2)) * 16 + ww.cls * 4 + (jj & 3) : 4LL * kg + jj;
+        const long long o = __ldg(p.off + tid);
+        const int n = __ldg(p.cnt + tid);
+        int nin = steps_inside(p.xy + o, n, ww.valid, dxlo, dxhi, dylo, dyhi);
+        if (p.fix && n > 0) {
+            const unsigned e = __ldg(reinterpret_cast<const unsigned *>(p.xy + o));
+            const int dx = (int)(short)(e & 0xffffu), dy = (int)(short)(e >> 16);
+            if (dx < dxlo || dx > dxhi || dy < dylo || dy > dyhi) nin = 0;
+        }
+        mine += (unsigned long long)nin;
     }
     for (int o = 16; o > 0; o >>= 1) mine += __shfl_down_sync(FULL, mine, o);
     if (lane == 0 && mine) atomicAdd(total, mine);
 }
 
 cudaError_t launch_count(const MarchParams &p, unsigned long long *total, cudaStream_t st) {
-    const long long nwarps = (long long)p.npatch_x * p.npatch_y * p.ngroups;
+    const long long nwarps = (long long)p.npatch_x * p.npatch_y * (p.fix ? 4 : 1) * p.ngroups;
     const long long blocks = (nwarps + WARPS_PER_BLOCK - 1) / WARPS_PER_BLOCK;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     count_kernel<<<(unsigned)blocks, WARPS_PER_BLOCK * 32, 0, st>>>(p, total);

@@ -355,3 +355,32 @@ def test_inclined_moving_line_matches_the_oracle(oracle, kw, n):
     atm = A.with_inclinations(A.line_config2(**kw), n)
     e = check(atm, oracle)
     print(atm.name, kw, n, "max rel err", e)
+
+
+# ------------------------------------------------------------------ bilinear fix (f3)
+def _fixed(atm):
+    import dataclasses
+    return dataclasses.replace(atm, name=atm.name + "_fix", bilinear_fix=True)
+
+
+@pytest.mark.parametrize("idx,kw", [
+    (0, dict(nx=64, ny=64, nlambda=1, ncascades=5)),
+    (1, dict(nx=128, ny=128, nlambda=16, ncascades=6)),
+    (2, dict(nx=96, ny=48, nlambda=11, ncascades=5)),
+    (3, dict(nx=128, ny=128, nlambda=8, ncascades=6)),
+    (4, dict(nx=256, ny=64, nlambda=9, ncascades=5)),
+    (0, dict(nx=2, ny=2, nlambda=1, ncascades=2)),
+    (0, dict(nx=16, ny=8, nlambda=3, ncascades=4)),
+])
+def test_bilinear_fix_matches_the_oracle(oracle, idx, kw):
+    """PAPER.md:243 (RC_BILINEAR_FIX): four sub-rays per interval, one towards each parent; all five recipes
+    (boundary illumination, Jbar accumulation, the sparse march of config 4), ragged batches, lattices down
+    to a single parent probe."""
+    atm = _fixed(A.make_config(idx, **kw))
+    e = check(atm, oracle)
+    print(atm.name, kw, "max rel err", e)
+
+
+def test_bilinear_fix_with_inclinations_and_moving_line(oracle):
+    check(_fixed(A.with_inclinations(A.make_config(2, nx=64, ny=64, nlambda=3, ncascades=5), 4)), oracle)
+    check(_fixed(A.line_config2(nx=64, ny=64, nlambda=6, ncascades=5)), oracle)
