@@ -206,6 +206,33 @@ def solve_line(line, xl, ncascades, c0=1.0, I_below=None, I_above=None, weights=
     return out
 
 
+def alo(chi=None, line=None, xl=None, mu=None, w_mu=None):
+    """Diagonal approximate lambda operator of cascade 0 (eq. 17): Lambda*(k) = exp(-tau),
+    tau = chi ds "from the centre to the edge of cell k along direction w".  Cascade 0's directions are the four
+    diagonals: ds = sqrt(2)/2 in the plane, divided by sin(inclination) for an inclined ray.  Returned: the mean
+    over the 4 directions, summed over the inclinations with their weights, [ny][nx][L] float64.  GivenFs mode:
+    chi [ny][nx][L]; line mode: the opacity seen along each diagonal (cell_chi_eta's formula, written out)."""
+    mu = np.zeros(1) if mu is None else np.asarray(mu, np.float64)
+    w_mu = np.ones(1) if w_mu is None else np.asarray(w_mu, np.float64)
+    out = 0.0
+    for m in range(len(mu)):
+        si = np.sqrt(1.0 - mu[m] ** 2)
+        ds = np.sqrt(2.0) / 2.0 / si
+        if line is None:
+            out = out + w_mu[m] * np.exp(-np.asarray(chi, np.float32).astype(np.float64) * ds)
+        else:
+            f = np.asarray(line, np.float32).astype(np.float64)
+            x = np.asarray(xl, np.float64)
+            acc = 0.0
+            for k in range(4):
+                th = 2.0 * np.pi * (k + 0.5) / 4.0
+                a = x[None, None, :] + si * (f[..., 4] * np.cos(th) + f[..., 5] * np.sin(th))[..., None]
+                c = f[..., 0:1] + f[..., 2:3] * np.exp(-a * a) / np.sqrt(np.pi)
+                acc = acc + np.exp(-c * ds) / 4.0
+            out = out + w_mu[m] * acc
+    return out
+
+
 def solve_atmosphere(atm, **kw):
     """Convenience: oracle solve of a paper_2408_14425_b200.atmospheres.Atmosphere-like object."""
     if getattr(atm, "bilinear_fix", False):

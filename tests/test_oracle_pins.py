@@ -624,3 +624,31 @@ def test_F3_bilinear_fix_reduces_the_ringing(oracle):
     assert np.all(err[True] > 0)
     assert np.sqrt(np.mean(err[True] ** 2)) < 0.65 * np.sqrt(np.mean(err[False] ** 2))
     assert err[True].max() < 0.65 * err[False].max()
+
+
+# ----------------------------------------------------------------------------- diagonal ALO (f4)
+def test_A1_alo_is_the_own_cell_transmittance_of_cascade_0(oracle):
+    """eq. 17: Lambda* = exp(-chi ds), ds from the cell centre to its edge along the ray.  Cascade
+    0's interval [0, 1] covers the own cell over sqrt2/2 and the diagonal neighbour over 1 - sqrt2/2 (P13): in an
+    atmosphere whose occupied cells have vacuum diagonal neighbours, the oracle's own cascade-0 transmittances
+    (dump_T, all four directions) ARE the ALO.  Also: vacuum gives 1; weights of the inclinations sum to 1."""
+    rng = np.random.default_rng(3)
+    ny = nx = 16
+    y, x = np.mgrid[0:ny, 0:nx]
+    occ = (x % 2 == 0) & (y % 2 == 0)           # diagonal neighbours of an occupied cell are (odd, odd): empty
+    chi = np.where(occ, rng.uniform(0.1, 3.0, (ny, nx)), 0.0).astype(np.float32)[..., None]
+    d = oracle.solve(chi, chi.copy(), 2, dump_cascade=0)
+    lam = oracle.alo(chi=chi)
+    for k in range(4):
+        assert np.allclose(d["dump_T"][:, :, k, :][occ], lam[occ], rtol=1e-14)
+    assert np.all(lam[~occ] == 1.0)
+    mu, w = A.gauss_radau(4)
+    big = oracle.alo(chi=np.full((2, 2, 1), 1e-9, np.float32), mu=mu, w_mu=w)
+    assert np.allclose(big, 1.0, atol=1e-8)
+    li = oracle.alo(chi=chi, mu=mu, w_mu=w)
+    assert np.all(li[occ] < lam[occ]) and np.all(li[occ] > 0)        # inclined rays see more optical depth
+    # line mode with v = 0 is the GivenFs value of the static opacities
+    a = A.line_config2(nx=8, ny=8, nlambda=3, ncascades=2)
+    a.line[..., 4:6] = 0
+    c, _ = _static_fields(a.line, a.xl)
+    assert np.allclose(oracle.alo(line=a.line, xl=a.xl), np.exp(-c * np.sqrt(0.5)), rtol=1e-12)
