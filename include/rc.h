@@ -146,6 +146,13 @@ int rc_set_lambda_weights(rc_ctx *ctx, const float *w);
 /* Enqueue one full solve.  J_out: device, [ny][nx][nlambda] float32, or [ny][nx] with RC_ACCUM_J. */
 int rc_solve_J(rc_ctx *ctx, float *J_out);
 
+/* Diagonal approximate lambda operator (eq. 17): for the current
+ * atmosphere (either mode) and inclination set, Lambda*[y][x][l] = sum_m w_m <exp(-chi_l ds_m)> over the four
+ * cascade-0 directions, ds_m = (sqrt2/2) / sqrt(1 - mu_m^2) the path from the cell centre to its edge.  "Purely
+ * local ... only computed for cascade 0": an elementwise launch on the context's stream, not synchronised.
+ * alo_out: device, [ny][nx][nlambda] float32. */
+int rc_compute_alo(rc_ctx *ctx, float *alo_out);
+
 /* Same path with HOST buffers: copies chi, eta to the device (workspace, host_io != 0), solves,
  * copies J back, synchronises the stream.  Pinned host memory makes the copies asynchronous. */
 int rc_solve_J_host(rc_ctx *ctx, const float *chi_host, const float *eta_host, int nx, int ny,

@@ -45,6 +45,7 @@ SYMBOLS = {
     "rc_set_lambda_weights": (C.c_int, [C.c_void_p, C.c_void_p]),
     "rc_set_inclinations": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]),
     "rc_solve_J": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "rc_compute_alo": (C.c_int, [C.c_void_p, C.c_void_p]),
     "rc_solve_J_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p]),
     "rc_set_timing": (C.c_int, [C.c_void_p, C.c_int]),
     "rc_get_stats": (C.c_int, [C.c_void_p, C.POINTER(rc_stats)]),
@@ -211,6 +212,14 @@ class RadianceCascades:
                                              nx, ny, L, C.c_void_p(out_host.data_ptr())))
         self.shape = (ny, nx, L)
         return out_host
+
+    def compute_alo(self):
+        """Diagonal ALO of cascade 0 (eq. 17) of the current atmosphere: CUDA tensor [ny][nx][nlambda]."""
+        import torch
+        out = torch.empty(self.shape, dtype=torch.float32, device=f"cuda:{self.device}")
+        self.set_stream()
+        self._check(self.lib.rc_compute_alo(self.handle, C.c_void_p(out.data_ptr())))
+        return out
 
     def set_timing(self, nsets=1):
         self._check(self.lib.rc_set_timing(self.handle, int(nsets)))

@@ -254,7 +254,7 @@ bool make_plan_uncached(const rc_config &cfg, int nm, bool line, int nx, int ny,
     if (P.has_occ) { P.occ = cur; cur += align_up((ncell / 32) * P.nb * sizeof(unsigned)); }
     if (line) {
         P.chiT = cur; cur += align_up(ncell * 6 * sizeof(float));
-        P.xls = cur;  cur += align_up(P.Lpad * sizeof(float));
+        P.xls = cur;  cur += align_up(2 * P.Lpad * sizeof(float));  // x_l sqrt(log2 e), then x_l
     } else {
         P.chiT = cur; cur += field;
         P.ST = cur;   cur += field;
@@ -485,8 +485,11 @@ int rc_set_line_atmosphere(rc_ctx *ctx, const float *line, int nx, int ny, const
     }
     for (int l = 0; l < nlambda; l++)
         if (!std::isfinite(x_lambda[l])) return fail(ctx, RC_ERR_BAD_VALUE, "x_lambda[%d] is not finite", l);
-    std::vector<float> h((size_t)ctx->plan.Lpad, 0.f);
-    for (int l = 0; l < nlambda; l++) h[l] = (float)((double)x_lambda[l] * 1.2011224087864498);  // sqrt(log2 e)
+    std::vector<float> h((size_t)2 * ctx->plan.Lpad, 0.f);
+    for (int l = 0; l < nlambda; l++) {
+        h[l] = (float)((double)x_lambda[l] * 1.2011224087864498);  // sqrt(log2 e)
+        h[(size_t)ctx->plan.Lpad + l] = x_lambda[l];
+    }
     RC_CUDA(ctx, cudaMemcpyAsync(ctx->ws + ctx->plan.xls, h.data(), h.size() * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
     RC_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     ctx->line = line;
@@ -728,6 +731,24 @@ int rc_solve_J_host(rc_ctx *ctx, const float *chi_host, const float *eta_host, i
     const size_t nout = (ctx->cfg.flags & RC_ACCUM_J) ? (size_t)nx * ny * sizeof(float) : n;
     RC_CUDA(ctx, cudaMemcpyAsync(J_host, dJ, nout, cudaMemcpyDeviceToHost, ctx->stream));
     RC_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return RC_OK;
+}
+
+// Diagonal ALO of cascade 0 (eq. 17) for the current atmosphere and inclination set.
+int rc_compute_alo(rc_ctx *ctx, float *alo_out) {
+    if (!ctx || !alo_out) return ctx ? fail(ctx, RC_ERR_NULL_ARG, "null alo_out") : RC_ERR_NULL_ARG;
+    if (!ctx->have_atm) return fail(ctx, RC_ERR_NO_ATMOSPHERE, "call rc_set_atmosphere first");
+    RC_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    rc::AloParams ap;
+    ap.chi = ctx->line ? nullptr : ctx->chi;
+    ap.line = ctx->line;
+    ap.xl = ctx->line ? (const float *)(ctx->ws + ctx->plan.xls) + ctx->plan.Lpad : nullptr;  // unscaled copy
+    ap.out = alo_out;
+    ap.ncell = (long long)ctx->plan.nx * ctx->plan.ny;
+    ap.L = ctx->plan.L;
+    ap.nm = ctx->nm;
+    for (int m = 0; m < 8; m++) { ap.f[m] = ctx->incl_f[m]; ap.w[m] = ctx->incl_w[m]; }
+    RC_CUDA(ctx, rc::launch_alo(ap, ctx->stream));
     return RC_OK;
 }
 

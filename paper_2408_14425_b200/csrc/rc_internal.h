@@ -71,6 +71,16 @@ struct PackParams {
     int nx, ny, L, nb, shift;
 };
 
+struct AloParams {
+    const float *chi;   // GivenFs: [ncell][L]; null in line mode
+    const float *line;  // line mode: [ncell][6] as given by the caller; else null
+    const float *xl;    // line mode: [L] wavelengths (Doppler widths, unscaled), device
+    float *out;         // [ncell][L]
+    long long ncell;
+    int L, nm;
+    float f[8], w[8];   // path scale and weight of each inclination
+};
+
 struct TableBuildParams {
     Step *steps;
     StepXY *xy;
@@ -93,6 +103,7 @@ cudaError_t launch_reduce_jbar(const float *Jpart, float *Jbar, long long ncell,
 cudaError_t launch_count(const MarchParams &p, unsigned long long *total, cudaStream_t st);
 cudaError_t launch_gather_probe(const float *buf, unsigned long long nsector, int iters, int blocks, float *sink, cudaStream_t st);
 cudaError_t launch_count_empty(const float *chi, long long ncell, int L, int *mark, unsigned long long *count, cudaStream_t st);
+cudaError_t launch_alo(const AloParams &p, cudaStream_t st);
 cudaError_t launch_validate(const float *chi, const float *eta, long long n, int *flag, cudaStream_t st);
 
 }  // namespace rc

@@ -929,6 +929,44 @@ cudaError_t launch_count(const MarchParams &p, unsigned long long *total, cudaSt
 }
 
 // ------------------------------------------------------------------------------------------------
+// Diagonal approximate lambda operator of cascade 0 (eq. 17): Lambda* = exp(-chi ds), ds from
+// the cell centre to its edge along a cascade-0 ray = sqrt2/2 (diagonals), over sin(inclination) when inclined;
+// mean over the 4 directions, summed over the inclinations with their weights.  One thread per (cell, wavelength).
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) alo_kernel(AloParams p) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= p.ncell * p.L) return;
+    const float HALF_DIAG = 0.70710678118654752f;
+    float out = 0.f;
+    if (p.line == nullptr) {
+        const float c = __ldg(p.chi + i);
+        for (int m = 0; m < p.nm; m++) out = fmaf(p.w[m], expf(-c * HALF_DIAG * p.f[m]), out);
+    } else {
+        const long long cell = i / p.L;
+        const int l = (int)(i - cell * p.L);
+        const float *q = p.line + cell * 6;
+        const float chi_c = __ldg(q), chi_l = __ldg(q + 2), vx = __ldg(q + 4), vy = __ldg(q + 5), x = __ldg(p.xl + l);
+        for (int m = 0; m < p.nm; m++) {
+            float acc = 0.f;
+            for (int k = 0; k < 4; k++) {  // the four diagonals; photons travel along -w: a = x_l + v.w sin(inclination)
+                const float wx = (k == 0 || k == 3) ? HALF_DIAG : -HALF_DIAG, wy = k < 2 ? HALF_DIAG : -HALF_DIAG;
+                const float a = x + (vx * wx + vy * wy) / p.f[m];
+                const float c = fmaf(chi_l, expf(-a * a) * 0.5641895835477563f, chi_c);
+                acc += expf(-c * HALF_DIAG * p.f[m]);
+            }
+            out = fmaf(p.w[m], 0.25f * acc, out);
+        }
+    }
+    p.out[i] = out;
+}
+
+cudaError_t launch_alo(const AloParams &p, cudaStream_t st) {
+    const long long n = p.ncell * p.L;
+    alo_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(p);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
 // Measurement aid (rc_probe_gather_bandwidth): the march's access pattern with nothing else — every
 // warp reads pseudo-random 1 KB runs (32 lanes x 32 B, LDG.256), two in flight per warp, 48 warps per
 // SM — over a region of `nsector` 32-byte sectors.  Region inside L2: the L2 -> SM gather ceiling.

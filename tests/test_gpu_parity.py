@@ -384,3 +384,23 @@ def test_bilinear_fix_matches_the_oracle(oracle, idx, kw):
 def test_bilinear_fix_with_inclinations_and_moving_line(oracle):
     check(_fixed(A.with_inclinations(A.make_config(2, nx=64, ny=64, nlambda=3, ncascades=5), 4)), oracle)
     check(_fixed(A.line_config2(nx=64, ny=64, nlambda=6, ncascades=5)), oracle)
+
+
+# ------------------------------------------------------------------ diagonal ALO (f4)
+def test_alo_matches_the_oracle(oracle):
+    """rc_compute_alo (eq. 17) against the oracle's plain definition: GivenFs, with inclinations, and the
+    moving line with inclinations (direction-dependent opacity on the four diagonals)."""
+    import torch
+    from paper_2408_14425_b200 import binding
+    mu, w = A.gauss_radau(8)
+    for atm in (A.make_config(1, nx=64, ny=64, nlambda=5, ncascades=5),
+                A.with_inclinations(A.make_config(4, nx=128, ny=64, nlambda=7, ncascades=5), 8),
+                A.with_inclinations(A.line_config2(nx=64, ny=32, nlambda=9, ncascades=5), 4),
+                A.line_config2(nx=32, ny=32, nlambda=4, ncascades=4)):
+        J, rc = binding.solve_atmosphere(atm)
+        got = rc.compute_alo().cpu().numpy().astype(np.float64)
+        rc.close()
+        want = oracle.alo(chi=atm.chi, line=atm.line, xl=atm.xl, mu=atm.mu, w_mu=atm.w_mu)
+        assert got.shape == want.shape
+        # exp(-tau) in fp32: relative error ~ tau x 6e-8 (tau up to ~100 here); flushed values compare absolutely
+        assert np.all(np.abs(got - want) <= 2e-5 * want + 1e-37), atm.name
