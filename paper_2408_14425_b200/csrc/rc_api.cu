@@ -67,6 +67,7 @@ struct rc_ctx {
     // developer overrides (environment, read by rc_create): RC_MARCH_VARIANT = 0..3 (register ring depth /
     // occupancy of march_kernel), RC_PATCH_LOG2 = 2..5 forces the lane patch width for cascades >= RC_PATCH_FROM
     int tune_variant = 2, tune_patch = -1, tune_patch_from = 0;
+    float tau_cut = 126.f;  // early-exit threshold on tau log2(e); 126: the fp32 transmittance is exactly 0
     // 2.5D inclination quadrature (rc_set_inclinations); nm = 1, f = w = 1: flatland
     int nm = 1;
     float incl_f[8] = {1, 1, 1, 1, 1, 1, 1, 1}, incl_w[8] = {1, 0, 0, 0, 0, 0, 0, 0};
@@ -331,6 +332,7 @@ int rc_create(rc_ctx **out, const rc_config *cfg) {
     if (const char *e = std::getenv("RC_MARCH_VARIANT")) ctx->tune_variant = std::max(0, std::min(3, std::atoi(e)));
     if (const char *e = std::getenv("RC_PATCH_LOG2")) ctx->tune_patch = std::max(2, std::min(5, std::atoi(e)));
     if (const char *e = std::getenv("RC_PATCH_FROM")) ctx->tune_patch_from = std::atoi(e);
+    if (const char *e = std::getenv("RC_TAU_CUT")) ctx->tau_cut = std::max(1.f, (float)std::atof(e));
     *out = ctx;
     return RC_OK;
 }
@@ -567,6 +569,7 @@ static rc::MarchParams march_params(const rc_ctx *ctx, int i, float *J_out) {
     mp.ngroups = 1 << (2 * i);
     mp.mode = i > 0 ? 0 : (accum ? 2 : 1);
     mp.early_exit = (ctx->cfg.flags & RC_NO_EARLY_EXIT) ? 0 : 1;
+    mp.tau_cut = ctx->tau_cut;
     mp.pw_log2 = ctx->tune_patch >= 0 && i >= ctx->tune_patch_from ? ctx->tune_patch : c.pw_log2;
     mp.fix = c.fix && !c.empty;
     mp.subdir = mp.fix ? (const float2 *)(ctx->ws + c.subdir_off) : nullptr;

@@ -50,6 +50,7 @@ struct MarchParams {
     int ngroups;           // direction groups = 4^cascade (4 directions each)
     int mode;
     int early_exit;
+    float tau_cut;         // a warp stops once every live lane has tau log2(e) above this at all its channels (126: T == 0 exactly)
     int pw_log2;           // one warp's 32 probes form a patch 2^pw_log2 wide, 32 >> pw_log2 high
     int npatch_x, npatch_y;  // patches per axis
     int fix;               // bilinear fix: 4 sub-rays per ray, lanes = probes of one parity class,

@@ -630,7 +630,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
 #pragma unroll
                     for (int v = 1; v < LV; v++) tmin = fminf(tmin, tau[v]);
                     // every live lane opaque at every wavelength: T is exactly 0, nothing more can arrive
-                    if (__all_sync(FULL, st + PD >= nin || tmin > 126.f)) break;
+                    if (__all_sync(FULL, st + PD >= nin || tmin > p.tau_cut)) break;
                 }
             }
             if constexpr (BANDED) {
