@@ -31,9 +31,9 @@ from paper_2408_14425_b200 import atmospheres  # noqa: E402
 METRIC = "probe-ray-wavelength segments/sec"
 UNIT = "seg-lambda/s"
 SM_COUNT, MUFU_PER_CLK_SM = 148, 16  # one ex2 per segment-wavelength; DESIGN.md §7
-# dram__bytes_read.sum + dram__bytes_write.sum of the dominant launch, from the committed ncu --set full
-# capture (profiles/ncu_r1b_march.md): configs[2], march_kernel cascade 5
-NCU_TRAFFIC_BYTES = {(2, 5): 9.20e9}
+# dram__bytes_read.sum + dram__bytes_write.sum of the dominant launch (march_kernel, cascade 5), from the committed
+# ncu --set full captures (profiles/ncu_r1b_march.md, ncu_r1c_modes.md), keyed by (mode, config, cascade)
+NCU_TRAFFIC_BYTES = {("flat", 2, 5): 9.20e9, ("incl8", 2, 5): 7.88e9, ("line", 2, 5): 1.03e9, ("flat", 4, 5): 8.83e9}
 
 
 def peaks():
@@ -266,7 +266,11 @@ def main():
         casc_bytes = 2 * 4 * atm.nx * atm.ny * atm.nlambda * nincl  # read merged cascade i+1, write cascade i
         alg_bytes = 8 * seg[dom] * atm.nlambda + casc_bytes  # chi+eta gather: 8 B per segment-wavelength
         ach = alg_bytes / (ms_march[dom] * 1e-3) / 1e9
-        sfu_peak = SM_COUNT * MUFU_PER_CLK_SM * sm_max_mhz * 1e6
+        mode = ("line" if atm.line is not None else "flat") + (f"_incl{nincl}" if atm.line is not None and nincl > 1 else
+                                                                   f"incl{nincl}" if nincl > 1 else "")
+        mode = {"flatincl8": "incl8"}.get(mode, mode) + ("_fix" if args.bilinear_fix else "")
+        mufu_per_unit = 3 if atm.line is not None else 1  # line mode: ex2 (profile), rcp (eta/chi), ex2 (transmittance)
+        sfu_peak = SM_COUNT * MUFU_PER_CLK_SM * sm_max_mhz * 1e6 / mufu_per_unit
         ach_alu = seg[dom] * atm.nlambda * nincl / (ms_march[dom] * 1e-3)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -280,8 +284,8 @@ def main():
             "solve_ms": ms_step,
             "hbm_effective_frac": (8 * segl_per_step + 2 * casc_bytes * atm.ncascades) / (ms_step * 1e-3) / 1e9 / hbm_peak,
             "roofline": {"bound": "hbm", "kernel": f"march_kernel<{st.lambda_batch}> cascade {dom}", "achieved": ach,
-                         "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak, "traffic": NCU_TRAFFIC_BYTES.get((args.config, dom)),
-                         "traffic_unit": "bytes per launch (ncu --set full, profiles/ncu_r1b_march.md)",
+                         "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak, "traffic": NCU_TRAFFIC_BYTES.get((mode, args.config, dom)),
+                         "traffic_unit": "bytes per launch (ncu --set full; profiles/ncu_r1b_march.md, ncu_r1c_modes.md)",
                          "algorithmic_bytes": alg_bytes,
                          "peak_source": peak_src, "ms_per_launch": ms_march[dom],
                          "note": "effective: algorithmic gather bytes (8 B per segment-wavelength) are mostly served "
@@ -290,7 +294,7 @@ def main():
                             "peak_source": "rc_probe_gather_bandwidth(64 MB), measured in this run: random 1 KB warp-wide runs "
                                            "(LDG.256), 48 warps/SM, region L2-resident",
                             "hbm_gather_gbs_1GB_region": hbm_gather_gbs},
-            "roofline_alu": {"bound": "alu", "pipe": "MUFU.EX2, 16/clk/SM x 148 SMs at sm_max_mhz", "achieved": ach_alu,
+            "roofline_alu": {"bound": "alu", "pipe": f"MUFU, 16/clk/SM x 148 SMs at sm_max_mhz, {mufu_per_unit} per unit", "achieved": ach_alu,
                              "peak": sfu_peak, "unit": UNIT, "frac": ach_alu / sfu_peak},
             "per_cascade_ms": {"march": ms_march, "pack": [st.ms_pack[i] for i in range(atm.ncascades)]},
             "segments_per_cascade": seg,
