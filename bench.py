@@ -194,6 +194,7 @@ def main():
     rc.set_lambda_weights(atm.weights)
     seg = rc.count_segments()
     l2_gather_gbs = rc.probe_gather_bandwidth(64)      # L2 -> SM ceiling of the gather pattern (64 MB region)
+    tma_bulk_gbs = rc.probe_bulk_copy_bandwidth(64)    # the same pattern through TMA bulk copies + shared memory
     hbm_gather_gbs = rc.probe_gather_bandwidth(1024) if rc._ws.numel() > (1100 << 20) else None
     nincl = 1 if atm.mu is None else len(atm.mu)
     segl_per_step = sum(seg) * atm.nlambda * nincl
@@ -293,7 +294,8 @@ def main():
             "roofline_l2": {"bound": "l2", "achieved": ach, "peak": l2_gather_gbs, "unit": "GB/s", "frac": ach / l2_gather_gbs,
                             "peak_source": "rc_probe_gather_bandwidth(64 MB), measured in this run: random 1 KB warp-wide runs "
                                            "(LDG.256), 48 warps/SM, region L2-resident",
-                            "hbm_gather_gbs_1GB_region": hbm_gather_gbs},
+                            "hbm_gather_gbs_1GB_region": hbm_gather_gbs,
+                            "tma_bulk_copy_gbs_same_pattern": tma_bulk_gbs},
             "roofline_alu": {"bound": "alu", "pipe": f"MUFU, 16/clk/SM x 148 SMs at sm_max_mhz, {mufu_per_unit} per unit", "achieved": ach_alu,
                              "peak": sfu_peak, "unit": UNIT, "frac": ach_alu / sfu_peak},
             "per_cascade_ms": {"march": ms_march, "pack": [st.ms_pack[i] for i in range(atm.ncascades)]},

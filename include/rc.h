@@ -176,6 +176,11 @@ int rc_count_segments(rc_ctx *ctx, int64_t *per_cascade);
  * Runs on the context's stream and synchronises it.  RC_ERR_BAD_VALUE if the region does not fit. */
 int rc_probe_gather_bandwidth(rc_ctx *ctx, int mbytes, double *gbs);
 
+/* The same pattern staged through shared memory by the TMA bulk-copy engine (per warp a ring of 4 stages x
+ * 2 KB filled by `cp.async.bulk` 1 KB copies completing on mbarriers, read back with LDS.128; 24 warps per SM):
+ * the alternative design DESIGN.md §7 measures the LDG path against.  Same arguments and errors. */
+int rc_probe_bulk_copy_bandwidth(rc_ctx *ctx, int mbytes, double *gbs);
+
 const char *rc_last_error(const rc_ctx *ctx);
 const char *rc_version(void);
 int rc_destroy(rc_ctx *ctx);

@@ -51,6 +51,7 @@ SYMBOLS = {
     "rc_get_stats": (C.c_int, [C.c_void_p, C.POINTER(rc_stats)]),
     "rc_count_segments": (C.c_int, [C.c_void_p, C.c_void_p]),
     "rc_probe_gather_bandwidth": (C.c_int, [C.c_void_p, C.c_int, C.POINTER(C.c_double)]),
+    "rc_probe_bulk_copy_bandwidth": (C.c_int, [C.c_void_p, C.c_int, C.POINTER(C.c_double)]),
     "rc_last_error": (C.c_char_p, [C.c_void_p]),
     "rc_version": (C.c_char_p, []),
     "rc_destroy": (C.c_int, [C.c_void_p]),
@@ -234,6 +235,12 @@ class RadianceCascades:
         """GB/s of the march's gather pattern alone over the first `mbytes` MB of the workspace."""
         gbs = C.c_double(0.0)
         self._check(self.lib.rc_probe_gather_bandwidth(self.handle, int(mbytes), C.byref(gbs)))
+        return float(gbs.value)
+
+    def probe_bulk_copy_bandwidth(self, mbytes=64):
+        """GB/s of the same pattern staged through shared memory with TMA bulk copies (the design not taken)."""
+        gbs = C.c_double(0.0)
+        self._check(self.lib.rc_probe_bulk_copy_bandwidth(self.handle, int(mbytes), C.byref(gbs)))
         return float(gbs.value)
 
     def get_stats(self) -> rc_stats:

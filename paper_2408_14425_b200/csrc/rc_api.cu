@@ -755,8 +755,9 @@ int rc_compute_alo(rc_ctx *ctx, float *alo_out) {
     return RC_OK;
 }
 
-// Achieved GB/s of the march's gather pattern alone over the first `mbytes` MB of the workspace.
-int rc_probe_gather_bandwidth(rc_ctx *ctx, int mbytes, double *gbs) {
+// Achieved GB/s of the march's gather pattern alone over the first `mbytes` MB of the workspace:
+// path 0 = LDG.256 (what the march uses), path 1 = TMA bulk copies into a shared-memory ring.
+static int probe_bandwidth(rc_ctx *ctx, int mbytes, int path, double *gbs) {
     if (!ctx || !gbs) return ctx ? fail(ctx, RC_ERR_NULL_ARG, "null output") : RC_ERR_NULL_ARG;
     if (!ctx->ws) return fail(ctx, RC_ERR_NO_WORKSPACE, "rc_set_workspace has not been called");
     const size_t bytes = (size_t)mbytes << 20;
@@ -765,15 +766,19 @@ int rc_probe_gather_bandwidth(rc_ctx *ctx, int mbytes, double *gbs) {
     RC_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
     cudaDeviceProp prop;
     RC_CUDA(ctx, cudaGetDeviceProperties(&prop, ctx->cfg.device));
-    const int blocks = prop.multiProcessorCount * 6, iters = 2048;  // 48 warps per SM
+    const int blocks = prop.multiProcessorCount * 6, iters = 2048;  // LDG path: 48 warps per SM
     float *sink = (float *)(ctx->ws + bytes);
     cudaEvent_t e0, e1;
     RC_CUDA(ctx, cudaEventCreate(&e0));
     RC_CUDA(ctx, cudaEventCreate(&e1));
     float best = 1e30f;
+    long long moved = (long long)blocks * 8 * iters * 1024LL;
     for (int rep = 0; rep < 4; rep++) {  // the first pass also brings the region into L2
         RC_CUDA(ctx, cudaEventRecord(e0, ctx->stream));
-        RC_CUDA(ctx, rc::launch_gather_probe((const float *)ctx->ws, bytes / 32, iters, blocks, sink, ctx->stream));
+        if (path == 0)
+            RC_CUDA(ctx, rc::launch_gather_probe((const float *)ctx->ws, bytes / 32, iters, blocks, sink, ctx->stream));
+        else
+            RC_CUDA(ctx, rc::launch_bulk_probe((const float *)ctx->ws, bytes / 32, iters, prop.multiProcessorCount, sink, ctx->stream, &moved));
         RC_CUDA(ctx, cudaEventRecord(e1, ctx->stream));
         RC_CUDA(ctx, cudaEventSynchronize(e1));
         float ms = 0.f;
@@ -782,9 +787,12 @@ int rc_probe_gather_bandwidth(rc_ctx *ctx, int mbytes, double *gbs) {
     }
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
-    *gbs = (double)blocks * 8 * iters * 1024.0 / (best * 1e-3) / 1e9;
+    *gbs = (double)moved / (best * 1e-3) / 1e9;
     return RC_OK;
 }
+
+int rc_probe_gather_bandwidth(rc_ctx *ctx, int mbytes, double *gbs) { return probe_bandwidth(ctx, mbytes, 0, gbs); }
+int rc_probe_bulk_copy_bandwidth(rc_ctx *ctx, int mbytes, double *gbs) { return probe_bandwidth(ctx, mbytes, 1, gbs); }
 
 int rc_get_stats(rc_ctx *ctx, rc_stats *out) {
     if (!ctx || !out) return RC_ERR_NULL_ARG;

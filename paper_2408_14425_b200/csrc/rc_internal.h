@@ -105,6 +105,7 @@ cudaError_t launch_count(const MarchParams &p, unsigned long long *total, cudaSt
 cudaError_t launch_gather_probe(const float *buf, unsigned long long nsector, int iters, int blocks, float *sink, cudaStream_t st);
 cudaError_t launch_count_empty(const float *chi, long long ncell, int L, int *mark, unsigned long long *count, cudaStream_t st);
 cudaError_t launch_alo(const AloParams &p, cudaStream_t st);
+cudaError_t launch_bulk_probe(const float *buf, unsigned long long nsector, int iters, int sms, float *sink, cudaStream_t st, long long *bytes);
 cudaError_t launch_validate(const float *chi, const float *eta, long long n, int *flag, cudaStream_t st);
 
 }  // namespace rc

@@ -995,6 +995,61 @@ __global__ void __launch_bounds__(256) gather_probe_kernel(const float *buf, uns
     if (acc == 12345.678f) sink[0] = acc;  // never true in practice: keeps the loads alive
 }
 
+// The same pattern staged through shared memory with the TMA bulk-copy engine instead of LDG: every warp owns a
+// ring of D = 4 stages x 2 KB, one lane issues two 1 KB `cp.async.bulk` copies per step (SASS: UBLKCP) that
+// complete on an mbarrier, all lanes then read their 2 x 32 bytes with LDS.128.  This is the "TMA staging of
+// the grid tile" design measured against the LDG path in DESIGN.md §7 (it is slower for 1 KB runs, so the
+// march does not use it); kept as a probe so that the comparison can be repeated.
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+template <int D, int WARPS>
+__global__ void __launch_bounds__(WARPS * 32) bulk_probe_kernel(const float *buf, unsigned long long nsector, int iters, float *sink) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const unsigned warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    unsigned char *ring = smem + (size_t)w * D * 2048;
+    unsigned long long *bars = reinterpret_cast<unsigned long long *>(smem + (size_t)WARPS * D * 2048) + w * D;
+    if (lane == 0)
+        for (int d = 0; d < D; d++) asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(bars + d)));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    __syncwarp();
+    auto issue = [&](int it) {
+        const unsigned bar = smem_u32(bars + it % D), dst = smem_u32(ring + (it % D) * 2048);
+        const unsigned h = hash32(warp * 7919u + it);
+        const float *s0 = buf + (h % (nsector - 64)) * 8, *s1 = buf + (hash32(h) % (nsector - 64)) * 8;
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], 2048;" ::"r"(bar) : "memory");
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], 1024, [%2];"
+                     ::"r"(dst), "l"(s0), "r"(bar) : "memory");
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], 1024, [%2];"
+                     ::"r"(dst + 1024), "l"(s1), "r"(bar) : "memory");
+    };
+    if (lane == 0)
+        for (int d = 0; d < D - 1 && d < iters; d++) issue(d);
+    float acc = 0.f;
+    for (int it = 0; it < iters; it++) {
+        const unsigned bar = smem_u32(bars + it % D), parity = (it / D) & 1;
+        asm volatile("{\n\t.reg .pred q;\n\tW_%=:\n\tmbarrier.try_wait.parity.shared::cta.b64 q, [%0], %1;\n\t@!q bra W_%=;\n\t}"
+                     ::"r"(bar), "r"(parity) : "memory");
+        const float4 *s4 = reinterpret_cast<const float4 *>(ring + (it % D) * 2048);
+        const float4 a = s4[lane * 2], b = s4[lane * 2 + 1], c = s4[64 + lane * 2], d = s4[64 + lane * 2 + 1];
+        __syncwarp();
+        if (lane == 0 && it + D - 1 < iters) issue(it + D - 1);
+        acc += a.x + a.y + a.z + a.w + b.x + b.y + b.z + b.w + c.x + c.y + c.z + c.w + d.x + d.y + d.z + d.w;
+    }
+    if (acc == 12345.678f) sink[0] = acc;
+}
+
+cudaError_t launch_bulk_probe(const float *buf, unsigned long long nsector, int iters, int sms, float *sink, cudaStream_t st, long long *bytes) {
+    constexpr int D = 4, WARPS = 8;
+    const size_t smem = (size_t)WARPS * D * 2048 + WARPS * D * 8;
+    cudaError_t e = cudaFuncSetAttribute(bulk_probe_kernel<D, WARPS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    const int blocks = sms * 3;  // 24 warps per SM, 192 KB of staging per SM
+    bulk_probe_kernel<D, WARPS><<<blocks, WARPS * 32, smem, st>>>(buf, nsector, iters, sink);
+    *bytes = (long long)blocks * WARPS * iters * 2048LL;
+    return cudaGetLastError();
+}
+
 cudaError_t launch_gather_probe(const float *buf, unsigned long long nsector, int iters, int blocks, float *sink, cudaStream_t st) {
     gather_probe_kernel<<<blocks, 256, 0, st>>>(buf, nsector, iters, sink);
     return cudaGetLastError();
