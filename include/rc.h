@@ -93,6 +93,24 @@ typedef struct {
     int64_t empty_cells;                  /* cells with chi == 0 at every wavelength (counted by rc_set_atmosphere) */
 } rc_stats;
 
+/* The launch plan the library would use for a problem, computed on the host alone (no device, no context):
+ * what the tests of the host logic and capacity planning read. */
+typedef struct {
+    size_t workspace_bytes;            /* = rc_workspace_bytes(..., host_io = 0) for the same arguments */
+    int lambda_batch;                  /* wavelengths per thread */
+    int channels;                      /* lambda_batch x inclinations carried by one thread (<= 8) */
+    int nbatches;                      /* wavelength batches per launch */
+    int nbands, band_axis;             /* L2 banding: bands (1 = none) along rows (0) or columns (1) */
+    int cascade_empty[RC_MAX_CASCADES];   /* interval wholly outside any box of this size: boundary term only */
+    int cascade_banded[RC_MAX_CASCADES];  /* marched band by band */
+    int patch_w[RC_MAX_CASCADES];      /* a warp's 32 probes form a patch patch_w wide, 32 / patch_w high */
+    int64_t table_steps[RC_MAX_CASCADES]; /* step-table capacity, all directions (x16 with RC_BILINEAR_FIX) */
+} rc_plan_info;
+
+/* cfg->device is ignored.  line_mode != 0: rc_set_line_atmosphere.  RC_ERR_BAD_SHAPE / RC_ERR_BAD_VALUE as the
+ * calls it mirrors. */
+int rc_plan_query(const rc_config *cfg, int ninclinations, int line_mode, int nx, int ny, int nlambda, rc_plan_info *out);
+
 /* Create a context on cfg->device.  Fails with RC_ERR_NO_DEVICE unless that device is sm_100. */
 int rc_create(rc_ctx **out, const rc_config *cfg);
 

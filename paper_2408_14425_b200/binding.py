@@ -33,8 +33,26 @@ class rc_stats(C.Structure):
                 ("workspace_bytes", C.c_size_t), ("empty_cells", C.c_int64)]
 
 
+class rc_plan_info(C.Structure):
+    _fields_ = [("workspace_bytes", C.c_size_t), ("lambda_batch", C.c_int), ("channels", C.c_int), ("nbatches", C.c_int),
+                ("nbands", C.c_int), ("band_axis", C.c_int), ("cascade_empty", C.c_int * RC_MAX_CASCADES),
+                ("cascade_banded", C.c_int * RC_MAX_CASCADES), ("patch_w", C.c_int * RC_MAX_CASCADES),
+                ("table_steps", C.c_int64 * RC_MAX_CASCADES)]
+
+
+def plan_query(ncascades, nx, ny, nlambda, ninclinations=1, line_mode=False, c0_interval=1.0, lambda_batch=0, flags=0):
+    """Host-only: the launch plan for a problem (no device needed)."""
+    cfg = rc_config(int(ncascades), float(c0_interval), 0, int(lambda_batch), int(flags))
+    info = rc_plan_info()
+    rc = load().rc_plan_query(C.byref(cfg), int(ninclinations), int(bool(line_mode)), int(nx), int(ny), int(nlambda), C.byref(info))
+    if rc != RC_OK:
+        raise RcError(rc, "rc_plan_query failed")
+    return info
+
+
 # every symbol include/rc.h declares: name -> (restype, argtypes)
 SYMBOLS = {
+    "rc_plan_query": (C.c_int, [C.POINTER(rc_config), C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(rc_plan_info)]),
     "rc_create": (C.c_int, [C.POINTER(C.c_void_p), C.POINTER(rc_config)]),
     "rc_workspace_bytes": (C.c_size_t, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int]),
     "rc_set_workspace": (C.c_int, [C.c_void_p, C.c_void_p, C.c_size_t]),

@@ -309,6 +309,29 @@ const char *rc_version(void) { return "rc-b200 0.1 (sm_100a)"; }
 
 const char *rc_last_error(const rc_ctx *ctx) { return ctx ? ctx->err : "null context"; }
 
+int rc_plan_query(const rc_config *cfg, int ninclinations, int line_mode, int nx, int ny, int nlambda, rc_plan_info *out) {
+    if (!cfg || !out) return RC_ERR_NULL_ARG;
+    if (cfg->ncascades < 1 || cfg->ncascades > RC_MAX_CASCADES || !(cfg->c0_interval > 0.f) || !std::isfinite(cfg->c0_interval))
+        return RC_ERR_BAD_VALUE;
+    if (ninclinations != 1 && ninclinations != 2 && ninclinations != 4 && ninclinations != 8) return RC_ERR_BAD_VALUE;
+    Plan P;
+    if (!make_plan(*cfg, ninclinations, line_mode != 0, nx, ny, nlambda, false, P, nullptr)) return RC_ERR_BAD_SHAPE;
+    std::memset(out, 0, sizeof(*out));
+    out->workspace_bytes = P.total;
+    out->lambda_batch = P.LV;
+    out->channels = P.LV * P.NM;
+    out->nbatches = P.nb;
+    out->nbands = P.nbands;
+    out->band_axis = P.band_axis;
+    for (int i = 0; i < cfg->ncascades; i++) {
+        out->cascade_empty[i] = P.c[i].empty;
+        out->cascade_banded[i] = P.c[i].banded;
+        out->patch_w[i] = 1 << P.c[i].pw_log2;
+        out->table_steps[i] = P.c[i].slots;
+    }
+    return RC_OK;
+}
+
 int rc_create(rc_ctx **out, const rc_config *cfg) {
     if (!out || !cfg) return RC_ERR_NULL_ARG;
     *out = nullptr;
