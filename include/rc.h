@@ -148,6 +148,11 @@ int rc_set_line_atmosphere(rc_ctx *ctx, const float *line, int nx, int ny, const
  * PAPER.md:371).  Call after rc_set_atmosphere. */
 int rc_set_boundary(rc_ctx *ctx, const float *I_below, const float *I_above);
 
+/* The same with one value per inclination (after rc_set_inclinations and rc_set_atmosphere): host,
+ * [ninclinations][nlambda] each, NULL = 0 - the "table of emergent intensity ... as a function of inclination
+ * and wavelength" of PAPER.md:374 in the plane-parallel reading G9 (e.g. a limb-darkened disc below). */
+int rc_set_boundary_inclined(rc_ctx *ctx, const float *I_below, const float *I_above);
+
 /* 2.5D inclination quadrature: the model is taken homogeneous along
  * the axis perpendicular to the grid, and every flatland ray is replaced by n rays with the same
  * projection and direction cosine mu[m] to that axis (0 <= mu < 1): the same cells, path lengths

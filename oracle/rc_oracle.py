@@ -148,8 +148,13 @@ def solve_inclined(chi, eta, ncascades, mu, w_mu, **kw):
     w_mu = np.asarray(w_mu, np.float64)
     assert mu.shape == w_mu.shape and mu.ndim == 1 and np.all(mu >= 0.0) and np.all(mu < 1.0)
     out = None
+    # boundary intensities may be given per inclination, [len(mu)][L] (a table over inclination
+    # and wavelength): inclination m then sees row m
+    Ib, Ia = kw.pop("I_below", None), kw.pop("I_above", None)
     for m in range(len(mu)):
-        o = solve(chi, eta, ncascades, path_scale=1.0 / np.sqrt(1.0 - mu[m] * mu[m]), **kw)
+        bm = None if Ib is None else (np.asarray(Ib)[m] if np.ndim(Ib) == 2 else Ib)
+        am = None if Ia is None else (np.asarray(Ia)[m] if np.ndim(Ia) == 2 else Ia)
+        o = solve(chi, eta, ncascades, path_scale=1.0 / np.sqrt(1.0 - mu[m] * mu[m]), I_below=bm, I_above=am, **kw)
         if out is None:
             out = {"J": w_mu[m] * o["J"], "Jbar": w_mu[m] * o["Jbar"]}
             for key in ("intervals", "segments"):
@@ -171,7 +176,9 @@ def solve_line(line, xl, ncascades, c0=1.0, I_below=None, I_above=None, weights=
         # summed with the quadrature weights, exactly as solve_inclined does for the GivenFs mode
         out = None
         for m in range(len(mu)):
-            o = solve_line(line, xl, ncascades, c0, I_below, I_above, weights, window, nthreads, order, want_counts,
+            bm = None if I_below is None else (np.asarray(I_below)[m] if np.ndim(I_below) == 2 else I_below)
+            am = None if I_above is None else (np.asarray(I_above)[m] if np.ndim(I_above) == 2 else I_above)
+            o = solve_line(line, xl, ncascades, c0, bm, am, weights, window, nthreads, order, want_counts,
                            path_scale=1.0 / np.sqrt(1.0 - float(mu[m]) ** 2), bilinear_fix=bilinear_fix)
             if out is None:
                 out = dict(o)

@@ -60,6 +60,7 @@ SYMBOLS = {
     "rc_set_atmosphere": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int]),
     "rc_set_line_atmosphere": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_int]),
     "rc_set_boundary": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
+    "rc_set_boundary_inclined": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
     "rc_set_lambda_weights": (C.c_int, [C.c_void_p, C.c_void_p]),
     "rc_set_inclinations": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]),
     "rc_solve_J": (C.c_int, [C.c_void_p, C.c_void_p]),
@@ -184,7 +185,15 @@ class RadianceCascades:
         self.shape = (ny, nx, int(x.size))
 
     def set_boundary(self, I_below=None, I_above=None):
+        """[nlambda] arrays, or [ninclinations][nlambda] (one value per inclined ray set)."""
         L = self.shape[2]
+        two_d = any(x is not None and np.ndim(x) == 2 for x in (I_below, I_above))
+        if two_d:
+            n = next(np.shape(x)[0] for x in (I_below, I_above) if x is not None and np.ndim(x) == 2)
+            a, pa = _host_f32(None if I_below is None else np.broadcast_to(I_below, (n, L)), n * L)
+            b, pb = _host_f32(None if I_above is None else np.broadcast_to(I_above, (n, L)), n * L)
+            self._check(self.lib.rc_set_boundary_inclined(self.handle, pa, pb))
+            return
         a, pa = _host_f32(I_below, L)
         b, pb = _host_f32(I_above, L)
         self._check(self.lib.rc_set_boundary(self.handle, pa, pb))

@@ -263,8 +263,8 @@ bool make_plan_uncached(const rc_config &cfg, int nm, bool line, int nx, int ny,
     P.A[0] = cur; cur += field * P.NM;  // merged cascades hold every (wavelength, inclination) channel
     P.A[1] = cur; cur += field * P.NM;
     if (cfg.flags & RC_ACCUM_J) { P.Jpart = cur; cur += align_up(ncell * P.nb * sizeof(float)); }
-    P.bc_below = cur; cur += align_up(P.Lpad * sizeof(float));
-    P.bc_above = cur; cur += align_up(P.Lpad * sizeof(float));
+    P.bc_below = cur; cur += align_up((size_t)P.Lpad * P.NM * sizeof(float));  // [Lpad][NM]: one value per channel
+    P.bc_above = cur; cur += align_up((size_t)P.Lpad * P.NM * sizeof(float));
     P.weights = cur;  cur += align_up(P.Lpad * sizeof(float));
     P.flag = cur;     cur += ALIGN;
     if (host_io) {
@@ -452,8 +452,8 @@ static int prepare_shape(rc_ctx *ctx, int nx, int ny, int nlambda, bool line) {
         }
         // defaults: free-space boundary, unit weights
         ctx->stage.assign((size_t)ctx->plan.Lpad, 0.f);
-        RC_CUDA(ctx, cudaMemsetAsync(ctx->ws + ctx->plan.bc_below, 0, ctx->plan.Lpad * sizeof(float), ctx->stream));
-        RC_CUDA(ctx, cudaMemsetAsync(ctx->ws + ctx->plan.bc_above, 0, ctx->plan.Lpad * sizeof(float), ctx->stream));
+        RC_CUDA(ctx, cudaMemsetAsync(ctx->ws + ctx->plan.bc_below, 0, (size_t)ctx->plan.Lpad * ctx->plan.NM * sizeof(float), ctx->stream));
+        RC_CUDA(ctx, cudaMemsetAsync(ctx->ws + ctx->plan.bc_above, 0, (size_t)ctx->plan.Lpad * ctx->plan.NM * sizeof(float), ctx->stream));
         std::vector<float> ones((size_t)ctx->plan.Lpad, 0.f);
         for (int l = 0; l < nlambda; l++) ones[l] = 1.f;
         RC_CUDA(ctx, cudaMemcpyAsync(ctx->ws + ctx->plan.weights, ones.data(), ones.size() * sizeof(float),
@@ -534,11 +534,35 @@ static int upload_lambda_array(rc_ctx *ctx, const float *src, size_t dst_off, fl
     return RC_OK;
 }
 
+// Boundary arrays on the device are [Lpad][NM] (channel order).  per_inclination: src is [NM][L], else [L].
+static int upload_boundary(rc_ctx *ctx, const float *src, size_t dst_off, bool per_inclination) {
+    if (!ctx->have_atm) return fail(ctx, RC_ERR_NO_ATMOSPHERE, "call rc_set_atmosphere first");
+    RC_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    const int NM = ctx->plan.NM, L = ctx->plan.L;
+    std::vector<float> h((size_t)ctx->plan.Lpad * NM, 0.f);
+    for (int l = 0; l < L && src; l++)
+        for (int m = 0; m < NM; m++) {
+            const float v = per_inclination ? src[(size_t)m * L + l] : src[l];
+            if (!(v >= 0.f) || !std::isfinite(v)) return fail(ctx, RC_ERR_BAD_VALUE, "boundary intensity must be finite and >= 0");
+            h[(size_t)l * NM + m] = v;
+        }
+    RC_CUDA(ctx, cudaMemcpyAsync(ctx->ws + dst_off, h.data(), h.size() * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
+    RC_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return RC_OK;
+}
+
 int rc_set_boundary(rc_ctx *ctx, const float *I_below, const float *I_above) {
     if (!ctx) return RC_ERR_NULL_ARG;
-    int rc = upload_lambda_array(ctx, I_below, ctx->plan.bc_below, 0.f);
+    int rc = upload_boundary(ctx, I_below, ctx->plan.bc_below, false);
     if (rc != RC_OK) return rc;
-    return upload_lambda_array(ctx, I_above, ctx->plan.bc_above, 0.f);
+    return upload_boundary(ctx, I_above, ctx->plan.bc_above, false);
+}
+
+int rc_set_boundary_inclined(rc_ctx *ctx, const float *I_below, const float *I_above) {
+    if (!ctx) return RC_ERR_NULL_ARG;
+    int rc = upload_boundary(ctx, I_below, ctx->plan.bc_below, true);
+    if (rc != RC_OK) return rc;
+    return upload_boundary(ctx, I_above, ctx->plan.bc_above, true);
 }
 
 // 2.5D: every flatland ray becomes n rays with the same projection and direction cosine mu[m] to the

@@ -41,8 +41,8 @@ struct MarchParams {
     const StepXY *xy;
     const long long *off;
     const int *cnt;
-    const float *I_below;  // [Lpad] device
-    const float *I_above;  // [Lpad] device
+    const float *I_below;  // [Lpad][NM] device (one value per channel)
+    const float *I_above;  // [Lpad][NM] device
     const float *weights;  // [Lpad] device
     int nx, ny, L, nb;
     int cascade, shift;    // s = 1 << shift

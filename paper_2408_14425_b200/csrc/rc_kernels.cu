@@ -15,6 +15,16 @@
 //                       One warp = a pw x ph patch of 32 probes x 1 direction group (4 child directions
 //                       in turn) x LV wavelengths per lane; geometry is warp-uniform (no divergence from
 //                       the DDA itself), radiance in fp32, I and T never leave registers.
+//                       Template switches: NM inclinations per wavelength (2.5D), PD = depth
+//                       of the register ring the gathers run ahead in, BANDED (grids larger than L2: one
+//                       band of rows/columns per launch, ray state parked in between), SPARSE (occupancy
+//                       bitmap in front of every gather), LINE (opacity evaluated per ray
+//                       from the projected velocity).  Run-time switch: the bilinear fix
+//                       (4 sub-rays per interval, 16 tables per direction).
+//   pack_line_kernel, alo_kernel, reduce_jbar_kernel, validate / mark_occupied / count_* kernels: small
+//                       elementwise or counting passes;  gather_probe_kernel, bulk_probe_kernel: the
+//                       march's gather pattern alone, through LDG.256 and through TMA bulk copies, for
+//                       the roofline (rc_probe_*_bandwidth).
 #include "rc_internal.h"
 
 #include <math_constants.h>
@@ -650,7 +660,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
             // (sin theta_k > 0  <=>  k < N/2) see I_above, rays heading down I_below
             const float *Ib = (2 * k < ndir) ? p.I_above : p.I_below;
 #pragma unroll
-            for (int v = 0; v < LV; v++) I[v] = fmaf(T[v], __ldg(Ib + nbI * LL + v / NM), I[v]);
+            for (int v = 0; v < LV; v++) I[v] = fmaf(T[v], __ldg(Ib + nbI * LV + v), I[v]);  // [wavelength][inclination]
         } else if (valid && p.fix) {
             // a3 with the bilinear fix: this sub-ray ends where parent `slot`'s child cone starts; merge it with that
             // parent alone (eq. 11), then weight it bilinearly.  At the lattice edge both slots of an axis are the

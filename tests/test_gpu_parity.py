@@ -404,3 +404,15 @@ def test_alo_matches_the_oracle(oracle):
         assert got.shape == want.shape
         # exp(-tau) in fp32: relative error ~ tau x 6e-8 (tau up to ~100 here); flushed values compare absolutely
         assert np.all(np.abs(got - want) <= 2e-5 * want + 1e-37), atm.name
+
+
+def test_boundary_per_inclination_matches_the_oracle(oracle):
+    """rc_set_boundary_inclined: a limb-darkened illumination from below, one value per inclination and wavelength."""
+    atm = A.with_inclinations(A.make_config(3, nx=64, ny=64, nlambda=5, ncascades=5), 8)
+    limb = 1.0 - 0.6 * atm.mu                                   # brighter for rays closer to the plane's normal... a table
+    atm.I_below = (limb[:, None] * np.linspace(0.5, 1.0, 5)[None, :]).astype(np.float32)
+    atm.I_above = np.zeros((8, 5), np.float32)
+    check(atm, oracle)
+    line = A.with_inclinations(A.line_config2(nx=64, ny=32, nlambda=3, ncascades=4), 4)
+    line.I_below = np.outer([1.0, 0.7, 0.5, 0.2], [0.3, 0.6, 0.9]).astype(np.float32)
+    check(line, oracle)

@@ -652,3 +652,20 @@ def test_A1_alo_is_the_own_cell_transmittance_of_cascade_0(oracle):
     a.line[..., 4:6] = 0
     c, _ = _static_fields(a.line, a.xl)
     assert np.allclose(oracle.alo(line=a.line, xl=a.xl), np.exp(-c * np.sqrt(0.5)), rtol=1e-12)
+
+
+def test_I4_boundary_per_inclination(oracle):
+    """A boundary intensity table over inclination: in an empty domain every constructed ray returns
+    its own boundary value, so J_l = sum_m w_m (I_below[m][l] + I_above[m][l]) / 2; a table with equal rows is the
+    plain per-wavelength boundary."""
+    mu, w = A.gauss_radau(4)
+    z = np.zeros((16, 16, 2), np.float32)
+    Ib = np.array([[1.0, 0.5], [0.8, 0.4], [0.6, 0.3], [0.2, 0.1]])
+    Ia = 0.25 * Ib[::-1]
+    J = oracle.solve_inclined(z, z, 3, mu, w, I_below=Ib, I_above=Ia)["J"]
+    want = (w[:, None] * (Ib + Ia) / 2).sum(0)
+    assert np.allclose(J, want[None, None, :], rtol=1e-14)
+    a = A.make_config(0, nx=16, ny=16, nlambda=2, ncascades=3)
+    J1 = oracle.solve_inclined(a.chi, a.eta, 3, mu, w, I_below=[0.7, 0.2])["J"]
+    J2 = oracle.solve_inclined(a.chi, a.eta, 3, mu, w, I_below=np.tile([0.7, 0.2], (4, 1)))["J"]
+    assert np.array_equal(J1, J2)
