@@ -56,6 +56,7 @@ struct MarchParams {
     int fix;               // bilinear fix: 4 sub-rays per ray, lanes = probes of one parity class,
                            // packed layout of spacing 2s, tables indexed (k*16 + class*4 + slot)
     const float2 *subdir;  // fix: unit direction of each sub-ray (line mode)
+    int cpw;               // child-per-warp: the 4 child directions of a group in 4 neighbouring warps (8 warps per block)
     int kg_n, kg_off;      // the launch covers direction groups (kg_off + 0 .. kg_n-1) mod ngroups
     // banded launch (state != null): only the steps inside [band_lo, band_hi) along band_axis
     // (0 = rows, 1 = columns), for rays travelling in direction band_sign along that axis
