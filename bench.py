@@ -32,8 +32,8 @@ METRIC = "probe-ray-wavelength segments/sec"
 UNIT = "seg-lambda/s"
 SM_COUNT, MUFU_PER_CLK_SM = 148, 16  # one ex2 per segment-wavelength; DESIGN.md §7
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant launch (march_kernel, cascade 5), from the committed
-# ncu --set full captures (profiles/ncu_r1b_march.md, ncu_r1c_modes.md), keyed by (mode, config, cascade)
-NCU_TRAFFIC_BYTES = {("flat", 2, 5): 9.20e9, ("incl8", 2, 5): 7.88e9, ("line", 2, 5): 1.03e9, ("flat", 4, 5): 8.83e9}
+# ncu --set full captures (profiles/bench_r1d.md, ncu_r1c_modes.md), keyed by (mode, config, cascade)
+NCU_TRAFFIC_BYTES = {("flat", 2, 5): 2.21e9, ("incl8", 2, 5): 7.88e9, ("line", 2, 5): 1.03e9, ("flat", 4, 5): 8.83e9}
 
 
 def peaks():
@@ -286,11 +286,11 @@ def main():
             "hbm_effective_frac": (8 * segl_per_step + 2 * casc_bytes * atm.ncascades) / (ms_step * 1e-3) / 1e9 / hbm_peak,
             "roofline": {"bound": "hbm", "kernel": f"march_kernel<{st.lambda_batch}> cascade {dom}", "achieved": ach,
                          "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak, "traffic": NCU_TRAFFIC_BYTES.get((mode, args.config, dom)),
-                         "traffic_unit": "bytes per launch (ncu --set full; profiles/ncu_r1b_march.md, ncu_r1c_modes.md)",
+                         "traffic_unit": "bytes per launch (ncu --set full; profiles/bench_r1d.md, ncu_r1c_modes.md)",
                          "algorithmic_bytes": alg_bytes,
                          "peak_source": peak_src, "ms_per_launch": ms_march[dom],
                          "note": "effective: algorithmic gather bytes (8 B per segment-wavelength) are mostly served "
-                                 "from L1/L2, so frac may exceed 1; see roofline_alu for the binding on-chip ceiling"},
+                                 "from L2 (and ~20 % from L1), so frac exceeds 1; roofline_l2 and roofline_alu give the on-chip ceilings"},
             "roofline_l2": {"bound": "l2", "achieved": ach, "peak": l2_gather_gbs, "unit": "GB/s", "frac": ach / l2_gather_gbs,
                             "peak_source": "rc_probe_gather_bandwidth(64 MB), measured in this run: random 1 KB warp-wide runs "
                                            "(LDG.256), 48 warps/SM, region L2-resident",
