@@ -66,7 +66,7 @@ struct rc_ctx {
     bool sparse = false;  // most cells have chi == 0 at every wavelength (counted by rc_set_atmosphere): skip their gathers
     // developer overrides (environment, read by rc_create): RC_MARCH_VARIANT = 0..3 (register ring depth /
     // occupancy of march_kernel), RC_PATCH_LOG2 = 2..5 forces the lane patch width for cascades >= RC_PATCH_FROM
-    int tune_variant = 2, tune_patch = -1, tune_patch_from = 0;
+    int tune_variant = -1, tune_patch = -1, tune_patch_from = 0;  // variant -1: chosen per cascade (march_variant)
     int tune_cpw = 3;        // RC_CPW_FROM: cascades >= this run one child direction per warp (-1: off)
     float tau_cut = 126.f;  // early-exit threshold on tau log2(e); 126: the fp32 transmittance is exactly 0
     // 2.5D inclination quadrature (rc_set_inclinations); nm = 1, f = w = 1: flatland
@@ -353,7 +353,7 @@ int rc_create(rc_ctx **out, const rc_config *cfg) {
     rc_ctx *ctx = new (std::nothrow) rc_ctx();
     if (!ctx) return RC_ERR_CUDA;
     ctx->cfg = *cfg;
-    if (const char *e = std::getenv("RC_MARCH_VARIANT")) ctx->tune_variant = std::max(0, std::min(3, std::atoi(e)));
+    if (const char *e = std::getenv("RC_MARCH_VARIANT")) ctx->tune_variant = std::max(0, std::min(4, std::atoi(e)));
     if (const char *e = std::getenv("RC_PATCH_LOG2")) ctx->tune_patch = std::max(2, std::min(5, std::atoi(e)));
     if (const char *e = std::getenv("RC_PATCH_FROM")) ctx->tune_patch_from = std::atoi(e);
     if (const char *e = std::getenv("RC_CPW_FROM")) ctx->tune_cpw = std::atoi(e);
@@ -591,6 +591,10 @@ int rc_set_lambda_weights(rc_ctx *ctx, const float *w) {
     return upload_lambda_array(ctx, w, ctx->plan.weights, 1.f);
 }
 
+// Register-ring depth / occupancy variant of cascade i's march launch (rc_kernels.cu, launch_march_flat): measured
+// on config 2, short rays (cascades <= 3) like 20 warps/SM with a ring of 2, long rays 16 warps/SM with a ring of 3.
+static int march_variant(const rc_ctx *ctx, int i) { return ctx->tune_variant >= 0 ? ctx->tune_variant : (i <= 3 ? 4 : 2); }
+
 // Parameters of cascade i's march launch.
 static rc::MarchParams march_params(const rc_ctx *ctx, int i, float *J_out) {
     const Plan &P = ctx->plan;
@@ -630,7 +634,7 @@ static rc::MarchParams march_params(const rc_ctx *ctx, int i, float *J_out) {
     mp.kg_n = mp.ngroups; mp.kg_off = 0;
     // child-per-warp where the march is bound by the L2 -> SM gathers (measured: config 2 77.0 -> 73.7 ms, config 3
     // 331 -> 315 ms, bilinear fix 341 -> 321 ms); not in the MUFU-bound modes (inclinations, moving line)
-    mp.cpw = J_out != nullptr && ctx->tune_cpw >= 0 && i >= ctx->tune_cpw && !c.empty && ctx->tune_variant != 1 &&
+    mp.cpw = J_out != nullptr && ctx->tune_cpw >= 0 && i >= ctx->tune_cpw && !c.empty &&
              P.NM == 1 && !ctx->line ? 1 : 0;
     for (int m = 0; m < 8; m++) { mp.incl_f[m] = ctx->incl_f[m]; mp.incl_w[m] = ctx->incl_w[m]; mp.incl_s[m] = 1.f / ctx->incl_f[m]; }
     mp.state = nullptr;
@@ -668,7 +672,7 @@ static int enqueue_solve(rc_ctx *ctx, float *J_out) {
         if (ev) RC_CUDA(ctx, cudaEventRecord(ev[1 + 2 * (top - i)], ctx->stream));
         rc::MarchParams mp = march_params(ctx, i, J_out);
         if (!c.banded) {
-            RC_CUDA(ctx, rc::launch_march(mp, P.LV * P.NM, P.NM, ctx->tune_variant, ctx->stream));
+            RC_CUDA(ctx, rc::launch_march(mp, P.LV * P.NM, P.NM, march_variant(ctx, i), ctx->stream));
             launches++;
         } else {
             // rays heading up (right) cross the bands in ascending order, the others in descending order;
@@ -686,7 +690,7 @@ static int enqueue_solve(rc_ctx *ctx, float *J_out) {
                     mp.band_lo = beta * ext;
                     mp.band_hi = std::min(n_axis, (beta + 1) * ext);
                     mp.band_final = bi == P.nbands - 1;
-                    RC_CUDA(ctx, rc::launch_march(mp, P.LV * P.NM, P.NM, ctx->tune_variant, ctx->stream));
+                    RC_CUDA(ctx, rc::launch_march(mp, P.LV * P.NM, P.NM, march_variant(ctx, i), ctx->stream));
                     launches++;
                 }
             }

@@ -774,8 +774,8 @@ static cudaError_t launch_march_variant(const MarchParams &p, cudaStream_t st) {
     return cudaGetLastError();
 }
 
-// variant: 0 = ring of 2 steps, 24 warps/SM (<= 80 registers); 1 = ring of 3, 20 warps/SM (<= 96);
-//          2 = ring of 3, 16 warps/SM (<= 128); 3 = ring of 4, 16 warps/SM (<= 128)
+// variant: 0 = ring of 2 steps, 24 warps/SM (<= 80 registers); 1 = ring of 3, 20 warps/SM (<= 96, blocks of 4 warps);
+//          2 = ring of 3, 16 warps/SM (<= 128); 3 = ring of 4, 16 warps/SM (<= 128); 4 = ring of 2, 20 warps/SM (<= 96)
 // Mostly-empty atmospheres (occ != null): the occupancy test in front of every gather.  Ring of 2, 24 warps/SM
 // (the dependent chain occupancy word -> predicate -> gather wants warps more than depth); variant 3: ring of 3, 16 warps/SM.
 template <int LV, int PD, int MINB>
@@ -811,8 +811,9 @@ static cudaError_t launch_march_flat(const MarchParams &p, int variant, cudaStre
     if (p.occ != nullptr) return launch_march_sparse<LV>(p, variant, st);
     switch (variant) {
         case 0: return launch_march_variant<LV, 1, 2, 8, 3>(p, st);
-        case 1: return launch_march_variant<LV, 1, 3, 5, 4>(p, st);
+        case 1: return launch_march_variant<LV, 1, 3, 4, 5>(p, st);
         case 3: return launch_march_variant<LV, 1, 4, 8, 2>(p, st);
+        case 4: return launch_march_variant<LV, 1, 2, 4, 5>(p, st);
         default: return launch_march_variant<LV, 1, 3, 8, 2>(p, st);
     }
 }

@@ -189,7 +189,7 @@ def test_segment_counts_match_the_oracle(oracle):
 
 
 # ------------------------------------------------------------------ launch variants
-@pytest.mark.parametrize("variant", [0, 1, 2, 3])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4])
 @pytest.mark.parametrize("patch", [None, 2, 3, 4, 5])
 def test_patch_shapes_and_ring_depths_are_bit_identical(oracle, monkeypatch, variant, patch):
     """The lane patch (32x1 .. 4x8 probes per warp) and the register-ring depth / occupancy variant of
