@@ -416,3 +416,12 @@ def test_boundary_per_inclination_matches_the_oracle(oracle):
     line = A.with_inclinations(A.line_config2(nx=64, ny=32, nlambda=3, ncascades=4), 4)
     line.I_below = np.outer([1.0, 0.7, 0.5, 0.2], [0.3, 0.6, 0.9]).astype(np.float32)
     check(line, oracle)
+
+
+def test_moving_line_jbar_accumulation(oracle):
+    """RC_ACCUM_J in the line mode: Jbar = sum_l w_l J_l with profile weights, against the oracle."""
+    import dataclasses
+    atm = A.line_config2(nx=64, ny=64, nlambda=13, ncascades=5)
+    w = np.exp(-atm.xl ** 2)
+    atm = dataclasses.replace(atm, accumulate=True, weights=(w / w.sum()).astype(np.float32))
+    check(atm, oracle)
