@@ -57,3 +57,27 @@ def test_two_rank_gloo_matches_single_rank(oracle):
     ref = oracle.solve_atmosphere(atm)
     assert np.array_equal(J, ref["J"])
     assert np.allclose(Jbar, ref["Jbar"], rtol=1e-14, atol=0)
+
+
+def test_bench_reference_arm_single_and_multi_rank():
+    """bench.py --impl reference: rank 0 alone times the oracle and prints ONE JSON line with the contract's keys;
+    under a multi-rank launch the other ranks exit 0 without work or output."""
+    import json
+    import os
+    import subprocess
+    import sys
+    from pathlib import Path
+    root = Path(__file__).resolve().parent.parent
+    cmd = [sys.executable, str(root / "bench.py"), "--impl", "reference", "--config", "0", "--steps", "2", "--warmup", "1"]
+    env = dict(os.environ, RANK="0", WORLD_SIZE="2", LOCAL_RANK="0")
+    out = subprocess.run(cmd + ["--gpus", "2"], capture_output=True, text=True, env=env, timeout=300)
+    assert out.returncode == 0, out.stderr
+    lines = [ln for ln in out.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["unit"] == "seg-lambda/s" and d["value"] > 0 and d["n_gpus"] == 2
+    assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["cores"] >= 1 and d["cpu_baseline"]["value"] == d["value"]
+    assert d["e2e"] == {"value": d["value"], "unit": d["unit"], "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
+    env["RANK"] = "1"
+    out = subprocess.run(cmd + ["--gpus", "2"], capture_output=True, text=True, env=env, timeout=300)
+    assert out.returncode == 0 and out.stdout.strip() == ""
