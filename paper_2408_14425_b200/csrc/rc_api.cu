@@ -634,7 +634,10 @@ static rc::MarchParams march_params(const rc_ctx *ctx, int i, float *J_out) {
     mp.kg_n = mp.ngroups; mp.kg_off = 0;
     // child-per-warp where the march is bound by the L2 -> SM gathers (measured: config 2 77.0 -> 73.7 ms, config 3
     // 331 -> 315 ms, bilinear fix 341 -> 321 ms); not in the MUFU-bound modes (inclinations, moving line)
-    mp.cpw = J_out != nullptr && ctx->tune_cpw >= 0 && i >= ctx->tune_cpw && !c.empty &&
+    // ... nor on a cascade that barely reaches into the box (config 2, cascade 6: 0.014 % of its rays are live)
+    const double diag = std::sqrt((double)P.nx * P.nx + (double)P.ny * P.ny);
+    const bool reaches = std::fmin(c.tb, diag) - c.ta > 0.2 * c.ta || i == 0;
+    mp.cpw = J_out != nullptr && ctx->tune_cpw >= 0 && i >= ctx->tune_cpw && !c.empty && (reaches || std::getenv("RC_CPW_FROM")) &&
              P.NM == 1 && !ctx->line ? 1 : 0;
     for (int m = 0; m < 8; m++) { mp.incl_f[m] = ctx->incl_f[m]; mp.incl_w[m] = ctx->incl_w[m]; mp.incl_s[m] = 1.f / ctx->incl_f[m]; }
     mp.state = nullptr;
