@@ -91,6 +91,8 @@ typedef struct {
     int64_t table_steps[RC_MAX_CASCADES]; /* step-table entries per cascade (all directions) */
     size_t workspace_bytes;
     int64_t empty_cells;                  /* cells with chi == 0 at every wavelength (counted by rc_set_atmosphere) */
+    int thin_batches;                     /* wavelength batches marched with the thin-accurate update: they hold a wavelength
+                                             whose optical depth across the whole box is < 1 with no boundary intensity */
 } rc_stats;
 
 /* The launch plan the library would use for a problem, computed on the host alone (no device, no context):

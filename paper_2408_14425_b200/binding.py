@@ -30,7 +30,7 @@ class rc_stats(C.Structure):
                 ("solves_timed", C.c_int), ("ms_pack", C.c_float * RC_MAX_CASCADES),
                 ("ms_march", C.c_float * RC_MAX_CASCADES), ("ms_total", C.c_float),
                 ("rays", C.c_int64 * RC_MAX_CASCADES), ("table_steps", C.c_int64 * RC_MAX_CASCADES),
-                ("workspace_bytes", C.c_size_t), ("empty_cells", C.c_int64)]
+                ("workspace_bytes", C.c_size_t), ("empty_cells", C.c_int64), ("thin_batches", C.c_int)]
 
 
 class rc_plan_info(C.Structure):

@@ -352,6 +352,20 @@ __device__ __forceinline__ void store_vec_cs(float *p, const float (&v)[LV]) {
     }
 }
 
+// eq. 16 for one cell and one channel.  x = optical depth of the segment in units of ln 2.  Normal form: the
+// emission is S (T_(n-1) - T_n) with T_n = 2^-tau_n from the accumulated tau (absolute error ~1e-7 S).
+// Thin form: for x < 1/32 the same quantity as S T_(n-1) (1 - 2^-x) with 1 - 2^-x = y - y^2/2 + y^3/6, y = x ln 2
+// (relative error < 4e-7), so that emission far below the resolution of T survives.
+__device__ __forceinline__ void thin_update(float chi2, float Sv, float dsv, float &tau, float &T, float &I) {
+    const float x = chi2 * dsv;
+    tau += x;
+    const float Tn = ex2_neg(tau);
+    const float y = x * 0.6931471805599453f;
+    const float w = y * fmaf(y, fmaf(y, 0.16666667f, -0.5f), 1.f);
+    I = fmaf(Sv, x < 0.03125f ? T * w : T - Tn, I);
+    T = Tn;
+}
+
 // Position of child probe a among the n parents per axis: a/2 - 1/4 in parent index units, clamped
 // at the lattice edge.  Weight `f` goes to q1.
 __device__ __forceinline__ void parent_axis(int a, int n, int &q0, int &q1, float &f) {
@@ -453,7 +467,7 @@ __device__ __forceinline__ int first_step_reaching(const StepXY *xy, int n, int 
 // half of the directions that crosses the bands in ascending (or descending) order; a ray's (I, tau)
 // is carried from band to band through `state`, so the arithmetic - and the result - is that of the
 // unbanded launch, bit for bit, while the cells gathered by one launch fit L2.
-template <int LV, int NM, int PD, int WARPS, int MINB, bool BANDED, bool SPARSE, bool LINE>
+template <int LV, int NM, int PD, int WARPS, int MINB, bool BANDED, bool SPARSE, bool LINE, bool THIN = false>
 __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) {
     // sum over the 4 child directions, per thread: parked in shared memory between children so the
     // marching loop has the registers to itself
@@ -483,6 +497,9 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
         for (int v = 0; v < LL; v++) xs[v] = __ldg(p.xls + nbI * LL + v);
     }
     const unsigned *occB = SPARSE ? p.occ + (long long)nbI * (ncell >> 5) : nullptr;
+    // THIN: the solve holds an optically thin wavelength (flagged by the host): T = 2^-tau stays within a
+    // few ulp of 1 along whole rays and the differences T_(n-1) - T_n lose the emission; thin_update() keeps it.
+    // A compile-time switch: as a run-time branch it cost the normal path 20 % (registers, scheduling).
     // (dx, dy) ranges that keep this lane's ray inside the box
     const int dxlo = -(a << p.shift) - half, dxhi = ((p.npx - a) << p.shift) - 1 - half;
     const int dylo = -Y0, dyhi = p.ny - 1 - Y0;
@@ -622,11 +639,18 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
                             const float chi2 = fmaf(c2[u][2], phi, c2[u][0]);
                             const float num = fmaf(c2[u][3], phi, c2[u][1]);
                             const float Sv = chi2 > 0.f ? __fdividef(num, chi2) : 0.f;  // eta/chi; vacuum emits nothing
-                            tau[v] = fmaf(chi2, dsm[v % NM], tau[v]);
-                            const float Tn = ex2_neg(tau[v]);
-                            I[v] = fmaf(Sv, T[v] - Tn, I[v]);
-                            T[v] = Tn;
+                            if constexpr (THIN) {
+                                thin_update(chi2, Sv, dsm[v % NM], tau[v], T[v], I[v]);
+                            } else {
+                                tau[v] = fmaf(chi2, dsm[v % NM], tau[v]);
+                                const float Tn = ex2_neg(tau[v]);
+                                I[v] = fmaf(Sv, T[v] - Tn, I[v]);
+                                T[v] = Tn;
+                            }
                         }
+                    } else if constexpr (THIN) {
+#pragma unroll
+                        for (int v = 0; v < LV; v++) thin_update(c2[u][v / NM], S[u][v / NM], dsm[v % NM], tau[v], T[v], I[v]);
                     } else if (!SPARSE || __any_sync(FULL, ds[u] != 0.f)) {  // SPARSE: no lane has an occupied cell: nothing to do
 #pragma unroll
                         for (int v = 0; v < LV; v++) {
@@ -818,9 +842,39 @@ static cudaError_t launch_march_flat(const MarchParams &p, int variant, cudaStre
     }
 }
 
+// Solves that hold an optically thin wavelength (p.thin != null): every mode in one plain variant (ring of 2, 16
+// warps/SM, never banded or sparse) with the thin-accurate update.
+template <int LV, int NM, bool LINE>
+static cudaError_t launch_march_thin(const MarchParams &p, cudaStream_t st) {
+    constexpr int WARPS = 8;
+    const long long blocks = (march_warps(p) + WARPS - 1) / WARPS;
+    if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+    march_kernel<LV, NM, 2, WARPS, 2, false, false, LINE, true><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
+    return cudaGetLastError();
+}
+
+template <bool LINE>
+static cudaError_t launch_march_thin_any(const MarchParams &p, int LV, int NM, cudaStream_t st) {
+    switch (LV * 16 + NM) {
+        case 8 * 16 + 8: return launch_march_thin<8, 8, LINE>(p, st);
+        case 8 * 16 + 4: return launch_march_thin<8, 4, LINE>(p, st);
+        case 8 * 16 + 2: return launch_march_thin<8, 2, LINE>(p, st);
+        case 8 * 16 + 1: return launch_march_thin<8, 1, LINE>(p, st);
+        case 4 * 16 + 4: return launch_march_thin<4, 4, LINE>(p, st);
+        case 4 * 16 + 2: return launch_march_thin<4, 2, LINE>(p, st);
+        case 4 * 16 + 1: return launch_march_thin<4, 1, LINE>(p, st);
+        case 2 * 16 + 2: return launch_march_thin<2, 2, LINE>(p, st);
+        case 2 * 16 + 1: return launch_march_thin<2, 1, LINE>(p, st);
+        case 1 * 16 + 1: return launch_march_thin<1, 1, LINE>(p, st);
+        default: return cudaErrorInvalidValue;
+    }
+}
+
 // LV = channels per lane = (wavelengths per lane) x NM inclinations; the inclined launches come in one
 // variant only
 cudaError_t launch_march(const MarchParams &p, int LV, int NM, int variant, cudaStream_t st) {
+    if (p.thin != nullptr)
+        return p.linepk != nullptr ? launch_march_thin_any<true>(p, LV, NM, st) : launch_march_thin_any<false>(p, LV, NM, st);
     if (NM == 1) {
         switch (LV) {
             case 8: return launch_march_flat<8>(p, variant, st);
@@ -883,17 +937,59 @@ __global__ void validate_kernel(const float *chi, const float *eta, long long n,
 // Number of cells with chi == 0 at every wavelength (rc_set_atmosphere: is the atmosphere mostly empty?).
 // Pass 1 marks the cells that have a non-zero value (coalesced over the whole array), pass 2 counts the rest.
 template <int W>  // floats per thread: 4 when nlambda is a multiple of 4, else 1
-__global__ void mark_occupied_kernel(const float *chi, long long nchunk, int chunks_per_cell, int *mark) {
+__global__ void mark_occupied_kernel(const float *chi, long long nchunk, int chunks_per_cell, int *mark, int *maxchi, int L) {
+    // also the largest chi of every wavelength (non-negative floats order like their bit patterns): block-wide in
+    // shared memory, then one global atomicMax per wavelength and block
+    extern __shared__ int mx[];
+    for (int l = threadIdx.x; l < L; l += blockDim.x) mx[l] = 0;
+    __syncthreads();
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < nchunk; i += (long long)gridDim.x * blockDim.x) {
         bool nz;
+        const int c = (int)(i % chunks_per_cell);
         if constexpr (W == 4) {
             const float4 v = __ldg(reinterpret_cast<const float4 *>(chi) + i);
             nz = v.x != 0.f || v.y != 0.f || v.z != 0.f || v.w != 0.f;
+            if (maxchi && nz) {
+                atomicMax(mx + 4 * c, __float_as_int(v.x)); atomicMax(mx + 4 * c + 1, __float_as_int(v.y));
+                atomicMax(mx + 4 * c + 2, __float_as_int(v.z)); atomicMax(mx + 4 * c + 3, __float_as_int(v.w));
+            }
         } else {
-            nz = __ldg(chi + i) != 0.f;
+            const float v = __ldg(chi + i);
+            nz = v != 0.f;
+            if (maxchi && nz) atomicMax(mx + c, __float_as_int(v));
         }
         if (nz) mark[i / chunks_per_cell] = 1;
     }
+    __syncthreads();
+    if (maxchi)
+        for (int l = threadIdx.x; l < L; l += blockDim.x)
+            if (mx[l] != 0) atomicMax(maxchi + l, mx[l]);
+}
+
+// Line mode: upper bound over directions of the opacity of every wavelength, chi_c + chi_line phi(max(0, |x_l| - |v|)).
+__global__ void line_maxchi_kernel(const float *line, const float *xl, long long ncell, int L, int *maxchi) {
+    extern __shared__ int mx[];
+    for (int l = threadIdx.x; l < L; l += blockDim.x) mx[l] = 0;
+    __syncthreads();
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < ncell * L; i += (long long)gridDim.x * blockDim.x) {
+        const long long cell = i / L;
+        const int l = (int)(i - cell * L);
+        const float *q = line + cell * 6;
+        const float v = sqrtf(q[4] * q[4] + q[5] * q[5]);
+        const float a = fmaxf(fabsf(__ldg(xl + l)) - v, 0.f);
+        const float c = fmaf(q[2], expf(-a * a) * 0.5641895835477563f, q[0]);
+        if (c > 0.f) atomicMax(mx + l, __float_as_int(c));
+    }
+    __syncthreads();
+    for (int l = threadIdx.x; l < L; l += blockDim.x)
+        if (mx[l] != 0) atomicMax(maxchi + l, mx[l]);
+}
+
+cudaError_t launch_line_maxchi(const float *line, const float *xl, long long ncell, int L, int *maxchi, cudaStream_t st) {
+    cudaError_t e = cudaMemsetAsync(maxchi, 0, sizeof(int) * (size_t)L, st);
+    if (e != cudaSuccess) return e;
+    line_maxchi_kernel<<<148 * 8, 256, sizeof(int) * (size_t)L, st>>>(line, xl, ncell, L, maxchi);
+    return cudaGetLastError();
 }
 
 __global__ void count_unmarked_kernel(const int *mark, long long ncell, unsigned long long *count) {
@@ -904,14 +1000,19 @@ __global__ void count_unmarked_kernel(const int *mark, long long ncell, unsigned
     if ((threadIdx.x & 31) == 0 && mine) atomicAdd(count, mine);
 }
 
-// mark: scratch of ncell ints (device); count: zeroed by the caller
-cudaError_t launch_count_empty(const float *chi, long long ncell, int L, int *mark, unsigned long long *count, cudaStream_t st) {
+// mark: scratch of ncell ints (device); count: zeroed by the caller; maxchi: null or [L] ints (float bit patterns)
+cudaError_t launch_count_empty(const float *chi, long long ncell, int L, int *mark, unsigned long long *count, int *maxchi, cudaStream_t st) {
     cudaError_t e = cudaMemsetAsync(mark, 0, sizeof(int) * (size_t)ncell, st);
     if (e != cudaSuccess) return e;
+    if (maxchi) {
+        e = cudaMemsetAsync(maxchi, 0, sizeof(int) * (size_t)L, st);
+        if (e != cudaSuccess) return e;
+    }
+    const size_t sm = sizeof(int) * (size_t)L;
     if (L % 4 == 0 && (reinterpret_cast<uintptr_t>(chi) & 15) == 0)
-        mark_occupied_kernel<4><<<148 * 16, 256, 0, st>>>(chi, ncell * (L / 4), L / 4, mark);
+        mark_occupied_kernel<4><<<148 * 16, 256, sm, st>>>(chi, ncell * (L / 4), L / 4, mark, maxchi, L);
     else
-        mark_occupied_kernel<1><<<148 * 16, 256, 0, st>>>(chi, ncell * L, L, mark);
+        mark_occupied_kernel<1><<<148 * 16, 256, sm, st>>>(chi, ncell * L, L, mark, maxchi, L);
     count_unmarked_kernel<<<148 * 4, 256, 0, st>>>(mark, ncell, count);
     return cudaGetLastError();
 }

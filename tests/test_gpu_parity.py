@@ -425,3 +425,33 @@ def test_moving_line_jbar_accumulation(oracle):
     w = np.exp(-atm.xl ** 2)
     atm = dataclasses.replace(atm, accumulate=True, weights=(w / w.sum()).astype(np.float32))
     check(atm, oracle)
+
+
+# ------------------------------------------------------------------ optically thin wavelengths
+def test_optically_thin_planes_keep_their_emission(oracle):
+    """A wavelength whose optical depth across the whole box is tiny and that has no boundary illumination has
+    J ~ S tau: far below the ~1e-7 S resolution of the transmittance differences of the normal fp32 update (found by
+    a randomised sweep: config 4's recipe at two far-wing wavelengths, J ~ 1e-9).  rc_set_atmosphere flags such
+    batches from the largest opacity of each wavelength and they take the thin-accurate update; the bar holds."""
+    from paper_2408_14425_b200 import binding
+    atm = A.make_config(4, nx=128, ny=16, nlambda=2, ncascades=1)     # x_l = -5, +5 only; chi ~ 1e-10
+    J, rc = binding.solve_atmosphere(atm)
+    assert rc.get_stats().thin_batches == 1
+    rc.close()
+    check(atm, oracle)
+    base = A.make_config(0, nx=64, ny=64, nlambda=3, ncascades=5)
+    import dataclasses
+    for scale in (1e-9, 1e-6, 1e-4):                                    # the same atmosphere, ever thinner
+        thin = dataclasses.replace(base, chi=(base.chi * scale).astype(np.float32), eta=(base.eta * scale).astype(np.float32))
+        check(thin, oracle)
+        check(A.with_inclinations(thin, 4), oracle)
+    line = A.line_config2(nx=64, ny=64, nlambda=4, ncascades=5)
+    line.line[..., 0] *= 1e-6
+    line.line[..., 2] *= 1e-7
+    check(line, oracle)
+    # the standard recipes are not flagged (no cost for them), and a lit thin plane is not either
+    for idx, kw in ((1, dict(nx=128, ny=128, nlambda=16, ncascades=6)), (2, dict(nx=128, ny=128, nlambda=64, ncascades=6)),
+                    (3, dict(nx=256, ny=256, nlambda=8, ncascades=7))):
+        J, rc = binding.solve_atmosphere(A.make_config(idx, **kw))
+        assert rc.get_stats().thin_batches == 0, idx
+        rc.close()
