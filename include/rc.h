@@ -69,6 +69,12 @@ extern "C" {
                              each of the four parent probes, merged with that parent alone and then weighted
                              bilinearly: removes most of the ringing around bright compact sources at 4x the rays */
 
+#define RC_ACCURATE_THIN 16 /* always march with the thin-accurate update (every segment's emission to ~3e-6 relative,
+                               at ~2x the arithmetic).  Default: only solves that hold a wavelength which is optically
+                               thin across the whole box and unlit take it (rc_stats.thin_batches); elsewhere the
+                               emission of a ray is exact to ~1e-7 S, which matters only for cells that no ray with
+                               optical depth >~ 1e-3 reaches while J elsewhere on that plane is of order S */
+
 typedef struct rc_ctx rc_ctx; /* opaque, owned by the library */
 
 typedef struct {
@@ -76,7 +82,7 @@ typedef struct {
     float c0_interval; /* length of the cascade-0 interval in cells; > 0; the configs use 1 */
     int device;        /* CUDA ordinal */
     int lambda_batch;  /* wavelengths per thread (1, 2, 4 or 8); 0 = library chooses */
-    int flags;         /* RC_ACCUM_J | RC_VALIDATE | RC_NO_EARLY_EXIT | RC_BILINEAR_FIX */
+    int flags;         /* RC_ACCUM_J | RC_VALIDATE | RC_NO_EARLY_EXIT | RC_BILINEAR_FIX | RC_ACCURATE_THIN */
 } rc_config;
 
 typedef struct {

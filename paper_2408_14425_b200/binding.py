@@ -14,7 +14,7 @@ import numpy as np
 from . import build as _build
 
 RC_OK = 0
-RC_ACCUM_J, RC_VALIDATE, RC_NO_EARLY_EXIT, RC_BILINEAR_FIX = 1, 2, 4, 8
+RC_ACCUM_J, RC_VALIDATE, RC_NO_EARLY_EXIT, RC_BILINEAR_FIX, RC_ACCURATE_THIN = 1, 2, 4, 8, 16
 RC_MAX_CASCADES = 12
 ERRORS = {-1: "RC_ERR_NULL_ARG", -2: "RC_ERR_BAD_SHAPE", -3: "RC_ERR_NO_DEVICE", -4: "RC_ERR_NO_WORKSPACE",
           -5: "RC_ERR_BAD_VALUE", -6: "RC_ERR_CUDA", -7: "RC_ERR_NO_ATMOSPHERE"}

@@ -427,10 +427,10 @@ static int update_thin_flags(rc_ctx *ctx) {
     const Plan &P = ctx->plan;
     std::vector<int> flags((size_t)P.nb, 0);
     const double diag = std::sqrt((double)P.nx * P.nx + (double)P.ny * P.ny);
-    const bool force = std::getenv("RC_FORCE_THIN") != nullptr, off = std::getenv("RC_NO_THIN") != nullptr;
+    const bool force = std::getenv("RC_FORCE_THIN") != nullptr || (ctx->cfg.flags & RC_ACCURATE_THIN) != 0, off = std::getenv("RC_NO_THIN") != nullptr;
     int n = 0;
-    for (int l = 0; l < P.L && (int)ctx->maxchi_h.size() == P.L; l++) {
-        const bool thin = ctx->maxchi_h[l] > 0.f && (double)ctx->maxchi_h[l] * diag < 1.0 && !(l < (int)ctx->lit_h.size() && ctx->lit_h[l]);
+    for (int l = 0; l < P.L; l++) {
+        const bool thin = (int)ctx->maxchi_h.size() == P.L && ctx->maxchi_h[l] > 0.f && (double)ctx->maxchi_h[l] * diag < 1.0 && !(l < (int)ctx->lit_h.size() && ctx->lit_h[l]);
         if ((thin || force) && !off) flags[l / P.LV] = 1;
     }
     for (int b = 0; b < P.nb; b++) n += flags[b];

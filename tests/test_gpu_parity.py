@@ -455,3 +455,14 @@ def test_optically_thin_planes_keep_their_emission(oracle):
         J, rc = binding.solve_atmosphere(A.make_config(idx, **kw))
         assert rc.get_stats().thin_batches == 0, idx
         rc.close()
+
+
+def test_accurate_thin_flag_for_mixed_thin_and_thick_planes(oracle):
+    """RC_ACCURATE_THIN.  On a plane with a few opaque blobs in exact vacuum and a single cascade (4 rays per cell) some
+    cells are reached only through the faint outskirts of a blob (ray optical depth ~1e-4) while J elsewhere is of order S:
+    the default update's ~1e-7 S resolution is then ~1e-3 of their J (a randomised sweep found 7e-4 here).  The flag marches
+    everything with the thin-accurate update and restores the bar; the five configurations do not need it."""
+    from paper_2408_14425_b200 import binding
+    atm = A.make_config(4, nx=101, ny=147, nlambda=1, ncascades=1, seed=431)
+    check(atm, oracle, flags=binding.RC_ACCURATE_THIN)
+    check(A.make_config(2, nx=64, ny=64, nlambda=5, ncascades=5), oracle, flags=binding.RC_ACCURATE_THIN)
