@@ -1,0 +1,68 @@
+"""GPU parity on a seeded random sweep over grid shapes, cascade counts, recipes, modes (inclinations, moving line,
+bilinear fix, Jbar) and launch knobs (bands, child-per-warp, forced sparse march, ring variants, lane patches).
+The sweep that found the optically thin limit; every case must meet the 2e-4 bar."""
+import dataclasses
+import os
+
+import numpy as np
+import pytest
+
+from paper_2408_14425_b200 import atmospheres as A
+
+pytestmark = pytest.mark.gpu
+KNOBS = ("RC_BANDS", "RC_CPW_FROM", "RC_FORCE_SPARSE", "RC_MARCH_VARIANT", "RC_PATCH_LOG2")
+
+
+def _cases(seed, n):
+    rng = np.random.default_rng(seed)
+    for it in range(n):
+        nc = int(rng.integers(1, 7))
+        m = 1 << (nc - 1)
+        nx = m * int(rng.integers(1, max(2, 160 // m)))
+        ny = m * int(rng.integers(1, max(2, 160 // m)))
+        L = int(rng.integers(1, 12))
+        kind = str(rng.choice(["cfg0", "cfg1", "cfg3", "cfg4", "line"]))
+        kw = dict(nx=nx, ny=ny, nlambda=L, ncascades=nc, seed=int(rng.integers(1, 10**6)))
+        nincl = int(rng.choice([1, 1, 2, 4, 8]))
+        fix = bool(rng.integers(0, 2)) and nc > 1
+        lit = bool(rng.integers(0, 2))
+        bc = (rng.uniform(0, 1, L).astype(np.float32), rng.uniform(0, 1, L).astype(np.float32))
+        env = {}
+        if rng.integers(0, 3) == 0: env["RC_BANDS"] = str(int(rng.integers(2, 5)))
+        if rng.integers(0, 3) == 0: env["RC_CPW_FROM"] = str(int(rng.integers(0, 3)))
+        if rng.integers(0, 4) == 0: env["RC_FORCE_SPARSE"] = "1"
+        if rng.integers(0, 3) == 0: env["RC_MARCH_VARIANT"] = str(int(rng.integers(0, 5)))
+        if rng.integers(0, 3) == 0: env["RC_PATCH_LOG2"] = str(int(rng.integers(2, 6)))
+        lb = int(rng.choice([0, 0, 1, 2, 4, 8]))
+        yield it, kind, kw, nincl, fix, lit, bc, env, (lb if lb * nincl <= 8 else 0)
+
+
+@pytest.mark.parametrize("seed,n", [(1, 40), (4, 30)])
+def test_random_sweep(oracle, monkeypatch, seed, n):
+    from paper_2408_14425_b200 import binding
+    worst = 0.0
+    for it, kind, kw, nincl, fix, lit, bc, env, lb in _cases(seed, n):
+        atm = A.line_config2(**kw) if kind == "line" else A.make_config(int(kind[3]), **kw)
+        if nincl > 1:
+            atm = A.with_inclinations(atm, nincl)
+        atm = dataclasses.replace(atm, bilinear_fix=fix)
+        if lit:
+            atm.I_below, atm.I_above = bc
+        for k in KNOBS:
+            monkeypatch.delenv(k, raising=False)
+        for k, v in env.items():
+            monkeypatch.setenv(k, v)
+        J, rc = binding.solve_atmosphere(atm, lambda_batch=lb)
+        Jg = J.cpu().numpy().astype(np.float64)
+        rc.close()
+        o = oracle.solve_atmosphere(atm)
+        Jo = o["Jbar"] if atm.accumulate else o["J"]
+        if Jo.ndim == 2:
+            Jo, Jg = Jo[..., None], Jg[..., None]
+        for l in range(Jo.shape[-1]):
+            mk = Jo[..., l] > 1e-6 * Jo[..., l].max()
+            if mk.any():
+                err = float(np.max(np.abs(Jg[..., l][mk] - Jo[..., l][mk]) / Jo[..., l][mk]))
+                assert err <= 2e-4, (it, kind, kw, nincl, fix, env, lb, err)
+                worst = max(worst, err)
+    print("sweep", seed, "worst rel err", worst)
