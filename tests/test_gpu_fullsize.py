@@ -26,9 +26,9 @@ def windows(atm, n, size, seed):
     return w[:n]
 
 
-def run(idx, nwin, size, oracle, full=False):
+def run(idx, nwin, size, oracle, full=False, atm=None):
     from paper_2408_14425_b200 import binding
-    atm = A.make_config(idx)
+    atm = A.make_config(idx) if atm is None else atm
     J, rc = binding.solve_atmosphere(atm)
     Jg = J.cpu().numpy().astype(np.float64)
     rc.close()
@@ -46,7 +46,7 @@ def run(idx, nwin, size, oracle, full=False):
             m = ol > 1e-6 * scale
             if m.any():
                 worst = max(worst, float(np.max(np.abs(gl[m] - ol[m]) / ol[m])))
-    print(f"cfg{idx} full size: max rel err over {nwin} windows of {size}x{size} cells = {worst:.3e}")
+    print(f"{atm.name} full size: max rel err over {nwin} windows of {size}x{size} cells = {worst:.3e}")
     assert worst <= TOL, worst
     if full:
         o = oracle.solve_atmosphere(atm)["J"]
@@ -70,3 +70,17 @@ def test_config3_sampled(oracle):
 
 def test_config4_sampled_jbar(oracle):
     run(4, 3, 2, oracle)
+
+
+# ------------------------------------------------------------------ the widened modes at size (512 x 512 x 16, 7 cascades)
+def test_config1_size_bilinear_fix(oracle):
+    import dataclasses
+    run(1, 3, 3, oracle, atm=dataclasses.replace(A.make_config(1), name="cfg1_fix", bilinear_fix=True))
+
+
+def test_config1_size_inclinations(oracle):
+    run(1, 3, 3, oracle, atm=A.with_inclinations(A.make_config(1), 8))
+
+
+def test_config1_size_moving_line_with_inclinations(oracle):
+    run(1, 3, 3, oracle, atm=A.with_inclinations(A.line_config2(nx=512, ny=512, nlambda=16, ncascades=7), 4))
