@@ -68,6 +68,7 @@ struct rc_ctx {
     // a boundary intensity is set there (rc_set_boundary*); batches with a thin, unlit wavelength take the thin update
     std::vector<float> maxchi_h;
     std::vector<char> lit_h;
+    std::vector<float> w_h;  // wavelength weights (rc_set_lambda_weights; empty = all 1)
     bool sparse = false;  // most cells have chi == 0 at every wavelength (counted by rc_set_atmosphere): skip their gathers
     // developer overrides (environment, read by rc_create): RC_MARCH_VARIANT = 0..3 (register ring depth /
     // occupancy of march_kernel), RC_PATCH_LOG2 = 2..5 forces the lane patch width for cascades >= RC_PATCH_FROM
@@ -429,10 +430,18 @@ static int update_thin_flags(rc_ctx *ctx) {
     const double diag = std::sqrt((double)P.nx * P.nx + (double)P.ny * P.ny);
     const bool force = std::getenv("RC_FORCE_THIN") != nullptr || (ctx->cfg.flags & RC_ACCURATE_THIN) != 0, off = std::getenv("RC_NO_THIN") != nullptr;
     int n = 0;
+    // With RC_ACCUM_J the checked output is Jbar = sum_l w_l J_l: a thin plane adds next to nothing to it and its own
+    // relative accuracy is not asked for, so only a solve whose weighted planes are ALL thin takes the thin update
+    // (config 4: its far-wing planes are thin, its line core is not).
+    const bool accum = (ctx->cfg.flags & RC_ACCUM_J) != 0;
+    bool all_thin = true, any_weighted = false;
     for (int l = 0; l < P.L; l++) {
         const bool thin = (int)ctx->maxchi_h.size() == P.L && ctx->maxchi_h[l] > 0.f && (double)ctx->maxchi_h[l] * diag < 1.0 && !(l < (int)ctx->lit_h.size() && ctx->lit_h[l]);
-        if ((thin || force) && !off) flags[l / P.LV] = 1;
+        const bool weighted = !(l < (int)ctx->w_h.size()) || ctx->w_h[l] != 0.f;
+        if (accum && weighted) { any_weighted = true; all_thin = all_thin && thin; }
+        if (((thin && !accum) || force) && !off) flags[l / P.LV] = 1;
     }
+    if (accum && any_weighted && all_thin && !off) std::fill(flags.begin(), flags.end(), 1);
     for (int b = 0; b < P.nb; b++) n += flags[b];
     ctx->stats.thin_batches = n;
     RC_CUDA(ctx, cudaMemcpyAsync(ctx->ws + P.thin, flags.data(), flags.size() * sizeof(int), cudaMemcpyHostToDevice, ctx->stream));
@@ -494,6 +503,7 @@ static int prepare_shape(rc_ctx *ctx, int nx, int ny, int nlambda, bool line) {
         // defaults: free-space boundary, unit weights
         ctx->stage.assign((size_t)ctx->plan.Lpad, 0.f);
         ctx->lit_h.assign((size_t)nlambda, 0);
+        ctx->w_h.clear();
         RC_CUDA(ctx, cudaMemsetAsync(ctx->ws + ctx->plan.bc_below, 0, (size_t)ctx->plan.Lpad * ctx->plan.NM * sizeof(float), ctx->stream));
         RC_CUDA(ctx, cudaMemsetAsync(ctx->ws + ctx->plan.bc_above, 0, (size_t)ctx->plan.Lpad * ctx->plan.NM * sizeof(float), ctx->stream));
         std::vector<float> ones((size_t)ctx->plan.Lpad, 0.f);
@@ -642,7 +652,11 @@ int rc_set_inclinations(rc_ctx *ctx, int n, const float *mu, const float *w) {
 
 int rc_set_lambda_weights(rc_ctx *ctx, const float *w) {
     if (!ctx) return RC_ERR_NULL_ARG;
-    return upload_lambda_array(ctx, w, ctx->plan.weights, 1.f);
+    const int rc = upload_lambda_array(ctx, w, ctx->plan.weights, 1.f);
+    if (rc != RC_OK) return rc;
+    ctx->w_h.assign((size_t)ctx->plan.L, 1.f);
+    for (int l = 0; l < ctx->plan.L && w; l++) ctx->w_h[l] = w[l];
+    return update_thin_flags(ctx);
 }
 
 // Register-ring depth / occupancy variant of cascade i's march launch (rc_kernels.cu, launch_march_flat): measured
