@@ -37,7 +37,7 @@ struct Plan {
     size_t state = 0;               // parked ray state of the banded launches
     bool line = false;              // velocity-dependent line mode: chiT holds 6 packed line parameters per cell
     size_t xls = 0;                 // line mode: scaled wavelengths [Lpad]
-    size_t maxchi = 0, thin = 0;    // per-wavelength largest opacity (float bits), per-batch "optically thin" flags
+    size_t maxchi = 0, sumchi = 0, thin = 0;  // per-wavelength largest opacity (float bits) and fixed-point sum; per-batch thin flags
     size_t occ = 0;                 // occupancy bitmap of the packed cells (0: none, nx ny not a multiple of 32)
     bool has_occ = false;
     CascadePlan c[RC_MAX_CASCADES];
@@ -67,6 +67,7 @@ struct rc_ctx {
     // optically thin wavelengths: largest opacity of every wavelength (rc_set_*atmosphere) and whether
     // a boundary intensity is set there (rc_set_boundary*); batches with a thin, unlit wavelength take the thin update
     std::vector<float> maxchi_h;
+    std::vector<double> meanchi_h;
     std::vector<char> lit_h;
     std::vector<float> w_h;  // wavelength weights (rc_set_lambda_weights; empty = all 1)
     bool sparse = false;  // most cells have chi == 0 at every wavelength (counted by rc_set_atmosphere): skip their gathers
@@ -259,6 +260,7 @@ bool make_plan_uncached(const rc_config &cfg, int nm, bool line, int nx, int ny,
         if (any) { P.state = cur; cur += 8 * field * P.NM; }
     }
     P.maxchi = cur; cur += align_up((size_t)std::max(L, 1) * sizeof(int));
+    P.sumchi = cur; cur += align_up((size_t)std::max(L, 1) * sizeof(unsigned long long));
     P.thin = cur;   cur += align_up((size_t)P.nb * sizeof(int));
     P.has_occ = ncell % 32 == 0 && P.NM == 1 && !line;
     if (P.has_occ) { P.occ = cur; cur += align_up((ncell / 32) * P.nb * sizeof(unsigned)); }
@@ -436,7 +438,10 @@ static int update_thin_flags(rc_ctx *ctx) {
     const bool accum = (ctx->cfg.flags & RC_ACCUM_J) != 0;
     bool all_thin = true, any_weighted = false;
     for (int l = 0; l < P.L; l++) {
-        const bool thin = (int)ctx->maxchi_h.size() == P.L && ctx->maxchi_h[l] > 0.f && (double)ctx->maxchi_h[l] * diag < 1.0 && !(l < (int)ctx->lit_h.size() && ctx->lit_h[l]);
+        // thin: even the most opaque cell x the diagonal is below 1, or the plane is mostly empty (mean opacity x diagonal
+        // below 0.05: compact structure in near-vacuum, most rays see almost nothing)
+        const bool thin = (int)ctx->maxchi_h.size() == P.L && ctx->maxchi_h[l] > 0.f &&
+                          ((double)ctx->maxchi_h[l] * diag < 1.0 || ctx->meanchi_h[l] * diag < 0.05) && !(l < (int)ctx->lit_h.size() && ctx->lit_h[l]);
         const bool weighted = !(l < (int)ctx->w_h.size()) || ctx->w_h[l] != 0.f;
         if (accum && weighted) { any_weighted = true; all_thin = all_thin && thin; }
         if (((thin && !accum) || force) && !off) flags[l / P.LV] = 1;
@@ -455,8 +460,14 @@ static int fetch_maxchi(rc_ctx *ctx) {
     std::vector<int> bits((size_t)P.L, 0);
     RC_CUDA(ctx, cudaMemcpyAsync(bits.data(), ctx->ws + P.maxchi, bits.size() * sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
     RC_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    std::vector<unsigned long long> sums((size_t)P.L, 0);
+    RC_CUDA(ctx, cudaMemcpy(sums.data(), ctx->ws + P.sumchi, sums.size() * sizeof(unsigned long long), cudaMemcpyDeviceToHost));
     ctx->maxchi_h.resize((size_t)P.L);
-    for (int l = 0; l < P.L; l++) std::memcpy(&ctx->maxchi_h[l], &bits[l], sizeof(float));
+    ctx->meanchi_h.resize((size_t)P.L);
+    for (int l = 0; l < P.L; l++) {
+        std::memcpy(&ctx->maxchi_h[l], &bits[l], sizeof(float));
+        ctx->meanchi_h[l] = (double)sums[l] / 1048576.0 / ((double)P.nx * P.ny);
+    }
     return RC_OK;
 }
 
@@ -539,10 +550,11 @@ int rc_set_atmosphere(rc_ctx *ctx, const float *chi, const float *eta, int nx, i
         unsigned long long h = 0;
         ctx->sparse = false;
         // one pass over chi: empty cells (for the sparse march) and the largest opacity of every wavelength (thin flags)
-        const bool want_max = (size_t)nlambda * sizeof(int) <= 40000;
+        const bool want_max = (size_t)nlambda * 12 <= 40000;
         RC_CUDA(ctx, cudaMemsetAsync(cnt, 0, sizeof(*cnt), ctx->stream));
         RC_CUDA(ctx, rc::launch_count_empty(chi, (long long)nx * ny, nlambda, (int *)(ctx->ws + ctx->plan.A[0]), cnt,
-                                            want_max ? (int *)(ctx->ws + ctx->plan.maxchi) : nullptr, ctx->stream));  // A[0] is free between solves
+                                            want_max ? (int *)(ctx->ws + ctx->plan.maxchi) : nullptr,
+                                            (unsigned long long *)(ctx->ws + ctx->plan.sumchi), ctx->stream));  // A[0] is free between solves
         RC_CUDA(ctx, cudaMemcpyAsync(&h, cnt, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream));
         ctx->maxchi_h.clear();
         if (want_max) { const int rc = fetch_maxchi(ctx); if (rc != RC_OK) return rc; }
@@ -573,9 +585,9 @@ int rc_set_line_atmosphere(rc_ctx *ctx, const float *line, int nx, int ny, const
     RC_CUDA(ctx, cudaMemcpyAsync(ctx->ws + ctx->plan.xls, h.data(), h.size() * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
     RC_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     ctx->maxchi_h.clear();
-    if ((size_t)nlambda * sizeof(int) <= 40000) {
+    if ((size_t)nlambda * 12 <= 40000) {
         RC_CUDA(ctx, rc::launch_line_maxchi(line, (const float *)(ctx->ws + ctx->plan.xls) + ctx->plan.Lpad, (long long)nx * ny, nlambda,
-                                            (int *)(ctx->ws + ctx->plan.maxchi), ctx->stream));
+                                            (int *)(ctx->ws + ctx->plan.maxchi), (unsigned long long *)(ctx->ws + ctx->plan.sumchi), ctx->stream));
         const int rc = fetch_maxchi(ctx);
         if (rc != RC_OK) return rc;
     }

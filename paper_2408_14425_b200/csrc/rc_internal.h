@@ -105,8 +105,9 @@ cudaError_t launch_table_build(const TableBuildParams &p, cudaStream_t st);
 cudaError_t launch_reduce_jbar(const float *Jpart, float *Jbar, long long ncell, int nb, cudaStream_t st);
 cudaError_t launch_count(const MarchParams &p, unsigned long long *total, cudaStream_t st);
 cudaError_t launch_gather_probe(const float *buf, unsigned long long nsector, int iters, int blocks, float *sink, cudaStream_t st);
-cudaError_t launch_count_empty(const float *chi, long long ncell, int L, int *mark, unsigned long long *count, int *maxchi, cudaStream_t st);
-cudaError_t launch_line_maxchi(const float *line, const float *xl, long long ncell, int L, int *maxchi, cudaStream_t st);
+cudaError_t launch_count_empty(const float *chi, long long ncell, int L, int *mark, unsigned long long *count, int *maxchi,
+                               unsigned long long *sumchi, cudaStream_t st);
+cudaError_t launch_line_maxchi(const float *line, const float *xl, long long ncell, int L, int *maxchi, unsigned long long *sumchi, cudaStream_t st);
 cudaError_t launch_alo(const AloParams &p, cudaStream_t st);
 cudaError_t launch_bulk_probe(const float *buf, unsigned long long nsector, int iters, int sms, float *sink, cudaStream_t st, long long *bytes);
 cudaError_t launch_validate(const float *chi, const float *eta, long long n, int *flag, cudaStream_t st);

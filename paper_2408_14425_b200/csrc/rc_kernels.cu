@@ -937,39 +937,46 @@ __global__ void validate_kernel(const float *chi, const float *eta, long long n,
 // Number of cells with chi == 0 at every wavelength (rc_set_atmosphere: is the atmosphere mostly empty?).
 // Pass 1 marks the cells that have a non-zero value (coalesced over the whole array), pass 2 counts the rest.
 template <int W>  // floats per thread: 4 when nlambda is a multiple of 4, else 1
-__global__ void mark_occupied_kernel(const float *chi, long long nchunk, int chunks_per_cell, int *mark, int *maxchi, int L) {
-    // also the largest chi of every wavelength (non-negative floats order like their bit patterns): block-wide in
-    // shared memory, then one global atomicMax per wavelength and block
-    extern __shared__ int mx[];
-    for (int l = threadIdx.x; l < L; l += blockDim.x) mx[l] = 0;
+__global__ void mark_occupied_kernel(const float *chi, long long nchunk, int chunks_per_cell, int *mark, int *maxchi,
+                                     unsigned long long *sumchi, int L) {
+    // also, for every wavelength, the largest chi (non-negative floats order like their bit patterns) and the sum of
+    // chi in fixed point (2^-20; integer adds: the same result whatever the order): block-wide in shared memory,
+    // then one global atomic per wavelength and block
+    extern __shared__ unsigned long long sm[];
+    unsigned long long *sx = sm;
+    int *mx = reinterpret_cast<int *>(sm + L);
+    for (int l = threadIdx.x; l < L; l += blockDim.x) { mx[l] = 0; sx[l] = 0ull; }
     __syncthreads();
+    auto note = [&](int l, float v) {
+        atomicMax(mx + l, __float_as_int(v));
+        atomicAdd(sx + l, (unsigned long long)(fminf(v, 1e12f) * 1048576.f));
+    };
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < nchunk; i += (long long)gridDim.x * blockDim.x) {
         bool nz;
         const int c = (int)(i % chunks_per_cell);
         if constexpr (W == 4) {
             const float4 v = __ldg(reinterpret_cast<const float4 *>(chi) + i);
             nz = v.x != 0.f || v.y != 0.f || v.z != 0.f || v.w != 0.f;
-            if (maxchi && nz) {
-                atomicMax(mx + 4 * c, __float_as_int(v.x)); atomicMax(mx + 4 * c + 1, __float_as_int(v.y));
-                atomicMax(mx + 4 * c + 2, __float_as_int(v.z)); atomicMax(mx + 4 * c + 3, __float_as_int(v.w));
-            }
+            if (maxchi && nz) { note(4 * c, v.x); note(4 * c + 1, v.y); note(4 * c + 2, v.z); note(4 * c + 3, v.w); }
         } else {
             const float v = __ldg(chi + i);
             nz = v != 0.f;
-            if (maxchi && nz) atomicMax(mx + c, __float_as_int(v));
+            if (maxchi && nz) note(c, v);
         }
         if (nz) mark[i / chunks_per_cell] = 1;
     }
     __syncthreads();
     if (maxchi)
         for (int l = threadIdx.x; l < L; l += blockDim.x)
-            if (mx[l] != 0) atomicMax(maxchi + l, mx[l]);
+            if (mx[l] != 0) { atomicMax(maxchi + l, mx[l]); atomicAdd(sumchi + l, sx[l]); }
 }
 
 // Line mode: upper bound over directions of the opacity of every wavelength, chi_c + chi_line phi(max(0, |x_l| - |v|)).
-__global__ void line_maxchi_kernel(const float *line, const float *xl, long long ncell, int L, int *maxchi) {
-    extern __shared__ int mx[];
-    for (int l = threadIdx.x; l < L; l += blockDim.x) mx[l] = 0;
+__global__ void line_maxchi_kernel(const float *line, const float *xl, long long ncell, int L, int *maxchi, unsigned long long *sumchi) {
+    extern __shared__ unsigned long long sm[];
+    unsigned long long *sx = sm;
+    int *mx = reinterpret_cast<int *>(sm + L);
+    for (int l = threadIdx.x; l < L; l += blockDim.x) { mx[l] = 0; sx[l] = 0ull; }
     __syncthreads();
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < ncell * L; i += (long long)gridDim.x * blockDim.x) {
         const long long cell = i / L;
@@ -978,17 +985,23 @@ __global__ void line_maxchi_kernel(const float *line, const float *xl, long long
         const float v = sqrtf(q[4] * q[4] + q[5] * q[5]);
         const float a = fmaxf(fabsf(__ldg(xl + l)) - v, 0.f);
         const float c = fmaf(q[2], expf(-a * a) * 0.5641895835477563f, q[0]);
-        if (c > 0.f) atomicMax(mx + l, __float_as_int(c));
+        if (c > 0.f) {
+            atomicMax(mx + l, __float_as_int(c));
+            atomicAdd(sx + l, (unsigned long long)(fminf(c, 1e12f) * 1048576.f));
+        }
     }
     __syncthreads();
     for (int l = threadIdx.x; l < L; l += blockDim.x)
-        if (mx[l] != 0) atomicMax(maxchi + l, mx[l]);
+        if (mx[l] != 0) { atomicMax(maxchi + l, mx[l]); atomicAdd(sumchi + l, sx[l]); }
 }
 
-cudaError_t launch_line_maxchi(const float *line, const float *xl, long long ncell, int L, int *maxchi, cudaStream_t st) {
+// maxchi: [L] ints (float bit patterns) followed, 8-byte aligned, by sumchi: [L] unsigned long long (see rc_api.cu)
+cudaError_t launch_line_maxchi(const float *line, const float *xl, long long ncell, int L, int *maxchi, unsigned long long *sumchi, cudaStream_t st) {
     cudaError_t e = cudaMemsetAsync(maxchi, 0, sizeof(int) * (size_t)L, st);
     if (e != cudaSuccess) return e;
-    line_maxchi_kernel<<<148 * 8, 256, sizeof(int) * (size_t)L, st>>>(line, xl, ncell, L, maxchi);
+    e = cudaMemsetAsync(sumchi, 0, sizeof(unsigned long long) * (size_t)L, st);
+    if (e != cudaSuccess) return e;
+    line_maxchi_kernel<<<148 * 8, 256, 12 * (size_t)L, st>>>(line, xl, ncell, L, maxchi, sumchi);
     return cudaGetLastError();
 }
 
@@ -1001,18 +1014,21 @@ __global__ void count_unmarked_kernel(const int *mark, long long ncell, unsigned
 }
 
 // mark: scratch of ncell ints (device); count: zeroed by the caller; maxchi: null or [L] ints (float bit patterns)
-cudaError_t launch_count_empty(const float *chi, long long ncell, int L, int *mark, unsigned long long *count, int *maxchi, cudaStream_t st) {
+cudaError_t launch_count_empty(const float *chi, long long ncell, int L, int *mark, unsigned long long *count, int *maxchi,
+                               unsigned long long *sumchi, cudaStream_t st) {
     cudaError_t e = cudaMemsetAsync(mark, 0, sizeof(int) * (size_t)ncell, st);
     if (e != cudaSuccess) return e;
     if (maxchi) {
         e = cudaMemsetAsync(maxchi, 0, sizeof(int) * (size_t)L, st);
         if (e != cudaSuccess) return e;
+        e = cudaMemsetAsync(sumchi, 0, sizeof(unsigned long long) * (size_t)L, st);
+        if (e != cudaSuccess) return e;
     }
-    const size_t sm = sizeof(int) * (size_t)L;
+    const size_t sm = 12 * (size_t)L;
     if (L % 4 == 0 && (reinterpret_cast<uintptr_t>(chi) & 15) == 0)
-        mark_occupied_kernel<4><<<148 * 16, 256, sm, st>>>(chi, ncell * (L / 4), L / 4, mark, maxchi, L);
+        mark_occupied_kernel<4><<<148 * 16, 256, sm, st>>>(chi, ncell * (L / 4), L / 4, mark, maxchi, sumchi, L);
     else
-        mark_occupied_kernel<1><<<148 * 16, 256, sm, st>>>(chi, ncell * L, L, mark, maxchi, L);
+        mark_occupied_kernel<1><<<148 * 16, 256, sm, st>>>(chi, ncell * L, L, mark, maxchi, sumchi, L);
     count_unmarked_kernel<<<148 * 4, 256, 0, st>>>(mark, ncell, count);
     return cudaGetLastError();
 }
