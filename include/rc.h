@@ -33,6 +33,14 @@
  *   Inputs   chi >= 0, eta >= 0, finite; eta must be 0 where chi is 0 (emission without opacity
  *            is not representable as chi*S; such cells are treated as vacuum).
  *   There is no CPU fallback and no other backend: without an sm_100 device rc_create fails.
+ *
+ * Developer overrides (environment variables, for measurements and tests; none changes a result beyond rounding
+ * unless noted): RC_MARCH_VARIANT=0..4 (register-ring depth / occupancy of the march), RC_PATCH_LOG2=2..5 with
+ * RC_PATCH_FROM=i (lane patch width for cascades >= i), RC_CPW_FROM=i (child-per-warp for cascades >= i, -1 off),
+ * RC_BANDS=n / RC_L2_MB=x (L2 banding), RC_NO_SPARSE / RC_FORCE_SPARSE (occupancy-bitmap march), RC_NO_THIN /
+ * RC_FORCE_THIN (thin-accurate update; RC_NO_THIN can cost accuracy on optically thin planes), RC_NO_GRAPH (no CUDA
+ * graph replay on small grids), RC_TAU_CUT=x (early-exit threshold on tau log2 e; below 126 it drops transmittances
+ * below 2^-x).
  */
 #ifndef RC_H_
 #define RC_H_
