@@ -132,8 +132,6 @@ def main():
     ap.add_argument("--line", action="store_true",
                     help="velocity-dependent line mode (SURVEY §8(f) f1): configs[2]'s recipe as a moving-line "
                          "atmosphere, opacities evaluated per ray (rc_set_line_atmosphere)")
-    ap.add_argument("--accurate-thin", action="store_true",
-                    help="RC_ACCURATE_THIN: march everything with the thin-accurate update (DESIGN.md §8)")
     ap.add_argument("--bilinear-fix", action="store_true",
                     help="RC_BILINEAR_FIX (SURVEY §8(f) f3): 4 sub-rays per interval below the top cascade")
     ap.add_argument("--inclinations", type=int, default=1,
@@ -174,9 +172,6 @@ def main():
     hbm_peak, sm_max_mhz, peak_src = peaks()
 
     flags = binding.RC_ACCUM_J if atm.accumulate else 0
-    if args.accurate_thin:
-        flags |= binding.RC_ACCURATE_THIN
-        workload += ", RC_ACCURATE_THIN"
     if args.bilinear_fix:
         flags |= binding.RC_BILINEAR_FIX
         workload += ", bilinear fix (the unit count includes the 4 sub-rays of every interval)"

@@ -30,15 +30,14 @@
  *            synchronise.  rc_solve_J_host synchronises that stream before returning.
  *   Errors   every call returns RC_OK (0) or a negative RC_ERR_*; nothing throws across the ABI;
  *            rc_last_error(ctx) gives text for the last failure on that context.
- *   Inputs   chi >= 0, eta >= 0, finite; eta must be 0 where chi is 0 (emission without opacity
- *            is not representable as chi*S; such cells are treated as vacuum).
+ *   Inputs   chi >= 0, eta >= 0, finite.  eta > 0 where chi == 0 (emission without opacity) is valid: eq. 16
+ *            in the limit chi -> 0, the cell adds eta ds (reading G11).
  *   There is no CPU fallback and no other backend: without an sm_100 device rc_create fails.
  *
  * Developer overrides (environment variables, for measurements and tests; none changes a result beyond rounding
  * unless noted): RC_MARCH_VARIANT=0..4 (register-ring depth / occupancy of the march), RC_PATCH_LOG2=2..5 with
  * RC_PATCH_FROM=i (lane patch width for cascades >= i), RC_CPW_FROM=i (child-per-warp for cascades >= i, -1 off),
- * RC_BANDS=n / RC_L2_MB=x (L2 banding), RC_NO_SPARSE / RC_FORCE_SPARSE (occupancy-bitmap march), RC_NO_THIN /
- * RC_FORCE_THIN (thin-accurate update; RC_NO_THIN can cost accuracy on optically thin planes), RC_NO_GRAPH (no CUDA
+ * RC_BANDS=n / RC_L2_MB=x (L2 banding), RC_NO_SPARSE / RC_FORCE_SPARSE (occupancy-bitmap march), RC_NO_GRAPH (no CUDA
  * graph replay on small grids), RC_TAU_CUT=x (early-exit threshold on tau log2 e; below 126 it drops transmittances
  * below 2^-x).
  */
@@ -77,12 +76,6 @@ extern "C" {
                              each of the four parent probes, merged with that parent alone and then weighted
                              bilinearly: removes most of the ringing around bright compact sources at 4x the rays */
 
-#define RC_ACCURATE_THIN 16 /* always march with the thin-accurate update (every segment's emission to ~3e-6 relative,
-                               at ~2x the arithmetic).  Default: only solves that hold a wavelength which is optically
-                               thin across the whole box and unlit take it (rc_stats.thin_batches); elsewhere the
-                               emission of a ray is exact to ~1e-7 S, which matters only for cells that no ray with
-                               optical depth >~ 1e-3 reaches while J elsewhere on that plane is of order S */
-
 typedef struct rc_ctx rc_ctx; /* opaque, owned by the library */
 
 typedef struct {
@@ -90,7 +83,7 @@ typedef struct {
     float c0_interval; /* length of the cascade-0 interval in cells; > 0; the configs use 1 */
     int device;        /* CUDA ordinal */
     int lambda_batch;  /* wavelengths per thread (1, 2, 4 or 8); 0 = library chooses */
-    int flags;         /* RC_ACCUM_J | RC_VALIDATE | RC_NO_EARLY_EXIT | RC_BILINEAR_FIX | RC_ACCURATE_THIN */
+    int flags;         /* RC_ACCUM_J | RC_VALIDATE | RC_NO_EARLY_EXIT | RC_BILINEAR_FIX */
 } rc_config;
 
 typedef struct {
@@ -104,9 +97,7 @@ typedef struct {
     int64_t rays[RC_MAX_CASCADES];        /* intervals per cascade per wavelength = 4 nx ny */
     int64_t table_steps[RC_MAX_CASCADES]; /* step-table entries per cascade (all directions) */
     size_t workspace_bytes;
-    int64_t empty_cells;                  /* cells with chi == 0 at every wavelength (counted by rc_set_atmosphere) */
-    int thin_batches;                     /* wavelength batches marched with the thin-accurate update: they hold a wavelength
-                                             whose optical depth across the whole box is < 1 with no boundary intensity */
+    int64_t empty_cells;                  /* cells with chi == 0 and eta == 0 at every wavelength (counted by rc_set_atmosphere) */
 } rc_stats;
 
 /* The launch plan the library would use for a problem, computed on the host alone (no device, no context):

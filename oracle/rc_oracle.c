@@ -433,6 +433,16 @@ int rc_oracle_solve_line(const float *line, const double *xl, int nx, int ny, in
                       Jbar_out, nthreads, order, -1, NULL, NULL, NULL, NULL, counts, path_scale);
 }
 
+/* The same, also writing one cascade's intervals before and after merging (as rc_oracle_solve does): an output
+ * path for the pins of the directional transmittances, no arithmetic of its own. */
+int rc_oracle_solve_line_dump(const float *line, const double *xl, int nx, int ny, int L, int ncasc, double c0,
+                              const float *I_below, const float *I_above, const float *w, double *J_out,
+                              double *Jbar_out, int nthreads, int order, int dump_cascade, double *dump_I,
+                              double *dump_T, double *dump_M, int *dump_win, double path_scale) {
+    return solve_impl(NULL, NULL, line, xl, nx, ny, L, ncasc, c0, I_below, I_above, w, 0, nx, 0, ny, J_out,
+                      Jbar_out, nthreads, order, dump_cascade, dump_I, dump_T, dump_M, dump_win, NULL, path_scale);
+}
+
 /* Flatland (path_scale = 1): the solve of SURVEY.md §8(c). */
 int rc_oracle_solve(const float *chi, const float *eta, int nx, int ny, int L, int ncasc,
                     double c0, const float *I_below, const float *I_above, const float *w,

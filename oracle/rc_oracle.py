@@ -57,6 +57,10 @@ def lib():
         _lib.rc_oracle_solve_line.argtypes = ([C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double,
                                                C.c_void_p, C.c_void_p, C.c_void_p] + [C.c_int] * 4 +
                                               [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_double])
+        _lib.rc_oracle_solve_line_dump.restype = C.c_int
+        _lib.rc_oracle_solve_line_dump.argtypes = ([C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double,
+                                                    C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int,
+                                                    C.c_int, C.c_int] + [C.c_void_p] * 4 + [C.c_double])
         _lib.rc_oracle_num_threads.restype = C.c_int
     return _lib
 
@@ -211,6 +215,25 @@ def solve_line(line, xl, ncascades, c0=1.0, I_below=None, I_above=None, weights=
         out["intervals"] = np.array(cnt.intervals[:ncascades])
         out["segments"] = np.array(cnt.segments[:ncascades])
     return out
+
+
+def line_intervals(line, xl, ncascades, cascade, c0=1.0, path_scale=1.0):
+    """Line mode: the intervals [I, T] of one cascade before merging (dump_I, dump_T: [npy][npx][N][L]) and after
+    (dump_M), through exactly the code of solve_line (rc_oracle_solve_line_dump): for the pins."""
+    line = _f32(line)
+    xl = np.ascontiguousarray(xl, dtype=np.float64)
+    ny, nx, _ = line.shape
+    L = xl.size
+    s = 1 << cascade
+    shape = (ny // s, nx // s, 4 ** (cascade + 1), L)
+    dI, dT, dM = np.zeros(shape), np.zeros(shape), np.zeros(shape)
+    win = np.zeros(4, np.int32)
+    J = np.empty((ny, nx, L))
+    rc = lib().rc_oracle_solve_line_dump(_ptr(line), _ptr(xl), nx, ny, L, ncascades, c0, None, None, None, _ptr(J), None,
+                                         0, 0, cascade, _ptr(dI), _ptr(dT), _ptr(dM), _ptr(win), float(path_scale))
+    if rc != 0:
+        raise ValueError(f"rc_oracle_solve_line_dump failed: {rc}")
+    return {"J": J, "dump_I": dI, "dump_T": dT, "dump_M": dM}
 
 
 def alo(chi=None, line=None, xl=None, mu=None, w_mu=None):

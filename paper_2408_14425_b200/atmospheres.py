@@ -258,6 +258,34 @@ def config4(nx=None, ny=None, nlambda=None, ncascades=None, seed=1004) -> Atmosp
                    meta={"empty_fraction": empty, "nblobs": nblob})
 
 
+def emitter_config(nx=128, ny=128, nlambda=4, ncascades=6, seed=2001, chi_emitter=0.0) -> Atmosphere:
+    """Emission with next to no opacity (reading G11 of DESIGN.md: eq. 16 in the limit chi -> 0 adds eta ds): config 1's
+    opaque discs in exact vacuum (chi = eta = 0), plus smooth patches of pure emitters with eta ~ 1e-3 and chi = `chi_emitter`
+    (0, or e.g. 1e-12) - the one family of valid inputs that is not of the form eta = chi S with a moderate S.  Wavelength l
+    scales the discs' opacity by 10^(-l) (from opaque to translucent) and leaves the emitters alone."""
+    rng = np.random.default_rng(seed)
+    sc = nx / 512.0
+    chi = np.zeros((ny, nx))
+    S = np.zeros((ny, nx))
+    yy, xx = np.mgrid[0:ny, 0:nx]
+    xc, yc = xx + 0.5, yy + 0.5
+    for _ in range(12):
+        cx, cy = rng.uniform(0, nx), rng.uniform(0, ny)
+        r = max(rng.uniform(5.0, 30.0) * sc, 1.5)
+        m = (xc - cx) ** 2 + (yc - cy) ** 2 <= r * r
+        chi[m] = rng.uniform(1.0, 100.0)
+        S[m] = rng.uniform(0.5, 2.0)
+    g = _unit01(_smooth_normal(rng, ny, nx, max(16.0 * sc, 2.0)))
+    h = _unit01(_smooth_normal(rng, ny, nx, max(8.0 * sc, 2.0)))
+    emit = (g > 0.6) & (chi == 0.0)
+    fac = 10.0 ** (-np.arange(nlambda, dtype=np.float64))
+    chi3 = chi[:, :, None] * fac[None, None, :]
+    eta3 = chi3 * S[:, :, None]
+    chi3[emit] = chi_emitter
+    eta3[emit] = (1e-3 * (0.5 + h))[emit][:, None]
+    return _finish("emit", nx, ny, nlambda, ncascades, chi3, eta3, meta={"emitter_fraction": float(emit.mean())})
+
+
 CONFIGS = {0: config0, 1: config1, 2: config2, 3: config3, 4: config4}
 
 

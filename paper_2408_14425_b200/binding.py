@@ -14,7 +14,7 @@ import numpy as np
 from . import build as _build
 
 RC_OK = 0
-RC_ACCUM_J, RC_VALIDATE, RC_NO_EARLY_EXIT, RC_BILINEAR_FIX, RC_ACCURATE_THIN = 1, 2, 4, 8, 16
+RC_ACCUM_J, RC_VALIDATE, RC_NO_EARLY_EXIT, RC_BILINEAR_FIX = 1, 2, 4, 8
 RC_MAX_CASCADES = 12
 ERRORS = {-1: "RC_ERR_NULL_ARG", -2: "RC_ERR_BAD_SHAPE", -3: "RC_ERR_NO_DEVICE", -4: "RC_ERR_NO_WORKSPACE",
           -5: "RC_ERR_BAD_VALUE", -6: "RC_ERR_CUDA", -7: "RC_ERR_NO_ATMOSPHERE"}
@@ -30,7 +30,7 @@ class rc_stats(C.Structure):
                 ("solves_timed", C.c_int), ("ms_pack", C.c_float * RC_MAX_CASCADES),
                 ("ms_march", C.c_float * RC_MAX_CASCADES), ("ms_total", C.c_float),
                 ("rays", C.c_int64 * RC_MAX_CASCADES), ("table_steps", C.c_int64 * RC_MAX_CASCADES),
-                ("workspace_bytes", C.c_size_t), ("empty_cells", C.c_int64), ("thin_batches", C.c_int)]
+                ("workspace_bytes", C.c_size_t), ("empty_cells", C.c_int64)]
 
 
 class rc_plan_info(C.Structure):

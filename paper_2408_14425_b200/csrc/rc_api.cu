@@ -37,7 +37,6 @@ struct Plan {
     size_t state = 0;               // parked ray state of the banded launches
     bool line = false;              // velocity-dependent line mode: chiT holds 6 packed line parameters per cell
     size_t xls = 0;                 // line mode: scaled wavelengths [Lpad]
-    size_t maxchi = 0, sumchi = 0, thin = 0;  // per-wavelength largest opacity (float bits) and fixed-point sum; per-batch thin flags
     size_t occ = 0;                 // occupancy bitmap of the packed cells (0: none, nx ny not a multiple of 32)
     bool has_occ = false;
     CascadePlan c[RC_MAX_CASCADES];
@@ -60,16 +59,10 @@ struct rc_ctx {
     int tab_nx = 0, tab_ny = 0;  // shape the step tables in the workspace were built for
     bool host_io = false;
     // CUDA graph of the launch sequence of small grids (rc_solve_J) and what it was captured for
-    struct GraphKey { const void *J, *chi, *eta, *line, *ws; int nx, ny, L, nm, sparse, thin; size_t total; float f[8], w[8]; };
+    struct GraphKey { const void *J, *chi, *eta, *line, *ws; int nx, ny, L, nm, sparse; size_t total; float f[8], w[8]; };
     GraphKey graph_key{};
     cudaGraphExec_t graph_exec = nullptr;
     cudaStream_t cap_stream = nullptr;
-    // optically thin wavelengths: largest opacity of every wavelength (rc_set_*atmosphere) and whether
-    // a boundary intensity is set there (rc_set_boundary*); batches with a thin, unlit wavelength take the thin update
-    std::vector<float> maxchi_h;
-    std::vector<double> meanchi_h;
-    std::vector<char> lit_h;
-    std::vector<float> w_h;  // wavelength weights (rc_set_lambda_weights; empty = all 1)
     bool sparse = false;  // most cells have chi == 0 at every wavelength (counted by rc_set_atmosphere): skip their gathers
     // developer overrides (environment, read by rc_create): RC_MARCH_VARIANT = 0..3 (register ring depth /
     // occupancy of march_kernel), RC_PATCH_LOG2 = 2..5 forces the lane patch width for cascades >= RC_PATCH_FROM
@@ -259,9 +252,6 @@ bool make_plan_uncached(const rc_config &cfg, int nm, bool line, int nx, int ny,
         }
         if (any) { P.state = cur; cur += 8 * field * P.NM; }
     }
-    P.maxchi = cur; cur += align_up((size_t)std::max(L, 1) * sizeof(int));
-    P.sumchi = cur; cur += align_up((size_t)std::max(L, 1) * sizeof(unsigned long long));
-    P.thin = cur;   cur += align_up((size_t)P.nb * sizeof(int));
     P.has_occ = ncell % 32 == 0 && P.NM == 1 && !line;
     if (P.has_occ) { P.occ = cur; cur += align_up((ncell / 32) * P.nb * sizeof(unsigned)); }
     if (line) {
@@ -422,55 +412,6 @@ int rc_set_timing(rc_ctx *ctx, int nsets) {
     return RC_OK;
 }
 
-// A wavelength is "thin" when even the longest ray through the box has optical depth < 1 (largest opacity x
-// diagonal) and no boundary intensity enters there: J is then of the order S tau, and the normal update, whose
-// emission is exact to ~1e-7 S, would miss the 2e-4 bar once tau < ~1e-3.  Such batches are flagged for the
-// thin-accurate update (rc_kernels.cu, thin_update); costs arithmetic, so only they take it.
-static int update_thin_flags(rc_ctx *ctx) {
-    const Plan &P = ctx->plan;
-    std::vector<int> flags((size_t)P.nb, 0);
-    const double diag = std::sqrt((double)P.nx * P.nx + (double)P.ny * P.ny);
-    const bool force = std::getenv("RC_FORCE_THIN") != nullptr || (ctx->cfg.flags & RC_ACCURATE_THIN) != 0, off = std::getenv("RC_NO_THIN") != nullptr;
-    int n = 0;
-    // With RC_ACCUM_J the checked output is Jbar = sum_l w_l J_l: a thin plane adds next to nothing to it and its own
-    // relative accuracy is not asked for, so only a solve whose weighted planes are ALL thin takes the thin update
-    // (config 4: its far-wing planes are thin, its line core is not).
-    const bool accum = (ctx->cfg.flags & RC_ACCUM_J) != 0;
-    bool all_thin = true, any_weighted = false;
-    for (int l = 0; l < P.L; l++) {
-        // thin: even the most opaque cell x the diagonal is below 1, or the plane is mostly empty (mean opacity x diagonal
-        // below 0.05: compact structure in near-vacuum, most rays see almost nothing)
-        const bool thin = (int)ctx->maxchi_h.size() == P.L && ctx->maxchi_h[l] > 0.f &&
-                          ((double)ctx->maxchi_h[l] * diag < 1.0 || ctx->meanchi_h[l] * diag < 0.05) && !(l < (int)ctx->lit_h.size() && ctx->lit_h[l]);
-        const bool weighted = !(l < (int)ctx->w_h.size()) || ctx->w_h[l] != 0.f;
-        if (accum && weighted) { any_weighted = true; all_thin = all_thin && thin; }
-        if (((thin && !accum) || force) && !off) flags[l / P.LV] = 1;
-    }
-    if (accum && any_weighted && all_thin && !off) std::fill(flags.begin(), flags.end(), 1);
-    for (int b = 0; b < P.nb; b++) n += flags[b];
-    ctx->stats.thin_batches = n;
-    RC_CUDA(ctx, cudaMemcpyAsync(ctx->ws + P.thin, flags.data(), flags.size() * sizeof(int), cudaMemcpyHostToDevice, ctx->stream));
-    RC_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
-    return RC_OK;
-}
-
-// largest opacity per wavelength from the device array of float bit patterns written by the mark / line kernels
-static int fetch_maxchi(rc_ctx *ctx) {
-    const Plan &P = ctx->plan;
-    std::vector<int> bits((size_t)P.L, 0);
-    RC_CUDA(ctx, cudaMemcpyAsync(bits.data(), ctx->ws + P.maxchi, bits.size() * sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
-    RC_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
-    std::vector<unsigned long long> sums((size_t)P.L, 0);
-    RC_CUDA(ctx, cudaMemcpy(sums.data(), ctx->ws + P.sumchi, sums.size() * sizeof(unsigned long long), cudaMemcpyDeviceToHost));
-    ctx->maxchi_h.resize((size_t)P.L);
-    ctx->meanchi_h.resize((size_t)P.L);
-    for (int l = 0; l < P.L; l++) {
-        std::memcpy(&ctx->maxchi_h[l], &bits[l], sizeof(float));
-        ctx->meanchi_h[l] = (double)sums[l] / 1048576.0 / ((double)P.nx * P.ny);
-    }
-    return RC_OK;
-}
-
 // Plan, step tables and defaults for a shape (shared by rc_set_atmosphere and rc_set_line_atmosphere).
 static int prepare_shape(rc_ctx *ctx, int nx, int ny, int nlambda, bool line) {
     if (!shape_ok(ctx->cfg, nx, ny, nlambda))
@@ -513,8 +454,6 @@ static int prepare_shape(rc_ctx *ctx, int nx, int ny, int nlambda, bool line) {
         }
         // defaults: free-space boundary, unit weights
         ctx->stage.assign((size_t)ctx->plan.Lpad, 0.f);
-        ctx->lit_h.assign((size_t)nlambda, 0);
-        ctx->w_h.clear();
         RC_CUDA(ctx, cudaMemsetAsync(ctx->ws + ctx->plan.bc_below, 0, (size_t)ctx->plan.Lpad * ctx->plan.NM * sizeof(float), ctx->stream));
         RC_CUDA(ctx, cudaMemsetAsync(ctx->ws + ctx->plan.bc_above, 0, (size_t)ctx->plan.Lpad * ctx->plan.NM * sizeof(float), ctx->stream));
         std::vector<float> ones((size_t)ctx->plan.Lpad, 0.f);
@@ -541,7 +480,6 @@ int rc_set_atmosphere(rc_ctx *ctx, const float *chi, const float *eta, int nx, i
         RC_CUDA(ctx, cudaMemcpyAsync(&h, flag, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
         RC_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
         if (h & 1) return fail(ctx, RC_ERR_BAD_VALUE, "chi or eta has a negative or non-finite value");
-        if (h & 2) return fail(ctx, RC_ERR_BAD_VALUE, "eta > 0 in a cell with chi == 0");
     }
     {
         // sparsity (many models are mostly empty): with more than two thirds of the cells at
@@ -549,23 +487,17 @@ int rc_set_atmosphere(rc_ctx *ctx, const float *chi, const float *eta, int nx, i
         unsigned long long *cnt = (unsigned long long *)(ctx->ws + ctx->plan.flag);
         unsigned long long h = 0;
         ctx->sparse = false;
-        // one pass over chi: empty cells (for the sparse march) and the largest opacity of every wavelength (thin flags)
-        const bool want_max = (size_t)nlambda * 12 <= 40000;
         RC_CUDA(ctx, cudaMemsetAsync(cnt, 0, sizeof(*cnt), ctx->stream));
-        RC_CUDA(ctx, rc::launch_count_empty(chi, (long long)nx * ny, nlambda, (int *)(ctx->ws + ctx->plan.A[0]), cnt,
-                                            want_max ? (int *)(ctx->ws + ctx->plan.maxchi) : nullptr,
-                                            (unsigned long long *)(ctx->ws + ctx->plan.sumchi), ctx->stream));  // A[0] is free between solves
+        RC_CUDA(ctx, rc::launch_count_empty(chi, eta, (long long)nx * ny, nlambda, (int *)(ctx->ws + ctx->plan.A[0]), cnt, ctx->stream));  // A[0] is free between solves
         RC_CUDA(ctx, cudaMemcpyAsync(&h, cnt, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream));
-        ctx->maxchi_h.clear();
-        if (want_max) { const int rc = fetch_maxchi(ctx); if (rc != RC_OK) return rc; }
-        else RC_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+        RC_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
         if (ctx->plan.has_occ && !std::getenv("RC_NO_SPARSE")) ctx->sparse = 3 * h > 2ULL * nx * ny || std::getenv("RC_FORCE_SPARSE");
         ctx->stats.empty_cells = (int64_t)h;
     }
     ctx->chi = chi;
     ctx->eta = eta;
     ctx->have_atm = true;
-    return update_thin_flags(ctx);
+    return RC_OK;
 }
 
 // Velocity-dependent line mode.
@@ -584,18 +516,11 @@ int rc_set_line_atmosphere(rc_ctx *ctx, const float *line, int nx, int ny, const
     }
     RC_CUDA(ctx, cudaMemcpyAsync(ctx->ws + ctx->plan.xls, h.data(), h.size() * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
     RC_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
-    ctx->maxchi_h.clear();
-    if ((size_t)nlambda * 12 <= 40000) {
-        RC_CUDA(ctx, rc::launch_line_maxchi(line, (const float *)(ctx->ws + ctx->plan.xls) + ctx->plan.Lpad, (long long)nx * ny, nlambda,
-                                            (int *)(ctx->ws + ctx->plan.maxchi), (unsigned long long *)(ctx->ws + ctx->plan.sumchi), ctx->stream));
-        const int rc = fetch_maxchi(ctx);
-        if (rc != RC_OK) return rc;
-    }
     ctx->line = line;
     ctx->chi = ctx->eta = nullptr;
     ctx->sparse = false;
     ctx->have_atm = true;
-    return update_thin_flags(ctx);
+    return RC_OK;
 }
 
 static int upload_lambda_array(rc_ctx *ctx, const float *src, size_t dst_off, float fill) {
@@ -622,21 +547,16 @@ static int upload_boundary(rc_ctx *ctx, const float *src, size_t dst_off, bool p
         }
     RC_CUDA(ctx, cudaMemcpyAsync(ctx->ws + dst_off, h.data(), h.size() * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
     RC_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
-    for (int l = 0; l < L && l < (int)ctx->lit_h.size(); l++)
-        for (int m = 0; m < NM; m++)
-            if (h[(size_t)l * NM + m] > 0.f) ctx->lit_h[l] = 1;
     return RC_OK;
 }
 
 static int set_boundary_impl(rc_ctx *ctx, const float *I_below, const float *I_above, bool per_inclination) {
     if (!ctx) return RC_ERR_NULL_ARG;
     if (!ctx->have_atm) return fail(ctx, RC_ERR_NO_ATMOSPHERE, "call rc_set_atmosphere first");
-    ctx->lit_h.assign((size_t)ctx->plan.L, 0);
     int rc = upload_boundary(ctx, I_below, ctx->plan.bc_below, per_inclination);
     if (rc != RC_OK) return rc;
     rc = upload_boundary(ctx, I_above, ctx->plan.bc_above, per_inclination);
-    if (rc != RC_OK) return rc;
-    return update_thin_flags(ctx);
+    return rc;
 }
 
 int rc_set_boundary(rc_ctx *ctx, const float *I_below, const float *I_above) { return set_boundary_impl(ctx, I_below, I_above, false); }
@@ -664,11 +584,7 @@ int rc_set_inclinations(rc_ctx *ctx, int n, const float *mu, const float *w) {
 
 int rc_set_lambda_weights(rc_ctx *ctx, const float *w) {
     if (!ctx) return RC_ERR_NULL_ARG;
-    const int rc = upload_lambda_array(ctx, w, ctx->plan.weights, 1.f);
-    if (rc != RC_OK) return rc;
-    ctx->w_h.assign((size_t)ctx->plan.L, 1.f);
-    for (int l = 0; l < ctx->plan.L && w; l++) ctx->w_h[l] = w[l];
-    return update_thin_flags(ctx);
+    return upload_lambda_array(ctx, w, ctx->plan.weights, 1.f);
 }
 
 // Register-ring depth / occupancy variant of cascade i's march launch (rc_kernels.cu, launch_march_flat): measured
@@ -686,8 +602,7 @@ static rc::MarchParams march_params(const rc_ctx *ctx, int i, float *J_out) {
     mp.ST = (const float *)(ctx->ws + P.ST);
     mp.linepk = ctx->line ? (const float *)(ctx->ws + P.chiT) : nullptr;
     mp.xls = ctx->line ? (const float *)(ctx->ws + P.xls) : nullptr;
-    mp.thin = ctx->stats.thin_batches > 0 ? (const int *)(ctx->ws + P.thin) : nullptr;
-    mp.occ = mp.thin == nullptr && ctx->sparse && P.has_occ && !c.empty ? (const unsigned *)(ctx->ws + P.occ) : nullptr;
+    mp.occ = ctx->sparse && P.has_occ && !c.empty ? (const unsigned *)(ctx->ws + P.occ) : nullptr;
     mp.Aup = i == top ? nullptr : (const float *)(ctx->ws + P.A[(i + 1) & 1]);
     mp.out = i > 0 ? (float *)(ctx->ws + P.A[i & 1]) : (accum ? (float *)(ctx->ws + P.Jpart) : J_out);
     mp.steps = c.empty ? nullptr : (const rc::Step *)(ctx->ws + c.steps_off);
@@ -755,7 +670,7 @@ static int enqueue_solve(rc_ctx *ctx, float *J_out) {
         }
         if (ev) RC_CUDA(ctx, cudaEventRecord(ev[1 + 2 * (top - i)], ctx->stream));
         rc::MarchParams mp = march_params(ctx, i, J_out);
-        if (!c.banded || mp.thin != nullptr) {  // the thin-accurate kernels are not banded
+        if (!c.banded) {
             RC_CUDA(ctx, rc::launch_march(mp, P.LV * P.NM, P.NM, march_variant(ctx, i), ctx->stream));
             launches++;
         } else {
@@ -813,7 +728,7 @@ int rc_solve_J(rc_ctx *ctx, float *J_out) {
     rc_ctx::GraphKey key;
     std::memset(&key, 0, sizeof(key));
     key.J = J_out; key.chi = ctx->chi; key.eta = ctx->eta; key.line = ctx->line; key.ws = ctx->ws;
-    key.nx = P.nx; key.ny = P.ny; key.L = P.L; key.nm = P.NM; key.sparse = ctx->sparse; key.thin = ctx->stats.thin_batches > 0; key.total = P.total;
+    key.nx = P.nx; key.ny = P.ny; key.L = P.L; key.nm = P.NM; key.sparse = ctx->sparse; key.total = P.total;
     for (int m = 0; m < 8; m++) { key.f[m] = ctx->incl_f[m]; key.w[m] = ctx->incl_w[m]; }
     if (!ctx->graph_exec || std::memcmp(&key, &ctx->graph_key, sizeof(key)) != 0) {
         if (ctx->graph_exec) { cudaGraphExecDestroy(ctx->graph_exec); ctx->graph_exec = nullptr; }

@@ -34,7 +34,6 @@ struct MarchParams {
     const float *ST;    // packed source function eta/chi, same layout
     const float *linepk;  // null, or line mode: packed line parameters [s][s][npy][npx][6] (pack_line_kernel)
     const float *xls;     // line mode: [Lpad] wavelengths x_l * sqrt(log2 e), device
-    const int *thin;      // non-null: the solve holds an optically thin wavelength: launch the thin-accurate kernels ([nb] flags, informative)
     const unsigned *occ;  // null (dense), or the occupancy bitmap pack_kernel wrote: empty cells are not gathered
     const float *Aup;   // merged cascade i+1, pre-averaged over the 4 children: [nb][N_i][npy/2][npx/2][LV]; null on the top cascade
     float *out;         // mode 0: A_i [nb][N_i/4][npy][npx][LV]; mode 1: J [ny][nx][L]; mode 2: Jpart [nb][ny][nx]
@@ -105,9 +104,7 @@ cudaError_t launch_table_build(const TableBuildParams &p, cudaStream_t st);
 cudaError_t launch_reduce_jbar(const float *Jpart, float *Jbar, long long ncell, int nb, cudaStream_t st);
 cudaError_t launch_count(const MarchParams &p, unsigned long long *total, cudaStream_t st);
 cudaError_t launch_gather_probe(const float *buf, unsigned long long nsector, int iters, int blocks, float *sink, cudaStream_t st);
-cudaError_t launch_count_empty(const float *chi, long long ncell, int L, int *mark, unsigned long long *count, int *maxchi,
-                               unsigned long long *sumchi, cudaStream_t st);
-cudaError_t launch_line_maxchi(const float *line, const float *xl, long long ncell, int L, int *maxchi, unsigned long long *sumchi, cudaStream_t st);
+cudaError_t launch_count_empty(const float *chi, const float *eta, long long ncell, int L, int *mark, unsigned long long *count, cudaStream_t st);
 cudaError_t launch_alo(const AloParams &p, cudaStream_t st);
 cudaError_t launch_bulk_probe(const float *buf, unsigned long long nsector, int iters, int sms, float *sink, cudaStream_t st, long long *bytes);
 cudaError_t launch_validate(const float *chi, const float *eta, long long n, int *flag, cudaStream_t st);

@@ -253,8 +253,13 @@ __global__ void __launch_bounds__(256) pack_kernel(PackParams p) {
     }
 #pragma unroll
     for (int v = 0; v < LV; v++) {
-        c2[v] = ch[v] * 1.4426950408889634f;            // tau in units of ln 2: T = 2^-tau2
-        S[v] = ch[v] > 0.f ? et[v] / ch[v] : 0.f;        // vacuum cells emit nothing (include/rc.h "Inputs")
+        // Emission without (or with next to no) opacity, reading G11 (eq. 16 in the limit chi -> 0 is eta ds): the march
+        // works with S = eta/chi, so where eta > 0 the opacity is raised to at least 2^-100 max(eta, 1) - S stays finite
+        // (<= 2^100), chi ds stays a normal number, and the optical depth this adds (< 1e-26 per cell for eta < 1e4) is
+        // far below anything fp32 can resolve.  The thin branch of seg_update() then gives exactly eta ds T.
+        const float cf = et[v] > 0.f ? fmaxf(ch[v], 7.888609052210118e-31f * fmaxf(et[v], 1.f)) : ch[v];
+        c2[v] = cf * 1.4426950408889634f;                // tau in units of ln 2: T = 2^-tau2
+        S[v] = et[v] > 0.f ? et[v] / cf : 0.f;
     }
     if (p.occ != nullptr) {
         // occupancy bitmap of the packed cells of this batch (ncell is a multiple of 32 when occ is given, so a
@@ -352,17 +357,80 @@ __device__ __forceinline__ void store_vec_cs(float *p, const float (&v)[LV]) {
     }
 }
 
-// eq. 16 for one cell and one channel.  x = optical depth of the segment in units of ln 2.  Normal form: the
-// emission is S (T_(n-1) - T_n) with T_n = 2^-tau_n from the accumulated tau (absolute error ~1e-7 S).
-// Thin form: for x < 1/32 the same quantity as S T_(n-1) (1 - 2^-x) with 1 - 2^-x = y - y^2/2 + y^3/6, y = x ln 2
-// (relative error < 4e-7), so that emission far below the resolution of T survives.
-__device__ __forceinline__ void thin_update(float chi2, float Sv, float dsv, float &tau, float &T, float &I) {
-    const float x = chi2 * dsv;
-    tau += x;
-    const float Tn = ex2_neg(tau);
-    const float y = x * 0.6931471805599453f;
-    const float w = y * fmaf(y, fmaf(y, 0.16666667f, -0.5f), 1.f);
-    I = fmaf(Sv, x < 0.03125f ? T * w : T - Tn, I);
+// ------------------------------------------------------------------------------------------------
+// eq. 16 for one cell, accurate at every optical depth.  x = chi ds log2 e is the optical depth of
+// the segment in units of ln 2; tau accumulates (one rounding per cell) and T_n = 2^-tau_n.  The cell emits
+// S T_(n-1) (1 - 2^-x), evaluated as
+//   x >= 1/64:  S (T_(n-1) - T_n)              difference of two transmittances, each good to ~1e-7 T: relative error
+//                                              < 2e-5 per cell, and the roundings of T_n cancel between neighbouring cells
+//   x <  1/64:  S (x ln2 / 2) (T_(n-1) + T_n)  trapezoid of the attenuation across the cell: 1 - e^-y = (y/2)(1 + e^-y)
+//                                              (1 - y^2/12 + ...), relative error < 1e-5; exact as chi -> 0 (S x = eta ds
+//                                              log2 e, reading G11) and blind to the resolution of T, so optically thin
+//                                              rays and thin emitters behind absorbers keep their emission
+// One form for every launch: there is no "thin" variant and no host-side detection any more.
+// Channels are processed two at a time with the packed fp32 instructions of sm_100 (FFMA2 / FADD2 / FMUL2).
+// ------------------------------------------------------------------------------------------------
+static constexpr float KAPPA = 0.34657359027997264f;  // ln 2 / 2
+static constexpr float XK_THIN = KAPPA / 64.f;         // threshold on x ln2 / 2
+
+typedef unsigned long long f32x2;  // two floats in one 64-bit register pair (lo, hi)
+__device__ __forceinline__ f32x2 pk2(float lo, float hi) {
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void up2(f32x2 v, float &lo, float &hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {
+    f32x2 r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) {
+    f32x2 r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) {
+    f32x2 r;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) {
+    f32x2 r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+
+// two channels: c = chi log2e, S, ds = path length, dk = ds ln2/2 (pairs); state tau, T, I (pairs)
+__device__ __forceinline__ void seg_update2(f32x2 c, f32x2 S, f32x2 ds, f32x2 dk, f32x2 &tau, f32x2 &T, f32x2 &I) {
+    tau = fma2(c, ds, tau);
+    const f32x2 xk = mul2(c, dk);
+    float t0, t1;
+    up2(tau, t0, t1);
+    const f32x2 Tn = pk2(ex2_neg(t0), ex2_neg(t1));
+    const f32x2 d = sub2(T, Tn), ms = mul2(xk, add2(T, Tn));
+    float x0, x1, d0, d1, m0, m1;
+    up2(xk, x0, x1);
+    up2(d, d0, d1);
+    up2(ms, m0, m1);
+    I = fma2(S, pk2(x0 < XK_THIN ? m0 : d0, x1 < XK_THIN ? m1 : d1), I);
+    T = Tn;
+}
+
+// one channel (single-wavelength launches)
+__device__ __forceinline__ void seg_update1(float c, float S, float ds, float dk, float &tau, float &T, float &I) {
+    tau = fmaf(c, ds, tau);
+    const float xk = c * dk, Tn = ex2_neg(tau);
+    I = fmaf(S, xk < XK_THIN ? xk * (T + Tn) : T - Tn, I);
+    T = Tn;
+}
+
+// line mode: the cell's eta log2e (num) and chi log2e (c) are evaluated per ray; emission eta ds T in the thin branch
+__device__ __forceinline__ void seg_update_line(float c, float num, float ds, float dk, float &tau, float &T, float &I) {
+    const float Sv = c > 0.f ? __fdividef(num, c) : 0.f;  // eta/chi
+    tau = fmaf(c, ds, tau);
+    const float xk = c * dk, Tn = ex2_neg(tau);
+    I += xk < XK_THIN ? (num * dk) * (T + Tn) : Sv * (T - Tn);
     T = Tn;
 }
 
@@ -467,7 +535,7 @@ __device__ __forceinline__ int first_step_reaching(const StepXY *xy, int n, int 
 // half of the directions that crosses the bands in ascending (or descending) order; a ray's (I, tau)
 // is carried from band to band through `state`, so the arithmetic - and the result - is that of the
 // unbanded launch, bit for bit, while the cells gathered by one launch fit L2.
-template <int LV, int NM, int PD, int WARPS, int MINB, bool BANDED, bool SPARSE, bool LINE, bool THIN = false>
+template <int LV, int NM, int PD, int WARPS, int MINB, bool BANDED, bool SPARSE, bool LINE>
 __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) {
     // sum over the 4 child directions, per thread: parked in shared memory between children so the
     // marching loop has the registers to itself
@@ -497,9 +565,6 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
         for (int v = 0; v < LL; v++) xs[v] = __ldg(p.xls + nbI * LL + v);
     }
     const unsigned *occB = SPARSE ? p.occ + (long long)nbI * (ncell >> 5) : nullptr;
-    // THIN: the solve holds an optically thin wavelength (flagged by the host): T = 2^-tau stays within a
-    // few ulp of 1 along whole rays and the differences T_(n-1) - T_n lose the emission; thin_update() keeps it.
-    // A compile-time switch: as a run-time branch it cost the normal path 20 % (registers, scheduling).
     // (dx, dy) ranges that keep this lane's ray inside the box
     const int dxlo = -(a << p.shift) - half, dxhi = ((p.npx - a) << p.shift) - 1 - half;
     const int dylo = -Y0, dyhi = p.ny - 1 - Y0;
@@ -603,8 +668,23 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
                 en_next = __ldg(tab + PD);
                 if (PD < nin && (!BANDED || PD >= n0)) occ_next = __ldg(occB + ((gidx + en_next.x) >> 5));
             }
-            // a1: eq. 16 along the interval, front to back: with tau accumulated,
-            // T_n = 2^-tau2_n and the cell's contribution is S (T_{n-1} - T_n)  [= S T (1 - e^{-chi ds})]
+            // the channels of a lane two at a time (FFMA2 / FADD2 / FMUL2).  Pair q holds, when the lane has at least two
+            // wavelengths, inclination q % NM of wavelengths 2 (q / NM) and 2 (q / NM) + 1 (two neighbouring gathered values,
+            // one path length); with a single wavelength, inclinations 2q and 2q + 1 of it (one gathered value, two lengths)
+            constexpr bool PACKED = !LINE && LV >= 2;
+            constexpr int NP = PACKED ? LV / 2 : 1;
+            [[maybe_unused]] f32x2 I2[NP], tau2[NP], T2[NP];
+            [[maybe_unused]] auto ch_lo = [](int q) { return LL >= 2 ? (2 * (q / NM)) * NM + q % NM : 2 * q; };
+            [[maybe_unused]] auto ch_hi = [](int q) { return LL >= 2 ? (2 * (q / NM) + 1) * NM + q % NM : 2 * q + 1; };
+            if constexpr (PACKED) {
+#pragma unroll
+                for (int q = 0; q < NP; q++) {
+                    I2[q] = pk2(I[ch_lo(q)], I[ch_hi(q)]);
+                    tau2[q] = pk2(tau[ch_lo(q)], tau[ch_hi(q)]);
+                    T2[q] = pk2(T[ch_lo(q)], T[ch_hi(q)]);
+                }
+            }
+            // a1: eq. 16 along the interval, front to back, seg_update*() per cell and channel
             for (int st = 0; st < nw; st += PD) {
 #pragma unroll
                 for (int u = 0; u < PD; u++) {
@@ -622,9 +702,12 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
                     }
                     // integrate step st + u (a slot past the lane's last in-box step has ds = 0: no effect)
                     // 2.5D: inclination m crosses the same cell over ds / sin(inclination)
-                    float dsm[NM];
+                    float dsm[NM], dkm[NM];
 #pragma unroll
-                    for (int m = 0; m < NM; m++) dsm[m] = NM == 1 ? ds[u] : ds[u] * p.incl_f[m];
+                    for (int m = 0; m < NM; m++) {
+                        dsm[m] = NM == 1 ? ds[u] : ds[u] * p.incl_f[m];
+                        dkm[m] = dsm[m] * KAPPA;
+                    }
                     if constexpr (LINE) {
                         // packed cell: chi_c', chi_c' S_c, chi_line', chi_line' S_line, v_x', v_y'   (' = scaled, pack_line_kernel)
                         // inclination m sees the in-plane velocity projected with sin(inclination) (2.5D line mode)
@@ -638,26 +721,25 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
                             const float phi = ex2_neg(aa * aa);
                             const float chi2 = fmaf(c2[u][2], phi, c2[u][0]);
                             const float num = fmaf(c2[u][3], phi, c2[u][1]);
-                            const float Sv = chi2 > 0.f ? __fdividef(num, chi2) : 0.f;  // eta/chi; vacuum emits nothing
-                            if constexpr (THIN) {
-                                thin_update(chi2, Sv, dsm[v % NM], tau[v], T[v], I[v]);
-                            } else {
-                                tau[v] = fmaf(chi2, dsm[v % NM], tau[v]);
-                                const float Tn = ex2_neg(tau[v]);
-                                I[v] = fmaf(Sv, T[v] - Tn, I[v]);
-                                T[v] = Tn;
-                            }
+                            seg_update_line(chi2, num, dsm[v % NM], dkm[v % NM], tau[v], T[v], I[v]);
                         }
-                    } else if constexpr (THIN) {
-#pragma unroll
-                        for (int v = 0; v < LV; v++) thin_update(c2[u][v / NM], S[u][v / NM], dsm[v % NM], tau[v], T[v], I[v]);
                     } else if (!SPARSE || __any_sync(FULL, ds[u] != 0.f)) {  // SPARSE: no lane has an occupied cell: nothing to do
+                        if constexpr (PACKED) {
 #pragma unroll
-                        for (int v = 0; v < LV; v++) {
-                            tau[v] = fmaf(c2[u][v / NM], dsm[v % NM], tau[v]);
-                            const float Tn = ex2_neg(tau[v]);
-                            I[v] = fmaf(S[u][v / NM], T[v] - Tn, I[v]);
-                            T[v] = Tn;
+                            for (int q = 0; q < NP; q++) {
+                                if constexpr (LL >= 2) {
+                                    const int l = 2 * (q / NM), m = q % NM;
+                                    seg_update2(pk2(c2[u][l], c2[u][l + 1]), pk2(S[u][l], S[u][l + 1]), pk2(dsm[m], dsm[m]),
+                                                pk2(dkm[m], dkm[m]), tau2[q], T2[q], I2[q]);
+                                } else {
+                                    seg_update2(pk2(c2[u][0], c2[u][0]), pk2(S[u][0], S[u][0]), pk2(dsm[2 * q], dsm[2 * q + 1]),
+                                                pk2(dkm[2 * q], dkm[2 * q + 1]), tau2[q], T2[q], I2[q]);
+                                }
+                            }
+                        } else {
+#pragma unroll
+                            for (int v = 0; v < LV; v++)
+                                seg_update1(c2[u][v / NM], S[u][v / NM], dsm[v % NM], dkm[v % NM], tau[v], T[v], I[v]);
                         }
                     }
                     // refill the slot with step st + u + PD
@@ -667,11 +749,23 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
                     ds[u] = in ? __uint_as_float(en.y) : 0.f;
                 }
                 if (p.early_exit && (++chk & 3) == 0) {
+                    if constexpr (PACKED) {
+#pragma unroll
+                        for (int q = 0; q < NP; q++) up2(tau2[q], tau[ch_lo(q)], tau[ch_hi(q)]);
+                    }
                     float tmin = tau[0];
 #pragma unroll
                     for (int v = 1; v < LV; v++) tmin = fminf(tmin, tau[v]);
                     // every live lane opaque at every wavelength: T is exactly 0, nothing more can arrive
                     if (__all_sync(FULL, st + PD >= nin || tmin > p.tau_cut)) break;
+                }
+            }
+            if constexpr (PACKED) {
+#pragma unroll
+                for (int q = 0; q < NP; q++) {
+                    up2(I2[q], I[ch_lo(q)], I[ch_hi(q)]);
+                    up2(tau2[q], tau[ch_lo(q)], tau[ch_hi(q)]);
+                    up2(T2[q], T[ch_lo(q)], T[ch_hi(q)]);
                 }
             }
             if constexpr (BANDED) {
@@ -842,39 +936,9 @@ static cudaError_t launch_march_flat(const MarchParams &p, int variant, cudaStre
     }
 }
 
-// Solves that hold an optically thin wavelength (p.thin != null): every mode in one plain variant (ring of 2, 16
-// warps/SM, never banded or sparse) with the thin-accurate update.
-template <int LV, int NM, bool LINE>
-static cudaError_t launch_march_thin(const MarchParams &p, cudaStream_t st) {
-    constexpr int WARPS = 8;
-    const long long blocks = (march_warps(p) + WARPS - 1) / WARPS;
-    if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-    march_kernel<LV, NM, 2, WARPS, 2, false, false, LINE, true><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
-    return cudaGetLastError();
-}
-
-template <bool LINE>
-static cudaError_t launch_march_thin_any(const MarchParams &p, int LV, int NM, cudaStream_t st) {
-    switch (LV * 16 + NM) {
-        case 8 * 16 + 8: return launch_march_thin<8, 8, LINE>(p, st);
-        case 8 * 16 + 4: return launch_march_thin<8, 4, LINE>(p, st);
-        case 8 * 16 + 2: return launch_march_thin<8, 2, LINE>(p, st);
-        case 8 * 16 + 1: return launch_march_thin<8, 1, LINE>(p, st);
-        case 4 * 16 + 4: return launch_march_thin<4, 4, LINE>(p, st);
-        case 4 * 16 + 2: return launch_march_thin<4, 2, LINE>(p, st);
-        case 4 * 16 + 1: return launch_march_thin<4, 1, LINE>(p, st);
-        case 2 * 16 + 2: return launch_march_thin<2, 2, LINE>(p, st);
-        case 2 * 16 + 1: return launch_march_thin<2, 1, LINE>(p, st);
-        case 1 * 16 + 1: return launch_march_thin<1, 1, LINE>(p, st);
-        default: return cudaErrorInvalidValue;
-    }
-}
-
 // LV = channels per lane = (wavelengths per lane) x NM inclinations; the inclined launches come in one
 // variant only
 cudaError_t launch_march(const MarchParams &p, int LV, int NM, int variant, cudaStream_t st) {
-    if (p.thin != nullptr)
-        return p.linepk != nullptr ? launch_march_thin_any<true>(p, LV, NM, st) : launch_march_thin_any<false>(p, LV, NM, st);
     if (NM == 1) {
         switch (LV) {
             case 8: return launch_march_flat<8>(p, variant, st);
@@ -922,87 +986,31 @@ cudaError_t launch_reduce_jbar(const float *Jpart, float *Jbar, long long ncell,
     return cudaGetLastError();
 }
 
-// RC_VALIDATE: flag |= 1 if any chi/eta is negative or non-finite, |= 2 if eta > 0 where chi == 0.
+// RC_VALIDATE: flag |= 1 if any chi/eta is negative or non-finite.
 __global__ void validate_kernel(const float *chi, const float *eta, long long n, int *flag) {
     int bad = 0;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n;
          i += (long long)gridDim.x * blockDim.x) {
         const float c = chi[i], e = eta[i];
         if (!(c >= 0.f) || !(e >= 0.f) || isinf(c) || isinf(e)) bad |= 1;
-        if (c == 0.f && e > 0.f) bad |= 2;
     }
     if (bad) atomicOr(flag, bad);
 }
 
-// Number of cells with chi == 0 at every wavelength (rc_set_atmosphere: is the atmosphere mostly empty?).
+// Number of cells with chi == 0 at every wavelength (is the atmosphere mostly empty?).
 // Pass 1 marks the cells that have a non-zero value (coalesced over the whole array), pass 2 counts the rest.
 template <int W>  // floats per thread: 4 when nlambda is a multiple of 4, else 1
-__global__ void mark_occupied_kernel(const float *chi, long long nchunk, int chunks_per_cell, int *mark, int *maxchi,
-                                     unsigned long long *sumchi, int L) {
-    // also, for every wavelength, the largest chi (non-negative floats order like their bit patterns) and the sum of
-    // chi in fixed point (2^-20; integer adds: the same result whatever the order): block-wide in shared memory,
-    // then one global atomic per wavelength and block
-    extern __shared__ unsigned long long sm[];
-    unsigned long long *sx = sm;
-    int *mx = reinterpret_cast<int *>(sm + L);
-    for (int l = threadIdx.x; l < L; l += blockDim.x) { mx[l] = 0; sx[l] = 0ull; }
-    __syncthreads();
-    auto note = [&](int l, float v) {
-        atomicMax(mx + l, __float_as_int(v));
-        atomicAdd(sx + l, (unsigned long long)(fminf(v, 1e12f) * 1048576.f));
-    };
+__global__ void mark_occupied_kernel(const float *chi, long long nchunk, int chunks_per_cell, int *mark) {
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < nchunk; i += (long long)gridDim.x * blockDim.x) {
         bool nz;
-        const int c = (int)(i % chunks_per_cell);
         if constexpr (W == 4) {
             const float4 v = __ldg(reinterpret_cast<const float4 *>(chi) + i);
             nz = v.x != 0.f || v.y != 0.f || v.z != 0.f || v.w != 0.f;
-            if (maxchi && nz) { note(4 * c, v.x); note(4 * c + 1, v.y); note(4 * c + 2, v.z); note(4 * c + 3, v.w); }
         } else {
-            const float v = __ldg(chi + i);
-            nz = v != 0.f;
-            if (maxchi && nz) note(c, v);
+            nz = __ldg(chi + i) != 0.f;
         }
         if (nz) mark[i / chunks_per_cell] = 1;
     }
-    __syncthreads();
-    if (maxchi)
-        for (int l = threadIdx.x; l < L; l += blockDim.x)
-            if (mx[l] != 0) { atomicMax(maxchi + l, mx[l]); atomicAdd(sumchi + l, sx[l]); }
-}
-
-// Line mode: upper bound over directions of the opacity of every wavelength, chi_c + chi_line phi(max(0, |x_l| - |v|)).
-__global__ void line_maxchi_kernel(const float *line, const float *xl, long long ncell, int L, int *maxchi, unsigned long long *sumchi) {
-    extern __shared__ unsigned long long sm[];
-    unsigned long long *sx = sm;
-    int *mx = reinterpret_cast<int *>(sm + L);
-    for (int l = threadIdx.x; l < L; l += blockDim.x) { mx[l] = 0; sx[l] = 0ull; }
-    __syncthreads();
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < ncell * L; i += (long long)gridDim.x * blockDim.x) {
-        const long long cell = i / L;
-        const int l = (int)(i - cell * L);
-        const float *q = line + cell * 6;
-        const float v = sqrtf(q[4] * q[4] + q[5] * q[5]);
-        const float a = fmaxf(fabsf(__ldg(xl + l)) - v, 0.f);
-        const float c = fmaf(q[2], expf(-a * a) * 0.5641895835477563f, q[0]);
-        if (c > 0.f) {
-            atomicMax(mx + l, __float_as_int(c));
-            atomicAdd(sx + l, (unsigned long long)(fminf(c, 1e12f) * 1048576.f));
-        }
-    }
-    __syncthreads();
-    for (int l = threadIdx.x; l < L; l += blockDim.x)
-        if (mx[l] != 0) { atomicMax(maxchi + l, mx[l]); atomicAdd(sumchi + l, sx[l]); }
-}
-
-// maxchi: [L] ints (float bit patterns) followed, 8-byte aligned, by sumchi: [L] unsigned long long (see rc_api.cu)
-cudaError_t launch_line_maxchi(const float *line, const float *xl, long long ncell, int L, int *maxchi, unsigned long long *sumchi, cudaStream_t st) {
-    cudaError_t e = cudaMemsetAsync(maxchi, 0, sizeof(int) * (size_t)L, st);
-    if (e != cudaSuccess) return e;
-    e = cudaMemsetAsync(sumchi, 0, sizeof(unsigned long long) * (size_t)L, st);
-    if (e != cudaSuccess) return e;
-    line_maxchi_kernel<<<148 * 8, 256, 12 * (size_t)L, st>>>(line, xl, ncell, L, maxchi, sumchi);
-    return cudaGetLastError();
 }
 
 __global__ void count_unmarked_kernel(const int *mark, long long ncell, unsigned long long *count) {
@@ -1013,22 +1021,17 @@ __global__ void count_unmarked_kernel(const int *mark, long long ncell, unsigned
     if ((threadIdx.x & 31) == 0 && mine) atomicAdd(count, mine);
 }
 
-// mark: scratch of ncell ints (device); count: zeroed by the caller; maxchi: null or [L] ints (float bit patterns)
-cudaError_t launch_count_empty(const float *chi, long long ncell, int L, int *mark, unsigned long long *count, int *maxchi,
-                               unsigned long long *sumchi, cudaStream_t st) {
+// mark: scratch of ncell ints (device); count: zeroed by the caller
+cudaError_t launch_count_empty(const float *chi, const float *eta, long long ncell, int L, int *mark, unsigned long long *count, cudaStream_t st) {
     cudaError_t e = cudaMemsetAsync(mark, 0, sizeof(int) * (size_t)ncell, st);
     if (e != cudaSuccess) return e;
-    if (maxchi) {
-        e = cudaMemsetAsync(maxchi, 0, sizeof(int) * (size_t)L, st);
-        if (e != cudaSuccess) return e;
-        e = cudaMemsetAsync(sumchi, 0, sizeof(unsigned long long) * (size_t)L, st);
-        if (e != cudaSuccess) return e;
+    // a cell is empty when chi and eta vanish at every wavelength (emission without opacity counts, reading G11)
+    for (const float *f : {chi, eta}) {
+        if (L % 4 == 0 && (reinterpret_cast<uintptr_t>(f) & 15) == 0)
+            mark_occupied_kernel<4><<<148 * 16, 256, 0, st>>>(f, ncell * (L / 4), L / 4, mark);
+        else
+            mark_occupied_kernel<1><<<148 * 16, 256, 0, st>>>(f, ncell * L, L, mark);
     }
-    const size_t sm = 12 * (size_t)L;
-    if (L % 4 == 0 && (reinterpret_cast<uintptr_t>(chi) & 15) == 0)
-        mark_occupied_kernel<4><<<148 * 16, 256, sm, st>>>(chi, ncell * (L / 4), L / 4, mark, maxchi, sumchi, L);
-    else
-        mark_occupied_kernel<1><<<148 * 16, 256, sm, st>>>(chi, ncell * L, L, mark, maxchi, sumchi, L);
     count_unmarked_kernel<<<148 * 4, 256, 0, st>>>(mark, ncell, count);
     return cudaGetLastError();
 }

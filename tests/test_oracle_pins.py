@@ -654,6 +654,125 @@ def test_A1_alo_is_the_own_cell_transmittance_of_cascade_0(oracle):
     assert np.allclose(oracle.alo(line=a.line, xl=a.xl), np.exp(-c * np.sqrt(0.5)), rtol=1e-12)
 
 
+def _checkerboard(rng, n=16):
+    y, x = np.mgrid[0:n, 0:n]
+    occ = (x % 2 == 0) & (y % 2 == 0)           # diagonal neighbours of an occupied cell are (odd, odd): empty
+    return occ
+
+
+def test_A2_inclined_alo_is_the_inclined_cascade_0_transmittance(oracle):
+    """eq. 17 with the 2.5D rays of PAPER.md:281: for EVERY inclination separately, the ALO of that inclination alone
+    (mu = [mu_m], weight 1) equals the cascade-0 transmittances of the oracle's own inclined march (path_scale =
+    1/sin(inclination), dump_T, all four directions) on the checkerboard atmosphere, where the diagonal neighbour of
+    an occupied cell is vacuum; and the quadrature is the weighted sum of those.  Fails if the path from the cell
+    centre to its edge is scaled by anything but 1/sin(inclination)."""
+    rng = np.random.default_rng(31)
+    occ = _checkerboard(rng)
+    chi = np.where(occ[..., None], rng.uniform(0.1, 3.0, occ.shape + (3,)), 0.0).astype(np.float32)
+    mu, w = A.gauss_radau(8)
+    total = 0.0
+    for m in range(1, 8):                        # mu[0] = 0 is the flatland ray of A1
+        ps = 1.0 / np.sqrt(1.0 - mu[m] ** 2)
+        d = oracle.solve(chi, chi.copy(), 2, dump_cascade=0, path_scale=ps)
+        lam = oracle.alo(chi=chi, mu=[mu[m]], w_mu=[1.0])
+        for k in range(4):
+            assert np.allclose(d["dump_T"][:, :, k, :][occ], lam[occ], rtol=1e-13), (m, k)
+        assert np.max(np.abs(lam[occ] / oracle.alo(chi=chi)[occ] - 1)) > 1e-3 * m   # and it is not the flatland value
+        total = total + w[m] * d["dump_T"][:, :, 0, :]
+    total = total + w[0] * oracle.solve(chi, chi.copy(), 2, dump_cascade=0)["dump_T"][:, :, 0, :]
+    assert np.allclose(oracle.alo(chi=chi, mu=mu, w_mu=w)[occ], total[occ], rtol=1e-13)
+
+
+@pytest.mark.parametrize("mu_m", [0.0, 0.6, 0.95])
+def test_A3_moving_line_alo_is_the_directional_cascade_0_transmittance(oracle, mu_m):
+    """eq. 17 in the line mode with v != 0 ("the monochromatic, directional ALO"): the opacity a
+    cascade-0 ray sees depends on its direction through the projected velocity, and for an inclined ray on
+    sin(inclination) too (path / sin, in-plane velocity x sin).  On the checkerboard atmosphere the mean over the four
+    directions of the oracle's own line-mode cascade-0 transmittances (dump_T of the march, rc_oracle.c) is the ALO.
+    Fails if the velocity projection or the path scale of the restated formula is wrong."""
+    rng = np.random.default_rng(32)
+    occ = _checkerboard(rng)
+    n = occ.shape[0]
+    line = np.zeros((n, n, 6), np.float32)
+    line[..., 0] = np.where(occ, rng.uniform(0.01, 0.3, occ.shape), 0.0)
+    line[..., 1] = 1.0
+    line[..., 2] = np.where(occ, rng.uniform(0.5, 5.0, occ.shape), 0.0)
+    line[..., 3] = 2.0
+    line[..., 4] = rng.uniform(-2.0, 2.0, occ.shape)        # v_x, v_y != 0: the four diagonals see four different opacities
+    line[..., 5] = rng.uniform(-2.0, 2.0, occ.shape)
+    xl = np.array([-1.5, -0.3, 0.0, 0.8, 2.0])
+    ps = 1.0 / np.sqrt(1.0 - mu_m ** 2)
+    d = oracle.line_intervals(line, xl, 2, 0, path_scale=ps)
+    T = d["dump_T"]                                          # [ny][nx][4][L]
+    lam = oracle.alo(line=line, xl=xl, mu=[mu_m], w_mu=[1.0])
+    assert np.allclose(T.mean(axis=2)[occ], lam[occ], rtol=1e-13)
+    spread = T[occ].max(axis=1) / T[occ].min(axis=1)
+    assert np.median(spread) > 1.05                          # the direction dependence is really there
+    if mu_m > 0:                                             # and so is the dependence on the inclination beyond the path scale
+        flat = oracle.alo(line=line, xl=xl)
+        assert np.max(np.abs(np.log(lam[occ]) / (np.log(flat[occ]) * ps) - 1)) > 1e-2
+
+
+def test_A4_plain_bilinear_weights_against_independent_two_cascade_reference(oracle):
+    """The non-fix twin of F2 ("the sample for each interval is bilinearly interpolated from the four
+    closest probes of cascade i+1", 241 clamp): an independent two-cascade brute force on 8 x 6 cells with the
+    sorting-based ray/cell intersection of tests/refs.py, the interpolation weights written from the GEOMETRIC position
+    of the cascade-0 probe among the cascade-1 probes - child centre x + 1/2, parents at 2 (q + 1/2): u = x/2 - 1/4 in
+    parent index units, lower parent floor(u), weight of the upper parent u - floor(u) - and the indices clamped to the
+    lattice.  Swapping 3/4 and 1/4 in the oracle fails this exactly."""
+    nx, ny = 8, 6
+    rng = np.random.default_rng(14)
+    chi = rng.uniform(0.05, 1.5, (ny, nx, 1)).astype(np.float32)
+    eta = (chi * rng.uniform(0.2, 2.0, (ny, nx, 1))).astype(np.float32)
+    Ib, Ia = 0.4, 0.1
+    J = oracle.solve(chi, eta, 2, I_below=[Ib], I_above=[Ia])["J"][..., 0]
+    c, e = chi[..., 0].astype(np.float64).ravel(), eta[..., 0].astype(np.float64).ravel()
+    t1 = 1.0
+    M1 = np.zeros((ny // 2, nx // 2, 16))
+    for b in range(ny // 2):
+        for a_ in range(nx // 2):
+            for k in range(16):
+                th = 2 * np.pi * (k + 0.5) / 16
+                cells, ds = refs.segments_by_sorting(nx, ny, (a_ + 0.5) * 2, (b + 0.5) * 2, th, t1, 1e9)
+                I, T = refs.integrate(c, e, cells, ds)
+                M1[b, a_, k] = I + T * (Ib if np.sin(th) < 0 else Ia)
+
+    def interp(a_, n):
+        u = (a_ + 0.5) / 2.0 - 0.5                          # position among the parents, in parent index units
+        lo = int(np.floor(u))
+        f = u - lo
+        cl = lambda q: min(max(q, 0), n - 1)
+        return (cl(lo), 1.0 - f), (cl(lo + 1), f)
+
+    want = np.zeros((ny, nx))
+    for y in range(ny):
+        for x in range(nx):
+            for k in range(4):
+                th = 2 * np.pi * (k + 0.5) / 4
+                cells, ds = refs.segments_by_sorting(nx, ny, x + 0.5, y + 0.5, th, 0.0, t1)
+                I, T = refs.integrate(c, e, cells, ds)
+                U = 0.0
+                for (bq, wb) in interp(y, ny // 2):
+                    for (aq, wa) in interp(x, nx // 2):
+                        U += wa * wb * M1[bq, aq, 4 * k:4 * k + 4].mean()
+                want[y, x] += 0.25 * (I + T * U)
+    assert np.allclose(J, want, rtol=1e-10)
+    # the weights matter at this precision: the swapped pair (1/4 to the nearer parent) is off by far more
+    def swapped(a_, n):
+        (q0, w0), (q1, w1) = interp(a_, n)
+        return (q0, w1), (q1, w0)
+    wrong = np.zeros((ny, nx))
+    for y in range(ny):
+        for x in range(nx):
+            for k in range(4):
+                th = 2 * np.pi * (k + 0.5) / 4
+                cells, ds = refs.segments_by_sorting(nx, ny, x + 0.5, y + 0.5, th, 0.0, t1)
+                I, T = refs.integrate(c, e, cells, ds)
+                U = sum(wa * wb * M1[bq, aq, 4 * k:4 * k + 4].mean() for (bq, wb) in swapped(y, ny // 2) for (aq, wa) in swapped(x, nx // 2))
+                wrong[y, x] += 0.25 * (I + T * U)
+    assert np.max(np.abs(wrong / J - 1)) > 1e-3
+
+
 def test_I4_boundary_per_inclination(oracle):
     """A boundary intensity table over inclination: in an empty domain every constructed ray returns
     its own boundary value, so J_l = sum_m w_m (I_below[m][l] + I_above[m][l]) / 2; a table with equal rows is the
