@@ -25,6 +25,11 @@
  *                      different inclinations to the invariant axis: same cells, path length
  *                      ds / sin(inclination); J = sum_m w_m J_m
  *                      (rc_oracle_solve_scaled does one inclination; oracle/rc_oracle.py sums)
+ *   sparsity  "we can first determine the cells of interest ... This flag then defines the
+ *                      probes of cascade 0 that may be involved ... Their bilinear "parents" are recursively
+ *                      flagged up to the maximum cascade, and the radiance intervals are only computed for these
+ *                      flagged probes, and non-flagged cells are treated as transparent with no emission"
+ *                                                                         PAPER.md:380 (rc_oracle_solve_active)
  *
  * Readings where the paper is silent or garbled are DESIGN.md §3 (G1..G19 of SURVEY.md §8(c)).
  * The only loop restructuring relative to SURVEY.md's listing: the wavelength loop is innermost
@@ -67,6 +72,8 @@ typedef struct {
     double vel_scale;   /* 2.5D line mode: an inclined ray with direction cosine mu to the invariant axis has the
                            in-plane direction sqrt(1-mu^2) (wx, wy); velocities are in the plane, so v.n is scaled by
                            sqrt(1-mu^2) = 1/path_scale.  1 in flatland. */
+    const unsigned char *active; /* [ny][nx] or NULL: cells of interest; a cell that is not flagged
+                                    is "treated as transparent with no emission" whatever chi, eta hold there */
 } grid_t;
 
 /* Opacity and emissivity of cell `cell` at wavelength l for the photons that travel along a ray traced
@@ -75,6 +82,7 @@ typedef struct {
  *     a = x_l - v.n ,  phi = exp(-a^2)/sqrt(pi) ,
  *     chi = chi_c + chi_line phi ,  eta = chi_c S_c + chi_line S_line phi . */
 static void cell_chi_eta(const grid_t *g, int cell, int l, double wx, double wy, double *chi, double *eta) {
+    if (g->active && !g->active[cell]) { *chi = 0.0; *eta = 0.0; return; }
     if (!g->line) {
         size_t c = (size_t)cell * g->L + l;
         *chi = (double)g->chi[c];
@@ -230,7 +238,7 @@ int rc_oracle_ray_segments(int nx, int ny, double px, double py, double theta, i
 int rc_oracle_interval(const float *chi, const float *eta, int nx, int ny, int L, double px,
                        double py, double theta, int diag_q, double ta, double tb, int order,
                        double *I, double *T) {
-    grid_t g = {nx, ny, L, chi, eta, 1.0, NULL, NULL, 1.0};
+    grid_t g = {nx, ny, L, chi, eta, 1.0, NULL, NULL, 1.0, NULL};
     seg_t *seg = (seg_t *)malloc(sizeof(seg_t) * (size_t)(nx + ny + 4));
     int n = diag_q >= 0 ? diag_segments(nx, ny, (int)floor(px), (int)floor(py), diag_q, ta, tb, seg)
                         : dda_segments(nx, ny, px, py, cos(theta), sin(theta), ta, tb, seg);
@@ -272,13 +280,14 @@ static int solve_impl(const float *chi, const float *eta, const float *line, con
                            double c0, const float *I_below, const float *I_above, const float *w,
                            int x0, int x1, int y0, int y1, double *J_out, double *Jbar_out, int nthreads,
                            int order, int dump_cascade, double *dump_I, double *dump_T, double *dump_M,
-                           int *dump_win, rc_oracle_counts *counts, double path_scale) {
+                           int *dump_win, rc_oracle_counts *counts, double path_scale,
+                           const unsigned char *active) {
     if (!((chi && eta) || (line && xl)) || !J_out || nx <= 0 || ny <= 0 || L <= 0 || ncasc < 1 || ncasc > 15)
         return -1;
     int top = ncasc - 1;
     if (nx % (1 << top) || ny % (1 << top)) return -1; /* reading G19 */
     if (x0 < 0 || y0 < 0 || x1 > nx || y1 > ny || x0 >= x1 || y0 >= y1) return -1;
-    grid_t g = {nx, ny, L, chi, eta, path_scale, line, xl, 1.0 / path_scale};
+    grid_t g = {nx, ny, L, chi, eta, path_scale, line, xl, 1.0 / path_scale, active};
     const int fix = (order & 2) != 0; /* order: bit 0 = back-to-front (G13), bit 1 = bilinear fix */
     if (counts) memset(counts, 0, sizeof(*counts));
 #ifdef _OPENMP
@@ -294,6 +303,31 @@ static int solve_impl(const float *chi, const float *eta, const float *line, con
         parent_axis(by0[i], npy, &q0, &q1, &fr); by0[i + 1] = q0;
         parent_axis(by1[i], npy, &q0, &q1, &fr); by1[i + 1] = q1;
     }
+    /* Sparsity: flag[0] = the cells of interest = the cascade-0 probes that may be involved; the
+     * bilinear parents of every flagged probe of cascade i are flagged in cascade i+1, up to the top.  Intervals are
+     * computed for flagged probes only; everything else in a cascade's storage stays NaN, so a read of a value
+     * that was never computed would poison J (the pins check it never happens).  active == NULL: all flagged. */
+    unsigned char *flag[16];
+    for (int i = 0; i <= top; i++) flag[i] = NULL;
+    if (active) {
+        for (int i = 0; i <= top; i++) {
+            flag[i] = (unsigned char *)calloc((size_t)(nx >> i) * (ny >> i), 1);
+            if (!flag[i]) { for (int j = 0; j < i; j++) free(flag[j]); return -2; }
+        }
+        for (size_t c = 0; c < (size_t)nx * ny; c++) flag[0][c] = active[c] != 0;
+        for (int i = 0; i < top; i++) {
+            int npx = nx >> i, npy = ny >> i, upx = npx / 2, upy = npy / 2;
+            for (int b = 0; b < npy; b++)
+                for (int a = 0; a < npx; a++) {
+                    if (!flag[i][(size_t)b * npx + a]) continue;
+                    int a0, a1, b0, b1; double fr;
+                    parent_axis(a, upx, &a0, &a1, &fr);
+                    parent_axis(b, upy, &b0, &b1, &fr);
+                    flag[i + 1][(size_t)b0 * upx + a0] = 1; flag[i + 1][(size_t)b0 * upx + a1] = 1;
+                    flag[i + 1][(size_t)b1 * upx + a0] = 1; flag[i + 1][(size_t)b1 * upx + a1] = 1;
+                }
+        }
+    }
     double *Mup = NULL; /* merged cascade i+1: [wy][wx][N_{i+1}][L] */
     int upx0 = 0, upy0 = 0, upwx = 0;
     long upN = 0;
@@ -306,6 +340,10 @@ static int solve_impl(const float *chi, const float *eta, const float *line, con
         int wx = ax1[i] - ax0[i] + 1, wy = by1[i] - by0[i] + 1;
         double *M = (double *)malloc(sizeof(double) * (size_t)wx * wy * N * L);
         if (!M) { status = -2; break; }
+        if (active) for (size_t q = 0; q < (size_t)wx * wy * N * L; q++) M[q] = NAN;
+        int64_t nflagged = 0;
+        for (int b = by0[i]; b <= by1[i]; b++)
+            for (int a = ax0[i]; a <= ax1[i]; a++) nflagged += !active || flag[i][(size_t)b * npx + a];
         int dump = i == dump_cascade;
         if (dump && dump_win) { dump_win[0] = ax0[i]; dump_win[1] = ax1[i]; dump_win[2] = by0[i]; dump_win[3] = by1[i]; }
         int64_t nseg_total = 0;
@@ -318,6 +356,7 @@ static int solve_impl(const float *chi, const float *eta, const float *line, con
             for (int b = by0[i]; b <= by1[i]; b++) {
                 for (int a = ax0[i]; a <= ax1[i]; a++) {
                     for (long k = 0; k < N; k++) {
+                        if (active && !flag[i][(size_t)b * npx + a]) continue; /* not flagged: not computed */
                         double px = (a + 0.5) * s, py = (b + 0.5) * s; /* PAPER.md:312, reading G5 */
                         double theta = 2.0 * M_PI * (k + 0.5) / (double)N; /* reading G4 */
                         size_t o = ((((size_t)(b - by0[i])) * wx + (a - ax0[i])) * N + k) * L;
@@ -392,7 +431,7 @@ static int solve_impl(const float *chi, const float *eta, const float *line, con
             }
             free(seg); free(I); free(T);
         }
-        if (counts) { counts->intervals[i] = (int64_t)wx * wy * N; counts->segments[i] = nseg_total; }
+        if (counts) { counts->intervals[i] = nflagged * N; counts->segments[i] = nseg_total; }
         free(Mup);
         Mup = M; upx0 = ax0[i]; upy0 = by0[i]; upwx = wx; upN = N;
     }
@@ -402,9 +441,11 @@ static int solve_impl(const float *chi, const float *eta, const float *line, con
         for (int y = 0; y < wy; y++)
             for (int x = 0; x < wx; x++) {
                 double jb = 0.0;
+                int on = !active || active[(size_t)(y0 + y) * nx + (x0 + x)];
                 for (int l = 0; l < L; l++) {
                     const double *m = Mup + (((size_t)y * wx + x) * 4) * L + l;
-                    double J = (m[0] + m[(size_t)L] + m[2 * (size_t)L] + m[3 * (size_t)L]) / 4.0;
+                    /* J is defined on the cells of interest; elsewhere it is not computed: 0 */
+                    double J = on ? (m[0] + m[(size_t)L] + m[2 * (size_t)L] + m[3 * (size_t)L]) / 4.0 : 0.0;
                     J_out[((size_t)y * wx + x) * L + l] = J;
                     jb += (w ? (double)w[l] : 1.0) * J;
                 }
@@ -412,6 +453,7 @@ static int solve_impl(const float *chi, const float *eta, const float *line, con
             }
     }
     free(Mup);
+    for (int i = 0; i <= top; i++) free(flag[i]);
     return status;
 }
 
@@ -421,7 +463,17 @@ int rc_oracle_solve_scaled(const float *chi, const float *eta, int nx, int ny, i
                            int order, int dump_cascade, double *dump_I, double *dump_T, double *dump_M,
                            int *dump_win, rc_oracle_counts *counts, double path_scale) {
     return solve_impl(chi, eta, NULL, NULL, nx, ny, L, ncasc, c0, I_below, I_above, w, x0, x1, y0, y1, J_out,
-                      Jbar_out, nthreads, order, dump_cascade, dump_I, dump_T, dump_M, dump_win, counts, path_scale);
+                      Jbar_out, nthreads, order, dump_cascade, dump_I, dump_T, dump_M, dump_win, counts, path_scale, NULL);
+}
+
+/* Sparse solve: `active` [ny][nx] flags the cells of interest (non-zero = flagged).  Either mode:
+ * chi, eta or line, xl (the other pair NULL). */
+int rc_oracle_solve_active(const float *chi, const float *eta, const float *line, const double *xl, int nx, int ny,
+                           int L, int ncasc, double c0, const float *I_below, const float *I_above, const float *w,
+                           int x0, int x1, int y0, int y1, double *J_out, double *Jbar_out, int nthreads, int order,
+                           rc_oracle_counts *counts, double path_scale, const unsigned char *active) {
+    return solve_impl(chi, eta, line, xl, nx, ny, L, ncasc, c0, I_below, I_above, w, x0, x1, y0, y1, J_out, Jbar_out,
+                      nthreads, order, -1, NULL, NULL, NULL, NULL, counts, path_scale, active);
 }
 
 /* Velocity-dependent line mode: line [ny][nx][6] and xl [L] instead of chi, eta (cell_chi_eta above). */
@@ -430,7 +482,7 @@ int rc_oracle_solve_line(const float *line, const double *xl, int nx, int ny, in
                          int y1, double *J_out, double *Jbar_out, int nthreads, int order,
                          rc_oracle_counts *counts, double path_scale) {
     return solve_impl(NULL, NULL, line, xl, nx, ny, L, ncasc, c0, I_below, I_above, w, x0, x1, y0, y1, J_out,
-                      Jbar_out, nthreads, order, -1, NULL, NULL, NULL, NULL, counts, path_scale);
+                      Jbar_out, nthreads, order, -1, NULL, NULL, NULL, NULL, counts, path_scale, NULL);
 }
 
 /* The same, also writing one cascade's intervals before and after merging (as rc_oracle_solve does): an output
@@ -440,7 +492,7 @@ int rc_oracle_solve_line_dump(const float *line, const double *xl, int nx, int n
                               double *Jbar_out, int nthreads, int order, int dump_cascade, double *dump_I,
                               double *dump_T, double *dump_M, int *dump_win, double path_scale) {
     return solve_impl(NULL, NULL, line, xl, nx, ny, L, ncasc, c0, I_below, I_above, w, 0, nx, 0, ny, J_out,
-                      Jbar_out, nthreads, order, dump_cascade, dump_I, dump_T, dump_M, dump_win, NULL, path_scale);
+                      Jbar_out, nthreads, order, dump_cascade, dump_I, dump_T, dump_M, dump_win, NULL, path_scale, NULL);
 }
 
 /* Flatland (path_scale = 1): the solve of SURVEY.md §8(c). */

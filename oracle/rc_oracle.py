@@ -57,6 +57,10 @@ def lib():
         _lib.rc_oracle_solve_line.argtypes = ([C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double,
                                                C.c_void_p, C.c_void_p, C.c_void_p] + [C.c_int] * 4 +
                                               [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_double])
+        _lib.rc_oracle_solve_active.restype = C.c_int
+        _lib.rc_oracle_solve_active.argtypes = ([C.c_void_p] * 4 + [C.c_int, C.c_int, C.c_int, C.c_int, C.c_double,
+                                                 C.c_void_p, C.c_void_p, C.c_void_p] + [C.c_int] * 4 +
+                                                [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_double, C.c_void_p])
         _lib.rc_oracle_solve_line_dump.restype = C.c_int
         _lib.rc_oracle_solve_line_dump.argtypes = ([C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double,
                                                     C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int,
@@ -101,8 +105,14 @@ def merge(I_near, tau_near, I_far, tau_far):
     return a.value, b.value
 
 
+def _active_u8(active, ny, nx):
+    a = np.ascontiguousarray(np.asarray(active) != 0, dtype=np.uint8)
+    assert a.shape == (ny, nx), f"active mask must be [ny][nx] = {(ny, nx)}, got {a.shape}"
+    return a
+
+
 def solve(chi, eta, ncascades, c0=1.0, I_below=None, I_above=None, weights=None, window=None,
-          nthreads=0, order=0, dump_cascade=-1, want_counts=False, path_scale=1.0, bilinear_fix=False):
+          nthreads=0, order=0, dump_cascade=-1, want_counts=False, path_scale=1.0, bilinear_fix=False, active=None):
     """J [wy][wx][L] (float64) for the cascade-0 cell window (x0, x1, y0, y1) (default: whole grid).
 
     Returns a dict: J, Jbar, and if asked counts / dump_{I,T,M,win} of one cascade."""
@@ -126,6 +136,20 @@ def solve(chi, eta, ncascades, c0=1.0, I_below=None, I_above=None, weights=None,
         dI, dT, dM = np.zeros(shape), np.zeros(shape), np.zeros(shape)
         assert window is None, "dump only with the full window (dense layout)"
     order = int(order) | (2 if bilinear_fix else 0)  # bit 1: the bilinear fix
+    if active is not None:
+        # sparse solve: intervals only for the flagged probes, non-flagged cells transparent
+        assert dump_cascade < 0
+        act = _active_u8(active, ny, nx)
+        rc = lib().rc_oracle_solve_active(_ptr(chi), _ptr(eta), None, None, nx, ny, L, ncascades, c0, _ptr(Ib), _ptr(Ia),
+                                          _ptr(w), x0, x1, y0, y1, _ptr(J), _ptr(Jbar), nthreads, order, C.byref(cnt),
+                                          float(path_scale), _ptr(act))
+        if rc != 0:
+            raise ValueError(f"rc_oracle_solve_active failed: {rc}")
+        out = {"J": J, "Jbar": Jbar}
+        if want_counts:
+            out["intervals"] = np.array(cnt.intervals[:ncascades])
+            out["segments"] = np.array(cnt.segments[:ncascades])
+        return out
     rc = lib().rc_oracle_solve_scaled(_ptr(chi), _ptr(eta), nx, ny, L, ncascades, c0, _ptr(Ib), _ptr(Ia),
                                       _ptr(w), x0, x1, y0, y1, _ptr(J), _ptr(Jbar), nthreads, order,
                                       dump_cascade, _ptr(dI), _ptr(dT), _ptr(dM), _ptr(win), C.byref(cnt),
@@ -171,7 +195,7 @@ def solve_inclined(chi, eta, ncascades, mu, w_mu, **kw):
 
 
 def solve_line(line, xl, ncascades, c0=1.0, I_below=None, I_above=None, weights=None, window=None,
-               nthreads=0, order=0, want_counts=False, mu=None, w_mu=None, path_scale=1.0, bilinear_fix=False):
+               nthreads=0, order=0, want_counts=False, mu=None, w_mu=None, path_scale=1.0, bilinear_fix=False, active=None):
     """Velocity-dependent line mode: per cell chi_c, S_c, chi_line, S_line,
     v_x, v_y; opacity and emissivity are evaluated per ray from the projected velocity (rc_oracle.c,
     cell_chi_eta).  line: float32 [ny][nx][6]; xl: [L] Doppler-width offsets.  Returns J, Jbar like solve()."""
@@ -183,7 +207,7 @@ def solve_line(line, xl, ncascades, c0=1.0, I_below=None, I_above=None, weights=
             bm = None if I_below is None else (np.asarray(I_below)[m] if np.ndim(I_below) == 2 else I_below)
             am = None if I_above is None else (np.asarray(I_above)[m] if np.ndim(I_above) == 2 else I_above)
             o = solve_line(line, xl, ncascades, c0, bm, am, weights, window, nthreads, order, want_counts,
-                           path_scale=1.0 / np.sqrt(1.0 - float(mu[m]) ** 2), bilinear_fix=bilinear_fix)
+                           path_scale=1.0 / np.sqrt(1.0 - float(mu[m]) ** 2), bilinear_fix=bilinear_fix, active=active)
             if out is None:
                 out = dict(o)
                 out["J"] = w_mu[m] * o["J"]
@@ -205,9 +229,15 @@ def solve_line(line, xl, ncascades, c0=1.0, I_below=None, I_above=None, weights=
     w = None if weights is None else _f32(weights)
     cnt = Counts()
     order = int(order) | (2 if bilinear_fix else 0)
-    rc = lib().rc_oracle_solve_line(_ptr(line), _ptr(xl), nx, ny, L, ncascades, c0, _ptr(Ib), _ptr(Ia), _ptr(w),
-                                    x0, x1, y0, y1, _ptr(J), _ptr(Jbar), nthreads, order, C.byref(cnt),
-                                    float(path_scale))
+    if active is not None:
+        act = _active_u8(active, ny, nx)
+        rc = lib().rc_oracle_solve_active(None, None, _ptr(line), _ptr(xl), nx, ny, L, ncascades, c0, _ptr(Ib), _ptr(Ia),
+                                          _ptr(w), x0, x1, y0, y1, _ptr(J), _ptr(Jbar), nthreads, order, C.byref(cnt),
+                                          float(path_scale), _ptr(act))
+    else:
+        rc = lib().rc_oracle_solve_line(_ptr(line), _ptr(xl), nx, ny, L, ncascades, c0, _ptr(Ib), _ptr(Ia), _ptr(w),
+                                        x0, x1, y0, y1, _ptr(J), _ptr(Jbar), nthreads, order, C.byref(cnt),
+                                        float(path_scale))
     if rc != 0:
         raise ValueError(f"rc_oracle_solve_line failed: {rc}")
     out = {"J": J, "Jbar": Jbar}
@@ -267,6 +297,8 @@ def solve_atmosphere(atm, **kw):
     """Convenience: oracle solve of a paper_2408_14425_b200.atmospheres.Atmosphere-like object."""
     if getattr(atm, "bilinear_fix", False):
         kw.setdefault("bilinear_fix", True)
+    if getattr(atm, "active", None) is not None:
+        kw.setdefault("active", atm.active)
     if getattr(atm, "line", None) is not None:
         return solve_line(atm.line, atm.xl, atm.ncascades, c0=atm.c0_interval, I_below=atm.I_below,
                           I_above=atm.I_above, weights=atm.weights, mu=getattr(atm, "mu", None),

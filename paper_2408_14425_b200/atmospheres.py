@@ -45,6 +45,9 @@ class Atmosphere:
     line: np.ndarray | None = None  # float32 [ny][nx][6]: chi_c, S_c, chi_line, S_line, v_x, v_y (Doppler widths)
     xl: np.ndarray | None = None    # float64 [nlambda] offsets from line centre in Doppler widths
     bilinear_fix: bool = False      # solve with the bilinear fix
+    # sparsity: uint8 [ny][nx], non-zero = cell of interest; None = every cell.  J is computed on the
+    # flagged cells only (0 elsewhere) and the other cells are treated as transparent with no emission
+    active: np.ndarray | None = None
 
 
 # (nx, ny, nlambda, ncascades) of BASELINE.json's configs
@@ -314,6 +317,29 @@ def with_inclinations(atm: Atmosphere, n: int) -> Atmosphere:
     import dataclasses
     mu, w = gauss_radau(n)
     return dataclasses.replace(atm, name=f"{atm.name}_incl{n}", mu=mu, w_mu=w)
+
+
+def with_active_cells(atm: Atmosphere, mode="occupied", fraction=None, dilate=0) -> Atmosphere:
+    """The same atmosphere with a cells-of-interest flag ("in the current implementation this is simply a
+    temperature flag"; here, with no temperature, the stand-in is where the opacity is).  mode "occupied": cells whose
+    opacity (any wavelength; line mode: chi_c + chi_line) exceeds the smallest positive value by a factor 10, dilated by
+    `dilate` cells; "fraction": the `fraction` of cells with the largest wavelength-summed opacity (e.g. 0.25, the paper's
+    production run)."""
+    import dataclasses
+    op = (atm.line[..., 0] + atm.line[..., 2]).astype(np.float64) if atm.line is not None else atm.chi.astype(np.float64).sum(axis=2)
+    if mode == "fraction":
+        k = int(round(fraction * op.size))
+        thr = np.partition(op.ravel(), op.size - k)[op.size - k] if k > 0 else np.inf
+        act = op >= thr
+    else:
+        pos = op[op > 0]
+        act = op > (10.0 * pos.min() if pos.size else 0.0)
+    for _ in range(dilate):
+        a = act.copy()
+        a[1:, :] |= act[:-1, :]; a[:-1, :] |= act[1:, :]; a[:, 1:] |= act[:, :-1]; a[:, :-1] |= act[:, 1:]
+        act = a
+    return dataclasses.replace(atm, name=f"{atm.name}_active", active=act.astype(np.uint8),
+                               meta=dict(atm.meta, active_fraction=float(act.mean())))
 
 
 def make_config(idx: int, **kw) -> Atmosphere:

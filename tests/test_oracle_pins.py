@@ -788,3 +788,115 @@ def test_I4_boundary_per_inclination(oracle):
     J1 = oracle.solve_inclined(a.chi, a.eta, 3, mu, w, I_below=[0.7, 0.2])["J"]
     J2 = oracle.solve_inclined(a.chi, a.eta, 3, mu, w, I_below=np.tile([0.7, 0.2], (4, 1)))["J"]
     assert np.array_equal(J1, J2)
+
+
+# ----------------------------------------------------------------------------- sparsity (f4)
+def _flagged_counts_geometric(active, ncasc):
+    """Flagged probes per cascade from the GEOMETRY alone (no parity rule): the bilinear parents of a probe at
+    position p (cell units, per axis) among the cascade-(i+1) probes at (q + 1/2) 2^(i+1) are the two nearest ones,
+    q = floor(p / 2^(i+1) - 1/2) and q + 1, clamped to the lattice."""
+    ny, nx = active.shape
+    flag = active.astype(bool)
+    counts = [int(flag.sum())]
+    for i in range(ncasc - 1):
+        S = 2 ** (i + 1)
+        up = np.zeros((ny // S, nx // S), bool)
+        bs, as_ = np.nonzero(flag)
+        py, px = (bs + 0.5) * 2 ** i, (as_ + 0.5) * 2 ** i
+        for dy in (0, 1):
+            for dx in (0, 1):
+                qy = np.clip(np.floor(py / S - 0.5).astype(int) + dy, 0, ny // S - 1)
+                qx = np.clip(np.floor(px / S - 0.5).astype(int) + dx, 0, nx // S - 1)
+                up[qy, qx] = True
+        flag = up
+        counts.append(int(flag.sum()))
+    return counts
+
+
+def test_S1_all_cells_flagged_is_the_dense_solve_bit_for_bit(oracle):
+    a = A.make_config(3, nx=64, ny=32, nlambda=3, ncascades=5)
+    dense = oracle.solve_atmosphere(a, want_counts=True)
+    ones = oracle.solve_atmosphere(a, active=np.ones((32, 64), np.uint8), want_counts=True)
+    assert np.array_equal(dense["J"], ones["J"]) and np.array_equal(dense["Jbar"], ones["Jbar"])
+    assert np.array_equal(dense["intervals"], ones["intervals"]) and np.array_equal(dense["segments"], ones["segments"])
+    line = A.line_config2(nx=32, ny=32, nlambda=3, ncascades=4)
+    assert np.array_equal(oracle.solve_atmosphere(line)["J"], oracle.solve_atmosphere(line, active=np.ones((32, 32)))["J"])
+
+
+@pytest.mark.parametrize("seed", [0, 1, 2])
+def test_S2_flagged_probes_are_the_recursive_bilinear_parents(oracle, seed):
+    """PAPER.md:380: "This flag then defines the probes of cascade 0 that may be involved ... Their bilinear "parents"
+    are recursively flagged up to the maximum cascade, and the radiance intervals are only computed for these flagged
+    probes": the number of intervals the oracle computes per cascade = 4^(i+1) x the flagged probes, counted here from
+    the geometry (nearest two parents per axis).  A single flagged cell away from the edges flags 2 x 2 parents."""
+    rng = np.random.default_rng(seed)
+    nx, ny, nc = 64, 48, 5
+    act = np.zeros((ny, nx), np.uint8)
+    for _ in range(3 + seed):                                  # a few blobs and single cells, some on the edges
+        cx, cy, r = rng.integers(0, nx), rng.integers(0, ny), rng.integers(0, 6)
+        yy, xx = np.mgrid[0:ny, 0:nx]
+        act[(xx - cx) ** 2 + (yy - cy) ** 2 <= r * r] = 1
+    act[0, 0] = 1
+    chi, eta = A.random_field(nx, ny, 1, seed=seed)
+    out = oracle.solve(chi, eta, nc, active=act, want_counts=True)
+    want = _flagged_counts_geometric(act, nc)
+    assert [int(n) // 4 ** (i + 1) for i, n in enumerate(out["intervals"])] == want
+    single = np.zeros((ny, nx), np.uint8)
+    single[20, 30] = 1
+    out = oracle.solve(chi, eta, 3, active=single, want_counts=True)
+    # by hand: cell x = 30 sits at 30.5, between the cascade-1 probes 14 (at 29) and 15 (at 31); those sit between the
+    # cascade-2 probes {6, 7} (at 26, 30) and {7, 8}: 3 columns.  y = 20 -> {9, 10} (at 19, 21) -> {4, 5} both: 2 rows.
+    assert list(out["intervals"]) == [4 * 1, 16 * (2 * 2), 64 * (3 * 2)]
+
+
+def test_S3_flagged_cells_keep_their_J_when_the_rest_is_vacuum_anyway(oracle):
+    """If the cells that are not flagged hold nothing, the sparse solve must give, on the flagged cells, exactly the dense
+    solve (every interval it computes is the same interval) - and 0 on the others; it never reads an interval it did
+    not compute (those are NaN inside the oracle)."""
+    a = A.make_config(4, nx=128, ny=64, nlambda=3, ncascades=5)
+    act = (a.chi.sum(axis=2) > 0).astype(np.uint8)
+    assert 0.02 < act.mean() < 0.5
+    dense = oracle.solve_atmosphere(a, want_counts=True)
+    sparse = oracle.solve_atmosphere(a, active=act, want_counts=True)
+    on = act > 0
+    assert np.array_equal(sparse["J"][on], dense["J"][on]) and np.array_equal(sparse["Jbar"][on], dense["Jbar"][on])
+    assert np.all(sparse["J"][~on] == 0.0) and np.all(np.isfinite(sparse["J"]))
+    assert sparse["intervals"][0] == 4 * on.sum() and np.all(sparse["intervals"] <= dense["intervals"])
+    assert sparse["segments"].sum() < dense["segments"].sum()
+    # with the bilinear fix and inclinations too
+    fx = oracle.solve_atmosphere(a, active=act, bilinear_fix=True)["J"]
+    assert np.array_equal(fx[on], oracle.solve_atmosphere(a, bilinear_fix=True)["J"][on])
+    mu, w = A.gauss_radau(2)
+    inc = oracle.solve_inclined(a.chi, a.eta, 5, mu, w, active=act)["J"]
+    assert np.array_equal(inc[on], oracle.solve_inclined(a.chi, a.eta, 5, mu, w)["J"][on])
+
+
+def test_S4_cells_that_are_not_flagged_are_transparent_and_dark(oracle):
+    """"non-flagged cells are treated as transparent with no emission": whatever chi, eta hold there."""
+    a = A.make_config(0, nx=64, ny=64, nlambda=2, ncascades=5)
+    yy, xx = np.mgrid[0:64, 0:64]
+    act = (((xx - 20) ** 2 + (yy - 30) ** 2 < 15 ** 2) | ((xx > 50) & (yy < 10))).astype(np.uint8)
+    on = act > 0
+    zeroed_chi, zeroed_eta = a.chi.copy(), a.eta.copy()
+    zeroed_chi[~on] = 0
+    zeroed_eta[~on] = 0
+    got = oracle.solve(a.chi, a.eta, 5, active=act, I_below=[0.3, 0.1])["J"]
+    ref = oracle.solve(zeroed_chi, zeroed_eta, 5, I_below=[0.3, 0.1])["J"]
+    assert np.array_equal(got[on], ref[on])
+    assert np.max(np.abs(got[on] / oracle.solve(a.chi, a.eta, 5, I_below=[0.3, 0.1])["J"][on] - 1)) > 0.05   # the flag matters
+    line = A.line_config2(nx=32, ny=32, nlambda=2, ncascades=4)
+    lact = act[:32, :32]
+    lz = line.line.copy()
+    lz[lact == 0] = 0
+    assert np.array_equal(oracle.solve_line(line.line, line.xl, 4, active=lact)["J"][lact > 0],
+                          oracle.solve_line(lz, line.xl, 4)["J"][lact > 0])
+
+
+def test_S5_sparse_window_solve_is_the_sparse_full_solve_restricted(oracle):
+    a = A.make_config(4, nx=128, ny=64, nlambda=2, ncascades=5)
+    act = (a.chi.sum(axis=2) > 0).astype(np.uint8)
+    full = oracle.solve_atmosphere(a, active=act)
+    for win in ((0, 8, 0, 8), (60, 75, 20, 41), (120, 128, 56, 64)):
+        x0, x1, y0, y1 = win
+        w = oracle.solve_atmosphere(a, active=act, window=win)
+        assert np.array_equal(w["J"], full["J"][y0:y1, x0:x1]) and np.array_equal(w["Jbar"], full["Jbar"][y0:y1, x0:x1])
