@@ -8,7 +8,8 @@ atmosphere.  Default workload: BASELINE.json configs[2] (1024x1024 cells, 64 wav
 the configuration the metric's target is quoted on.  value = probe-ray-wavelength segments per second,
 whole job, inputs resident in HBM; e2e = the same through rc_solve_J_host with pinned HOST buffers
 (H2D of chi, eta and D2H of J inside the timed region).  N > 1: one process per GPU, each solving its
-own wavelength block of 64 (the path shards by wavelength with no exchange) - weak scaling.
+wavelength block of the SAME atmosphere (the path shards by wavelength with no exchange; Jbar: one NCCL
+all-reduce) - strong scaling; without a launcher `--gpus N` starts the N ranks itself.
 """
 from __future__ import annotations
 
@@ -31,9 +32,11 @@ from paper_2408_14425_b200 import atmospheres  # noqa: E402
 METRIC = "probe-ray-wavelength segments/sec"
 UNIT = "seg-lambda/s"
 SM_COUNT, MUFU_PER_CLK_SM = 148, 16  # one ex2 per segment-wavelength; DESIGN.md §7
-# dram__bytes_read.sum + dram__bytes_write.sum of the dominant launch (march_kernel, cascade 5), from the committed
-# ncu --set full captures (profiles/bench_r1d.md, ncu_r1c_modes.md), keyed by (mode, config, cascade)
-NCU_TRAFFIC_BYTES = {("flat", 2, 5): 2.21e9, ("incl8", 2, 5): 7.88e9, ("line", 2, 5): 1.03e9, ("flat", 4, 5): 8.83e9}
+L2_PORT_BYTES_PER_CLK_SM = 64        # L2 -> SM (L1 fill) path; the gather probe reaches 62 of it
+# ncu --set full captures of the dominant launch that are committed under profiles/, keyed by (mode, config, cascade):
+# dram__bytes_read.sum + dram__bytes_write.sum per launch, lts__t_sectors % of peak, and where the capture is.  A run
+# whose mode / config / launch plan has no entry reports traffic = null.
+NCU_CAPTURES = {}
 
 
 def peaks():
@@ -121,6 +124,17 @@ def run_reference(args, atm, workload):
         "gpu_launches": 0}))
 
 
+def spawn_ranks(args):
+    """`python bench.py --gpus N` without a launcher: start N ranks of this very command line (one per GPU) and wait."""
+    import socket
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), str(Path(__file__).resolve()), *sys.argv[1:]]
+    sys.exit(subprocess.call(cmd))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -137,10 +151,20 @@ def main():
     ap.add_argument("--inclinations", type=int, default=1,
                     help="2.5D: N Gauss-Radau inclined rays per flatland ray (SURVEY §8(f) f2); the unit count "
                          "becomes segment-wavelength-inclinations")
+    ap.add_argument("--active", default="",
+                    help="sparsity as the paper defines it (PAPER.md:380, SURVEY §8(f) f4): 'occupied' flags the cells that hold "
+                         "opacity, a number in (0, 1) the densest fraction of the cells (0.25: the paper's production run)")
+    ap.add_argument("--no-analyse", action="store_true",
+                    help="skip rc_analyse_atmosphere (free-space acceleration of mostly-empty atmospheres, config 4)")
+    ap.add_argument("--tune", default="", help="rc_set_tuning knobs, e.g. march_variant=0,bands=3")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--e2e-steps", type=int, default=0, help="end-to-end steps (default: the same as --steps)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    e2e_steps = args.e2e_steps or args.steps
+
+    if args.impl == "ours" and args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        spawn_ranks(args)
 
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -148,39 +172,54 @@ def main():
     fx, fy, fl, fc = atmospheres.FULL_SHAPES[args.config]
     workload = (f"BASELINE.json configs[{args.config}]: {fx}x{fy} cells, {fl} wavelengths, {fc} cascades, "
                 f"seeded synthetic atmosphere (DESIGN.md §4)")
-    atm = atmospheres.make_config(args.config, seed=1000 + args.config + 17 * rank)
+    atm = atmospheres.make_config(args.config)      # ONE atmosphere for the whole job; ranks take wavelength blocks of it
     if args.line:
-        atm = atmospheres.line_config2(seed=1002 + 17 * rank)
+        atm = atmospheres.line_config2()
         fx, fy, fl, fc = atm.nx, atm.ny, atm.nlambda, atm.ncascades
         workload = (f"moving-line variant of BASELINE.json configs[2]: {fx}x{fy} cells, {fl} wavelengths, {fc} cascades, "
                     "line opacity evaluated per ray from the projected velocity (SURVEY §8(f) f1)")
     if args.inclinations > 1:
         atm = atmospheres.with_inclinations(atm, args.inclinations)
         workload += f", 2.5D with {args.inclinations} Gauss-Radau inclinations per ray (value counts segment-wavelength-inclinations)"
+    if args.active:
+        atm = (atmospheres.with_active_cells(atm) if args.active == "occupied" else
+               atmospheres.with_active_cells(atm, mode="fraction", fraction=float(args.active)))
+        workload += (f", cells of interest: {args.active} ({100 * atm.meta['active_fraction']:.1f} % of the cells flagged; "
+                     "value counts the segments of flagged probes only)")
     if args.impl == "reference":
         run_reference(args, atm, workload)
         return
 
     import torch
     import torch.distributed as dist
-    from paper_2408_14425_b200 import binding
+    from paper_2408_14425_b200 import binding, sharding
     if world > 1:
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
     torch.cuda.set_device(local_rank)
     dev = f"cuda:{local_rank}"
     hbm_peak, sm_max_mhz, peak_src = peaks()
+    nlambda_job = atm.nlambda
+    if world > 1:
+        # the path shards by wavelength: rank r solves its contiguous block of the SAME
+        # atmosphere; per-wavelength J needs no exchange, Jbar one all-reduce of nx ny floats (inside the timed region)
+        assert atm.line is None, "the multi-rank leg shards chi/eta planes (GivenFs mode)"
+        atm = sharding.shard_atmosphere(atm, rank, world)
+        assert atm.nlambda > 0, f"{nlambda_job} wavelengths do not cover {world} ranks"
 
     flags = binding.RC_ACCUM_J if atm.accumulate else 0
     if args.bilinear_fix:
         flags |= binding.RC_BILINEAR_FIX
         workload += ", bilinear fix (the unit count includes the 4 sub-rays of every interval)"
     rc = binding.RadianceCascades(atm.ncascades, atm.c0_interval, local_rank, args.lambda_batch, flags)
+    if args.tune:
+        rc.set_tuning(**{k: float(v) for k, v in (kv.split("=") for kv in args.tune.split(","))})
     if atm.mu is not None:
         rc.set_inclinations(atm.mu, atm.w_mu)
     rc.ensure_workspace(atm.nx, atm.ny, atm.nlambda, host_io=True)
     if rc._ws.numel() < (80 << 20):  # room for the 64 MB region of the gather-bandwidth probe
         rc.set_workspace(torch.empty(80 << 20, dtype=torch.uint8, device=dev))
+    active_d = None if atm.active is None else torch.from_numpy(np.ascontiguousarray(atm.active)).to(dev)
     if atm.line is not None:
         line_h = torch.from_numpy(atm.line).pin_memory()
         line_d = line_h.to(dev)
@@ -190,17 +229,30 @@ def main():
         eta_h = torch.from_numpy(atm.eta).pin_memory()
         chi, eta = chi_h.to(dev), eta_h.to(dev)
         rc.set_atmosphere(chi, eta)
-    rc.set_boundary(atm.I_below, atm.I_above)
-    rc.set_lambda_weights(atm.weights)
+
+    def configure():
+        rc.set_boundary(atm.I_below, atm.I_above)
+        rc.set_lambda_weights(atm.weights)
+        if active_d is not None:
+            rc.set_active_cells(active_d)
+    configure()
+    analysed = None
+    if atm.line is None and not args.no_analyse:
+        analysed = rc.analyse_atmosphere()   # empty-cell scan; switches the distance-field march on when > 2/3 is empty
     seg = rc.count_segments()
     l2_gather_gbs = rc.probe_gather_bandwidth(64)      # L2 -> SM ceiling of the gather pattern (64 MB region)
     tma_bulk_gbs = rc.probe_bulk_copy_bandwidth(64)    # the same pattern through TMA bulk copies + shared memory
-    hbm_gather_gbs = rc.probe_gather_bandwidth(1024) if rc._ws.numel() > (1100 << 20) else None
     nincl = 1 if atm.mu is None else len(atm.mu)
-    segl_per_step = sum(seg) * atm.nlambda * nincl
+    segl_job = sum(seg) * nlambda_job * nincl          # the whole job's units per step (every rank has the same geometry)
     J = rc.solve_J()
-    for _ in range(args.warmup - 1):
+    walked = rc.count_walked(out=J)                    # segments actually integrated (early exit, sparsity, free-space jumps)
+
+    def step():
         rc.solve_J(out=J)
+        if world > 1 and atm.accumulate:
+            sharding.allreduce_jbar(J)                  # NCCL all-reduce of the ranks' weighted partial sums
+    for _ in range(args.warmup):
+        step()
     torch.cuda.synchronize()
     rc.set_timing(args.steps)
 
@@ -214,7 +266,7 @@ def main():
     barrier(); torch.cuda.synchronize()
     e0.record()
     for _ in range(args.steps):
-        rc.solve_J(out=J)
+        step()
     e1.record()
     torch.cuda.synchronize(); barrier()
     clocks = sampler.stop()
@@ -223,88 +275,110 @@ def main():
         dist.all_reduce(ms, op=dist.ReduceOp.MAX)
     ms_total = float(ms.item())
     st = rc.get_stats()
-    launches = st.kernel_launches * args.steps
+    launches = (st.kernel_launches + (1 if world > 1 and atm.accumulate else 0)) * args.steps
     rc.set_timing(0)
 
-    # end to end: host buffers in, host buffer out, every step
+    # end to end through the C ABI with HOST buffers: H2D of the inputs, solve, D2H of J, every step
     out_h = torch.empty(J.shape, dtype=torch.float32, pin_memory=True)
     if atm.line is not None:
         h2d_bytes = int(atm.line.nbytes)
 
-        def e2e_step():  # line mode: the same public calls a user makes, host buffers both ends
-            line_d.copy_(line_h, non_blocking=True)
-            rc.set_line_atmosphere(line_d, atm.xl)
-            rc.solve_J(out=J)
-            out_h.copy_(J, non_blocking=True)
-            torch.cuda.synchronize()
+        def e2e_step():
+            rc.solve_J_line_host(line_h, atm.xl, out_h)
     else:
         h2d_bytes = int(2 * atm.chi.nbytes)
 
         def e2e_step():
             rc.solve_J_host(chi_h, eta_h, out_h)
+            if world > 1 and atm.accumulate:
+                Jd = out_h.to(dev, non_blocking=True)
+                sharding.allreduce_jbar(Jd)
+                out_h.copy_(Jd)
     e2e_step()
-    rc.set_boundary(atm.I_below, atm.I_above)
-    rc.set_lambda_weights(atm.weights)
+    configure()      # the host path may have moved the atmosphere inside the workspace: boundary, weights, flags again
     e2e_step()
     barrier(); torch.cuda.synchronize()
     e0.record()
-    for _ in range(args.e2e_steps):
+    for _ in range(e2e_steps):
         e2e_step()
     e1.record()
     torch.cuda.synchronize(); barrier()
     ms2 = torch.tensor([e0.elapsed_time(e1)], device=dev)
     if world > 1:
         dist.all_reduce(ms2, op=dist.ReduceOp.MAX)
-    e2e_ms = float(ms2.item()) / args.e2e_steps
+    e2e_ms = float(ms2.item()) / e2e_steps
     same = bool(torch.equal(out_h, J.cpu()))
 
     if rank == 0:
         ms_step = ms_total / args.steps
-        value = world * segl_per_step / (ms_step * 1e-3)
-        # dominant kernel: the march+merge launch of the heaviest cascade
+        value = segl_job / (ms_step * 1e-3)
+        # dominant kernel: the march+merge launch of the heaviest cascade (of this rank's wavelength block)
         ms_march = [st.ms_march[i] for i in range(atm.ncascades)]
         dom = int(np.argmax(ms_march))
         casc_bytes = 2 * 4 * atm.nx * atm.ny * atm.nlambda * nincl  # read merged cascade i+1, write cascade i
-        alg_bytes = 8 * seg[dom] * atm.nlambda + casc_bytes  # chi+eta gather: 8 B per segment-wavelength
+        alg_bytes = 8 * seg[dom] * atm.nlambda + casc_bytes  # chi+eta gather: 8 B per segment-wavelength (SURVEY §8(d))
         ach = alg_bytes / (ms_march[dom] * 1e-3) / 1e9
-        mode = ("line" if atm.line is not None else "flat") + (f"_incl{nincl}" if atm.line is not None and nincl > 1 else
-                                                                   f"incl{nincl}" if nincl > 1 else "")
-        mode = {"flatincl8": "incl8"}.get(mode, mode) + ("_fix" if args.bilinear_fix else "")
+        mode = ("line" if atm.line is not None else "flat") + (f"_incl{nincl}" if nincl > 1 else "") + ("_fix" if args.bilinear_fix else "")
+        cap = NCU_CAPTURES.get((mode, args.config, dom)) if world == 1 and not args.active and not args.tune else None
+        dram = None if cap is None else cap["dram_bytes"]
         mufu_per_unit = 3 if atm.line is not None else 1  # line mode: ex2 (profile), rcp (eta/chi), ex2 (transmittance)
         sfu_peak = SM_COUNT * MUFU_PER_CLK_SM * sm_max_mhz * 1e6 / mufu_per_unit
         ach_alu = seg[dom] * atm.nlambda * nincl / (ms_march[dom] * 1e-3)
+        port_gbs = SM_COUNT * L2_PORT_BYTES_PER_CLK_SM * sm_max_mhz * 1e6 / 1e9
+        mufu_bound = ach_alu / sfu_peak > ach / port_gbs
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
-            "data": "synthetic",
-            "config": {"workload": workload, "seg_lambda_per_step_per_gpu": segl_per_step, "lambda_batch": st.lambda_batch,
-                       "l2": ("inputs (chi+eta %.0f MB) larger than L2" % (h2d_bytes / 1e6)) if atm.line is None else
+            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "strong" if world > 1 else "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": workload, "seg_lambda_per_step": segl_job, "lambda_batch": st.lambda_batch,
+                       "l2": ("inputs (chi+eta %.0f MB per rank) larger than L2" % (h2d_bytes / 1e6)) if atm.line is None else
                              "line parameters (%.0f MB) fit L2; merged cascades (2 x %.0f MB per cascade) stream through it"
                              % (h2d_bytes / 1e6, 4 * atm.nx * atm.ny * atm.nlambda / 1e6),
-                       "parallelism": f"wavelength blocks x{world}, no collective"},
+                       "parallelism": (f"1 GPU" if world == 1 else
+                                       f"{world} ranks x {atm.nlambda} of the {nlambda_job} wavelengths of one atmosphere (contiguous blocks, "
+                                       f"no exchange during the solve" + ("; Jbar: one NCCL all-reduce of nx ny floats per step)" if atm.accumulate else ")")),
+                       "early_exit": True,
+                       "segments_geometric_per_wavelength": sum(seg), "segments_walked_per_wavelength": sum(walked),
+                       "walked_fraction": sum(walked) / max(sum(seg), 1),
+                       "empty_cell_fraction": None if analysed is None else analysed.empty_cells / (atm.nx * atm.ny),
+                       "distance_field_march": None if analysed is None else bool(analysed.sparse_march),
+                       "active_cell_fraction": None if atm.active is None else atm.meta["active_fraction"]},
             "solve_ms": ms_step,
-            "hbm_effective_frac": (8 * segl_per_step + 2 * casc_bytes * atm.ncascades) / (ms_step * 1e-3) / 1e9 / hbm_peak,
-            "roofline": {"bound": "hbm", "kernel": f"march_kernel<{st.lambda_batch}> cascade {dom}", "achieved": ach,
-                         "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak, "traffic": NCU_TRAFFIC_BYTES.get((mode, args.config, dom)),
-                         "traffic_unit": "bytes per launch (ncu --set full; profiles/bench_r1d.md, ncu_r1c_modes.md)",
-                         "algorithmic_bytes": alg_bytes,
-                         "peak_source": peak_src, "ms_per_launch": ms_march[dom],
-                         "note": "effective: algorithmic gather bytes (8 B per segment-wavelength) are mostly served "
-                                 "from L2 (and ~20 % from L1), so frac exceeds 1; roofline_l2 and roofline_alu give the on-chip ceilings"},
-            "roofline_l2": {"bound": "l2", "achieved": ach, "peak": l2_gather_gbs, "unit": "GB/s", "frac": ach / l2_gather_gbs,
-                            "peak_source": "rc_probe_gather_bandwidth(64 MB), measured in this run: random 1 KB warp-wide runs "
-                                           "(LDG.256), 48 warps/SM, region L2-resident",
-                            "hbm_gather_gbs_1GB_region": hbm_gather_gbs,
-                            "tma_bulk_copy_gbs_same_pattern": tma_bulk_gbs},
+            # the binding roof of the dominant kernel: the L2 -> SM gather path (64 B/clk/SM), or the MUFU pipe where one
+            # gather feeds several exponentials (inclinations, moving line); HBM is NOT the roof: the same bytes are
+            # served from L2, so the HBM figures are reported beside it, from the committed ncu capture
+            "roofline": ({"bound": "alu", "pipe": f"MUFU, 16/clk/SM x 148 SMs at sm_max_mhz, {mufu_per_unit} per unit",
+                          "kernel": f"march_kernel<{st.lambda_batch * nincl}> cascade {dom}", "achieved": ach_alu, "peak": sfu_peak,
+                          "unit": UNIT, "frac": ach_alu / sfu_peak} if mufu_bound else
+                         {"bound": "l2", "kernel": f"march_kernel<{st.lambda_batch}> cascade {dom}", "achieved": ach, "peak": port_gbs,
+                          "unit": "GB/s", "frac": ach / port_gbs,
+                          "peak_source": "derived: L2 -> SM port 64 B/clk/SM x 148 SMs x sm_max_mhz (DESIGN.md §7); the fraction can "
+                                         "exceed what L2 alone delivers because part of the algorithmic bytes is served by L1"}),
+            "roofline_l2_probe": {"bound": "l2", "achieved": ach, "peak": l2_gather_gbs, "unit": "GB/s", "frac": ach / l2_gather_gbs,
+                                  "peak_source": "achieved by a micro-kernel (rc_probe_gather_bandwidth(64 MB), this run: random 1 KB "
+                                                 "warp-wide runs, LDG.256, 48 warps/SM, region L2-resident), not a hardware peak",
+                                  "ncu_lts_t_sectors_pct": None if cap is None else cap.get("lts_pct"),
+                                  "tma_bulk_copy_gbs_same_pattern": tma_bulk_gbs},
             "roofline_alu": {"bound": "alu", "pipe": f"MUFU, 16/clk/SM x 148 SMs at sm_max_mhz, {mufu_per_unit} per unit", "achieved": ach_alu,
                              "peak": sfu_peak, "unit": UNIT, "frac": ach_alu / sfu_peak},
+            "hbm": {"peak": hbm_peak, "peak_source": peak_src, "unit": "GB/s", "algorithmic_bytes": alg_bytes,
+                    "algorithmic_over_hbm": ach / hbm_peak,
+                    "solve_algorithmic_over_hbm": (8 * sum(seg) * atm.nlambda * world + 2 * casc_bytes * world * atm.ncascades) / (ms_step * 1e-3) / 1e9 / hbm_peak,
+                    "traffic": dram, "dram_gbs": None if dram is None else dram / (ms_march[dom] * 1e-3) / 1e9,
+                    "frac": None if dram is None else dram / (ms_march[dom] * 1e-3) / 1e9 / hbm_peak,
+                    "traffic_source": ("no ncu capture of this mode, config and launch plan is committed" if cap is None else cap["source"]),
+                    "note": "traffic = dram__bytes_read.sum + dram__bytes_write.sum of the dominant launch (ncu --set full); "
+                            "algorithmic = 8 B per segment-wavelength + merged cascade read/write"},
+            "ms_per_launch": ms_march[dom],
             "per_cascade_ms": {"march": ms_march, "pack": [st.ms_pack[i] for i in range(atm.ncascades)]},
-            "segments_per_cascade": seg,
-            "e2e": {"value": world * segl_per_step / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms,
+            "segments_per_cascade": seg, "segments_walked_per_cascade": walked,
+            "e2e": {"value": segl_job / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms, "steps": e2e_steps,
                     "h2d_bytes_per_step": h2d_bytes, "d2h_bytes_per_step": int(out_h.numel() * 4),
+                    "call": "rc_solve_J_line_host" if atm.line is not None else "rc_solve_J_host",
                     "matches_device_path": same},
             "gpu_launches": launches, "clocks": clocks,
         }
+        line["roofline"]["traffic"] = dram
         if world == 1 and not args.no_cpu_baseline:
             nwin = 3
             segl, secs, cores = oracle_sample(atm, nwin)

@@ -34,12 +34,7 @@
  *            in the limit chi -> 0, the cell adds eta ds (reading G11).
  *   There is no CPU fallback and no other backend: without an sm_100 device rc_create fails.
  *
- * Developer overrides (environment variables, for measurements and tests; none changes a result beyond rounding
- * unless noted): RC_MARCH_VARIANT=0..4 (register-ring depth / occupancy of the march), RC_PATCH_LOG2=2..5 with
- * RC_PATCH_FROM=i (lane patch width for cascades >= i), RC_CPW_FROM=i (child-per-warp for cascades >= i, -1 off),
- * RC_BANDS=n / RC_L2_MB=x (L2 banding), RC_NO_SPARSE / RC_FORCE_SPARSE (occupancy-bitmap march), RC_NO_GRAPH (no CUDA
- * graph replay on small grids), RC_TAU_CUT=x (early-exit threshold on tau log2 e; below 126 it drops transmittances
- * below 2^-x).
+ * The library reads no environment variables; launch knobs for measurements and tests go through rc_set_tuning.
  */
 #ifndef RC_H_
 #define RC_H_
@@ -97,7 +92,11 @@ typedef struct {
     int64_t rays[RC_MAX_CASCADES];        /* intervals per cascade per wavelength = 4 nx ny */
     int64_t table_steps[RC_MAX_CASCADES]; /* step-table entries per cascade (all directions) */
     size_t workspace_bytes;
-    int64_t empty_cells;                  /* cells with chi == 0 and eta == 0 at every wavelength (counted by rc_set_atmosphere) */
+    int64_t empty_cells;                  /* cells that are not flagged, or hold chi == 0 and eta == 0 at every wavelength
+                                             (counted by rc_analyse_atmosphere; 0 before) */
+    int sparse_march;                     /* the march walks the distance field (rc_analyse_atmosphere found > 2/3 empty) */
+    int64_t active_cells;                 /* cells of interest (rc_set_active_cells); -1 = every cell */
+    int64_t probes_flagged[RC_MAX_CASCADES]; /* with active cells: flagged probes of cascade i */
 } rc_stats;
 
 /* The launch plan the library would use for a problem, computed on the host alone (no device, no context):
@@ -131,11 +130,24 @@ int rc_set_workspace(rc_ctx *ctx, void *dev_ptr, size_t bytes);
 /* Caller-owned CUDA stream (cudaStream_t as void*; NULL = the legacy default stream). */
 int rc_set_stream(rc_ctx *ctx, void *cuda_stream);
 
+/* Launch knobs, for measurements and tests (none changes a result beyond rounding, except tau_cut < 126).  Call before
+ * rc_set_atmosphere: it drops the atmosphere and the active cells (plan, patch lists and captured graph may depend on a
+ * knob).  name / value:
+ *   "march_variant" -1 | 0..4   register-ring depth and occupancy of the march (-1: chosen per cascade)
+ *   "patch_log2"    -1 | 2..5   lane patch width 2^n for cascades >= "patch_from" (-1: chosen per cascade from the geometry)
+ *   "cpw_from"      -1 | i      cascades >= i run one child direction per warp (-1: never; default 3)
+ *   "bands" n, "l2_mb" x        L2 banding of grids whose wavelength batch exceeds L2: n bands (0: from the budget x, 72 MB)
+ *   "sparse"        -1 | 0 | 1  distance-field march after rc_analyse_atmosphere: automatic (> 2/3 empty) / never / always
+ *   "sparse_mode"   0 | 1       that march at 24 warps/SM (<= 80 registers) / 16 warps/SM (<= 128)
+ *   "graph"         0 | 1       CUDA graph replay on small grids
+ *   "tau_cut"       x >= 1      early-exit threshold on tau log2 e; below 126 it drops transmittances below 2^-x
+ * RC_ERR_BAD_VALUE for an unknown name or a value out of range. */
+int rc_set_tuning(rc_ctx *ctx, const char *name, double value);
+
 /* chi, eta: device, [ny][nx][nlambda] float32, borrowed.  Builds the per-direction step tables for
  * this grid size (device kernels, fp64 geometry) if the shape changed; needs the workspace set.
- * Also counts the cells that are empty (chi == 0 at every wavelength) and synchronises the stream: when
- * more than two thirds are, the march skips the gathers of empty cells (sparsity; the result
- * is bit-identical).  PAPER.md:409. */
+ * With an unchanged shape the call only records the pointers: no device work, no synchronisation (the iteration of
+ * PAPER.md:316-342 calls it once per formal solution).  PAPER.md:409. */
 int rc_set_atmosphere(rc_ctx *ctx, const float *chi, const float *eta, int nx, int ny, int nlambda);
 
 /* Velocity-dependent line mode ("velocity-dependent terms (spectral lines) are computed on the
@@ -147,8 +159,28 @@ int rc_set_atmosphere(rc_ctx *ctx, const float *chi, const float *eta, int nx, i
  *     a = x_l + v.w,  phi = exp(-a^2)/sqrt(pi),  chi = chi_c + chi_line phi,  eta = chi_c S_c + chi_line S_line phi
  * enter eq. 16.  With inclinations set (rc_set_inclinations, before this call) the velocities are taken to lie
  * in the plane: inclination m sees v.w sqrt(1 - mu_m^2) over the path ds / sqrt(1 - mu_m^2).  rc_solve_J,
- * rc_set_boundary, rc_set_lambda_weights, RC_ACCUM_J work as usual; rc_solve_J_host does not apply. */
+ * rc_set_boundary, rc_set_lambda_weights, RC_ACCUM_J work as usual; host buffers: rc_solve_J_line_host. */
 int rc_set_line_atmosphere(rc_ctx *ctx, const float *line, int nx, int ny, const float *x_lambda, int nlambda);
+
+/* Sparsity as the paper defines it (§3.5): "we can first determine the cells of
+ * interest ...  This flag then defines the probes of cascade 0 that may be involved ... Their bilinear "parents" are
+ * recursively flagged up to the maximum cascade, and the radiance intervals are only computed for these flagged probes,
+ * and non-flagged cells are treated as transparent with no emission."  active: device, [ny][nx] bytes, non-zero = cell
+ * of interest; copied (not borrowed).  NULL = every cell (the default).  Afterwards J_out holds J on the flagged cells
+ * and 0 on the others, whatever chi, eta hold there; probe patches without a flagged probe launch no warp.  Call
+ * after rc_set_atmosphere; stays in force for later atmospheres of the same shape; synchronises the stream (the
+ * number of flagged patches sizes the launches). */
+int rc_set_active_cells(rc_ctx *ctx, const unsigned char *active);
+
+/* Free-space acceleration ("accelerating the traversal of long-range radiance intervals through
+ * free-space"): scans the current atmosphere (and flags) for empty cells - not flagged, or chi == eta == 0 at every
+ * wavelength - and builds their Chebyshev distance transform.  When more than two thirds of the cells are empty the
+ * march of the next solves lets every lane walk its own ray and jump over empty space; the result is bit-identical
+ * to the lock-step march.  Explicit because it synchronises the stream and belongs to one atmosphere: the next
+ * rc_set_atmosphere / rc_set_line_atmosphere / rc_set_active_cells switches it off again (rc_solve_J_host repeats it
+ * by itself once it has been used on the context).  Plain mode only (no inclinations, moving line or bilinear fix:
+ * there it only counts).  rc_stats.empty_cells, rc_stats.sparse_march report the outcome. */
+int rc_analyse_atmosphere(rc_ctx *ctx);
 
 /* Boundary intensity sampled by the top cascade: I_below[l] is seen by rays heading
  * down (omega_y < 0), I_above[l] by rays heading up.  host, [nlambda] each; NULL = 0 (free space,
@@ -188,6 +220,10 @@ int rc_compute_alo(rc_ctx *ctx, float *alo_out);
 int rc_solve_J_host(rc_ctx *ctx, const float *chi_host, const float *eta_host, int nx, int ny,
                     int nlambda, float *J_host);
 
+/* The line mode with HOST buffers: line_host [ny][nx][6] (host), x_lambda as rc_set_line_atmosphere, J_host as
+ * rc_solve_J_host; the workspace must have been sized with host_io != 0.  Copies, solves, copies back, synchronises. */
+int rc_solve_J_line_host(rc_ctx *ctx, const float *line_host, int nx, int ny, const float *x_lambda, int nlambda, float *J_host);
+
 /* nsets > 0: the next solves record CUDA events on the context's stream around every kernel, solve
  * number n into event set n % nsets (no synchronisation is added); 0 switches timing off.
  * rc_get_stats waits for the recorded sets and averages over them. */
@@ -198,6 +234,12 @@ int rc_get_stats(rc_ctx *ctx, rc_stats *out);
  * [ncascades]) = number of (probe, direction) cell segments of cascade i inside the box, per
  * wavelength.  Counted on the device from the step tables; synchronises. */
 int rc_count_segments(rc_ctx *ctx, int64_t *per_cascade);
+
+/* One solve into J_out (device, as rc_solve_J) that also counts the cell segments the march actually integrated, per
+ * cascade and wavelength (host, [ncascades]; the mean over the wavelength batches): the early exit of opaque rays
+ * (PAPER.md:308), unflagged probes and the jumps over free space leave the rest of rc_count_segments'
+ * geometric count unwalked.  Synchronises. */
+int rc_count_walked(rc_ctx *ctx, float *J_out, int64_t *per_cascade);
 
 /* Measurement aid for the roofline: achieved GB/s (*gbs, host) of the access pattern the
  * march gathers with and nothing else - every warp reads pseudo-random 1 KB runs (32 lanes x 32 B), 48

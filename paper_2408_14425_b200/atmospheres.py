@@ -329,8 +329,10 @@ def with_active_cells(atm: Atmosphere, mode="occupied", fraction=None, dilate=0)
     op = (atm.line[..., 0] + atm.line[..., 2]).astype(np.float64) if atm.line is not None else atm.chi.astype(np.float64).sum(axis=2)
     if mode == "fraction":
         k = int(round(fraction * op.size))
-        thr = np.partition(op.ravel(), op.size - k)[op.size - k] if k > 0 else np.inf
-        act = op >= thr
+        order = np.argsort(-op.ravel(), kind="stable")       # ties (e.g. a uniform corona) go by cell index: exactly k cells
+        act = np.zeros(op.size, bool)
+        act[order[:k]] = True
+        act = act.reshape(op.shape)
     else:
         pos = op[op > 0]
         act = op > (10.0 * pos.min() if pos.size else 0.0)

@@ -30,7 +30,8 @@ class rc_stats(C.Structure):
                 ("solves_timed", C.c_int), ("ms_pack", C.c_float * RC_MAX_CASCADES),
                 ("ms_march", C.c_float * RC_MAX_CASCADES), ("ms_total", C.c_float),
                 ("rays", C.c_int64 * RC_MAX_CASCADES), ("table_steps", C.c_int64 * RC_MAX_CASCADES),
-                ("workspace_bytes", C.c_size_t), ("empty_cells", C.c_int64)]
+                ("workspace_bytes", C.c_size_t), ("empty_cells", C.c_int64), ("sparse_march", C.c_int),
+                ("active_cells", C.c_int64), ("probes_flagged", C.c_int64 * RC_MAX_CASCADES)]
 
 
 class rc_plan_info(C.Structure):
@@ -57,8 +58,11 @@ SYMBOLS = {
     "rc_workspace_bytes": (C.c_size_t, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int]),
     "rc_set_workspace": (C.c_int, [C.c_void_p, C.c_void_p, C.c_size_t]),
     "rc_set_stream": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "rc_set_tuning": (C.c_int, [C.c_void_p, C.c_char_p, C.c_double]),
     "rc_set_atmosphere": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int]),
     "rc_set_line_atmosphere": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_int]),
+    "rc_set_active_cells": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "rc_analyse_atmosphere": (C.c_int, [C.c_void_p]),
     "rc_set_boundary": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
     "rc_set_boundary_inclined": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
     "rc_set_lambda_weights": (C.c_int, [C.c_void_p, C.c_void_p]),
@@ -66,6 +70,8 @@ SYMBOLS = {
     "rc_solve_J": (C.c_int, [C.c_void_p, C.c_void_p]),
     "rc_compute_alo": (C.c_int, [C.c_void_p, C.c_void_p]),
     "rc_solve_J_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p]),
+    "rc_solve_J_line_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_int, C.c_void_p]),
+    "rc_count_walked": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
     "rc_set_timing": (C.c_int, [C.c_void_p, C.c_int]),
     "rc_get_stats": (C.c_int, [C.c_void_p, C.POINTER(rc_stats)]),
     "rc_count_segments": (C.c_int, [C.c_void_p, C.c_void_p]),
@@ -160,6 +166,11 @@ class RadianceCascades:
         s = torch.cuda.current_stream(self.device) if stream is None else stream
         self._check(self.lib.rc_set_stream(self.handle, C.c_void_p(s.cuda_stream)))
 
+    def set_tuning(self, **knobs):
+        """Launch knobs (rc_set_tuning): e.g. set_tuning(march_variant=0, bands=3).  Before set_atmosphere."""
+        for k, v in knobs.items():
+            self._check(self.lib.rc_set_tuning(self.handle, k.encode(), float(v)))
+
     def set_atmosphere(self, chi, eta):
         """chi, eta: CUDA float32 tensors [ny][nx][nlambda] (borrowed until replaced)."""
         assert chi.is_cuda and eta.is_cuda and chi.dtype == eta.dtype and chi.shape == eta.shape
@@ -183,6 +194,22 @@ class RadianceCascades:
                                                     x.ctypes.data_as(C.c_void_p), int(x.size)))
         self._keep = (line,)
         self.shape = (ny, nx, int(x.size))
+
+    def set_active_cells(self, active=None):
+        """active: CUDA uint8 tensor [ny][nx] (non-zero = cell of interest; copied by the library) or None = every cell."""
+        if active is None:
+            self._check(self.lib.rc_set_active_cells(self.handle, None))
+            return
+        ny, nx, _ = self.shape
+        assert active.is_cuda and active.is_contiguous() and active.element_size() == 1 and tuple(active.shape) == (ny, nx)
+        self.set_stream()
+        self._check(self.lib.rc_set_active_cells(self.handle, C.c_void_p(active.data_ptr())))
+
+    def analyse_atmosphere(self):
+        """Empty-cell scan + distance field of the current atmosphere (synchronises); see rc_analyse_atmosphere."""
+        self.set_stream()
+        self._check(self.lib.rc_analyse_atmosphere(self.handle))
+        return self.get_stats()
 
     def set_boundary(self, I_below=None, I_above=None):
         """[nlambda] arrays, or [ninclinations][nlambda] (one value per inclined ray set)."""
@@ -241,6 +268,34 @@ class RadianceCascades:
         self.shape = (ny, nx, L)
         return out_host
 
+    def solve_J_line_host(self, line_host, xl, out_host=None):
+        """Line mode, host tensors (ideally pinned) in and out: H2D + solve + D2H through rc_solve_J_line_host."""
+        import torch
+        ny, nx, _ = line_host.shape
+        x = np.ascontiguousarray(xl, dtype=np.float32)
+        L = int(x.size)
+        self.ensure_workspace(nx, ny, L, host_io=True)
+        self.set_stream()
+        shape = (ny, nx) if self.flags & RC_ACCUM_J else (ny, nx, L)
+        if out_host is None:
+            out_host = torch.empty(shape, dtype=torch.float32, pin_memory=True)
+        self._check(self.lib.rc_solve_J_line_host(self.handle, C.c_void_p(line_host.data_ptr()), nx, ny,
+                                                  x.ctypes.data_as(C.c_void_p), L, C.c_void_p(out_host.data_ptr())))
+        self.shape = (ny, nx, L)
+        return out_host
+
+    def count_walked(self, out=None):
+        """One solve with counters: cell segments actually integrated per cascade and wavelength (rc_count_walked)."""
+        import torch
+        ny, nx, L = self.shape
+        shape = (ny, nx) if self.flags & RC_ACCUM_J else (ny, nx, L)
+        if out is None:
+            out = torch.empty(shape, dtype=torch.float32, device=f"cuda:{self.device}")
+        self.set_stream()
+        res = (C.c_int64 * RC_MAX_CASCADES)()
+        self._check(self.lib.rc_count_walked(self.handle, C.c_void_p(out.data_ptr()), res))
+        return [int(res[i]) for i in range(self.cfg.ncascades)]
+
     def compute_alo(self):
         """Diagonal ALO of cascade 0 (eq. 17) of the current atmosphere: CUDA tensor [ny][nx][nlambda]."""
         import torch
@@ -287,13 +342,15 @@ class RadianceCascades:
             pass
 
 
-def solve_atmosphere(atm, device=0, lambda_batch=0, flags=0, rc=None):
+def solve_atmosphere(atm, device=0, lambda_batch=0, flags=0, rc=None, analyse=False, tuning=None):
     """Convenience for tests/bench: upload an `atmospheres.Atmosphere`, solve, return (J tensor, ctx)."""
     import torch
     dev = f"cuda:{device}"
     fl = flags | (RC_ACCUM_J if atm.accumulate else 0) | (RC_BILINEAR_FIX if getattr(atm, "bilinear_fix", False) else 0)
     if rc is None:
         rc = RadianceCascades(atm.ncascades, atm.c0_interval, device, lambda_batch, fl)
+    if tuning:
+        rc.set_tuning(**tuning)
     if getattr(atm, "line", None) is not None:
         if getattr(atm, "mu", None) is not None:
             rc.set_inclinations(atm.mu, atm.w_mu)
@@ -306,6 +363,10 @@ def solve_atmosphere(atm, device=0, lambda_batch=0, flags=0, rc=None):
         rc.set_atmosphere(chi, eta)
     rc.set_boundary(atm.I_below, atm.I_above)
     rc.set_lambda_weights(atm.weights)
+    if getattr(atm, "active", None) is not None:
+        rc.set_active_cells(torch.from_numpy(np.ascontiguousarray(atm.active, dtype=np.uint8)).to(dev))
+    if analyse:
+        rc.analyse_atmosphere()
     J = rc.solve_J()
     torch.cuda.synchronize(device)
     return J, rc

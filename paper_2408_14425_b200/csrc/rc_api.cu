@@ -7,6 +7,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <new>
+#include <string>
 #include <vector>
 
 #include "../../include/rc.h"
@@ -16,6 +17,21 @@ namespace {
 
 constexpr size_t ALIGN = 256;
 inline size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
+
+// Launch knobs (rc_set_tuning): measurement and test aids; none changes a result beyond rounding unless noted.
+struct Tuning {
+    int variant = -1;      // march_variant 0..4: register-ring depth / occupancy of the march; -1: chosen per cascade
+    int patch_log2 = -1;   // 2..5: lane patch width 2^n for cascades >= patch_from; -1: chosen per cascade (choose_patch)
+    int patch_from = 0;
+    int cpw_from = 3;      // cascades >= this run one child direction per warp; -1: off
+    bool cpw_forced = false;
+    float tau_cut = 126.f; // early-exit threshold on tau log2(e); 126: the fp32 transmittance is exactly 0 (below: changes J)
+    int bands = 0;         // L2 banding: number of bands; 0: from the L2 budget
+    double l2_mb = 72.0;   // L2 budget of one wavelength batch of packed chi, S
+    int sparse = -1;       // distance-field march: -1 automatic (> 2/3 of the cells empty), 0 never, 1 whenever analysed
+    int graph = 1;         // CUDA graph replay on small grids
+    int sparse_mode = 0;   // distance-field march variant, 0..3
+};
 
 struct CascadePlan {
     bool fix = false;           // bilinear fix: 16 tables per direction, lanes = one parity class, packed with spacing 2s
@@ -37,8 +53,10 @@ struct Plan {
     size_t state = 0;               // parked ray state of the banded launches
     bool line = false;              // velocity-dependent line mode: chiT holds 6 packed line parameters per cell
     size_t xls = 0;                 // line mode: scaled wavelengths [Lpad]
-    size_t occ = 0;                 // occupancy bitmap of the packed cells (0: none, nx ny not a multiple of 32)
-    bool has_occ = false;
+    // sparsity: flagged probes per cascade (bytes), compacted patch lists, and the distance field
+    size_t pflag[RC_MAX_CASCADES] = {0}, plist[RC_MAX_CASCADES] = {0}, pmark = 0, pcount = 0;
+    int plist_cap[RC_MAX_CASCADES] = {0};
+    size_t occ8 = 0, d1 = 0, dist = 0;
     CascadePlan c[RC_MAX_CASCADES];
     size_t chiT = 0, ST = 0, A[2] = {0, 0}, Jpart = 0, bc_below = 0, bc_above = 0, weights = 0, flag = 0;
     size_t io_chi = 0, io_eta = 0, io_J = 0;
@@ -63,12 +81,16 @@ struct rc_ctx {
     GraphKey graph_key{};
     cudaGraphExec_t graph_exec = nullptr;
     cudaStream_t cap_stream = nullptr;
-    bool sparse = false;  // most cells have chi == 0 at every wavelength (counted by rc_set_atmosphere): skip their gathers
-    // developer overrides (environment, read by rc_create): RC_MARCH_VARIANT = 0..3 (register ring depth /
-    // occupancy of march_kernel), RC_PATCH_LOG2 = 2..5 forces the lane patch width for cascades >= RC_PATCH_FROM
-    int tune_variant = -1, tune_patch = -1, tune_patch_from = 0;  // variant -1: chosen per cascade (march_variant)
-    int tune_cpw = 3;        // RC_CPW_FROM: cascades >= this run one child direction per warp (-1: off)
-    float tau_cut = 126.f;  // early-exit threshold on tau log2(e); 126: the fp32 transmittance is exactly 0
+    // sparsity
+    bool active_set = false;   // rc_set_active_cells: flagged probes per cascade are in the workspace
+    bool lists_dirty = false;  // the compacted patch lists must be rebuilt (before the next solve; synchronises once)
+    int npatch_act[RC_MAX_CASCADES] = {0};
+    int list_version = 0;
+    bool sparse = false;       // rc_analyse_atmosphere found the atmosphere mostly empty: the march walks the distance field
+    bool count_walked = false; // the solve being enqueued counts the segments it integrates (rc_count_walked)
+    bool analysed = false;     // rc_analyse_atmosphere has been used on this context (rc_solve_J_host then repeats it)
+    std::vector<float> xl_stage;  // line mode: host copy of the scaled wavelengths (kept alive for the async upload)
+    Tuning tune{};
     // 2.5D inclination quadrature (rc_set_inclinations); nm = 1, f = w = 1: flatland
     int nm = 1;
     float incl_f[8] = {1, 1, 1, 1, 1, 1, 1, 1}, incl_w[8] = {1, 0, 0, 0, 0, 0, 0, 0};
@@ -168,7 +190,7 @@ int choose_lv(const rc_config &cfg, int L, int nm) {
 }
 
 // Workspace layout for a shape.  When `offs` is given, also fills the per-direction slot offsets.
-bool make_plan_uncached(const rc_config &cfg, int nm, bool line, int nx, int ny, int L, bool host_io, Plan &P,
+bool make_plan_uncached(const rc_config &cfg, const Tuning &tune, int nm, bool line, int nx, int ny, int L, bool host_io, Plan &P,
                         std::vector<std::vector<long long>> *offs) {
     if (!shape_ok(cfg, nx, ny, L)) return false;
     P = Plan{};
@@ -233,10 +255,8 @@ bool make_plan_uncached(const rc_config &cfg, int nm, bool line, int nx, int ny,
     // L2 budget the cascades with long rays are marched band by band
     {
         const double batch_mb = line ? 0.0 : (double)ncell * P.LV * 8.0 / (1 << 20);  // line mode: 24 B per cell
-        double budget_mb = 72.0;
-        if (const char *e = std::getenv("RC_L2_MB")) budget_mb = std::max(1.0, std::atof(e));
-        P.nbands = (int)std::ceil(batch_mb / budget_mb);
-        if (const char *e = std::getenv("RC_BANDS")) P.nbands = std::max(1, std::atoi(e));
+        P.nbands = (int)std::ceil(batch_mb / std::max(1.0, tune.l2_mb));
+        if (tune.bands > 0) P.nbands = tune.bands;
         P.band_axis = nx > ny ? 1 : 0;
         const int n_axis = P.band_axis ? nx : ny;
         P.nbands = std::max(1, std::min(P.nbands, n_axis / 32));
@@ -247,13 +267,27 @@ bool make_plan_uncached(const rc_config &cfg, int nm, bool line, int nx, int ny,
             // worth it for long rays only, and only while one warp's patch of probes is small against a
             // band (its lanes enter and leave a band at different steps: lock-step waste otherwise)
             const int patch_ext = (P.band_axis ? 1 << c.pw_log2 : 32 >> c.pw_log2) << i;
-            c.banded = P.nbands > 1 && !c.empty && !c.fix && std::fmin(c.tb, diag) > 100.0 && (4 * patch_ext <= ext || std::getenv("RC_BANDS"));
+            c.banded = P.nbands > 1 && !c.empty && !c.fix && std::fmin(c.tb, diag) > 100.0 && (4 * patch_ext <= ext || tune.bands > 0);
             any = any || c.banded;
         }
         if (any) { P.state = cur; cur += 8 * field * P.NM; }
     }
-    P.has_occ = ncell % 32 == 0 && P.NM == 1 && !line;
-    if (P.has_occ) { P.occ = cur; cur += align_up((ncell / 32) * P.nb * sizeof(unsigned)); }
+    {
+        int cap_max = 1;
+        for (int i = 0; i <= top; i++) {
+            const size_t np = (size_t)(nx >> i) * (ny >> i);
+            P.pflag[i] = cur; cur += align_up(np);
+            // patches of 32 probes of any shape 2^k x 2^(5-k), x 4 parity classes with the bilinear fix
+            P.plist_cap[i] = (int)std::min<size_t>(4 * (np / 32 + (size_t)(nx >> i) + (size_t)(ny >> i) + 4), 0x7fffffff);
+            P.plist[i] = cur; cur += align_up(sizeof(int) * (size_t)P.plist_cap[i]);
+            cap_max = std::max(cap_max, P.plist_cap[i]);
+        }
+        P.pmark = cur;  cur += align_up((size_t)cap_max);
+        P.pcount = cur; cur += align_up(sizeof(int) * RC_MAX_CASCADES);
+        P.occ8 = cur; cur += align_up(ncell);
+        P.d1 = cur;   cur += align_up(ncell);
+        P.dist = cur; cur += align_up(ncell);
+    }
     if (line) {
         P.chiT = cur; cur += align_up(ncell * 6 * sizeof(float));
         P.xls = cur;  cur += align_up(2 * P.Lpad * sizeof(float));  // x_l sqrt(log2 e), then x_l
@@ -267,7 +301,7 @@ bool make_plan_uncached(const rc_config &cfg, int nm, bool line, int nx, int ny,
     P.bc_below = cur; cur += align_up((size_t)P.Lpad * P.NM * sizeof(float));  // [Lpad][NM]: one value per channel
     P.bc_above = cur; cur += align_up((size_t)P.Lpad * P.NM * sizeof(float));
     P.weights = cur;  cur += align_up(P.Lpad * sizeof(float));
-    P.flag = cur;     cur += ALIGN;
+    P.flag = cur;     cur += 2 * ALIGN;  // scalar flags and counters: [0..15] scratch, [16..31] segments walked per cascade
     if (host_io) {
         const size_t io = align_up(ncell * L * sizeof(float));
         P.io_chi = cur; cur += io;
@@ -279,18 +313,17 @@ bool make_plan_uncached(const rc_config &cfg, int nm, bool line, int nx, int ny,
 }
 
 // The plan is pure host arithmetic but not free (choose_patch); the last few are remembered.
-bool make_plan(const rc_config &cfg, int nm, bool line, int nx, int ny, int L, bool host_io, Plan &P,
+bool make_plan(const rc_config &cfg, const Tuning &tune, int nm, bool line, int nx, int ny, int L, bool host_io, Plan &P,
                std::vector<std::vector<long long>> *offs) {
     struct Entry { double k[13]; Plan p; };
     static thread_local std::vector<Entry> cache;
-    if (offs) return make_plan_uncached(cfg, nm, line, nx, ny, L, host_io, P, offs);
-    const char *e1 = std::getenv("RC_BANDS"), *e2 = std::getenv("RC_L2_MB");
+    if (offs) return make_plan_uncached(cfg, tune, nm, line, nx, ny, L, host_io, P, offs);
     const double k[13] = {(double)cfg.ncascades, (double)cfg.lambda_batch, (double)cfg.flags, (double)nm, (double)line,
                           (double)nx, (double)ny, (double)L, (double)host_io, (double)cfg.c0_interval,
-                          e1 ? std::atof(e1) : -1.0, e2 ? std::atof(e2) : -1.0, 0.0};
+                          (double)tune.bands, tune.l2_mb, 0.0};
     for (const Entry &e : cache)
         if (std::equal(k, k + 13, e.k)) { P = e.p; return true; }
-    if (!make_plan_uncached(cfg, nm, line, nx, ny, L, host_io, P, nullptr)) return false;
+    if (!make_plan_uncached(cfg, tune, nm, line, nx, ny, L, host_io, P, nullptr)) return false;
     if (cache.size() >= 16) cache.erase(cache.begin());
     Entry en;
     std::copy(k, k + 13, en.k);
@@ -316,7 +349,7 @@ int rc_plan_query(const rc_config *cfg, int ninclinations, int line_mode, int nx
         return RC_ERR_BAD_VALUE;
     if (ninclinations != 1 && ninclinations != 2 && ninclinations != 4 && ninclinations != 8) return RC_ERR_BAD_VALUE;
     Plan P;
-    if (!make_plan(*cfg, ninclinations, line_mode != 0, nx, ny, nlambda, false, P, nullptr)) return RC_ERR_BAD_SHAPE;
+    if (!make_plan(*cfg, Tuning{}, ninclinations, line_mode != 0, nx, ny, nlambda, false, P, nullptr)) return RC_ERR_BAD_SHAPE;
     std::memset(out, 0, sizeof(*out));
     out->workspace_bytes = P.total;
     out->lambda_batch = P.LV;
@@ -353,11 +386,6 @@ int rc_create(rc_ctx **out, const rc_config *cfg) {
     rc_ctx *ctx = new (std::nothrow) rc_ctx();
     if (!ctx) return RC_ERR_CUDA;
     ctx->cfg = *cfg;
-    if (const char *e = std::getenv("RC_MARCH_VARIANT")) ctx->tune_variant = std::max(0, std::min(4, std::atoi(e)));
-    if (const char *e = std::getenv("RC_PATCH_LOG2")) ctx->tune_patch = std::max(2, std::min(5, std::atoi(e)));
-    if (const char *e = std::getenv("RC_PATCH_FROM")) ctx->tune_patch_from = std::atoi(e);
-    if (const char *e = std::getenv("RC_CPW_FROM")) ctx->tune_cpw = std::atoi(e);
-    if (const char *e = std::getenv("RC_TAU_CUT")) ctx->tau_cut = std::max(1.f, (float)std::atof(e));
     *out = ctx;
     return RC_OK;
 }
@@ -375,9 +403,9 @@ int rc_destroy(rc_ctx *ctx) {
 size_t rc_workspace_bytes(const rc_ctx *ctx, int nx, int ny, int nlambda, int host_io) {
     if (!ctx) return 0;
     Plan P;
-    if (!make_plan(ctx->cfg, ctx->nm, false, nx, ny, nlambda, host_io != 0, P, nullptr)) return 0;
+    if (!make_plan(ctx->cfg, ctx->tune, ctx->nm, false, nx, ny, nlambda, host_io != 0, P, nullptr)) return 0;
     size_t need = P.total;
-    if (make_plan(ctx->cfg, ctx->nm, true, nx, ny, nlambda, false, P, nullptr)) need = std::max(need, P.total);  // line mode
+    if (make_plan(ctx->cfg, ctx->tune, ctx->nm, true, nx, ny, nlambda, false, P, nullptr)) need = std::max(need, P.total);  // line mode
     return need;
 }
 
@@ -396,6 +424,30 @@ int rc_set_stream(rc_ctx *ctx, void *cuda_stream) {
     if (!ctx) return RC_ERR_NULL_ARG;
     ctx->stream = (cudaStream_t)cuda_stream;
     return RC_OK;
+}
+
+int rc_set_tuning(rc_ctx *ctx, const char *name, double value) {
+    if (!ctx || !name) return RC_ERR_NULL_ARG;
+    Tuning &t = ctx->tune;
+    const std::string n(name);
+    const int iv = (int)std::lround(value);
+    if (n == "march_variant") { if (iv < -1 || iv > 4) goto bad; t.variant = iv; }
+    else if (n == "patch_log2") { if (iv != -1 && (iv < 2 || iv > 5)) goto bad; t.patch_log2 = iv; }
+    else if (n == "patch_from") { if (iv < 0) goto bad; t.patch_from = iv; }
+    else if (n == "cpw_from") { if (iv < -1) goto bad; t.cpw_from = iv; t.cpw_forced = true; }
+    else if (n == "tau_cut") { if (!(value >= 1.0)) goto bad; t.tau_cut = (float)value; }
+    else if (n == "bands") { if (iv < 0) goto bad; t.bands = iv; }
+    else if (n == "l2_mb") { if (!(value >= 1.0)) goto bad; t.l2_mb = value; }
+    else if (n == "sparse") { if (iv < -1 || iv > 1) goto bad; t.sparse = iv; }
+    else if (n == "graph") { t.graph = iv != 0; }
+    else if (n == "sparse_mode") { if (iv < 0 || iv > 1) goto bad; t.sparse_mode = iv; }
+    else return fail(ctx, RC_ERR_BAD_VALUE, "rc_set_tuning: unknown knob '%s'", name);
+    // the plan (bands), the patch lists and a captured graph may depend on a knob: start over
+    ctx->have_atm = false;
+    ctx->active_set = false; ctx->lists_dirty = false; ctx->sparse = false;
+    return RC_OK;
+bad:
+    return fail(ctx, RC_ERR_BAD_VALUE, "rc_set_tuning: %s = %g is out of range", name, value);
 }
 
 int rc_set_timing(rc_ctx *ctx, int nsets) {
@@ -423,13 +475,15 @@ static int prepare_shape(rc_ctx *ctx, int nx, int ny, int nlambda, bool line) {
     if (!same_shape) {
         Plan P, Pio;
         std::vector<std::vector<long long>> offs;
-        make_plan(ctx->cfg, ctx->nm, line, nx, ny, nlambda, false, P, &offs);
+        make_plan(ctx->cfg, ctx->tune, ctx->nm, line, nx, ny, nlambda, false, P, &offs);
         if (P.total > ctx->ws_bytes)
             return fail(ctx, RC_ERR_NO_WORKSPACE, "workspace has %zu bytes, %zu needed", ctx->ws_bytes, P.total);
-        make_plan(ctx->cfg, ctx->nm, line, nx, ny, nlambda, true, Pio, nullptr);
+        make_plan(ctx->cfg, ctx->tune, ctx->nm, line, nx, ny, nlambda, true, Pio, nullptr);
         ctx->host_io = Pio.total <= ctx->ws_bytes;
         ctx->plan = ctx->host_io ? Pio : P;
         ctx->have_atm = false;
+        ctx->active_set = false; ctx->lists_dirty = false; ctx->sparse = false;
+        ctx->stats.active_cells = -1;
         // geometry tables: only when the grid size changed (they do not depend on nlambda)
         if (ctx->tab_nx != nx || ctx->tab_ny != ny) {
             ctx->off_host.swap(offs);
@@ -481,19 +535,8 @@ int rc_set_atmosphere(rc_ctx *ctx, const float *chi, const float *eta, int nx, i
         RC_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
         if (h & 1) return fail(ctx, RC_ERR_BAD_VALUE, "chi or eta has a negative or non-finite value");
     }
-    {
-        // sparsity (many models are mostly empty): with more than two thirds of the cells at
-        // chi == 0 for every wavelength the march tests an occupancy bitmap before each gather
-        unsigned long long *cnt = (unsigned long long *)(ctx->ws + ctx->plan.flag);
-        unsigned long long h = 0;
-        ctx->sparse = false;
-        RC_CUDA(ctx, cudaMemsetAsync(cnt, 0, sizeof(*cnt), ctx->stream));
-        RC_CUDA(ctx, rc::launch_count_empty(chi, eta, (long long)nx * ny, nlambda, (int *)(ctx->ws + ctx->plan.A[0]), cnt, ctx->stream));  // A[0] is free between solves
-        RC_CUDA(ctx, cudaMemcpyAsync(&h, cnt, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream));
-        RC_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
-        if (ctx->plan.has_occ && !std::getenv("RC_NO_SPARSE")) ctx->sparse = 3 * h > 2ULL * nx * ny || std::getenv("RC_FORCE_SPARSE");
-        ctx->stats.empty_cells = (int64_t)h;
-    }
+    ctx->sparse = false;  // the distance field belongs to the atmosphere it was built from: rc_analyse_atmosphere again
+    ctx->stats.sparse_march = 0;
     ctx->chi = chi;
     ctx->eta = eta;
     ctx->have_atm = true;
@@ -514,8 +557,12 @@ int rc_set_line_atmosphere(rc_ctx *ctx, const float *line, int nx, int ny, const
         h[l] = (float)((double)x_lambda[l] * 1.2011224087864498);  // sqrt(log2 e)
         h[(size_t)ctx->plan.Lpad + l] = x_lambda[l];
     }
-    RC_CUDA(ctx, cudaMemcpyAsync(ctx->ws + ctx->plan.xls, h.data(), h.size() * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
-    RC_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    if (h != ctx->xl_stage) {  // steady state (same wavelengths again): nothing to upload, nothing to wait for
+        RC_CUDA(ctx, cudaStreamSynchronize(ctx->stream));  // an earlier upload may still be reading xl_stage
+        ctx->xl_stage.swap(h);
+        RC_CUDA(ctx, cudaMemcpyAsync(ctx->ws + ctx->plan.xls, ctx->xl_stage.data(), ctx->xl_stage.size() * sizeof(float),
+                                     cudaMemcpyHostToDevice, ctx->stream));
+    }
     ctx->line = line;
     ctx->chi = ctx->eta = nullptr;
     ctx->sparse = false;
@@ -589,7 +636,7 @@ int rc_set_lambda_weights(rc_ctx *ctx, const float *w) {
 
 // Register-ring depth / occupancy variant of cascade i's march launch (rc_kernels.cu, launch_march_flat): measured
 // on config 2, short rays (cascades <= 3) like 20 warps/SM with a ring of 2, long rays 16 warps/SM with a ring of 3.
-static int march_variant(const rc_ctx *ctx, int i) { return ctx->tune_variant >= 0 ? ctx->tune_variant : (i <= 3 ? 4 : 2); }
+static int march_variant(const rc_ctx *ctx, int i) { return ctx->tune.variant >= 0 ? ctx->tune.variant : (i <= 3 ? 4 : 2); }
 
 // Parameters of cascade i's march launch.
 static rc::MarchParams march_params(const rc_ctx *ctx, int i, float *J_out) {
@@ -602,7 +649,12 @@ static rc::MarchParams march_params(const rc_ctx *ctx, int i, float *J_out) {
     mp.ST = (const float *)(ctx->ws + P.ST);
     mp.linepk = ctx->line ? (const float *)(ctx->ws + P.chiT) : nullptr;
     mp.xls = ctx->line ? (const float *)(ctx->ws + P.xls) : nullptr;
-    mp.occ = ctx->sparse && P.has_occ && !c.empty ? (const unsigned *)(ctx->ws + P.occ) : nullptr;
+    mp.dist = ctx->sparse ? (const unsigned char *)(ctx->ws + P.dist) : nullptr;
+    mp.sparse_mode = ctx->tune.sparse_mode;
+    mp.walked = ctx->count_walked ? (unsigned long long *)(ctx->ws + P.flag) + 16 + i : nullptr;
+    mp.flags = ctx->active_set ? (const unsigned char *)(ctx->ws + P.pflag[i]) : nullptr;
+    mp.plist = ctx->active_set && !ctx->lists_dirty ? (const int *)(ctx->ws + P.plist[i]) : nullptr;
+    mp.npatch_act = ctx->npatch_act[i];
     mp.Aup = i == top ? nullptr : (const float *)(ctx->ws + P.A[(i + 1) & 1]);
     mp.out = i > 0 ? (float *)(ctx->ws + P.A[i & 1]) : (accum ? (float *)(ctx->ws + P.Jpart) : J_out);
     mp.steps = c.empty ? nullptr : (const rc::Step *)(ctx->ws + c.steps_off);
@@ -618,8 +670,8 @@ static rc::MarchParams march_params(const rc_ctx *ctx, int i, float *J_out) {
     mp.ngroups = 1 << (2 * i);
     mp.mode = i > 0 ? 0 : (accum ? 2 : 1);
     mp.early_exit = (ctx->cfg.flags & RC_NO_EARLY_EXIT) ? 0 : 1;
-    mp.tau_cut = ctx->tau_cut;
-    mp.pw_log2 = ctx->tune_patch >= 0 && i >= ctx->tune_patch_from ? ctx->tune_patch : c.pw_log2;
+    mp.tau_cut = ctx->tune.tau_cut;
+    mp.pw_log2 = ctx->tune.patch_log2 >= 0 && i >= ctx->tune.patch_from ? ctx->tune.patch_log2 : c.pw_log2;
     mp.fix = c.fix && !c.empty;
     mp.subdir = mp.fix ? (const float2 *)(ctx->ws + c.subdir_off) : nullptr;
     const int lx = mp.fix ? mp.npx >> 1 : mp.npx, ly = mp.fix ? mp.npy >> 1 : mp.npy;  // lane lattice
@@ -633,12 +685,36 @@ static rc::MarchParams march_params(const rc_ctx *ctx, int i, float *J_out) {
     // ... nor on a cascade that barely reaches into the box (config 2, cascade 6: 0.014 % of its rays are live)
     const double diag = std::sqrt((double)P.nx * P.nx + (double)P.ny * P.ny);
     const bool reaches = std::fmin(c.tb, diag) - c.ta > 0.2 * c.ta || i == 0;
-    mp.cpw = J_out != nullptr && ctx->tune_cpw >= 0 && i >= ctx->tune_cpw && !c.empty && (reaches || std::getenv("RC_CPW_FROM")) &&
+    mp.cpw = J_out != nullptr && ctx->tune.cpw_from >= 0 && i >= ctx->tune.cpw_from && !c.empty && (reaches || ctx->tune.cpw_forced) && !ctx->sparse &&
              P.NM == 1 && !ctx->line ? 1 : 0;
     for (int m = 0; m < 8; m++) { mp.incl_f[m] = ctx->incl_f[m]; mp.incl_w[m] = ctx->incl_w[m]; mp.incl_s[m] = 1.f / ctx->incl_f[m]; }
     mp.state = nullptr;
     mp.band_axis = 0; mp.band_sign = 1; mp.band_lo = 0; mp.band_hi = 0; mp.band_final = 1;
     return mp;
+}
+
+// Compacted patch lists ("the radiance intervals are only computed for these flagged probes"): for every
+// cascade the numbers of the patches - in the numbering of the march's own warp -> probe mapping - that hold a flagged
+// probe.  Synchronises (the counts size the launches).
+static int build_patch_lists(rc_ctx *ctx) {
+    const Plan &P = ctx->plan;
+    ctx->lists_dirty = true;  // march_params must describe the full patch grid while the lists are built
+    int *cnt = (int *)(ctx->ws + P.pcount);
+    for (int i = 0; i < ctx->cfg.ncascades; i++) {
+        rc::MarchParams mp = march_params(ctx, i, nullptr);
+        mp.nb = 1; mp.cpw = 0; mp.plist = nullptr;
+        const long long npatch = (long long)mp.npatch_x * mp.npatch_y * (mp.fix ? 4 : 1);
+        if (npatch > P.plist_cap[i]) return fail(ctx, RC_ERR_CUDA, "patch list of cascade %d: %lld > capacity %d", i, npatch, P.plist_cap[i]);
+        RC_CUDA(ctx, rc::launch_mark_and_compact_patches(mp, (int)npatch, (unsigned char *)(ctx->ws + P.pmark), (int *)(ctx->ws + P.plist[i]),
+                                                         cnt + i, ctx->stream));
+    }
+    int h[RC_MAX_CASCADES];
+    RC_CUDA(ctx, cudaMemcpyAsync(h, cnt, sizeof(int) * ctx->cfg.ncascades, cudaMemcpyDeviceToHost, ctx->stream));
+    RC_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    for (int i = 0; i < ctx->cfg.ncascades; i++) ctx->npatch_act[i] = h[i];
+    ctx->lists_dirty = false;
+    ctx->list_version++;
+    return RC_OK;
 }
 
 // One full solve: for cascade i = top .. 0 { pack chi/eta for spacing 2^i ; march + merge }  (PAPER.md:207:
@@ -652,25 +728,35 @@ static int enqueue_solve(rc_ctx *ctx, float *J_out) {
     cudaEvent_t *ev = ctx->nsets > 0 ? ctx->ev.data() + (size_t)(ctx->solves_timed % ctx->nsets) * per : nullptr;
     int launches = 0;
     if (ev) RC_CUDA(ctx, cudaEventRecord(ev[0], ctx->stream));
+    if (ctx->active_set) {
+        // J is computed on the cells of interest only: the others read 0
+        const size_t ncell = (size_t)P.nx * P.ny;
+        if (accum) RC_CUDA(ctx, cudaMemsetAsync(ctx->ws + P.Jpart, 0, ncell * P.nb * sizeof(float), ctx->stream));
+        else RC_CUDA(ctx, cudaMemsetAsync(J_out, 0, ncell * P.L * sizeof(float), ctx->stream));
+    }
+    auto pack = [&](int shift) -> int {
+        rc::PackParams pp;
+        pp.chi = ctx->chi; pp.eta = ctx->eta;
+        pp.chiT = (float *)(ctx->ws + P.chiT); pp.ST = (float *)(ctx->ws + P.ST);
+        pp.active = ctx->active_set ? (const unsigned char *)(ctx->ws + P.pflag[0]) : nullptr;
+        pp.nx = P.nx; pp.ny = P.ny; pp.L = P.L; pp.nb = P.nb; pp.shift = shift;
+        if (ctx->line) {
+            pp.chi = ctx->line; pp.eta = nullptr;
+            RC_CUDA(ctx, rc::launch_pack_line(pp, ctx->stream));
+        } else {
+            RC_CUDA(ctx, rc::launch_pack(pp, P.LV, ctx->stream));
+        }
+        launches++;
+        return RC_OK;
+    };
+    // the distance-field march gathers from plain cell order: one pack for every cascade
+    if (ctx->sparse) { const int rc = pack(0); if (rc != RC_OK) return rc; }
     for (int i = top; i >= 0; i--) {
         const CascadePlan &c = P.c[i];
-        if (!c.empty) {
-            rc::PackParams pp;
-            pp.chi = ctx->chi; pp.eta = ctx->eta;
-            pp.chiT = (float *)(ctx->ws + P.chiT); pp.ST = (float *)(ctx->ws + P.ST);
-            pp.occ = ctx->sparse && P.has_occ ? (unsigned *)(ctx->ws + P.occ) : nullptr;
-            pp.nx = P.nx; pp.ny = P.ny; pp.L = P.L; pp.nb = P.nb; pp.shift = c.fix ? i + 1 : i;
-            if (ctx->line) {
-                pp.chi = ctx->line; pp.eta = nullptr; pp.occ = nullptr;
-                RC_CUDA(ctx, rc::launch_pack_line(pp, ctx->stream));
-            } else {
-                RC_CUDA(ctx, rc::launch_pack(pp, P.LV, ctx->stream));
-            }
-            launches++;
-        }
+        if (!c.empty && !ctx->sparse) { const int rc = pack(c.fix ? i + 1 : i); if (rc != RC_OK) return rc; }
         if (ev) RC_CUDA(ctx, cudaEventRecord(ev[1 + 2 * (top - i)], ctx->stream));
         rc::MarchParams mp = march_params(ctx, i, J_out);
-        if (!c.banded) {
+        if (!c.banded || ctx->sparse) {  // the distance-field march gathers occupied cells only: they fit L2
             RC_CUDA(ctx, rc::launch_march(mp, P.LV * P.NM, P.NM, march_variant(ctx, i), ctx->stream));
             launches++;
         } else {
@@ -715,8 +801,9 @@ int rc_solve_J(rc_ctx *ctx, float *J_out) {
     if (!ctx || !J_out) return ctx ? fail(ctx, RC_ERR_NULL_ARG, "null J_out") : RC_ERR_NULL_ARG;
     if (!ctx->have_atm) return fail(ctx, RC_ERR_NO_ATMOSPHERE, "call rc_set_atmosphere first");
     RC_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    if (ctx->lists_dirty) { const int rc = build_patch_lists(ctx); if (rc != RC_OK) return rc; }
     const Plan &P = ctx->plan;
-    bool use_graph = ctx->nsets == 0 && (long long)P.nx * P.ny * P.Lpad * P.NM <= (1LL << 21) && !std::getenv("RC_NO_GRAPH");
+    bool use_graph = ctx->nsets == 0 && (long long)P.nx * P.ny * P.Lpad * P.NM <= (1LL << 21) && ctx->tune.graph != 0;
     if (use_graph) {
         cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
         if (cudaStreamIsCapturing(ctx->stream, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) {
@@ -728,7 +815,7 @@ int rc_solve_J(rc_ctx *ctx, float *J_out) {
     rc_ctx::GraphKey key;
     std::memset(&key, 0, sizeof(key));
     key.J = J_out; key.chi = ctx->chi; key.eta = ctx->eta; key.line = ctx->line; key.ws = ctx->ws;
-    key.nx = P.nx; key.ny = P.ny; key.L = P.L; key.nm = P.NM; key.sparse = ctx->sparse; key.total = P.total;
+    key.nx = P.nx; key.ny = P.ny; key.L = P.L; key.nm = P.NM; key.sparse = (ctx->sparse ? 1 : 0) + (ctx->active_set ? 2 : 0) + 4 * ctx->list_version; key.total = P.total;
     for (int m = 0; m < 8; m++) { key.f[m] = ctx->incl_f[m]; key.w[m] = ctx->incl_w[m]; }
     if (!ctx->graph_exec || std::memcmp(&key, &ctx->graph_key, sizeof(key)) != 0) {
         if (ctx->graph_exec) { cudaGraphExecDestroy(ctx->graph_exec); ctx->graph_exec = nullptr; }
@@ -753,6 +840,68 @@ int rc_solve_J(rc_ctx *ctx, float *J_out) {
     return RC_OK;
 }
 
+// Sparsity as the paper defines it.
+int rc_set_active_cells(rc_ctx *ctx, const unsigned char *active) {
+    if (!ctx) return RC_ERR_NULL_ARG;
+    if (!ctx->have_atm) return fail(ctx, RC_ERR_NO_ATMOSPHERE, "call rc_set_atmosphere first");
+    RC_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    const Plan &P = ctx->plan;
+    ctx->sparse = false;  // the distance field depends on the flags
+    if (!active) {
+        ctx->active_set = false; ctx->lists_dirty = false;
+        ctx->stats.active_cells = -1;
+        ctx->list_version++;
+        return RC_OK;
+    }
+    const int top = ctx->cfg.ncascades - 1;
+    RC_CUDA(ctx, rc::launch_flags_from_active(active, (unsigned char *)(ctx->ws + P.pflag[0]), (long long)P.nx * P.ny, ctx->stream));
+    for (int i = 0; i < top; i++) {
+        RC_CUDA(ctx, cudaMemsetAsync(ctx->ws + P.pflag[i + 1], 0, (size_t)(P.nx >> (i + 1)) * (P.ny >> (i + 1)), ctx->stream));
+        RC_CUDA(ctx, rc::launch_flag_parents((const unsigned char *)(ctx->ws + P.pflag[i]), P.nx >> i, P.ny >> i,
+                                             (unsigned char *)(ctx->ws + P.pflag[i + 1]), ctx->stream));
+    }
+    ctx->active_set = true;
+    {
+        const int rc = build_patch_lists(ctx);
+        if (rc != RC_OK) { ctx->active_set = false; return rc; }
+    }
+    // flagged probes per cascade, for the statistics
+    for (int i = 0; i <= top; i++) {
+        std::vector<unsigned char> h((size_t)(P.nx >> i) * (P.ny >> i));
+        RC_CUDA(ctx, cudaMemcpy(h.data(), ctx->ws + P.pflag[i], h.size(), cudaMemcpyDeviceToHost));
+        int64_t n = 0;
+        for (unsigned char v : h) n += v;
+        ctx->stats.probes_flagged[i] = n;
+    }
+    ctx->stats.active_cells = ctx->stats.probes_flagged[0];
+    return RC_OK;
+}
+
+// Free-space acceleration: occupancy and its distance transform for the current atmosphere and flags.
+int rc_analyse_atmosphere(rc_ctx *ctx) {
+    if (!ctx) return RC_ERR_NULL_ARG;
+    if (!ctx->have_atm) return fail(ctx, RC_ERR_NO_ATMOSPHERE, "call rc_set_atmosphere first");
+    RC_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    const Plan &P = ctx->plan;
+    unsigned long long *cnt = (unsigned long long *)(ctx->ws + P.flag);
+    unsigned long long h = 0;
+    RC_CUDA(ctx, rc::launch_build_distance_field(ctx->chi, ctx->eta, ctx->line,
+                                                 ctx->active_set ? (const unsigned char *)(ctx->ws + P.pflag[0]) : nullptr, P.nx, P.ny, P.L,
+                                                 (int *)(ctx->ws + P.A[0]), (unsigned char *)(ctx->ws + P.occ8), (unsigned char *)(ctx->ws + P.d1),
+                                                 (unsigned char *)(ctx->ws + P.dist), cnt, ctx->stream));  // A[0] is free between solves
+    RC_CUDA(ctx, cudaMemcpyAsync(&h, cnt, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream));
+    RC_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    ctx->stats.empty_cells = (int64_t)h;
+    ctx->analysed = true;
+    // the distance-field march exists for the plain mode (no inclinations, no moving line, no bilinear fix)
+    const bool can = P.NM == 1 && !ctx->line && !(ctx->cfg.flags & RC_BILINEAR_FIX);
+    const bool want = ctx->tune.sparse >= 0 ? ctx->tune.sparse != 0 : 3 * h > 2ULL * P.nx * P.ny;
+    ctx->sparse = can && want;
+    ctx->stats.sparse_march = ctx->sparse;
+    ctx->list_version++;
+    return RC_OK;
+}
+
 // Geometric segment count per cascade and wavelength (the unit of the throughput metric).
 int rc_count_segments(rc_ctx *ctx, int64_t *per_cascade) {
     if (!ctx || !per_cascade) return ctx ? fail(ctx, RC_ERR_NULL_ARG, "null output") : RC_ERR_NULL_ARG;
@@ -769,6 +918,50 @@ int rc_count_segments(rc_ctx *ctx, int64_t *per_cascade) {
     return RC_OK;
 }
 
+// One solve with counters: the cell segments the march integrated (early exit, sparsity and free-space jumps leave the
+// rest out), per cascade, summed over the wavelength batches and divided by their number.
+int rc_count_walked(rc_ctx *ctx, float *J_out, int64_t *per_cascade) {
+    if (!ctx || !J_out || !per_cascade) return ctx ? fail(ctx, RC_ERR_NULL_ARG, "null argument") : RC_ERR_NULL_ARG;
+    if (!ctx->have_atm) return fail(ctx, RC_ERR_NO_ATMOSPHERE, "call rc_set_atmosphere first");
+    RC_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    if (ctx->lists_dirty) { const int rc = build_patch_lists(ctx); if (rc != RC_OK) return rc; }
+    unsigned long long *d = (unsigned long long *)(ctx->ws + ctx->plan.flag) + 16;
+    RC_CUDA(ctx, cudaMemsetAsync(d, 0, 16 * sizeof(*d), ctx->stream));
+    ctx->count_walked = true;
+    const int rc = enqueue_solve(ctx, J_out);
+    ctx->count_walked = false;
+    if (rc != RC_OK) return rc;
+    unsigned long long h[16];
+    RC_CUDA(ctx, cudaMemcpyAsync(h, d, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream));
+    RC_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    for (int i = 0; i < ctx->cfg.ncascades; i++) per_cascade[i] = (int64_t)(h[i] / (unsigned long long)ctx->plan.nb);
+    return RC_OK;
+}
+
+// Line mode with HOST buffers: line_host [ny][nx][6], J_host as rc_solve_J_host.
+int rc_solve_J_line_host(rc_ctx *ctx, const float *line_host, int nx, int ny, const float *x_lambda, int nlambda, float *J_host) {
+    if (!ctx || !line_host || !x_lambda || !J_host) return ctx ? fail(ctx, RC_ERR_NULL_ARG, "null host buffer") : RC_ERR_NULL_ARG;
+    if (!shape_ok(ctx->cfg, nx, ny, nlambda)) return fail(ctx, RC_ERR_BAD_SHAPE, "bad shape %dx%dx%d", nx, ny, nlambda);
+    if (!ctx->ws) return fail(ctx, RC_ERR_NO_WORKSPACE, "rc_set_workspace has not been called");
+    RC_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    Plan Pio;
+    make_plan(ctx->cfg, ctx->tune, ctx->nm, false, nx, ny, nlambda, true, Pio, nullptr);  // the host_io region of the GivenFs plan holds both
+    if (Pio.total > ctx->ws_bytes)
+        return fail(ctx, RC_ERR_NO_WORKSPACE, "workspace has %zu bytes, %zu needed with host_io", ctx->ws_bytes, Pio.total);
+    const size_t nline = (size_t)nx * ny * 6 * sizeof(float);
+    float *dline = (float *)(ctx->ws + Pio.io_chi), *dJ = (float *)(ctx->ws + Pio.io_J);
+    if (nline > Pio.io_J - Pio.io_chi) return fail(ctx, RC_ERR_NO_WORKSPACE, "host_io region too small for the line parameters");
+    RC_CUDA(ctx, cudaMemcpyAsync(dline, line_host, nline, cudaMemcpyHostToDevice, ctx->stream));
+    int rc = rc_set_line_atmosphere(ctx, dline, nx, ny, x_lambda, nlambda);
+    if (rc != RC_OK) return rc;
+    rc = rc_solve_J(ctx, dJ);
+    if (rc != RC_OK) return rc;
+    const size_t nout = (size_t)nx * ny * ((ctx->cfg.flags & RC_ACCUM_J) ? 1 : nlambda) * sizeof(float);
+    RC_CUDA(ctx, cudaMemcpyAsync(J_host, dJ, nout, cudaMemcpyDeviceToHost, ctx->stream));
+    RC_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return RC_OK;
+}
+
 int rc_solve_J_host(rc_ctx *ctx, const float *chi_host, const float *eta_host, int nx, int ny,
                     int nlambda, float *J_host) {
     if (!ctx || !chi_host || !eta_host || !J_host) return ctx ? fail(ctx, RC_ERR_NULL_ARG, "null host buffer") : RC_ERR_NULL_ARG;
@@ -776,7 +969,7 @@ int rc_solve_J_host(rc_ctx *ctx, const float *chi_host, const float *eta_host, i
     if (!ctx->ws) return fail(ctx, RC_ERR_NO_WORKSPACE, "rc_set_workspace has not been called");
     RC_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
     Plan Pio;
-    make_plan(ctx->cfg, ctx->nm, false, nx, ny, nlambda, true, Pio, nullptr);
+    make_plan(ctx->cfg, ctx->tune, ctx->nm, false, nx, ny, nlambda, true, Pio, nullptr);
     if (Pio.total > ctx->ws_bytes)
         return fail(ctx, RC_ERR_NO_WORKSPACE, "workspace has %zu bytes, %zu needed with host_io", ctx->ws_bytes, Pio.total);
     const size_t n = (size_t)nx * ny * nlambda * sizeof(float);
@@ -785,6 +978,7 @@ int rc_solve_J_host(rc_ctx *ctx, const float *chi_host, const float *eta_host, i
     RC_CUDA(ctx, cudaMemcpyAsync(deta, eta_host, n, cudaMemcpyHostToDevice, ctx->stream));
     int rc = rc_set_atmosphere(ctx, dchi, deta, nx, ny, nlambda);
     if (rc != RC_OK) return rc;
+    if (ctx->analysed) { rc = rc_analyse_atmosphere(ctx); if (rc != RC_OK) return rc; }
     rc = rc_solve_J(ctx, dJ);
     if (rc != RC_OK) return rc;
     const size_t nout = (ctx->cfg.flags & RC_ACCUM_J) ? (size_t)nx * ny * sizeof(float) : n;

@@ -34,7 +34,13 @@ struct MarchParams {
     const float *ST;    // packed source function eta/chi, same layout
     const float *linepk;  // null, or line mode: packed line parameters [s][s][npy][npx][6] (pack_line_kernel)
     const float *xls;     // line mode: [Lpad] wavelengths x_l * sqrt(log2 e), device
-    const unsigned *occ;  // null (dense), or the occupancy bitmap pack_kernel wrote: empty cells are not gathered
+    const unsigned char *dist;  // null (lock-step march), or [ny][nx] Chebyshev distance to the nearest occupied cell (0 = occupied):
+                                // every lane walks its own ray and jumps over empty space; packed arrays in cell order (shift 0)
+    int sparse_mode;            // launch variant of the distance-field march (rc_kernels.cu, launch_march_sparse)
+    unsigned long long *walked; // null, or a counter of the cell segments actually integrated (rc_count_walked; per wavelength batch)
+    const unsigned char *flags; // null (every probe), or [npy][npx]: the flagged probes of this cascade
+    const int *plist;           // null, or the numbers of the patches that hold a flagged probe (npatch_act of them)
+    int npatch_act;
     const float *Aup;   // merged cascade i+1, pre-averaged over the 4 children: [nb][N_i][npy/2][npx/2][LV]; null on the top cascade
     float *out;         // mode 0: A_i [nb][N_i/4][npy][npx][LV]; mode 1: J [ny][nx][L]; mode 2: Jpart [nb][ny][nx]
     const Step *steps;
@@ -69,7 +75,7 @@ struct MarchParams {
 struct PackParams {
     const float *chi, *eta;  // [ny][nx][L]
     float *chiT, *ST;        // [nb][s][s][npy][npx][LV]
-    unsigned *occ;           // null, or [nb][nx ny / 32]: bit = packed cell has chi > 0 at some wavelength of the batch
+    const unsigned char *active;  // null, or [ny][nx]: cells that are not flagged are packed as vacuum
     int nx, ny, L, nb, shift;
 };
 
@@ -104,7 +110,12 @@ cudaError_t launch_table_build(const TableBuildParams &p, cudaStream_t st);
 cudaError_t launch_reduce_jbar(const float *Jpart, float *Jbar, long long ncell, int nb, cudaStream_t st);
 cudaError_t launch_count(const MarchParams &p, unsigned long long *total, cudaStream_t st);
 cudaError_t launch_gather_probe(const float *buf, unsigned long long nsector, int iters, int blocks, float *sink, cudaStream_t st);
-cudaError_t launch_count_empty(const float *chi, const float *eta, long long ncell, int L, int *mark, unsigned long long *count, cudaStream_t st);
+cudaError_t launch_flags_from_active(const unsigned char *active, unsigned char *flag0, long long ncell, cudaStream_t st);
+cudaError_t launch_flag_parents(const unsigned char *child, int npx, int npy, unsigned char *parent, cudaStream_t st);
+cudaError_t launch_mark_and_compact_patches(const MarchParams &p, int npatch, unsigned char *mark, int *list, int *count, cudaStream_t st);
+cudaError_t launch_build_distance_field(const float *chi, const float *eta, const float *line, const unsigned char *active, int nx, int ny,
+                                        int L, int *mark, unsigned char *occ, unsigned char *d1, unsigned char *dist,
+                                        unsigned long long *nempty, cudaStream_t st);
 cudaError_t launch_alo(const AloParams &p, cudaStream_t st);
 cudaError_t launch_bulk_probe(const float *buf, unsigned long long nsector, int iters, int sms, float *sink, cudaStream_t st, long long *bytes);
 cudaError_t launch_validate(const float *chi, const float *eta, long long n, int *flag, cudaStream_t st);

@@ -17,10 +17,11 @@
 //                       the DDA itself), radiance in fp32, I and T never leave registers.
 //                       Template switches: NM inclinations per wavelength (2.5D), PD = depth
 //                       of the register ring the gathers run ahead in, BANDED (grids larger than L2: one
-//                       band of rows/columns per launch, ray state parked in between), SPARSE (occupancy
-//                       bitmap in front of every gather), LINE (opacity evaluated per ray
+//                       band of rows/columns per launch, ray state parked in between), LINE (opacity evaluated per ray
 //                       from the projected velocity).  Run-time switch: the bilinear fix
 //                       (4 sub-rays per interval, 16 tables per direction).
+//   march_fan_kernel    the same for mostly empty atmospheres: lanes = a fan of adjacent directions,
+//                       every lane walks its own ray and jumps over free space on a distance field.
 //   pack_line_kernel, alo_kernel, reduce_jbar_kernel, validate / mark_occupied / count_* kernels: small
 //                       elementwise or counting passes;  gather_probe_kernel, bulk_probe_kernel: the
 //                       march's gather pattern alone, through LDG.256 and through TMA bulk copies, for
@@ -261,14 +262,10 @@ __global__ void __launch_bounds__(256) pack_kernel(PackParams p) {
         c2[v] = cf * 1.4426950408889634f;                // tau in units of ln 2: T = 2^-tau2
         S[v] = et[v] > 0.f ? et[v] / cf : 0.f;
     }
-    if (p.occ != nullptr) {
-        // occupancy bitmap of the packed cells of this batch (ncell is a multiple of 32 when occ is given, so a
-        // warp's 32 consecutive cells are one word): bit = some wavelength of the batch has chi > 0
-        bool nz = false;
+    if (p.active != nullptr && __ldg(p.active + (long long)y * p.nx + x) == 0) {
+        // sparsity: "non-flagged cells are treated as transparent with no emission"
 #pragma unroll
-        for (int v = 0; v < LV; v++) nz = nz || c2[v] != 0.f;
-        const unsigned w = __ballot_sync(FULL, nz);
-        if ((threadIdx.x & 31) == 0) p.occ[idx >> 5] = w;
+        for (int v = 0; v < LV; v++) { c2[v] = 0.f; S[v] = 0.f; }
     }
     float *oc = p.chiT + idx * LV, *os = p.ST + idx * LV;
     if constexpr (LV == 8) {
@@ -305,7 +302,8 @@ __global__ void __launch_bounds__(256) pack_line_kernel(PackParams p) {
     const float2 *src = reinterpret_cast<const float2 *>(p.chi + ((long long)y * p.nx + x) * 6);
     const float2 a = __ldg(src), b = __ldg(src + 1), v = __ldg(src + 2);
     const float L2E = 1.4426950408889634f, RSPI = 0.5641895835477563f, SL2E = 1.2011224087864498f;
-    const float cc = a.x * L2E, cl = b.x * L2E * RSPI;
+    float cc = a.x * L2E, cl = b.x * L2E * RSPI;
+    if (p.active != nullptr && __ldg(p.active + (long long)y * p.nx + x) == 0) { cc = 0.f; cl = 0.f; }  // not flagged: vacuum
     float2 *dst = reinterpret_cast<float2 *>(p.chiT + c * 6);
     dst[0] = make_float2(cc, cc * a.y);
     dst[1] = make_float2(cl, cl * b.y);
@@ -459,12 +457,14 @@ __device__ __forceinline__ WarpWork warp_work(const MarchParams &p, long long W,
     if (p.cpw) W >>= 2;  // child-per-warp: 4 consecutive warps (one per child direction) share everything else
     const int G = min(p.kg_n, 8);
     const int ncls = p.fix ? 4 : 1;
-    const long long npatch = (long long)p.npatch_x * p.npatch_y * ncls;
+    const long long npatch = p.plist != nullptr ? p.npatch_act : (long long)p.npatch_x * p.npatch_y * ncls;
     WarpWork r;
     const int kg_lo = (int)(W % G);
     W /= G;
     long long patch = W % npatch;
     W /= npatch;
+    // sparsity: only the patches that hold a flagged probe are launched (plist: their numbers, in order)
+    if (p.plist != nullptr) patch = __ldg(p.plist + patch);
     r.cls = (int)(patch % ncls);
     patch /= ncls;
     const int kgb_n = p.kg_n / G;
@@ -481,12 +481,15 @@ __device__ __forceinline__ WarpWork warp_work(const MarchParams &p, long long W,
     r.a = p.fix ? 2 * la + (r.cls & 1) : la;
     r.b = p.fix ? 2 * lb + (r.cls >> 1) : lb;
     r.gidx = (unsigned)lb * lx + la;
+    // a probe that is not flagged computes nothing and writes nothing; nothing flagged ever reads it
+    if (r.valid && p.flags != nullptr) r.valid = __ldg(p.flags + (long long)r.b * p.npx + r.a) != 0;
     if (!r.valid) { r.a = r.cls & 1; r.b = r.cls >> 1; r.gidx = 0; }
     return r;
 }
 
 __host__ __device__ inline long long march_warps(const MarchParams &p) {
-    return (long long)p.npatch_x * p.npatch_y * (p.fix ? 4 : 1) * p.kg_n * p.nb * (p.cpw ? 4 : 1);
+    const long long npatch = p.plist != nullptr ? p.npatch_act : (long long)p.npatch_x * p.npatch_y * (p.fix ? 4 : 1);
+    return npatch * p.kg_n * p.nb * (p.cpw ? 4 : 1);
 }
 
 // Number of leading steps of direction k's table that lie inside the box for this lane's probe.
@@ -535,7 +538,7 @@ __device__ __forceinline__ int first_step_reaching(const StepXY *xy, int n, int 
 // half of the directions that crosses the bands in ascending (or descending) order; a ray's (I, tau)
 // is carried from band to band through `state`, so the arithmetic - and the result - is that of the
 // unbanded launch, bit for bit, while the cells gathered by one launch fit L2.
-template <int LV, int NM, int PD, int WARPS, int MINB, bool BANDED, bool SPARSE, bool LINE>
+template <int LV, int NM, int PD, int WARPS, int MINB, bool BANDED, bool LINE>
 __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) {
     // sum over the 4 child directions, per thread: parked in shared memory between children so the
     // marching loop has the registers to itself
@@ -564,7 +567,6 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
 #pragma unroll
         for (int v = 0; v < LL; v++) xs[v] = __ldg(p.xls + nbI * LL + v);
     }
-    const unsigned *occB = SPARSE ? p.occ + (long long)nbI * (ncell >> 5) : nullptr;
     // (dx, dy) ranges that keep this lane's ray inside the box
     const int dxlo = -(a << p.shift) - half, dxhi = ((p.npx - a) << p.shift) - 1 - half;
     const int dylo = -Y0, dyhi = p.ny - 1 - Y0;
@@ -598,8 +600,8 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
                 const int dx = (int)(short)(e & 0xffffu), dy = (int)(short)(e >> 16);
                 if (dx < dxlo || dx > dxhi || dy < dylo || dy > dyhi) nin = 0;
             }
-            int n0 = 0;       // this lane's first step of this launch
             bool has = true;  // banded: the lane has steps in this band
+            int n0 = 0;       // this lane's first step of this launch
             if constexpr (BANDED) {
                 const int c0 = p.band_axis ? (a << p.shift) + half : Y0;
                 const int sg = p.band_sign;
@@ -652,22 +654,11 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
 #pragma unroll
                 for (int v = 0; v < (LINE ? 1 : LL); v++) S[u][v] = 0.f;
                 const uint2 e = __ldg(tab + u);
-                bool in = u < nin && (!BANDED || u >= n0);
-                if constexpr (SPARSE) {  // empty cells (chi = 0 at every wavelength of the batch) are not gathered
-                    const unsigned c = gidx + e.x;
-                    if (in) in = (__ldg(occB + (c >> 5)) >> (c & 31)) & 1u;
-                }
+                const bool in = u < nin && (!BANDED || u >= n0);
                 gather(u, e.x, in);
                 ds[u] = in ? __uint_as_float(e.y) : 0.f;
             }
             int chk = 0;
-            // SPARSE: the table entry and the occupancy word of the NEXT step to gather, read one step early
-            uint2 en_next = make_uint2(0u, 0u);
-            unsigned occ_next = 0u;
-            if constexpr (SPARSE) {
-                en_next = __ldg(tab + PD);
-                if (PD < nin && (!BANDED || PD >= n0)) occ_next = __ldg(occB + ((gidx + en_next.x) >> 5));
-            }
             // the channels of a lane two at a time (FFMA2 / FADD2 / FMUL2).  Pair q holds, when the lane has at least two
             // wavelengths, inclination q % NM of wavelengths 2 (q / NM) and 2 (q / NM) + 1 (two neighbouring gathered values,
             // one path length); with a single wavelength, inclinations 2q and 2q + 1 of it (one gathered value, two lengths)
@@ -685,21 +676,11 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
                 }
             }
             // a1: eq. 16 along the interval, front to back, seg_update*() per cell and channel
+            int st_done = nw;  // steps the warp took (early exit: fewer)
             for (int st = 0; st < nw; st += PD) {
 #pragma unroll
                 for (int u = 0; u < PD; u++) {
-                    uint2 en;
-                    unsigned occ_cur = 0u;
-                    if constexpr (SPARSE) {
-                        en = en_next;
-                        occ_cur = occ_next;
-                        en_next = __ldg(tab + st + u + PD + 1);
-                        occ_next = 0u;
-                        if (st + u + PD + 1 < nin && (!BANDED || st + u + PD + 1 >= n0))
-                            occ_next = __ldg(occB + ((gidx + en_next.x) >> 5));
-                    } else {
-                        en = __ldg(tab + st + u + PD);
-                    }
+                    const uint2 en = __ldg(tab + st + u + PD);
                     // integrate step st + u (a slot past the lane's last in-box step has ds = 0: no effect)
                     // 2.5D: inclination m crosses the same cell over ds / sin(inclination)
                     float dsm[NM], dkm[NM];
@@ -723,7 +704,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
                             const float num = fmaf(c2[u][3], phi, c2[u][1]);
                             seg_update_line(chi2, num, dsm[v % NM], dkm[v % NM], tau[v], T[v], I[v]);
                         }
-                    } else if (!SPARSE || __any_sync(FULL, ds[u] != 0.f)) {  // SPARSE: no lane has an occupied cell: nothing to do
+                    } else {
                         if constexpr (PACKED) {
 #pragma unroll
                             for (int q = 0; q < NP; q++) {
@@ -743,8 +724,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
                         }
                     }
                     // refill the slot with step st + u + PD
-                    bool in = st + u + PD < nin && (!BANDED || st + u + PD >= n0);
-                    if constexpr (SPARSE) in = in && ((occ_cur >> ((gidx + en.x) & 31)) & 1u);
+                    const bool in = st + u + PD < nin && (!BANDED || st + u + PD >= n0);
                     gather(u, en.x, in);
                     ds[u] = in ? __uint_as_float(en.y) : 0.f;
                 }
@@ -757,8 +737,13 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
 #pragma unroll
                     for (int v = 1; v < LV; v++) tmin = fminf(tmin, tau[v]);
                     // every live lane opaque at every wavelength: T is exactly 0, nothing more can arrive
-                    if (__all_sync(FULL, st + PD >= nin || tmin > p.tau_cut)) break;
+                    if (__all_sync(FULL, st + PD >= nin || tmin > p.tau_cut)) { st_done = st + PD; break; }
                 }
+            }
+            if (p.walked != nullptr) {  // measurement only (rc_count_walked): in-box steps this launch integrated
+                unsigned long long mine = (unsigned long long)max(0, min(nin, st_done) - n0);
+                for (int sh = 16; sh > 0; sh >>= 1) mine += __shfl_down_sync(FULL, mine, sh);
+                if (lane == 0 && mine) atomicAdd(p.walked, mine);
             }
             if constexpr (PACKED) {
 #pragma unroll
@@ -885,32 +870,202 @@ template <int LV, int NM, int PD, int WARPS, int MINB>
 static cudaError_t launch_march_variant(const MarchParams &p, cudaStream_t st) {
     const long long blocks = (march_warps(p) + WARPS - 1) / WARPS;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+    if (blocks == 0) return cudaSuccess;  // sparsity: no flagged probe in this cascade
     if (p.state != nullptr)
-        march_kernel<LV, NM, PD, WARPS, MINB, true, false, false><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
+        march_kernel<LV, NM, PD, WARPS, MINB, true, false><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
     else
-        march_kernel<LV, NM, PD, WARPS, MINB, false, false, false><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
+        march_kernel<LV, NM, PD, WARPS, MINB, false, false><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
     return cudaGetLastError();
 }
 
 // variant: 0 = ring of 2 steps, 24 warps/SM (<= 80 registers); 1 = ring of 3, 20 warps/SM (<= 96, blocks of 4 warps);
 //          2 = ring of 3, 16 warps/SM (<= 128); 3 = ring of 4, 16 warps/SM (<= 128); 4 = ring of 2, 20 warps/SM (<= 96)
-// Mostly-empty atmospheres (occ != null): the occupancy test in front of every gather.  Ring of 2, 24 warps/SM
-// (the dependent chain occupancy word -> predicate -> gather wants warps more than depth); variant 3: ring of 3, 16 warps/SM.
-template <int LV, int PD, int MINB>
-static cudaError_t launch_march_sparse_v(const MarchParams &p, cudaStream_t st) {
-    constexpr int WARPS = 8;
-    const long long blocks = (march_warps(p) + WARPS - 1) / WARPS;
-    if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-    if (p.state != nullptr)
-        march_kernel<LV, 1, PD, WARPS, MINB, true, true, false><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
-    else
-        march_kernel<LV, 1, PD, WARPS, MINB, false, true, false><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
-    return cudaGetLastError();
+// ------------------------------------------------------------------------------------------------
+// Mostly empty atmospheres ("accelerating the traversal of long-range radiance intervals through
+// free-space"): the FAN march.  The packed arrays are in plain cell order (shift 0) and every lane walks its OWN ray: it
+// looks its cell up in `dist` - the Chebyshev distance to the nearest occupied cell, 0 = occupied - and jumps over the
+// steps that cannot meet one; only occupied cells are gathered and integrated.  An empty cell changes no bit of
+// (tau, T, I), so the result is that of the lock-step march, bit for bit.
+//   Lanes: a warp takes min(32, N_i) ADJACENT DIRECTIONS of one probe (and 32 / N_i neighbouring probes on cascades 0
+// and 1).  Rays of a fan meet the same structure at nearly the same steps, so the lanes of a warp have similar work -
+// with 32 probes of one direction (the lock-step mapping; 32-128 cells apart on the heavy cascades) a warp waited for
+// its one lane inside a blob - and neighbouring lanes look up and gather neighbouring (often the same) cells.
+//   Jump: after j steps the ray is at most j m + 2 cells (Chebyshev) from where it was, m = max(|wx|, |wy|) / (|wx| +
+// |wy|) (j crossings of grid lines, shared between the axes in proportion, each count within one of its expectation);
+// the cells closer than r are empty, so the steps before n + 1 + (r - 3)/m - and in any case before n + r, one cell per
+// step - are skipped unseen.  Cascade 0's diagonals move one cell in x and y per step: m = 1.
+//   The in-box prefix of the step table is not searched for: a ray ends at the first step outside the box.
+// ------------------------------------------------------------------------------------------------
+template <int LV, int WARPS, int MINB>
+__global__ void __launch_bounds__(WARPS * 32, MINB) march_fan_kernel(MarchParams p) {
+    const int lane = threadIdx.x & 31;
+    long long W = (long long)blockIdx.x * WARPS + (threadIdx.x >> 5);
+    const long long ndir = 4LL * p.ngroups;
+    const int ndl = (int)min(32LL, ndir), ppw = 32 / ndl;       // directions and probes per warp
+    const long long nprobe = (long long)p.npx * p.npy;
+    const long long ndb = ndir / ndl, npb = (nprobe + ppw - 1) / ppw;
+    // warp order: direction block (fastest: the fans of one probe share cells near it), probe block, wavelength batch
+    const long long db = W % ndb;
+    W /= ndb;
+    const long long pb = W % npb;
+    const int nbI = (int)(W / npb);
+    if (nbI >= p.nb) return;
+    const long long k = db * ndl + (lane % ndl);
+    const long long probe = pb * ppw + lane / ndl;
+    bool valid = probe < nprobe;
+    const int b = valid ? (int)(probe / p.npx) : 0, a = valid ? (int)(probe - (long long)b * p.npx) : 0;
+    // a probe that is not flagged computes nothing and writes nothing; nothing flagged ever reads it
+    if (valid && p.flags != nullptr) valid = __ldg(p.flags + probe) != 0;
+    if (!__any_sync(FULL, valid)) return;
+    const int half = (1 << p.shift) >> 1;
+    const int X0 = (a << p.shift) + half, Y0 = (b << p.shift) + half;
+    const long long ncell = (long long)p.nx * p.ny;
+    const float *chiB = p.chiT + (long long)nbI * ncell * LV, *SB = p.ST + (long long)nbI * ncell * LV;
+
+    float I[LV], tau[LV], T[LV];
+#pragma unroll
+    for (int v = 0; v < LV; v++) { I[v] = 0.f; tau[v] = 0.f; T[v] = 1.f; }
+    unsigned nwalk = 0;
+    if (p.cnt != nullptr && valid) {  // cnt == null: the cascade lies outside any box of this size (boundary term only)
+        const long long o = __ldg(p.off + k);
+        const int n = __ldg(p.cnt + k);
+        const uint2 *tab = reinterpret_cast<const uint2 *>(p.steps + o);
+        const unsigned *xyt = reinterpret_cast<const unsigned *>(p.xy + o);
+        float invm = 1.f;
+        if (p.cascade > 0) {
+            float sw, cw;
+            sincospif(2.f * ((float)k + 0.5f) / (float)ndir, &sw, &cw);
+            sw = fabsf(sw); cw = fabsf(cw);
+            invm = 0.999f * (sw + cw) / fmaxf(sw, cw);
+        }
+        int sn = 0;
+        bool pend = false;
+        float cP[LV], SP[LV], dsP = 0.f;
+#pragma unroll
+        for (int v = 0; v < LV; v++) { cP[v] = 0.f; SP[v] = 0.f; }
+        while (true) {
+            bool found = false;
+            int cf = 0;
+            while (sn < n) {  // next occupied step of this lane's ray
+                const unsigned e = __ldg(xyt + sn);
+                const int x = X0 + (int)(short)(e & 0xffffu), y = Y0 + (int)(short)(e >> 16);
+                if ((unsigned)x >= (unsigned)p.nx || (unsigned)y >= (unsigned)p.ny) { sn = n; break; }  // left the box: for good
+                cf = y * p.nx + x;
+                const int r = __ldg(p.dist + cf);
+                if (r == 0) { found = true; break; }
+                sn += max(r, 1 + (int)((float)(r - 3) * invm));
+            }
+            float cN[LV], SN[LV], dsN = 0.f;
+#pragma unroll
+            for (int v = 0; v < LV; v++) { cN[v] = 0.f; SN[v] = 0.f; }
+            if (found) {
+                const unsigned long long d = (unsigned long long)cf * (LV * sizeof(float));
+                load_vec<LV>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(chiB) + d), cN);
+                load_vec<LV>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(SB) + d), SN);
+                dsN = __uint_as_float(__ldg(tab + sn).y);
+                sn++;
+            }
+            if (pend) {  // integrate the cell gathered one round earlier
+                nwalk++;
+                const float dkP = dsP * KAPPA;
+                if constexpr (LV >= 2) {
+#pragma unroll
+                    for (int q = 0; q < LV / 2; q++) {
+                        f32x2 t2 = pk2(tau[2 * q], tau[2 * q + 1]), T2 = pk2(T[2 * q], T[2 * q + 1]), I2 = pk2(I[2 * q], I[2 * q + 1]);
+                        seg_update2(pk2(cP[2 * q], cP[2 * q + 1]), pk2(SP[2 * q], SP[2 * q + 1]), pk2(dsP, dsP), pk2(dkP, dkP), t2, T2, I2);
+                        up2(t2, tau[2 * q], tau[2 * q + 1]);
+                        up2(T2, T[2 * q], T[2 * q + 1]);
+                        up2(I2, I[2 * q], I[2 * q + 1]);
+                    }
+                } else {
+                    seg_update1(cP[0], SP[0], dsP, dkP, tau[0], T[0], I[0]);
+                }
+                if (p.early_exit) {  // this ray is opaque at every wavelength: nothing more can arrive
+                    float tmin = tau[0];
+#pragma unroll
+                    for (int v = 1; v < LV; v++) tmin = fminf(tmin, tau[v]);
+                    if (tmin > p.tau_cut) { sn = n; found = false; }
+                }
+            }
+            if (!found) break;  // per lane: nothing pending any more, nothing ahead
+            pend = true;
+            dsP = dsN;
+#pragma unroll
+            for (int v = 0; v < LV; v++) { cP[v] = cN[v]; SP[v] = SN[v]; }
+        }
+    }
+    if (p.walked != nullptr) {
+        unsigned long long mine = nwalk;
+        for (int sh = 16; sh > 0; sh >>= 1) mine += __shfl_down_sync(FULL, mine, sh);
+        if (lane == 0 && mine) atomicAdd(p.walked, mine);
+    }
+    // a2 (top cascade: boundary intensity) or a3 (bilinear parents, eq. 11): as in march_kernel
+    if (valid) {
+        if (p.Aup == nullptr) {
+            const float *Ib = (2 * k < ndir) ? p.I_above : p.I_below;
+#pragma unroll
+            for (int v = 0; v < LV; v++) I[v] = fmaf(T[v], __ldg(Ib + nbI * LV + v), I[v]);
+        } else {
+            const int npxu = p.npx >> 1, npyu = p.npy >> 1;
+            int a0, a1, b0, b1;
+            float fa, fb;
+            parent_axis(a, npxu, a0, a1, fa);
+            parent_axis(b, npyu, b0, b1, fb);
+            const float *up = p.Aup + (((long long)nbI * ndir + k) * npyu) * (long long)npxu * LV;
+            float u00[LV], u01[LV], u10[LV], u11[LV];
+            load_vec<LV>(up + ((long long)b0 * npxu + a0) * LV, u00);
+            load_vec<LV>(up + ((long long)b0 * npxu + a1) * LV, u01);
+            load_vec<LV>(up + ((long long)b1 * npxu + a0) * LV, u10);
+            load_vec<LV>(up + ((long long)b1 * npxu + a1) * LV, u11);
+#pragma unroll
+            for (int v = 0; v < LV; v++) {
+                const float lo = fmaf(fa, u01[v] - u00[v], u00[v]);
+                const float hi = fmaf(fa, u11[v] - u10[v], u10[v]);
+                I[v] = fmaf(T[v], fmaf(fb, hi - lo, lo), I[v]);
+            }
+        }
+    }
+    // mean over the 4 children of a direction group: 4 neighbouring lanes, added in child order like the lock-step march
+    float acc[LV];
+#pragma unroll
+    for (int v = 0; v < LV; v++) {
+        const float m1 = __shfl_down_sync(FULL, I[v], 1), m2 = __shfl_down_sync(FULL, I[v], 2), m3 = __shfl_down_sync(FULL, I[v], 3);
+        acc[v] = 0.25f * ((((0.f + I[v]) + m1) + m2) + m3);
+    }
+    if (!valid || (lane & 3) != 0) return;
+    const long long kg = k >> 2;
+    if (p.mode == 0) {
+        store_vec<LV>(p.out + (((long long)nbI * p.ngroups + kg) * nprobe + probe) * LV, acc);
+    } else if (p.mode == 1) {  // cascade 0: a4, J
+        float *o = p.out + probe * p.L + nbI * LV;
+        if ((nbI + 1) * LV <= p.L && (p.L % LV) == 0) {
+            store_vec<LV>(o, acc);
+        } else {
+#pragma unroll
+            for (int v = 0; v < LV; v++)
+                if (nbI * LV + v < p.L) o[v] = acc[v];
+        }
+    } else {
+        float sum = 0.f;
+#pragma unroll
+        for (int v = 0; v < LV; v++) sum = fmaf(__ldg(p.weights + nbI * LV + v), acc[v], sum);
+        p.out[(long long)nbI * nprobe + probe] = sum;
+    }
 }
 
 template <int LV>
-static cudaError_t launch_march_sparse(const MarchParams &p, int variant, cudaStream_t st) {
-    return variant == 3 ? launch_march_sparse_v<LV, 3, 2>(p, st) : launch_march_sparse_v<LV, 2, 3>(p, st);  // measured: 559 vs 599 ms on config 4
+static cudaError_t launch_march_sparse(const MarchParams &p, cudaStream_t st) {
+    constexpr int WARPS = 8;
+    const long long ndir = 4LL * p.ngroups, ndl = ndir < 32 ? ndir : 32, ppw = 32 / ndl;
+    const long long nprobe = (long long)p.npx * p.npy;
+    const long long warps = (ndir / ndl) * ((nprobe + ppw - 1) / ppw) * p.nb;
+    const long long blocks = (warps + WARPS - 1) / WARPS;
+    if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+    if (blocks == 0) return cudaSuccess;
+    // sparse_mode 1: 16 warps/SM at <= 128 registers instead of 24 at <= 80
+    if (p.sparse_mode & 1) march_fan_kernel<LV, WARPS, 2><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
+    else march_fan_kernel<LV, WARPS, 3><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
+    return cudaGetLastError();
 }
 
 // Velocity-dependent line mode (linepk != null): 3 MUFU per segment-channel, ring of 2, 24 warps/SM.
@@ -919,14 +1074,15 @@ static cudaError_t launch_march_line(const MarchParams &p, cudaStream_t st) {
     constexpr int WARPS = 8;
     const long long blocks = (march_warps(p) + WARPS - 1) / WARPS;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-    march_kernel<LV, NM, 2, WARPS, 3, false, false, true><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
+    if (blocks == 0) return cudaSuccess;
+    march_kernel<LV, NM, 2, WARPS, 3, false, true><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
     return cudaGetLastError();
 }
 
 template <int LV>
 static cudaError_t launch_march_flat(const MarchParams &p, int variant, cudaStream_t st) {
     if (p.linepk != nullptr) return launch_march_line<LV>(p, st);
-    if (p.occ != nullptr) return launch_march_sparse<LV>(p, variant, st);
+    if (p.dist != nullptr) return launch_march_sparse<LV>(p, st);
     switch (variant) {
         case 0: return launch_march_variant<LV, 1, 2, 8, 3>(p, st);
         case 1: return launch_march_variant<LV, 1, 3, 4, 5>(p, st);
@@ -997,47 +1153,173 @@ __global__ void validate_kernel(const float *chi, const float *eta, long long n,
     if (bad) atomicOr(flag, bad);
 }
 
-// Number of cells with chi == 0 at every wavelength (is the atmosphere mostly empty?).
-// Pass 1 marks the cells that have a non-zero value (coalesced over the whole array), pass 2 counts the rest.
-template <int W>  // floats per thread: 4 when nlambda is a multiple of 4, else 1
-__global__ void mark_occupied_kernel(const float *chi, long long nchunk, int chunks_per_cell, int *mark) {
+// Marks the cells that hold a non-zero value (coalesced over the whole array).  W floats per thread: 4 when the
+// row width is a multiple of 4, else 1; `posmask`: bit (position within the cell's row, mod 32) set = position counts
+// (all of chi / eta; in line mode positions 0 and 2 of the six parameters, chi_c and chi_line).
+template <int W>
+__global__ void mark_occupied_kernel(const float *f, long long nchunk, int chunks_per_cell, int *mark, unsigned posmask) {
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < nchunk; i += (long long)gridDim.x * blockDim.x) {
         bool nz;
         if constexpr (W == 4) {
-            const float4 v = __ldg(reinterpret_cast<const float4 *>(chi) + i);
+            const float4 v = __ldg(reinterpret_cast<const float4 *>(f) + i);
             nz = v.x != 0.f || v.y != 0.f || v.z != 0.f || v.w != 0.f;
         } else {
-            nz = __ldg(chi + i) != 0.f;
+            nz = __ldg(f + i) != 0.f && (chunks_per_cell > 32 || ((posmask >> (unsigned)(i % chunks_per_cell)) & 1u));
         }
         if (nz) mark[i / chunks_per_cell] = 1;
     }
 }
 
-__global__ void count_unmarked_kernel(const int *mark, long long ncell, unsigned long long *count) {
-    unsigned long long mine = 0;
-    for (long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x; c < ncell; c += (long long)gridDim.x * blockDim.x)
-        mine += mark[c] == 0;
-    for (int o = 16; o > 0; o >>= 1) mine += __shfl_down_sync(FULL, mine, o);
-    if ((threadIdx.x & 31) == 0 && mine) atomicAdd(count, mine);
-}
-
-// mark: scratch of ncell ints (device); count: zeroed by the caller
-cudaError_t launch_count_empty(const float *chi, const float *eta, long long ncell, int L, int *mark, unsigned long long *count, cudaStream_t st) {
-    cudaError_t e = cudaMemsetAsync(mark, 0, sizeof(int) * (size_t)ncell, st);
-    if (e != cudaSuccess) return e;
-    // a cell is empty when chi and eta vanish at every wavelength (emission without opacity counts, reading G11)
-    for (const float *f : {chi, eta}) {
-        if (L % 4 == 0 && (reinterpret_cast<uintptr_t>(f) & 15) == 0)
-            mark_occupied_kernel<4><<<148 * 16, 256, 0, st>>>(f, ncell * (L / 4), L / 4, mark);
-        else
-            mark_occupied_kernel<1><<<148 * 16, 256, 0, st>>>(f, ncell * L, L, mark);
-    }
-    count_unmarked_kernel<<<148 * 4, 256, 0, st>>>(mark, ncell, count);
+cudaError_t launch_validate(const float *chi, const float *eta, long long n, int *flag, cudaStream_t st) {
+    validate_kernel<<<148 * 8, 256, 0, st>>>(chi, eta, n, flag);
     return cudaGetLastError();
 }
 
-cudaError_t launch_validate(const float *chi, const float *eta, long long n, int *flag, cudaStream_t st) {
-    validate_kernel<<<148 * 8, 256, 0, st>>>(chi, eta, n, flag);
+// ------------------------------------------------------------------------------------------------
+// Sparsity as the paper defines it: "this flag then defines the probes of cascade 0 that may be involved
+// ... Their bilinear "parents" are recursively flagged up to the maximum cascade, and the radiance intervals are only
+// computed for these flagged probes".
+// ------------------------------------------------------------------------------------------------
+// flag[0] = the cells of interest (any non-zero byte), as 0 / 1
+__global__ void flags_from_active_kernel(const unsigned char *active, unsigned char *flag0, long long ncell) {
+    const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c < ncell) flag0[c] = active[c] != 0;
+}
+
+// every flagged probe of cascade i flags its four bilinear parents in cascade i+1 (stores of the same value: no race)
+__global__ void flag_parents_kernel(const unsigned char *child, int npx, int npy, unsigned char *parent) {
+    const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= (long long)npx * npy || child[c] == 0) return;
+    const int b = (int)(c / npx), a = (int)(c - (long long)b * npx), upx = npx >> 1, upy = npy >> 1;
+    int a0, a1, b0, b1;
+    float f;
+    parent_axis(a, upx, a0, a1, f);
+    parent_axis(b, upy, b0, b1, f);
+    parent[(long long)b0 * upx + a0] = 1; parent[(long long)b0 * upx + a1] = 1;
+    parent[(long long)b1 * upx + a0] = 1; parent[(long long)b1 * upx + a1] = 1;
+}
+
+// one warp per patch of the march's own warp -> probe mapping (warp_work): does the patch hold a flagged probe?
+__global__ void mark_patches_kernel(MarchParams p, unsigned char *mark, int npatch) {
+    const int lane = threadIdx.x & 31;
+    const long long W = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    if (W >= npatch) return;
+    // p arrives with kg_n = ngroups, nb = 1, cpw = 0, plist = null: warp W * G is direction group 0 of patch W
+    const WarpWork ww = warp_work(p, W * min(p.kg_n, 8), lane);
+    const unsigned any = __ballot_sync(FULL, ww.valid);
+    if (lane == 0) mark[W] = any != 0u;
+}
+
+// ordered compaction of the marked patch numbers by one block (setup time only): list[0 .. *count)
+__global__ void __launch_bounds__(1024) compact_patches_kernel(const unsigned char *mark, int n, int *list, int *count) {
+    __shared__ int wsum[32];
+    __shared__ int base;
+    if (threadIdx.x == 0) base = 0;
+    __syncthreads();
+    for (int start = 0; start < n; start += 1024) {
+        const int i = start + threadIdx.x;
+        const int m = i < n && mark[i] != 0;
+        const unsigned bal = __ballot_sync(FULL, m);
+        const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+        if (lane == 0) wsum[w] = __popc(bal);
+        __syncthreads();
+        int off = base;
+        for (int q = 0; q < w; q++) off += wsum[q];
+        if (m) list[off + __popc(bal & ((1u << lane) - 1u))] = i;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            int t = 0;
+            for (int q = 0; q < 32; q++) t += wsum[q];
+            base += t;
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) *count = base;
+}
+
+cudaError_t launch_flags_from_active(const unsigned char *active, unsigned char *flag0, long long ncell, cudaStream_t st) {
+    flags_from_active_kernel<<<(unsigned)((ncell + 255) / 256), 256, 0, st>>>(active, flag0, ncell);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_flag_parents(const unsigned char *child, int npx, int npy, unsigned char *parent, cudaStream_t st) {
+    const long long n = (long long)npx * npy;
+    flag_parents_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(child, npx, npy, parent);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_mark_and_compact_patches(const MarchParams &p, int npatch, unsigned char *mark, int *list, int *count, cudaStream_t st) {
+    mark_patches_kernel<<<(unsigned)(((long long)npatch * 32 + 255) / 256), 256, 0, st>>>(p, mark, npatch);
+    compact_patches_kernel<<<1, 1024, 0, st>>>(mark, npatch, list, count);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
+// Free-space acceleration: occupancy of the cells (flagged, and chi or eta non-zero at some
+// wavelength) and its Chebyshev distance transform, clamped at 255: dist = 0 on an occupied cell, else the distance to
+// the nearest one.  Setup time only; separable brute force with early termination.
+// ------------------------------------------------------------------------------------------------
+__global__ void occupancy_kernel(const int *mark, const unsigned char *active, unsigned char *occ, long long ncell, unsigned long long *nempty) {
+    const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    bool e = false;
+    if (c < ncell) {
+        const bool o = mark[c] != 0 && (active == nullptr || active[c] != 0);
+        occ[c] = o;
+        e = !o;
+    }
+    const unsigned bal = __ballot_sync(FULL, e);
+    if ((threadIdx.x & 31) == 0 && bal) atomicAdd(nempty, (unsigned long long)__popc(bal));
+}
+
+// d1[y][x] = distance along the row to the nearest occupied cell of row y (255: none within 254)
+__global__ void dist_rows_kernel(const unsigned char *occ, unsigned char *d1, int nx, int ny) {
+    const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= (long long)nx * ny) return;
+    const int y = (int)(c / nx), x = (int)(c - (long long)y * nx);
+    const unsigned char *row = occ + (long long)y * nx;
+    int best = 255;
+    for (int r = 0; r < best; r++)
+        if ((x - r >= 0 && row[x - r]) || (x + r < nx && row[x + r])) { best = r; break; }
+    d1[c] = (unsigned char)best;
+}
+
+// dist[y][x] = min over rows y' of max(|y - y'|, d1[y'][x])
+__global__ void dist_cols_kernel(const unsigned char *d1, unsigned char *dist, int nx, int ny) {
+    const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= (long long)nx * ny) return;
+    const int y = (int)(c / nx);
+    int best = d1[c];
+    for (int r = 1; r < best; r++) {
+        if (y - r >= 0) best = min(best, max(r, (int)d1[c - (long long)r * nx]));
+        if (y + r < ny) best = min(best, max(r, (int)d1[c + (long long)r * nx]));
+    }
+    dist[c] = (unsigned char)best;
+}
+
+// mark: scratch of ncell ints; d1: scratch of ncell bytes; occ, dist: ncell bytes each; nempty: zeroed here
+cudaError_t launch_build_distance_field(const float *chi, const float *eta, const float *line, const unsigned char *active, int nx, int ny,
+                                        int L, int *mark, unsigned char *occ, unsigned char *d1, unsigned char *dist,
+                                        unsigned long long *nempty, cudaStream_t st) {
+    const long long ncell = (long long)nx * ny;
+    cudaError_t e = cudaMemsetAsync(mark, 0, sizeof(int) * (size_t)ncell, st);
+    if (e != cudaSuccess) return e;
+    e = cudaMemsetAsync(nempty, 0, sizeof(*nempty), st);
+    if (e != cudaSuccess) return e;
+    // a cell is empty when chi and eta vanish at every wavelength (emission without opacity counts, reading G11);
+    // line mode: the six line parameters, of which chi_c and chi_line decide - S and v alone emit and absorb nothing
+    const float *fields[2] = {line ? line : chi, line ? nullptr : eta};
+    const int width = line ? 6 : L;
+    for (const float *f : fields) {
+        if (f == nullptr) continue;
+        if (!line && width % 4 == 0 && (reinterpret_cast<uintptr_t>(f) & 15) == 0)
+            mark_occupied_kernel<4><<<148 * 16, 256, 0, st>>>(f, ncell * (width / 4), width / 4, mark, 0xf);
+        else
+            mark_occupied_kernel<1><<<148 * 16, 256, 0, st>>>(f, ncell * width, width, mark, line ? 0x5 : 0xffffffffu);
+    }
+    const unsigned blocks = (unsigned)((ncell + 255) / 256);
+    occupancy_kernel<<<blocks, 256, 0, st>>>(mark, active, occ, ncell, nempty);
+    dist_rows_kernel<<<blocks, 256, 0, st>>>(occ, d1, nx, ny);
+    dist_cols_kernel<<<blocks, 256, 0, st>>>(d1, dist, nx, ny);
     return cudaGetLastError();
 }
 
@@ -1049,7 +1331,7 @@ cudaError_t launch_validate(const float *chi, const float *eta, long long n, int
 __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) count_kernel(MarchParams p, unsigned long long *total) {
     const int lane = threadIdx.x & 31;
     const long long W = (long long)blockIdx.x * WARPS_PER_BLOCK + (threadIdx.x >> 5);
-    if (W >= (long long)p.npatch_x * p.npatch_y * (p.fix ? 4 : 1) * p.ngroups || p.cnt == nullptr) return;
+    if (W >= (p.plist != nullptr ? (long long)p.npatch_act : (long long)p.npatch_x * p.npatch_y * (p.fix ? 4 : 1)) * p.ngroups || p.cnt == nullptr) return;
     const WarpWork ww = warp_work(p, W, lane);  // batch index is the slowest: W covers batch 0 only
     const int a = ww.a, b = ww.b, kg = ww.kg;
     const int s = 1 << p.shift, half = s >> 1;
@@ -1074,9 +1356,10 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) count_kernel(MarchParams
 }
 
 cudaError_t launch_count(const MarchParams &p, unsigned long long *total, cudaStream_t st) {
-    const long long nwarps = (long long)p.npatch_x * p.npatch_y * (p.fix ? 4 : 1) * p.ngroups;
+    const long long nwarps = (p.plist != nullptr ? (long long)p.npatch_act : (long long)p.npatch_x * p.npatch_y * (p.fix ? 4 : 1)) * p.ngroups;
     const long long blocks = (nwarps + WARPS_PER_BLOCK - 1) / WARPS_PER_BLOCK;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+    if (blocks == 0) return cudaSuccess;
     count_kernel<<<(unsigned)blocks, WARPS_PER_BLOCK * 32, 0, st>>>(p, total);
     return cudaGetLastError();
 }

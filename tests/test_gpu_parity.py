@@ -191,17 +191,17 @@ def test_segment_counts_match_the_oracle(oracle):
 # ------------------------------------------------------------------ launch variants
 @pytest.mark.parametrize("variant", [0, 1, 2, 3, 4])
 @pytest.mark.parametrize("patch", [None, 2, 3, 4, 5])
-def test_patch_shapes_and_ring_depths_are_bit_identical(oracle, monkeypatch, variant, patch):
+def test_patch_shapes_and_ring_depths_are_bit_identical(oracle, variant, patch):
     """The lane patch (32x1 .. 4x8 probes per warp) and the register-ring depth / occupancy variant of
     march_kernel only change which lane marches which ray and how far ahead it gathers: every ray's
     arithmetic is the same, so J is bit-identical to the default launch, and within TOL of the oracle.
     Non-square grid with a ragged last wavelength batch; 6 cascades so that the top ones are clipped."""
     atm = A.make_config(3, nx=192, ny=128, nlambda=11, ncascades=6, seed=5)
     ref = gpu_solve(atm)
-    monkeypatch.setenv("RC_MARCH_VARIANT", str(variant))
+    knobs = dict(march_variant=variant)
     if patch is not None:
-        monkeypatch.setenv("RC_PATCH_LOG2", str(patch))
-    got = gpu_solve(atm)
+        knobs["patch_log2"] = patch
+    got = gpu_solve(atm, tuning=knobs)
     assert np.array_equal(ref, got)
     if variant == 0 and patch is None:
         Jo = oracle.solve_atmosphere(atm)["J"]
@@ -210,21 +210,17 @@ def test_patch_shapes_and_ring_depths_are_bit_identical(oracle, monkeypatch, var
 
 @pytest.mark.parametrize("nx,ny", [(192, 128), (128, 192), (128, 128)])
 @pytest.mark.parametrize("bands", [2, 3, 5])
-def test_banded_march_is_bit_identical(monkeypatch, nx, ny, bands):
+def test_banded_march_is_bit_identical(nx, ny, bands):
     """L2 banding (grids whose wavelength batch exceeds L2): the long-ray cascades are marched band by
     band, each ray's (I, tau) parked between bands, rays heading up/right in ascending band order and the
     others in descending order.  The arithmetic per ray is unchanged, so J must be bit-identical to the
     unbanded solve.  Forced here on small grids (bands along columns, along rows, and a square grid), with
     a boundary intensity so that the top-cascade epilogue of parked rays is exercised too."""
     atm = A.make_config(3, nx=nx, ny=ny, nlambda=11, ncascades=6, seed=9)
-    monkeypatch.setenv("RC_BANDS", "1")
-    ref = gpu_solve(atm)
-    monkeypatch.setenv("RC_BANDS", str(bands))
-    got = gpu_solve(atm)
+    ref = gpu_solve(atm, tuning=dict(bands=1))
+    got = gpu_solve(atm, tuning=dict(bands=bands))
     assert np.array_equal(ref, got)
-    monkeypatch.setenv("RC_PATCH_LOG2", "5")
-    monkeypatch.setenv("RC_MARCH_VARIANT", "0")
-    assert np.array_equal(ref, gpu_solve(atm))
+    assert np.array_equal(ref, gpu_solve(atm, tuning=dict(bands=bands, patch_log2=5, march_variant=0)))
 
 
 # ------------------------------------------------------------------ 2.5D inclination quadrature (f2)
@@ -260,33 +256,6 @@ def test_inclinations_reset_to_flatland(oracle):
     rc.close()
 
 
-# ------------------------------------------------------------------ sparsity
-@pytest.mark.parametrize("bands", [1, 3])
-def test_sparse_march_is_bit_identical(oracle, monkeypatch, bands):
-    """Mostly-empty atmospheres (config 4's recipe: > 90 % of cells exactly 0): rc_set_atmosphere counts the
-    empty cells, pack_kernel writes an occupancy bitmap and the march gathers occupied cells only.  An empty
-    cell contributes nothing (chi = 0, S = 0), so J must be bit-identical to the dense march (RC_NO_SPARSE),
-    also when banded, and match the oracle."""
-    from paper_2408_14425_b200 import binding
-    atm = A.make_config(4, nx=256, ny=128, nlambda=11, ncascades=6)
-    monkeypatch.setenv("RC_BANDS", str(bands))
-    J, rc = binding.solve_atmosphere(atm, flags=0)
-    st = rc.get_stats()
-    rc.close()
-    assert st.empty_cells > 0.8 * atm.nx * atm.ny
-    monkeypatch.setenv("RC_NO_SPARSE", "1")
-    J2, rc2 = binding.solve_atmosphere(atm, flags=0)
-    rc2.close()
-    assert np.array_equal(J.cpu().numpy(), J2.cpu().numpy())
-    monkeypatch.delenv("RC_NO_SPARSE")
-    check(atm, oracle)
-    # and forced on a dense atmosphere (every bit set): still bit-identical
-    dense = A.make_config(2, nx=128, ny=64, nlambda=5, ncascades=5)
-    ref = gpu_solve(dense)
-    monkeypatch.setenv("RC_FORCE_SPARSE", "1")
-    assert np.array_equal(ref, gpu_solve(dense))
-
-
 # ------------------------------------------------------------------ moving line (f1)
 @pytest.mark.parametrize("kw", [
     dict(nx=128, ny=128, nlambda=16, ncascades=6),
@@ -318,18 +287,16 @@ def test_static_line_equals_givenfs_path(oracle):
 
 
 # ------------------------------------------------------------------ CUDA graph replay (small grids)
-def test_graph_replay_matches_plain_launches(monkeypatch):
+def test_graph_replay_matches_plain_launches():
     """Small grids replay a captured CUDA graph of the launch sequence.  Same bits as plain launches
-    (RC_NO_GRAPH), on first use and on replay; boundary / weights updates (device buffers the kernels read)
+    (rc_set_tuning "graph" = 0), on first use and on replay; boundary / weights updates (device buffers the kernels read)
     take effect without re-capture; a new atmosphere or output buffer re-captures."""
     import torch
     from paper_2408_14425_b200 import binding
     atm = A.make_config(3, nx=64, ny=64, nlambda=3, ncascades=5)
-    monkeypatch.setenv("RC_NO_GRAPH", "1")
-    ref = gpu_solve(atm)
+    ref = gpu_solve(atm, tuning=dict(graph=0))
     atm2 = A.make_config(0, nx=64, ny=64, nlambda=3, ncascades=5, seed=5)
-    ref2 = gpu_solve(atm2)
-    monkeypatch.delenv("RC_NO_GRAPH")
+    ref2 = gpu_solve(atm2, tuning=dict(graph=0))
     J, rc = binding.solve_atmosphere(atm)
     assert np.array_equal(J.cpu().numpy(), ref)
     J2 = rc.solve_J(out=J)                                   # replay into the same buffer
