@@ -138,7 +138,7 @@ int rc_set_stream(rc_ctx *ctx, void *cuda_stream);
  *   "cpw_from"      -1 | i      cascades >= i run one child direction per warp (-1: never; default 3)
  *   "bands" n, "l2_mb" x        L2 banding of grids whose wavelength batch exceeds L2: n bands (0: from the budget x, 72 MB)
  *   "sparse"        -1 | 0 | 1  distance-field march after rc_analyse_atmosphere: automatic (> 2/3 empty) / never / always
- *   "sparse_mode"   0 | 1       that march at 24 warps/SM (<= 80 registers) / 16 warps/SM (<= 128)
+ *   "sparse_mode"   0..3        that march in blocks of 8 / 4 / 2 warps at <= 80 registers, or (3) 4 warps at <= 128
  *   "graph"         0 | 1       CUDA graph replay on small grids
  *   "tau_cut"       x >= 1      early-exit threshold on tau log2 e; below 126 it drops transmittances below 2^-x
  * RC_ERR_BAD_VALUE for an unknown name or a value out of range. */

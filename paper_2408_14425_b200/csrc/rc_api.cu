@@ -30,7 +30,7 @@ struct Tuning {
     double l2_mb = 72.0;   // L2 budget of one wavelength batch of packed chi, S
     int sparse = -1;       // distance-field march: -1 automatic (> 2/3 of the cells empty), 0 never, 1 whenever analysed
     int graph = 1;         // CUDA graph replay on small grids
-    int sparse_mode = 0;   // distance-field march variant, 0..3
+    int sparse_mode = 1;   // fan march variant, 0..3 (blocks of 8 / 4 / 2 warps, or 4 warps at 128 registers)
 };
 
 struct CascadePlan {
@@ -440,7 +440,7 @@ int rc_set_tuning(rc_ctx *ctx, const char *name, double value) {
     else if (n == "l2_mb") { if (!(value >= 1.0)) goto bad; t.l2_mb = value; }
     else if (n == "sparse") { if (iv < -1 || iv > 1) goto bad; t.sparse = iv; }
     else if (n == "graph") { t.graph = iv != 0; }
-    else if (n == "sparse_mode") { if (iv < 0 || iv > 1) goto bad; t.sparse_mode = iv; }
+    else if (n == "sparse_mode") { if (iv < 0 || iv > 3) goto bad; t.sparse_mode = iv; }
     else return fail(ctx, RC_ERR_BAD_VALUE, "rc_set_tuning: unknown knob '%s'", name);
     // the plan (bands), the patch lists and a captured graph may depend on a knob: start over
     ctx->have_atm = false;

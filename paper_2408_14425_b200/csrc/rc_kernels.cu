@@ -163,6 +163,12 @@ __device__ __forceinline__ float ex2_neg(float tau2) {  // 2^-tau2, flushes to 0
     return r;
 }
 
+__device__ __forceinline__ float rcp_approx(float x) {
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+
 template <int LV>
 __device__ __forceinline__ void load_vec(const float *p, float (&v)[LV]) {
     if constexpr (LV == 8) {
@@ -423,6 +429,31 @@ __device__ __forceinline__ void seg_update1(float c, float S, float ds, float dk
     T = Tn;
 }
 
+// line mode, two channels: a = x_l + v.w (pairs), the six packed line parameters of the cell broadcast; profile, opacity,
+// emissivity and the update of seg_update2 with S = num / chi (thin branch: num dk (T + Tn), no division involved)
+__device__ __forceinline__ void seg_update_line2(f32x2 aa, float cc, float ccS, float cl, float clS, f32x2 ds, f32x2 dk, f32x2 &tau, f32x2 &T, f32x2 &I) {
+    float q0, q1;
+    up2(mul2(aa, aa), q0, q1);
+    const f32x2 phi = pk2(ex2_neg(q0), ex2_neg(q1));
+    const f32x2 c = fma2(pk2(cl, cl), phi, pk2(cc, cc)), num = fma2(pk2(clS, clS), phi, pk2(ccS, ccS));
+    float c0, c1;
+    up2(c, c0, c1);
+    // pack_line_kernel keeps chi_c >= 1e-37 where the cell holds anything, so c > 0 there; exact vacuum: num = 0, guarded
+    const f32x2 Sv = mul2(num, pk2(c0 > 0.f ? rcp_approx(c0) : 0.f, c1 > 0.f ? rcp_approx(c1) : 0.f));
+    tau = fma2(c, ds, tau);
+    const f32x2 xk = mul2(c, dk);
+    float t0, t1;
+    up2(tau, t0, t1);
+    const f32x2 Tn = pk2(ex2_neg(t0), ex2_neg(t1));
+    const f32x2 thick = mul2(Sv, sub2(T, Tn)), thin = mul2(mul2(num, dk), add2(T, Tn));
+    float x0, x1, a0, a1, b0, b1;
+    up2(xk, x0, x1);
+    up2(thick, a0, a1);
+    up2(thin, b0, b1);
+    I = add2(I, pk2(x0 < XK_THIN ? b0 : a0, x1 < XK_THIN ? b1 : a1));
+    T = Tn;
+}
+
 // line mode: the cell's eta log2e (num) and chi log2e (c) are evaluated per ray; emission eta ds T in the thin branch
 __device__ __forceinline__ void seg_update_line(float c, float num, float ds, float dk, float &tau, float &T, float &I) {
     const float Sv = c > 0.f ? __fdividef(num, c) : 0.f;  // eta/chi
@@ -662,7 +693,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
             // the channels of a lane two at a time (FFMA2 / FADD2 / FMUL2).  Pair q holds, when the lane has at least two
             // wavelengths, inclination q % NM of wavelengths 2 (q / NM) and 2 (q / NM) + 1 (two neighbouring gathered values,
             // one path length); with a single wavelength, inclinations 2q and 2q + 1 of it (one gathered value, two lengths)
-            constexpr bool PACKED = !LINE && LV >= 2;
+            constexpr bool PACKED = LV >= 2;
             constexpr int NP = PACKED ? LV / 2 : 1;
             [[maybe_unused]] f32x2 I2[NP], tau2[NP], T2[NP];
             [[maybe_unused]] auto ch_lo = [](int q) { return LL >= 2 ? (2 * (q / NM)) * NM + q % NM : 2 * q; };
@@ -696,13 +727,27 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
                         float vwm[NM];
 #pragma unroll
                         for (int m = 0; m < NM; m++) vwm[m] = NM == 1 ? vw : vw * p.incl_s[m];
+                        if constexpr (PACKED) {
 #pragma unroll
-                        for (int v = 0; v < LV; v++) {
-                            const float aa = xs[v / NM] + vwm[v % NM];
-                            const float phi = ex2_neg(aa * aa);
-                            const float chi2 = fmaf(c2[u][2], phi, c2[u][0]);
-                            const float num = fmaf(c2[u][3], phi, c2[u][1]);
-                            seg_update_line(chi2, num, dsm[v % NM], dkm[v % NM], tau[v], T[v], I[v]);
+                            for (int q = 0; q < NP; q++) {
+                                if constexpr (LL >= 2) {
+                                    const int l = 2 * (q / NM), m = q % NM;
+                                    seg_update_line2(add2(pk2(xs[l], xs[l + 1]), pk2(vwm[m], vwm[m])), c2[u][0], c2[u][1], c2[u][2], c2[u][3],
+                                                     pk2(dsm[m], dsm[m]), pk2(dkm[m], dkm[m]), tau2[q], T2[q], I2[q]);
+                                } else {
+                                    seg_update_line2(add2(pk2(xs[0], xs[0]), pk2(vwm[2 * q], vwm[2 * q + 1])), c2[u][0], c2[u][1], c2[u][2], c2[u][3],
+                                                     pk2(dsm[2 * q], dsm[2 * q + 1]), pk2(dkm[2 * q], dkm[2 * q + 1]), tau2[q], T2[q], I2[q]);
+                                }
+                            }
+                        } else {
+#pragma unroll
+                            for (int v = 0; v < LV; v++) {
+                                const float aa = xs[v / NM] + vwm[v % NM];
+                                const float phi = ex2_neg(aa * aa);
+                                const float chi2 = fmaf(c2[u][2], phi, c2[u][0]);
+                                const float num = fmaf(c2[u][3], phi, c2[u][1]);
+                                seg_update_line(chi2, num, dsm[v % NM], dkm[v % NM], tau[v], T[v], I[v]);
+                            }
                         }
                     } else {
                         if constexpr (PACKED) {
@@ -943,15 +988,24 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_fan_kernel(MarchParams
         float cP[LV], SP[LV], dsP = 0.f;
 #pragma unroll
         for (int v = 0; v < LV; v++) { cP[v] = 0.f; SP[v] = 0.f; }
+        // (cell, distance) of step sn when they have been looked up ahead of time: inside a blob the next step is the next
+        // occupied cell, and its look-ups then overlap the integration of the previous one instead of following it
+        bool ahead = false;
+        int c_ahead = 0, r_ahead = 0;
         while (true) {
             bool found = false;
             int cf = 0;
             while (sn < n) {  // next occupied step of this lane's ray
-                const unsigned e = __ldg(xyt + sn);
-                const int x = X0 + (int)(short)(e & 0xffffu), y = Y0 + (int)(short)(e >> 16);
-                if ((unsigned)x >= (unsigned)p.nx || (unsigned)y >= (unsigned)p.ny) { sn = n; break; }  // left the box: for good
-                cf = y * p.nx + x;
-                const int r = __ldg(p.dist + cf);
+                int r;
+                if (ahead) {
+                    cf = c_ahead; r = r_ahead; ahead = false;
+                } else {
+                    const unsigned e = __ldg(xyt + sn);
+                    const int x = X0 + (int)(short)(e & 0xffffu), y = Y0 + (int)(short)(e >> 16);
+                    if ((unsigned)x >= (unsigned)p.nx || (unsigned)y >= (unsigned)p.ny) { sn = n; break; }  // left the box: for good
+                    cf = y * p.nx + x;
+                    r = __ldg(p.dist + cf);
+                }
                 if (r == 0) { found = true; break; }
                 sn += max(r, 1 + (int)((float)(r - 3) * invm));
             }
@@ -964,6 +1018,17 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_fan_kernel(MarchParams
                 load_vec<LV>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(SB) + d), SN);
                 dsN = __uint_as_float(__ldg(tab + sn).y);
                 sn++;
+                if (sn < n) {  // look the next step up now
+                    const unsigned e = __ldg(xyt + sn);
+                    const int x = X0 + (int)(short)(e & 0xffffu), y = Y0 + (int)(short)(e >> 16);
+                    if ((unsigned)x >= (unsigned)p.nx || (unsigned)y >= (unsigned)p.ny) {
+                        sn = n;
+                    } else {
+                        c_ahead = y * p.nx + x;
+                        r_ahead = __ldg(p.dist + c_ahead);
+                        ahead = true;
+                    }
+                }
             }
             if (pend) {  // integrate the cell gathered one round earlier
                 nwalk++;
@@ -984,7 +1049,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_fan_kernel(MarchParams
                     float tmin = tau[0];
 #pragma unroll
                     for (int v = 1; v < LV; v++) tmin = fminf(tmin, tau[v]);
-                    if (tmin > p.tau_cut) { sn = n; found = false; }
+                    if (tmin > p.tau_cut) { sn = n; found = false; ahead = false; }
                 }
             }
             if (!found) break;  // per lane: nothing pending any more, nothing ahead
@@ -1062,9 +1127,14 @@ static cudaError_t launch_march_sparse(const MarchParams &p, cudaStream_t st) {
     const long long blocks = (warps + WARPS - 1) / WARPS;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     if (blocks == 0) return cudaSuccess;
-    // sparse_mode 1: 16 warps/SM at <= 128 registers instead of 24 at <= 80
-    if (p.sparse_mode & 1) march_fan_kernel<LV, WARPS, 2><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
-    else march_fan_kernel<LV, WARPS, 3><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
+    // sparse_mode: blocks of 8 / 4 / 2 warps at <= 80 registers (24 warps/SM; a block keeps its slots until its last warp
+    // is done, and the work of a warp depends on what its fan meets), or 3: blocks of 4 warps at <= 128 registers (16 warps/SM)
+    switch (p.sparse_mode) {
+        case 1: march_fan_kernel<LV, 4, 6><<<(unsigned)((warps + 3) / 4), 128, 0, st>>>(p); break;
+        case 2: march_fan_kernel<LV, 2, 12><<<(unsigned)((warps + 1) / 2), 64, 0, st>>>(p); break;
+        case 3: march_fan_kernel<LV, 4, 4><<<(unsigned)((warps + 3) / 4), 128, 0, st>>>(p); break;
+        default: march_fan_kernel<LV, WARPS, 3><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p); break;
+    }
     return cudaGetLastError();
 }
 

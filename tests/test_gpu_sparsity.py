@@ -143,7 +143,7 @@ def test_distance_field_march_is_bit_identical(oracle, kw):
     assert st0.sparse_march == 0 and st1.sparse_march == 1
     assert st1.empty_cells > 0.8 * atm.nx * atm.ny
     assert np.array_equal(dense, walk)
-    for mode in (0, 1):                          # launch variants of the walk (rc_set_tuning "sparse_mode")
+    for mode in (0, 1, 2, 3):                    # launch variants of the walk (rc_set_tuning "sparse_mode")
         got, st = gpu(atm, analyse=True, tuning=dict(sparse_mode=mode))
         assert st.sparse_march == 1 and np.array_equal(dense, got), mode
     check(atm, oracle, analyse=True)
