@@ -740,6 +740,11 @@ static int enqueue_solve(rc_ctx *ctx, float *J_out) {
         pp.chiT = (float *)(ctx->ws + P.chiT); pp.ST = (float *)(ctx->ws + P.ST);
         pp.active = ctx->active_set ? (const unsigned char *)(ctx->ws + P.pflag[0]) : nullptr;
         pp.nx = P.nx; pp.ny = P.ny; pp.L = P.L; pp.nb = P.nb; pp.shift = shift;
+        // thin form below chi ds log2e = 1/64 for the longest segment (sqrt2 cells) of the most inclined ray, roughly:
+        // there the trapezoid is good to 2e-5 (seg_update*() in rc_kernels.cu)
+        float fmax = 1.f;
+        for (int m = 0; m < ctx->nm; m++) fmax = std::max(fmax, ctx->incl_f[m]);
+        pp.c_thin = (1.f / 64.f) / fmax;
         if (ctx->line) {
             pp.chi = ctx->line; pp.eta = nullptr;
             RC_CUDA(ctx, rc::launch_pack_line(pp, ctx->stream));

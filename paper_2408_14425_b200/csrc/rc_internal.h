@@ -77,6 +77,7 @@ struct PackParams {
     float *chiT, *ST;        // [nb][s][s][npy][npx][LV]
     const unsigned char *active;  // null, or [ny][nx]: cells that are not flagged are packed as vacuum
     int nx, ny, L, nb, shift;
+    float c_thin;            // cells with chi log2e below this are packed in the thin form (seg_update*() in rc_kernels.cu)
 };
 
 struct AloParams {

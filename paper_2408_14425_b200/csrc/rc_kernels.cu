@@ -234,16 +234,21 @@ __device__ __forceinline__ void store_vec(float *p, const float (&v)[LV]) {
 template <int LV>
 __global__ void __launch_bounds__(256) pack_kernel(PackParams p) {
     const long long ncell = (long long)p.nx * p.ny;
-    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (idx >= ncell * p.nb) return;
-    const int nbI = (int)(idx / ncell);
-    const long long c = idx - (long long)nbI * ncell;  // output cell index ((ym*s + xm)*npy + yd)*npx + xd
+    // thread -> (output cell c, batch nbI): 4 consecutive output cells x the batches are neighbours, so that a warp
+    // reads whole cells (4 x nb LV floats: full 128-byte lines of the caller's arrays) and writes one full 128-byte
+    // line per batch.  (Batch-slowest threads read one 32-byte sector of every cell at a time: 39 % of the HBM peak.)
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long grp = t >> 2;
+    const int nbI = (int)(grp % p.nb);
+    const long long c = (grp / p.nb) * 4 + (t & 3);  // output cell index ((ym*s + xm)*npy + yd)*npx + xd
+    if (c >= ncell) return;
+    const long long idx = (long long)nbI * ncell + c;
     const int npx = p.nx >> p.shift, npy = p.ny >> p.shift, smask = (1 << p.shift) - 1;
     const int xd = (int)(c % npx);
-    long long t = c / npx;
-    const int yd = (int)(t % npy);
-    t /= npy;
-    const int xm = (int)t & smask, ym = (int)(t >> p.shift);
+    long long r = c / npx;
+    const int yd = (int)(r % npy);
+    r /= npy;
+    const int xm = (int)r & smask, ym = (int)(r >> p.shift);
     const int x = (xd << p.shift) + xm, y = (yd << p.shift) + ym;
     const long long src = ((long long)y * p.nx + x) * p.L + (long long)nbI * LV;
     float ch[LV], et[LV], c2[LV], S[LV];
@@ -260,13 +265,12 @@ __global__ void __launch_bounds__(256) pack_kernel(PackParams p) {
     }
 #pragma unroll
     for (int v = 0; v < LV; v++) {
-        // Emission without (or with next to no) opacity, reading G11 (eq. 16 in the limit chi -> 0 is eta ds): the march
-        // works with S = eta/chi, so where eta > 0 the opacity is raised to at least 2^-100 max(eta, 1) - S stays finite
-        // (<= 2^100), chi ds stays a normal number, and the optical depth this adds (< 1e-26 per cell for eta < 1e4) is
-        // far below anything fp32 can resolve.  The thin branch of seg_update() then gives exactly eta ds T.
-        const float cf = et[v] > 0.f ? fmaxf(ch[v], 7.888609052210118e-31f * fmaxf(et[v], 1.f)) : ch[v];
-        c2[v] = cf * 1.4426950408889634f;                // tau in units of ln 2: T = 2^-tau2
-        S[v] = et[v] > 0.f ? et[v] / cf : 0.f;
+        // The march updates a channel in one of two forms (seg_update*()), and which one is decided HERE, per cell and
+        // wavelength, from the opacity alone: optically thick enough (chi log2e >= c_thin) -> S = eta/chi, stored as it
+        // is; thin -> -eta/2, the sign being the flag.  Emission without (or with next to no) opacity is thus valid
+        // input and adds eta ds (eq. 16 in the limit chi -> 0, reading G11): the thin form never divides by chi.
+        c2[v] = ch[v] * 1.4426950408889634f;             // tau in units of ln 2: T = 2^-tau2
+        S[v] = c2[v] < p.c_thin ? (et[v] > 0.f ? -0.5f * et[v] : 0.f) : et[v] / ch[v];
     }
     if (p.active != nullptr && __ldg(p.active + (long long)y * p.nx + x) == 0) {
         // sparsity: "non-flagged cells are treated as transparent with no emission"
@@ -323,7 +327,7 @@ cudaError_t launch_pack_line(const PackParams &p, cudaStream_t st) {
 }
 
 cudaError_t launch_pack(const PackParams &p, int LV, cudaStream_t st) {
-    const long long n = (long long)p.nx * p.ny * p.nb;
+    const long long n = (((long long)p.nx * p.ny + 3) / 4) * 4 * p.nb;
     const unsigned blocks = (unsigned)((n + 255) / 256);
     switch (LV) {
         case 8: pack_kernel<8><<<blocks, 256, 0, st>>>(p); break;
@@ -364,18 +368,20 @@ __device__ __forceinline__ void store_vec_cs(float *p, const float (&v)[LV]) {
 // ------------------------------------------------------------------------------------------------
 // eq. 16 for one cell, accurate at every optical depth.  x = chi ds log2 e is the optical depth of
 // the segment in units of ln 2; tau accumulates (one rounding per cell) and T_n = 2^-tau_n.  The cell emits
-// S T_(n-1) (1 - 2^-x), evaluated as
-//   x >= 1/64:  S (T_(n-1) - T_n)              difference of two transmittances, each good to ~1e-7 T: relative error
-//                                              < 2e-5 per cell, and the roundings of T_n cancel between neighbouring cells
-//   x <  1/64:  S (x ln2 / 2) (T_(n-1) + T_n)  trapezoid of the attenuation across the cell: 1 - e^-y = (y/2)(1 + e^-y)
-//                                              (1 - y^2/12 + ...), relative error < 1e-5; exact as chi -> 0 (S x = eta ds
-//                                              log2 e, reading G11) and blind to the resolution of T, so optically thin
-//                                              rays and thin emitters behind absorbers keep their emission
-// One form for every launch: there is no "thin" variant and no host-side detection any more.
+// S T_(n-1) (1 - 2^-x), evaluated in one of two forms chosen per cell and channel by pack_kernel (from chi alone, so
+// that the march spends no multiplication on the decision; the sign of the packed source term is the flag):
+//   thick (chi log2e >= c_thin = 1/64 / max over inclinations of 1/sin):  S (T_(n-1) - T_n), S = eta/chi packed.
+//       Difference of two transmittances, each good to ~1e-7 T: relative error < 2e-5 per cell of typical length, and
+//       the roundings of T_n cancel between neighbouring cells
+//   thin:  (eta/2) ds (T_(n-1) + T_n), -eta/2 packed.  Trapezoid of the attenuation across the cell:
+//       1 - e^-y = (y/2)(1 + e^-y)(1 - y^2/12 + ...), y = x ln 2 <= 0.0153: relative error < 2e-5; exact as chi -> 0
+//       (eta ds T, reading G11) and blind to the resolution of T, so optically thin rays and thin emitters behind
+//       absorbers keep their emission
+// One form for every launch: there is no "thin" kernel variant and no host-side detection.
 // Channels are processed two at a time with the packed fp32 instructions of sm_100 (FFMA2 / FADD2 / FMUL2).
 // ------------------------------------------------------------------------------------------------
-static constexpr float KAPPA = 0.34657359027997264f;  // ln 2 / 2
-static constexpr float XK_THIN = KAPPA / 64.f;         // threshold on x ln2 / 2
+static constexpr float KAPPA = 0.34657359027997264f;  // ln 2 / 2   (line mode, where chi is evaluated per ray)
+static constexpr float XK_THIN = KAPPA / 64.f;         // line mode: threshold on x ln2 / 2
 
 typedef unsigned long long f32x2;  // two floats in one 64-bit register pair (lo, hi)
 __device__ __forceinline__ f32x2 pk2(float lo, float hi) {
@@ -405,27 +411,27 @@ __device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) {
     return r;
 }
 
-// two channels: c = chi log2e, S, ds = path length, dk = ds ln2/2 (pairs); state tau, T, I (pairs)
-__device__ __forceinline__ void seg_update2(f32x2 c, f32x2 S, f32x2 ds, f32x2 dk, f32x2 &tau, f32x2 &T, f32x2 &I) {
+// two channels: c = chi log2e, S = packed source term (eta/chi, or -eta/2 in a thin cell), ds = path length, mds = -ds
+// (pairs); state tau, T, I (pairs)
+__device__ __forceinline__ void seg_update2(f32x2 c, f32x2 S, f32x2 ds, f32x2 mds, f32x2 &tau, f32x2 &T, f32x2 &I) {
     tau = fma2(c, ds, tau);
-    const f32x2 xk = mul2(c, dk);
     float t0, t1;
     up2(tau, t0, t1);
     const f32x2 Tn = pk2(ex2_neg(t0), ex2_neg(t1));
-    const f32x2 d = sub2(T, Tn), ms = mul2(xk, add2(T, Tn));
-    float x0, x1, d0, d1, m0, m1;
-    up2(xk, x0, x1);
+    const f32x2 d = sub2(T, Tn), ms = mul2(add2(T, Tn), mds);
+    float s0, s1, d0, d1, m0, m1;
+    up2(S, s0, s1);
     up2(d, d0, d1);
     up2(ms, m0, m1);
-    I = fma2(S, pk2(x0 < XK_THIN ? m0 : d0, x1 < XK_THIN ? m1 : d1), I);
+    I = fma2(S, pk2(s0 < 0.f ? m0 : d0, s1 < 0.f ? m1 : d1), I);
     T = Tn;
 }
 
 // one channel (single-wavelength launches)
-__device__ __forceinline__ void seg_update1(float c, float S, float ds, float dk, float &tau, float &T, float &I) {
+__device__ __forceinline__ void seg_update1(float c, float S, float ds, float &tau, float &T, float &I) {
     tau = fmaf(c, ds, tau);
-    const float xk = c * dk, Tn = ex2_neg(tau);
-    I = fmaf(S, xk < XK_THIN ? xk * (T + Tn) : T - Tn, I);
+    const float Tn = ex2_neg(tau);
+    I = fmaf(S, S < 0.f ? -ds * (T + Tn) : T - Tn, I);
     T = Tn;
 }
 
@@ -714,11 +720,11 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
                     const uint2 en = __ldg(tab + st + u + PD);
                     // integrate step st + u (a slot past the lane's last in-box step has ds = 0: no effect)
                     // 2.5D: inclination m crosses the same cell over ds / sin(inclination)
-                    float dsm[NM], dkm[NM];
+                    float dsm[NM], dkm[NM];  // dkm: ds ln2/2 in line mode, -ds otherwise (thin form of seg_update*())
 #pragma unroll
                     for (int m = 0; m < NM; m++) {
                         dsm[m] = NM == 1 ? ds[u] : ds[u] * p.incl_f[m];
-                        dkm[m] = dsm[m] * KAPPA;
+                        dkm[m] = LINE ? dsm[m] * KAPPA : -dsm[m];
                     }
                     if constexpr (LINE) {
                         // packed cell: chi_c', chi_c' S_c, chi_line', chi_line' S_line, v_x', v_y'   (' = scaled, pack_line_kernel)
@@ -765,7 +771,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_kernel(MarchParams p) 
                         } else {
 #pragma unroll
                             for (int v = 0; v < LV; v++)
-                                seg_update1(c2[u][v / NM], S[u][v / NM], dsm[v % NM], dkm[v % NM], tau[v], T[v], I[v]);
+                                seg_update1(c2[u][v / NM], S[u][v / NM], dsm[v % NM], tau[v], T[v], I[v]);
                         }
                     }
                     // refill the slot with step st + u + PD
@@ -1032,7 +1038,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_fan_kernel(MarchParams
             }
             if (pend) {  // integrate the cell gathered one round earlier
                 nwalk++;
-                const float dkP = dsP * KAPPA;
+                const float dkP = -dsP;
                 if constexpr (LV >= 2) {
 #pragma unroll
                     for (int q = 0; q < LV / 2; q++) {
@@ -1043,7 +1049,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_fan_kernel(MarchParams
                         up2(I2, I[2 * q], I[2 * q + 1]);
                     }
                 } else {
-                    seg_update1(cP[0], SP[0], dsP, dkP, tau[0], T[0], I[0]);
+                    seg_update1(cP[0], SP[0], dsP, tau[0], T[0], I[0]);
                 }
                 if (p.early_exit) {  // this ray is opaque at every wavelength: nothing more can arrive
                     float tmin = tau[0];
