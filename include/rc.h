@@ -110,6 +110,8 @@ typedef struct {
     int cascade_empty[RC_MAX_CASCADES];   /* interval wholly outside any box of this size: boundary term only */
     int cascade_banded[RC_MAX_CASCADES];  /* marched band by band */
     int patch_w[RC_MAX_CASCADES];      /* a warp's 32 probes form a patch patch_w wide, 32 / patch_w high */
+    int cascade_sorted[RC_MAX_CASCADES];  /* instead: 8 quads of 4 x-adjacent probes from a list sorted by ray length */
+    float lane_utilisation[RC_MAX_CASCADES]; /* estimated share of a warp's lock-step lane-steps that are inside the box */
     int64_t table_steps[RC_MAX_CASCADES]; /* step-table capacity, all directions (x16 with RC_BILINEAR_FIX) */
 } rc_plan_info;
 
@@ -133,8 +135,9 @@ int rc_set_stream(rc_ctx *ctx, void *cuda_stream);
 /* Launch knobs, for measurements and tests (none changes a result beyond rounding, except tau_cut < 126).  Call before
  * rc_set_atmosphere: it drops the atmosphere and the active cells (plan, patch lists and captured graph may depend on a
  * knob).  name / value:
- *   "march_variant" -1 | 0..4   register-ring depth and occupancy of the march (-1: chosen per cascade)
+ *   "march_variant" -1 | 0..5   register-ring depth and occupancy of the march (-1: chosen per cascade)
  *   "patch_log2"    -1 | 2..5   lane patch width 2^n for cascades >= "patch_from" (-1: chosen per cascade from the geometry)
+ *   "sorted"        -1 | 0 | 1  lanes from quads of probes sorted by ray length: where the geometry says it pays / never / wherever possible
  *   "cpw_from"      -1 | i      cascades >= i run one child direction per warp (-1: never; default 3)
  *   "bands" n, "l2_mb" x        L2 banding of grids whose wavelength batch exceeds L2: n bands (0: from the budget x, 72 MB)
  *   "sparse"        -1 | 0 | 1  distance-field march after rc_analyse_atmosphere: automatic (> 2/3 empty) / never / always

@@ -38,6 +38,7 @@ class rc_plan_info(C.Structure):
     _fields_ = [("workspace_bytes", C.c_size_t), ("lambda_batch", C.c_int), ("channels", C.c_int), ("nbatches", C.c_int),
                 ("nbands", C.c_int), ("band_axis", C.c_int), ("cascade_empty", C.c_int * RC_MAX_CASCADES),
                 ("cascade_banded", C.c_int * RC_MAX_CASCADES), ("patch_w", C.c_int * RC_MAX_CASCADES),
+                ("cascade_sorted", C.c_int * RC_MAX_CASCADES), ("lane_utilisation", C.c_float * RC_MAX_CASCADES),
                 ("table_steps", C.c_int64 * RC_MAX_CASCADES)]
 
 

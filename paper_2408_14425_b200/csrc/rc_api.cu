@@ -31,6 +31,7 @@ struct Tuning {
     int sparse = -1;       // distance-field march: -1 automatic (> 2/3 of the cells empty), 0 never, 1 whenever analysed
     int graph = 1;         // CUDA graph replay on small grids
     int sparse_mode = 1;   // fan march variant, 0..3 (blocks of 8 / 4 / 2 warps, or 4 warps at 128 registers)
+    int sorted = -1;       // lanes from sorted quads: -1 where the geometry says it pays, 0 never, 1 wherever possible
 };
 
 struct CascadePlan {
@@ -38,6 +39,10 @@ struct CascadePlan {
     size_t subdir_off = 0;      // fix: unit directions of the sub-rays [ndir*16] float2
     bool banded = false;        // marched band by band (Plan::nbands launches per direction half)
     int pw_log2 = 5;            // lane patch of the march: 2^pw_log2 probes wide, 32 >> pw_log2 high
+    double patch_util = 1.0;    // estimated lock-step lane utilisation of that patch shape
+    bool sorted = false;        // lanes = 8 quads of probes taken from a list sorted by ray length (per block of 8 direction groups)
+    int qpad = 0;               // entries per block of direction groups (quads, padded to a multiple of 8)
+    size_t qlist_off = 0;       // [ngroups / 8][qpad] uint16
     long long ndir = 0;         // 4^(i+1)
     bool empty = true;          // interval starts beyond the box diagonal: no ray of it is inside
     long long slots = 0;        // step-table capacity, all directions
@@ -95,6 +100,7 @@ struct rc_ctx {
     int nm = 1;
     float incl_f[8] = {1, 1, 1, 1, 1, 1, 1, 1}, incl_w[8] = {1, 0, 0, 0, 0, 0, 0, 0};
     std::vector<std::vector<long long>> off_host;  // kept alive for the async uploads
+    std::vector<std::vector<unsigned short>> qlist_host;
     std::vector<float> stage;                      // host staging for boundary / weights
     // timing: `nsets` rings of (2 per cascade + 2) events; solve number n records into set n % nsets
     int nsets = 0;
@@ -138,7 +144,8 @@ bool shape_ok(const rc_config &cfg, int nx, int ny, int L) {
 // estimated here from the geometry alone (ray length to the box edge, clipped to the interval) for
 // the candidate shapes 32x1 .. 4x8, over a sample of directions.  Wider patches gather longer
 // contiguous runs, so the widest shape within 2 % of the best utilisation wins.
-int choose_patch(int nx, int ny, int i, double ta, double tb) {
+int choose_patch(int nx, int ny, int i, double ta, double tb, double *util) {
+    *util = 1.0;
     const int s = 1 << i, npx = nx >> i, npy = ny >> i;
     int widest = 5;
     while (widest > 0 && (1 << widest) > npx) widest--;
@@ -174,8 +181,45 @@ int choose_patch(int nx, int ny, int i, double ta, double tb) {
     double best = 0.0;
     for (int c = narrowest; c <= widest; c++) best = std::fmax(best, total / cost[c]);
     for (int c = widest; c >= narrowest; c--)
-        if (total / cost[c] >= best - 0.02) return c;
+        if (total / cost[c] >= best - 0.02) { *util = total / cost[c]; return c; }
     return widest;
+}
+
+// Sorted quads: the lanes of a warp need not be a rectangle of probes - the gathers only want runs of 4 x-adjacent
+// probes (one 128-byte line at 8 wavelengths per lane).  For a block of 8 direction groups (32 adjacent directions) the
+// quads of the lattice are ordered by the length of their longest ray inside the box (geometry alone, as in
+// choose_patch) and a warp takes 8 consecutive quads: its 32 lock-step lanes then finish almost together wherever the
+// quads sit.  Returns the estimated utilisation; fills `list` ([nblocks][qpad], 0xffff = padding) when given.
+double sorted_quads(int nx, int ny, int i, double ta, double tb, int qpad, std::vector<unsigned short> *list) {
+    const int s = 1 << i, npx = nx >> i, npy = ny >> i, qx = npx / 4, nq = qx * npy;
+    const long long ndir = 1LL << (2 * (i + 1));
+    const int nblocks = (int)(ndir / 32);
+    if (list) list->assign((size_t)nblocks * qpad, (unsigned short)0xffff);
+    const int stride = list ? 1 : std::max(1, nblocks / 32);  // the estimate looks at a sample of the blocks
+    std::vector<double> key((size_t)nq);
+    std::vector<int> order((size_t)nq);
+    double total = 0.0, cost = 0.0;
+    for (int blk = 0; blk < nblocks; blk += stride) {
+        const double th = 2.0 * M_PI * (32.0 * blk + 16.0) / (double)ndir, cx = std::cos(th), sy = std::sin(th);
+        for (int b = 0; b < npy; b++)
+            for (int q = 0; q < qx; q++) {
+                double m = 0.0;
+                for (int j = 0; j < 4; j++) {
+                    const double X = (4 * q + j + 0.5) * s, Y = (b + 0.5) * s;
+                    const double te = std::fmin(cx > 0 ? (nx - X) / cx : -X / cx, sy > 0 ? (ny - Y) / sy : -Y / sy);
+                    const double l = std::fmax(std::fmin(te, tb) - ta, 0.0) * (std::fabs(cx) + std::fabs(sy));
+                    total += l;
+                    m = std::fmax(m, l);
+                }
+                key[(size_t)b * qx + q] = m;
+            }
+        for (int q = 0; q < nq; q++) order[q] = q;
+        std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return key[x] > key[y]; });
+        for (int q0 = 0; q0 < nq; q0 += 8) cost += 32.0 * key[order[q0]];
+        if (list)
+            for (int q = 0; q < nq; q++) (*list)[(size_t)blk * qpad + q] = (unsigned short)order[q];
+    }
+    return cost > 0.0 ? total / cost : 1.0;
 }
 
 // Wavelengths per lane: a lane carries LV * nm <= 8 channels (registers).
@@ -215,7 +259,7 @@ bool make_plan_uncached(const rc_config &cfg, const Tuning &tune, int nm, bool l
         c.pw_log2 = 5;
         while (c.pw_log2 > 0 && (1 << c.pw_log2) > (nx >> i)) c.pw_log2--;
         if (c.empty) continue;
-        c.pw_log2 = choose_patch(nx, ny, i, c.ta, c.tb);
+        c.pw_log2 = choose_patch(nx, ny, i, c.ta, c.tb, &c.patch_util);
         c.fix = (cfg.flags & RC_BILINEAR_FIX) != 0 && i < top;
         std::vector<long long> local;
         std::vector<long long> &o = offs ? (*offs)[i] : local;
@@ -272,6 +316,17 @@ bool make_plan_uncached(const rc_config &cfg, const Tuning &tune, int nm, bool l
         }
         if (any) { P.state = cur; cur += 8 * field * P.NM; }
     }
+    // lanes from sorted quads where that beats the best rectangular patch (long, clipped rays: the upper cascades)
+    for (int i = 2; i <= top; i++) {
+        CascadePlan &c = P.c[i];
+        const int npx = nx >> i, npy = ny >> i;
+        const long long nq = (long long)(npx / 4) * npy;
+        if (c.empty || c.fix || c.banded || npx % 4 != 0 || nq < 8 || nq > 65535 || c.patch_util > 0.985 || tune.sorted == 0) continue;
+        c.qpad = (int)((nq + 7) / 8 * 8);
+        if (sorted_quads(nx, ny, i, c.ta, c.tb, c.qpad, nullptr) < c.patch_util + 0.015 && tune.sorted != 1) continue;
+        c.sorted = true;
+        c.qlist_off = cur; cur = align_up(cur + sizeof(unsigned short) * (size_t)(c.ndir / 32) * c.qpad);
+    }
     {
         int cap_max = 1;
         for (int i = 0; i <= top; i++) {
@@ -320,7 +375,7 @@ bool make_plan(const rc_config &cfg, const Tuning &tune, int nm, bool line, int 
     if (offs) return make_plan_uncached(cfg, tune, nm, line, nx, ny, L, host_io, P, offs);
     const double k[13] = {(double)cfg.ncascades, (double)cfg.lambda_batch, (double)cfg.flags, (double)nm, (double)line,
                           (double)nx, (double)ny, (double)L, (double)host_io, (double)cfg.c0_interval,
-                          (double)tune.bands, tune.l2_mb, 0.0};
+                          (double)tune.bands, tune.l2_mb, (double)tune.sorted};
     for (const Entry &e : cache)
         if (std::equal(k, k + 13, e.k)) { P = e.p; return true; }
     if (!make_plan_uncached(cfg, tune, nm, line, nx, ny, L, host_io, P, nullptr)) return false;
@@ -361,6 +416,8 @@ int rc_plan_query(const rc_config *cfg, int ninclinations, int line_mode, int nx
         out->cascade_empty[i] = P.c[i].empty;
         out->cascade_banded[i] = P.c[i].banded;
         out->patch_w[i] = 1 << P.c[i].pw_log2;
+        out->cascade_sorted[i] = P.c[i].sorted;
+        out->lane_utilisation[i] = (float)(P.c[i].sorted ? sorted_quads(nx, ny, i, P.c[i].ta, P.c[i].tb, P.c[i].qpad, nullptr) : P.c[i].patch_util);
         out->table_steps[i] = P.c[i].slots;
     }
     return RC_OK;
@@ -441,6 +498,7 @@ int rc_set_tuning(rc_ctx *ctx, const char *name, double value) {
     else if (n == "sparse") { if (iv < -1 || iv > 1) goto bad; t.sparse = iv; }
     else if (n == "graph") { t.graph = iv != 0; }
     else if (n == "sparse_mode") { if (iv < 0 || iv > 3) goto bad; t.sparse_mode = iv; }
+    else if (n == "sorted") { if (iv < -1 || iv > 1) goto bad; t.sorted = iv; }
     else return fail(ctx, RC_ERR_BAD_VALUE, "rc_set_tuning: unknown knob '%s'", name);
     // the plan (bands), the patch lists and a captured graph may depend on a knob: start over
     ctx->have_atm = false;
@@ -505,6 +563,15 @@ static int prepare_shape(rc_ctx *ctx, int nx, int ny, int nlambda, bool line) {
                 RC_CUDA(ctx, rc::launch_table_build(tp, ctx->stream));
             }
             ctx->tab_nx = nx; ctx->tab_ny = ny;
+        }
+        // sorted quad lists (they depend on the plan: banding, the fix - not only on the grid size)
+        ctx->qlist_host.assign(ctx->cfg.ncascades, {});
+        for (int i = 0; i < ctx->cfg.ncascades; i++) {
+            const CascadePlan &c = ctx->plan.c[i];
+            if (!c.sorted) continue;
+            sorted_quads(nx, ny, i, c.ta, c.tb, c.qpad, &ctx->qlist_host[i]);
+            RC_CUDA(ctx, cudaMemcpyAsync(ctx->ws + c.qlist_off, ctx->qlist_host[i].data(), sizeof(unsigned short) * ctx->qlist_host[i].size(),
+                                         cudaMemcpyHostToDevice, ctx->stream));
         }
         // defaults: free-space boundary, unit weights
         ctx->stage.assign((size_t)ctx->plan.Lpad, 0.f);
@@ -680,6 +747,11 @@ static rc::MarchParams march_params(const rc_ctx *ctx, int i, float *J_out) {
     mp.npatch_x = (lx + pw - 1) / pw;
     mp.npatch_y = (ly + ph - 1) / ph;
     mp.kg_n = mp.ngroups; mp.kg_off = 0;
+    // sorted quads: dense, unbanded launches of the whole direction circle (not with flagged probes, whose compacted
+    // patch lists number rectangular patches, and not under the distance-field march)
+    const bool sorted = c.sorted && !ctx->active_set && !ctx->sparse;
+    mp.qlist = sorted ? (const unsigned short *)(ctx->ws + c.qlist_off) : nullptr;
+    mp.qpad = sorted ? c.qpad : 0;
     // child-per-warp where the march is bound by the L2 -> SM gathers (measured: config 2 77.0 -> 73.7 ms, config 3
     // 331 -> 315 ms, bilinear fix 341 -> 321 ms); not in the MUFU-bound modes (inclinations, moving line)
     // ... nor on a cascade that barely reaches into the box (config 2, cascade 6: 0.014 % of its rays are live)

@@ -41,6 +41,11 @@ struct MarchParams {
     const unsigned char *flags; // null (every probe), or [npy][npx]: the flagged probes of this cascade
     const int *plist;           // null, or the numbers of the patches that hold a flagged probe (npatch_act of them)
     int npatch_act;
+    // null, or [ngroups / 8][qpad]: for every block of 8 direction groups the quads (4 x-adjacent probes) of the lattice
+    // ordered by the in-box length of their rays; a warp takes 8 consecutive entries (0xffff: none), so that its 32
+    // lock-step lanes finish together (DESIGN.md §7 "lane utilisation")
+    const unsigned short *qlist;
+    int qpad;
     const float *Aup;   // merged cascade i+1, pre-averaged over the 4 children: [nb][N_i][npy/2][npx/2][LV]; null on the top cascade
     float *out;         // mode 0: A_i [nb][N_i/4][npy][npx][LV]; mode 1: J [ny][nx][L]; mode 2: Jpart [nb][ny][nx]
     const Step *steps;
