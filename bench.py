@@ -158,6 +158,9 @@ def main():
                     help="skip rc_analyse_atmosphere (free-space acceleration of mostly-empty atmospheres, config 4)")
     ap.add_argument("--tune", default="", help="rc_set_tuning knobs, e.g. march_variant=0,bands=3")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-baseline-whole", action="store_true",
+                    help="also time the oracle on ONE WHOLE solve of the workload (config 2: ~3 minutes on 16 cores) and check "
+                         "the GPU J against it on every cell")
     ap.add_argument("--e2e-steps", type=int, default=0, help="end-to-end steps (default: the same as --steps)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
@@ -385,6 +388,16 @@ def main():
             line["cpu_baseline"] = {"value": segl / secs, "unit": UNIT, "cores": cores, "kind": "oracle",
                                     "sample": f"{nwin} windows of 8x8 cells x {atm.nlambda} wavelengths, "
                                               f"{segl:.3e} segment-wavelengths in {secs:.1f} s"}
+            if args.cpu_baseline_whole:
+                from oracle import rc_oracle
+                t0 = time.perf_counter()
+                ref = rc_oracle.solve_atmosphere(atm)
+                secs = time.perf_counter() - t0
+                Jo = ref["Jbar"] if atm.accumulate else ref["J"]
+                Jg = J.cpu().numpy().astype(np.float64)
+                m = Jo > 1e-6 * Jo.max(axis=(0, 1), keepdims=True) if Jo.ndim == 3 else Jo > 1e-6 * Jo.max()
+                line["cpu_baseline"]["whole_solve"] = {"seconds": secs, "value": segl_job / secs, "unit": UNIT,
+                                                       "gpu_max_rel_err_all_cells": float(np.max(np.abs(Jg[m] - Jo[m]) / Jo[m]))}
         print(json.dumps(line))
     rc.close()
     if world > 1:

@@ -20,7 +20,8 @@
  *
  * Conventions
  *   Layout   chi[(y*nx + x)*nlambda + l], wavelength fastest, y = 0 the bottom row; same for eta
- *            and J_out.  float32.  chi in 1/cell, eta = chi * S.
+ *            and J_out.  float32.  chi in 1/cell, eta = chi * S.  Device arrays (chi, eta, line, J_out)
+ *            must be 32-byte aligned (RC_ERR_BAD_VALUE otherwise): the kernels move one 32-byte sector per thread.
  *   Memory   "device" pointers are CUDA device memory of the context's device, "host" pointers
  *            ordinary host memory.  The library never allocates device memory: inputs, output,
  *            workspace and the stream are the caller's (e.g. torch tensors / torch streams).
@@ -135,7 +136,7 @@ int rc_set_stream(rc_ctx *ctx, void *cuda_stream);
 /* Launch knobs, for measurements and tests (none changes a result beyond rounding, except tau_cut < 126).  Call before
  * rc_set_atmosphere: it drops the atmosphere and the active cells (plan, patch lists and captured graph may depend on a
  * knob).  name / value:
- *   "march_variant" -1 | 0..5   register-ring depth and occupancy of the march (-1: chosen per cascade)
+ *   "march_variant" -1 | 0..4   register-ring depth and occupancy of the march (-1: chosen per cascade)
  *   "patch_log2"    -1 | 2..5   lane patch width 2^n for cascades >= "patch_from" (-1: chosen per cascade from the geometry)
  *   "sorted"        -1 | 0 | 1  lanes from quads of probes sorted by ray length: where the geometry says it pays / never / wherever possible
  *   "cpw_from"      -1 | i      cascades >= i run one child direction per warp (-1: never; default 3)

@@ -289,6 +289,24 @@ def emitter_config(nx=128, ny=128, nlambda=4, ncascades=6, seed=2001, chi_emitte
     return _finish("emit", nx, ny, nlambda, ncascades, chi3, eta3, meta={"emitter_fraction": float(emit.mean())})
 
 
+def wild_config(nx=96, ny=96, nlambda=8, ncascades=5, seed=3001) -> Atmosphere:
+    """Neighbouring wavelengths whose opacities differ by many orders of magnitude in the same cell (nothing a spectral
+    line does, but valid input): smooth fields chi0, S0 times a per-wavelength factor that jumps between 1e-9 and 1e2,
+    plus a faint wavelength-independent emissivity everywhere - so that in one cell a wavelength emits from the optically
+    thin limit (eta ds) right beside one that is opaque.  For the march's per-channel form of the cell update."""
+    rng = np.random.default_rng(seed)
+    sc = max(nx / 64.0, 1.0)
+    g = _unit01(_smooth_normal(rng, ny, nx, 4.0 * sc))
+    h = _unit01(_smooth_normal(rng, ny, nx, 3.0 * sc))
+    e = _unit01(_smooth_normal(rng, ny, nx, 5.0 * sc))
+    chi0 = 10.0 ** (2.0 * g - 1.0)                       # 0.1 .. 10 per cell
+    S0 = 0.5 + h
+    fac = np.array([1.0, 1e-9, 1e2, 1e-5, 3e-2, 1e-12, 1.0, 1e-3])[np.arange(nlambda) % 8]
+    chi3 = chi0[:, :, None] * fac[None, None, :]
+    eta3 = chi3 * S0[:, :, None] + (1e-4 * (0.2 + e))[:, :, None]
+    return _finish("wild", nx, ny, nlambda, ncascades, chi3, eta3, meta={"factors": fac.tolist()})
+
+
 CONFIGS = {0: config0, 1: config1, 2: config2, 3: config3, 4: config4}
 
 

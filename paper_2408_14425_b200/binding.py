@@ -98,8 +98,8 @@ def load(build_if_missing: bool = True):
             try:
                 _build.build()
             except Exception:
-                if not _build.LIB.exists():
-                    raise
+                if not _build.LIB.exists() or _build.stale():
+                    raise  # never run a library older than its sources
         if not _build.LIB.exists():
             raise RuntimeError(f"{_build.LIB} is missing: build it with paper_2408_14425_b200.build.build(); "
                                "there is no CPU fallback")

@@ -586,8 +586,12 @@ static int prepare_shape(rc_ctx *ctx, int nx, int ny, int nlambda, bool line) {
     return RC_OK;
 }
 
+// The kernels read and write the caller's arrays with 32-byte vector accesses (one sector per thread).
+static bool aligned32(const void *p) { return ((uintptr_t)p & 31) == 0; }
+
 int rc_set_atmosphere(rc_ctx *ctx, const float *chi, const float *eta, int nx, int ny, int nlambda) {
     if (!ctx || !chi || !eta) return ctx ? fail(ctx, RC_ERR_NULL_ARG, "null chi/eta") : RC_ERR_NULL_ARG;
+    if (!aligned32(chi) || !aligned32(eta)) return fail(ctx, RC_ERR_BAD_VALUE, "chi and eta must be 32-byte aligned");
     {
         const int rc = prepare_shape(ctx, nx, ny, nlambda, false);
         if (rc != RC_OK) return rc;
@@ -613,6 +617,7 @@ int rc_set_atmosphere(rc_ctx *ctx, const float *chi, const float *eta, int nx, i
 // Velocity-dependent line mode.
 int rc_set_line_atmosphere(rc_ctx *ctx, const float *line, int nx, int ny, const float *x_lambda, int nlambda) {
     if (!ctx || !line || !x_lambda) return ctx ? fail(ctx, RC_ERR_NULL_ARG, "null line / x_lambda") : RC_ERR_NULL_ARG;
+    if (!aligned32(line)) return fail(ctx, RC_ERR_BAD_VALUE, "line must be 32-byte aligned");
     {
         const int rc = prepare_shape(ctx, nx, ny, nlambda, true);
         if (rc != RC_OK) return rc;
@@ -876,6 +881,7 @@ static int enqueue_solve(rc_ctx *ctx, float *J_out) {
 // stream) and replayed into the caller's stream until anything the launches depend on changes.
 int rc_solve_J(rc_ctx *ctx, float *J_out) {
     if (!ctx || !J_out) return ctx ? fail(ctx, RC_ERR_NULL_ARG, "null J_out") : RC_ERR_NULL_ARG;
+    if (!aligned32(J_out)) return fail(ctx, RC_ERR_BAD_VALUE, "J_out must be 32-byte aligned");
     if (!ctx->have_atm) return fail(ctx, RC_ERR_NO_ATMOSPHERE, "call rc_set_atmosphere first");
     RC_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
     if (ctx->lists_dirty) { const int rc = build_patch_lists(ctx); if (rc != RC_OK) return rc; }

@@ -171,6 +171,37 @@ def test_error_codes():
         rc.set_atmosphere(bad, bad.abs())
     assert e.value.code == -5
     rc.close()
+    # borrowed device arrays must be 32-byte aligned (the kernels move whole sectors): an error, not a fault
+    rc = binding.RadianceCascades(3)
+    buf = torch.ones(16 * 16 * 8 + 8, device="cuda")
+    rc.ensure_workspace(16, 16, 8)
+    off = buf[1:1 + 16 * 16 * 8]
+    assert off.data_ptr() % 32 != 0
+    assert rc.lib.rc_set_atmosphere(rc.handle, off.data_ptr(), buf.data_ptr(), 16, 16, 8) == -5
+    assert b"aligned" in rc.lib.rc_last_error(rc.handle)
+    assert rc.lib.rc_set_atmosphere(rc.handle, buf.data_ptr(), buf.data_ptr(), 16, 16, 8) == 0
+    assert rc.lib.rc_solve_J(rc.handle, off.data_ptr()) == -5
+    rc.close()
+
+
+def test_sorted_quads_are_bit_identical(oracle):
+    """Lanes taken from the sorted quad lists (the clipped upper cascades) or from rectangular patches: the same rays,
+    the same arithmetic - J must not change by a bit; and the plan must actually use the lists on this shape."""
+    import torch
+    from paper_2408_14425_b200 import binding
+    atm = A.make_config(2, nx=256, ny=256, nlambda=8, ncascades=7)
+    plan = binding.plan_query(atm.ncascades, atm.nx, atm.ny, atm.nlambda)
+    assert any(plan.cascade_sorted[i] for i in range(atm.ncascades))
+    outs = []
+    for knob in (0, -1, 1):
+        J, rc = binding.solve_atmosphere(atm, tuning={"sorted": knob})
+        seg = rc.count_segments()
+        rc.close()
+        outs.append((J.cpu(), seg))
+    assert torch.equal(outs[0][0], outs[1][0]) and torch.equal(outs[0][0], outs[2][0])
+    assert outs[0][1] == outs[1][1] == outs[2][1]          # and the same segments are counted
+    ref = torch.from_numpy(oracle.solve_atmosphere(atm)["J"])
+    assert rel_err(outs[1][0], ref) < TOL
 
 
 def test_segment_counts_match_the_oracle(oracle):
@@ -435,6 +466,16 @@ def test_emission_without_opacity(oracle, chi_emitter, kw):
         check(A.with_inclinations(atm, 4), oracle)
         check(dataclasses.replace(atm, bilinear_fix=True), oracle)
         check(atm, oracle, lambda_batch=1)
+
+
+def test_neighbouring_wavelengths_orders_of_magnitude_apart(oracle):
+    """Neighbouring wavelengths of one cell whose opacities are many orders of magnitude apart (one emits from the optically
+    thin limit right beside one that is opaque): the form of the cell update is a per-channel decision, also within
+    the pairs the packed fp32 instructions work on."""
+    check(A.wild_config(), oracle)
+    check(A.wild_config(nx=64, ny=128, nlambda=16, ncascades=6, seed=5), oracle)
+    check(A.with_inclinations(A.wild_config(nx=64, ny=64, nlambda=4, ncascades=5), 2), oracle)
+    check(A.wild_config(), oracle, lambda_batch=2)
 
 
 def test_emission_without_opacity_is_valid_input():

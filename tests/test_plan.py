@@ -27,6 +27,20 @@ def test_lane_patches_follow_the_clipping_of_the_cascades():
     assert p4.patch_w[5] >= 16 and p4.patch_w[4] == 32
 
 
+def test_sorted_quads_where_the_box_clips_the_rays():
+    """Lanes from quads sorted by ray length replace the rectangular patch where that raises the estimated lock-step
+    utilisation (config 2: cascade 5 0.75 -> 0.88, cascade 4 0.92 -> 0.97); never on the short cascades, never with the
+    bilinear fix (lanes = one parity class) and never on banded cascades (config 3, cascades 4-5)."""
+    p = plan(2)
+    assert [p.cascade_sorted[i] for i in range(8)] == [0, 0, 0, 1, 1, 1, 0, 0]
+    assert 0.86 < p.lane_utilisation[5] < 0.90 and 0.96 < p.lane_utilisation[4] < 0.98
+    assert all(p.lane_utilisation[i] > 0.99 for i in range(3))
+    assert not any(plan(2, flags=FIX).cascade_sorted[i] for i in range(7))
+    p3 = plan(3)
+    assert p3.cascade_banded[4] == p3.cascade_banded[5] == 1 and p3.cascade_sorted[4] == p3.cascade_sorted[5] == 0
+    assert p3.cascade_sorted[6] == 1
+
+
 def test_wavelength_batches_and_channels():
     assert (plan(2).lambda_batch, plan(2).nbatches, plan(2).channels) == (8, 8, 8)
     assert (plan(0).lambda_batch, plan(0).nbatches) == (1, 1)
