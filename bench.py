@@ -32,11 +32,18 @@ from paper_2408_14425_b200 import atmospheres  # noqa: E402
 METRIC = "probe-ray-wavelength segments/sec"
 UNIT = "seg-lambda/s"
 SM_COUNT, MUFU_PER_CLK_SM = 148, 16  # one ex2 per segment-wavelength; DESIGN.md §7
-L2_PORT_BYTES_PER_CLK_SM = 64        # L2 -> SM (L1 fill) path; the gather probe reaches 62 of it
 # ncu --set full captures of the dominant launch that are committed under profiles/, keyed by (mode, config, cascade):
-# dram__bytes_read.sum + dram__bytes_write.sum per launch, lts__t_sectors % of peak, and where the capture is.  A run
-# whose mode / config / launch plan has no entry reports traffic = null.
-NCU_CAPTURES = {}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch, l1tex__m_xbar2l1tex_read_bytes.sum (bytes that really came over
+# the L2 -> SM path; the algorithmic bytes also count what L1 served), lts__t_sectors % of peak, and where the capture is.
+# A run whose mode / config / launch plan has no entry reports traffic = null.  Re-capture when the dominant kernel changes.
+NCU_CAPTURES = {
+    ("flat", 2, 5): {"dram_bytes": 2.032214e9 + 0.268770e9, "l2_to_sm_bytes": 486.879790e9, "lts_pct": 45.92,
+                     "source": "profiles/ncu_r2_march.md: ncu --set full of march_kernel<8,1,3,8,2,0,0>, cascade 5 of config 2, "
+                               "commit 0eaea15 (30.87 ms under ncu)"},
+    ("line_incl8", 2, 5): {"dram_bytes": 5.789094e9 + 2.674684e9, "l2_to_sm_bytes": 1879.661e9, "lts_pct": 11.03,
+                           "source": "profiles/ncu_r2_modes.md: ncu --set full of march_kernel<8,8,2,8,3,0,1>, cascade 5 of the "
+                                     "moving line x 8 inclinations on the config-2 grid, commit 0eaea15 (497.3 ms under ncu)"},
+}
 
 
 def peaks():
@@ -327,8 +334,8 @@ def main():
         mufu_per_unit = 3 if atm.line is not None else 1  # line mode: ex2 (profile), rcp (eta/chi), ex2 (transmittance)
         sfu_peak = SM_COUNT * MUFU_PER_CLK_SM * sm_max_mhz * 1e6 / mufu_per_unit
         ach_alu = seg[dom] * atm.nlambda * nincl / (ms_march[dom] * 1e-3)
-        port_gbs = SM_COUNT * L2_PORT_BYTES_PER_CLK_SM * sm_max_mhz * 1e6 / 1e9
-        mufu_bound = ach_alu / sfu_peak > ach / port_gbs
+        mufu_bound = ach_alu / sfu_peak > ach / l2_gather_gbs
+        l2_meas = None if cap is None else cap["l2_to_sm_bytes"] / (ms_march[dom] * 1e-3) / 1e9
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "strong" if world > 1 else "weak", "vs_baseline": None,
@@ -347,16 +354,24 @@ def main():
                        "distance_field_march": None if analysed is None else bool(analysed.sparse_march),
                        "active_cell_fraction": None if atm.active is None else atm.meta["active_fraction"]},
             "solve_ms": ms_step,
-            # the binding roof of the dominant kernel: the L2 -> SM gather path (64 B/clk/SM), or the MUFU pipe where one
-            # gather feeds several exponentials (inclinations, moving line); HBM is NOT the roof: the same bytes are
-            # served from L2, so the HBM figures are reported beside it, from the committed ncu capture
+            # The binding roof of the dominant kernel.  HBM is NOT it: the gathers (8 B per segment-wavelength, each cell
+            # crossed ~5 x 4^i times per cascade) are served by L2 and L1, DRAM sees 0.4 % of them (the `hbm` object).
+            # bound "l2": algorithmic gather bytes over the L2 -> SM gather ceiling measured in this very run by
+            # rc_probe_gather_bandwidth (the march's access pattern alone: random 1 KB warp-wide runs, LDG.256, 48 warps/SM,
+            # 64 MB L2-resident region) - an achieved figure of a micro-kernel, not a data-sheet peak (the guides give none);
+            # part of the algorithmic bytes is served by L1 (the children of a direction group share cells), which is why
+            # `l2_measured` (ncu: bytes that crossed L2 -> SM / this run's launch time) is reported beside it.
+            # bound "alu": the MUFU pipe (16 ex2/clk/SM), where one gather feeds several exponentials (inclinations, line).
             "roofline": ({"bound": "alu", "pipe": f"MUFU, 16/clk/SM x 148 SMs at sm_max_mhz, {mufu_per_unit} per unit",
                           "kernel": f"march_kernel<{st.lambda_batch * nincl}> cascade {dom}", "achieved": ach_alu, "peak": sfu_peak,
                           "unit": UNIT, "frac": ach_alu / sfu_peak} if mufu_bound else
-                         {"bound": "l2", "kernel": f"march_kernel<{st.lambda_batch}> cascade {dom}", "achieved": ach, "peak": port_gbs,
-                          "unit": "GB/s", "frac": ach / port_gbs,
-                          "peak_source": "derived: L2 -> SM port 64 B/clk/SM x 148 SMs x sm_max_mhz (DESIGN.md §7); the fraction can "
-                                         "exceed what L2 alone delivers because part of the algorithmic bytes is served by L1"}),
+                         {"bound": "l2", "kernel": f"march_kernel<{st.lambda_batch}> cascade {dom}", "achieved": ach, "peak": l2_gather_gbs,
+                          "unit": "GB/s", "frac": ach / l2_gather_gbs,
+                          "peak_source": "measured in this run by rc_probe_gather_bandwidth(64 MB): the march's gather pattern alone from "
+                                         "L2; achieved by a micro-kernel, not a hardware peak",
+                          "l2_measured": {"achieved": l2_meas, "frac": None if l2_meas is None else l2_meas / l2_gather_gbs,
+                                          "ncu_lts_t_sectors_pct": None if cap is None else cap.get("lts_pct"),
+                                          "note": "ncu l1tex__m_xbar2l1tex_read_bytes.sum of the committed capture / this run's launch time"}}),
             "roofline_l2_probe": {"bound": "l2", "achieved": ach, "peak": l2_gather_gbs, "unit": "GB/s", "frac": ach / l2_gather_gbs,
                                   "peak_source": "achieved by a micro-kernel (rc_probe_gather_bandwidth(64 MB), this run: random 1 KB "
                                                  "warp-wide runs, LDG.256, 48 warps/SM, region L2-resident), not a hardware peak",
