@@ -120,7 +120,9 @@ typedef struct {
  * calls it mirrors. */
 int rc_plan_query(const rc_config *cfg, int ninclinations, int line_mode, int nx, int ny, int nlambda, rc_plan_info *out);
 
-/* Create a context on cfg->device.  Fails with RC_ERR_NO_DEVICE unless that device is sm_100. */
+/* Create a context on cfg->device for the cascade hierarchy of PAPER.md:171-181 (eq. 12-13, alpha = 2): cfg->ncascades
+ * cascades, cascade-0 interval cfg->c0_interval cells (1 in BASELINE.json's configs).  Fails with RC_ERR_NO_DEVICE unless
+ * that device is sm_100; RC_ERR_BAD_VALUE for a bad config.  Allocates host memory only. */
 int rc_create(rc_ctx **out, const rc_config *cfg);
 
 /* Bytes of device workspace rc_solve_J needs for an nx x ny x nlambda atmosphere (0 on bad shape).
@@ -206,7 +208,10 @@ int rc_set_boundary_inclined(rc_ctx *ctx, const float *I_below, const float *I_a
  * it changes the workspace size (merged cascades hold n x nlambda channels) and drops the atmosphere. */
 int rc_set_inclinations(rc_ctx *ctx, int n, const float *mu, const float *w);
 
-/* Wavelength weights for RC_ACCUM_J: host, [nlambda]; NULL = all 1.  After rc_set_atmosphere. */
+/* Wavelength weights for RC_ACCUM_J: Jbar = sum_l w_l J_l (J of PAPER.md:36, eq. 1, summed over the wavelength grid:
+ * "to correctly integrate J and the necessary radiative rates", and the wavelength integration of
+ * PAPER.md:359; BASELINE.json configs[4]: "J accumulated across all wavelengths per solve").  host, [nlambda], copied;
+ * NULL = all 1.  After rc_set_atmosphere; synchronises. */
 int rc_set_lambda_weights(rc_ctx *ctx, const float *w);
 
 /* Enqueue one full solve.  J_out: device, [ny][nx][nlambda] float32, or [ny][nx] with RC_ACCUM_J. */
@@ -232,6 +237,9 @@ int rc_solve_J_line_host(rc_ctx *ctx, const float *line_host, int nx, int ny, co
  * number n into event set n % nsets (no synchronisation is added); 0 switches timing off.
  * rc_get_stats waits for the recorded sets and averages over them. */
 int rc_set_timing(rc_ctx *ctx, int nsets);
+/* Per-cascade work and timing of the last solves (every cascade has 4 nx ny intervals; PAPER.md:545-552:
+ * the upper cascades are the cost): rays, table sizes, mean pack / march milliseconds per cascade over the recorded
+ * event sets, flagged probes, empty cells.  Waits for the recorded events (hence the non-const context). */
 int rc_get_stats(rc_ctx *ctx, rc_stats *out);
 
 /* Geometric work of one solve, the unit of the throughput metric: per_cascade[i] (host,

@@ -19,7 +19,7 @@ def _cases(seed, n):
         nx = m * int(rng.integers(1, max(2, 160 // m)))
         ny = m * int(rng.integers(1, max(2, 160 // m)))
         L = int(rng.integers(1, 12))
-        kind = str(rng.choice(["cfg0", "cfg1", "cfg3", "cfg4", "line"]))
+        kind = str(rng.choice(["cfg0", "cfg1", "cfg3", "cfg4", "line"] + (["cfg2", "emit", "wild"] if seed >= 7 else [])))
         kw = dict(nx=nx, ny=ny, nlambda=L, ncascades=nc, seed=int(rng.integers(1, 10**6)))
         nincl = int(rng.choice([1, 1, 2, 4, 8]))
         fix = bool(rng.integers(0, 2)) and nc > 1
@@ -31,16 +31,22 @@ def _cases(seed, n):
         if rng.integers(0, 4) == 0: env["sparse"] = 1
         if rng.integers(0, 3) == 0: env["march_variant"] = int(rng.integers(0, 5))
         if rng.integers(0, 3) == 0: env["patch_log2"] = int(rng.integers(2, 6))
+        if seed >= 7 and rng.integers(0, 2) == 0: env["sorted"] = 1          # lanes from sorted quads wherever possible
         lb = int(rng.choice([0, 0, 1, 2, 4, 8]))
         yield it, kind, kw, nincl, fix, lit, bc, env, (lb if lb * nincl <= 8 else 0)
 
 
-@pytest.mark.parametrize("seed,n", [(1, 40), (4, 30)])
+@pytest.mark.parametrize("seed,n", [(1, 40), (4, 30), (7, 30)])
 def test_random_sweep(oracle, seed, n):
     from paper_2408_14425_b200 import binding
     worst = 0.0
     for it, kind, kw, nincl, fix, lit, bc, env, lb in _cases(seed, n):
-        atm = A.line_config2(**kw) if kind == "line" else A.make_config(int(kind[3]), **kw)
+        if kind == "emit":
+            atm = A.emitter_config(chi_emitter=[0.0, 1e-12, 1e-5][it % 3], **kw)
+        elif kind == "wild":
+            atm = A.wild_config(**kw)
+        else:
+            atm = A.line_config2(**kw) if kind == "line" else A.make_config(int(kind[3]), **kw)
         if nincl > 1:
             atm = A.with_inclinations(atm, nincl)
         atm = dataclasses.replace(atm, bilinear_fix=fix)
