@@ -352,6 +352,8 @@ def main():
                        "walked_fraction": sum(walked) / max(sum(seg), 1),
                        "empty_cell_fraction": None if analysed is None else analysed.empty_cells / (atm.nx * atm.ny),
                        "distance_field_march": None if analysed is None else bool(analysed.sparse_march),
+                       "hit_lists": None if analysed is None else bool(analysed.sparse_lists),
+                       "hit_list_bytes": None if analysed is None else int(analysed.sparse_list_bytes),
                        "active_cell_fraction": None if atm.active is None else atm.meta["active_fraction"]},
             "solve_ms": ms_step,
             # The binding roof of the dominant kernel.  HBM is NOT it: the gathers (8 B per segment-wavelength, each cell

@@ -98,6 +98,8 @@ typedef struct {
     int sparse_march;                     /* the march walks the distance field (rc_analyse_atmosphere found > 2/3 empty) */
     int64_t active_cells;                 /* cells of interest (rc_set_active_cells); -1 = every cell */
     int64_t probes_flagged[RC_MAX_CASCADES]; /* with active cells: flagged probes of cascade i */
+    int sparse_lists;                     /* the sparse march runs over hit lists (rc_set_sparse_workspace was large enough) */
+    int64_t sparse_list_bytes;            /* bytes the hit lists of the analysed atmosphere need in that buffer (0: not sparse) */
 } rc_stats;
 
 /* The launch plan the library would use for a problem, computed on the host alone (no device, no context):
@@ -140,6 +142,7 @@ int rc_set_stream(rc_ctx *ctx, void *cuda_stream);
  * knob).  name / value:
  *   "march_variant" -1 | 0..4   register-ring depth and occupancy of the march (-1: chosen per cascade)
  *   "patch_log2"    -1 | 2..5   lane patch width 2^n for cascades >= "patch_from" (-1: chosen per cascade from the geometry)
+ *   "lists"         0 | 1       hit lists for the sparse march when rc_set_sparse_workspace lends room (default 1)
  *   "sorted"        -1 | 0 | 1  lanes from quads of probes sorted by ray length: where the geometry says it pays / never / wherever possible
  *   "cpw_from"      -1 | i      cascades >= i run one child direction per warp (-1: never; default 3)
  *   "bands" n, "l2_mb" x        L2 banding of grids whose wavelength batch exceeds L2: n bands (0: from the budget x, 72 MB)
@@ -187,6 +190,15 @@ int rc_set_active_cells(rc_ctx *ctx, const unsigned char *active);
  * by itself once it has been used on the context).  Plain mode only (no inclinations, moving line or bilinear fix:
  * there it only counts).  rc_stats.empty_cells, rc_stats.sparse_march report the outcome. */
 int rc_analyse_atmosphere(rc_ctx *ctx);
+
+/* A second caller-owned device buffer (256-byte aligned, borrowed; NULL takes it back) for the HIT LISTS of the sparse
+ * march: which steps of a ray meet an occupied cell depends on the geometry and the occupancy alone, so
+ * rc_analyse_atmosphere can find them once - per cascade and ray the numbers of its occupied in-box steps - instead of the
+ * march finding them again for every wavelength batch of every solve; the march then only gathers and integrates (the same
+ * cells in the same order: bit-identical).  Their size is only known after counting: rc_analyse_atmosphere always counts
+ * and reports rc_stats.sparse_list_bytes; when this buffer is missing or smaller the distance-field march stays in use
+ * (rc_stats.sparse_lists = 0) - lend at least that many bytes and analyse again.  Config 4: 3.6 GB, 435 -> see DESIGN.md. */
+int rc_set_sparse_workspace(rc_ctx *ctx, void *dev_ptr, size_t bytes);
 
 /* Boundary intensity sampled by the top cascade: I_below[l] is seen by rays heading
  * down (omega_y < 0), I_above[l] by rays heading up.  host, [nlambda] each; NULL = 0 (free space,

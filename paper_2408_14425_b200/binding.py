@@ -31,7 +31,8 @@ class rc_stats(C.Structure):
                 ("ms_march", C.c_float * RC_MAX_CASCADES), ("ms_total", C.c_float),
                 ("rays", C.c_int64 * RC_MAX_CASCADES), ("table_steps", C.c_int64 * RC_MAX_CASCADES),
                 ("workspace_bytes", C.c_size_t), ("empty_cells", C.c_int64), ("sparse_march", C.c_int),
-                ("active_cells", C.c_int64), ("probes_flagged", C.c_int64 * RC_MAX_CASCADES)]
+                ("active_cells", C.c_int64), ("probes_flagged", C.c_int64 * RC_MAX_CASCADES),
+                ("sparse_lists", C.c_int), ("sparse_list_bytes", C.c_int64)]
 
 
 class rc_plan_info(C.Structure):
@@ -64,6 +65,7 @@ SYMBOLS = {
     "rc_set_line_atmosphere": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_int]),
     "rc_set_active_cells": (C.c_int, [C.c_void_p, C.c_void_p]),
     "rc_analyse_atmosphere": (C.c_int, [C.c_void_p]),
+    "rc_set_sparse_workspace": (C.c_int, [C.c_void_p, C.c_void_p, C.c_size_t]),
     "rc_set_boundary": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
     "rc_set_boundary_inclined": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
     "rc_set_lambda_weights": (C.c_int, [C.c_void_p, C.c_void_p]),
@@ -139,6 +141,7 @@ class RadianceCascades:
         self.device = int(device)
         self.flags = int(flags)
         self._ws = None
+        self._sws = None
         self._keep = ()
         self.shape = None
 
@@ -206,11 +209,22 @@ class RadianceCascades:
         self.set_stream()
         self._check(self.lib.rc_set_active_cells(self.handle, C.c_void_p(active.data_ptr())))
 
-    def analyse_atmosphere(self):
-        """Empty-cell scan + distance field of the current atmosphere (synchronises); see rc_analyse_atmosphere."""
+    def analyse_atmosphere(self, lists=True):
+        """Empty-cell scan + distance field of the current atmosphere (synchronises); see rc_analyse_atmosphere.
+        lists: when the atmosphere is sparse, lend the library a second buffer of the size it reports for its hit
+        lists (rc_set_sparse_workspace) and analyse again."""
+        import torch
         self.set_stream()
         self._check(self.lib.rc_analyse_atmosphere(self.handle))
-        return self.get_stats()
+        st = self.get_stats()
+        if lists and st.sparse_march and not st.sparse_lists and st.sparse_list_bytes > 0:
+            if self._sws is None or self._sws.numel() < st.sparse_list_bytes:
+                self._sws = None
+                self._sws = torch.empty(int(st.sparse_list_bytes * 1.02) + 4096, dtype=torch.uint8, device=f"cuda:{self.device}")
+                self._check(self.lib.rc_set_sparse_workspace(self.handle, C.c_void_p(self._sws.data_ptr()), self._sws.numel()))
+            self._check(self.lib.rc_analyse_atmosphere(self.handle))
+            st = self.get_stats()
+        return st
 
     def set_boundary(self, I_below=None, I_above=None):
         """[nlambda] arrays, or [ninclinations][nlambda] (one value per inclined ray set)."""

@@ -31,6 +31,7 @@ struct Tuning {
     int sparse = -1;       // distance-field march: -1 automatic (> 2/3 of the cells empty), 0 never, 1 whenever analysed
     int graph = 1;         // CUDA graph replay on small grids
     int sparse_mode = 1;   // fan march variant, 0..3 (blocks of 8 / 4 / 2 warps, or 4 warps at 128 registers)
+    int lists = 1;         // hit lists for the sparse march when the caller lends a buffer (rc_set_sparse_workspace): 0 never
     int sorted = -1;       // lanes from sorted quads: -1 where the geometry says it pays, 0 never, 1 wherever possible
 };
 
@@ -92,6 +93,11 @@ struct rc_ctx {
     int npatch_act[RC_MAX_CASCADES] = {0};
     int list_version = 0;
     bool sparse = false;       // rc_analyse_atmosphere found the atmosphere mostly empty: the march walks the distance field
+    // hit lists of the sparse march (valid while `sparse`): in the caller's second buffer (rc_set_sparse_workspace)
+    char *sws = nullptr;
+    size_t sws_bytes = 0;
+    bool lists = false;
+    size_t hit_off[RC_MAX_CASCADES] = {0}, hit_list[RC_MAX_CASCADES] = {0};  // byte offsets into sws
     bool count_walked = false; // the solve being enqueued counts the segments it integrates (rc_count_walked)
     bool analysed = false;     // rc_analyse_atmosphere has been used on this context (rc_solve_J_host then repeats it)
     std::vector<float> xl_stage;  // line mode: host copy of the scaled wavelengths (kept alive for the async upload)
@@ -498,6 +504,7 @@ int rc_set_tuning(rc_ctx *ctx, const char *name, double value) {
     else if (n == "sparse") { if (iv < -1 || iv > 1) goto bad; t.sparse = iv; }
     else if (n == "graph") { t.graph = iv != 0; }
     else if (n == "sparse_mode") { if (iv < 0 || iv > 3) goto bad; t.sparse_mode = iv; }
+    else if (n == "lists") { t.lists = iv != 0; }
     else if (n == "sorted") { if (iv < -1 || iv > 1) goto bad; t.sorted = iv; }
     else return fail(ctx, RC_ERR_BAD_VALUE, "rc_set_tuning: unknown knob '%s'", name);
     // the plan (bands), the patch lists and a captured graph may depend on a knob: start over
@@ -723,6 +730,10 @@ static rc::MarchParams march_params(const rc_ctx *ctx, int i, float *J_out) {
     mp.xls = ctx->line ? (const float *)(ctx->ws + P.xls) : nullptr;
     mp.dist = ctx->sparse ? (const unsigned char *)(ctx->ws + P.dist) : nullptr;
     mp.sparse_mode = ctx->tune.sparse_mode;
+    const bool lists = ctx->sparse && ctx->lists;
+    mp.hit_off = lists ? (const unsigned *)(ctx->sws + ctx->hit_off[i]) : nullptr;
+    mp.hit_list = lists ? (const unsigned short *)(ctx->sws + ctx->hit_list[i]) : nullptr;
+    mp.list_b = P.nb >= 5 ? 8 : 1;
     mp.walked = ctx->count_walked ? (unsigned long long *)(ctx->ws + P.flag) + 16 + i : nullptr;
     mp.flags = ctx->active_set ? (const unsigned char *)(ctx->ws + P.pflag[i]) : nullptr;
     mp.plist = ctx->active_set && !ctx->lists_dirty ? (const int *)(ctx->ws + P.plist[i]) : nullptr;
@@ -825,6 +836,7 @@ static int enqueue_solve(rc_ctx *ctx, float *J_out) {
         float fmax = 1.f;
         for (int m = 0; m < ctx->nm; m++) fmax = std::max(fmax, ctx->incl_f[m]);
         pp.c_thin = (1.f / 64.f) / fmax;
+        pp.cellmajor = ctx->sparse && ctx->lists ? 1 : 0;
         if (ctx->line) {
             pp.chi = ctx->line; pp.eta = nullptr;
             RC_CUDA(ctx, rc::launch_pack_line(pp, ctx->stream));
@@ -901,7 +913,7 @@ int rc_solve_J(rc_ctx *ctx, float *J_out) {
     rc_ctx::GraphKey key;
     std::memset(&key, 0, sizeof(key));
     key.J = J_out; key.chi = ctx->chi; key.eta = ctx->eta; key.line = ctx->line; key.ws = ctx->ws;
-    key.nx = P.nx; key.ny = P.ny; key.L = P.L; key.nm = P.NM; key.sparse = (ctx->sparse ? 1 : 0) + (ctx->active_set ? 2 : 0) + 4 * ctx->list_version; key.total = P.total;
+    key.nx = P.nx; key.ny = P.ny; key.L = P.L; key.nm = P.NM; key.sparse = (ctx->sparse ? 1 : 0) + (ctx->active_set ? 2 : 0) + 4 * ctx->list_version;  // (list_version also counts the analyses) key.total = P.total;
     for (int m = 0; m < 8; m++) { key.f[m] = ctx->incl_f[m]; key.w[m] = ctx->incl_w[m]; }
     if (!ctx->graph_exec || std::memcmp(&key, &ctx->graph_key, sizeof(key)) != 0) {
         if (ctx->graph_exec) { cudaGraphExecDestroy(ctx->graph_exec); ctx->graph_exec = nullptr; }
@@ -963,6 +975,55 @@ int rc_set_active_cells(rc_ctx *ctx, const unsigned char *active) {
     return RC_OK;
 }
 
+// Hit lists of the sparse march (rc_kernels.cu "Hit lists"): per cascade the occupied in-box steps of every ray, found once
+// per analysed atmosphere instead of once per wavelength batch and solve.  They live in the caller's second buffer
+// (rc_set_sparse_workspace); how much they need is only known after counting, so the count always runs and
+// rc_stats.sparse_list_bytes reports it - when the buffer is missing or too small the distance-field march stays in use.
+static int build_hit_lists(rc_ctx *ctx) {
+    const Plan &P = ctx->plan;
+    const int nc = ctx->cfg.ncascades;
+    const size_t nrays = 4 * (size_t)P.nx * P.ny;                 // per cascade
+    const size_t off_bytes = align_up(sizeof(unsigned) * (nrays + 1));
+    const size_t bsum_bytes = align_up(sizeof(unsigned) * ((nrays + 1023) / 1024 + 1));
+    unsigned long long *tot_d = (unsigned long long *)(ctx->ws + P.flag);  // [0..15] scratch counters
+    RC_CUDA(ctx, cudaMemsetAsync(tot_d, 0, sizeof(*tot_d) * 16, ctx->stream));
+    // room for the offsets? then count per ray, else only the totals (to report the size)
+    size_t cur = bsum_bytes;
+    for (int i = 0; i < nc; i++) {
+        if (P.c[i].empty) continue;
+        ctx->hit_off[i] = cur; cur += off_bytes;
+    }
+    const bool have_off = ctx->sws != nullptr && cur <= ctx->sws_bytes;
+    for (int i = 0; i < nc; i++) {
+        if (P.c[i].empty) continue;
+        rc::MarchParams mp = march_params(ctx, i, nullptr);
+        RC_CUDA(ctx, rc::launch_hit_walk(mp, false, have_off ? (unsigned *)(ctx->sws + ctx->hit_off[i]) : nullptr, nullptr, tot_d + i, ctx->stream));
+    }
+    unsigned long long tot[16] = {0};
+    RC_CUDA(ctx, cudaMemcpyAsync(tot, tot_d, sizeof(tot), cudaMemcpyDeviceToHost, ctx->stream));
+    RC_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    bool fits32 = true;
+    for (int i = 0; i < nc; i++) {
+        if (P.c[i].empty) continue;
+        ctx->hit_list[i] = cur; cur += align_up(sizeof(unsigned short) * (size_t)tot[i] + 2);
+        fits32 = fits32 && tot[i] < 0xffffffffULL;
+    }
+    ctx->stats.sparse_list_bytes = (int64_t)cur;
+    if (!have_off || cur > ctx->sws_bytes || !fits32) return RC_OK;  // no room (or too many hits): the distance-field march
+    for (int i = 0; i < nc; i++) {
+        if (P.c[i].empty) continue;
+        rc::MarchParams mp = march_params(ctx, i, nullptr);
+        unsigned *off = (unsigned *)(ctx->sws + ctx->hit_off[i]);
+        RC_CUDA(ctx, rc::launch_hit_scan(off, (long long)nrays, (unsigned *)ctx->sws, tot[i], ctx->stream));
+        RC_CUDA(ctx, rc::launch_hit_walk(mp, true, off, (unsigned short *)(ctx->sws + ctx->hit_list[i]), nullptr, ctx->stream));
+    }
+    for (int i = 0; i < nc; i++)
+        if (P.c[i].empty) { ctx->hit_off[i] = 0; ctx->hit_list[i] = 0; }  // any valid address: never read (cnt == null)
+    ctx->lists = true;
+    ctx->stats.sparse_lists = 1;
+    return RC_OK;
+}
+
 // Free-space acceleration: occupancy and its distance transform for the current atmosphere and flags.
 int rc_analyse_atmosphere(rc_ctx *ctx) {
     if (!ctx) return RC_ERR_NULL_ARG;
@@ -984,6 +1045,20 @@ int rc_analyse_atmosphere(rc_ctx *ctx) {
     const bool want = ctx->tune.sparse >= 0 ? ctx->tune.sparse != 0 : 3 * h > 2ULL * P.nx * P.ny;
     ctx->sparse = can && want;
     ctx->stats.sparse_march = ctx->sparse;
+    ctx->list_version++;
+    ctx->lists = false;
+    ctx->stats.sparse_lists = 0;
+    ctx->stats.sparse_list_bytes = 0;
+    if (ctx->sparse && ctx->tune.lists != 0) { const int rc = build_hit_lists(ctx); if (rc != RC_OK) return rc; }
+    return RC_OK;
+}
+
+int rc_set_sparse_workspace(rc_ctx *ctx, void *dev_ptr, size_t bytes) {
+    if (!ctx) return RC_ERR_NULL_ARG;
+    if (dev_ptr && ((uintptr_t)dev_ptr % ALIGN) != 0) return fail(ctx, RC_ERR_NO_WORKSPACE, "sparse workspace pointer is not %zu-byte aligned", ALIGN);
+    ctx->sws = (char *)dev_ptr;
+    ctx->sws_bytes = dev_ptr ? bytes : 0;
+    ctx->lists = false;  // the lists lived in the old buffer: rc_analyse_atmosphere again
     ctx->list_version++;
     return RC_OK;
 }

@@ -37,6 +37,9 @@ struct MarchParams {
     const unsigned char *dist;  // null (lock-step march), or [ny][nx] Chebyshev distance to the nearest occupied cell (0 = occupied):
                                 // every lane walks its own ray and jumps over empty space; packed arrays in cell order (shift 0)
     int sparse_mode;            // launch variant of the distance-field march (rc_kernels.cu, launch_march_sparse)
+    const unsigned *hit_off;    // null, or the hit lists of this cascade (rc_analyse_atmosphere): [4 nx ny + 1] offsets, ray = probe * N_i + k,
+    const unsigned short *hit_list;  // and the step numbers of every ray's occupied in-box cells; the packed arrays are then cell-major
+    int list_b;                 // wavelength batches per warp of the march over hit lists: 8 or 1
     unsigned long long *walked; // null, or a counter of the cell segments actually integrated (rc_count_walked; per wavelength batch)
     const unsigned char *flags; // null (every probe), or [npy][npx]: the flagged probes of this cascade
     const int *plist;           // null, or the numbers of the patches that hold a flagged probe (npatch_act of them)
@@ -83,6 +86,7 @@ struct PackParams {
     const unsigned char *active;  // null, or [ny][nx]: cells that are not flagged are packed as vacuum
     int nx, ny, L, nb, shift;
     float c_thin;            // cells with chi log2e below this are packed in the thin form (seg_update*() in rc_kernels.cu)
+    int cellmajor;           // 1: write [cell][batch][LV] (march over hit lists, shift 0) instead of [batch][phase planes][LV]
 };
 
 struct AloParams {
@@ -123,6 +127,8 @@ cudaError_t launch_build_distance_field(const float *chi, const float *eta, cons
                                         int L, int *mark, unsigned char *occ, unsigned char *d1, unsigned char *dist,
                                         unsigned long long *nempty, cudaStream_t st);
 cudaError_t launch_alo(const AloParams &p, cudaStream_t st);
+cudaError_t launch_hit_walk(const MarchParams &p, bool fill, unsigned *cnt_or_off, unsigned short *list, unsigned long long *total, cudaStream_t st);
+cudaError_t launch_hit_scan(unsigned *a, long long n, unsigned *bsum, unsigned long long total, cudaStream_t st);
 cudaError_t launch_bulk_probe(const float *buf, unsigned long long nsector, int iters, int sms, float *sink, cudaStream_t st, long long *bytes);
 cudaError_t launch_validate(const float *chi, const float *eta, long long n, int *flag, cudaStream_t st);
 

@@ -242,7 +242,8 @@ __global__ void __launch_bounds__(256) pack_kernel(PackParams p) {
     const int nbI = (int)(grp % p.nb);
     const long long c = (grp / p.nb) * 4 + (t & 3);  // output cell index ((ym*s + xm)*npy + yd)*npx + xd
     if (c >= ncell) return;
-    const long long idx = (long long)nbI * ncell + c;
+    // output order: batch-major planes for the lock-step and fan marches, cell-major records for the march over hit lists
+    const long long idx = p.cellmajor ? c * p.nb + nbI : (long long)nbI * ncell + c;
     const int npx = p.nx >> p.shift, npy = p.ny >> p.shift, smask = (1 << p.shift) - 1;
     const int xd = (int)(c % npx);
     long long r = c / npx;
@@ -1160,6 +1161,322 @@ static cudaError_t launch_march_sparse(const MarchParams &p, cudaStream_t st) {
     return cudaGetLastError();
 }
 
+// ------------------------------------------------------------------------------------------------
+// Hit lists (mostly empty atmospheres, built by rc_analyse_atmosphere when the caller lends room for them): which steps
+// of a ray meet an occupied cell depends on the geometry and the occupancy alone - not on the wavelength, not on the
+// values.  The fan march finds them again for every wavelength batch of every solve (half of its time on config 4);
+// here they are found once: per cascade, hit_off[ray] .. hit_off[ray + 1] index the ray's occupied in-box steps (their
+// numbers in the direction's step table, uint16) in hit_list, ray = probe * N_i + k.  march_list_kernel then only
+// gathers and integrates - the same cells in the same order as the fan and the lock-step march: bit-identical.
+// ------------------------------------------------------------------------------------------------
+// 32 rays per warp (a fan of adjacent directions of one probe, as march_fan_kernel).  FILL = false: cnt[ray] = number of
+// hits (and *total += them); FILL = true: list[off[ray] + i] = step of the i-th hit.
+template <bool FILL>
+__global__ void __launch_bounds__(256) hit_walk_kernel(MarchParams p, unsigned *cnt_or_off, unsigned short *list, unsigned long long *total) {
+    const int lane = threadIdx.x & 31;
+    long long W = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const long long ndir = 4LL * p.ngroups;
+    const int ndl = (int)min(32LL, ndir), ppw = 32 / ndl;
+    const long long nprobe = (long long)p.npx * p.npy;
+    const long long ndb = ndir / ndl, npb = (nprobe + ppw - 1) / ppw;
+    if (W >= ndb * npb) return;
+    const long long db = W % ndb, pb = W / ndb;
+    const long long k = db * ndl + (lane % ndl);
+    const long long probe = pb * ppw + lane / ndl;
+    bool valid = probe < nprobe;
+    const int b = valid ? (int)(probe / p.npx) : 0, a = valid ? (int)(probe - (long long)b * p.npx) : 0;
+    if (valid && p.flags != nullptr) valid = __ldg(p.flags + probe) != 0;
+    const int half = (1 << p.shift) >> 1;
+    const int X0 = (a << p.shift) + half, Y0 = (b << p.shift) + half;
+    unsigned nhit = 0;
+    if (p.cnt != nullptr && valid) {
+        const long long o = __ldg(p.off + k);
+        const int n = __ldg(p.cnt + k);
+        const unsigned *xyt = reinterpret_cast<const unsigned *>(p.xy + o);
+        float invm = 1.f;
+        if (p.cascade > 0) {  // the same jump rule as march_fan_kernel
+            float sw, cw;
+            sincospif(2.f * ((float)k + 0.5f) / (float)ndir, &sw, &cw);
+            sw = fabsf(sw); cw = fabsf(cw);
+            invm = 0.999f * (sw + cw) / fmaxf(sw, cw);
+        }
+        unsigned short *out = nullptr;
+        if constexpr (FILL) out = list + __ldg(cnt_or_off + probe * ndir + k);
+        int sn = 0;
+        while (sn < n) {
+            const unsigned e = __ldg(xyt + sn);
+            const int x = X0 + (int)(short)(e & 0xffffu), y = Y0 + (int)(short)(e >> 16);
+            if ((unsigned)x >= (unsigned)p.nx || (unsigned)y >= (unsigned)p.ny) break;  // left the box: for good
+            const int r = __ldg(p.dist + (long long)y * p.nx + x);
+            if (r == 0) {
+                if constexpr (FILL) out[nhit] = (unsigned short)sn;
+                nhit++;
+                sn++;
+            } else {
+                sn += max(r, 1 + (int)((float)(r - 3) * invm));
+            }
+        }
+    }
+    if constexpr (!FILL) {
+        if (probe < nprobe && cnt_or_off != nullptr) cnt_or_off[probe * ndir + k] = nhit;
+        unsigned long long mine = nhit;
+        for (int sh = 16; sh > 0; sh >>= 1) mine += __shfl_down_sync(FULL, mine, sh);
+        if (lane == 0 && mine) atomicAdd(total, mine);
+    }
+}
+
+// Exclusive prefix sum of n counts, in place (a[n] = the total): per-block sums, one block over those, add back.
+__global__ void __launch_bounds__(1024) scan_block_kernel(unsigned *a, long long n, unsigned *bsum) {
+    __shared__ unsigned ws[32];
+    const long long i = (long long)blockIdx.x * 1024 + threadIdx.x;
+    const unsigned v = i < n ? a[i] : 0u;
+    unsigned x = v;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    for (int sh = 1; sh < 32; sh <<= 1) { const unsigned y = __shfl_up_sync(FULL, x, sh); if (lane >= sh) x += y; }
+    if (lane == 31) ws[w] = x;
+    __syncthreads();
+    if (w == 0) {
+        unsigned t = ws[lane];
+        for (int sh = 1; sh < 32; sh <<= 1) { const unsigned y = __shfl_up_sync(FULL, t, sh); if (lane >= sh) t += y; }
+        ws[lane] = t;
+    }
+    __syncthreads();
+    const unsigned incl = x + (w > 0 ? ws[w - 1] : 0u);
+    if (i < n) a[i] = incl - v;  // exclusive within the block
+    if (threadIdx.x == 1023) bsum[blockIdx.x] = incl;
+}
+
+__global__ void __launch_bounds__(1024) scan_sums_kernel(unsigned *bsum, int nblocks) {  // one block: exclusive scan of the block sums
+    __shared__ unsigned ws[32];
+    __shared__ unsigned carry;
+    if (threadIdx.x == 0) carry = 0;
+    __syncthreads();
+    for (int start = 0; start < nblocks; start += 1024) {
+        const int i = start + threadIdx.x;
+        const unsigned v = i < nblocks ? bsum[i] : 0u;
+        unsigned x = v;
+        const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+        for (int sh = 1; sh < 32; sh <<= 1) { const unsigned y = __shfl_up_sync(FULL, x, sh); if (lane >= sh) x += y; }
+        if (lane == 31) ws[w] = x;
+        __syncthreads();
+        if (w == 0) {
+            unsigned t = ws[lane];
+            for (int sh = 1; sh < 32; sh <<= 1) { const unsigned y = __shfl_up_sync(FULL, t, sh); if (lane >= sh) t += y; }
+            ws[lane] = t;
+        }
+        __syncthreads();
+        const unsigned incl = x + (w > 0 ? ws[w - 1] : 0u) + carry;
+        if (i < nblocks) bsum[i] = incl - v;
+        __syncthreads();
+        if (threadIdx.x == 1023) carry = incl;
+        __syncthreads();
+    }
+}
+
+__global__ void __launch_bounds__(1024) scan_add_kernel(unsigned *a, long long n, const unsigned *bsum, unsigned long long total) {
+    const long long i = (long long)blockIdx.x * 1024 + threadIdx.x;
+    if (i < n) a[i] += bsum[blockIdx.x];
+    if (i == n) a[n] = (unsigned)total;
+}
+
+// counts -> offsets for one cascade; `total` (host) must be the sum already known from the counting pass
+cudaError_t launch_hit_scan(unsigned *a, long long n, unsigned *bsum, unsigned long long total, cudaStream_t st) {
+    const long long nblocks = (n + 1023) / 1024;
+    scan_block_kernel<<<(unsigned)nblocks, 1024, 0, st>>>(a, n, bsum);
+    scan_sums_kernel<<<1, 1024, 0, st>>>(bsum, (int)nblocks);
+    scan_add_kernel<<<(unsigned)((n + 1 + 1023) / 1024), 1024, 0, st>>>(a, n, bsum, total);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_hit_walk(const MarchParams &p, bool fill, unsigned *cnt_or_off, unsigned short *list, unsigned long long *total, cudaStream_t st) {
+    const long long ndir = 4LL * p.ngroups, ndl = ndir < 32 ? ndir : 32, ppw = 32 / ndl;
+    const long long nprobe = (long long)p.npx * p.npy;
+    const long long warps = (ndir / ndl) * ((nprobe + ppw - 1) / ppw);
+    const long long blocks = (warps + 7) / 8;
+    if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+    if (fill) hit_walk_kernel<true><<<(unsigned)blocks, 256, 0, st>>>(p, cnt_or_off, list, total);
+    else hit_walk_kernel<false><<<(unsigned)blocks, 256, 0, st>>>(p, cnt_or_off, list, total);
+    return cudaGetLastError();
+}
+
+// The march over hit lists.  A warp = R = 32 / B adjacent directions of one probe (or of R / N_i probes on cascades 0, 1) x
+// B wavelength batches: the B lanes of a ray read the same list entries and table steps (one sector, broadcast) and gather
+// B x LV consecutive floats of the cell (the packed arrays are cell-major under this march: [cell][batch][LV]).  The next
+// hit's step, cell and path length are looked up while the previous cell is integrated.
+template <int LV, int B, int WARPS, int MINB>
+__global__ void __launch_bounds__(WARPS * 32, MINB) march_list_kernel(MarchParams p) {
+    constexpr int R = 32 / B;
+    const int lane = threadIdx.x & 31;
+    long long W = (long long)blockIdx.x * WARPS + (threadIdx.x >> 5);
+    const long long ndir = 4LL * p.ngroups;
+    const int ndl = (int)min((long long)R, ndir), ppw = R / ndl;  // directions and probes per warp
+    const long long nprobe = (long long)p.npx * p.npy;
+    const long long ndb = ndir / ndl, npb = (nprobe + ppw - 1) / ppw;
+    const int nbg = (p.nb + B - 1) / B;
+    const long long db = W % ndb;
+    W /= ndb;
+    const long long pb = W % npb;
+    const int bg = (int)(W / npb);
+    if (bg >= nbg) return;
+    const int r = lane / B, nbI = bg * B + lane % B;
+    const long long k = db * ndl + (r % ndl);
+    const long long probe = pb * ppw + r / ndl;
+    bool valid = probe < nprobe && nbI < p.nb;
+    const int b = probe < nprobe ? (int)(probe / p.npx) : 0, a = probe < nprobe ? (int)(probe - (long long)b * p.npx) : 0;
+    if (valid && p.flags != nullptr) valid = __ldg(p.flags + probe) != 0;
+    if (!__any_sync(FULL, valid)) return;
+    const int half = (1 << p.shift) >> 1;
+    const int X0 = (a << p.shift) + half, Y0 = (b << p.shift) + half;
+    const float *chiB = p.chiT + (long long)nbI * LV, *SB = p.ST + (long long)nbI * LV;  // + cell * nb * LV
+    const unsigned long long cstride = (unsigned long long)p.nb * (LV * sizeof(float));
+
+    float I[LV], tau[LV], T[LV];
+#pragma unroll
+    for (int v = 0; v < LV; v++) { I[v] = 0.f; tau[v] = 0.f; T[v] = 1.f; }
+    unsigned nwalk = 0;
+    if (p.cnt != nullptr && valid) {
+        const long long o = __ldg(p.off + k);
+        const uint2 *tab = reinterpret_cast<const uint2 *>(p.steps + o);
+        const unsigned *xyt = reinterpret_cast<const unsigned *>(p.xy + o);
+        const unsigned h0 = __ldg(p.hit_off + probe * ndir + k), h1 = __ldg(p.hit_off + probe * ndir + k + 1);
+        const unsigned short *hl = p.hit_list;
+        // three stages in flight: the step number two hits ahead, (cell, ds) one hit ahead, (chi, S) of the hit being integrated
+        unsigned h = h0;
+        int s2 = h < h1 ? (int)__ldg(hl + h) : -1;
+        h++;
+        int c1 = -1;
+        float d1 = 0.f;
+        auto lookup = [&]() {  // stage 2 <- stage 1; stage 1 <- list
+            if (s2 >= 0) {
+                const unsigned e = __ldg(xyt + s2);
+                c1 = (Y0 + (int)(short)(e >> 16)) * p.nx + X0 + (int)(short)(e & 0xffffu);
+                d1 = __uint_as_float(__ldg(tab + s2).y);
+            } else {
+                c1 = -1;
+            }
+            s2 = h < h1 ? (int)__ldg(hl + h) : -1;
+            h++;
+        };
+        lookup();
+        float cP[LV], SP[LV], dsP = 0.f;
+        bool pend = false;
+        while (true) {
+            float cN[LV], SN[LV];
+            const bool have = c1 >= 0;
+            const float dsN = d1;
+            if (have) {
+                const unsigned long long d = (unsigned long long)(unsigned)c1 * cstride;
+                load_vec<LV>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(chiB) + d), cN);
+                load_vec<LV>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(SB) + d), SN);
+                lookup();
+            }
+            bool stop = !have;
+            if (pend) {  // integrate the cell gathered one round earlier
+                nwalk++;
+                const float mdsP = -dsP;
+                if constexpr (LV >= 2) {
+#pragma unroll
+                    for (int q = 0; q < LV / 2; q++) {
+                        f32x2 t2 = pk2(tau[2 * q], tau[2 * q + 1]), T2 = pk2(T[2 * q], T[2 * q + 1]), I2 = pk2(I[2 * q], I[2 * q + 1]);
+                        seg_update2(pk2(cP[2 * q], cP[2 * q + 1]), pk2(SP[2 * q], SP[2 * q + 1]), pk2(dsP, dsP), pk2(mdsP, mdsP), t2, T2, I2);
+                        up2(t2, tau[2 * q], tau[2 * q + 1]);
+                        up2(T2, T[2 * q], T[2 * q + 1]);
+                        up2(I2, I[2 * q], I[2 * q + 1]);
+                    }
+                } else {
+                    seg_update1(cP[0], SP[0], dsP, tau[0], T[0], I[0]);
+                }
+                if (p.early_exit) {  // this ray is opaque at every wavelength of the lane: nothing more can arrive
+                    float tmin = tau[0];
+#pragma unroll
+                    for (int v = 1; v < LV; v++) tmin = fminf(tmin, tau[v]);
+                    if (tmin > p.tau_cut) stop = true;
+                }
+            }
+            if (stop) break;
+            pend = true;
+            dsP = dsN;
+#pragma unroll
+            for (int v = 0; v < LV; v++) { cP[v] = cN[v]; SP[v] = SN[v]; }
+        }
+    }
+    if (p.walked != nullptr) {
+        unsigned long long mine = nwalk;
+        for (int sh = 16; sh > 0; sh >>= 1) mine += __shfl_down_sync(FULL, mine, sh);
+        if (lane == 0 && mine) atomicAdd(p.walked, mine);
+    }
+    // a2 / a3 as in march_kernel
+    if (valid) {
+        if (p.Aup == nullptr) {
+            const float *Ib = (2 * k < ndir) ? p.I_above : p.I_below;
+#pragma unroll
+            for (int v = 0; v < LV; v++) I[v] = fmaf(T[v], __ldg(Ib + nbI * LV + v), I[v]);
+        } else {
+            const int npxu = p.npx >> 1, npyu = p.npy >> 1;
+            int a0, a1, b0, b1;
+            float fa, fb;
+            parent_axis(a, npxu, a0, a1, fa);
+            parent_axis(b, npyu, b0, b1, fb);
+            const float *up = p.Aup + (((long long)nbI * ndir + k) * npyu) * (long long)npxu * LV;
+            float u00[LV], u01[LV], u10[LV], u11[LV];
+            load_vec<LV>(up + ((long long)b0 * npxu + a0) * LV, u00);
+            load_vec<LV>(up + ((long long)b0 * npxu + a1) * LV, u01);
+            load_vec<LV>(up + ((long long)b1 * npxu + a0) * LV, u10);
+            load_vec<LV>(up + ((long long)b1 * npxu + a1) * LV, u11);
+#pragma unroll
+            for (int v = 0; v < LV; v++) {
+                const float lo = fmaf(fa, u01[v] - u00[v], u00[v]);
+                const float hi = fmaf(fa, u11[v] - u10[v], u10[v]);
+                I[v] = fmaf(T[v], fmaf(fb, hi - lo, lo), I[v]);
+            }
+        }
+    }
+    // mean over the 4 children of a direction group: lanes B apart, added in child order like the lock-step march
+    float acc[LV];
+#pragma unroll
+    for (int v = 0; v < LV; v++) {
+        const float m1 = __shfl_down_sync(FULL, I[v], B), m2 = __shfl_down_sync(FULL, I[v], 2 * B), m3 = __shfl_down_sync(FULL, I[v], 3 * B);
+        acc[v] = 0.25f * ((((0.f + I[v]) + m1) + m2) + m3);
+    }
+    if (!valid || (r & 3) != 0) return;
+    const long long kg = k >> 2;
+    if (p.mode == 0) {
+        store_vec<LV>(p.out + (((long long)nbI * p.ngroups + kg) * nprobe + probe) * LV, acc);
+    } else if (p.mode == 1) {  // cascade 0: a4, J
+        float *o = p.out + probe * p.L + nbI * LV;
+        if ((nbI + 1) * LV <= p.L && (p.L % LV) == 0) {
+            store_vec<LV>(o, acc);
+        } else {
+#pragma unroll
+            for (int v = 0; v < LV; v++)
+                if (nbI * LV + v < p.L) o[v] = acc[v];
+        }
+    } else {
+        float sum = 0.f;
+#pragma unroll
+        for (int v = 0; v < LV; v++) sum = fmaf(__ldg(p.weights + nbI * LV + v), acc[v], sum);
+        p.out[(long long)nbI * nprobe + probe] = sum;
+    }
+}
+
+template <int LV, int B>
+static cudaError_t launch_march_list_b(const MarchParams &p, cudaStream_t st) {
+    constexpr int R = 32 / B, WARPS = 4;
+    const long long ndir = 4LL * p.ngroups, ndl = ndir < R ? ndir : R, ppw = R / ndl;
+    const long long nprobe = (long long)p.npx * p.npy;
+    const long long warps = (ndir / ndl) * ((nprobe + ppw - 1) / ppw) * ((p.nb + B - 1) / B);
+    const long long blocks = (warps + WARPS - 1) / WARPS;
+    if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+    if (blocks == 0) return cudaSuccess;
+    march_list_kernel<LV, B, WARPS, 6><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
+    return cudaGetLastError();
+}
+
+template <int LV>
+static cudaError_t launch_march_list(const MarchParams &p, cudaStream_t st) {
+    return p.list_b == 8 ? launch_march_list_b<LV, 8>(p, st) : launch_march_list_b<LV, 1>(p, st);
+}
+
 // Velocity-dependent line mode (linepk != null): 3 MUFU per segment-channel, ring of 2, 24 warps/SM.
 template <int LV, int NM = 1>
 static cudaError_t launch_march_line(const MarchParams &p, cudaStream_t st) {
@@ -1174,6 +1491,7 @@ static cudaError_t launch_march_line(const MarchParams &p, cudaStream_t st) {
 template <int LV>
 static cudaError_t launch_march_flat(const MarchParams &p, int variant, cudaStream_t st) {
     if (p.linepk != nullptr) return launch_march_line<LV>(p, st);
+    if (p.hit_list != nullptr) return launch_march_list<LV>(p, st);
     if (p.dist != nullptr) return launch_march_sparse<LV>(p, st);
     switch (variant) {
         case 0: return launch_march_variant<LV, 1, 2, 8, 3>(p, st);

@@ -144,8 +144,8 @@ def test_distance_field_march_is_bit_identical(oracle, kw):
     assert st1.empty_cells > 0.8 * atm.nx * atm.ny
     assert np.array_equal(dense, walk)
     for mode in (0, 1, 2, 3):                    # launch variants of the walk (rc_set_tuning "sparse_mode")
-        got, st = gpu(atm, analyse=True, tuning=dict(sparse_mode=mode))
-        assert st.sparse_march == 1 and np.array_equal(dense, got), mode
+        got, st = gpu(atm, analyse=True, tuning=dict(sparse_mode=mode, lists=0))
+        assert st.sparse_march == 1 and st.sparse_lists == 0 and np.array_equal(dense, got), mode
     check(atm, oracle, analyse=True)
     # per-wavelength J too (config 4 accumulates Jbar), with a boundary intensity so that the top cascade matters
     pl = dataclasses.replace(atm, accumulate=False)
@@ -153,6 +153,40 @@ def test_distance_field_march_is_bit_identical(oracle, kw):
     a, _ = gpu(pl)
     b, _ = gpu(pl, analyse=True)
     assert np.array_equal(a, b)
+
+
+@pytest.mark.parametrize("nlambda", [3, 16, 40, 43])
+def test_march_over_hit_lists_is_bit_identical(oracle, nlambda):
+    """rc_set_sparse_workspace: the occupied steps of every ray are found once per analysed atmosphere (they depend on
+    the geometry and the occupancy alone) and the march only gathers and integrates them - the same cells in the same order
+    as the distance-field walk and the lock-step march, so J agrees bit for bit; 8 wavelength batches per warp (cell-major
+    packed arrays) from 5 batches on, one otherwise; ragged last batch; without the second buffer the walk stays in use."""
+    import torch
+    from paper_2408_14425_b200 import binding
+    atm = dataclasses.replace(A.make_config(4, nx=256, ny=128, nlambda=nlambda, ncascades=6), accumulate=nlambda == 40)
+    dense, _ = gpu(atm)
+    walk, st0 = gpu(atm, analyse=True, tuning=dict(lists=0))
+    lists, st1 = gpu(atm, analyse=True)
+    assert st0.sparse_march == 1 and st0.sparse_lists == 0
+    assert st1.sparse_march == 1 and st1.sparse_lists == 1 and st1.sparse_list_bytes > 0
+    assert np.array_equal(dense, walk) and np.array_equal(dense, lists)
+    flagged = A.with_active_cells(atm)
+    a, _ = gpu(flagged)
+    b, st = gpu(flagged, analyse=True)
+    assert st.sparse_lists == 1 and np.array_equal(a, b)
+    # through the raw ABI without a second buffer: the size is reported, the walk is used
+    J, rc = binding.solve_atmosphere(atm)
+    assert rc.lib.rc_analyse_atmosphere(rc.handle) == 0
+    st = rc.get_stats()
+    assert st.sparse_march == 1 and st.sparse_lists == 0 and st.sparse_list_bytes == st1.sparse_list_bytes
+    assert np.array_equal(rc.solve_J().cpu().numpy(), dense)
+    small = torch.empty(1 << 16, dtype=torch.uint8, device="cuda")       # too small: still the walk
+    assert rc.lib.rc_set_sparse_workspace(rc.handle, small.data_ptr(), small.numel()) == 0
+    assert rc.lib.rc_analyse_atmosphere(rc.handle) == 0 and rc.get_stats().sparse_lists == 0
+    assert np.array_equal(rc.solve_J().cpu().numpy(), dense)
+    rc.close()
+    if nlambda == 3:
+        check(atm, oracle, analyse=True)
 
 
 def test_distance_field_march_on_dense_and_flagged_atmospheres(oracle):
