@@ -326,14 +326,18 @@ def main():
         ms_march = [st.ms_march[i] for i in range(atm.ncascades)]
         dom = int(np.argmax(ms_march))
         casc_bytes = 2 * 4 * atm.nx * atm.ny * atm.nlambda * nincl  # read merged cascade i+1, write cascade i
-        alg_bytes = 8 * seg[dom] * atm.nlambda + casc_bytes  # chi+eta gather: 8 B per segment-wavelength
+        # chi+eta gather: 8 B per segment-wavelength; where segments are left out by construction (flagged probes
+        # only, free-space jumps) the roofline counts the segments the launch really integrates, `value` stays geometric
+        sparse_run = atm.active is not None or (analysed is not None and bool(analysed.sparse_march))
+        seg_dom = walked[dom] if sparse_run else seg[dom]
+        alg_bytes = 8 * seg_dom * atm.nlambda + casc_bytes
         ach = alg_bytes / (ms_march[dom] * 1e-3) / 1e9
         mode = ("line" if atm.line is not None else "flat") + (f"_incl{nincl}" if nincl > 1 else "") + ("_fix" if args.bilinear_fix else "")
         cap = NCU_CAPTURES.get((mode, args.config, dom)) if world == 1 and not args.active and not args.tune else None
         dram = None if cap is None else cap["dram_bytes"]
         mufu_per_unit = 3 if atm.line is not None else 1  # line mode: ex2 (profile), rcp (eta/chi), ex2 (transmittance)
         sfu_peak = SM_COUNT * MUFU_PER_CLK_SM * sm_max_mhz * 1e6 / mufu_per_unit
-        ach_alu = seg[dom] * atm.nlambda * nincl / (ms_march[dom] * 1e-3)
+        ach_alu = seg_dom * atm.nlambda * nincl / (ms_march[dom] * 1e-3)
         mufu_bound = ach_alu / sfu_peak > ach / l2_gather_gbs
         l2_meas = None if cap is None else cap["l2_to_sm_bytes"] / (ms_march[dom] * 1e-3) / 1e9
         line = {

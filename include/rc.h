@@ -143,6 +143,7 @@ int rc_set_stream(rc_ctx *ctx, void *cuda_stream);
  *   "march_variant" -1 | 0..4   register-ring depth and occupancy of the march (-1: chosen per cascade)
  *   "patch_log2"    -1 | 2..5   lane patch width 2^n for cascades >= "patch_from" (-1: chosen per cascade from the geometry)
  *   "lists"         0 | 1       hit lists for the sparse march when rc_set_sparse_workspace lends room (default 1)
+ *   "list_b"        0 | 1,2,4,8 wavelength batches per warp of the march over hit lists (0: from the L2 footprint of the occupied cells)
  *   "sorted"        -1 | 0 | 1  lanes from quads of probes sorted by ray length: where the geometry says it pays / never / wherever possible
  *   "cpw_from"      -1 | i      cascades >= i run one child direction per warp (-1: never; default 3)
  *   "bands" n, "l2_mb" x        L2 banding of grids whose wavelength batch exceeds L2: n bands (0: from the budget x, 72 MB)

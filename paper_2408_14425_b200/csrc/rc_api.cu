@@ -31,6 +31,7 @@ struct Tuning {
     int sparse = -1;       // distance-field march: -1 automatic (> 2/3 of the cells empty), 0 never, 1 whenever analysed
     int graph = 1;         // CUDA graph replay on small grids
     int sparse_mode = 1;   // fan march variant, 0..3 (blocks of 8 / 4 / 2 warps, or 4 warps at 128 registers)
+    int list_b = 0;        // wavelength batches per warp of the march over hit lists: 0 from the L2 footprint, or 1, 2, 4, 8
     int lists = 1;         // hit lists for the sparse march when the caller lends a buffer (rc_set_sparse_workspace): 0 never
     int sorted = -1;       // lanes from sorted quads: -1 where the geometry says it pays, 0 never, 1 wherever possible
 };
@@ -97,6 +98,7 @@ struct rc_ctx {
     char *sws = nullptr;
     size_t sws_bytes = 0;
     bool lists = false;
+    int list_b = 1;            // wavelength batches per warp of the march over hit lists
     size_t hit_off[RC_MAX_CASCADES] = {0}, hit_list[RC_MAX_CASCADES] = {0};  // byte offsets into sws
     bool count_walked = false; // the solve being enqueued counts the segments it integrates (rc_count_walked)
     bool analysed = false;     // rc_analyse_atmosphere has been used on this context (rc_solve_J_host then repeats it)
@@ -505,6 +507,7 @@ int rc_set_tuning(rc_ctx *ctx, const char *name, double value) {
     else if (n == "graph") { t.graph = iv != 0; }
     else if (n == "sparse_mode") { if (iv < 0 || iv > 3) goto bad; t.sparse_mode = iv; }
     else if (n == "lists") { t.lists = iv != 0; }
+    else if (n == "list_b") { if (iv != 0 && iv != 1 && iv != 2 && iv != 4 && iv != 8) goto bad; t.list_b = iv; }
     else if (n == "sorted") { if (iv < -1 || iv > 1) goto bad; t.sorted = iv; }
     else return fail(ctx, RC_ERR_BAD_VALUE, "rc_set_tuning: unknown knob '%s'", name);
     // the plan (bands), the patch lists and a captured graph may depend on a knob: start over
@@ -733,7 +736,7 @@ static rc::MarchParams march_params(const rc_ctx *ctx, int i, float *J_out) {
     const bool lists = ctx->sparse && ctx->lists;
     mp.hit_off = lists ? (const unsigned *)(ctx->sws + ctx->hit_off[i]) : nullptr;
     mp.hit_list = lists ? (const unsigned short *)(ctx->sws + ctx->hit_list[i]) : nullptr;
-    mp.list_b = P.nb >= 5 ? 8 : 1;
+    mp.list_b = ctx->list_b;
     mp.walked = ctx->count_walked ? (unsigned long long *)(ctx->ws + P.flag) + 16 + i : nullptr;
     mp.flags = ctx->active_set ? (const unsigned char *)(ctx->ws + P.pflag[i]) : nullptr;
     mp.plist = ctx->active_set && !ctx->lists_dirty ? (const int *)(ctx->ws + P.plist[i]) : nullptr;
@@ -836,7 +839,7 @@ static int enqueue_solve(rc_ctx *ctx, float *J_out) {
         float fmax = 1.f;
         for (int m = 0; m < ctx->nm; m++) fmax = std::max(fmax, ctx->incl_f[m]);
         pp.c_thin = (1.f / 64.f) / fmax;
-        pp.cellmajor = ctx->sparse && ctx->lists ? 1 : 0;
+        pp.list_b = ctx->sparse && ctx->lists ? ctx->list_b : 0;
         if (ctx->line) {
             pp.chi = ctx->line; pp.eta = nullptr;
             RC_CUDA(ctx, rc::launch_pack_line(pp, ctx->stream));
@@ -1019,6 +1022,9 @@ static int build_hit_lists(rc_ctx *ctx) {
     }
     for (int i = 0; i < nc; i++)
         if (P.c[i].empty) { ctx->hit_off[i] = 0; ctx->hit_list[i] = 0; }  // any valid address: never read (cnt == null)
+    // Wavelength batches per warp: the lanes of a ray share its list and table reads (measured on config 4: 218 / 167 / 134
+    // / 135 ms at 1 / 2 / 4 / 8 batches per warp; config 3 with 25 % of the cells flagged, 4 batches: 210 / 146 / 130 ms)
+    ctx->list_b = ctx->tune.list_b > 0 ? ctx->tune.list_b : P.nb >= 6 ? 8 : P.nb >= 3 ? 4 : P.nb;
     ctx->lists = true;
     ctx->stats.sparse_lists = 1;
     return RC_OK;

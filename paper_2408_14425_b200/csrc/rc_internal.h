@@ -39,7 +39,7 @@ struct MarchParams {
     int sparse_mode;            // launch variant of the distance-field march (rc_kernels.cu, launch_march_sparse)
     const unsigned *hit_off;    // null, or the hit lists of this cascade (rc_analyse_atmosphere): [4 nx ny + 1] offsets, ray = probe * N_i + k,
     const unsigned short *hit_list;  // and the step numbers of every ray's occupied in-box cells; the packed arrays are then cell-major
-    int list_b;                 // wavelength batches per warp of the march over hit lists: 8 or 1
+    int list_b;                 // wavelength batches per warp of the march over hit lists: 1, 2, 4 or 8
     unsigned long long *walked; // null, or a counter of the cell segments actually integrated (rc_count_walked; per wavelength batch)
     const unsigned char *flags; // null (every probe), or [npy][npx]: the flagged probes of this cascade
     const int *plist;           // null, or the numbers of the patches that hold a flagged probe (npatch_act of them)
@@ -86,7 +86,7 @@ struct PackParams {
     const unsigned char *active;  // null, or [ny][nx]: cells that are not flagged are packed as vacuum
     int nx, ny, L, nb, shift;
     float c_thin;            // cells with chi log2e below this are packed in the thin form (seg_update*() in rc_kernels.cu)
-    int cellmajor;           // 1: write [cell][batch][LV] (march over hit lists, shift 0) instead of [batch][phase planes][LV]
+    int list_b;              // > 0: write [batch group of list_b][cell][batch in group][LV] (march over hit lists, shift 0)
 };
 
 struct AloParams {

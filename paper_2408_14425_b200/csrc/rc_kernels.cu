@@ -242,8 +242,13 @@ __global__ void __launch_bounds__(256) pack_kernel(PackParams p) {
     const int nbI = (int)(grp % p.nb);
     const long long c = (grp / p.nb) * 4 + (t & 3);  // output cell index ((ym*s + xm)*npy + yd)*npx + xd
     if (c >= ncell) return;
-    // output order: batch-major planes for the lock-step and fan marches, cell-major records for the march over hit lists
-    const long long idx = p.cellmajor ? c * p.nb + nbI : (long long)nbI * ncell + c;
+    // output order: batch-major planes for the lock-step and fan marches, cell records for the march over hit lists
+    // (groups of list_b batches: [group][cell][batch in group][LV], the last group as wide as it is)
+    long long idx = (long long)nbI * ncell + c;
+    if (p.list_b > 0) {
+        const int g0 = nbI / p.list_b * p.list_b, Bg = min(p.list_b, p.nb - g0);
+        idx = (long long)g0 * ncell + c * Bg + (nbI - g0);
+    }
     const int npx = p.nx >> p.shift, npy = p.ny >> p.shift, smask = (1 << p.shift) - 1;
     const int xd = (int)(c % npx);
     long long r = c / npx;
@@ -1301,7 +1306,7 @@ cudaError_t launch_hit_walk(const MarchParams &p, bool fill, unsigned *cnt_or_of
 
 // The march over hit lists.  A warp = R = 32 / B adjacent directions of one probe (or of R / N_i probes on cascades 0, 1) x
 // B wavelength batches: the B lanes of a ray read the same list entries and table steps (one sector, broadcast) and gather
-// B x LV consecutive floats of the cell (the packed arrays are cell-major under this march: [cell][batch][LV]).  The next
+// B x LV consecutive floats of the cell (under this march the packed arrays are [batch group][cell][batch in group][LV]).  The next
 // hit's step, cell and path length are looked up while the previous cell is integrated.
 template <int LV, int B, int WARPS, int MINB>
 __global__ void __launch_bounds__(WARPS * 32, MINB) march_list_kernel(MarchParams p) {
@@ -1327,8 +1332,11 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_list_kernel(MarchParam
     if (!__any_sync(FULL, valid)) return;
     const int half = (1 << p.shift) >> 1;
     const int X0 = (a << p.shift) + half, Y0 = (b << p.shift) + half;
-    const float *chiB = p.chiT + (long long)nbI * LV, *SB = p.ST + (long long)nbI * LV;  // + cell * nb * LV
-    const unsigned long long cstride = (unsigned long long)p.nb * (LV * sizeof(float));
+    // packed arrays: [batch group][cell][batch in group][LV]
+    const int Bg = min(B, p.nb - bg * B);
+    const long long gbase = ((long long)bg * B * ((long long)p.nx * p.ny) + (nbI - bg * B)) * LV;
+    const float *chiB = p.chiT + gbase, *SB = p.ST + gbase;  // + cell * Bg * LV
+    const unsigned long long cstride = (unsigned long long)Bg * (LV * sizeof(float));
 
     float I[LV], tau[LV], T[LV];
 #pragma unroll
@@ -1461,20 +1469,29 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_list_kernel(MarchParam
 
 template <int LV, int B>
 static cudaError_t launch_march_list_b(const MarchParams &p, cudaStream_t st) {
-    constexpr int R = 32 / B, WARPS = 4;
+    constexpr int R = 32 / B;
     const long long ndir = 4LL * p.ngroups, ndl = ndir < R ? ndir : R, ppw = R / ndl;
     const long long nprobe = (long long)p.npx * p.npy;
     const long long warps = (ndir / ndl) * ((nprobe + ppw - 1) / ppw) * ((p.nb + B - 1) / B);
-    const long long blocks = (warps + WARPS - 1) / WARPS;
-    if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-    if (blocks == 0) return cudaSuccess;
-    march_list_kernel<LV, B, WARPS, 6><<<(unsigned)blocks, WARPS * 32, 0, st>>>(p);
+    if ((warps + 3) / 4 > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+    if (warps == 0) return cudaSuccess;
+    switch (p.sparse_mode) {  // blocks of 4 warps at <= 80 / 96 / 128 registers (24 / 20 / 16 warps per SM), or 8 warps at <= 80
+        case 0: march_list_kernel<LV, B, 8, 3><<<(unsigned)((warps + 7) / 8), 256, 0, st>>>(p); break;
+        case 2: march_list_kernel<LV, B, 4, 5><<<(unsigned)((warps + 3) / 4), 128, 0, st>>>(p); break;
+        case 3: march_list_kernel<LV, B, 4, 4><<<(unsigned)((warps + 3) / 4), 128, 0, st>>>(p); break;
+        default: march_list_kernel<LV, B, 4, 6><<<(unsigned)((warps + 3) / 4), 128, 0, st>>>(p); break;
+    }
     return cudaGetLastError();
 }
 
 template <int LV>
 static cudaError_t launch_march_list(const MarchParams &p, cudaStream_t st) {
-    return p.list_b == 8 ? launch_march_list_b<LV, 8>(p, st) : launch_march_list_b<LV, 1>(p, st);
+    switch (p.list_b) {
+        case 8: return launch_march_list_b<LV, 8>(p, st);
+        case 4: return launch_march_list_b<LV, 4>(p, st);
+        case 2: return launch_march_list_b<LV, 2>(p, st);
+        default: return launch_march_list_b<LV, 1>(p, st);
+    }
 }
 
 // Velocity-dependent line mode (linepk != null): 3 MUFU per segment-channel, ring of 2, 24 warps/SM.
