@@ -198,7 +198,7 @@ int rc_analyse_atmosphere(rc_ctx *ctx);
  * march finding them again for every wavelength batch of every solve; the march then only gathers and integrates (the same
  * cells in the same order: bit-identical).  Their size is only known after counting: rc_analyse_atmosphere always counts
  * and reports rc_stats.sparse_list_bytes; when this buffer is missing or smaller the distance-field march stays in use
- * (rc_stats.sparse_lists = 0) - lend at least that many bytes and analyse again.  Config 4: 3.6 GB, 435 -> see DESIGN.md. */
+ * (rc_stats.sparse_lists = 0) - lend at least that many bytes and analyse again.  Config 4: 3.6 GB, 435 -> 134 ms per solve. */
 int rc_set_sparse_workspace(rc_ctx *ctx, void *dev_ptr, size_t bytes);
 
 /* Boundary intensity sampled by the top cascade: I_below[l] is seen by rays heading
