@@ -30,14 +30,15 @@ def test_lane_patches_follow_the_clipping_of_the_cascades():
 def test_sorted_quads_where_the_box_clips_the_rays():
     """Lanes from quads sorted by ray length replace the rectangular patch where that raises the estimated lock-step
     utilisation (config 2: cascade 5 0.75 -> 0.88, cascade 4 0.92 -> 0.97); never on the short cascades, never with the
-    bilinear fix (lanes = one parity class) and never on banded cascades (config 3, cascades 4-5)."""
+    bilinear fix (lanes = one parity class) and never on banded cascades (config 3, cascade 5)."""
     p = plan(2)
     assert [p.cascade_sorted[i] for i in range(8)] == [0, 0, 0, 1, 1, 1, 0, 0]
     assert 0.86 < p.lane_utilisation[5] < 0.90 and 0.96 < p.lane_utilisation[4] < 0.98
     assert all(p.lane_utilisation[i] > 0.99 for i in range(3))
     assert not any(plan(2, flags=FIX).cascade_sorted[i] for i in range(7))
     p3 = plan(3)
-    assert p3.cascade_banded[4] == p3.cascade_banded[5] == 1 and p3.cascade_sorted[4] == p3.cascade_sorted[5] == 0
+    assert p3.cascade_banded[5] == 1 and p3.cascade_sorted[5] == 0
+    assert p3.cascade_banded[4] == 0 and p3.cascade_sorted[4] == 1    # rays short against the banded axis: no bands needed
     assert p3.cascade_sorted[6] == 1
 
 
@@ -55,11 +56,12 @@ def test_wavelength_batches_and_channels():
 
 def test_l2_banding_only_where_a_batch_exceeds_l2():
     """Config 2: one batch of packed chi, S is 64 MB: no bands.  Configs 3 and 4: 256 MB: 4 bands along the
-    longer axis, for the long-ray cascades whose patches are small against a band; never cascades 0-3."""
+    longer axis, for the cascades whose rays are long against that axis (> 0.3 of it) and whose patches are small against
+    a band: cascade 5 of config 3; never cascades 0-4."""
     assert plan(2).nbands == 1 and not any(plan(2).cascade_banded[i] for i in range(8))
     p3, p4 = plan(3), plan(4)
     assert (p3.nbands, p3.band_axis) == (4, 0) and (p4.nbands, p4.band_axis) == (4, 1)
-    assert [p3.cascade_banded[i] for i in range(9)] == [0, 0, 0, 0, 1, 1, 0, 0, 0]
+    assert [p3.cascade_banded[i] for i in range(9)] == [0, 0, 0, 0, 0, 1, 0, 0, 0]
     assert not any(p4.cascade_banded[i] for i in range(4))
     # the moving-line mode gathers 24 bytes per cell for all wavelengths: always L2-resident
     assert plan(3, line_mode=True).nbands == 1 or not any(plan(3, line_mode=True).cascade_banded[i] for i in range(9))
