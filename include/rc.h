@@ -98,7 +98,8 @@ typedef struct {
     int sparse_march;                     /* the march walks the distance field (rc_analyse_atmosphere found > 2/3 empty) */
     int64_t active_cells;                 /* cells of interest (rc_set_active_cells); -1 = every cell */
     int64_t probes_flagged[RC_MAX_CASCADES]; /* with active cells: flagged probes of cascade i */
-    int sparse_lists;                     /* the sparse march runs over hit lists (rc_set_sparse_workspace was large enough) */
+    int sparse_lists;                     /* the sparse march runs over hit lists (rc_set_sparse_workspace was large enough): 1 = built by
+                                             the last rc_analyse_atmosphere, 2 = kept from an earlier one (same occupancy map) */
     int64_t sparse_list_bytes;            /* bytes the hit lists of the analysed atmosphere need in that buffer (0: not sparse) */
 } rc_stats;
 
@@ -198,7 +199,9 @@ int rc_analyse_atmosphere(rc_ctx *ctx);
  * march finding them again for every wavelength batch of every solve; the march then only gathers and integrates (the same
  * cells in the same order: bit-identical).  Their size is only known after counting: rc_analyse_atmosphere always counts
  * and reports rc_stats.sparse_list_bytes; when this buffer is missing or smaller the distance-field march stays in use
- * (rc_stats.sparse_lists = 0) - lend at least that many bytes and analyse again.  Config 4: 3.6 GB, 435 -> 134 ms per solve. */
+ * (rc_stats.sparse_lists = 0) - lend at least that many bytes and analyse again.  The lists are kept across atmospheres
+ * of the same shape and flags for as long as rc_analyse_atmosphere finds the same occupancy map (the formal solutions of an
+ * iteration change chi and eta, not where they vanish): the analysis then costs one scan.  Config 4: 3.6 GB, 435 -> 134 ms per solve. */
 int rc_set_sparse_workspace(rc_ctx *ctx, void *dev_ptr, size_t bytes);
 
 /* Boundary intensity sampled by the top cascade: I_below[l] is seen by rays heading

@@ -98,6 +98,8 @@ struct rc_ctx {
     char *sws = nullptr;
     size_t sws_bytes = 0;
     bool lists = false;
+    int64_t list_bytes = 0;
+    bool lists_built = false;  // the buffer holds lists for the occupancy map stored at its start: an analysis that finds the same map keeps them
     int list_b = 1;            // wavelength batches per warp of the march over hit lists
     size_t hit_off[RC_MAX_CASCADES] = {0}, hit_list[RC_MAX_CASCADES] = {0};  // byte offsets into sws
     bool count_walked = false; // the solve being enqueued counts the segments it integrates (rc_count_walked)
@@ -515,7 +517,7 @@ int rc_set_tuning(rc_ctx *ctx, const char *name, double value) {
     else return fail(ctx, RC_ERR_BAD_VALUE, "rc_set_tuning: unknown knob '%s'", name);
     // the plan (bands), the patch lists and a captured graph may depend on a knob: start over
     ctx->have_atm = false;
-    ctx->active_set = false; ctx->lists_dirty = false; ctx->sparse = false;
+    ctx->active_set = false; ctx->lists_dirty = false; ctx->sparse = false; ctx->lists_built = false;
     return RC_OK;
 bad:
     return fail(ctx, RC_ERR_BAD_VALUE, "rc_set_tuning: %s = %g is out of range", name, value);
@@ -553,7 +555,7 @@ static int prepare_shape(rc_ctx *ctx, int nx, int ny, int nlambda, bool line) {
         ctx->host_io = Pio.total <= ctx->ws_bytes;
         ctx->plan = ctx->host_io ? Pio : P;
         ctx->have_atm = false;
-        ctx->active_set = false; ctx->lists_dirty = false; ctx->sparse = false;
+        ctx->active_set = false; ctx->lists_dirty = false; ctx->sparse = false; ctx->lists_built = false;
         ctx->stats.active_cells = -1;
         // geometry tables: only when the grid size changed (they do not depend on nlambda)
         if (ctx->tab_nx != nx || ctx->tab_ny != ny) {
@@ -951,6 +953,7 @@ int rc_set_active_cells(rc_ctx *ctx, const unsigned char *active) {
     RC_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
     const Plan &P = ctx->plan;
     ctx->sparse = false;  // the distance field depends on the flags
+    ctx->lists_built = false;
     if (!active) {
         ctx->active_set = false; ctx->lists_dirty = false;
         ctx->stats.active_cells = -1;
@@ -994,7 +997,8 @@ static int build_hit_lists(rc_ctx *ctx) {
     unsigned long long *tot_d = (unsigned long long *)(ctx->ws + P.flag);  // [0..15] scratch counters
     RC_CUDA(ctx, cudaMemsetAsync(tot_d, 0, sizeof(*tot_d) * 16, ctx->stream));
     // room for the offsets? then count per ray, else only the totals (to report the size)
-    size_t cur = bsum_bytes;
+    const size_t occ_bytes = align_up((size_t)P.nx * P.ny);      // the occupancy map the lists belong to
+    size_t cur = occ_bytes + bsum_bytes;
     for (int i = 0; i < nc; i++) {
         if (P.c[i].empty) continue;
         ctx->hit_off[i] = cur; cur += off_bytes;
@@ -1015,12 +1019,13 @@ static int build_hit_lists(rc_ctx *ctx) {
         fits32 = fits32 && tot[i] < 0xffffffffULL;
     }
     ctx->stats.sparse_list_bytes = (int64_t)cur;
+    ctx->list_bytes = (int64_t)cur;
     if (!have_off || cur > ctx->sws_bytes || !fits32) return RC_OK;  // no room (or too many hits): the distance-field march
     for (int i = 0; i < nc; i++) {
         if (P.c[i].empty) continue;
         rc::MarchParams mp = march_params(ctx, i, nullptr);
         unsigned *off = (unsigned *)(ctx->sws + ctx->hit_off[i]);
-        RC_CUDA(ctx, rc::launch_hit_scan(off, (long long)nrays, (unsigned *)ctx->sws, tot[i], ctx->stream));
+        RC_CUDA(ctx, rc::launch_hit_scan(off, (long long)nrays, (unsigned *)(ctx->sws + occ_bytes), tot[i], ctx->stream));
         RC_CUDA(ctx, rc::launch_hit_walk(mp, true, off, (unsigned short *)(ctx->sws + ctx->hit_list[i]), nullptr, ctx->stream));
     }
     for (int i = 0; i < nc; i++)
@@ -1028,7 +1033,9 @@ static int build_hit_lists(rc_ctx *ctx) {
     // Wavelength batches per warp: the lanes of a ray share its list and table reads (measured on config 4: 218 / 167 / 134
     // / 135 ms at 1 / 2 / 4 / 8 batches per warp; config 3 with 25 % of the cells flagged, 4 batches: 210 / 146 / 130 ms)
     ctx->list_b = ctx->tune.list_b > 0 ? ctx->tune.list_b : P.nb >= 6 ? 8 : P.nb >= 3 ? 4 : P.nb;
+    RC_CUDA(ctx, cudaMemcpyAsync(ctx->sws, ctx->ws + P.occ8, (size_t)P.nx * P.ny, cudaMemcpyDeviceToDevice, ctx->stream));
     ctx->lists = true;
+    ctx->lists_built = true;
     ctx->stats.sparse_lists = 1;
     return RC_OK;
 }
@@ -1045,6 +1052,15 @@ int rc_analyse_atmosphere(rc_ctx *ctx) {
                                                  ctx->active_set ? (const unsigned char *)(ctx->ws + P.pflag[0]) : nullptr, P.nx, P.ny, P.L,
                                                  (int *)(ctx->ws + P.A[0]), (unsigned char *)(ctx->ws + P.occ8), (unsigned char *)(ctx->ws + P.d1),
                                                  (unsigned char *)(ctx->ws + P.dist), cnt, ctx->stream));  // A[0] is free between solves
+    // hit lists built for an earlier atmosphere of the same shape and flags stay good while the occupancy map is the same
+    // (the formal solutions of an iteration, change chi and eta, not where they vanish)
+    int differs = 1;
+    int *dflag = (int *)(cnt + 1);
+    if (ctx->lists_built) {
+        RC_CUDA(ctx, cudaMemsetAsync(dflag, 0, sizeof(int), ctx->stream));
+        RC_CUDA(ctx, rc::launch_occ_differs((const unsigned char *)(ctx->ws + P.occ8), (const unsigned char *)ctx->sws, (long long)P.nx * P.ny, dflag, ctx->stream));
+        RC_CUDA(ctx, cudaMemcpyAsync(&differs, dflag, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+    }
     RC_CUDA(ctx, cudaMemcpyAsync(&h, cnt, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream));
     RC_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     ctx->stats.empty_cells = (int64_t)h;
@@ -1058,7 +1074,17 @@ int rc_analyse_atmosphere(rc_ctx *ctx) {
     ctx->lists = false;
     ctx->stats.sparse_lists = 0;
     ctx->stats.sparse_list_bytes = 0;
-    if (ctx->sparse && ctx->tune.lists != 0) { const int rc = build_hit_lists(ctx); if (rc != RC_OK) return rc; }
+    if (ctx->sparse && ctx->tune.lists != 0) {
+        if (ctx->lists_built && !differs) {
+            ctx->lists = true;
+            ctx->stats.sparse_lists = 2;
+            ctx->stats.sparse_list_bytes = ctx->list_bytes;
+        } else {
+            ctx->lists_built = false;
+            const int rc = build_hit_lists(ctx);
+            if (rc != RC_OK) return rc;
+        }
+    }
     return RC_OK;
 }
 
@@ -1067,7 +1093,7 @@ int rc_set_sparse_workspace(rc_ctx *ctx, void *dev_ptr, size_t bytes) {
     if (dev_ptr && ((uintptr_t)dev_ptr % ALIGN) != 0) return fail(ctx, RC_ERR_NO_WORKSPACE, "sparse workspace pointer is not %zu-byte aligned", ALIGN);
     ctx->sws = (char *)dev_ptr;
     ctx->sws_bytes = dev_ptr ? bytes : 0;
-    ctx->lists = false;  // the lists lived in the old buffer: rc_analyse_atmosphere again
+    ctx->lists = false; ctx->lists_built = false;  // the lists lived in the old buffer: rc_analyse_atmosphere again
     ctx->list_version++;
     return RC_OK;
 }

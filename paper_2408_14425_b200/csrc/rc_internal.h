@@ -128,6 +128,7 @@ cudaError_t launch_build_distance_field(const float *chi, const float *eta, cons
                                         unsigned long long *nempty, cudaStream_t st);
 cudaError_t launch_alo(const AloParams &p, cudaStream_t st);
 cudaError_t launch_hit_walk(const MarchParams &p, bool fill, unsigned *cnt_or_off, unsigned short *list, unsigned long long *total, cudaStream_t st);
+cudaError_t launch_occ_differs(const unsigned char *a, const unsigned char *b, long long n, int *flag, cudaStream_t st);
 cudaError_t launch_hit_scan(unsigned *a, long long n, unsigned *bsum, unsigned long long total, cudaStream_t st);
 cudaError_t launch_bulk_probe(const float *buf, unsigned long long nsector, int iters, int sms, float *sink, cudaStream_t st, long long *bytes);
 cudaError_t launch_validate(const float *chi, const float *eta, long long n, int *flag, cudaStream_t st);

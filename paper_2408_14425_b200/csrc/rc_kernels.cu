@@ -1284,6 +1284,18 @@ __global__ void __launch_bounds__(1024) scan_add_kernel(unsigned *a, long long n
     if (i == n) a[n] = (unsigned)total;
 }
 
+// *flag = 1 if the two occupancy maps differ anywhere (hit lists are kept while the occupancy they were built for stands)
+__global__ void occ_differs_kernel(const unsigned char *a, const unsigned char *b, long long n, int *flag) {
+    bool d = false;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) d = d || a[i] != b[i];
+    if (__any_sync(FULL, d) && (threadIdx.x & 31) == 0) *flag = 1;
+}
+
+cudaError_t launch_occ_differs(const unsigned char *a, const unsigned char *b, long long n, int *flag, cudaStream_t st) {
+    occ_differs_kernel<<<148 * 4, 256, 0, st>>>(a, b, n, flag);
+    return cudaGetLastError();
+}
+
 // counts -> offsets for one cascade; `total` (host) must be the sum already known from the counting pass
 cudaError_t launch_hit_scan(unsigned *a, long long n, unsigned *bsum, unsigned long long total, cudaStream_t st) {
     const long long nblocks = (n + 1023) / 1024;

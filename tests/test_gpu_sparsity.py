@@ -211,6 +211,27 @@ def test_distance_field_march_on_dense_and_flagged_atmospheres(oracle):
     check(emit, oracle, analyse=True, tuning=dict(sparse=1))
 
 
+def test_hit_lists_are_kept_while_the_occupancy_stands():
+    """A new atmosphere with the same occupancy map (other values in the same cells) keeps the hit lists (sparse_lists = 2);
+    another map rebuilds them (1); both give the lock-step result bit for bit."""
+    import torch
+    from paper_2408_14425_b200 import binding
+    atm = dataclasses.replace(A.make_config(4, nx=256, ny=128, nlambda=8, ncascades=6), accumulate=False)
+    J, rc = binding.solve_atmosphere(atm, analyse=True)
+    assert rc.get_stats().sparse_lists == 1
+    for scale, seed, want in ((3.0, None, 2), (1.0, 99, 1), (0.5, 99, 2)):
+        other = atm if seed is None else dataclasses.replace(A.make_config(4, nx=256, ny=128, nlambda=8, ncascades=6, seed=seed), accumulate=False)
+        other = dataclasses.replace(other, chi=(other.chi * scale).astype(np.float32), eta=(other.eta * scale * 0.7).astype(np.float32))
+        chi, eta = torch.from_numpy(other.chi).cuda(), torch.from_numpy(other.eta).cuda()
+        rc.set_atmosphere(chi, eta)
+        st = rc.analyse_atmosphere()
+        assert st.sparse_march == 1 and st.sparse_lists == want, (scale, seed, st.sparse_lists)
+        got = rc.solve_J().cpu().numpy()
+        ref, _ = gpu(other)
+        assert np.array_equal(ref, got)
+    rc.close()
+
+
 def test_analysis_belongs_to_one_atmosphere():
     """A new atmosphere switches the distance-field march off until it is analysed again; rc_solve_J_host repeats the
     analysis by itself once the context has used it."""
