@@ -65,6 +65,8 @@ struct Plan {
     int plist_cap[RC_MAX_CASCADES] = {0};
     size_t occ8 = 0, d1 = 0, dist = 0;
     CascadePlan c[RC_MAX_CASCADES];
+    bool multi_pack = false;        // small grids: per-cascade packed arrays, one pack launch per solve
+    size_t chiT_c[RC_MAX_CASCADES] = {0}, ST_c[RC_MAX_CASCADES] = {0};
     size_t chiT = 0, ST = 0, A[2] = {0, 0}, Jpart = 0, bc_below = 0, bc_above = 0, weights = 0, flag = 0;
     size_t io_chi = 0, io_eta = 0, io_J = 0;
     size_t total = 0;
@@ -362,6 +364,14 @@ bool make_plan_uncached(const rc_config &cfg, const Tuning &tune, int nm, bool l
     } else {
         P.chiT = cur; cur += field;
         P.ST = cur;   cur += field;
+        // launch-bound grids (config 0): every cascade gets its own packed arrays so that ONE launch packs for all of them
+        static_assert(RC_MAX_CASCADES == 12, "PackParams::shifts");
+        P.multi_pack = (long long)ncell * P.Lpad * P.NM <= (1LL << 21);
+        for (int i = 0; i <= top && P.multi_pack; i++) {
+            if (P.c[i].empty) continue;
+            P.chiT_c[i] = cur; cur += field;
+            P.ST_c[i] = cur;   cur += field;
+        }
     }
     P.A[0] = cur; cur += field * P.NM;  // merged cascades hold every (wavelength, inclination) channel
     P.A[1] = cur; cur += field * P.NM;
@@ -732,8 +742,9 @@ static rc::MarchParams march_params(const rc_ctx *ctx, int i, float *J_out) {
     const int top = ctx->cfg.ncascades - 1;
     const bool accum = (ctx->cfg.flags & RC_ACCUM_J) != 0;
     rc::MarchParams mp;
-    mp.chiT = (const float *)(ctx->ws + P.chiT);
-    mp.ST = (const float *)(ctx->ws + P.ST);
+    const bool multi = P.multi_pack && !ctx->sparse && !ctx->line && !c.empty;
+    mp.chiT = (const float *)(ctx->ws + (multi ? P.chiT_c[i] : P.chiT));
+    mp.ST = (const float *)(ctx->ws + (multi ? P.ST_c[i] : P.ST));
     mp.linepk = ctx->line ? (const float *)(ctx->ws + P.chiT) : nullptr;
     mp.xls = ctx->line ? (const float *)(ctx->ws + P.xls) : nullptr;
     mp.dist = ctx->sparse ? (const unsigned char *)(ctx->ws + P.dist) : nullptr;
@@ -834,7 +845,7 @@ static int enqueue_solve(rc_ctx *ctx, float *J_out) {
         else RC_CUDA(ctx, cudaMemsetAsync(J_out, 0, ncell * P.L * sizeof(float), ctx->stream));
     }
     auto pack = [&](int shift) -> int {
-        rc::PackParams pp;
+        rc::PackParams pp{};
         pp.chi = ctx->chi; pp.eta = ctx->eta;
         pp.chiT = (float *)(ctx->ws + P.chiT); pp.ST = (float *)(ctx->ws + P.ST);
         pp.active = ctx->active_set ? (const unsigned char *)(ctx->ws + P.pflag[0]) : nullptr;
@@ -856,9 +867,28 @@ static int enqueue_solve(rc_ctx *ctx, float *J_out) {
     };
     // the distance-field march gathers from plain cell order: one pack for every cascade
     if (ctx->sparse) { const int rc = pack(0); if (rc != RC_OK) return rc; }
+    const bool multi = P.multi_pack && !ctx->sparse && !ctx->line;
+    if (multi) {  // small grids: one launch packs for every cascade
+        rc::PackParams pp{};
+        pp.chi = ctx->chi; pp.eta = ctx->eta;
+        pp.active = ctx->active_set ? (const unsigned char *)(ctx->ws + P.pflag[0]) : nullptr;
+        pp.nx = P.nx; pp.ny = P.ny; pp.L = P.L; pp.nb = P.nb;
+        float fmax = 1.f;
+        for (int m = 0; m < ctx->nm; m++) fmax = std::max(fmax, ctx->incl_f[m]);
+        pp.c_thin = (1.f / 64.f) / fmax;
+        pp.list_b = 0;
+        for (int i = top; i >= 0; i--) {
+            if (P.c[i].empty) continue;
+            pp.shifts[pp.nmulti] = P.c[i].fix ? i + 1 : i;
+            pp.chiTm[pp.nmulti] = (float *)(ctx->ws + P.chiT_c[i]);
+            pp.STm[pp.nmulti] = (float *)(ctx->ws + P.ST_c[i]);
+            pp.nmulti++;
+        }
+        if (pp.nmulti > 0) { RC_CUDA(ctx, rc::launch_pack(pp, P.LV, ctx->stream)); launches++; }
+    }
     for (int i = top; i >= 0; i--) {
         const CascadePlan &c = P.c[i];
-        if (!c.empty && !ctx->sparse) { const int rc = pack(c.fix ? i + 1 : i); if (rc != RC_OK) return rc; }
+        if (!c.empty && !ctx->sparse && !multi) { const int rc = pack(c.fix ? i + 1 : i); if (rc != RC_OK) return rc; }
         if (ev) RC_CUDA(ctx, cudaEventRecord(ev[1 + 2 * (top - i)], ctx->stream));
         rc::MarchParams mp = march_params(ctx, i, J_out);
         if (!c.banded || ctx->sparse) {  // the distance-field march gathers occupied cells only: they fit L2

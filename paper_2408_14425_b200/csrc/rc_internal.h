@@ -87,6 +87,11 @@ struct PackParams {
     int nx, ny, L, nb, shift;
     float c_thin;            // cells with chi log2e below this are packed in the thin form (seg_update*() in rc_kernels.cu)
     int list_b;              // > 0: write [batch group of list_b][cell][batch in group][LV] (march over hit lists, shift 0)
+    // small grids (launch bound): nmulti > 0 packs for nmulti cascades in one launch, cascade j (blockIdx.y) with spacing
+    // 2^shifts[j] into chiTm[j], STm[j]; shift, chiT, ST above are then unused
+    int nmulti;
+    int shifts[12];                    // (12 = RC_MAX_CASCADES of rc.h)
+    float *chiTm[12], *STm[12];
 };
 
 struct AloParams {

@@ -249,13 +249,16 @@ __global__ void __launch_bounds__(256) pack_kernel(PackParams p) {
         const int g0 = nbI / p.list_b * p.list_b, Bg = min(p.list_b, p.nb - g0);
         idx = (long long)g0 * ncell + c * Bg + (nbI - g0);
     }
-    const int npx = p.nx >> p.shift, npy = p.ny >> p.shift, smask = (1 << p.shift) - 1;
+    // small grids: one launch packs for every cascade (blockIdx.y), each into its own arrays
+    const int shift = p.nmulti > 0 ? p.shifts[blockIdx.y] : p.shift;
+    float *const chiT = p.nmulti > 0 ? p.chiTm[blockIdx.y] : p.chiT, *const ST = p.nmulti > 0 ? p.STm[blockIdx.y] : p.ST;
+    const int npx = p.nx >> shift, npy = p.ny >> shift, smask = (1 << shift) - 1;
     const int xd = (int)(c % npx);
     long long r = c / npx;
     const int yd = (int)(r % npy);
     r /= npy;
-    const int xm = (int)r & smask, ym = (int)(r >> p.shift);
-    const int x = (xd << p.shift) + xm, y = (yd << p.shift) + ym;
+    const int xm = (int)r & smask, ym = (int)(r >> shift);
+    const int x = (xd << shift) + xm, y = (yd << shift) + ym;
     const long long src = ((long long)y * p.nx + x) * p.L + (long long)nbI * LV;
     float ch[LV], et[LV], c2[LV], S[LV];
     if ((nbI + 1) * LV <= p.L && (p.L % LV) == 0) {
@@ -283,7 +286,7 @@ __global__ void __launch_bounds__(256) pack_kernel(PackParams p) {
 #pragma unroll
         for (int v = 0; v < LV; v++) { c2[v] = 0.f; S[v] = 0.f; }
     }
-    float *oc = p.chiT + idx * LV, *os = p.ST + idx * LV;
+    float *oc = chiT + idx * LV, *os = ST + idx * LV;
     if constexpr (LV == 8) {
         reinterpret_cast<float4 *>(oc)[0] = make_float4(c2[0], c2[1], c2[2], c2[3]);
         reinterpret_cast<float4 *>(oc)[1] = make_float4(c2[4], c2[5], c2[6], c2[7]);
@@ -334,7 +337,7 @@ cudaError_t launch_pack_line(const PackParams &p, cudaStream_t st) {
 
 cudaError_t launch_pack(const PackParams &p, int LV, cudaStream_t st) {
     const long long n = (((long long)p.nx * p.ny + 3) / 4) * 4 * p.nb;
-    const unsigned blocks = (unsigned)((n + 255) / 256);
+    const dim3 blocks((unsigned)((n + 255) / 256), (unsigned)(p.nmulti > 0 ? p.nmulti : 1));
     switch (LV) {
         case 8: pack_kernel<8><<<blocks, 256, 0, st>>>(p); break;
         case 4: pack_kernel<4><<<blocks, 256, 0, st>>>(p); break;
