@@ -156,9 +156,9 @@ bool shape_ok(const rc_config &cfg, int nx, int ny, int L) {
 // estimated here from the geometry alone (ray length to the box edge, clipped to the interval) for
 // the candidate shapes 32x1 .. 4x8, over a sample of directions.  Wider patches gather longer
 // contiguous runs, so the widest shape within 2 % of the best utilisation wins.
-int choose_patch(int nx, int ny, int i, double ta, double tb, double *util) {
+int choose_patch(int nx, int ny, int i, double ta, double tb, double *util, int step = 1) {  // step 2: one parity class (bilinear fix)
     *util = 1.0;
-    const int s = 1 << i, npx = nx >> i, npy = ny >> i;
+    const int s = 1 << i, npx = (nx >> i) / step, npy = (ny >> i) / step;
     int widest = 5;
     while (widest > 0 && (1 << widest) > npx) widest--;
     if (std::fmin(tb, std::hypot((double)nx, (double)ny)) <= std::min(nx, ny) / 16.0) return widest;
@@ -172,7 +172,7 @@ int choose_patch(int nx, int ny, int i, double ta, double tb, double *util) {
         const double th = 2.0 * M_PI * ((double)k + 0.5) / (double)ndir, cx = std::cos(th), sy = std::sin(th);
         for (int b = 0; b < npy; b++)
             for (int a = 0; a < npx; a++) {
-                const double X = (a + 0.5) * s, Y = (b + 0.5) * s;
+                const double X = (step * a + 0.5) * s, Y = (step * b + 0.5) * s;
                 const double te = std::fmin(cx > 0 ? (nx - X) / cx : -X / cx, sy > 0 ? (ny - Y) / sy : -Y / sy);
                 const double l = std::fmax(std::fmin(te, tb) - ta, 0.0) * (std::fabs(cx) + std::fabs(sy));
                 len[(size_t)b * npx + a] = l;
@@ -202,8 +202,9 @@ int choose_patch(int nx, int ny, int i, double ta, double tb, double *util) {
 // quads of the lattice are ordered by the length of their longest ray inside the box (geometry alone, as in
 // choose_patch) and a warp takes 8 consecutive quads: its 32 lock-step lanes then finish almost together wherever the
 // quads sit.  Returns the estimated utilisation; fills `list` ([nblocks][qpad], 0xffff = padding) when given.
-double sorted_quads(int nx, int ny, int i, double ta, double tb, int qpad, std::vector<unsigned short> *list) {
-    const int s = 1 << i, npx = nx >> i, npy = ny >> i, qx = npx / 4, nq = qx * npy;
+// `step` = 2: the lattice of one parity class of the bilinear fix (every other probe per axis).
+double sorted_quads(int nx, int ny, int i, double ta, double tb, int qpad, std::vector<unsigned short> *list, int step = 1) {
+    const int s = 1 << i, npx = (nx >> i) / step, npy = (ny >> i) / step, qx = npx / 4, nq = qx * npy;
     const long long ndir = 1LL << (2 * (i + 1));
     const int nblocks = (int)(ndir / 32);
     if (list) list->assign((size_t)nblocks * qpad, (unsigned short)0xffff);
@@ -217,7 +218,7 @@ double sorted_quads(int nx, int ny, int i, double ta, double tb, int qpad, std::
             for (int q = 0; q < qx; q++) {
                 double m = 0.0;
                 for (int j = 0; j < 4; j++) {
-                    const double X = (4 * q + j + 0.5) * s, Y = (b + 0.5) * s;
+                    const double X = (step * (4 * q + j) + 0.5) * s, Y = (step * b + 0.5) * s;
                     const double te = std::fmin(cx > 0 ? (nx - X) / cx : -X / cx, sy > 0 ? (ny - Y) / sy : -Y / sy);
                     const double l = std::fmax(std::fmin(te, tb) - ta, 0.0) * (std::fabs(cx) + std::fabs(sy));
                     total += l;
@@ -271,8 +272,8 @@ bool make_plan_uncached(const rc_config &cfg, const Tuning &tune, int nm, bool l
         c.pw_log2 = 5;
         while (c.pw_log2 > 0 && (1 << c.pw_log2) > (nx >> i)) c.pw_log2--;
         if (c.empty) continue;
-        c.pw_log2 = choose_patch(nx, ny, i, c.ta, c.tb, &c.patch_util);
         c.fix = (cfg.flags & RC_BILINEAR_FIX) != 0 && i < top;
+        c.pw_log2 = choose_patch(nx, ny, i, c.ta, c.tb, &c.patch_util, c.fix && (nx >> i) >= 2 && (ny >> i) >= 2 ? 2 : 1);
         std::vector<long long> local;
         std::vector<long long> &o = offs ? (*offs)[i] : local;
         const int nsub = c.fix ? 16 : 1;
@@ -334,11 +335,12 @@ bool make_plan_uncached(const rc_config &cfg, const Tuning &tune, int nm, bool l
     // lanes from sorted quads where that beats the best rectangular patch (long, clipped rays: the upper cascades)
     for (int i = 2; i <= top; i++) {
         CascadePlan &c = P.c[i];
-        const int npx = nx >> i, npy = ny >> i;
+        const int step = c.fix ? 2 : 1;   // bilinear fix: lanes are probes of one parity class
+        const int npx = (nx >> i) / step, npy = (ny >> i) / step;
         const long long nq = (long long)(npx / 4) * npy;
-        if (c.empty || c.fix || c.banded || npx % 4 != 0 || nq < 8 || nq > 65535 || c.patch_util > 0.985 || tune.sorted == 0) continue;
+        if (c.empty || c.banded || npx % 4 != 0 || nq < 8 || nq > 65535 || c.patch_util > 0.985 || tune.sorted == 0) continue;
         c.qpad = (int)((nq + 7) / 8 * 8);
-        if (sorted_quads(nx, ny, i, c.ta, c.tb, c.qpad, nullptr) < c.patch_util + 0.015 && tune.sorted != 1) continue;
+        if (sorted_quads(nx, ny, i, c.ta, c.tb, c.qpad, nullptr, step) < c.patch_util + 0.015 && tune.sorted != 1) continue;
         c.sorted = true;
         c.qlist_off = cur; cur = align_up(cur + sizeof(unsigned short) * (size_t)(c.ndir / 32) * c.qpad);
     }
@@ -440,7 +442,7 @@ int rc_plan_query(const rc_config *cfg, int ninclinations, int line_mode, int nx
         out->cascade_banded[i] = P.c[i].banded;
         out->patch_w[i] = 1 << P.c[i].pw_log2;
         out->cascade_sorted[i] = P.c[i].sorted;
-        out->lane_utilisation[i] = (float)(P.c[i].sorted ? sorted_quads(nx, ny, i, P.c[i].ta, P.c[i].tb, P.c[i].qpad, nullptr) : P.c[i].patch_util);
+        out->lane_utilisation[i] = (float)(P.c[i].sorted ? sorted_quads(nx, ny, i, P.c[i].ta, P.c[i].tb, P.c[i].qpad, nullptr, P.c[i].fix ? 2 : 1) : P.c[i].patch_util);
         out->table_steps[i] = P.c[i].slots;
     }
     return RC_OK;
@@ -594,7 +596,7 @@ static int prepare_shape(rc_ctx *ctx, int nx, int ny, int nlambda, bool line) {
         for (int i = 0; i < ctx->cfg.ncascades; i++) {
             const CascadePlan &c = ctx->plan.c[i];
             if (!c.sorted) continue;
-            sorted_quads(nx, ny, i, c.ta, c.tb, c.qpad, &ctx->qlist_host[i]);
+            sorted_quads(nx, ny, i, c.ta, c.tb, c.qpad, &ctx->qlist_host[i], c.fix ? 2 : 1);
             RC_CUDA(ctx, cudaMemcpyAsync(ctx->ws + c.qlist_off, ctx->qlist_host[i].data(), sizeof(unsigned short) * ctx->qlist_host[i].size(),
                                          cudaMemcpyHostToDevice, ctx->stream));
         }

@@ -503,7 +503,7 @@ __device__ __forceinline__ WarpWork warp_work(const MarchParams &p, long long W,
     if (p.cpw) W >>= 2;  // child-per-warp: 4 consecutive warps (one per child direction) share everything else
     const int G = min(p.kg_n, 8);
     const int ncls = p.fix ? 4 : 1;
-    const long long npatch = p.qlist != nullptr ? p.qpad >> 3 : p.plist != nullptr ? p.npatch_act : (long long)p.npatch_x * p.npatch_y * ncls;
+    const long long npatch = p.qlist != nullptr ? (long long)(p.qpad >> 3) * ncls : p.plist != nullptr ? p.npatch_act : (long long)p.npatch_x * p.npatch_y * ncls;
     WarpWork r;
     const int kg_lo = (int)(W % G);
     W /= G;
@@ -516,13 +516,16 @@ __device__ __forceinline__ WarpWork warp_work(const MarchParams &p, long long W,
         r.kg = (kgb * G + kg_lo + p.kg_off) & (p.ngroups - 1);
         r.nbI = (int)(W / kgb_n);
         r.any = r.nbI < p.nb;
-        r.cls = 0;
+        // (bilinear fix: the lattice of one parity class, spacing 2s; the same list serves the four classes)
+        r.cls = (int)(patch % ncls);
+        patch /= ncls;
         const unsigned q = __ldg(p.qlist + (long long)kgb * p.qpad + patch * 8 + (lane >> 2));
-        const int qx = p.npx >> 2;
+        const int lxq = p.fix ? p.npx >> 1 : p.npx, qx = lxq >> 2;
         r.valid = q != 0xffffu;
-        r.b = r.valid ? (int)(q / qx) : 0;
-        r.a = r.valid ? (int)(q - (unsigned)r.b * qx) * 4 + (lane & 3) : 0;
-        r.gidx = (unsigned)r.b * p.npx + r.a;
+        const int lbq = r.valid ? (int)(q / qx) : 0, laq = r.valid ? (int)(q - (unsigned)lbq * qx) * 4 + (lane & 3) : 0;
+        r.a = p.fix ? 2 * laq + (r.cls & 1) : laq;
+        r.b = p.fix ? 2 * lbq + (r.cls >> 1) : lbq;
+        r.gidx = (unsigned)lbq * lxq + laq;
         return r;
     }
     // sparsity: only the patches that hold a flagged probe are launched (plist: their numbers, in order)
@@ -550,7 +553,7 @@ __device__ __forceinline__ WarpWork warp_work(const MarchParams &p, long long W,
 }
 
 __host__ __device__ inline long long march_warps(const MarchParams &p) {
-    const long long npatch = p.qlist != nullptr ? p.qpad >> 3 : p.plist != nullptr ? p.npatch_act : (long long)p.npatch_x * p.npatch_y * (p.fix ? 4 : 1);
+    const long long npatch = p.qlist != nullptr ? (long long)(p.qpad >> 3) * (p.fix ? 4 : 1) : p.plist != nullptr ? p.npatch_act : (long long)p.npatch_x * p.npatch_y * (p.fix ? 4 : 1);
     return npatch * p.kg_n * p.nb * (p.cpw ? 4 : 1);
 }
 
@@ -1773,7 +1776,7 @@ cudaError_t launch_build_distance_field(const float *chi, const float *eta, cons
 __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) count_kernel(MarchParams p, unsigned long long *total) {
     const int lane = threadIdx.x & 31;
     const long long W = (long long)blockIdx.x * WARPS_PER_BLOCK + (threadIdx.x >> 5);
-    if (W >= (p.qlist != nullptr ? (long long)(p.qpad >> 3) : p.plist != nullptr ? (long long)p.npatch_act : (long long)p.npatch_x * p.npatch_y * (p.fix ? 4 : 1)) * p.ngroups || p.cnt == nullptr) return;
+    if (W >= (p.qlist != nullptr ? (long long)(p.qpad >> 3) * (p.fix ? 4 : 1) : p.plist != nullptr ? (long long)p.npatch_act : (long long)p.npatch_x * p.npatch_y * (p.fix ? 4 : 1)) * p.ngroups || p.cnt == nullptr) return;
     const WarpWork ww = warp_work(p, W, lane);  // batch index is the slowest: W covers batch 0 only
     const int a = ww.a, b = ww.b, kg = ww.kg;
     const int s = 1 << p.shift, half = s >> 1;
@@ -1798,7 +1801,7 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) count_kernel(MarchParams
 }
 
 cudaError_t launch_count(const MarchParams &p, unsigned long long *total, cudaStream_t st) {
-    const long long nwarps = (p.qlist != nullptr ? (long long)(p.qpad >> 3) : p.plist != nullptr ? (long long)p.npatch_act : (long long)p.npatch_x * p.npatch_y * (p.fix ? 4 : 1)) * p.ngroups;
+    const long long nwarps = (p.qlist != nullptr ? (long long)(p.qpad >> 3) * (p.fix ? 4 : 1) : p.plist != nullptr ? (long long)p.npatch_act : (long long)p.npatch_x * p.npatch_y * (p.fix ? 4 : 1)) * p.ngroups;
     const long long blocks = (nwarps + WARPS_PER_BLOCK - 1) / WARPS_PER_BLOCK;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     if (blocks == 0) return cudaSuccess;
