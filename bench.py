@@ -162,7 +162,9 @@ def main():
                     help="sparsity as the paper defines it (PAPER.md:380, SURVEY §8(f) f4): 'occupied' flags the cells that hold "
                          "opacity, a number in (0, 1) the densest fraction of the cells (0.25: the paper's production run)")
     ap.add_argument("--no-analyse", action="store_true",
-                    help="skip rc_analyse_atmosphere (free-space acceleration of mostly-empty atmospheres, config 4)")
+                    help="skip rc_analyse_atmosphere (free-space acceleration of mostly-empty atmospheres: by default called for "
+                         "config 4, whose recipe is > 90 %% empty, and with --active, where the unflagged cells count as empty)")
+    ap.add_argument("--analyse", action="store_true", help="call rc_analyse_atmosphere whatever the workload")
     ap.add_argument("--tune", default="", help="rc_set_tuning knobs, e.g. march_variant=0,bands=3")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-baseline-whole", action="store_true",
@@ -247,7 +249,7 @@ def main():
             rc.set_active_cells(active_d)
     configure()
     analysed = None
-    if atm.line is None and not args.no_analyse:
+    if atm.line is None and not args.no_analyse and (args.analyse or args.config == 4 or args.active):
         analysed = rc.analyse_atmosphere()   # empty-cell scan; switches the distance-field march on when > 2/3 is empty
     seg = rc.count_segments()
     l2_gather_gbs = rc.probe_gather_bandwidth(64)      # L2 -> SM ceiling of the gather pattern (64 MB region)

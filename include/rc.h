@@ -143,6 +143,7 @@ int rc_set_stream(rc_ctx *ctx, void *cuda_stream);
  * knob).  name / value:
  *   "march_variant" -1 | 0..4   register-ring depth and occupancy of the march (-1: chosen per cascade)
  *   "patch_log2"    -1 | 2..5   lane patch width 2^n for cascades >= "patch_from" (-1: chosen per cascade from the geometry)
+ *   "pipeline"      0 | 1       rc_solve_J_host in two halves of the wavelength batches with overlapped copies (default 1)
  *   "lists"         0 | 1       hit lists for the sparse march when rc_set_sparse_workspace lends room (default 1)
  *   "list_b"        0 | 1,2,4,8 wavelength batches per warp of the march over hit lists (0: from the L2 footprint of the occupied cells)
  *   "sorted"        -1 | 0 | 1  lanes from quads of probes sorted by ray length: where the geometry says it pays / never / wherever possible
@@ -241,7 +242,9 @@ int rc_solve_J(rc_ctx *ctx, float *J_out);
 int rc_compute_alo(rc_ctx *ctx, float *alo_out);
 
 /* Same path with HOST buffers: copies chi, eta to the device (workspace, host_io != 0), solves,
- * copies J back, synchronises the stream.  Pinned host memory makes the copies asynchronous. */
+ * copies J back, synchronises the stream.  Pinned host memory makes the copies asynchronous; large dense solves
+ * then run as two halves of the wavelength batches (wavelengths are independent) on the context's stream
+ * while a private stream moves the other half's inputs and results (same arithmetic, same J). */
 int rc_solve_J_host(rc_ctx *ctx, const float *chi_host, const float *eta_host, int nx, int ny,
                     int nlambda, float *J_host);
 

@@ -32,6 +32,7 @@ struct Tuning {
     int graph = 1;         // CUDA graph replay on small grids
     int sparse_mode = 1;   // fan march variant, 0..3 (blocks of 8 / 4 / 2 warps, or 4 warps at 128 registers)
     int list_b = 0;        // wavelength batches per warp of the march over hit lists: 0 from the L2 footprint, or 1, 2, 4, 8
+    int pipeline = 1;      // rc_solve_J_host: two halves of the wavelength batches, copies overlapped with the other half's solve
     int lists = 1;         // hit lists for the sparse march when the caller lends a buffer (rc_set_sparse_workspace): 0 never
     int sorted = -1;       // lanes from sorted quads: -1 where the geometry says it pays, 0 never, 1 wherever possible
 };
@@ -90,6 +91,8 @@ struct rc_ctx {
     GraphKey graph_key{};
     cudaGraphExec_t graph_exec = nullptr;
     cudaStream_t cap_stream = nullptr;
+    cudaStream_t copy_stream = nullptr;   // rc_solve_J_host's pipeline: the other half's copies
+    cudaEvent_t pipe_ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
     // sparsity
     bool active_set = false;   // rc_set_active_cells: flagged probes per cascade are in the workspace
     bool lists_dirty = false;  // the compacted patch lists must be rebuilt (before the next solve; synchronises once)
@@ -474,10 +477,14 @@ int rc_create(rc_ctx **out, const rc_config *cfg) {
 
 int rc_destroy(rc_ctx *ctx) {
     if (!ctx) return RC_ERR_NULL_ARG;
-    if (!ctx->ev.empty() || ctx->graph_exec || ctx->cap_stream) cudaSetDevice(ctx->cfg.device);
+    if (!ctx->ev.empty() || ctx->graph_exec || ctx->cap_stream || ctx->copy_stream) cudaSetDevice(ctx->cfg.device);
     for (auto &e : ctx->ev) cudaEventDestroy(e);
     if (ctx->graph_exec) cudaGraphExecDestroy(ctx->graph_exec);
     if (ctx->cap_stream) cudaStreamDestroy(ctx->cap_stream);
+    if (ctx->copy_stream) {
+        cudaStreamDestroy(ctx->copy_stream);
+        for (auto &e : ctx->pipe_ev) if (e) cudaEventDestroy(e);
+    }
     delete ctx;
     return RC_OK;
 }
@@ -524,6 +531,7 @@ int rc_set_tuning(rc_ctx *ctx, const char *name, double value) {
     else if (n == "graph") { t.graph = iv != 0; }
     else if (n == "sparse_mode") { if (iv < 0 || iv > 3) goto bad; t.sparse_mode = iv; }
     else if (n == "lists") { t.lists = iv != 0; }
+    else if (n == "pipeline") { t.pipeline = iv != 0; }
     else if (n == "list_b") { if (iv != 0 && iv != 1 && iv != 2 && iv != 4 && iv != 8) goto bad; t.list_b = iv; }
     else if (n == "sorted") { if (iv < -1 || iv > 1) goto bad; t.sorted = iv; }
     else return fail(ctx, RC_ERR_BAD_VALUE, "rc_set_tuning: unknown knob '%s'", name);
@@ -768,7 +776,7 @@ static rc::MarchParams march_params(const rc_ctx *ctx, int i, float *J_out) {
     mp.I_below = (const float *)(ctx->ws + P.bc_below);
     mp.I_above = (const float *)(ctx->ws + P.bc_above);
     mp.weights = (const float *)(ctx->ws + P.weights);
-    mp.nx = P.nx; mp.ny = P.ny; mp.L = P.L; mp.nb = P.nb;
+    mp.nx = P.nx; mp.ny = P.ny; mp.L = P.L; mp.nb = P.nb; mp.nb0 = 0;
     mp.cascade = i; mp.shift = i;
     mp.npx = P.nx >> i; mp.npy = P.ny >> i;
     mp.ngroups = 1 << (2 * i);
@@ -832,15 +840,19 @@ static int build_patch_lists(rc_ctx *ctx) {
 // One full solve: for cascade i = top .. 0 { pack chi/eta for spacing 2^i ; march + merge }  (PAPER.md:207:
 // "after calculation, each interval of cascade i merges with the child intervals of cascade i+1.
 // Cascade i-1 is then computed and merged with cascade i").
-static int enqueue_solve(rc_ctx *ctx, float *J_out) {
+// b0, bn: the wavelength batches to solve (default: all of them); wavelengths are independent, so
+// rc_solve_J_host solves them in two halves while the other half's copies are in flight.
+static int enqueue_solve(rc_ctx *ctx, float *J_out, int b0 = 0, int bn = -1) {
     const Plan &P = ctx->plan;
+    if (bn < 0) bn = P.nb;
+    const bool whole = b0 == 0 && bn == P.nb, last = b0 + bn == P.nb;
     const int top = ctx->cfg.ncascades - 1;
     const bool accum = (ctx->cfg.flags & RC_ACCUM_J) != 0;
     const int per = 2 * ctx->cfg.ncascades + 2;
-    cudaEvent_t *ev = ctx->nsets > 0 ? ctx->ev.data() + (size_t)(ctx->solves_timed % ctx->nsets) * per : nullptr;
-    int launches = 0;
+    cudaEvent_t *ev = ctx->nsets > 0 && whole ? ctx->ev.data() + (size_t)(ctx->solves_timed % ctx->nsets) * per : nullptr;
+    int launches = whole || b0 == 0 ? 0 : ctx->stats.kernel_launches;
     if (ev) RC_CUDA(ctx, cudaEventRecord(ev[0], ctx->stream));
-    if (ctx->active_set) {
+    if (ctx->active_set && b0 == 0) {
         // J is computed on the cells of interest only: the others read 0
         const size_t ncell = (size_t)P.nx * P.ny;
         if (accum) RC_CUDA(ctx, cudaMemsetAsync(ctx->ws + P.Jpart, 0, ncell * P.nb * sizeof(float), ctx->stream));
@@ -851,7 +863,7 @@ static int enqueue_solve(rc_ctx *ctx, float *J_out) {
         pp.chi = ctx->chi; pp.eta = ctx->eta;
         pp.chiT = (float *)(ctx->ws + P.chiT); pp.ST = (float *)(ctx->ws + P.ST);
         pp.active = ctx->active_set ? (const unsigned char *)(ctx->ws + P.pflag[0]) : nullptr;
-        pp.nx = P.nx; pp.ny = P.ny; pp.L = P.L; pp.nb = P.nb; pp.shift = shift;
+        pp.nx = P.nx; pp.ny = P.ny; pp.L = P.L; pp.nb = bn; pp.nb0 = b0; pp.shift = shift;
         // thin form below chi ds log2e = 1/64 for the longest segment (sqrt2 cells) of the most inclined ray, roughly:
         // there the trapezoid is good to 2e-5 (seg_update*() in rc_kernels.cu)
         float fmax = 1.f;
@@ -874,7 +886,7 @@ static int enqueue_solve(rc_ctx *ctx, float *J_out) {
         rc::PackParams pp{};
         pp.chi = ctx->chi; pp.eta = ctx->eta;
         pp.active = ctx->active_set ? (const unsigned char *)(ctx->ws + P.pflag[0]) : nullptr;
-        pp.nx = P.nx; pp.ny = P.ny; pp.L = P.L; pp.nb = P.nb;
+        pp.nx = P.nx; pp.ny = P.ny; pp.L = P.L; pp.nb = bn; pp.nb0 = b0;
         float fmax = 1.f;
         for (int m = 0; m < ctx->nm; m++) fmax = std::max(fmax, ctx->incl_f[m]);
         pp.c_thin = (1.f / 64.f) / fmax;
@@ -893,6 +905,7 @@ static int enqueue_solve(rc_ctx *ctx, float *J_out) {
         if (!c.empty && !ctx->sparse && !multi) { const int rc = pack(c.fix ? i + 1 : i); if (rc != RC_OK) return rc; }
         if (ev) RC_CUDA(ctx, cudaEventRecord(ev[1 + 2 * (top - i)], ctx->stream));
         rc::MarchParams mp = march_params(ctx, i, J_out);
+        mp.nb = bn; mp.nb0 = b0;
         if (!c.banded || ctx->sparse) {  // the distance-field march gathers occupied cells only: they fit L2
             RC_CUDA(ctx, rc::launch_march(mp, P.LV * P.NM, P.NM, march_variant(ctx, i), ctx->stream));
             launches++;
@@ -919,7 +932,7 @@ static int enqueue_solve(rc_ctx *ctx, float *J_out) {
         }
         if (ev) RC_CUDA(ctx, cudaEventRecord(ev[2 + 2 * (top - i)], ctx->stream));
     }
-    if (accum) {
+    if (accum && last) {
         RC_CUDA(ctx, rc::launch_reduce_jbar((const float *)(ctx->ws + P.Jpart), J_out, (long long)P.nx * P.ny, P.nb, ctx->stream));
         launches++;
     }
@@ -1202,6 +1215,49 @@ int rc_solve_J_host(rc_ctx *ctx, const float *chi_host, const float *eta_host, i
         return fail(ctx, RC_ERR_NO_WORKSPACE, "workspace has %zu bytes, %zu needed with host_io", ctx->ws_bytes, Pio.total);
     const size_t n = (size_t)nx * ny * nlambda * sizeof(float);
     float *dchi = (float *)(ctx->ws + Pio.io_chi), *deta = (float *)(ctx->ws + Pio.io_eta), *dJ = (float *)(ctx->ws + Pio.io_J);
+    // Wavelengths are independent: large dense solves run as two halves of the wavelength batches, the
+    // second half's inputs and the first half's J crossing PCIe (strided 2D copies on a private stream) while the other
+    // half is solved.  Exposed: the first half's H2D and the second half's D2H instead of all of both.
+    const size_t ncell = (size_t)nx * ny;
+    const bool pipelined = ctx->tune.pipeline != 0 && !ctx->analysed && ctx->nsets == 0 && !(ctx->cfg.flags & RC_ACCUM_J) &&
+                           Pio.nb >= 2 && (long long)ncell * Pio.Lpad * Pio.NM >= (1LL << 24);  // (config 1, 4 M cell-channels: slower in halves)
+    if (pipelined) {
+        int rc = rc_set_atmosphere(ctx, dchi, deta, nx, ny, nlambda);  // pointers (and, for a new shape, the tables)
+        if (rc != RC_OK) return rc;
+        if (ctx->lists_dirty) { rc = build_patch_lists(ctx); if (rc != RC_OK) return rc; }
+        if (!ctx->copy_stream) {
+            RC_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
+            for (auto &e : ctx->pipe_ev) RC_CUDA(ctx, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        }
+        const Plan &P = ctx->plan;
+        cudaStream_t st = ctx->stream, cs = ctx->copy_stream;
+        const int h = P.nb / 2;                                        // batches [0, h) and [h, nb)
+        const size_t pitch = (size_t)nlambda * sizeof(float);
+        const size_t col[3] = {0, (size_t)h * P.LV, (size_t)nlambda};  // their wavelength columns
+        cudaEvent_t *e = ctx->pipe_ev;
+        RC_CUDA(ctx, cudaEventRecord(e[0], st));
+        RC_CUDA(ctx, cudaStreamWaitEvent(cs, e[0], 0));
+        for (int g = 0; g < 2; g++) {
+            const size_t w = (col[g + 1] - col[g]) * sizeof(float);
+            RC_CUDA(ctx, cudaMemcpy2DAsync(dchi + col[g], pitch, chi_host + col[g], pitch, w, ncell, cudaMemcpyHostToDevice, cs));
+            RC_CUDA(ctx, cudaMemcpy2DAsync(deta + col[g], pitch, eta_host + col[g], pitch, w, ncell, cudaMemcpyHostToDevice, cs));
+            RC_CUDA(ctx, cudaEventRecord(e[1 + g], cs));
+        }
+        RC_CUDA(ctx, cudaStreamWaitEvent(st, e[1], 0));
+        rc = enqueue_solve(ctx, dJ, 0, h);
+        if (rc != RC_OK) return rc;
+        RC_CUDA(ctx, cudaEventRecord(e[3], st));
+        RC_CUDA(ctx, cudaStreamWaitEvent(st, e[2], 0));
+        rc = enqueue_solve(ctx, dJ, h, P.nb - h);
+        if (rc != RC_OK) return rc;
+        RC_CUDA(ctx, cudaStreamWaitEvent(cs, e[3], 0));
+        RC_CUDA(ctx, cudaMemcpy2DAsync(J_host + col[0], pitch, dJ + col[0], pitch, (col[1] - col[0]) * sizeof(float), ncell, cudaMemcpyDeviceToHost, cs));
+        RC_CUDA(ctx, cudaEventRecord(e[4], cs));
+        RC_CUDA(ctx, cudaMemcpy2DAsync(J_host + col[1], pitch, dJ + col[1], pitch, (col[2] - col[1]) * sizeof(float), ncell, cudaMemcpyDeviceToHost, st));
+        RC_CUDA(ctx, cudaStreamWaitEvent(st, e[4], 0));
+        RC_CUDA(ctx, cudaStreamSynchronize(st));
+        return RC_OK;
+    }
     RC_CUDA(ctx, cudaMemcpyAsync(dchi, chi_host, n, cudaMemcpyHostToDevice, ctx->stream));
     RC_CUDA(ctx, cudaMemcpyAsync(deta, eta_host, n, cudaMemcpyHostToDevice, ctx->stream));
     int rc = rc_set_atmosphere(ctx, dchi, deta, nx, ny, nlambda);

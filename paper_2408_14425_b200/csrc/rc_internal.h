@@ -58,7 +58,8 @@ struct MarchParams {
     const float *I_below;  // [Lpad][NM] device (one value per channel)
     const float *I_above;  // [Lpad][NM] device
     const float *weights;  // [Lpad] device
-    int nx, ny, L, nb;
+    int nx, ny, L, nb;     // nb: wavelength batches this launch covers,
+    int nb0;               // starting at batch nb0 (0 except for the two halves of rc_solve_J_host's pipeline)
     int cascade, shift;    // s = 1 << shift
     int npx, npy;          // probes per axis of this cascade
     int ngroups;           // direction groups = 4^cascade (4 directions each)
@@ -85,6 +86,7 @@ struct PackParams {
     float *chiT, *ST;        // [nb][s][s][npy][npx][LV]
     const unsigned char *active;  // null, or [ny][nx]: cells that are not flagged are packed as vacuum
     int nx, ny, L, nb, shift;
+    int nb0;                 // first wavelength batch of this launch (nb of them)
     float c_thin;            // cells with chi log2e below this are packed in the thin form (seg_update*() in rc_kernels.cu)
     int list_b;              // > 0: write [batch group of list_b][cell][batch in group][LV] (march over hit lists, shift 0)
     // small grids (launch bound): nmulti > 0 packs for nmulti cascades in one launch, cascade j (blockIdx.y) with spacing

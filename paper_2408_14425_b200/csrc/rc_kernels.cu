@@ -239,7 +239,7 @@ __global__ void __launch_bounds__(256) pack_kernel(PackParams p) {
     // line per batch.  (Batch-slowest threads read one 32-byte sector of every cell at a time: 39 % of the HBM peak.)
     const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const long long grp = t >> 2;
-    const int nbI = (int)(grp % p.nb);
+    const int nbI = p.nb0 + (int)(grp % p.nb);          // (a launch covers batches nb0 .. nb0 + nb - 1)
     const long long c = (grp / p.nb) * 4 + (t & 3);  // output cell index ((ym*s + xm)*npy + yd)*npx + xd
     if (c >= ncell) return;
     // output order: batch-major planes for the lock-step and fan marches, cell records for the march over hit lists
@@ -516,6 +516,7 @@ __device__ __forceinline__ WarpWork warp_work(const MarchParams &p, long long W,
         r.kg = (kgb * G + kg_lo + p.kg_off) & (p.ngroups - 1);
         r.nbI = (int)(W / kgb_n);
         r.any = r.nbI < p.nb;
+        r.nbI += p.nb0;
         // (bilinear fix: the lattice of one parity class, spacing 2s; the same list serves the four classes)
         r.cls = (int)(patch % ncls);
         patch /= ncls;
@@ -537,6 +538,7 @@ __device__ __forceinline__ WarpWork warp_work(const MarchParams &p, long long W,
     r.kg = ((int)(W % kgb_n) * G + kg_lo + p.kg_off) & (p.ngroups - 1);
     r.nbI = (int)(W / kgb_n);
     r.any = r.nbI < p.nb;
+    r.nbI += p.nb0;  // (a launch covers batches nb0 .. nb0 + nb - 1)
     const int py = (int)(patch / p.npatch_x), px = (int)(patch - (long long)py * p.npatch_x);
     const int pw = 1 << p.pw_log2;
     // lane lattice: all probes, or (bilinear fix) the probes of one parity class, spacing 2s

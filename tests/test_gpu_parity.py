@@ -147,6 +147,30 @@ def test_solve_is_repeatable_and_host_path_matches(oracle):
 
 
 # ------------------------------------------------------------------ error behaviour of the ABI
+@pytest.mark.parametrize("L", [64, 60, 20])
+def test_host_path_in_two_halves_matches_the_device_path(L):
+    """From 16 M cell-channels on rc_solve_J_host solves the wavelength batches in two halves while the other half's
+    inputs and J cross PCIe on a private stream (strided 2D copies): the same launches on the same data, so the same J bit
+    for bit - also with a ragged last batch, an odd number of batches, and against the unpipelined call."""
+    import torch
+    from paper_2408_14425_b200 import binding
+    nx = 512 if L >= 60 else 1024
+    atm = A.make_config(2, nx=nx, ny=nx, nlambda=L, ncascades=6)
+    J, rc = binding.solve_atmosphere(atm)
+    ref = J.cpu()
+    chi_h, eta_h = torch.from_numpy(atm.chi).pin_memory(), torch.from_numpy(atm.eta).pin_memory()
+    out = rc.solve_J_host(chi_h, eta_h)
+    rc.set_boundary(atm.I_below, atm.I_above)           # (a new workspace layout resets them)
+    out = rc.solve_J_host(chi_h, eta_h)
+    assert torch.equal(out, ref)
+    rc.close()
+    rc = binding.RadianceCascades(atm.ncascades)
+    rc.set_tuning(pipeline=0)
+    rc.ensure_workspace(atm.nx, atm.ny, atm.nlambda, host_io=True)
+    assert torch.equal(rc.solve_J_host(chi_h, eta_h), ref)
+    rc.close()
+
+
 def test_error_codes():
     import torch
     from paper_2408_14425_b200 import binding
