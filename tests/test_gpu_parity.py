@@ -171,6 +171,28 @@ def test_host_path_in_two_halves_matches_the_device_path(L):
     rc.close()
 
 
+def test_host_path_in_two_halves_with_bands_and_active_cells():
+    """The two halves with everything that keeps per-batch state between launches: banded cascades (parked ray state),
+    flagged probes (J zeroed once, compacted patch lists), and the bilinear fix."""
+    import dataclasses
+    import torch
+    from paper_2408_14425_b200 import binding
+    base = A.make_config(3, nx=512, ny=512, nlambda=64, ncascades=7)
+    for atm, tuning in ((base, dict(bands=3)), (A.with_active_cells(base, mode="fraction", fraction=0.3), dict(bands=3)),
+                        (dataclasses.replace(base, bilinear_fix=True), {})):
+        J, rc = binding.solve_atmosphere(atm, tuning=tuning)     # bands = 3: every long-ray cascade marched band by band
+        ref = J.cpu()
+        chi_h, eta_h = torch.from_numpy(atm.chi).pin_memory(), torch.from_numpy(atm.eta).pin_memory()
+        rc.ensure_workspace(atm.nx, atm.ny, atm.nlambda, host_io=True)
+        out = rc.solve_J_host(chi_h, eta_h)              # may move to a larger workspace: boundary, flags again
+        rc.set_boundary(atm.I_below, atm.I_above)
+        if atm.active is not None:
+            rc.set_active_cells(torch.from_numpy(np.ascontiguousarray(atm.active, dtype=np.uint8)).cuda())
+        out = rc.solve_J_host(chi_h, eta_h)
+        assert torch.equal(out, ref)
+        rc.close()
+
+
 def test_error_codes():
     import torch
     from paper_2408_14425_b200 import binding
