@@ -217,7 +217,7 @@ class RadianceCascades:
         self.set_stream()
         self._check(self.lib.rc_analyse_atmosphere(self.handle))
         st = self.get_stats()
-        if lists and st.sparse_march and not st.sparse_lists and st.sparse_list_bytes > 0:
+        if lists and not st.sparse_lists and st.sparse_list_bytes > 0:   # (> 0: the atmosphere is sparse)
             if self._sws is None or self._sws.numel() < st.sparse_list_bytes:
                 self._sws = None
                 self._sws = torch.empty(int(st.sparse_list_bytes * 1.02) + 4096, dtype=torch.uint8, device=f"cuda:{self.device}")

@@ -1110,10 +1110,12 @@ int rc_analyse_atmosphere(rc_ctx *ctx) {
     RC_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     ctx->stats.empty_cells = (int64_t)h;
     ctx->analysed = true;
-    // the distance-field march exists for the plain mode (no inclinations, no moving line, no bilinear fix)
-    const bool can = P.NM == 1 && !ctx->line && !(ctx->cfg.flags & RC_BILINEAR_FIX);
+    // the distance-field walk exists for the plain mode (no inclinations, no moving line, no bilinear fix); the march over
+    // hit lists also with inclinations (it then needs the lists: without the second buffer such a solve stays lock-step)
+    const bool can_list = !ctx->line && !(ctx->cfg.flags & RC_BILINEAR_FIX);
+    const bool can_walk = can_list && P.NM == 1;
     const bool want = ctx->tune.sparse >= 0 ? ctx->tune.sparse != 0 : 3 * h > 2ULL * P.nx * P.ny;
-    ctx->sparse = can && want;
+    ctx->sparse = want && (can_walk || (can_list && ctx->tune.lists != 0));
     ctx->stats.sparse_march = ctx->sparse;
     ctx->list_version++;
     ctx->lists = false;
@@ -1129,6 +1131,10 @@ int rc_analyse_atmosphere(rc_ctx *ctx) {
             const int rc = build_hit_lists(ctx);
             if (rc != RC_OK) return rc;
         }
+    }
+    if (ctx->sparse && !ctx->lists && !can_walk) {  // inclined, and no room for the lists: the lock-step march
+        ctx->sparse = false;
+        ctx->stats.sparse_march = 0;
     }
     return RC_OK;
 }

@@ -1328,9 +1328,10 @@ cudaError_t launch_hit_walk(const MarchParams &p, bool fill, unsigned *cnt_or_of
 // B wavelength batches: the B lanes of a ray read the same list entries and table steps (one sector, broadcast) and gather
 // B x LV consecutive floats of the cell (under this march the packed arrays are [batch group][cell][batch in group][LV]).  The next
 // hit's step, cell and path length are looked up while the previous cell is integrated.
-template <int LV, int B, int WARPS, int MINB>
+template <int LV, int NM, int B, int WARPS, int MINB>
 __global__ void __launch_bounds__(WARPS * 32, MINB) march_list_kernel(MarchParams p) {
     constexpr int R = 32 / B;
+    constexpr int LL = LV / NM;  // wavelengths per lane; channel ch = l * NM + m (2.5D: NM inclinations per wavelength)
     const int lane = threadIdx.x & 31;
     long long W = (long long)blockIdx.x * WARPS + (threadIdx.x >> 5);
     const long long ndir = 4LL * p.ngroups;
@@ -1352,11 +1353,11 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_list_kernel(MarchParam
     if (!__any_sync(FULL, valid)) return;
     const int half = (1 << p.shift) >> 1;
     const int X0 = (a << p.shift) + half, Y0 = (b << p.shift) + half;
-    // packed arrays: [batch group][cell][batch in group][LV]
+    // packed arrays: [batch group][cell][batch in group][LL]
     const int Bg = min(B, p.nb - bg * B);
-    const long long gbase = ((long long)bg * B * ((long long)p.nx * p.ny) + (nbI - bg * B)) * LV;
-    const float *chiB = p.chiT + gbase, *SB = p.ST + gbase;  // + cell * Bg * LV
-    const unsigned long long cstride = (unsigned long long)Bg * (LV * sizeof(float));
+    const long long gbase = ((long long)bg * B * ((long long)p.nx * p.ny) + (nbI - bg * B)) * LL;
+    const float *chiB = p.chiT + gbase, *SB = p.ST + gbase;  // + cell * Bg * LL
+    const unsigned long long cstride = (unsigned long long)Bg * (LL * sizeof(float));
 
     float I[LV], tau[LV], T[LV];
 #pragma unroll
@@ -1386,30 +1387,35 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_list_kernel(MarchParam
             h++;
         };
         lookup();
-        float cP[LV], SP[LV], dsP = 0.f;
+        float cP[LL], SP[LL], dsP = 0.f;
         bool pend = false;
         while (true) {
-            float cN[LV], SN[LV];
+            float cN[LL], SN[LL];
             const bool have = c1 >= 0;
             const float dsN = d1;
             if (have) {
                 const unsigned long long d = (unsigned long long)(unsigned)c1 * cstride;
-                load_vec<LV>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(chiB) + d), cN);
-                load_vec<LV>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(SB) + d), SN);
+                load_vec<LL>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(chiB) + d), cN);
+                load_vec<LL>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(SB) + d), SN);
                 lookup();
             }
             bool stop = !have;
             if (pend) {  // integrate the cell gathered one round earlier
                 nwalk++;
-                const float mdsP = -dsP;
+                float dsm[NM];  // inclination m crosses the same cell over ds / sin(inclination)
+#pragma unroll
+                for (int m = 0; m < NM; m++) dsm[m] = NM == 1 ? dsP : dsP * p.incl_f[m];
                 if constexpr (LV >= 2) {
 #pragma unroll
-                    for (int q = 0; q < LV / 2; q++) {
-                        f32x2 t2 = pk2(tau[2 * q], tau[2 * q + 1]), T2 = pk2(T[2 * q], T[2 * q + 1]), I2 = pk2(I[2 * q], I[2 * q + 1]);
-                        seg_update2(pk2(cP[2 * q], cP[2 * q + 1]), pk2(SP[2 * q], SP[2 * q + 1]), pk2(dsP, dsP), pk2(mdsP, mdsP), t2, T2, I2);
-                        up2(t2, tau[2 * q], tau[2 * q + 1]);
-                        up2(T2, T[2 * q], T[2 * q + 1]);
-                        up2(I2, I[2 * q], I[2 * q + 1]);
+                    for (int q = 0; q < LV / 2; q++) {  // the pairs of march_kernel: two wavelengths of one inclination, or (LL = 1) two inclinations
+                        const int lo = LL >= 2 ? (2 * (q / NM)) * NM + q % NM : 2 * q, hi = LL >= 2 ? (2 * (q / NM) + 1) * NM + q % NM : 2 * q + 1;
+                        const int l0 = LL >= 2 ? 2 * (q / NM) : 0, l1 = LL >= 2 ? l0 + 1 : 0;
+                        const int m0 = LL >= 2 ? q % NM : 2 * q, m1 = LL >= 2 ? m0 : 2 * q + 1;
+                        f32x2 t2 = pk2(tau[lo], tau[hi]), T2 = pk2(T[lo], T[hi]), I2 = pk2(I[lo], I[hi]);
+                        seg_update2(pk2(cP[l0], cP[l1]), pk2(SP[l0], SP[l1]), pk2(dsm[m0], dsm[m1]), pk2(-dsm[m0], -dsm[m1]), t2, T2, I2);
+                        up2(t2, tau[lo], tau[hi]);
+                        up2(T2, T[lo], T[hi]);
+                        up2(I2, I[lo], I[hi]);
                     }
                 } else {
                     seg_update1(cP[0], SP[0], dsP, tau[0], T[0], I[0]);
@@ -1470,24 +1476,36 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_list_kernel(MarchParam
     const long long kg = k >> 2;
     if (p.mode == 0) {
         store_vec<LV>(p.out + (((long long)nbI * p.ngroups + kg) * nprobe + probe) * LV, acc);
-    } else if (p.mode == 1) {  // cascade 0: a4, J
-        float *o = p.out + probe * p.L + nbI * LV;
-        if ((nbI + 1) * LV <= p.L && (p.L % LV) == 0) {
-            store_vec<LV>(o, acc);
-        } else {
-#pragma unroll
-            for (int v = 0; v < LV; v++)
-                if (nbI * LV + v < p.L) o[v] = acc[v];
-        }
     } else {
-        float sum = 0.f;
+        // cascade 0: J_l = sum over the inclinations of w_m x (mean of the 4 directions)  (a4)
+        float Jl[LL];
 #pragma unroll
-        for (int v = 0; v < LV; v++) sum = fmaf(__ldg(p.weights + nbI * LV + v), acc[v], sum);
-        p.out[(long long)nbI * nprobe + probe] = sum;
+        for (int l = 0; l < LL; l++) {
+            Jl[l] = NM == 1 ? acc[l] : 0.f;
+            if constexpr (NM > 1) {
+#pragma unroll
+                for (int m = 0; m < NM; m++) Jl[l] = fmaf(p.incl_w[m], acc[l * NM + m], Jl[l]);
+            }
+        }
+        if (p.mode == 1) {
+            float *o = p.out + probe * p.L + nbI * LL;
+            if ((nbI + 1) * LL <= p.L && (p.L % LL) == 0) {
+                store_vec<LL>(o, Jl);
+            } else {
+#pragma unroll
+                for (int v = 0; v < LL; v++)
+                    if (nbI * LL + v < p.L) o[v] = Jl[v];
+            }
+        } else {
+            float sum = 0.f;
+#pragma unroll
+            for (int v = 0; v < LL; v++) sum = fmaf(__ldg(p.weights + nbI * LL + v), Jl[v], sum);
+            p.out[(long long)nbI * nprobe + probe] = sum;
+        }
     }
 }
 
-template <int LV, int B>
+template <int LV, int NM, int B>
 static cudaError_t launch_march_list_b(const MarchParams &p, cudaStream_t st) {
     constexpr int R = 32 / B;
     const long long ndir = 4LL * p.ngroups, ndl = ndir < R ? ndir : R, ppw = R / ndl;
@@ -1495,22 +1513,25 @@ static cudaError_t launch_march_list_b(const MarchParams &p, cudaStream_t st) {
     const long long warps = (ndir / ndl) * ((nprobe + ppw - 1) / ppw) * ((p.nb + B - 1) / B);
     if ((warps + 3) / 4 > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     if (warps == 0) return cudaSuccess;
-    switch (p.sparse_mode) {  // blocks of 4 warps at <= 80 / 96 / 128 registers (24 / 20 / 16 warps per SM), or 8 warps at <= 80
-        case 0: march_list_kernel<LV, B, 8, 3><<<(unsigned)((warps + 7) / 8), 256, 0, st>>>(p); break;
-        case 2: march_list_kernel<LV, B, 4, 5><<<(unsigned)((warps + 3) / 4), 128, 0, st>>>(p); break;
-        case 3: march_list_kernel<LV, B, 4, 4><<<(unsigned)((warps + 3) / 4), 128, 0, st>>>(p); break;
-        default: march_list_kernel<LV, B, 4, 6><<<(unsigned)((warps + 3) / 4), 128, 0, st>>>(p); break;
+    if constexpr (NM == 1) {
+        switch (p.sparse_mode) {  // blocks of 4 warps at <= 80 / 96 / 128 registers (24 / 20 / 16 warps per SM), or 8 warps at <= 80
+            case 0: march_list_kernel<LV, NM, B, 8, 3><<<(unsigned)((warps + 7) / 8), 256, 0, st>>>(p); return cudaGetLastError();
+            case 2: march_list_kernel<LV, NM, B, 4, 5><<<(unsigned)((warps + 3) / 4), 128, 0, st>>>(p); return cudaGetLastError();
+            case 3: march_list_kernel<LV, NM, B, 4, 4><<<(unsigned)((warps + 3) / 4), 128, 0, st>>>(p); return cudaGetLastError();
+            default: break;
+        }
     }
+    march_list_kernel<LV, NM, B, 4, 6><<<(unsigned)((warps + 3) / 4), 128, 0, st>>>(p);
     return cudaGetLastError();
 }
 
-template <int LV>
+template <int LV, int NM = 1>
 static cudaError_t launch_march_list(const MarchParams &p, cudaStream_t st) {
     switch (p.list_b) {
-        case 8: return launch_march_list_b<LV, 8>(p, st);
-        case 4: return launch_march_list_b<LV, 4>(p, st);
-        case 2: return launch_march_list_b<LV, 2>(p, st);
-        default: return launch_march_list_b<LV, 1>(p, st);
+        case 8: return launch_march_list_b<LV, NM, 8>(p, st);
+        case 4: return launch_march_list_b<LV, NM, 4>(p, st);
+        case 2: return launch_march_list_b<LV, NM, 2>(p, st);
+        default: return launch_march_list_b<LV, NM, 1>(p, st);
     }
 }
 
@@ -1558,6 +1579,17 @@ cudaError_t launch_march(const MarchParams &p, int LV, int NM, int variant, cuda
             case 4 * 16 + 4: return launch_march_line<4, 4>(p, st);
             case 4 * 16 + 2: return launch_march_line<4, 2>(p, st);
             case 2 * 16 + 2: return launch_march_line<2, 2>(p, st);
+            default: return cudaErrorInvalidValue;
+        }
+    }
+    if (p.hit_list != nullptr) {  // the sparse march over hit lists, inclined
+        switch (LV * 16 + NM) {
+            case 8 * 16 + 8: return launch_march_list<8, 8>(p, st);
+            case 8 * 16 + 4: return launch_march_list<8, 4>(p, st);
+            case 8 * 16 + 2: return launch_march_list<8, 2>(p, st);
+            case 4 * 16 + 4: return launch_march_list<4, 4>(p, st);
+            case 4 * 16 + 2: return launch_march_list<4, 2>(p, st);
+            case 2 * 16 + 2: return launch_march_list<2, 2>(p, st);
             default: return cudaErrorInvalidValue;
         }
     }

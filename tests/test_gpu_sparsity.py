@@ -211,6 +211,30 @@ def test_distance_field_march_on_dense_and_flagged_atmospheres(oracle):
     check(emit, oracle, analyse=True, tuning=dict(sparse=1))
 
 
+@pytest.mark.parametrize("n,nlambda", [(2, 5), (4, 16), (8, 9), (8, 1)])
+def test_march_over_hit_lists_with_inclinations(oracle, n, nlambda):
+    """2.5D inclinations over hit lists (the distance-field walk has no inclined version: without the second buffer the
+    solve stays lock-step): bit-identical to the lock-step march, with flagged probes too, and against the oracle."""
+    from paper_2408_14425_b200 import binding
+    atm = A.with_inclinations(dataclasses.replace(A.make_config(4, nx=256, ny=64, nlambda=nlambda, ncascades=5), accumulate=nlambda == 9), n)
+    ref, st0 = gpu(atm)
+    got, st1 = gpu(atm, analyse=True)
+    assert st0.sparse_march == 0 and st1.sparse_march == 1 and st1.sparse_lists == 1
+    assert np.array_equal(ref, got)
+    flagged = A.with_active_cells(atm)
+    a, _ = gpu(flagged)
+    b, st = gpu(flagged, analyse=True)
+    assert st.sparse_lists == 1 and np.array_equal(a, b)
+    J, rc = binding.solve_atmosphere(atm)                 # raw analysis without a buffer: stays lock-step
+    assert rc.lib.rc_analyse_atmosphere(rc.handle) == 0
+    st = rc.get_stats()
+    assert st.sparse_march == 0 and st.sparse_list_bytes > 0
+    assert np.array_equal(rc.solve_J().cpu().numpy(), ref)
+    rc.close()
+    if n == 4:
+        check(atm, oracle, analyse=True)
+
+
 def test_hit_lists_are_kept_while_the_occupancy_stands():
     """A new atmosphere with the same occupancy map (other values in the same cells) keeps the hit lists (sparse_lists = 2);
     another map rebuilds them (1); both give the lock-step result bit for bit."""
