@@ -249,7 +249,7 @@ def main():
             rc.set_active_cells(active_d)
     configure()
     analysed = None
-    if atm.line is None and not args.no_analyse and (args.analyse or args.config == 4 or args.active):
+    if not args.no_analyse and (args.analyse or (args.config == 4 and atm.line is None) or args.active):
         analysed = rc.analyse_atmosphere()   # empty-cell scan; switches the distance-field march on when > 2/3 is empty
     seg = rc.count_segments()
     l2_gather_gbs = rc.probe_gather_bandwidth(64)      # L2 -> SM ceiling of the gather pattern (64 MB region)

@@ -190,8 +190,8 @@ int rc_set_active_cells(rc_ctx *ctx, const unsigned char *active);
  * march of the next solves lets every lane walk its own ray and jump over empty space; the result is bit-identical
  * to the lock-step march.  Explicit because it synchronises the stream and belongs to one atmosphere: the next
  * rc_set_atmosphere / rc_set_line_atmosphere / rc_set_active_cells switches it off again (rc_solve_J_host repeats it
- * by itself once it has been used on the context).  Not with the moving line or the bilinear fix (there it only counts);
- * with inclinations only through the hit lists of rc_set_sparse_workspace.  rc_stats.empty_cells, rc_stats.sparse_march
+ * by itself once it has been used on the context).  Not with the bilinear fix (there it only counts); with inclinations
+ * or the moving line only through the hit lists of rc_set_sparse_workspace.  rc_stats.empty_cells, rc_stats.sparse_march
  * report the outcome. */
 int rc_analyse_atmosphere(rc_ctx *ctx);
 

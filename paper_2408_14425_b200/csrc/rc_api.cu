@@ -1111,9 +1111,10 @@ int rc_analyse_atmosphere(rc_ctx *ctx) {
     ctx->stats.empty_cells = (int64_t)h;
     ctx->analysed = true;
     // the distance-field walk exists for the plain mode (no inclinations, no moving line, no bilinear fix); the march over
-    // hit lists also with inclinations (it then needs the lists: without the second buffer such a solve stays lock-step)
-    const bool can_list = !ctx->line && !(ctx->cfg.flags & RC_BILINEAR_FIX);
-    const bool can_walk = can_list && P.NM == 1;
+    // hit lists also with inclinations and the moving line (it then needs the lists: without the second buffer such a
+    // solve stays lock-step)
+    const bool can_list = !(ctx->cfg.flags & RC_BILINEAR_FIX);
+    const bool can_walk = can_list && P.NM == 1 && !ctx->line;
     const bool want = ctx->tune.sparse >= 0 ? ctx->tune.sparse != 0 : 3 * h > 2ULL * P.nx * P.ny;
     ctx->sparse = want && (can_walk || (can_list && ctx->tune.lists != 0));
     ctx->stats.sparse_march = ctx->sparse;
@@ -1201,6 +1202,7 @@ int rc_solve_J_line_host(rc_ctx *ctx, const float *line_host, int nx, int ny, co
     RC_CUDA(ctx, cudaMemcpyAsync(dline, line_host, nline, cudaMemcpyHostToDevice, ctx->stream));
     int rc = rc_set_line_atmosphere(ctx, dline, nx, ny, x_lambda, nlambda);
     if (rc != RC_OK) return rc;
+    if (ctx->analysed) { rc = rc_analyse_atmosphere(ctx); if (rc != RC_OK) return rc; }
     rc = rc_solve_J(ctx, dJ);
     if (rc != RC_OK) return rc;
     const size_t nout = (size_t)nx * ny * ((ctx->cfg.flags & RC_ACCUM_J) ? 1 : nlambda) * sizeof(float);

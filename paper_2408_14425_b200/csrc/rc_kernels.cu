@@ -1328,7 +1328,7 @@ cudaError_t launch_hit_walk(const MarchParams &p, bool fill, unsigned *cnt_or_of
 // B wavelength batches: the B lanes of a ray read the same list entries and table steps (one sector, broadcast) and gather
 // B x LV consecutive floats of the cell (under this march the packed arrays are [batch group][cell][batch in group][LV]).  The next
 // hit's step, cell and path length are looked up while the previous cell is integrated.
-template <int LV, int NM, int B, int WARPS, int MINB>
+template <int LV, int NM, int B, int WARPS, int MINB, bool LINE>
 __global__ void __launch_bounds__(WARPS * 32, MINB) march_list_kernel(MarchParams p) {
     constexpr int R = 32 / B;
     constexpr int LL = LV / NM;  // wavelengths per lane; channel ch = l * NM + m (2.5D: NM inclinations per wavelength)
@@ -1353,11 +1353,19 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_list_kernel(MarchParam
     if (!__any_sync(FULL, valid)) return;
     const int half = (1 << p.shift) >> 1;
     const int X0 = (a << p.shift) + half, Y0 = (b << p.shift) + half;
-    // packed arrays: [batch group][cell][batch in group][LL]
+    // packed arrays: [batch group][cell][batch in group][LL]; LINE: the six packed line parameters of the cell, [cell][6]
+    // (the same 24 bytes for every lane of the ray), opacity and source function evaluated per ray as in march_kernel
+    constexpr int NR = LINE ? 6 : LL;
     const int Bg = min(B, p.nb - bg * B);
-    const long long gbase = ((long long)bg * B * ((long long)p.nx * p.ny) + (nbI - bg * B)) * LL;
-    const float *chiB = p.chiT + gbase, *SB = p.ST + gbase;  // + cell * Bg * LL
-    const unsigned long long cstride = (unsigned long long)Bg * (LL * sizeof(float));
+    const long long gbase = LINE ? 0 : ((long long)bg * B * ((long long)p.nx * p.ny) + (nbI - bg * B)) * LL;
+    const float *chiB = LINE ? p.linepk : p.chiT + gbase, *SB = LINE ? nullptr : p.ST + gbase;  // + cell * Bg * LL
+    const unsigned long long cstride = LINE ? 24ull : (unsigned long long)Bg * (LL * sizeof(float));
+    float xs[LINE ? LL : 1], wx = 0.f, wy = 0.f;
+    if constexpr (LINE) {
+#pragma unroll
+        for (int v = 0; v < LL; v++) xs[v] = __ldg(p.xls + min(nbI, p.nb - 1) * LL + v);
+        sincospif(2.f * ((float)k + 0.5f) / (float)ndir, &wy, &wx);
+    }
 
     float I[LV], tau[LV], T[LV];
 #pragma unroll
@@ -1387,16 +1395,22 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_list_kernel(MarchParam
             h++;
         };
         lookup();
-        float cP[LL], SP[LL], dsP = 0.f;
+        float cP[NR], SP[LINE ? 1 : LL], dsP = 0.f;
         bool pend = false;
         while (true) {
-            float cN[LL], SN[LL];
+            float cN[NR], SN[LINE ? 1 : LL];
             const bool have = c1 >= 0;
             const float dsN = d1;
             if (have) {
                 const unsigned long long d = (unsigned long long)(unsigned)c1 * cstride;
-                load_vec<LL>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(chiB) + d), cN);
-                load_vec<LL>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(SB) + d), SN);
+                if constexpr (LINE) {
+                    const float2 *src = reinterpret_cast<const float2 *>(reinterpret_cast<const char *>(chiB) + d);
+                    const float2 q0 = __ldg(src), q1 = __ldg(src + 1), q2 = __ldg(src + 2);
+                    cN[0] = q0.x; cN[1] = q0.y; cN[2] = q1.x; cN[3] = q1.y; cN[4] = q2.x; cN[5] = q2.y;
+                } else {
+                    load_vec<LL>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(chiB) + d), cN);
+                    load_vec<LL>(reinterpret_cast<const float *>(reinterpret_cast<const char *>(SB) + d), SN);
+                }
                 lookup();
             }
             bool stop = !have;
@@ -1405,7 +1419,31 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_list_kernel(MarchParam
                 float dsm[NM];  // inclination m crosses the same cell over ds / sin(inclination)
 #pragma unroll
                 for (int m = 0; m < NM; m++) dsm[m] = NM == 1 ? dsP : dsP * p.incl_f[m];
-                if constexpr (LV >= 2) {
+                if constexpr (LINE) {
+                    // a = x_l + v.w (photons travel along -w), inclination m sees the in-plane velocity times sin(inclination)
+                    const float vw = fmaf(cP[4], wx, cP[5] * wy);
+                    float vwm[NM], dkm[NM];
+#pragma unroll
+                    for (int m = 0; m < NM; m++) { vwm[m] = NM == 1 ? vw : vw * p.incl_s[m]; dkm[m] = dsm[m] * KAPPA; }
+                    if constexpr (LV >= 2) {
+#pragma unroll
+                        for (int q = 0; q < LV / 2; q++) {
+                            const int lo = LL >= 2 ? (2 * (q / NM)) * NM + q % NM : 2 * q, hi = LL >= 2 ? (2 * (q / NM) + 1) * NM + q % NM : 2 * q + 1;
+                            const int l0 = LL >= 2 ? 2 * (q / NM) : 0, l1 = LL >= 2 ? l0 + 1 : 0;
+                            const int m0 = LL >= 2 ? q % NM : 2 * q, m1 = LL >= 2 ? m0 : 2 * q + 1;
+                            f32x2 t2 = pk2(tau[lo], tau[hi]), T2 = pk2(T[lo], T[hi]), I2 = pk2(I[lo], I[hi]);
+                            seg_update_line2(add2(pk2(xs[l0], xs[l1]), pk2(vwm[m0], vwm[m1])), cP[0], cP[1], cP[2], cP[3],
+                                             pk2(dsm[m0], dsm[m1]), pk2(dkm[m0], dkm[m1]), t2, T2, I2);
+                            up2(t2, tau[lo], tau[hi]);
+                            up2(T2, T[lo], T[hi]);
+                            up2(I2, I[lo], I[hi]);
+                        }
+                    } else {
+                        const float aa = xs[0] + vwm[0];
+                        const float phi = ex2_neg(aa * aa);
+                        seg_update_line(fmaf(cP[2], phi, cP[0]), fmaf(cP[3], phi, cP[1]), dsm[0], dkm[0], tau[0], T[0], I[0]);
+                    }
+                } else if constexpr (LV >= 2) {
 #pragma unroll
                     for (int q = 0; q < LV / 2; q++) {  // the pairs of march_kernel: two wavelengths of one inclination, or (LL = 1) two inclinations
                         const int lo = LL >= 2 ? (2 * (q / NM)) * NM + q % NM : 2 * q, hi = LL >= 2 ? (2 * (q / NM) + 1) * NM + q % NM : 2 * q + 1;
@@ -1431,7 +1469,11 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_list_kernel(MarchParam
             pend = true;
             dsP = dsN;
 #pragma unroll
-            for (int v = 0; v < LV; v++) { cP[v] = cN[v]; SP[v] = SN[v]; }
+            for (int v = 0; v < NR; v++) cP[v] = cN[v];
+            if constexpr (!LINE) {
+#pragma unroll
+                for (int v = 0; v < LL; v++) SP[v] = SN[v];
+            }
         }
     }
     if (p.walked != nullptr) {
@@ -1505,7 +1547,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) march_list_kernel(MarchParam
     }
 }
 
-template <int LV, int NM, int B>
+template <int LV, int NM, int B, bool LINE>
 static cudaError_t launch_march_list_b(const MarchParams &p, cudaStream_t st) {
     constexpr int R = 32 / B;
     const long long ndir = 4LL * p.ngroups, ndl = ndir < R ? ndir : R, ppw = R / ndl;
@@ -1513,26 +1555,31 @@ static cudaError_t launch_march_list_b(const MarchParams &p, cudaStream_t st) {
     const long long warps = (ndir / ndl) * ((nprobe + ppw - 1) / ppw) * ((p.nb + B - 1) / B);
     if ((warps + 3) / 4 > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     if (warps == 0) return cudaSuccess;
-    if constexpr (NM == 1) {
+    if constexpr (NM == 1 && !LINE) {
         switch (p.sparse_mode) {  // blocks of 4 warps at <= 80 / 96 / 128 registers (24 / 20 / 16 warps per SM), or 8 warps at <= 80
-            case 0: march_list_kernel<LV, NM, B, 8, 3><<<(unsigned)((warps + 7) / 8), 256, 0, st>>>(p); return cudaGetLastError();
-            case 2: march_list_kernel<LV, NM, B, 4, 5><<<(unsigned)((warps + 3) / 4), 128, 0, st>>>(p); return cudaGetLastError();
-            case 3: march_list_kernel<LV, NM, B, 4, 4><<<(unsigned)((warps + 3) / 4), 128, 0, st>>>(p); return cudaGetLastError();
+            case 0: march_list_kernel<LV, NM, B, 8, 3, false><<<(unsigned)((warps + 7) / 8), 256, 0, st>>>(p); return cudaGetLastError();
+            case 2: march_list_kernel<LV, NM, B, 4, 5, false><<<(unsigned)((warps + 3) / 4), 128, 0, st>>>(p); return cudaGetLastError();
+            case 3: march_list_kernel<LV, NM, B, 4, 4, false><<<(unsigned)((warps + 3) / 4), 128, 0, st>>>(p); return cudaGetLastError();
             default: break;
         }
     }
-    march_list_kernel<LV, NM, B, 4, 6><<<(unsigned)((warps + 3) / 4), 128, 0, st>>>(p);
+    march_list_kernel<LV, NM, B, 4, 6, LINE><<<(unsigned)((warps + 3) / 4), 128, 0, st>>>(p);
     return cudaGetLastError();
+}
+
+template <int LV, int NM, bool LINE>
+static cudaError_t launch_march_list_l(const MarchParams &p, cudaStream_t st) {
+    switch (p.list_b) {
+        case 8: return launch_march_list_b<LV, NM, 8, LINE>(p, st);
+        case 4: return launch_march_list_b<LV, NM, 4, LINE>(p, st);
+        case 2: return launch_march_list_b<LV, NM, 2, LINE>(p, st);
+        default: return launch_march_list_b<LV, NM, 1, LINE>(p, st);
+    }
 }
 
 template <int LV, int NM = 1>
 static cudaError_t launch_march_list(const MarchParams &p, cudaStream_t st) {
-    switch (p.list_b) {
-        case 8: return launch_march_list_b<LV, NM, 8>(p, st);
-        case 4: return launch_march_list_b<LV, NM, 4>(p, st);
-        case 2: return launch_march_list_b<LV, NM, 2>(p, st);
-        default: return launch_march_list_b<LV, NM, 1>(p, st);
-    }
+    return p.linepk != nullptr ? launch_march_list_l<LV, NM, true>(p, st) : launch_march_list_l<LV, NM, false>(p, st);
 }
 
 // Velocity-dependent line mode (linepk != null): 3 MUFU per segment-channel, ring of 2, 24 warps/SM.
@@ -1548,8 +1595,8 @@ static cudaError_t launch_march_line(const MarchParams &p, cudaStream_t st) {
 
 template <int LV>
 static cudaError_t launch_march_flat(const MarchParams &p, int variant, cudaStream_t st) {
+    if (p.hit_list != nullptr) return launch_march_list<LV>(p, st);  // (flat or moving line)
     if (p.linepk != nullptr) return launch_march_line<LV>(p, st);
-    if (p.hit_list != nullptr) return launch_march_list<LV>(p, st);
     if (p.dist != nullptr) return launch_march_sparse<LV>(p, st);
     switch (variant) {
         case 0: return launch_march_variant<LV, 1, 2, 8, 3>(p, st);
@@ -1571,6 +1618,17 @@ cudaError_t launch_march(const MarchParams &p, int LV, int NM, int variant, cuda
             default: return launch_march_flat<1>(p, variant, st);
         }
     }
+    if (p.hit_list != nullptr) {  // the sparse march over hit lists, inclined (flat or moving line)
+        switch (LV * 16 + NM) {
+            case 8 * 16 + 8: return launch_march_list<8, 8>(p, st);
+            case 8 * 16 + 4: return launch_march_list<8, 4>(p, st);
+            case 8 * 16 + 2: return launch_march_list<8, 2>(p, st);
+            case 4 * 16 + 4: return launch_march_list<4, 4>(p, st);
+            case 4 * 16 + 2: return launch_march_list<4, 2>(p, st);
+            case 2 * 16 + 2: return launch_march_list<2, 2>(p, st);
+            default: return cudaErrorInvalidValue;
+        }
+    }
     if (p.linepk != nullptr) {
         switch (LV * 16 + NM) {
             case 8 * 16 + 8: return launch_march_line<8, 8>(p, st);
@@ -1579,17 +1637,6 @@ cudaError_t launch_march(const MarchParams &p, int LV, int NM, int variant, cuda
             case 4 * 16 + 4: return launch_march_line<4, 4>(p, st);
             case 4 * 16 + 2: return launch_march_line<4, 2>(p, st);
             case 2 * 16 + 2: return launch_march_line<2, 2>(p, st);
-            default: return cudaErrorInvalidValue;
-        }
-    }
-    if (p.hit_list != nullptr) {  // the sparse march over hit lists, inclined
-        switch (LV * 16 + NM) {
-            case 8 * 16 + 8: return launch_march_list<8, 8>(p, st);
-            case 8 * 16 + 4: return launch_march_list<8, 4>(p, st);
-            case 8 * 16 + 2: return launch_march_list<8, 2>(p, st);
-            case 4 * 16 + 4: return launch_march_list<4, 4>(p, st);
-            case 4 * 16 + 2: return launch_march_list<4, 2>(p, st);
-            case 2 * 16 + 2: return launch_march_list<2, 2>(p, st);
             default: return cudaErrorInvalidValue;
         }
     }

@@ -235,6 +235,21 @@ def test_march_over_hit_lists_with_inclinations(oracle, n, nlambda):
         check(atm, oracle, analyse=True)
 
 
+@pytest.mark.parametrize("n,nlambda", [(1, 6), (1, 1), (2, 9), (8, 3)])
+def test_march_over_hit_lists_with_the_moving_line(oracle, n, nlambda):
+    """The paper's production set-up - velocity-dependent line, inclinations, a quarter of the cells flagged
+     - over hit lists: bit-identical to the lock-step march of the same flagged atmosphere."""
+    line = A.with_active_cells(A.line_config2(nx=128, ny=96, nlambda=nlambda, ncascades=5), mode="fraction", fraction=0.25)
+    if n > 1:
+        line = A.with_inclinations(line, n)
+    ref, st0 = gpu(line)
+    got, st1 = gpu(line, analyse=True)
+    assert st0.sparse_march == 0 and st1.sparse_march == 1 and st1.sparse_lists == 1
+    assert np.array_equal(ref, got)
+    if n <= 2:
+        check(line, oracle, analyse=True)
+
+
 def test_hit_lists_are_kept_while_the_occupancy_stands():
     """A new atmosphere with the same occupancy map (other values in the same cells) keeps the hit lists (sparse_lists = 2);
     another map rebuilds them (1); both give the lock-step result bit for bit."""
