@@ -40,6 +40,9 @@ NCU_CAPTURES = {
     ("flat", 2, 5): {"dram_bytes": 2.032214e9 + 0.268770e9, "l2_to_sm_bytes": 486.879790e9, "lts_pct": 45.92,
                      "source": "profiles/ncu_r2_march.md: ncu --set full of march_kernel<8,1,3,8,2,0,0>, cascade 5 of config 2, "
                                "commit 0eaea15 (30.87 ms under ncu)"},
+    ("flat", 4, 5): {"dram_bytes": 149.013561e9 + 3.931215e9, "l2_to_sm_bytes": 346.691831e9, "lts_pct": 29.76,
+                     "source": "profiles/ncu_r2_modes.md: ncu --set full of march_list_kernel<8,8,4,6> (hit lists), cascade 5 of config 4, "
+                               "commit 04f0446 (48.2 ms under ncu)"},
     ("line_incl8", 2, 5): {"dram_bytes": 5.789094e9 + 2.674684e9, "l2_to_sm_bytes": 1879.661e9, "lts_pct": 11.03,
                            "source": "profiles/ncu_r2_modes.md: ncu --set full of march_kernel<8,8,2,8,3,0,1>, cascade 5 of the "
                                      "moving line x 8 inclinations on the config-2 grid, commit 0eaea15 (497.3 ms under ncu)"},
