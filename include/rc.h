@@ -203,7 +203,7 @@ int rc_analyse_atmosphere(rc_ctx *ctx);
  * and reports rc_stats.sparse_list_bytes; when this buffer is missing or smaller the distance-field march stays in use
  * (rc_stats.sparse_lists = 0) - lend at least that many bytes and analyse again.  The lists are kept across atmospheres
  * of the same shape and flags for as long as rc_analyse_atmosphere finds the same occupancy map (the formal solutions of an
- * iteration change chi and eta, not where they vanish): the analysis then costs one scan.  Config 4: 3.6 GB, 435 -> 134 ms per solve. */
+ * iteration change chi and eta, not where they vanish): the analysis then costs one scan.  Config 4: 3.6 GB, 435 -> 124 ms per solve. */
 int rc_set_sparse_workspace(rc_ctx *ctx, void *dev_ptr, size_t bytes);
 
 /* Boundary intensity sampled by the top cascade: I_below[l] is seen by rays heading

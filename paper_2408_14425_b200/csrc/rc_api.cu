@@ -745,6 +745,10 @@ int rc_set_lambda_weights(rc_ctx *ctx, const float *w) {
 // on config 2, short rays (cascades <= 3) like 20 warps/SM with a ring of 2, long rays 16 warps/SM with a ring of 3.
 static int march_variant(const rc_ctx *ctx, int i) { return ctx->tune.variant >= 0 ? ctx->tune.variant : (i <= 3 ? 4 : 2); }
 
+// Under the march over hit lists: does cascade i use them (else it runs lock-step)?
+// (moving line: from cascade 1 - measured on the paper's regime, cascade 1: 8.2 ms over lists, 13.1 ms lock-step)
+static bool list_cascade(const rc_ctx *ctx, int i) { return i >= (ctx->line ? 1 : 2) && !ctx->plan.c[i].empty; }
+
 // Parameters of cascade i's march launch.
 static rc::MarchParams march_params(const rc_ctx *ctx, int i, float *J_out) {
     const Plan &P = ctx->plan;
@@ -759,7 +763,10 @@ static rc::MarchParams march_params(const rc_ctx *ctx, int i, float *J_out) {
     mp.xls = ctx->line ? (const float *)(ctx->ws + P.xls) : nullptr;
     mp.dist = ctx->sparse ? (const unsigned char *)(ctx->ws + P.dist) : nullptr;
     mp.sparse_mode = ctx->tune.sparse_mode;
-    const bool lists = ctx->sparse && ctx->lists;
+    // over hit lists from cascade 2 up; cascades 0 and 1 (rays of a few steps: nothing to skip, the merge is the work) and
+    // cascades outside the box (boundary term and merge only) run lock-step even then (config 4: 24 of 134 ms -> 15)
+    const bool lists = ctx->sparse && ctx->lists && list_cascade(ctx, i);
+    if (ctx->sparse && ctx->lists && !lists) mp.dist = nullptr;
     mp.hit_off = lists ? (const unsigned *)(ctx->sws + ctx->hit_off[i]) : nullptr;
     mp.hit_list = lists ? (const unsigned short *)(ctx->sws + ctx->hit_list[i]) : nullptr;
     mp.list_b = ctx->list_b;
@@ -858,7 +865,7 @@ static int enqueue_solve(rc_ctx *ctx, float *J_out, int b0 = 0, int bn = -1) {
         if (accum) RC_CUDA(ctx, cudaMemsetAsync(ctx->ws + P.Jpart, 0, ncell * P.nb * sizeof(float), ctx->stream));
         else RC_CUDA(ctx, cudaMemsetAsync(J_out, 0, ncell * P.L * sizeof(float), ctx->stream));
     }
-    auto pack = [&](int shift) -> int {
+    auto pack = [&](int shift, bool list_layout = true) -> int {
         rc::PackParams pp{};
         pp.chi = ctx->chi; pp.eta = ctx->eta;
         pp.chiT = (float *)(ctx->ws + P.chiT); pp.ST = (float *)(ctx->ws + P.ST);
@@ -869,7 +876,7 @@ static int enqueue_solve(rc_ctx *ctx, float *J_out, int b0 = 0, int bn = -1) {
         float fmax = 1.f;
         for (int m = 0; m < ctx->nm; m++) fmax = std::max(fmax, ctx->incl_f[m]);
         pp.c_thin = (1.f / 64.f) / fmax;
-        pp.list_b = ctx->sparse && ctx->lists ? ctx->list_b : 0;
+        pp.list_b = ctx->sparse && ctx->lists && list_layout ? ctx->list_b : 0;
         if (ctx->line) {
             pp.chi = ctx->line; pp.eta = nullptr;
             RC_CUDA(ctx, rc::launch_pack_line(pp, ctx->stream));
@@ -903,6 +910,9 @@ static int enqueue_solve(rc_ctx *ctx, float *J_out, int b0 = 0, int bn = -1) {
     for (int i = top; i >= 0; i--) {
         const CascadePlan &c = P.c[i];
         if (!c.empty && !ctx->sparse && !multi) { const int rc = pack(c.fix ? i + 1 : i); if (rc != RC_OK) return rc; }
+        // under the hit lists the lowest cascades run lock-step from their own phase-plane packing (the list cascades,
+        // marched before them, are done with the packed arrays by then)
+        if (!c.empty && ctx->sparse && ctx->lists && !list_cascade(ctx, i)) { const int rc = pack(i, false); if (rc != RC_OK) return rc; }
         if (ev) RC_CUDA(ctx, cudaEventRecord(ev[1 + 2 * (top - i)], ctx->stream));
         rc::MarchParams mp = march_params(ctx, i, J_out);
         mp.nb = bn; mp.nb0 = b0;
@@ -1045,12 +1055,12 @@ static int build_hit_lists(rc_ctx *ctx) {
     const size_t occ_bytes = align_up((size_t)P.nx * P.ny);      // the occupancy map the lists belong to
     size_t cur = occ_bytes + bsum_bytes;
     for (int i = 0; i < nc; i++) {
-        if (P.c[i].empty) continue;
+        if (!list_cascade(ctx, i)) continue;
         ctx->hit_off[i] = cur; cur += off_bytes;
     }
     const bool have_off = ctx->sws != nullptr && cur <= ctx->sws_bytes;
     for (int i = 0; i < nc; i++) {
-        if (P.c[i].empty) continue;
+        if (!list_cascade(ctx, i)) continue;
         rc::MarchParams mp = march_params(ctx, i, nullptr);
         RC_CUDA(ctx, rc::launch_hit_walk(mp, false, have_off ? (unsigned *)(ctx->sws + ctx->hit_off[i]) : nullptr, nullptr, tot_d + i, ctx->stream));
     }
@@ -1059,7 +1069,7 @@ static int build_hit_lists(rc_ctx *ctx) {
     RC_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     bool fits32 = true;
     for (int i = 0; i < nc; i++) {
-        if (P.c[i].empty) continue;
+        if (!list_cascade(ctx, i)) continue;
         ctx->hit_list[i] = cur; cur += align_up(sizeof(unsigned short) * (size_t)tot[i] + 2);
         fits32 = fits32 && tot[i] < 0xffffffffULL;
     }
@@ -1067,14 +1077,12 @@ static int build_hit_lists(rc_ctx *ctx) {
     ctx->list_bytes = (int64_t)cur;
     if (!have_off || cur > ctx->sws_bytes || !fits32) return RC_OK;  // no room (or too many hits): the distance-field march
     for (int i = 0; i < nc; i++) {
-        if (P.c[i].empty) continue;
+        if (!list_cascade(ctx, i)) continue;
         rc::MarchParams mp = march_params(ctx, i, nullptr);
         unsigned *off = (unsigned *)(ctx->sws + ctx->hit_off[i]);
         RC_CUDA(ctx, rc::launch_hit_scan(off, (long long)nrays, (unsigned *)(ctx->sws + occ_bytes), tot[i], ctx->stream));
         RC_CUDA(ctx, rc::launch_hit_walk(mp, true, off, (unsigned short *)(ctx->sws + ctx->hit_list[i]), nullptr, ctx->stream));
     }
-    for (int i = 0; i < nc; i++)
-        if (P.c[i].empty) { ctx->hit_off[i] = 0; ctx->hit_list[i] = 0; }  // any valid address: never read (cnt == null)
     // Wavelength batches per warp: the lanes of a ray share its list and table reads (measured on config 4: 218 / 167 / 134
     // / 135 ms at 1 / 2 / 4 / 8 batches per warp; config 3 with 25 % of the cells flagged, 4 batches: 210 / 146 / 130 ms)
     ctx->list_b = ctx->tune.list_b > 0 ? ctx->tune.list_b : P.nb >= 6 ? 8 : P.nb >= 3 ? 4 : P.nb;
