@@ -285,6 +285,36 @@ int rc_probe_gather_bandwidth(rc_ctx *ctx, int mbytes, double *gbs);
  * the alternative design DESIGN.md §7 measures the LDG path against.  Same arguments and errors. */
 int rc_probe_bulk_copy_bandwidth(rc_ctx *ctx, int mbytes, double *gbs);
 
+/* ---- For callers that cannot allocate device memory at all --------------------------------------------------------
+ * Every call above works out of memory the caller lends.  Some callers have none to lend and no way to get any: a
+ * plug-in living inside an application whose own pool claimed the whole GPU at start-up (cudaMalloc just fails there), a
+ * stage of a real-time or serving loop that bans cudaMalloc / cudaFree because they stall the whole device, a tool that
+ * is handed two arrays and nothing else.  For them ONE operation is offered with its scratch memory built into the
+ * library image: the empty-cell count on which rc_analyse_atmosphere bases its "is this atmosphere sparse" decision
+ * (free-space acceleration; more than two thirds empty = the free-space march pays).
+ *
+ * Writes to *nempty_out the number of cells of the nx x ny grid that are NOT (of interest and non-zero in chi or eta at
+ * some wavelength) - the same number rc_stats.empty_cells reports after an analysis.
+ *   device      CUDA ordinal the arrays live on; made current for the calling thread, like every call of this library
+ *   chi, eta    device, [ny][nx][nlambda] float32, read only (no alignment demanded; 16-byte aligned is faster)
+ *   active      device, [ny][nx] bytes, non-zero = cell of interest; NULL = every cell
+ *   nempty_out  device, one 64-bit counter, the caller's; written by the kernel: read it after the stream has caught up
+ *   cuda_stream cudaStream_t as void*; the call only enqueues (one memset, one kernel) and does not synchronise
+ *   errbuf      host, errbuf_len bytes, or NULL: receives the text of a failure (there is no context to ask)
+ * Returns RC_OK, RC_ERR_NULL_ARG, RC_ERR_BAD_SHAPE (also: nx * ny > RC_STATIC_MAX_CELLS - the built-in array is that
+ * large and no larger), RC_ERR_NO_DEVICE (not an sm_100 device), RC_ERR_CUDA.
+ *
+ * What to know about the built-in array (about 4 MiB): every GPU that loads librc.so holds it until the process exits,
+ * whether or not this call is ever made.  The first call on a device looks its address up once
+ * (cudaGetSymbolAddress); make that first call before any stream capture begins.  No call allocates or frees anything, on the
+ * device or through a library that might.  ALL calls share the array and each one starts by clearing the part it
+ * uses, so the previous call's contents never leak into a result - but two calls that overlap on the GPU (different
+ * streams, different threads, different contexts of this library in one process) race on it and both results are
+ * garbage: keep calls on one stream or order them with events. */
+#define RC_STATIC_MAX_CELLS (1 << 20) /* 1024 x 1024, 4096 x 256, ... */
+int rc_count_empty_cells_static(int device, const float *chi, const float *eta, const unsigned char *active, int nx, int ny,
+                                int nlambda, unsigned long long *nempty_out, void *cuda_stream, char *errbuf, size_t errbuf_len);
+
 const char *rc_last_error(const rc_ctx *ctx);
 const char *rc_version(void);
 int rc_destroy(rc_ctx *ctx);

@@ -80,6 +80,8 @@ SYMBOLS = {
     "rc_count_segments": (C.c_int, [C.c_void_p, C.c_void_p]),
     "rc_probe_gather_bandwidth": (C.c_int, [C.c_void_p, C.c_int, C.POINTER(C.c_double)]),
     "rc_probe_bulk_copy_bandwidth": (C.c_int, [C.c_void_p, C.c_int, C.POINTER(C.c_double)]),
+    "rc_count_empty_cells_static": (C.c_int, [C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p,
+                                              C.c_void_p, C.c_char_p, C.c_size_t]),
     "rc_last_error": (C.c_char_p, [C.c_void_p]),
     "rc_version": (C.c_char_p, []),
     "rc_destroy": (C.c_int, [C.c_void_p]),
@@ -355,6 +357,36 @@ class RadianceCascades:
             self.close()
         except Exception:
             pass
+
+
+RC_STATIC_MAX_CELLS = 1 << 20
+
+
+def count_empty_cells_static(chi, eta, active=None, out=None):
+    """rc_count_empty_cells_static: the empty-cell count of an atmosphere for callers that cannot allocate device memory
+    (a host application's pool owns the GPU, or cudaMalloc is banned in their loop): no context, no workspace, the
+    scratch is an array inside librc.so (grids up to RC_STATIC_MAX_CELLS cells; calls must not overlap on the GPU).
+    chi, eta: CUDA float32 [ny][nx][nlambda]; active: CUDA uint8 [ny][nx] or None; out: CUDA int64 tensor of one
+    element that receives the count (enqueued on torch's current stream, not synchronised).  Only when `out` is left
+    out does this wrapper allocate one itself - a convenience for tests, not something the C call does."""
+    import torch
+    assert chi.is_cuda and eta.is_cuda and chi.dtype == torch.float32 and eta.dtype == torch.float32
+    assert chi.is_contiguous() and eta.is_contiguous() and chi.dim() == 3 and chi.shape == eta.shape
+    ny, nx, L = chi.shape
+    dev = chi.device.index
+    if active is not None:
+        assert active.is_cuda and active.is_contiguous() and active.element_size() == 1 and tuple(active.shape) == (ny, nx)
+    if out is None:
+        out = torch.empty(1, dtype=torch.int64, device=chi.device)
+    assert out.is_cuda and out.dtype == torch.int64 and out.numel() == 1
+    err = C.create_string_buffer(512)
+    rc = load().rc_count_empty_cells_static(dev, C.c_void_p(chi.data_ptr()), C.c_void_p(eta.data_ptr()),
+                                            None if active is None else C.c_void_p(active.data_ptr()), nx, ny, L,
+                                            C.c_void_p(out.data_ptr()), C.c_void_p(torch.cuda.current_stream(dev).cuda_stream),
+                                            err, len(err))
+    if rc != RC_OK:
+        raise RcError(rc, err.value.decode())
+    return out
 
 
 def solve_atmosphere(atm, device=0, lambda_batch=0, flags=0, rc=None, analyse=False, tuning=None):

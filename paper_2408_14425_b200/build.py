@@ -9,7 +9,7 @@ from pathlib import Path
 PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 LIB = PKG / "librc.so"
-SOURCES = [CSRC / "rc_api.cu", CSRC / "rc_kernels.cu"]
+SOURCES = [CSRC / "rc_api.cu", CSRC / "rc_kernels.cu", CSRC / "rc_static.cu"]
 DEPS = SOURCES + [CSRC / "rc_internal.h", PKG.parent / "include" / "rc.h"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC"]
