@@ -900,3 +900,103 @@ def test_S5_sparse_window_solve_is_the_sparse_full_solve_restricted(oracle):
         x0, x1, y0, y1 = win
         w = oracle.solve_atmosphere(a, active=act, window=win)
         assert np.array_equal(w["J"], full["J"][y0:y1, x0:x1]) and np.array_equal(w["Jbar"], full["Jbar"][y0:y1, x0:x1])
+
+
+# ----------------------------------------------------------------------------- cascade-0 interval length != 1 (eq. 12-13)
+# PAPER.md:171-176 (eq. 12-13 with alpha = 2): t_i = c0 (4^i - 1)/3 for ANY cascade-0 interval length c0; PAPER.md:571 runs
+# the paper's models with c0 = 1.5 voxels.  Every pin above has c0 = 1, where c0, c0^2, 1/c0 ... are the same number.
+C0 = 1.5
+
+
+def test_C1_cascade0_closed_form_with_interval_one_and_a_half(oracle):
+    """P13 with the interval [0, 1.5]: sqrt2/2 in the own cell, 1.5 - sqrt2/2 in the diagonal neighbour (whose far
+    corner lies at 3 sqrt2/2 > 1.5), vacuum outside the box."""
+    nx, ny = 8, 8
+    chi, eta = A.random_field(nx, ny, 1, seed=17)
+    out = oracle.solve(chi, eta, 2, c0=C0, dump_cascade=0)
+    c64, e64 = chi[..., 0].astype(float), eta[..., 0].astype(float)
+    a, b = R2 / 2, C0 - R2 / 2
+    for y in range(ny):
+        for x in range(nx):
+            for q, (sx, sy) in enumerate([(1, 1), (-1, 1), (-1, -1), (1, -1)]):
+                xo, yo = x + sx, y + sy
+                inside = 0 <= xo < nx and 0 <= yo < ny
+                cd, ed = (c64[yo, xo], e64[yo, xo]) if inside else (0.0, 0.0)
+                To = np.exp(-c64[y, x] * a)
+                I = e64[y, x] / c64[y, x] * (1 - To) + To * (ed / cd * (1 - np.exp(-cd * b)) if inside else 0.0)
+                assert np.isclose(out["dump_I"][y, x, q, 0], I, rtol=1e-12)
+                assert np.isclose(out["dump_T"][y, x, q, 0], To * np.exp(-cd * b), rtol=1e-12)
+
+
+def test_C2_hand_derived_2x2_with_cascade_1_starting_outside_the_box(oracle):
+    """2 x 2 cells, 2 cascades, c0 = 1.5.  Cascade 1's single probe sits at the grid centre and its rays start at
+    t_1 = 1.5 > sqrt2 >= the distance to the box edge in any direction: every cascade-1 interval starts outside, is
+    empty, and carries the boundary intensity alone (reading G10).  Cascade 0 covers [0, 1.5]: own cell
+    sqrt2/2, then 1.5 - sqrt2/2 of the diagonal neighbour where there is one.  With t_1 = 1 (the c0 = 1 value) or 2.25
+    (c0^2) either cascade 1 or cascade 0 would integrate different lengths."""
+    chi = np.array([[[0.7], [1.3]], [[0.2], [2.1]]], np.float32)
+    eta = chi * np.array([[[1.0], [0.5]], [[2.0], [0.25]]], np.float32)
+    Ib, Ia = 0.3, 0.9
+    c, e = chi[..., 0].astype(float), eta[..., 0].astype(float)
+    a, b = R2 / 2, C0 - R2 / 2
+    J = np.zeros((2, 2))
+    for y in range(2):
+        for x in range(2):
+            for q, (sx, sy) in enumerate([(1, 1), (-1, 1), (-1, -1), (1, -1)]):
+                xo, yo = x + sx, y + sy
+                To = np.exp(-c[y, x] * a)
+                I, T = e[y, x] / c[y, x] * (1 - To), To
+                if 0 <= xo < 2 and 0 <= yo < 2:
+                    Td = np.exp(-c[yo, xo] * b)
+                    I, T = I + To * e[yo, xo] / c[yo, xo] * (1 - Td), T * Td
+                J[y, x] += 0.25 * (I + T * (Ia if sy > 0 else Ib))   # the 4 children of quadrant q all head the same way in y
+    out = oracle.solve(chi, eta, 2, c0=C0, I_below=[Ib], I_above=[Ia])
+    assert np.allclose(out["J"][..., 0], J, rtol=1e-13)
+
+
+def _independent_cascades(chi, eta, ncasc, c0, Ib, Ia):
+    """J by an independent brute force over `ncasc` cascades: ray/cell intersections by sorting (tests/refs.py), interval
+    ends t_i = c0 (4^i - 1)/3 typed out here, parents from the geometric position of the child among them (A4)."""
+    ny, nx = chi.shape[:2]
+    c, e = chi[..., 0].astype(np.float64).ravel(), eta[..., 0].astype(np.float64).ravel()
+    ends = [c0 * (4.0 ** i - 1.0) / 3.0 for i in range(ncasc)] + [1e9]
+
+    def interp(a_, n):
+        u = (a_ + 0.5) / 2.0 - 0.5
+        lo = int(np.floor(u))
+        cl = lambda q: min(max(q, 0), n - 1)
+        return (cl(lo), 1.0 - (u - lo)), (cl(lo + 1), u - lo)
+
+    M_up = None
+    for i in range(ncasc - 1, -1, -1):
+        s, nd = 2 ** i, 4 ** (i + 1)
+        M = np.zeros((ny // s, nx // s, nd))
+        for b in range(ny // s):
+            for a_ in range(nx // s):
+                for k in range(nd):
+                    th = 2 * np.pi * (k + 0.5) / nd
+                    cells, ds = refs.segments_by_sorting(nx, ny, (a_ + 0.5) * s, (b + 0.5) * s, th, ends[i], ends[i + 1])
+                    I, T = refs.integrate(c, e, cells, ds)
+                    if M_up is None:
+                        U = Ib if np.sin(th) < 0 else Ia
+                    else:
+                        U = sum(wa * wb * M_up[bq, aq, 4 * k:4 * k + 4].mean()
+                                for (bq, wb) in interp(b, ny // (2 * s)) for (aq, wa) in interp(a_, nx // (2 * s)))
+                    M[b, a_, k] = I + T * U
+        M_up = M
+    return M_up.mean(axis=2)
+
+
+def test_C3_three_cascades_with_interval_one_and_a_half_against_independent_reference(oracle):
+    """The twin of A4 with three cascades and c0 = 1.5: intervals [0, 1.5], [1.5, 7.5], [7.5, inf) on 12 x 8 cells, so
+    that t_1 and t_2 both lie inside the box and both scale with c0.  The same reference at c0 = 1
+    reproduces the oracle too, and the two differ by far more than the tolerance."""
+    nx, ny = 12, 8
+    rng = np.random.default_rng(31)
+    chi = rng.uniform(0.05, 0.6, (ny, nx, 1)).astype(np.float32)
+    eta = (chi * rng.uniform(0.2, 2.0, (ny, nx, 1))).astype(np.float32)
+    Ib, Ia = 0.4, 0.1
+    got = {c0: oracle.solve(chi, eta, 3, c0=c0, I_below=[Ib], I_above=[Ia])["J"][..., 0] for c0 in (1.0, C0)}
+    for c0 in (1.0, C0):
+        assert np.allclose(got[c0], _independent_cascades(chi, eta, 3, c0, Ib, Ia), rtol=1e-10)
+    assert np.max(np.abs(got[C0] / got[1.0] - 1)) > 1e-3
