@@ -87,9 +87,10 @@ struct rc_ctx {
     int tab_nx = 0, tab_ny = 0;  // shape the step tables in the workspace were built for
     bool host_io = false;
     // CUDA graph of the launch sequence of small grids (rc_solve_J) and what it was captured for
-    struct GraphKey { const void *J, *chi, *eta, *line, *ws; int nx, ny, L, nm, sparse; size_t total; float f[8], w[8]; };
+    struct GraphKey { const void *J, *chi, *eta, *line, *ws; int nx, ny, L, nm, sparse, tune_gen; size_t total; float f[8], w[8]; };
     GraphKey graph_key{};
     cudaGraphExec_t graph_exec = nullptr;
+    int tune_gen = 0;  // counts rc_set_tuning calls: a knob may change launch variants and workspace offsets
     cudaStream_t cap_stream = nullptr;
     cudaStream_t copy_stream = nullptr;   // rc_solve_J_host's pipeline: the other half's copies
     cudaEvent_t pipe_ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
@@ -110,6 +111,8 @@ struct rc_ctx {
     bool count_walked = false; // the solve being enqueued counts the segments it integrates (rc_count_walked)
     bool analysed = false;     // rc_analyse_atmosphere has been used on this context (rc_solve_J_host then repeats it)
     std::vector<float> xl_stage;  // line mode: host copy of the scaled wavelengths (kept alive for the async upload)
+    bool xl_on_device = false;    // the workspace holds xl_stage at plan.xls: false after anything that moves or overwrites that region
+                                  // (another workspace, a new plan, a GivenFs atmosphere whose packed arrays share the bytes)
     Tuning tune{};
     // 2.5D inclination quadrature (rc_set_inclinations); nm = 1, f = w = 1: flatland
     int nm = 1;
@@ -489,12 +492,30 @@ int rc_destroy(rc_ctx *ctx) {
     return RC_OK;
 }
 
+// Where rc_solve_J_line_host stages the line parameters and J: in the host_io region of the GivenFs plan (which
+// rc_workspace_bytes sizes), but never below the end of what the LINE plan's solve reads and writes - the two plans are
+// laid out independently.  Returns the bytes of workspace this needs.
+static size_t line_host_io_layout(const rc_ctx *ctx, int nx, int ny, int nlambda, size_t *o_line, size_t *o_J) {
+    Plan Pio, Pl;
+    make_plan(ctx->cfg, ctx->tune, ctx->nm, false, nx, ny, nlambda, true, Pio, nullptr);
+    make_plan(ctx->cfg, ctx->tune, ctx->nm, true, nx, ny, nlambda, false, Pl, nullptr);
+    const size_t ncell = (size_t)nx * ny;
+    const size_t nout = ncell * ((ctx->cfg.flags & RC_ACCUM_J) ? 1 : (size_t)nlambda) * sizeof(float);
+    *o_line = std::max(Pio.io_chi, align_up(Pl.total));
+    *o_J = std::max(Pio.io_J, *o_line + align_up(ncell * 6 * sizeof(float)));
+    return *o_J + align_up(nout);
+}
+
 size_t rc_workspace_bytes(const rc_ctx *ctx, int nx, int ny, int nlambda, int host_io) {
     if (!ctx) return 0;
     Plan P;
     if (!make_plan(ctx->cfg, ctx->tune, ctx->nm, false, nx, ny, nlambda, host_io != 0, P, nullptr)) return 0;
     size_t need = P.total;
     if (make_plan(ctx->cfg, ctx->tune, ctx->nm, true, nx, ny, nlambda, false, P, nullptr)) need = std::max(need, P.total);  // line mode
+    if (host_io) {
+        size_t a, b;
+        need = std::max(need, line_host_io_layout(ctx, nx, ny, nlambda, &a, &b));  // rc_solve_J_line_host
+    }
     return need;
 }
 
@@ -506,6 +527,7 @@ int rc_set_workspace(rc_ctx *ctx, void *dev_ptr, size_t bytes) {
     ctx->ws_bytes = bytes;
     ctx->tab_nx = ctx->tab_ny = 0;  // tables live in the workspace: rebuild
     ctx->have_atm = false;
+    ctx->xl_on_device = false;
     return RC_OK;
 }
 
@@ -536,6 +558,7 @@ int rc_set_tuning(rc_ctx *ctx, const char *name, double value) {
     else if (n == "sorted") { if (iv < -1 || iv > 1) goto bad; t.sorted = iv; }
     else return fail(ctx, RC_ERR_BAD_VALUE, "rc_set_tuning: unknown knob '%s'", name);
     // the plan (bands), the patch lists and a captured graph may depend on a knob: start over
+    ctx->tune_gen++;
     ctx->have_atm = false;
     ctx->active_set = false; ctx->lists_dirty = false; ctx->sparse = false; ctx->lists_built = false;
     return RC_OK;
@@ -575,6 +598,7 @@ static int prepare_shape(rc_ctx *ctx, int nx, int ny, int nlambda, bool line) {
         ctx->host_io = Pio.total <= ctx->ws_bytes;
         ctx->plan = ctx->host_io ? Pio : P;
         ctx->have_atm = false;
+        ctx->xl_on_device = false;  // plan.xls depends on the shape and the banding
         ctx->active_set = false; ctx->lists_dirty = false; ctx->sparse = false; ctx->lists_built = false;
         ctx->stats.active_cells = -1;
         // geometry tables: only when the grid size changed (they do not depend on nlambda)
@@ -632,6 +656,7 @@ int rc_set_atmosphere(rc_ctx *ctx, const float *chi, const float *eta, int nx, i
         if (rc != RC_OK) return rc;
     }
     ctx->line = nullptr;
+    ctx->xl_on_device = false;
     if (ctx->cfg.flags & RC_VALIDATE) {
         int *flag = (int *)(ctx->ws + ctx->plan.flag);
         int h = 0;
@@ -664,11 +689,12 @@ int rc_set_line_atmosphere(rc_ctx *ctx, const float *line, int nx, int ny, const
         h[l] = (float)((double)x_lambda[l] * 1.2011224087864498);  // sqrt(log2 e)
         h[(size_t)ctx->plan.Lpad + l] = x_lambda[l];
     }
-    if (h != ctx->xl_stage) {  // steady state (same wavelengths again): nothing to upload, nothing to wait for
+    if (!ctx->xl_on_device || h != ctx->xl_stage) {  // steady state (same wavelengths, same place): nothing to upload, nothing to wait for
         RC_CUDA(ctx, cudaStreamSynchronize(ctx->stream));  // an earlier upload may still be reading xl_stage
         ctx->xl_stage.swap(h);
         RC_CUDA(ctx, cudaMemcpyAsync(ctx->ws + ctx->plan.xls, ctx->xl_stage.data(), ctx->xl_stage.size() * sizeof(float),
                                      cudaMemcpyHostToDevice, ctx->stream));
+        ctx->xl_on_device = true;
     }
     ctx->line = line;
     ctx->chi = ctx->eta = nullptr;
@@ -976,7 +1002,9 @@ int rc_solve_J(rc_ctx *ctx, float *J_out) {
     rc_ctx::GraphKey key;
     std::memset(&key, 0, sizeof(key));
     key.J = J_out; key.chi = ctx->chi; key.eta = ctx->eta; key.line = ctx->line; key.ws = ctx->ws;
-    key.nx = P.nx; key.ny = P.ny; key.L = P.L; key.nm = P.NM; key.sparse = (ctx->sparse ? 1 : 0) + (ctx->active_set ? 2 : 0) + 4 * ctx->list_version;  // (list_version also counts the analyses) key.total = P.total;
+    key.nx = P.nx; key.ny = P.ny; key.L = P.L; key.nm = P.NM; key.sparse = (ctx->sparse ? 1 : 0) + (ctx->active_set ? 2 : 0) + 4 * ctx->list_version;  // (list_version also counts the analyses)
+    key.total = P.total;
+    key.tune_gen = ctx->tune_gen;
     for (int m = 0; m < 8; m++) { key.f[m] = ctx->incl_f[m]; key.w[m] = ctx->incl_w[m]; }
     if (!ctx->graph_exec || std::memcmp(&key, &ctx->graph_key, sizeof(key)) != 0) {
         if (ctx->graph_exec) { cudaGraphExecDestroy(ctx->graph_exec); ctx->graph_exec = nullptr; }
@@ -1200,13 +1228,12 @@ int rc_solve_J_line_host(rc_ctx *ctx, const float *line_host, int nx, int ny, co
     if (!shape_ok(ctx->cfg, nx, ny, nlambda)) return fail(ctx, RC_ERR_BAD_SHAPE, "bad shape %dx%dx%d", nx, ny, nlambda);
     if (!ctx->ws) return fail(ctx, RC_ERR_NO_WORKSPACE, "rc_set_workspace has not been called");
     RC_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
-    Plan Pio;
-    make_plan(ctx->cfg, ctx->tune, ctx->nm, false, nx, ny, nlambda, true, Pio, nullptr);  // the host_io region of the GivenFs plan holds both
-    if (Pio.total > ctx->ws_bytes)
-        return fail(ctx, RC_ERR_NO_WORKSPACE, "workspace has %zu bytes, %zu needed with host_io", ctx->ws_bytes, Pio.total);
+    size_t o_line, o_J;
+    const size_t need = line_host_io_layout(ctx, nx, ny, nlambda, &o_line, &o_J);
+    if (need > ctx->ws_bytes)
+        return fail(ctx, RC_ERR_NO_WORKSPACE, "workspace has %zu bytes, %zu needed with host_io", ctx->ws_bytes, need);
     const size_t nline = (size_t)nx * ny * 6 * sizeof(float);
-    float *dline = (float *)(ctx->ws + Pio.io_chi), *dJ = (float *)(ctx->ws + Pio.io_J);
-    if (nline > Pio.io_J - Pio.io_chi) return fail(ctx, RC_ERR_NO_WORKSPACE, "host_io region too small for the line parameters");
+    float *dline = (float *)(ctx->ws + o_line), *dJ = (float *)(ctx->ws + o_J);
     RC_CUDA(ctx, cudaMemcpyAsync(dline, line_host, nline, cudaMemcpyHostToDevice, ctx->stream));
     int rc = rc_set_line_atmosphere(ctx, dline, nx, ny, x_lambda, nlambda);
     if (rc != RC_OK) return rc;
@@ -1235,7 +1262,8 @@ int rc_solve_J_host(rc_ctx *ctx, const float *chi_host, const float *eta_host, i
     // second half's inputs and the first half's J crossing PCIe (strided 2D copies on a private stream) while the other
     // half is solved.  Exposed: the first half's H2D and the second half's D2H instead of all of both.
     const size_t ncell = (size_t)nx * ny;
-    const bool pipelined = ctx->tune.pipeline != 0 && !ctx->analysed && ctx->nsets == 0 && !(ctx->cfg.flags & RC_ACCUM_J) &&
+    // (not with RC_VALIDATE: the check reads the device copies, so they have to be complete before rc_set_atmosphere runs it)
+    const bool pipelined = ctx->tune.pipeline != 0 && !ctx->analysed && ctx->nsets == 0 && !(ctx->cfg.flags & (RC_ACCUM_J | RC_VALIDATE)) &&
                            Pio.nb >= 2 && (long long)ncell * Pio.Lpad * Pio.NM >= (1LL << 24);  // (config 1, 4 M cell-channels: slower in halves)
     if (pipelined) {
         int rc = rc_set_atmosphere(ctx, dchi, deta, nx, ny, nlambda);  // pointers (and, for a new shape, the tables)
