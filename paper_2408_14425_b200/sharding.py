@@ -23,8 +23,12 @@ def shard_atmosphere(atm, rank: int, world: int):
     l0, l1 = wavelength_block(atm.nlambda, rank, world)
     out = copy.copy(atm)
     out.nlambda = l1 - l0
-    out.chi = np.ascontiguousarray(atm.chi[:, :, l0:l1])
-    out.eta = np.ascontiguousarray(atm.eta[:, :, l0:l1])
+    if getattr(atm, "line", None) is not None:
+        # moving line: the six per-cell parameters are the same on every rank, the rank's block is its wavelengths x_l
+        out.xl = np.ascontiguousarray(atm.xl[l0:l1])
+    else:
+        out.chi = np.ascontiguousarray(atm.chi[:, :, l0:l1])
+        out.eta = np.ascontiguousarray(atm.eta[:, :, l0:l1])
     out.I_below = atm.I_below[l0:l1].copy()
     out.I_above = atm.I_above[l0:l1].copy()
     out.weights = atm.weights[l0:l1].copy()

@@ -14,7 +14,13 @@ from paper_2408_14425_b200 import atmospheres as A
 pytestmark = pytest.mark.gpu
 
 
-def _worker(rank, world, port, q, accumulate):
+def _atmosphere(mode):
+    if mode == "line":
+        return A.line_config2(nx=256, ny=128, nlambda=32, ncascades=6)
+    return A.make_config(4 if mode == "Jbar" else 2, nx=256, ny=128, nlambda=32, ncascades=6)
+
+
+def _worker(rank, world, port, q, mode):
     import torch
     import torch.distributed as dist
     from paper_2408_14425_b200 import binding, sharding
@@ -22,7 +28,8 @@ def _worker(rank, world, port, q, accumulate):
     os.environ["MASTER_PORT"] = str(port)
     torch.cuda.set_device(rank)
     dist.init_process_group("nccl", rank=rank, world_size=world, device_id=torch.device(f"cuda:{rank}"))
-    atm = A.make_config(4 if accumulate else 2, nx=256, ny=128, nlambda=32, ncascades=6)
+    accumulate = mode == "Jbar"
+    atm = _atmosphere(mode)
     mine = sharding.shard_atmosphere(atm, rank, world)
     J, rc = binding.solve_atmosphere(mine, device=rank)
     if accumulate:
@@ -37,8 +44,9 @@ def _worker(rank, world, port, q, accumulate):
     dist.destroy_process_group()
 
 
-@pytest.mark.parametrize("accumulate", [False, True])
-def test_two_ranks_nccl_match_one_rank(accumulate):
+@pytest.mark.parametrize("mode", ["J", "Jbar", "line"])
+def test_two_ranks_nccl_match_one_rank(mode):
+    accumulate = mode == "Jbar"
     import torch
     if torch.cuda.device_count() < 2:
         pytest.skip("needs two GPUs")
@@ -49,14 +57,14 @@ def test_two_ranks_nccl_match_one_rank(accumulate):
         port = s.getsockname()[1]
     ctx = mp.get_context("spawn")
     q = ctx.Queue()
-    procs = [ctx.Process(target=_worker, args=(r, 2, port, q, accumulate)) for r in range(2)]
+    procs = [ctx.Process(target=_worker, args=(r, 2, port, q, mode)) for r in range(2)]
     for p in procs:
         p.start()
     got = q.get(timeout=600)
     for p in procs:
         p.join(timeout=120)
         assert p.exitcode == 0
-    atm = A.make_config(4 if accumulate else 2, nx=256, ny=128, nlambda=32, ncascades=6)
+    atm = _atmosphere(mode)
     J, rc = binding.solve_atmosphere(atm)
     ref = J.cpu().numpy()
     rc.close()

@@ -21,15 +21,22 @@ def test_wavelength_blocks_partition():
             assert max(sizes) - min(sizes) <= 1
 
 
-def _worker(rank, world, port, q):
+def _atmosphere(line):
+    if line:   # the moving line shards by x_lambda: every rank holds the six per-cell line parameters
+        return A.line_config2(nx=64, ny=16, nlambda=5, ncascades=3)
+    return A.make_config(4, nx=64, ny=16, nlambda=5, ncascades=3)
+
+
+def _worker(rank, world, port, q, line):
     import torch
     import torch.distributed as dist
     from oracle import rc_oracle
     os.environ["MASTER_ADDR"] = "127.0.0.1"
     os.environ["MASTER_PORT"] = str(port)
     dist.init_process_group("gloo", rank=rank, world_size=world)
-    atm = A.make_config(4, nx=64, ny=16, nlambda=5, ncascades=3)
+    atm = _atmosphere(line)
     mine = sharding.shard_atmosphere(atm, rank, world)
+    assert mine.nlambda == (3 if rank == 0 else 2) and (not line or (mine.line is atm.line and len(mine.xl) == mine.nlambda))
     out = rc_oracle.solve_atmosphere(mine, nthreads=2)
     J = sharding.allgather_j(torch.from_numpy(out["J"]), atm.nlambda)
     Jbar = sharding.allreduce_jbar(torch.from_numpy(out["Jbar"].copy()))
@@ -39,21 +46,22 @@ def _worker(rank, world, port, q):
     dist.destroy_process_group()
 
 
-def test_two_rank_gloo_matches_single_rank(oracle):
+@pytest.mark.parametrize("line", [False, True])
+def test_two_rank_gloo_matches_single_rank(oracle, line):
     import torch.multiprocessing as mp
     with socket.socket() as s:
         s.bind(("127.0.0.1", 0))
         port = s.getsockname()[1]
     ctx = mp.get_context("spawn")
     q = ctx.Queue()
-    procs = [ctx.Process(target=_worker, args=(r, 2, port, q)) for r in range(2)]
+    procs = [ctx.Process(target=_worker, args=(r, 2, port, q, line)) for r in range(2)]
     for p in procs:
         p.start()
     J, Jbar = q.get(timeout=300)
     for p in procs:
         p.join(timeout=60)
         assert p.exitcode == 0
-    atm = A.make_config(4, nx=64, ny=16, nlambda=5, ncascades=3)
+    atm = _atmosphere(line)
     ref = oracle.solve_atmosphere(atm)
     assert np.array_equal(J, ref["J"])
     assert np.allclose(Jbar, ref["Jbar"], rtol=1e-14, atol=0)
