@@ -35,18 +35,66 @@ SM_COUNT, MUFU_PER_CLK_SM = 148, 16  # one ex2 per segment-wavelength; DESIGN.md
 # ncu --set full captures of the dominant launch that are committed under profiles/, keyed by (mode, config, cascade):
 # dram__bytes_read.sum + dram__bytes_write.sum per launch, l1tex__m_xbar2l1tex_read_bytes.sum (bytes that really came over
 # the L2 -> SM path; the algorithmic bytes also count what L1 served), lts__t_sectors % of peak, and where the capture is.
-# A run whose mode / config / launch plan has no entry reports traffic = null.  Re-capture when the dominant kernel changes.
+# A run whose mode / config / launch plan has no entry reports traffic = null.  Every entry names the kernel it is a capture
+# of and the sha of that kernel's source text at the capture's commit (kernel_text_sha): when HEAD's text differs the
+# capture describes another kernel, and the line reports its figures under `stale_capture` only, with traffic = null.
 NCU_CAPTURES = {
-    ("flat", 2, 5): {"dram_bytes": 2.032214e9 + 0.268770e9, "l2_to_sm_bytes": 486.879790e9, "lts_pct": 45.92,
-                     "source": "profiles/ncu_r2_march.md: ncu --set full of march_kernel<8,1,3,8,2,0,0>, cascade 5 of config 2, "
-                               "commit 0eaea15 (30.87 ms under ncu)"},
-    ("flat", 4, 5): {"dram_bytes": 149.013561e9 + 3.931215e9, "l2_to_sm_bytes": 346.691831e9, "lts_pct": 29.76,
-                     "source": "profiles/ncu_r2_modes.md: ncu --set full of march_list_kernel<8,8,4,6> (hit lists), cascade 5 of config 4, "
-                               "commit 04f0446 (48.2 ms under ncu)"},
-    ("line_incl8", 2, 5): {"dram_bytes": 5.789094e9 + 2.674684e9, "l2_to_sm_bytes": 1879.661e9, "lts_pct": 11.03,
+    ("flat", 2, 5): {"kernel": "march_kernel", "sha": "e6187b462936d78b", "commit": "e582544", "capture_ms": 30.78,
+                     "dram_bytes": 2.027300e9 + 0.269690e9, "l2_to_sm_bytes": 484.840640e9, "lts_pct": 46.02,
+                     "source": "profiles/ncu_r3.md: ncu --set full of march_kernel<8,1,3,8,2,0,0>, cascade 5 of config 2, "
+                               "commit e582544 (30.78 ms under ncu)"},
+    ("flat", 4, 5): {"kernel": "march_list_kernel", "sha": "7b7b5b40dbc40a63", "commit": "e582544", "capture_ms": 47.67,
+                     "dram_bytes": 149.293018e9 + 3.933113e9, "l2_to_sm_bytes": 348.052288e9, "lts_pct": 30.28,
+                     "source": "profiles/ncu_r3.md: ncu --set full of march_list_kernel<8,1,8,4,6,0> (hit lists), cascade 5 of config 4, "
+                               "commit e582544 (47.67 ms under ncu)"},
+    ("line_incl8", 2, 5): {"kernel": "march_kernel", "sha": "b9a7d603683de633", "commit": "0eaea15", "capture_ms": 497.3,
+                           "dram_bytes": 5.789094e9 + 2.674684e9, "l2_to_sm_bytes": 1879.661e9, "lts_pct": 11.03,
                            "source": "profiles/ncu_r2_modes.md: ncu --set full of march_kernel<8,8,2,8,3,0,1>, cascade 5 of the "
                                      "moving line x 8 inclinations on the config-2 grid, commit 0eaea15 (497.3 ms under ncu)"},
 }
+
+
+def kernel_text_sha(kernel: str):
+    """sha256 (16 hex digits) of the source text of one kernel of csrc/rc_kernels.cu together with the device helpers in front
+    of the march kernels (packed arithmetic, cell updates, warp -> probe mapping): what an ncu capture describes.  An entry
+    of NCU_CAPTURES whose sha differs from HEAD's text is a capture of another kernel and its numbers are not used."""
+    import hashlib
+    lines = (ROOT / "paper_2408_14425_b200" / "csrc" / "rc_kernels.cu").read_text().splitlines()
+    k = next((i for i, l in enumerate(lines) if l.startswith("__global__") and f" {kernel}(" in l), None)
+    if k is None:
+        return None
+    h0 = next(i for i, l in enumerate(lines) if "f32x2 pk2(" in l)
+    m = next(i for i, l in enumerate(lines) if l.startswith("__global__") and " march_kernel(" in l) - 1
+    b0 = k - 1 if lines[k - 1].startswith("template") else k
+    b1 = next(i for i in range(k, len(lines)) if lines[i] == "}")
+    return hashlib.sha256("\n".join(lines[h0:m] + lines[b0:b1 + 1]).encode()).hexdigest()[:16]
+
+
+def secondary_wanted(args, world):
+    """Only the plain default run (config 2, one GPU, no mode flags) carries the other configs along."""
+    return (world == 1 and args.config == 2 and not args.no_secondary and not args.line and not args.bilinear_fix
+            and args.inclinations == 1 and not args.active and not args.tune and not args.analyse and not args.no_analyse)
+
+
+def secondary_runs(configs=(0, 1, 3, 4), steps=3, warmup=3, timeout=420):
+    """The other BASELINE.json configs in the same driver run, so that each has a number under the driver's clock: this
+    script again, one child process per config (the GPU is idle while they run: the parent has finished timing), `steps`
+    timed steps each.  A child that fails or overruns leaves its error text, never an exception."""
+    out = {"note": f"bench.py --config N --steps {steps} --warmup {warmup} --no-cpu-baseline as child processes after the timed "
+                   "region of this line; ms are device-timed solves / end-to-end rc_solve_J_host steps as in the main line"}
+    for cfg in configs:
+        cmd = [sys.executable, str(Path(__file__).resolve()), "--config", str(cfg), "--steps", str(steps), "--warmup", str(warmup),
+               "--no-cpu-baseline", "--no-secondary"]
+        try:
+            r = subprocess.run(cmd, capture_output=True, text=True, timeout=timeout)
+            d = json.loads([l for l in r.stdout.splitlines() if l.startswith("{")][-1])
+            out[f"config{cfg}"] = {"workload": d["config"]["workload"], "solve_ms": d["solve_ms"], "e2e_ms": d["e2e"]["ms_per_step"],
+                                   "value": d["value"], "value_walked": d.get("value_walked"), "unit": d["unit"],
+                                   "walked_fraction": d["config"]["walked_fraction"], "e2e_matches_device_path": d["e2e"]["matches_device_path"],
+                                   "gpu_launches": d["gpu_launches"], "sm_mhz": d["clocks"].get("sm_mhz"), "reasons": d["clocks"].get("reasons")}
+        except Exception as ex:  # noqa: BLE001 - reported in the line
+            out[f"config{cfg}"] = {"error": f"{type(ex).__name__}: {str(ex)[:200]}"}
+    return out
 
 
 def peaks():
@@ -170,6 +218,8 @@ def main():
     ap.add_argument("--analyse", action="store_true", help="call rc_analyse_atmosphere whatever the workload")
     ap.add_argument("--tune", default="", help="rc_set_tuning knobs, e.g. march_variant=0,bands=3")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-secondary", action="store_true",
+                    help="skip the `secondary` object (the other BASELINE configs, 3 steps each, run as child processes of the default bench)")
     ap.add_argument("--cpu-baseline-whole", action="store_true",
                     help="also time the oracle on ONE WHOLE solve of the workload (config 2: ~3 minutes on 16 cores) and check "
                          "the GPU J against it on every cell")
@@ -218,7 +268,7 @@ def main():
     if world > 1:
         # the path shards by wavelength: rank r solves its contiguous block of the SAME
         # atmosphere; per-wavelength J needs no exchange, Jbar one all-reduce of nx ny floats (inside the timed region)
-        assert atm.line is None, "the multi-rank leg shards chi/eta planes (GivenFs mode)"
+        # (the moving line shards the same way: every rank holds the six line parameters, its block is a slice of x_lambda)
         atm = sharding.shard_atmosphere(atm, rank, world)
         assert atm.nlambda > 0, f"{nlambda_job} wavelengths do not cover {world} ranks"
 
@@ -339,6 +389,9 @@ def main():
         ach = alg_bytes / (ms_march[dom] * 1e-3) / 1e9
         mode = ("line" if atm.line is not None else "flat") + (f"_incl{nincl}" if nincl > 1 else "") + ("_fix" if args.bilinear_fix else "")
         cap = NCU_CAPTURES.get((mode, args.config, dom)) if world == 1 and not args.active and not args.tune else None
+        stale_cap = None
+        if cap is not None and kernel_text_sha(cap["kernel"]) != cap["sha"]:
+            stale_cap, cap = cap, None      # a capture of an earlier version of the kernel: reported, not used
         dram = None if cap is None else cap["dram_bytes"]
         mufu_per_unit = 3 if atm.line is not None else 1  # line mode: ex2 (profile), rcp (eta/chi), ex2 (transmittance)
         sfu_peak = SM_COUNT * MUFU_PER_CLK_SM * sm_max_mhz * 1e6 / mufu_per_unit
@@ -408,6 +461,23 @@ def main():
             "gpu_launches": launches, "clocks": clocks,
         }
         line["roofline"]["traffic"] = dram
+        # the tier's own figure beside `frac`: algorithmic bytes (8 B per segment-wavelength the launch integrates + the merged
+        # cascade read and written) / launch time / the measured HBM copy peak; above 1 because L2 and L1 serve the gathers
+        line["roofline"]["algorithmic_over_hbm"] = ach / hbm_peak
+        line["roofline"]["hbm_peak_gbs"] = hbm_peak
+        if cap is not None:
+            line["hbm"]["capture"] = {k: cap[k] for k in ("kernel", "sha", "commit", "capture_ms")}
+        if stale_cap is not None:
+            line["hbm"]["stale_capture"] = {**{k: stale_cap[k] for k in ("kernel", "sha", "commit", "capture_ms", "dram_bytes")},
+                                            "head_sha": kernel_text_sha(stale_cap["kernel"]),
+                                            "note": "the kernel's source changed after this capture: no traffic or derived fraction is reported from it"}
+        # `value` counts GEOMETRIC segments - every in-box cell segment of every ray, whether or not the march had to
+        # integrate it (early exit of opaque rays, unflagged probes, jumps over free space); `value_walked` counts only
+        # the segments the kernels really integrated.  They differ by `walked_fraction`; dense runs: ~1.
+        wf = sum(walked) / max(sum(seg), 1)
+        line["value_kind"] = "geometric segments x wavelengths / time"
+        line["value_walked"] = value * wf
+        line["e2e"]["value_walked"] = line["e2e"]["value"] * wf
         if world == 1 and not args.no_cpu_baseline:
             nwin = 3
             segl, secs, cores = oracle_sample(atm, nwin)
@@ -424,8 +494,15 @@ def main():
                 m = Jo > 1e-6 * Jo.max(axis=(0, 1), keepdims=True) if Jo.ndim == 3 else Jo > 1e-6 * Jo.max()
                 line["cpu_baseline"]["whole_solve"] = {"seconds": secs, "value": segl_job / secs, "unit": UNIT,
                                                        "gpu_max_rel_err_all_cells": float(np.max(np.abs(Jg[m] - Jo[m]) / Jo[m]))}
+        rc.close()
+        rc = None
+        if secondary_wanted(args, world):
+            del J, out_h
+            torch.cuda.empty_cache()
+            line["secondary"] = secondary_runs()
         print(json.dumps(line))
-    rc.close()
+    if rc is not None:
+        rc.close()
     if world > 1:
         dist.destroy_process_group()
 

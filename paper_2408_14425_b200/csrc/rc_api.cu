@@ -387,7 +387,7 @@ bool make_plan_uncached(const rc_config &cfg, const Tuning &tune, int nm, bool l
     P.bc_below = cur; cur += align_up((size_t)P.Lpad * P.NM * sizeof(float));  // [Lpad][NM]: one value per channel
     P.bc_above = cur; cur += align_up((size_t)P.Lpad * P.NM * sizeof(float));
     P.weights = cur;  cur += align_up(P.Lpad * sizeof(float));
-    P.flag = cur;     cur += 2 * ALIGN;  // scalar flags and counters: [0..15] scratch, [16..31] segments walked per cascade
+    P.flag = cur;     cur += 2 * ALIGN;  // scalar flags and counters (64-bit slots): [0..15] scratch, [16..31] segments walked per cascade, [32..43] flagged probes per cascade
     if (host_io) {
         const size_t io = align_up(ncell * L * sizeof(float));
         P.io_chi = cur; cur += io;
@@ -1055,13 +1055,15 @@ int rc_set_active_cells(rc_ctx *ctx, const unsigned char *active) {
         const int rc = build_patch_lists(ctx);
         if (rc != RC_OK) { ctx->active_set = false; return rc; }
     }
-    // flagged probes per cascade, for the statistics
-    for (int i = 0; i <= top; i++) {
-        std::vector<unsigned char> h((size_t)(P.nx >> i) * (P.ny >> i));
-        RC_CUDA(ctx, cudaMemcpy(h.data(), ctx->ws + P.pflag[i], h.size(), cudaMemcpyDeviceToHost));
-        int64_t n = 0;
-        for (unsigned char v : h) n += v;
-        ctx->stats.probes_flagged[i] = n;
+    // flagged probes per cascade, for the statistics: counted on the device, one small copy back (counters [32..43] of P.flag)
+    {
+        unsigned long long *d = (unsigned long long *)(ctx->ws + P.flag) + 32, h[RC_MAX_CASCADES] = {0};
+        RC_CUDA(ctx, cudaMemsetAsync(d, 0, sizeof(h), ctx->stream));
+        for (int i = 0; i <= top; i++)
+            RC_CUDA(ctx, rc::launch_count_flags((const unsigned char *)(ctx->ws + P.pflag[i]), (long long)(P.nx >> i) * (P.ny >> i), d + i, ctx->stream));
+        RC_CUDA(ctx, cudaMemcpyAsync(h, d, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream));
+        RC_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+        for (int i = 0; i <= top; i++) ctx->stats.probes_flagged[i] = (int64_t)h[i];
     }
     ctx->stats.active_cells = ctx->stats.probes_flagged[0];
     return RC_OK;

@@ -128,6 +128,7 @@ cudaError_t launch_reduce_jbar(const float *Jpart, float *Jbar, long long ncell,
 cudaError_t launch_count(const MarchParams &p, unsigned long long *total, cudaStream_t st);
 cudaError_t launch_gather_probe(const float *buf, unsigned long long nsector, int iters, int blocks, float *sink, cudaStream_t st);
 cudaError_t launch_flags_from_active(const unsigned char *active, unsigned char *flag0, long long ncell, cudaStream_t st);
+cudaError_t launch_count_flags(const unsigned char *a, long long n, unsigned long long *out, cudaStream_t st);
 cudaError_t launch_flag_parents(const unsigned char *child, int npx, int npy, unsigned char *parent, cudaStream_t st);
 cudaError_t launch_mark_and_compact_patches(const MarchParams &p, int npatch, unsigned char *mark, int *list, int *count, cudaStream_t st);
 cudaError_t launch_build_distance_field(const float *chi, const float *eta, const float *line, const unsigned char *active, int nx, int ny,

@@ -1763,6 +1763,20 @@ __global__ void __launch_bounds__(1024) compact_patches_kernel(const unsigned ch
     if (threadIdx.x == 0) *count = base;
 }
 
+// *out += the number of non-zero bytes of a[0 .. n): the flagged probes of one cascade, for rc_stats
+__global__ void __launch_bounds__(256) count_flags_kernel(const unsigned char *a, long long n, unsigned long long *out) {
+    unsigned mine = 0;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) mine += a[i] != 0;
+    for (int o = 16; o > 0; o >>= 1) mine += __shfl_down_sync(FULL, mine, o);
+    if ((threadIdx.x & 31) == 0 && mine) atomicAdd(out, (unsigned long long)mine);
+}
+
+cudaError_t launch_count_flags(const unsigned char *a, long long n, unsigned long long *out, cudaStream_t st) {
+    const long long want = (n + 255) / 256;
+    count_flags_kernel<<<(unsigned)(want < 148 * 8 ? want : 148 * 8), 256, 0, st>>>(a, n, out);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_flags_from_active(const unsigned char *active, unsigned char *flag0, long long ncell, cudaStream_t st) {
     flags_from_active_kernel<<<(unsigned)((ncell + 255) / 256), 256, 0, st>>>(active, flag0, ncell);
     return cudaGetLastError();

@@ -9,7 +9,9 @@
                        inside the structure, in its shadow, at its edges, at the four box edges and corners and across
                        every seam of the L2 bands; the mask scale comes from the oracle
   + at those sizes, on EVERY cell and without oracle time: J = S, the x-flip symmetry, and bit-identity of the
-    banded against the unbanded march and of the distance-field against the lock-step march.
+    banded against the unbanded march and of the hit-list and distance-field marches against the lock-step march.
+  + the widened modes at the sizes profiles/bench_*.md quotes times for: the bilinear fix on config 3 (its unbanded launches
+    gather from HBM), 8 inclinations and the moving line x 8 inclinations x 25 % of the cells flagged on the config-2 grid.
 """
 import dataclasses
 
@@ -84,9 +86,11 @@ def feature_windows(atm, size=4, nrand=4, seed=0):
     return out
 
 
-def run_windows(atm, oracle, size=4, nrand=4, min_windows=16, **kw):
+def run_windows(atm, oracle, size=4, nrand=4, min_windows=16, max_windows=None, **kw):
     Jg, st = gpu(atm, **kw)
     wins = feature_windows(atm, size, nrand, seed=atm.nx)
+    if max_windows is not None and len(wins) > max_windows:      # an even pick over box edges, seams and features
+        wins = [wins[i] for i in np.unique(np.linspace(0, len(wins) - 1, max_windows).round().astype(int))]
     assert len(wins) >= min_windows
     ref = []
     for w in wins:
@@ -146,10 +150,13 @@ def test_config3_windows_and_invariants(oracle):
 
 def test_config4_windows_and_invariants(oracle):
     atm = A.make_config(4)
-    Jg, st = run_windows(atm, oracle, analyse=True)               # as bench.py runs it: distance-field march, Jbar
-    assert st.sparse_march == 1 and st.empty_cells > 0.9 * atm.nx * atm.ny
+    Jg, st = run_windows(atm, oracle, analyse=True)               # as bench.py runs it: the march over hit lists, Jbar
+    assert st.sparse_march == 1 and st.sparse_lists >= 1 and st.empty_cells > 0.9 * atm.nx * atm.ny
     Jd, st = gpu(atm)                                             # the lock-step march (banded at this size): every cell, every bit
     assert st.sparse_march == 0 and np.array_equal(Jg, Jd)
+    # what a caller gets who lends no second buffer (rc_set_sparse_workspace): the distance-field fan march, at this size
+    Jfan, st = gpu(atm, analyse=True, tuning=dict(lists=0))
+    assert st.sparse_march == 1 and st.sparse_lists == 0 and np.array_equal(Jg, Jfan)
     flip = dataclasses.replace(atm, chi=np.ascontiguousarray(atm.chi[:, ::-1]), eta=np.ascontiguousarray(atm.eta[:, ::-1]))
     Jf, _ = gpu(flip, analyse=True)
     m = Jg > 1e-6 * Jg.max()
@@ -189,3 +196,61 @@ def test_config1_size_moving_line_with_inclinations(oracle):
         Jo = oracle.solve_atmosphere(atm, window=(x0, x1, y0, y1))["J"]
         worst = max(worst, plane_errors(Jg[y0:y1, x0:x1], Jo, scale=Jg.reshape(-1, atm.nlambda).max(axis=0)))
     assert worst <= TOL, worst
+
+
+# ------------------------------------------------------------------ the widened modes at the sizes their timings are quoted for
+def _windows_at(points, nx, ny, size):
+    out = []
+    for (px, py) in points:
+        x0, y0 = int(min(max(px - size // 2, 0), nx - size)), int(min(max(py - size // 2, 0), ny - size))
+        if (x0, x0 + size, y0, y0 + size) not in out:
+            out.append((x0, x0 + size, y0, y0 + size))
+    return out
+
+
+@pytest.mark.slow
+def test_config3_size_bilinear_fix(oracle):
+    """PAPER.md:243-249 on config 3's 2048 x 2048 grid: with the fix no cascade is banded, so cascades 5-6 gather from HBM -
+    launches that no smaller grid reaches."""
+    atm = dataclasses.replace(A.make_config(3), name="cfg3_fix", bilinear_fix=True)
+    run_windows(atm, oracle, size=3, nrand=0, min_windows=12, max_windows=12)
+
+
+@pytest.mark.slow
+def test_config2_size_eight_inclinations(oracle):
+    """PAPER.md:281, 571 (every result of the paper uses 8 inclinations) on config 2's 1024 x 1024 grid: 8 channels per lane,
+    one wavelength per batch (the shape profiles/bench_r2.md quotes 510 ms for)."""
+    atm = A.with_inclinations(A.make_config(2), 8)
+    run_windows(atm, oracle, size=2, nrand=0, min_windows=8, max_windows=8)
+
+
+@pytest.mark.slow
+def test_config2_size_moving_line_eight_inclinations_quarter_active(oracle):
+    """The paper's production regime: moving line x 8 inclinations x the densest 25 % of the cells
+    flagged, on config 2's 1024 x 1024 x 64 grid, marched over hit lists.  Windows sit on flagged
+    cells: deep inside, on the rim of the flagged set and next to the box edges."""
+    atm = A.with_active_cells(A.with_inclinations(A.line_config2(), 8), mode="fraction", fraction=0.25)
+    Jg, st = gpu(atm, analyse=True)
+    act = atm.active != 0
+    assert st.active_cells == int(act.sum()) and np.all(Jg[~act] == 0.0)
+    op = (atm.line[..., 0] + atm.line[..., 2]).astype(np.float64)
+    ys, xs = np.nonzero(act)
+    rim = act & ~(np.roll(act, 1, 0) & np.roll(act, -1, 0) & np.roll(act, 1, 1) & np.roll(act, -1, 1))
+    ry, rx = np.nonzero(rim)
+    rng = np.random.default_rng(8)
+    pts = [np.unravel_index(int(np.argmax(op)), op.shape)[::-1]]
+    pts += [(int(rx[i]), int(ry[i])) for i in rng.integers(0, rx.size, 3)]
+    pts += [(int(xs[i]), int(ys[i])) for i in (int(np.argmin(xs)), int(np.argmax(xs)), int(np.argmin(ys)), int(np.argmax(ys)))]
+    pts += [(int(xs[i]), int(ys[i])) for i in rng.integers(0, xs.size, 2)]
+    wins = _windows_at(pts, atm.nx, atm.ny, 2)
+    assert len(wins) >= 8
+    ref = [oracle.solve_atmosphere(atm, window=w)["J"] for w in wins]
+    scale = np.nanmax([np.nanmax(r.reshape(-1, r.shape[-1]), axis=0) for r in ref], axis=0)
+    worst, checked = 0.0, 0
+    for (x0, x1, y0, y1), Jo in zip(wins, ref):
+        a = act[y0:y1, x0:x1]
+        assert np.all(np.isfinite(Jo[a]))
+        worst = max(worst, plane_errors(np.where(a[..., None], Jg[y0:y1, x0:x1], 0.0), np.where(a[..., None], Jo, 0.0), scale))
+        checked += int(a.sum())
+    print(f"{atm.name}: max rel err over {checked} flagged cells in {len(wins)} windows = {worst:.3e}")
+    assert checked >= 16 and worst <= TOL, worst
