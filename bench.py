@@ -47,10 +47,14 @@ NCU_CAPTURES = {
                      "dram_bytes": 149.293018e9 + 3.933113e9, "l2_to_sm_bytes": 348.052288e9, "lts_pct": 30.28,
                      "source": "profiles/ncu_r3.md: ncu --set full of march_list_kernel<8,1,8,4,6,0> (hit lists), cascade 5 of config 4, "
                                "commit e582544 (47.67 ms under ncu)"},
-    ("line_incl8", 2, 5): {"kernel": "march_kernel", "sha": "b9a7d603683de633", "commit": "0eaea15", "capture_ms": 497.3,
-                           "dram_bytes": 5.789094e9 + 2.674684e9, "l2_to_sm_bytes": 1879.661e9, "lts_pct": 11.03,
-                           "source": "profiles/ncu_r2_modes.md: ncu --set full of march_kernel<8,8,2,8,3,0,1>, cascade 5 of the "
-                                     "moving line x 8 inclinations on the config-2 grid, commit 0eaea15 (497.3 ms under ncu)"},
+    ("flat_incl8", 2, 5): {"kernel": "march_kernel", "sha": "e6187b462936d78b", "commit": "e43f0bd", "capture_ms": 223.63,
+                           "dram_bytes": 5.754840e9 + 2.158622e9, "l2_to_sm_bytes": 1119.340e9, "lts_pct": 14.64,
+                           "source": "profiles/ncu_r3.md: ncu --set full of march_kernel<8,8,2,8,3,0,0>, cascade 5 of config 2 x 8 "
+                                     "inclinations, commit e43f0bd (223.6 ms under ncu)"},
+    ("line_incl8", 2, 5): {"kernel": "march_kernel", "sha": "e6187b462936d78b", "commit": "e43f0bd", "capture_ms": 497.19,
+                           "dram_bytes": 5.784382e9 + 2.636249e9, "l2_to_sm_bytes": 1878.842e9, "lts_pct": 11.05,
+                           "source": "profiles/ncu_r3.md: ncu --set full of march_kernel<8,8,2,8,3,0,1>, cascade 5 of the "
+                                     "moving line x 8 inclinations on the config-2 grid, commit e43f0bd (497.2 ms under ncu)"},
 }
 
 
